@@ -1,0 +1,148 @@
+"""ctypes front end of the CPU oracle (oracle/ref_tdh.c).  TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs import this module.
+It does not import the CUDA package's binding; arguments are plain numpy arrays on the host.
+
+Functions mirror the C exports one to one (see the header comment of ref_tdh.c for the passages they follow):
+    dft3d, kinetic, local, nonlocal_, apply_hamiltonian, propagate, num_threads
+``backend``: 0 = direct O(N^2)-per-pencil DFT (the definition), 1 = naive recursive radix-2/3 FFT.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from typing import Optional
+
+import numpy as np
+
+from . import build as _build
+
+DIRECT, NAIVE_FFT = 0, 1
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        for name in ("ref_dft3d", "ref_kinetic", "ref_local", "ref_nonlocal", "ref_apply_hamiltonian",
+                     "ref_propagate", "ref_num_threads"):
+            getattr(_lib, name).restype = C.c_int
+    return _lib
+
+
+def _i3(x):
+    return (C.c_int * 3)(*[int(v) for v in x])
+
+
+def _d3(x):
+    return (C.c_double * 3)(*[float(v) for v in x])
+
+
+def _ptr(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _c128(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.complex128)
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise RuntimeError(f"oracle {what} failed with code {rc}")
+
+
+class _Proj:
+    """Marshalled projector tables (keeps the contiguous arrays alive)."""
+
+    def __init__(self, proj):
+        if proj is None or proj.natoms == 0:
+            self.natoms = 0
+            self.args = (C.c_int(0), None, None, None, None, None, None)
+            return
+        self.natoms = int(proj.natoms)
+        self.sph_off = np.ascontiguousarray(proj.sph_off, dtype=np.int64)
+        self.sph_idx = np.ascontiguousarray(proj.sph_idx, dtype=np.int32)
+        self.sph_disp = None if proj.sph_disp is None else np.ascontiguousarray(proj.sph_disp, dtype=np.float64)
+        self.chan_off = np.ascontiguousarray(proj.chan_off, dtype=np.int32)
+        self.beta = np.ascontiguousarray(proj.beta, dtype=np.float64)
+        self.dcoef = np.ascontiguousarray(proj.dcoef, dtype=np.float64)
+        self.args = (C.c_int(self.natoms), _ptr(self.sph_off), _ptr(self.sph_idx), _ptr(self.sph_disp),
+                     _ptr(self.chan_off), _ptr(self.beta), _ptr(self.dcoef))
+
+
+def num_threads() -> int:
+    return int(lib().ref_num_threads())
+
+
+def dft3d(a: np.ndarray, sign: int, backend: int = DIRECT) -> np.ndarray:
+    """3-D DFT of a block (nst, n0, n1, n2) (or one state (n0, n1, n2)); sign -1 forward, +1 inverse (1/N_p)."""
+    a = _c128(a).copy()
+    n = a.shape[-3:]
+    nst = 1 if a.ndim == 3 else a.shape[0]
+    _check(lib().ref_dft3d(_i3(n), C.c_int(nst), _ptr(a), C.c_int(sign), C.c_int(backend)), "dft3d")
+    return a
+
+
+def kinetic(n, length, kpt, ecut, psi, backend: int = DIRECT) -> np.ndarray:
+    psi = _c128(psi)
+    out = np.empty_like(psi)
+    nst = 1 if psi.ndim == 3 else psi.shape[0]
+    _check(lib().ref_kinetic(_i3(n), _d3(length), _d3(kpt), C.c_double(ecut), C.c_int(nst), _ptr(psi), _ptr(out),
+                             C.c_int(backend)), "kinetic")
+    return out
+
+
+def local(n, v, psi) -> np.ndarray:
+    psi = _c128(psi)
+    out = np.empty_like(psi)
+    nst = 1 if psi.ndim == 3 else psi.shape[0]
+    v = None if v is None else np.ascontiguousarray(v, dtype=np.float64)
+    _check(lib().ref_local(_i3(n), _ptr(v), C.c_int(nst), _ptr(psi), _ptr(out)), "local")
+    return out
+
+
+def nonlocal_(n, length, kpt, proj, psi) -> np.ndarray:
+    psi = _c128(psi)
+    out = np.empty_like(psi)
+    nst = 1 if psi.ndim == 3 else psi.shape[0]
+    p = _Proj(proj)
+    _check(lib().ref_nonlocal(_i3(n), _d3(length), _d3(kpt), *p.args, C.c_int(nst), _ptr(psi), _ptr(out)), "nonlocal")
+    return out
+
+
+def apply_hamiltonian(n, length, kpt, ecut, v, proj, psi, backend: int = NAIVE_FFT) -> np.ndarray:
+    """H psi for a block (nst, n0, n1, n2) or a single state (n0, n1, n2).  Returns a new array."""
+    psi = _c128(psi)
+    out = np.empty_like(psi)
+    nst = 1 if psi.ndim == 3 else psi.shape[0]
+    v = None if v is None else np.ascontiguousarray(v, dtype=np.float64)
+    p = _Proj(proj)
+    _check(lib().ref_apply_hamiltonian(_i3(n), _d3(length), _d3(kpt), C.c_double(ecut), _ptr(v), *p.args,
+                                       C.c_int(nst), _ptr(psi), _ptr(out), C.c_int(backend)), "apply_hamiltonian")
+    return out
+
+
+def propagate(n, length, kpt, ecut, v, proj, psi, dt: float, nsteps: int, order: int = 4,
+              backend: int = NAIVE_FFT) -> np.ndarray:
+    """nsteps Taylor-`order` steps of exp(-i dt H).  Returns a new array (the input is not modified)."""
+    psi = _c128(psi).copy()
+    nst = 1 if psi.ndim == 3 else psi.shape[0]
+    v = None if v is None else np.ascontiguousarray(v, dtype=np.float64)
+    p = _Proj(proj)
+    _check(lib().ref_propagate(_i3(n), _d3(length), _d3(kpt), C.c_double(ecut), _ptr(v), *p.args, C.c_int(nst),
+                               _ptr(psi), C.c_double(dt), C.c_int(nsteps), C.c_int(order), C.c_int(backend)),
+           "propagate")
+    return psi
+
+
+def apply_workload(wl, psi, backend: int = NAIVE_FFT) -> np.ndarray:
+    """Convenience: H psi with a workloads.Workload."""
+    c = wl.cfg
+    return apply_hamiltonian(c.n, c.length, c.kpt, c.ecut_abi, wl.v, wl.proj, psi, backend)
+
+
+def propagate_workload(wl, psi, dt=None, nsteps=None, backend: int = NAIVE_FFT) -> np.ndarray:
+    c = wl.cfg
+    return propagate(c.n, c.length, c.kpt, c.ecut_abi, wl.v, wl.proj, psi, c.dt if dt is None else dt,
+                     c.nsteps if nsteps is None else nsteps, 4, backend)

@@ -1,0 +1,354 @@
+"""Pins P1-P8: the CPU oracle checked against what the mathematics fixes.
+
+Nothing here calls the CUDA path.  Each pin compares the oracle with something it does not itself compute:
+a brute-force triple sum, a closed form, an invariant, a library routine used as a third cross-check.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2106_03872_b200 import workloads as W
+
+TWO_PI = 2.0 * math.pi
+
+
+def rand_c(rng, shape):
+    return rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
+
+
+def rel(a, b):
+    return float(np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(b.ravel()), 1e-300))
+
+
+def small_cfg(cid=101, n=(6, 5, 4), length=(6.0, 5.5, 4.8), natoms=2, lmax=1, rc=1.9, **kw):
+    kw.setdefault("dl", (1.5, -0.7, 0.4)[: lmax + 1])
+    return W.test_config(cid, n, length, nst=3, natoms=natoms, lmax=lmax, rc=rc, proj_sigma=0.6,
+                         well_z=2.0, well_sigma=0.8, noise=0.01, **kw)
+
+
+def dense_matrix(oracle, cfg, wl, backend=0):
+    """Columns H e_p, built by applying the oracle's H to unit vectors (PAPER.md:229 'dense Hermitian matrix')."""
+    npts = cfg.npts
+    eye = np.eye(npts, dtype=np.complex128).reshape((npts,) + tuple(cfg.n))
+    cols = oracle.apply_hamiltonian(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, wl.v, wl.proj, eye, backend)
+    return cols.reshape(npts, npts).T.copy()   # H[:, p] = H e_p
+
+
+# --------------------------------------------------------------------------------------------- P1
+@pytest.mark.parametrize("n", [(4, 4, 4), (6, 6, 6), (8, 8, 8), (4, 6, 9), (5, 3, 2)])
+@pytest.mark.parametrize("backend", [0, 1])
+def test_p1_dft_bruteforce(oracle, n, backend):
+    """3-D DFT = brute-force triple sum over all points (the textbook definition); round trip; Parseval."""
+    rng = np.random.default_rng(11)
+    a = rand_c(rng, (2,) + n)
+    # brute force: out[q] = sum_p a[p] exp(-2 pi i (qx px/Nx + qy py/Ny + qz pz/Nz)), one 6-index phase tensor
+    ph = [np.exp(-2j * np.pi * np.outer(np.arange(m), np.arange(m)) / m) for m in n]
+    brute = np.einsum("sxyz,ax,by,cz->sabc", a, ph[0], ph[1], ph[2])
+    f = oracle.dft3d(a, -1, backend)
+    assert rel(f, brute) < 1e-13
+    assert rel(f, np.fft.fftn(a, axes=(1, 2, 3))) < 1e-13            # library, third cross-check
+    assert rel(oracle.dft3d(f, +1, backend), a) < 1e-13               # inverse carries 1/N_p
+    npts = n[0] * n[1] * n[2]
+    assert abs(np.sum(np.abs(f) ** 2) - npts * np.sum(np.abs(a) ** 2)) < 1e-11 * npts * np.sum(np.abs(a) ** 2)
+
+
+@pytest.mark.parametrize("N", [16, 32, 48, 64, 96])
+def test_p1_naive_fft_equals_direct_on_config_grids(oracle, N):
+    """The naive radix-2/3 FFT back-end is accepted only because it equals the direct DFT on every grid size used."""
+    rng = np.random.default_rng(N)
+    a = rand_c(rng, (1, N, N, N))
+    d = oracle.dft3d(a, -1, 0)
+    f = oracle.dft3d(a, -1, 1)
+    assert rel(f, d) < 1e-13
+    assert rel(oracle.dft3d(a, +1, 1), oracle.dft3d(a, +1, 0)) < 1e-13
+
+
+def test_p1_delta_and_shift_theorem(oracle):
+    """A unit impulse at r0 transforms to the plane wave exp(-i G.r0): fixes the sign and index convention."""
+    n = (6, 4, 8)
+    a = np.zeros(n, dtype=np.complex128)
+    r0 = (2, 3, 5)
+    a[r0] = 1.0
+    f = oracle.dft3d(a, -1, 0)
+    q = np.meshgrid(*[np.arange(m) for m in n], indexing="ij")
+    expect = np.exp(-2j * np.pi * sum(q[i] * r0[i] / n[i] for i in range(3)))
+    assert rel(f, expect) < 1e-14
+
+
+# --------------------------------------------------------------------------------------------- P2
+@pytest.mark.parametrize("n,kfrac,ecut", [((6, 4, 8), (0, 0, 0), None), ((6, 4, 8), (0.25, -0.4, 0.1), None),
+                                          ((5, 6, 3), (0.3, 0.0, 0.2), 4.0), ((4, 4, 4), (0.25, 0.0, 0.0), 3.0)])
+def test_p2_plane_waves_are_kinetic_eigenvectors(oracle, n, kfrac, ecut):
+    """psi = exp(i G.r) for EVERY G of the grid (incl. Nyquist): T psi = 1/2 |G+k|^2 psi inside the mask, 0 outside."""
+    length = (5.0, 4.0, 6.5)
+    kpt = [TWO_PI * kfrac[a] / length[a] for a in range(3)]
+    ii = np.meshgrid(*[np.arange(m) for m in n], indexing="ij")
+    # signed frequency range written out independently of the oracle: even N -> -N/2 .. N/2-1, odd N -> -(N-1)/2 .. (N-1)/2
+    ranges = [range(-(m // 2), m - m // 2) for m in n]
+    psis, eig = [], []
+    for mx in ranges[0]:
+        for my in ranges[1]:
+            for mz in ranges[2]:
+                m = (mx, my, mz)
+                psis.append(np.exp(2j * np.pi * sum(m[a] * ii[a] / n[a] for a in range(3))))
+                eig.append(0.5 * sum((TWO_PI * m[a] / length[a] + kpt[a]) ** 2 for a in range(3)))
+    psis = np.array(psis)
+    eig = np.array(eig)
+    if ecut is not None:
+        assert (eig > ecut).any() and (eig <= ecut).any()
+        eig = np.where(eig <= ecut, eig, 0.0)
+    for backend in (0, 1):
+        out = oracle.kinetic(n, length, kpt, -1.0 if ecut is None else ecut, psis, backend)
+        err = np.abs(out - eig[:, None, None, None] * psis).max()
+        assert err < 1e-12 * max(1.0, eig.max())
+
+
+# --------------------------------------------------------------------------------------------- P3
+def test_p3_constant_potential_is_a_shift(oracle):
+    cfg = small_cfg(102)
+    wl = W.make(cfg)
+    psi = W.states(cfg)
+    c = -0.37
+    h0 = oracle.apply_hamiltonian(cfg.n, cfg.length, cfg.kpt, -1.0, None, wl.proj, psi, 0)
+    hc = oracle.apply_hamiltonian(cfg.n, cfg.length, cfg.kpt, -1.0, np.full(cfg.n, c), wl.proj, psi, 0)
+    assert rel(hc - h0, c * psi) < 1e-13
+    # local term alone is the pointwise product with the real array V
+    assert rel(oracle.local(cfg.n, wl.v, psi), wl.v[None] * psi) == 0.0
+    # spectrum of the dense matrix shifts by c
+    wl_c = W.Workload(cfg=cfg, pos=wl.pos, v=wl.v + c, proj=wl.proj)
+    e0 = np.linalg.eigvalsh(dense_matrix(oracle, cfg, wl))
+    ec = np.linalg.eigvalsh(dense_matrix(oracle, cfg, wl_c))
+    assert np.abs(ec - e0 - c).max() < 1e-12
+
+
+# --------------------------------------------------------------------------------------------- P4
+def test_p4_single_projector_closed_form(oracle):
+    """One atom, one channel: V_nl = D dV |beta><beta|.  psi = 1 -> beta[q] D dV sum(beta) on the sphere, 0 elsewhere."""
+    cfg = W.test_config(103, (8, 7, 6), (7.0, 6.0, 5.5), nst=1, natoms=1, lmax=0, rc=2.1, dl=(1.5,))
+    wl = W.make(cfg)
+    pr = wl.proj
+    assert pr.natoms == 1 and 10 < len(pr.sph_idx) < cfg.npts
+    beta = pr.beta_of(0)[0]
+    one = np.ones(cfg.n, dtype=np.complex128)
+    out = oracle.nonlocal_(cfg.n, cfg.length, (0, 0, 0), pr, one)
+    expect = np.zeros(cfg.npts, dtype=np.complex128)
+    expect[pr.sph_idx] = beta * 1.5 * cfg.dv * beta.sum()
+    assert rel(out.ravel(), expect) < 1e-14
+    # dense matrix: rank one, single non-zero eigenvalue D dV sum(beta^2)
+    eye = np.eye(cfg.npts, dtype=np.complex128).reshape((cfg.npts,) + cfg.n)
+    m = oracle.nonlocal_(cfg.n, cfg.length, (0, 0, 0), pr, eye).reshape(cfg.npts, cfg.npts).T
+    ev = np.linalg.eigvalsh(0.5 * (m + m.conj().T))
+    assert abs(ev[-1] - 1.5 * cfg.dv * np.sum(beta ** 2)) < 1e-12
+    assert np.abs(ev[:-1]).max() < 1e-12
+    assert np.linalg.matrix_rank(m, tol=1e-10) == 1
+
+
+def test_p4_rank_and_overlap_additivity(oracle):
+    """Several atoms / channels: rank <= sum C; the operator is the sum of the per-atom operators (overlapping spheres add)."""
+    cfg = small_cfg(104, n=(6, 6, 5), length=(5.0, 5.0, 4.5), natoms=3, lmax=1, rc=2.2)
+    wl = W.make(cfg)
+    pr = wl.proj
+    counts = np.bincount(pr.sph_idx, minlength=cfg.npts)
+    assert counts.max() >= 2, "test geometry must have overlapping spheres"
+    eye = np.eye(cfg.npts, dtype=np.complex128).reshape((cfg.npts,) + cfg.n)
+    m = oracle.nonlocal_(cfg.n, cfg.length, (0, 0, 0), pr, eye).reshape(cfg.npts, cfg.npts).T
+    assert np.linalg.matrix_rank(m, tol=1e-10) <= int(pr.chan_off[-1])
+    # explicit sum of outer products, channel by channel
+    expect = np.zeros((cfg.npts, cfg.npts))
+    for a in range(pr.natoms):
+        idx = pr.sph_idx[pr.sph_off[a]:pr.sph_off[a + 1]]
+        for c, b in enumerate(pr.beta_of(a)):
+            full = np.zeros(cfg.npts)
+            full[idx] = b
+            expect += pr.dcoef[pr.chan_off[a] + c] * cfg.dv * np.outer(full, full)
+    assert np.abs(m - expect).max() < 1e-13
+
+
+def test_p4_ylm_orthonormal_on_a_fine_sphere():
+    """Input-generator check: the real Y_lm of R11 are orthonormal (Lebedev-free check by dense quadrature)."""
+    th = (np.arange(400) + 0.5) * math.pi / 400
+    ph = (np.arange(800) + 0.5) * TWO_PI / 800
+    T, P = np.meshgrid(th, ph, indexing="ij")
+    d = np.stack([np.sin(T) * np.cos(P), np.sin(T) * np.sin(P), np.cos(T)], axis=-1).reshape(-1, 3)
+    wgt = (np.sin(T) * (math.pi / 400) * (TWO_PI / 800)).ravel()
+    ys = [W.real_ylm(l, m, d) for l in range(3) for m in range(-l, l + 1)]
+    gram = np.array([[np.sum(wgt * a * b) for b in ys] for a in ys])
+    assert np.abs(gram - np.eye(9)).max() < 1e-4
+
+
+# --------------------------------------------------------------------------------------------- P5
+@pytest.mark.parametrize("kfrac,ecut", [((0, 0, 0), None), ((0.25, 0.1, -0.3), 6.0)])
+def test_p5_hermiticity(oracle, kfrac, ecut):
+    cfg = small_cfg(105, n=(8, 6, 9), length=(6.0, 5.0, 7.0), natoms=3, lmax=2, rc=2.2, kfrac=kfrac, ecut=ecut)
+    wl = W.make(cfg)
+    rng = np.random.default_rng(5)
+    phi, psi = rand_c(rng, cfg.n), rand_c(rng, cfg.n)
+    for backend in (0, 1):
+        hpsi = oracle.apply_workload(wl, psi, backend)
+        hphi = oracle.apply_workload(wl, phi, backend)
+        lhs = np.vdot(phi, hpsi)
+        rhs = np.conj(np.vdot(psi, hphi))      # <H phi|psi> = <psi|H phi>^*
+        assert abs(lhs - rhs) < 1e-12 * abs(lhs)
+
+
+@pytest.mark.parametrize("kfrac,ecut", [((0, 0, 0), None), ((0.25, 0.0, 0.0), 5.0)])
+def test_p5_dense_matrix_is_hermitian(oracle, kfrac, ecut):
+    cfg = small_cfg(106, n=(4, 6, 5), length=(4.4, 5.5, 5.0), natoms=2, lmax=1, rc=1.9, kfrac=kfrac, ecut=ecut)
+    wl = W.make(cfg)
+    h = dense_matrix(oracle, cfg, wl)
+    assert np.abs(h - h.conj().T).max() < 1e-13 * np.abs(h).max()
+    ev = np.linalg.eigvals(h)
+    assert np.abs(ev.imag).max() < 1e-12
+    # term by term: T + V + Vnl assembled from the separate exports equals H
+    eye = np.eye(cfg.npts, dtype=np.complex128).reshape((cfg.npts,) + cfg.n)
+    parts = (oracle.kinetic(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, eye, 0) + oracle.local(cfg.n, wl.v, eye)
+             + oracle.nonlocal_(cfg.n, cfg.length, cfg.kpt, wl.proj, eye))
+    assert np.abs(parts.reshape(cfg.npts, cfg.npts).T - h).max() < 1e-13
+
+
+# --------------------------------------------------------------------------------------------- P6
+@pytest.mark.parametrize("units", [(1, 0, 0), (1, 1, 0), (1, 1, 1)])
+def test_p6_bloch_phase_identity(oracle, units):
+    """k a reciprocal-lattice vector, no mask: H_k u = e^{-ik.r} H_Gamma (e^{ik.r} u)   (reading R2).
+
+    Holds for +1 unit on axes with EVEN N only: the shifted frequency N/2 folds to -N/2 (R7) with the same square;
+    for odd N, (N+1)/2 folds to -(N-1)/2 and the kinetic eigenvalue changes.  So every axis here is even."""
+    geo = dict(n=(6, 8, 10), length=(5.0, 6.0, 6.5), natoms=3, lmax=2, rc=2.2)
+    base = small_cfg(107, **geo)
+    cfg_k = small_cfg(107, kfrac=tuple(float(u) for u in units), **geo)
+    wl0, wlk = W.make(base), W.make(cfg_k)
+    assert np.array_equal(wl0.proj.sph_idx, wlk.proj.sph_idx)
+    rng = np.random.default_rng(6)
+    u = rand_c(rng, base.n)
+    ii = np.meshgrid(*[np.arange(m) for m in base.n], indexing="ij")
+    eikr = np.exp(2j * np.pi * sum(units[a] * ii[a] / base.n[a] for a in range(3)))   # k.r with r = i h, k = 2 pi units / L
+    lhs = oracle.apply_workload(wlk, u, 0)
+    rhs = np.conj(eikr) * oracle.apply_workload(wl0, eikr * u, 0)
+    assert rel(lhs, rhs) < 1e-13
+    # the projector part alone must satisfy it too (this is what fixes the phase in the gather AND the scatter)
+    nl_k = oracle.nonlocal_(base.n, base.length, cfg_k.kpt, wlk.proj, u)
+    nl_0 = np.conj(eikr) * oracle.nonlocal_(base.n, base.length, (0, 0, 0), wl0.proj, eikr * u)
+    assert rel(nl_k, nl_0) < 1e-13
+    assert np.linalg.norm(nl_k) > 1e-3
+
+
+def test_p6_translation_covariance(oracle):
+    """Shift V, atoms and psi by whole grid points -> H psi shifts identically (spheres crossing the cell boundary)."""
+    cfg = small_cfg(108, n=(8, 6, 10), length=(6.0, 4.8, 7.0), natoms=2, lmax=1, rc=2.0, kfrac=(0.2, 0.0, -0.1))
+    pos = W.atom_positions(cfg)
+    shift = (3, 5, 7)
+    h = cfg.spacing
+    pos2 = np.mod(pos + np.array([shift[a] * h[a] for a in range(3)]), np.array(cfg.length))
+    rng = np.random.default_rng(8)
+    v = rng.standard_normal(cfg.n)
+    psi = rand_c(rng, cfg.n)
+    wl1 = W.Workload(cfg=cfg, pos=pos, v=v, proj=W.projectors(cfg, pos))
+    wl2 = W.Workload(cfg=cfg, pos=pos2, v=np.roll(v, shift, axis=(0, 1, 2)), proj=W.projectors(cfg, pos2))
+    def wraps(pr, a):   # a sphere crosses the boundary on an axis if it holds index 0 and N-1 but not every index
+        ijk = np.unravel_index(pr.sph_idx[pr.sph_off[a]:pr.sph_off[a + 1]], cfg.n)
+        return any(0 in x and cfg.n[ax] - 1 in x and len(set(x.tolist())) < cfg.n[ax] for ax, x in enumerate(ijk))
+    wrapped = [wraps(wl2.proj, a) for a in range(2)]
+    assert any(wrapped), "geometry must have a sphere that crosses the cell boundary"
+    h1 = oracle.apply_workload(wl1, psi, 0)
+    h2 = oracle.apply_workload(wl2, np.roll(psi, shift, axis=(0, 1, 2)), 0)
+    assert rel(h2, np.roll(h1, shift, axis=(0, 1, 2))) < 1e-12
+
+
+# --------------------------------------------------------------------------------------------- P7
+def taylor4(x):
+    return 1.0 - 1j * x - x ** 2 / 2.0 + 1j * x ** 3 / 6.0 + x ** 4 / 24.0
+
+
+def test_p7_taylor_modulus_polynomial():
+    """|P(x)|^2 = 1 - x^6/72 + x^8/576 (R15), by exact polynomial multiplication of the Eq. 8 coefficients."""
+    from fractions import Fraction as F
+    re = [F(1), F(0), F(-1, 2), F(0), F(1, 24)]     # real part coefficients of P
+    im = [F(0), F(-1), F(0), F(1, 6), F(0)]
+    sq = [F(0)] * 9
+    for i in range(5):
+        for j in range(5):
+            sq[i + j] += re[i] * re[j] + im[i] * im[j]
+    assert sq == [F(1), 0, 0, 0, 0, 0, F(-1, 72), 0, F(1, 576)]
+
+
+def test_p7_kinetic_only_propagation_closed_form(oracle):
+    """V = 0, no atoms: psi_hat(n, j dt) = P(t[n] dt)^j psi_hat(n, 0); norm follows |P|^{2j}.  FFTs by numpy here."""
+    n, length = (8, 6, 12), (5.0, 4.0, 7.0)
+    kfrac = (0.25, 0.0, 0.0)
+    kpt = [TWO_PI * kfrac[a] / length[a] for a in range(3)]
+    rng = np.random.default_rng(7)
+    psi0 = rand_c(rng, (2,) + n)
+    dt, nsteps = 0.05, 7
+    g = [TWO_PI * np.fft.fftfreq(n[a], d=1.0 / n[a]) / length[a] + kpt[a] for a in range(3)]
+    t = 0.5 * (g[0][:, None, None] ** 2 + g[1][None, :, None] ** 2 + g[2][None, None, :] ** 2)
+    assert t.max() * dt > 0.5                                  # a regime where |P| visibly differs from 1
+    for backend in (0, 1):
+        out = oracle.propagate(n, length, kpt, -1.0, None, None, psi0, dt, nsteps, 4, backend)
+        expect = np.fft.ifftn(taylor4(t * dt) ** nsteps * np.fft.fftn(psi0, axes=(1, 2, 3)), axes=(1, 2, 3))
+        assert rel(out, expect) < 1e-12
+        x = t * dt
+        norm2 = np.sum(np.abs(np.fft.fftn(psi0, axes=(1, 2, 3))) ** 2 * (1 - x ** 6 / 72 + x ** 8 / 576) ** nsteps,
+                       axis=(1, 2, 3)) / (n[0] * n[1] * n[2])
+        assert np.allclose(np.sum(np.abs(out) ** 2, axis=(1, 2, 3)), norm2, rtol=1e-12)
+
+
+def test_p7_eigenvector_of_full_h(oracle):
+    """An eigenvector of the dense small-grid H is multiplied by P(eps dt) per step; one-step error vs exp ~ x^5/120."""
+    cfg = small_cfg(109, n=(4, 5, 6), length=(4.4, 5.0, 5.5), natoms=2, lmax=1, rc=1.9, kfrac=(0.1, 0.2, 0.0))
+    wl = W.make(cfg)
+    h = dense_matrix(oracle, cfg, wl)
+    ev, vec = np.linalg.eigh(0.5 * (h + h.conj().T))
+    for j in (0, len(ev) // 2, len(ev) - 1):
+        eps = ev[j]
+        v0 = vec[:, j].reshape(cfg.n)
+        dt, nsteps = 0.03, 5
+        out = oracle.propagate_workload(wl, v0, dt=dt, nsteps=nsteps, backend=0)
+        assert rel(out, taylor4(eps * dt) ** nsteps * v0) < 1e-11
+        one = oracle.propagate_workload(wl, v0, dt=dt, nsteps=1, backend=0)
+        x = eps * dt
+        err = np.linalg.norm(one - np.exp(-1j * x) * v0) / np.linalg.norm(v0)
+        assert err <= abs(x) ** 5 / 120 * 1.5 + 1e-13
+        if abs(x) > 0.05:
+            assert err >= abs(x) ** 5 / 120 * 0.5
+
+
+def test_p7_propagate_is_literal_eq8(oracle):
+    """One step = psi + c1 H psi + c2 H^2 psi + c3 H^3 psi + c4 H^4 psi with the Eq. 8 coefficients, via repeated apply."""
+    cfg = small_cfg(110)
+    wl = W.make(cfg)
+    psi = W.states(cfg)
+    dt = 0.04
+    acc, phi = psi.copy(), psi
+    for k, c in enumerate([-1j * dt, -dt ** 2 / 2, 1j * dt ** 3 / 6, dt ** 4 / 24], start=1):
+        phi = oracle.apply_workload(wl, phi, 0)
+        acc = acc + c * phi
+    assert rel(oracle.propagate_workload(wl, psi, dt=dt, nsteps=1, backend=0), acc) < 1e-14
+    # and nsteps composes
+    two = oracle.propagate_workload(wl, psi, dt=dt, nsteps=2, backend=0)
+    assert rel(two, oracle.propagate_workload(wl, acc, dt=dt, nsteps=1, backend=0)) < 1e-13
+
+
+# --------------------------------------------------------------------------------------------- P8
+def test_p8_independent_of_batching(oracle):
+    cfg = W.CONFIGS["tiny"]
+    wl = W.make(cfg)
+    psi = W.states(cfg)
+    full = oracle.apply_workload(wl, psi, 1)
+    for s in (0, 3, 7):
+        assert np.array_equal(oracle.apply_workload(wl, psi[s], 1), full[s])
+    part = oracle.apply_workload(wl, psi[2:5], 1)
+    assert np.array_equal(part, full[2:5])
+    # the generator is per-state seeded too
+    assert np.array_equal(W.states(cfg, 2, 5), psi[2:5])
+
+
+# --------------------------------------------------------------------------------------------- argument checks
+def test_oracle_rejects_bad_index(oracle):
+    cfg = small_cfg(111)
+    wl = W.make(cfg)
+    bad = W.Projectors(**{**wl.proj.__dict__})
+    bad.sph_idx = wl.proj.sph_idx.copy()
+    bad.sph_idx[3] = cfg.npts
+    with pytest.raises(RuntimeError):
+        oracle.apply_hamiltonian(cfg.n, cfg.length, cfg.kpt, -1.0, wl.v, bad, W.states(cfg), 0)
