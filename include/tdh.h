@@ -1,0 +1,130 @@
+/*
+ * tdh.h -- C ABI of the B200-native Kohn-Sham H|psi> / Taylor-4 real-time TDDFT library (libtdh.so).
+ *
+ * The operation is the one the paper states as an operator applied to a field set, returning a field set:
+ *     auto hphi = hamiltonian(phi);                                   PAPER.md:225 (section V)
+ *     "a routine that applies the Hamiltonian over a field set"       PAPER.md:478 (section VIII.E)
+ * with the field set one contiguous array holding all states          PAPER.md:466 (section VIII.D).
+ *
+ *     H psi = -1/2 nabla^2 psi + V(r) psi + V_nl psi                   Eq. 2
+ *       kinetic term in Fourier space (diagonal, 1/2 |G+k|^2), via two batched 3-D FFTs
+ *       local potential: pointwise product in real space
+ *       non-local Kleinman-Bylander projectors on spheres in real space                     Eq. 9
+ *     exp(-i dt H) psi ~= sum_{k=0..4} (-i dt)^k / k! H^k psi          Eq. 8
+ *
+ * Conventions (readings R1-R16 of DESIGN.md): orthorhombic periodic cell, atomic units (Hartree, bohr).
+ * Grid point (i,j,k) sits at r = (i h_x, j h_y, k h_z), h_a = len[a]/n[a]; flat index p = (i*n[1] + j)*n[2] + k.
+ *
+ * LAYOUT.  A state block is psi[s][ix][iy][iz], iz fastest, state slowest, complex128 with interleaved (re, im):
+ * exactly a contiguous torch tensor of shape (nst, n0, n1, n2), dtype complex128.  A sub-block of states is a
+ * contiguous slice.  All internal layouts are the library's business.
+ *
+ * MEMORY SPACES.  Every pointer argument says DEVICE or HOST.  Device pointers must belong to the CUDA device that
+ * was current when tdh_create_grid was called.
+ *
+ * OWNERSHIP.  The caller owns psi / hpsi.  The handle owns copies of V, of the projector tables, the FFT tables and
+ * all workspace; everything is allocated in tdh_create_grid / tdh_set_*; tdh_apply_hamiltonian and tdh_propagate
+ * allocate nothing (no allocation on hot paths).
+ *
+ * ASYNCHRONY.  tdh_apply_hamiltonian / tdh_propagate enqueue work on the handle's stream and return; the caller
+ * synchronises the stream.  tdh_set_* and the *_host calls synchronise internally.
+ *
+ * ERRORS.  Every call returns 0 on success or a negative code; nothing throws or exits across this boundary.
+ * tdh_last_error() returns a thread-local, statically stored message for the last failing call of this thread.
+ *
+ * There is no CPU fallback anywhere in this library.
+ */
+#ifndef TDH_H
+#define TDH_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tdh_grid tdh_grid;                 /* opaque handle */
+typedef struct { double re, im; } tdh_c128;      /* one complex128 value */
+
+enum {
+    TDH_OK = 0,
+    TDH_EINVAL = -1,        /* null pointer, nst < 1, nst > max_states, overlapping in/out, order != 4, ...       */
+    TDH_EUNSUPPORTED = -2,  /* grid size not supported: every n[a] must be one of 16, 32, 48, 64, 96              */
+    TDH_ENOMEM = -3,        /* host or device allocation failed                                                   */
+    TDH_ECUDA = -4,         /* CUDA runtime error (text in tdh_last_error)                                        */
+    TDH_EINDEX = -5         /* sph_idx entry outside [0, n0*n1*n2), or a grid point listed twice for one atom     */
+};
+
+/* Create a grid handle.
+ *   n[3]        HOST  grid points per axis; each must be in {16, 32, 48, 64, 96}   (else TDH_EUNSUPPORTED)
+ *   len[3]      HOST  cell lengths in bohr, > 0
+ *   kpt[3]      HOST  Bloch vector k, Cartesian, 1/bohr (reading R1: psi is the periodic part u_k; kinetic 1/2|G+k|^2)
+ *   ecut              plane-wave cutoff in Ha for the kinetic term: components with 1/2|G+k|^2 > ecut are zeroed in
+ *                     the kinetic term only (reading R6); ecut <= 0 or +inf means no mask
+ *   max_states        largest nst any later call will pass (sizes the workspace), >= 1
+ *   cuda_stream       a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream) or NULL for the default stream
+ *   out               receives the handle
+ * Initial state: V = 0, no projectors. */
+int tdh_create_grid(const int n[3], const double len[3], const double kpt[3], double ecut, int max_states,
+                    void* cuda_stream, tdh_grid** out);
+
+/* Free everything the handle owns.  NULL is accepted. */
+int tdh_destroy_grid(tdh_grid* g);
+
+/* Set the local potential V(r) (sum of v_loc + v_H + v_xc of Eq. 2; "a simple multiplicative
+ * potential").   v_dev: DEVICE, n0*n1*n2 doubles in grid layout; copied.  NULL resets V to 0. */
+int tdh_set_potential(tdh_grid* g, const double* v_dev);
+
+/* Set the Kleinman-Bylander projectors (Eq. 9; readings R2-R5).  All pointers are HOST; the
+ * tables are copied and re-indexed internally.  natoms = 0 clears the projectors (other pointers may be NULL).
+ *   sph_off   [natoms+1]   prefix sums of P_I (points in atom I's sphere), sph_off[0] = 0
+ *   sph_idx   [sum P_I]    flat grid index p of each sphere point; within one atom every p at most once
+ *   sph_disp  [sum P_I][3] minimum-image displacement r_p - R_I (bohr); used only for the Bloch phases
+ *                          e^{+-i k.d} when k != 0; may be NULL when k = 0
+ *   chan_off  [natoms+1]   prefix sums of C_I (projector channels of atom I), chan_off[0] = 0
+ *   beta      concatenated per atom: [C_I][P_I] real projector values beta_{I,c}(r_q - R_I)
+ *   dcoef     [sum C_I]    KB coefficients D_{I,c}
+ * Computes  (V_nl psi)[S_I[q]] += e^{-ik.d_q} sum_c beta_{I,c}[q] D_{I,c} dV sum_{q'} beta_{I,c}[q'] e^{+ik.d_q'} psi[S_I[q']]. */
+int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_off, const int32_t* sph_idx,
+                       const double* sph_disp, const int32_t* chan_off, const double* beta, const double* dcoef);
+
+/* hpsi = H psi for a block of nst states (Eq. 2).  psi_dev, hpsi_dev: DEVICE, nst*n0*n1*n2 complex128 each, must not
+ * overlap.  1 <= nst <= max_states.  Asynchronous on the handle's stream. */
+int tdh_apply_hamiltonian(tdh_grid* g, int nst, const tdh_c128* psi_dev, tdh_c128* hpsi_dev);
+
+/* nsteps steps of psi <- sum_{k=0..4} (-i dt)^k/k! H^k psi (Eq. 8 with lambda = -i dt; fixed H, reading R10), in place.
+ * psi_dev: DEVICE, nst*n0*n1*n2 complex128.  order must be 4.  nsteps >= 0.  Asynchronous on the handle's stream. */
+int tdh_propagate(tdh_grid* g, int nst, tdh_c128* psi_dev, double dt, int nsteps, int order);
+
+/* The same two operations with HOST buffers (pageable or pinned): the library stages state chunks through its own
+ * pinned buffers, overlapping host<->device copies with the kernels, and returns when hpsi_host / psi_host is complete.
+ * nst is not limited by max_states here (chunks are).  These are the end-to-end entry points timed by bench.py. */
+int tdh_apply_hamiltonian_host(tdh_grid* g, int nst, const tdh_c128* psi_host, tdh_c128* hpsi_host);
+int tdh_propagate_host(tdh_grid* g, int nst, tdh_c128* psi_host, double dt, int nsteps, int order);
+
+/* Batched 3-D FFT alone (rows a1 / a3 of the scope table), in place on a DEVICE block.
+ * sign = -1: forward, unnormalised, e^{-i G.r}; sign = +1: inverse, scaled by 1/(n0*n1*n2)   (reading R8). */
+int tdh_fft3d(tdh_grid* g, int nst, tdh_c128* psi_dev, int sign);
+
+/* Number of kernel launches the last tdh_apply_hamiltonian / tdh_propagate / *_host call of this handle enqueued. */
+int tdh_last_launch_count(const tdh_grid* g);
+
+/* Seconds (device time, CUDA events on the handle's stream) spent in each kernel family during the last call, when
+ * profiling was switched on with tdh_set_profiling(g, 1); profiling inserts events and synchronises at the end.
+ * out[0..TDH_NKERNELS-1]; order given by tdh_kernel_name(i).  Off by default. */
+#define TDH_NKERNELS 4
+int tdh_set_profiling(tdh_grid* g, int on);
+int tdh_last_kernel_seconds(const tdh_grid* g, double out[TDH_NKERNELS]);
+const char* tdh_kernel_name(int i);
+
+/* Tuning knob: how many states are pushed through the kernel chain together (0 = library default, chosen so that
+ * the inter-kernel workspace stays resident in the 126 MB L2). */
+int tdh_set_chunk_states(tdh_grid* g, int chunk);
+
+const char* tdh_last_error(void);                 /* thread-local, static storage; never NULL */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TDH_H */

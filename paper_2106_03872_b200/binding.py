@@ -1,0 +1,217 @@
+"""Thin ctypes binding of libtdh.so (include/tdh.h).  Argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels; PyTorch supplies device memory and the stream.
+There is no CPU fallback: importing this module without the built library, or creating a grid without a CUDA
+device, raises.
+
+    g = Grid(n, length, kpt, ecut, max_states)           # tdh_create_grid on torch's current stream
+    g.set_potential(v)                                    # torch float64 CUDA tensor (n0, n1, n2)
+    g.set_projectors(proj)                                # workloads.Projectors (host numpy tables)
+    hpsi = g.apply_hamiltonian(psi)                       # torch complex128 CUDA tensor (nst, n0, n1, n2)
+    g.propagate(psi, dt, nsteps)                          # in place
+    g.apply_hamiltonian_host(psi_host, out_host)          # numpy / pinned torch CPU tensors
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libtdh.so")
+
+#: every symbol include/tdh.h declares
+SYMBOLS = (
+    "tdh_create_grid", "tdh_destroy_grid", "tdh_set_potential", "tdh_set_projectors", "tdh_apply_hamiltonian",
+    "tdh_propagate", "tdh_apply_hamiltonian_host", "tdh_propagate_host", "tdh_fft3d", "tdh_last_launch_count",
+    "tdh_set_profiling", "tdh_last_kernel_seconds", "tdh_kernel_name", "tdh_set_chunk_states", "tdh_last_error",
+)
+NKERNELS = 4
+
+TDH_OK, TDH_EINVAL, TDH_EUNSUPPORTED, TDH_ENOMEM, TDH_ECUDA, TDH_EINDEX = 0, -1, -2, -3, -4, -5
+
+
+class TdhError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"libtdh error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load libtdh.so (fails loudly if it has not been built: python -m paper_2106_03872_b200.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing; build it with `python -m paper_2106_03872_b200.build` "
+                          "(there is no CPU fallback)")
+    l = C.CDLL(LIB_PATH)
+    vp, i, d = C.c_void_p, C.c_int, C.c_double
+    l.tdh_create_grid.argtypes = [C.POINTER(i), C.POINTER(d), C.POINTER(d), d, i, vp, C.POINTER(vp)]
+    l.tdh_destroy_grid.argtypes = [vp]
+    l.tdh_set_potential.argtypes = [vp, vp]
+    l.tdh_set_projectors.argtypes = [vp, i, vp, vp, vp, vp, vp, vp]
+    l.tdh_apply_hamiltonian.argtypes = [vp, i, vp, vp]
+    l.tdh_propagate.argtypes = [vp, i, vp, d, i, i]
+    l.tdh_apply_hamiltonian_host.argtypes = [vp, i, vp, vp]
+    l.tdh_propagate_host.argtypes = [vp, i, vp, d, i, i]
+    l.tdh_fft3d.argtypes = [vp, i, vp, i]
+    l.tdh_last_launch_count.argtypes = [vp]
+    l.tdh_set_profiling.argtypes = [vp, i]
+    l.tdh_last_kernel_seconds.argtypes = [vp, C.POINTER(d)]
+    l.tdh_kernel_name.argtypes = [i]
+    l.tdh_kernel_name.restype = C.c_char_p
+    l.tdh_set_chunk_states.argtypes = [vp, i]
+    l.tdh_last_error.argtypes = []
+    l.tdh_last_error.restype = C.c_char_p
+    for s in SYMBOLS:
+        if s not in ("tdh_kernel_name", "tdh_last_error"):
+            getattr(l, s).restype = i
+    _lib = l
+    return l
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise TdhError(rc, lib().tdh_last_error().decode(errors="replace"))
+
+
+def _host_ptr(a) -> int:
+    """Address of a contiguous host buffer: numpy array or CPU torch tensor."""
+    if isinstance(a, np.ndarray):
+        assert a.flags["C_CONTIGUOUS"]
+        return a.ctypes.data
+    assert not a.is_cuda and a.is_contiguous()
+    return a.data_ptr()
+
+
+class Grid:
+    """Owns one tdh_grid handle.  All tensors passed in must live on the device that was current at creation."""
+
+    def __init__(self, n: Sequence[int], length: Sequence[float], kpt: Sequence[float] = (0.0, 0.0, 0.0),
+                 ecut: float = -1.0, max_states: int = 1, stream: Optional[int] = None):
+        import torch
+        l = lib()
+        if stream is None:
+            if not torch.cuda.is_available():
+                raise TdhError(TDH_ECUDA, "no CUDA device available (there is no CPU fallback)")
+            stream = torch.cuda.current_stream().cuda_stream
+        self.n = tuple(int(x) for x in n)
+        self.npts = self.n[0] * self.n[1] * self.n[2]
+        self.max_states = int(max_states)
+        self._h = C.c_void_p()
+        _check(l.tdh_create_grid((C.c_int * 3)(*self.n), (C.c_double * 3)(*[float(x) for x in length]),
+                                 (C.c_double * 3)(*[float(x) for x in kpt]), float(ecut), int(max_states),
+                                 C.c_void_p(stream), C.byref(self._h)))
+
+    # -- lifetime
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().tdh_destroy_grid(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    # -- set-up
+    def set_potential(self, v):
+        if v is None:
+            _check(lib().tdh_set_potential(self._h, None))
+            return
+        import torch
+        assert v.is_cuda and v.dtype == torch.float64 and v.is_contiguous() and v.numel() == self.npts
+        _check(lib().tdh_set_potential(self._h, C.c_void_p(v.data_ptr())))
+
+    def set_projectors(self, proj):
+        """proj: workloads.Projectors-like object with host numpy tables, or None to clear."""
+        if proj is None or proj.natoms == 0:
+            _check(lib().tdh_set_projectors(self._h, 0, None, None, None, None, None, None))
+            return
+        sph_off = np.ascontiguousarray(proj.sph_off, dtype=np.int64)
+        sph_idx = np.ascontiguousarray(proj.sph_idx, dtype=np.int32)
+        sph_disp = None if proj.sph_disp is None else np.ascontiguousarray(proj.sph_disp, dtype=np.float64)
+        chan_off = np.ascontiguousarray(proj.chan_off, dtype=np.int32)
+        beta = np.ascontiguousarray(proj.beta, dtype=np.float64)
+        dcoef = np.ascontiguousarray(proj.dcoef, dtype=np.float64)
+        p = lambda a: None if a is None else C.c_void_p(a.ctypes.data)
+        _check(lib().tdh_set_projectors(self._h, int(proj.natoms), p(sph_off), p(sph_idx), p(sph_disp), p(chan_off),
+                                        p(beta), p(dcoef)))
+
+    # -- device entry points
+    def _block(self, psi):
+        import torch
+        assert psi.is_cuda and psi.dtype == torch.complex128 and psi.is_contiguous()
+        assert psi.numel() % self.npts == 0
+        return psi.numel() // self.npts
+
+    def apply_hamiltonian(self, psi, out=None):
+        import torch
+        nst = self._block(psi)
+        if out is None:
+            out = torch.empty_like(psi)
+        assert self._block(out) == nst
+        _check(lib().tdh_apply_hamiltonian(self._h, nst, C.c_void_p(psi.data_ptr()), C.c_void_p(out.data_ptr())))
+        return out
+
+    def propagate(self, psi, dt: float, nsteps: int, order: int = 4):
+        nst = self._block(psi)
+        _check(lib().tdh_propagate(self._h, nst, C.c_void_p(psi.data_ptr()), float(dt), int(nsteps), int(order)))
+        return psi
+
+    def fft3d(self, psi, sign: int):
+        nst = self._block(psi)
+        _check(lib().tdh_fft3d(self._h, nst, C.c_void_p(psi.data_ptr()), int(sign)))
+        return psi
+
+    # -- host entry points (end-to-end path)
+    def apply_hamiltonian_host(self, psi_host, out_host):
+        nst = psi_host.size // self.npts if isinstance(psi_host, np.ndarray) else psi_host.numel() // self.npts
+        _check(lib().tdh_apply_hamiltonian_host(self._h, int(nst), C.c_void_p(_host_ptr(psi_host)),
+                                                C.c_void_p(_host_ptr(out_host))))
+        return out_host
+
+    def propagate_host(self, psi_host, dt: float, nsteps: int, order: int = 4):
+        nst = psi_host.size // self.npts if isinstance(psi_host, np.ndarray) else psi_host.numel() // self.npts
+        _check(lib().tdh_propagate_host(self._h, int(nst), C.c_void_p(_host_ptr(psi_host)), float(dt), int(nsteps),
+                                        int(order)))
+        return psi_host
+
+    # -- statistics / knobs
+    def last_launch_count(self) -> int:
+        return int(lib().tdh_last_launch_count(self._h))
+
+    def set_profiling(self, on: bool):
+        _check(lib().tdh_set_profiling(self._h, 1 if on else 0))
+
+    def last_kernel_seconds(self) -> dict:
+        buf = (C.c_double * NKERNELS)()
+        _check(lib().tdh_last_kernel_seconds(self._h, buf))
+        return {lib().tdh_kernel_name(i).decode(): buf[i] for i in range(NKERNELS)}
+
+    def set_chunk_states(self, chunk: int):
+        _check(lib().tdh_set_chunk_states(self._h, int(chunk)))
+
+
+def grid_for(wl, max_states: Optional[int] = None, device_v=None) -> Grid:
+    """Create a Grid for a workloads.Workload and load its potential and projectors."""
+    import torch
+    c = wl.cfg
+    g = Grid(c.n, c.length, c.kpt, c.ecut_abi, max_states or c.nst)
+    v = device_v if device_v is not None else torch.from_numpy(wl.v).cuda()
+    g.set_potential(v)
+    g.set_projectors(wl.proj)
+    return g

@@ -1,0 +1,93 @@
+// nl_kernels.cuh -- Kleinman-Bylander projection (first half of Eq. 9) on FP64 tensor cores.
+//
+// For atom I and state s:   dpi[s][c] = D_{I,c} dV sum_q beta_{I,c}[q] e^{+ik.d_q} psi_s[S_I[q]]
+// This is a real (C_I x P_I) matrix times a complex (P_I x n_st) block, gathered from the sphere's grid points.
+// One warp owns 8 states; per step of 4 sphere points it issues, for each tile of 8 channels,
+//     mma.sync.m8n8k4.f64   D(8 chan x 8 states) += A(8 chan x 4 points) * B(4 points x 8 states)
+// twice (real and imaginary parts of psi).  Fragment layout of m8n8k4 (PTX ISA): lane l holds A[l/4][l%4],
+// B[l%4][l/4] and C[l/4][2*(l%4) + {0,1}].  So lane l gathers ONE complex value psi_{s0 + l/4}[S[q0 + l%4]] with a
+// 16-byte load and that is both B fragments.  The sum over q is sequential inside the warp: deterministic, no atomics.
+// The second half of Eq. 9 (back-projection and scatter) is fused into plane_inv's epilogue, point-centric.
+#pragma once
+#include "fft_codelets.cuh"
+
+namespace tdh {
+
+struct AtomDesc {
+    int q0;      // first entry in the (sorted) sphere arrays
+    int np;      // P_I
+    int boff;    // offset of beta_{I,0}[0]; channel c at boff + c*np
+    int chan0;   // first channel in the global channel list
+    int nchan;   // C_I
+};
+
+__device__ __forceinline__ void dmma_m8n8k4(double (&c)[2], double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c[0]), "+d"(c[1])
+                 : "d"(a), "d"(b));
+}
+
+constexpr int NLP_WARPS = 8;            // warps per CTA
+constexpr int NLP_STATES = 8 * NLP_WARPS;  // states per CTA
+
+// grid: (natoms, ceil(nst / NLP_STATES)); MT = number of 8-channel tiles (C_I <= 8*MT)
+template <int MT>
+__global__ void __launch_bounds__(32 * NLP_WARPS)
+nl_project_kernel(const cd* __restrict__ psi, size_t npts, int nst, const AtomDesc* __restrict__ atoms,
+                  const int* __restrict__ sidx, const double* __restrict__ sbeta, const cd* __restrict__ sphase,
+                  const double* __restrict__ dscale, cd* __restrict__ dpi, int nchan_tot)
+{
+    const AtomDesc at = atoms[blockIdx.x];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int kq = lane & 3, r8 = lane >> 2;
+    const int s = blockIdx.y * NLP_STATES + warp * 8 + r8;      // this lane's state (B fragment column)
+    if (blockIdx.y * NLP_STATES + warp * 8 >= nst) return;      // whole warp idle (warp-uniform)
+    const bool s_ok = s < nst;
+    const cd* ps = psi + (size_t)(s_ok ? s : 0) * npts;
+    const int* idx = sidx + at.q0;
+    const cd* phs = sphase ? sphase + at.q0 : nullptr;
+
+    // two accumulator sets (even / odd k-steps) to keep two independent MMA chains in flight
+    double cre[2][MT][2], cim[2][MT][2];
+#pragma unroll
+    for (int u = 0; u < 2; ++u)
+#pragma unroll
+        for (int m = 0; m < MT; ++m) cre[u][m][0] = cre[u][m][1] = cim[u][m][0] = cim[u][m][1] = 0.0;
+
+    for (int q0 = 0; q0 < at.np; q0 += 8) {
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            const int q = q0 + 4 * u + kq;
+            const bool q_ok = q < at.np;
+            cd b = make_double2(0.0, 0.0);
+            if (q_ok && s_ok) {
+                b = __ldg(ps + __ldg(idx + q));
+                if (phs) b = cmul(b, __ldg(phs + q));
+            }
+#pragma unroll
+            for (int m = 0; m < MT; ++m) {
+                const int c = 8 * m + r8;                                   // A fragment row = channel
+                const double a = (q_ok && c < at.nchan) ? __ldg(sbeta + at.boff + (size_t)c * at.np + q) : 0.0;
+                dmma_m8n8k4(cre[u][m], a, b.x);
+                dmma_m8n8k4(cim[u][m], a, b.y);
+            }
+        }
+    }
+    // C fragment: row = channel 8m + lane/4, columns = states 2*(lane%4) + {0,1} of this warp
+#pragma unroll
+    for (int m = 0; m < MT; ++m) {
+        const int c = 8 * m + r8;
+        if (c < at.nchan) {
+            const double d = __ldg(dscale + at.chan0 + c);
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                const int so = blockIdx.y * NLP_STATES + warp * 8 + 2 * kq + j;
+                if (so < nst)
+                    dpi[(size_t)so * nchan_tot + at.chan0 + c] =
+                        make_double2(d * (cre[0][m][j] + cre[1][m][j]), d * (cim[0][m][j] + cim[1][m][j]));
+            }
+        }
+    }
+}
+
+}  // namespace tdh

@@ -1,0 +1,667 @@
+// tdh.cu -- C ABI of libtdh.so (include/tdh.h): handle, tables, projector re-indexing, launch orchestration.
+//
+// One Hamiltonian application on a chunk of states is four launches:
+//     nl_project  (gather + FP64-MMA projection, only with projectors)
+//     plane_fwd   (z,y forward FFT per (state,x) plane)            in  -> work
+//     xpencil     (x forward, 1/2|G+k|^2 scale + mask, x inverse)   work in place
+//     plane_inv   (y,z inverse FFT + epilogue alpha*(T+V+Vnl)phi + y)  work -> out
+// States are independent, so a block is pushed through this chain chunk by chunk; the chunk is sized
+// so that `work` (and, for propagate, the two Horner buffers) stay resident in the 126 MB L2 between kernels.
+// propagate runs ALL steps of one chunk before moving to the next chunk (H is fixed: readings R10, R16), evaluating
+// Eq. 8 in Horner form  psi + a1 H(psi + a2 H(psi + a3 H(psi + a4 H psi))),  a_k = -i dt / k,  so that every
+// application's epilogue is a single fused axpy and no accumulator is read-modified-written.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/tdh.h"
+#include "fft_kernels.cuh"
+#include "launch_tables.h"
+#include "nl_kernels.cuh"
+
+using tdh::cd;
+
+// ------------------------------------------------------------------------------------------------------------
+// errors
+// ------------------------------------------------------------------------------------------------------------
+static thread_local char g_err[512] = "";
+
+static int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CU(call)                                                                                          \
+    do {                                                                                                  \
+        cudaError_t e_ = (call);                                                                          \
+        if (e_ != cudaSuccess)                                                                            \
+            return fail(e_ == cudaErrorMemoryAllocation ? TDH_ENOMEM : TDH_ECUDA, "%s: %s (%s:%d)", #call, \
+                        cudaGetErrorString(e_), __FILE__, __LINE__);                                      \
+    } while (0)
+
+extern "C" const char* tdh_last_error(void) { return g_err; }
+
+// ------------------------------------------------------------------------------------------------------------
+// handle
+// ------------------------------------------------------------------------------------------------------------
+enum { K_NLPROJ = 0, K_PLANE_FWD = 1, K_XPENCIL = 2, K_PLANE_INV = 3 };
+static const char* const kKernelNames[TDH_NKERNELS] = {"nl_project", "plane_fwd", "xpencil", "plane_inv"};
+
+struct ProfRec { cudaEvent_t a, b; int k; };
+
+struct tdh_grid {
+    int n[3];
+    double len[3], kpt[3], ecut;
+    int max_states;
+    cudaStream_t stream;
+    size_t np;
+    double dv;
+    bool have_k;
+
+    double* d_v;          // V(r); zero-filled until set
+    bool have_v;
+    double* d_g2[3];      // (G_a + k_a)^2
+    cd* d_tw[3];          // exp(+2 pi i m / N_a)
+
+    int chunk_cap;        // states the workspace can hold
+    int chunk;            // states pushed through the chain together
+    cd* d_work;
+    cd* d_phi[2];
+
+    tdh::PlaneLaunch pl;
+    tdh::XLaunch xl;
+
+    // projectors
+    int natoms, nchan_tot, mt;
+    tdh::AtomDesc* d_atoms;
+    int* d_sidx;
+    double* d_sbeta;
+    cd* d_sphase;
+    double* d_dscale;
+    cd* d_dpi;
+    int* d_nl_start;
+    int4* d_nl_ent;
+    cd* d_nl_phase;
+
+    // host-buffer path
+    int host_chunk;
+    cd* d_hin[2];
+    cd* d_hout[2];
+    cudaStream_t s_h2d, s_d2h;
+    cudaEvent_t ev_in[2], ev_k[2], ev_out[2];
+
+    // statistics
+    int launch_count;
+    bool profiling;
+    std::vector<ProfRec> prof_pool;
+    size_t prof_used;
+    double ksec[TDH_NKERNELS];
+};
+
+static int size_index(int n) {
+    switch (n) {
+        case 16: return 0;
+        case 32: return 1;
+        case 48: return 2;
+        case 64: return 3;
+        case 96: return 4;
+        default: return -1;
+    }
+}
+
+// frequency index of array index a (numpy fftfreq convention; reading R7)
+static int freq_index(int a, int n) {
+    if (n % 2 == 0) return a < n / 2 ? a : a - n;
+    return a <= (n - 1) / 2 ? a : a - n;
+}
+
+static void free_projectors(tdh_grid* g) {
+    cudaFree(g->d_atoms); cudaFree(g->d_sidx); cudaFree(g->d_sbeta); cudaFree(g->d_sphase); cudaFree(g->d_dscale);
+    cudaFree(g->d_dpi); cudaFree(g->d_nl_start); cudaFree(g->d_nl_ent); cudaFree(g->d_nl_phase);
+    g->d_atoms = nullptr; g->d_sidx = nullptr; g->d_sbeta = nullptr; g->d_sphase = nullptr; g->d_dscale = nullptr;
+    g->d_dpi = nullptr; g->d_nl_start = nullptr; g->d_nl_ent = nullptr; g->d_nl_phase = nullptr;
+    g->natoms = 0; g->nchan_tot = 0; g->mt = 1;
+}
+
+static int default_chunk(const tdh_grid* g) {
+    // Keep work (+ in + out) L2-resident: aim at ~24 MB of workspace, but never fewer states than fill the GPU once.
+    const double state_bytes = (double)g->np * sizeof(cd);
+    int c = (int)std::floor(24.0 * 1048576.0 / state_bytes);
+    const int ctas_per_state = g->n[0] / g->pl.ppc;
+    const int fill = (2 * 148 + ctas_per_state - 1) / ctas_per_state;
+    c = std::max(c, fill);
+    if (const char* e = getenv("TDH_CHUNK_STATES")) { int v = atoi(e); if (v > 0) c = v; }
+    return std::max(1, std::min(c, g->chunk_cap));
+}
+
+extern "C" int tdh_create_grid(const int n[3], const double len[3], const double kpt[3], double ecut, int max_states,
+                               void* cuda_stream, tdh_grid** out) {
+    if (!n || !len || !kpt || !out) return fail(TDH_EINVAL, "tdh_create_grid: null argument");
+    if (max_states < 1) return fail(TDH_EINVAL, "tdh_create_grid: max_states must be >= 1");
+    for (int a = 0; a < 3; ++a) {
+        if (!(len[a] > 0.0) || !std::isfinite(len[a])) return fail(TDH_EINVAL, "tdh_create_grid: len[%d] must be > 0", a);
+        if (!std::isfinite(kpt[a])) return fail(TDH_EINVAL, "tdh_create_grid: kpt[%d] not finite", a);
+        if (size_index(n[a]) < 0)
+            return fail(TDH_EUNSUPPORTED, "tdh_create_grid: n[%d] = %d unsupported (supported: 16, 32, 48, 64, 96)", a, n[a]);
+    }
+    int ndev = 0;
+    CU(cudaGetDeviceCount(&ndev));
+    if (ndev < 1) return fail(TDH_ECUDA, "tdh_create_grid: no CUDA device (there is no CPU fallback)");
+
+    tdh_grid* g = new (std::nothrow) tdh_grid();
+    if (!g) return fail(TDH_ENOMEM, "tdh_create_grid: host allocation failed");
+    for (int a = 0; a < 3; ++a) { g->n[a] = n[a]; g->len[a] = len[a]; g->kpt[a] = kpt[a]; }
+    g->ecut = (ecut > 0.0 && std::isfinite(ecut)) ? ecut : -1.0;
+    g->max_states = max_states;
+    g->stream = (cudaStream_t)cuda_stream;
+    g->np = (size_t)n[0] * n[1] * n[2];
+    g->dv = (len[0] / n[0]) * (len[1] / n[1]) * (len[2] / n[2]);
+    g->have_k = kpt[0] != 0.0 || kpt[1] != 0.0 || kpt[2] != 0.0;
+    g->mt = 1;
+
+    bool ok = false;
+    switch (n[2]) {
+        case 16: ok = tdh::plane_launch_nz16(n[1], &g->pl); break;
+        case 32: ok = tdh::plane_launch_nz32(n[1], &g->pl); break;
+        case 48: ok = tdh::plane_launch_nz48(n[1], &g->pl); break;
+        case 64: ok = tdh::plane_launch_nz64(n[1], &g->pl); break;
+        case 96: ok = tdh::plane_launch_nz96(n[1], &g->pl); break;
+    }
+    ok = ok && tdh::xpencil_launch(n[0], &g->xl);
+    if (!ok) { delete g; return fail(TDH_EUNSUPPORTED, "tdh_create_grid: no kernel for this grid"); }
+
+    int rc = TDH_OK;
+    auto body = [&]() -> int {
+        CU(cudaFuncSetAttribute(g->pl.fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g->pl.smem));
+        CU(cudaFuncSetAttribute(g->pl.inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g->pl.smem));
+        // tables: built on the host exactly as the oracle builds its G vectors (two_pi * m / L + k, then squared)
+        const double two_pi = 6.283185307179586476925286766559;
+        for (int a = 0; a < 3; ++a) {
+            std::vector<double> g2(n[a]);
+            std::vector<cd> tw(n[a]);
+            for (int i = 0; i < n[a]; ++i) {
+                const double ga = two_pi * freq_index(i, n[a]) / len[a] + kpt[a];
+                g2[i] = ga * ga;
+                const long double ang = 6.283185307179586476925286766559005768L * (long double)i / (long double)n[a];
+                tw[i] = make_double2((double)cosl(ang), (double)sinl(ang));
+            }
+            CU(cudaMalloc(&g->d_g2[a], sizeof(double) * n[a]));
+            CU(cudaMalloc(&g->d_tw[a], sizeof(cd) * n[a]));
+            CU(cudaMemcpy(g->d_g2[a], g2.data(), sizeof(double) * n[a], cudaMemcpyHostToDevice));
+            CU(cudaMemcpy(g->d_tw[a], tw.data(), sizeof(cd) * n[a], cudaMemcpyHostToDevice));
+        }
+        CU(cudaMalloc(&g->d_v, sizeof(double) * g->np));
+        CU(cudaMemset(g->d_v, 0, sizeof(double) * g->np));
+        g->have_v = false;
+        // workspace: up to 1 GiB per buffer
+        const size_t state_bytes = g->np * sizeof(cd);
+        size_t cap = std::max<size_t>(1, ((size_t)1 << 30) / state_bytes);
+        g->chunk_cap = (int)std::min<size_t>(cap, (size_t)max_states);
+        CU(cudaMalloc(&g->d_work, state_bytes * g->chunk_cap));
+        CU(cudaMalloc(&g->d_phi[0], state_bytes * g->chunk_cap));
+        CU(cudaMalloc(&g->d_phi[1], state_bytes * g->chunk_cap));
+        g->chunk = default_chunk(g);
+        return TDH_OK;
+    };
+    rc = body();
+    if (rc != TDH_OK) { tdh_destroy_grid(g); return rc; }
+    *out = g;
+    return TDH_OK;
+}
+
+extern "C" int tdh_destroy_grid(tdh_grid* g) {
+    if (!g) return TDH_OK;
+    cudaStreamSynchronize(g->stream);
+    free_projectors(g);
+    cudaFree(g->d_v);
+    for (int a = 0; a < 3; ++a) { cudaFree(g->d_g2[a]); cudaFree(g->d_tw[a]); }
+    cudaFree(g->d_work); cudaFree(g->d_phi[0]); cudaFree(g->d_phi[1]);
+    for (int i = 0; i < 2; ++i) {
+        cudaFree(g->d_hin[i]); cudaFree(g->d_hout[i]);
+        if (g->ev_in[i]) cudaEventDestroy(g->ev_in[i]);
+        if (g->ev_k[i]) cudaEventDestroy(g->ev_k[i]);
+        if (g->ev_out[i]) cudaEventDestroy(g->ev_out[i]);
+    }
+    if (g->s_h2d) cudaStreamDestroy(g->s_h2d);
+    if (g->s_d2h) cudaStreamDestroy(g->s_d2h);
+    for (auto& r : g->prof_pool) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    delete g;
+    return TDH_OK;
+}
+
+extern "C" int tdh_set_potential(tdh_grid* g, const double* v_dev) {
+    if (!g) return fail(TDH_EINVAL, "tdh_set_potential: null handle");
+    if (v_dev) {
+        CU(cudaMemcpyAsync(g->d_v, v_dev, sizeof(double) * g->np, cudaMemcpyDeviceToDevice, g->stream));
+        g->have_v = true;
+    } else {
+        CU(cudaMemsetAsync(g->d_v, 0, sizeof(double) * g->np, g->stream));
+        g->have_v = false;
+    }
+    CU(cudaStreamSynchronize(g->stream));
+    return TDH_OK;
+}
+
+extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_off, const int32_t* sph_idx,
+                                  const double* sph_disp, const int32_t* chan_off, const double* beta,
+                                  const double* dcoef) {
+    if (!g) return fail(TDH_EINVAL, "tdh_set_projectors: null handle");
+    if (natoms < 0) return fail(TDH_EINVAL, "tdh_set_projectors: natoms < 0");
+    CU(cudaStreamSynchronize(g->stream));
+    free_projectors(g);
+    if (natoms == 0) return TDH_OK;
+    if (!sph_off || !sph_idx || !chan_off || !beta || !dcoef)
+        return fail(TDH_EINVAL, "tdh_set_projectors: null table with natoms > 0");
+    if (g->have_k && !sph_disp) return fail(TDH_EINVAL, "tdh_set_projectors: sph_disp is required when k != 0");
+    if (sph_off[0] != 0 || chan_off[0] != 0) return fail(TDH_EINVAL, "tdh_set_projectors: offsets must start at 0");
+    for (int a = 0; a < natoms; ++a)
+        if (sph_off[a + 1] < sph_off[a] || chan_off[a + 1] < chan_off[a])
+            return fail(TDH_EINVAL, "tdh_set_projectors: offsets must be non-decreasing");
+    const int64_t ptot = sph_off[natoms];
+    const int ctot = chan_off[natoms];
+    if (ptot >= (int64_t)1 << 30) return fail(TDH_EUNSUPPORTED, "tdh_set_projectors: too many sphere points");
+
+    // ---- validate, sort each sphere by flat grid index (coalesced gathers), re-index beta, build phases
+    std::vector<int> stamp(g->np, -1);
+    std::vector<int> sidx(ptot);
+    std::vector<cd> sphase(g->have_k ? ptot : 0);
+    std::vector<tdh::AtomDesc> atoms(natoms);
+    std::vector<double> dscale(ctot);
+    size_t btot = 0;
+    int cmax = 0;
+    for (int a = 0; a < natoms; ++a) {
+        btot += (size_t)(chan_off[a + 1] - chan_off[a]) * (size_t)(sph_off[a + 1] - sph_off[a]);
+        cmax = std::max(cmax, chan_off[a + 1] - chan_off[a]);
+    }
+    if (btot >= (size_t)1 << 31) return fail(TDH_EUNSUPPORTED, "tdh_set_projectors: projector table too large");
+    if (cmax > 16) return fail(TDH_EUNSUPPORTED, "tdh_set_projectors: more than 16 channels on one atom");
+    std::vector<double> sbeta(btot);
+    std::vector<int> cover(g->np, 0);
+    std::vector<int> order;
+    size_t boff = 0;
+    for (int a = 0; a < natoms; ++a) {
+        const int64_t q0 = sph_off[a];
+        const int pn = (int)(sph_off[a + 1] - q0);
+        const int c0 = chan_off[a], nc = chan_off[a + 1] - c0;
+        for (int q = 0; q < pn; ++q) {
+            const int32_t p = sph_idx[q0 + q];
+            if (p < 0 || (size_t)p >= g->np)
+                return fail(TDH_EINDEX, "tdh_set_projectors: sph_idx[%lld] = %d out of range", (long long)(q0 + q), p);
+            if (stamp[p] == a)
+                return fail(TDH_EINDEX, "tdh_set_projectors: grid point %d listed twice for atom %d", p, a);
+            stamp[p] = a;
+            cover[p] += 1;
+        }
+        order.resize(pn);
+        for (int q = 0; q < pn; ++q) order[q] = q;
+        std::sort(order.begin(), order.end(), [&](int x, int y) { return sph_idx[q0 + x] < sph_idx[q0 + y]; });
+        for (int j = 0; j < pn; ++j) {
+            const int q = order[j];
+            sidx[q0 + j] = sph_idx[q0 + q];
+            if (g->have_k) {
+                const double* d = sph_disp + 3 * (q0 + q);
+                const double arg = g->kpt[0] * d[0] + g->kpt[1] * d[1] + g->kpt[2] * d[2];
+                sphase[q0 + j] = make_double2(cos(arg), sin(arg));
+            }
+            for (int c = 0; c < nc; ++c) sbeta[boff + (size_t)c * pn + j] = beta[boff + (size_t)c * pn + q];
+        }
+        for (int c = 0; c < nc; ++c) dscale[c0 + c] = dcoef[c0 + c] * g->dv;
+        atoms[a].q0 = (int)q0; atoms[a].np = pn; atoms[a].boff = (int)boff; atoms[a].chan0 = c0; atoms[a].nchan = nc;
+        boff += (size_t)nc * pn;
+    }
+    // ---- point-centric inverse map for the atomic-free scatter
+    std::vector<int> nl_start(g->np, -1);
+    {
+        int run = 0;
+        for (size_t p = 0; p < g->np; ++p)
+            if (cover[p] > 0) { nl_start[p] = run; run += cover[p]; }
+    }
+    std::vector<int4> ent(ptot);
+    std::vector<cd> ent_phase(g->have_k ? ptot : 0);
+    std::vector<int> fill(g->np, 0);
+    for (int a = 0; a < natoms; ++a) {
+        const tdh::AtomDesc& at = atoms[a];
+        for (int j = 0; j < at.np; ++j) {
+            const int p = sidx[at.q0 + j];
+            const int e = nl_start[p] + fill[p];
+            fill[p] += 1;
+            const int last = fill[p] == cover[p] ? 1 : 0;
+            ent[e] = make_int4(at.boff + j, at.np, at.chan0, at.nchan | (last << 16));
+            if (g->have_k) ent_phase[e] = sphase[at.q0 + j];
+        }
+    }
+
+    auto up = [&](auto** dptr, const auto& vec) -> int {
+        using T = typename std::remove_reference<decltype(vec)>::type::value_type;
+        if (vec.empty()) { *dptr = nullptr; return TDH_OK; }
+        CU(cudaMalloc(dptr, sizeof(T) * vec.size()));
+        CU(cudaMemcpy(*dptr, vec.data(), sizeof(T) * vec.size(), cudaMemcpyHostToDevice));
+        return TDH_OK;
+    };
+    int rc;
+    if ((rc = up(&g->d_atoms, atoms)) || (rc = up(&g->d_sidx, sidx)) || (rc = up(&g->d_sbeta, sbeta)) ||
+        (rc = up(&g->d_sphase, sphase)) || (rc = up(&g->d_dscale, dscale)) || (rc = up(&g->d_nl_start, nl_start)) ||
+        (rc = up(&g->d_nl_ent, ent)) || (rc = up(&g->d_nl_phase, ent_phase))) {
+        free_projectors(g);
+        return rc;
+    }
+    cudaError_t e = cudaMalloc(&g->d_dpi, sizeof(cd) * (size_t)g->chunk_cap * ctot);
+    if (e != cudaSuccess) { free_projectors(g); return fail(TDH_ENOMEM, "tdh_set_projectors: %s", cudaGetErrorString(e)); }
+    g->natoms = natoms;
+    g->nchan_tot = ctot;
+    g->mt = cmax <= 8 ? 1 : 2;
+    return TDH_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// launches
+// ------------------------------------------------------------------------------------------------------------
+static int prof_begin(tdh_grid* g, int k) {
+    if (!g->profiling) return TDH_OK;
+    if (g->prof_used == g->prof_pool.size()) {
+        ProfRec r;
+        CU(cudaEventCreate(&r.a));
+        CU(cudaEventCreate(&r.b));
+        r.k = k;
+        g->prof_pool.push_back(r);
+    }
+    g->prof_pool[g->prof_used].k = k;
+    CU(cudaEventRecord(g->prof_pool[g->prof_used].a, g->stream));
+    return TDH_OK;
+}
+static int prof_end(tdh_grid* g) {
+    if (!g->profiling) return TDH_OK;
+    CU(cudaEventRecord(g->prof_pool[g->prof_used].b, g->stream));
+    g->prof_used += 1;
+    return TDH_OK;
+}
+static int prof_collect(tdh_grid* g) {
+    if (!g->profiling) return TDH_OK;
+    CU(cudaStreamSynchronize(g->stream));
+    for (size_t i = 0; i < g->prof_used; ++i) {
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, g->prof_pool[i].a, g->prof_pool[i].b));
+        g->ksec[g->prof_pool[i].k] += 1e-3 * ms;
+    }
+    g->prof_used = 0;
+    return TDH_OK;
+}
+static void stats_reset(tdh_grid* g) {
+    g->launch_count = 0;
+    g->prof_used = 0;
+    for (int i = 0; i < TDH_NKERNELS; ++i) g->ksec[i] = 0.0;
+}
+
+#define LAUNCH(kid, func, grid, block, smem, args)                                                 \
+    do {                                                                                           \
+        int rc_ = prof_begin(g, kid);                                                              \
+        if (rc_) return rc_;                                                                       \
+        CU(cudaLaunchKernel(func, grid, block, args, smem, g->stream));                            \
+        g->launch_count += 1;                                                                      \
+        rc_ = prof_end(g);                                                                         \
+        if (rc_) return rc_;                                                                       \
+    } while (0)
+
+static int launch_plane_fwd(tdh_grid* g, int nst, const cd* in, cd* out) {
+    const cd* twy = g->d_tw[1];
+    const cd* twz = g->d_tw[2];
+    void* args[] = {(void*)&in, (void*)&out, (void*)&twy, (void*)&twz};
+    const unsigned grid = (unsigned)((size_t)nst * g->n[0] / g->pl.ppc);
+    LAUNCH(K_PLANE_FWD, g->pl.fwd, dim3(grid), dim3(g->pl.threads), g->pl.smem, args);
+    return TDH_OK;
+}
+
+static int launch_xpencil(tdh_grid* g, int nst, cd* w, int mode) {
+    tdh::Kinetic kin;
+    kin.g2x = g->d_g2[0]; kin.g2y = g->d_g2[1]; kin.g2z = g->d_g2[2];
+    kin.ecut = g->ecut;
+    kin.scale = 1.0 / (double)g->np;
+    kin.nz = g->n[2];
+    int nynz = g->n[1] * g->n[2];
+    const cd* twx = g->d_tw[0];
+    void* args[] = {(void*)&w, (void*)&nynz, (void*)&twx, (void*)&kin};
+    const void* f = mode == 0 ? g->xl.fused : (mode == 1 ? g->xl.fwd : g->xl.inv);
+    LAUNCH(K_XPENCIL, f, dim3(nynz / tdh::XP_LPC, nst), dim3(g->xl.threads), 0, args);
+    return TDH_OK;
+}
+
+static int launch_plane_inv(tdh_grid* g, int nst, const cd* in, cd* out, const tdh::Epilogue& ep) {
+    const cd* twy = g->d_tw[1];
+    const cd* twz = g->d_tw[2];
+    void* args[] = {(void*)&in, (void*)&out, (void*)&twy, (void*)&twz, (void*)&ep};
+    const unsigned grid = (unsigned)((size_t)nst * g->n[0] / g->pl.ppc);
+    LAUNCH(K_PLANE_INV, g->pl.inv, dim3(grid), dim3(g->pl.threads), g->pl.smem, args);
+    return TDH_OK;
+}
+
+static int launch_nl_project(tdh_grid* g, int nst, const cd* in) {
+    size_t npts = g->np;
+    const tdh::AtomDesc* atoms = g->d_atoms;
+    const int* sidx = g->d_sidx;
+    const double* sbeta = g->d_sbeta;
+    const cd* sphase = g->d_sphase;
+    const double* dscale = g->d_dscale;
+    cd* dpi = g->d_dpi;
+    int nct = g->nchan_tot;
+    void* args[] = {(void*)&in, (void*)&npts, (void*)&nst, (void*)&atoms, (void*)&sidx, (void*)&sbeta,
+                    (void*)&sphase, (void*)&dscale, (void*)&dpi, (void*)&nct};
+    const void* f = g->mt == 1 ? reinterpret_cast<const void*>(&tdh::nl_project_kernel<1>)
+                               : reinterpret_cast<const void*>(&tdh::nl_project_kernel<2>);
+    dim3 grid(g->natoms, (nst + tdh::NLP_STATES - 1) / tdh::NLP_STATES);
+    LAUNCH(K_NLPROJ, f, grid, dim3(32 * tdh::NLP_WARPS), 0, args);
+    return TDH_OK;
+}
+
+// out = alpha * H in + yv   for one chunk (nst <= chunk_cap); in/out/yv point at the chunk's first state
+static int apply_chunk(tdh_grid* g, int nst, const cd* in, cd* out, cd alpha, const cd* yv) {
+    int rc;
+    if (g->natoms > 0 && (rc = launch_nl_project(g, nst, in))) return rc;
+    if ((rc = launch_plane_fwd(g, nst, in, g->d_work))) return rc;
+    if ((rc = launch_xpencil(g, nst, g->d_work, 0))) return rc;
+    tdh::Epilogue ep;
+    ep.phi = in;
+    ep.v = g->have_v ? g->d_v : nullptr;
+    ep.yv = yv;
+    ep.alpha = alpha;
+    ep.nx = g->n[0];
+    ep.nl_start = g->natoms > 0 ? g->d_nl_start : nullptr;
+    ep.nl_ent = g->d_nl_ent;
+    ep.nl_phase = g->d_nl_phase;
+    ep.nl_beta = g->d_sbeta;
+    ep.dpi = g->d_dpi;
+    ep.nchan_tot = g->nchan_tot;
+    return launch_plane_inv(g, nst, g->d_work, out, ep);
+}
+
+static int apply_block(tdh_grid* g, int nst, const cd* psi, cd* hpsi) {
+    for (int s0 = 0; s0 < nst; s0 += g->chunk) {
+        const int c = std::min(g->chunk, nst - s0);
+        int rc = apply_chunk(g, c, psi + (size_t)s0 * g->np, hpsi + (size_t)s0 * g->np, make_double2(1.0, 0.0), nullptr);
+        if (rc) return rc;
+    }
+    return TDH_OK;
+}
+
+// all steps of one chunk, Horner form of Eq. 8
+static int propagate_chunk(tdh_grid* g, int nst, cd* psi, double dt, int nsteps) {
+    cd* pa = g->d_phi[0];
+    cd* pb = g->d_phi[1];
+    for (int step = 0; step < nsteps; ++step) {
+        int rc;
+        if ((rc = apply_chunk(g, nst, psi, pa, make_double2(0.0, -dt / 4.0), psi))) return rc;
+        if ((rc = apply_chunk(g, nst, pa, pb, make_double2(0.0, -dt / 3.0), psi))) return rc;
+        if ((rc = apply_chunk(g, nst, pb, pa, make_double2(0.0, -dt / 2.0), psi))) return rc;
+        if ((rc = apply_chunk(g, nst, pa, psi, make_double2(0.0, -dt), psi))) return rc;
+    }
+    return TDH_OK;
+}
+
+static int propagate_block(tdh_grid* g, int nst, cd* psi, double dt, int nsteps) {
+    for (int s0 = 0; s0 < nst; s0 += g->chunk) {
+        const int c = std::min(g->chunk, nst - s0);
+        int rc = propagate_chunk(g, c, psi + (size_t)s0 * g->np, dt, nsteps);
+        if (rc) return rc;
+    }
+    return TDH_OK;
+}
+
+static bool overlaps(const void* a, const void* b, size_t bytes) {
+    const char* x = (const char*)a;
+    const char* y = (const char*)b;
+    return x < y + bytes && y < x + bytes;
+}
+
+extern "C" int tdh_apply_hamiltonian(tdh_grid* g, int nst, const tdh_c128* psi_dev, tdh_c128* hpsi_dev) {
+    if (!g || !psi_dev || !hpsi_dev) return fail(TDH_EINVAL, "tdh_apply_hamiltonian: null argument");
+    if (nst < 1 || nst > g->max_states) return fail(TDH_EINVAL, "tdh_apply_hamiltonian: nst = %d outside [1, %d]", nst, g->max_states);
+    if (overlaps(psi_dev, hpsi_dev, (size_t)nst * g->np * sizeof(cd)))
+        return fail(TDH_EINVAL, "tdh_apply_hamiltonian: psi and hpsi overlap");
+    stats_reset(g);
+    int rc = apply_block(g, nst, (const cd*)psi_dev, (cd*)hpsi_dev);
+    if (rc) return rc;
+    return prof_collect(g);
+}
+
+extern "C" int tdh_propagate(tdh_grid* g, int nst, tdh_c128* psi_dev, double dt, int nsteps, int order) {
+    if (!g || !psi_dev) return fail(TDH_EINVAL, "tdh_propagate: null argument");
+    if (nst < 1 || nst > g->max_states) return fail(TDH_EINVAL, "tdh_propagate: nst = %d outside [1, %d]", nst, g->max_states);
+    if (order != 4) return fail(TDH_EINVAL, "tdh_propagate: order must be 4");
+    if (nsteps < 0 || !std::isfinite(dt)) return fail(TDH_EINVAL, "tdh_propagate: bad dt / nsteps");
+    stats_reset(g);
+    int rc = propagate_block(g, nst, (cd*)psi_dev, dt, nsteps);
+    if (rc) return rc;
+    return prof_collect(g);
+}
+
+extern "C" int tdh_fft3d(tdh_grid* g, int nst, tdh_c128* psi_dev, int sign) {
+    if (!g || !psi_dev) return fail(TDH_EINVAL, "tdh_fft3d: null argument");
+    if (nst < 1) return fail(TDH_EINVAL, "tdh_fft3d: nst < 1");
+    if (sign != 1 && sign != -1) return fail(TDH_EINVAL, "tdh_fft3d: sign must be -1 or +1");
+    stats_reset(g);
+    cd* p = (cd*)psi_dev;
+    // the launch grid's y dimension is limited to 65535 states per call
+    for (int s0 = 0; s0 < nst; s0 += 32768) {
+        const int c = std::min(32768, nst - s0);
+        cd* q = p + (size_t)s0 * g->np;
+        int rc;
+        if (sign < 0) {
+            if ((rc = launch_plane_fwd(g, c, q, q))) return rc;
+            if ((rc = launch_xpencil(g, c, q, 1))) return rc;
+        } else {
+            if ((rc = launch_xpencil(g, c, q, 2))) return rc;
+            tdh::Epilogue ep;
+            memset(&ep, 0, sizeof(ep));
+            ep.alpha = make_double2(1.0, 0.0);
+            ep.nx = g->n[0];
+            if ((rc = launch_plane_inv(g, c, q, q, ep))) return rc;
+        }
+    }
+    return prof_collect(g);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// host-buffer entry points: chunked, double-buffered H2D -> kernels -> D2H on three streams
+// ------------------------------------------------------------------------------------------------------------
+static int host_path_init(tdh_grid* g) {
+    if (g->d_hin[0]) return TDH_OK;
+    g->host_chunk = g->chunk_cap;
+    // bound the four staging buffers to 512 MiB each
+    const size_t state_bytes = g->np * sizeof(cd);
+    g->host_chunk = (int)std::max<size_t>(1, std::min<size_t>((size_t)g->host_chunk, ((size_t)512 << 20) / state_bytes));
+    for (int i = 0; i < 2; ++i) {
+        CU(cudaMalloc(&g->d_hin[i], state_bytes * g->host_chunk));
+        CU(cudaMalloc(&g->d_hout[i], state_bytes * g->host_chunk));
+        CU(cudaEventCreateWithFlags(&g->ev_in[i], cudaEventDisableTiming));
+        CU(cudaEventCreateWithFlags(&g->ev_k[i], cudaEventDisableTiming));
+        CU(cudaEventCreateWithFlags(&g->ev_out[i], cudaEventDisableTiming));
+    }
+    CU(cudaStreamCreateWithFlags(&g->s_h2d, cudaStreamNonBlocking));
+    CU(cudaStreamCreateWithFlags(&g->s_d2h, cudaStreamNonBlocking));
+    return TDH_OK;
+}
+
+static int host_pipeline(tdh_grid* g, int nst, const cd* in_host, cd* out_host, bool propagate, double dt, int nsteps) {
+    int rc = host_path_init(g);
+    if (rc) return rc;
+    stats_reset(g);
+    const size_t state_bytes = g->np * sizeof(cd);
+    const int hc = g->host_chunk;
+    int it = 0;
+    for (int s0 = 0; s0 < nst; s0 += hc, ++it) {
+        const int c = std::min(hc, nst - s0);
+        const int slot = it & 1;
+        const size_t off = (size_t)s0 * g->np;
+        // H2D into d_hin[slot] once the kernels (apply) or the D2H (propagate) that last used it are done
+        if (it >= 2) CU(cudaStreamWaitEvent(g->s_h2d, propagate ? g->ev_out[slot] : g->ev_k[slot], 0));
+        CU(cudaMemcpyAsync(g->d_hin[slot], in_host + off, state_bytes * c, cudaMemcpyHostToDevice, g->s_h2d));
+        CU(cudaEventRecord(g->ev_in[slot], g->s_h2d));
+        CU(cudaStreamWaitEvent(g->stream, g->ev_in[slot], 0));
+        if (propagate) {
+            if ((rc = propagate_block(g, c, g->d_hin[slot], dt, nsteps))) return rc;
+        } else {
+            if (it >= 2) CU(cudaStreamWaitEvent(g->stream, g->ev_out[slot], 0));
+            if ((rc = apply_block(g, c, g->d_hin[slot], g->d_hout[slot]))) return rc;
+        }
+        CU(cudaEventRecord(g->ev_k[slot], g->stream));
+        CU(cudaStreamWaitEvent(g->s_d2h, g->ev_k[slot], 0));
+        CU(cudaMemcpyAsync(out_host + off, propagate ? g->d_hin[slot] : g->d_hout[slot], state_bytes * c,
+                           cudaMemcpyDeviceToHost, g->s_d2h));
+        CU(cudaEventRecord(g->ev_out[slot], g->s_d2h));
+    }
+    CU(cudaStreamSynchronize(g->s_h2d));
+    CU(cudaStreamSynchronize(g->stream));
+    CU(cudaStreamSynchronize(g->s_d2h));
+    return prof_collect(g);
+}
+
+extern "C" int tdh_apply_hamiltonian_host(tdh_grid* g, int nst, const tdh_c128* psi_host, tdh_c128* hpsi_host) {
+    if (!g || !psi_host || !hpsi_host) return fail(TDH_EINVAL, "tdh_apply_hamiltonian_host: null argument");
+    if (nst < 1) return fail(TDH_EINVAL, "tdh_apply_hamiltonian_host: nst < 1");
+    if (overlaps(psi_host, hpsi_host, (size_t)nst * g->np * sizeof(cd)))
+        return fail(TDH_EINVAL, "tdh_apply_hamiltonian_host: psi and hpsi overlap");
+    return host_pipeline(g, nst, (const cd*)psi_host, (cd*)hpsi_host, false, 0.0, 0);
+}
+
+extern "C" int tdh_propagate_host(tdh_grid* g, int nst, tdh_c128* psi_host, double dt, int nsteps, int order) {
+    if (!g || !psi_host) return fail(TDH_EINVAL, "tdh_propagate_host: null argument");
+    if (nst < 1) return fail(TDH_EINVAL, "tdh_propagate_host: nst < 1");
+    if (order != 4) return fail(TDH_EINVAL, "tdh_propagate_host: order must be 4");
+    if (nsteps < 0 || !std::isfinite(dt)) return fail(TDH_EINVAL, "tdh_propagate_host: bad dt / nsteps");
+    return host_pipeline(g, nst, (const cd*)psi_host, (cd*)psi_host, true, dt, nsteps);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// statistics / knobs
+// ------------------------------------------------------------------------------------------------------------
+extern "C" int tdh_last_launch_count(const tdh_grid* g) { return g ? g->launch_count : 0; }
+
+extern "C" int tdh_set_profiling(tdh_grid* g, int on) {
+    if (!g) return fail(TDH_EINVAL, "tdh_set_profiling: null handle");
+    g->profiling = on != 0;
+    return TDH_OK;
+}
+
+extern "C" int tdh_last_kernel_seconds(const tdh_grid* g, double out[TDH_NKERNELS]) {
+    if (!g || !out) return fail(TDH_EINVAL, "tdh_last_kernel_seconds: null argument");
+    for (int i = 0; i < TDH_NKERNELS; ++i) out[i] = g->ksec[i];
+    return TDH_OK;
+}
+
+extern "C" const char* tdh_kernel_name(int i) { return (i >= 0 && i < TDH_NKERNELS) ? kKernelNames[i] : ""; }
+
+extern "C" int tdh_set_chunk_states(tdh_grid* g, int chunk) {
+    if (!g) return fail(TDH_EINVAL, "tdh_set_chunk_states: null handle");
+    if (chunk < 0) return fail(TDH_EINVAL, "tdh_set_chunk_states: chunk < 0");
+    g->chunk = chunk == 0 ? default_chunk(g) : std::min(chunk, g->chunk_cap);
+    return TDH_OK;
+}

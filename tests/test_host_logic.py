@@ -1,0 +1,148 @@
+"""CPU-only checks: the C-ABI library loads and exports every declared symbol, fails loudly without a GPU,
+the generator is deterministic, and the multi-rank sharding logic works under gloo with world_size 2."""
+import ctypes
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+from paper_2106_03872_b200 import shard
+from paper_2106_03872_b200 import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def tdh_lib():
+    from paper_2106_03872_b200 import build, binding
+    build.build()
+    return binding.lib()
+
+
+def test_library_exports_every_declared_symbol(tdh_lib):
+    from paper_2106_03872_b200 import binding
+    header = open(os.path.join(ROOT, "include", "tdh.h")).read()
+    declared = set(re.findall(r"\b(tdh_[a-z0-9_]+)\s*\(", header))
+    declared -= {"tdh_grid", "tdh_c128"}
+    assert declared == set(binding.SYMBOLS)
+    for name in declared:
+        assert hasattr(tdh_lib, name), name
+    assert isinstance(tdh_lib.tdh_last_error(), bytes)
+    assert tdh_lib.tdh_kernel_name(0) == b"nl_project"
+
+
+def test_argument_checks_need_no_gpu(tdh_lib):
+    """Invalid arguments are rejected before any CUDA call."""
+    h = ctypes.c_void_p()
+    n = (ctypes.c_int * 3)(20, 16, 16)
+    l3 = (ctypes.c_double * 3)(1.0, 1.0, 1.0)
+    k3 = (ctypes.c_double * 3)(0.0, 0.0, 0.0)
+    assert tdh_lib.tdh_create_grid(n, l3, k3, -1.0, 1, None, ctypes.byref(h)) == -2
+    assert b"unsupported" in tdh_lib.tdh_last_error()
+    n = (ctypes.c_int * 3)(16, 16, 16)
+    assert tdh_lib.tdh_create_grid(n, l3, k3, -1.0, 0, None, ctypes.byref(h)) == -1
+    assert tdh_lib.tdh_create_grid(None, l3, k3, -1.0, 1, None, ctypes.byref(h)) == -1
+    assert tdh_lib.tdh_apply_hamiltonian(None, 1, None, None) == -1
+    assert tdh_lib.tdh_destroy_grid(None) == 0
+
+
+def test_product_fails_loudly_without_gpu(tdh_lib):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    from paper_2106_03872_b200 import binding
+    with pytest.raises(binding.TdhError):
+        binding.Grid((16, 16, 16), (1.0, 1.0, 1.0))
+    h = ctypes.c_void_p()
+    n = (ctypes.c_int * 3)(16, 16, 16)
+    l3 = (ctypes.c_double * 3)(1.0, 1.0, 1.0)
+    k3 = (ctypes.c_double * 3)(0.0, 0.0, 0.0)
+    assert tdh_lib.tdh_create_grid(n, l3, k3, -1.0, 1, None, ctypes.byref(h)) == -4     # TDH_ECUDA, no fallback
+
+
+def test_product_does_not_import_oracle():
+    """The package must never reach into oracle/ (a product path through the oracle voids parity)."""
+    pkg = os.path.join(ROOT, "paper_2106_03872_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".inc")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in text and "from oracle" not in text and "ref_tdh" not in text, f
+    for f in ("ref_tdh.c", "ref.py", "build.py"):
+        text = open(os.path.join(ROOT, "oracle", f)).read()
+        assert "paper_2106_03872_b200" not in text.replace("paper_2106_03872_b200/csrc", ""), f
+
+
+def test_generator_is_deterministic_and_shaped():
+    for name in W.CONFIG_ORDER:
+        cfg = W.CONFIGS[name]
+        pos = W.atom_positions(cfg)
+        assert pos.shape == (cfg.natoms, 3) and (pos >= 0).all() and (pos < cfg.length[0]).all()
+        assert np.array_equal(pos, W.atom_positions(cfg))
+    cfg = W.CONFIGS["small"]
+    wl = W.make(cfg)
+    assert wl.v.shape == cfg.n and wl.v.min() < -3.0
+    pr = wl.proj
+    assert pr.chan_off[-1] == 8 * 4 and len(pr.beta) == 4 * len(pr.sph_idx)
+    per_sphere = np.diff(pr.sph_off)
+    assert 600 < per_sphere.min() and per_sphere.max() < 680          # P = 636 [627-647]
+    a = W.state(cfg, 5)
+    assert abs(cfg.dv * np.sum(np.abs(a) ** 2) - 1.0) < 1e-12
+    # sphere membership is strict |d| < rc and displacements are minimum images
+    r = np.linalg.norm(pr.sph_disp, axis=1)
+    assert r.max() < cfg.rc
+    # large config: overlapping spheres along x (R13)
+    big = W.CONFIGS["large"]
+    p2 = W.atom_positions(big)
+    assert len(p2) == 128
+
+
+def test_state_range_partitions():
+    for nst in (0, 1, 7, 64, 1024):
+        for world in (1, 2, 3, 8):
+            cover = []
+            for r in range(world):
+                s0, s1 = shard.state_range(r, world, nst)
+                assert 0 <= s0 <= s1 <= nst
+                cover += list(range(s0, s1))
+            assert cover == list(range(nst))
+            sizes = [shard.state_range(r, world, nst)[1] - shard.state_range(r, world, nst)[0] for r in range(world)]
+            assert max(sizes) - min(sizes) <= 1
+
+
+_WORKER = r"""
+import os, sys
+sys.path.insert(0, {root!r})
+import torch, torch.distributed as dist
+from paper_2106_03872_b200 import shard
+dist.init_process_group("gloo", init_method="tcp://127.0.0.1:{port}", rank=int(sys.argv[1]), world_size=2)
+rank = dist.get_rank()
+s0, s1 = shard.state_range(rank, 2, 9)
+got = [None, None]
+dist.all_gather_object(got, (s0, s1))
+assert got == [(0, 5), (5, 9)], got
+t = shard.max_over_ranks(1.0 + rank)
+assert t == 2.0, t
+dist.barrier()
+dist.destroy_process_group()
+print("ok", rank)
+"""
+
+
+def test_world_size_2_gloo(tmp_path):
+    """N>1 path on CPU: two gloo ranks shard the states with no data-path collective and agree on the max time."""
+    import socket
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    script = tmp_path / "worker.py"
+    script.write_text(_WORKER.format(root=ROOT, port=port))
+    procs = [subprocess.Popen([sys.executable, str(script), str(r)], stdout=subprocess.PIPE, stderr=subprocess.STDOUT)
+             for r in range(2)]
+    outs = [p.communicate(timeout=120)[0].decode() for p in procs]
+    for r, (p, o) in enumerate(zip(procs, outs)):
+        assert p.returncode == 0 and f"ok {r}" in o, o
