@@ -1,0 +1,467 @@
+#!/usr/bin/env python
+"""bench.py -- H|psi> throughput of libtdh.so on B200 (one JSON line on stdout, rank 0).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload large] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
+        bench.py --gpus N --steps K --warmup W
+
+A "step" is one tdh_apply_hamiltonian call (rows a1-a6 of DESIGN.md section 1) over the whole state block of the
+workload; metric = states*gridpoints/s in complex128.  Default workload: "large" (BASELINE.json configs[3]:
+96^3 grid, 1024 states, 13.5 GiB block -- far larger than the 126 MB L2, so no flush is needed between steps).
+Row a7 (Taylor-4 propagate, 4 H applications + fused axpys per step) is timed beside it on the "tddft" config and
+reported under "propagate"; the other configs are reported under "workloads" (context, not the headline).
+
+Keys beyond the driver's contract: "roofline" (dominant kernel family, CUDA events on the launching stream),
+"cpu_baseline" (the CPU oracle as it stands on a bounded sample; N=1 only), "kernels" (per-family seconds per step),
+"propagate", "workloads".
+
+--impl reference times the CPU oracle (oracle/ref_tdh.c, OpenMP over states) on the host cores, each step a bounded
+sample of the same workload.  The oracle is imported only by that leg and by the cpu_baseline leg.
+With N > 1 every rank owns its own block of `nst` states (distinct seeds; weak scaling, no data-path collective:
+PAPER.md:438 -- states are independent); torch.distributed only carries the barrier and the max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import concurrent.futures as cf
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+from paper_2106_03872_b200 import workloads as W
+
+METRIC = "H|psi> states*gridpoints/s (complex128)"
+UNIT = "states*gridpoints/s"
+
+# Algorithmic bytes per state*gridpoint of each kernel family: what the launch must read and
+# write if nothing were cached.  plane_inv: spectrum in (16) + phi for V*phi (16) + out (16); +16 with an axpy addend.
+ALG_BYTES = {"nl_project": None, "plane_fwd": 32.0, "xpencil": 32.0, "plane_inv": 48.0}
+
+
+def parse_args():
+    p = argparse.ArgumentParser()
+    p.add_argument("--gpus", type=int, default=1)
+    p.add_argument("--steps", type=int, default=10)
+    p.add_argument("--warmup", type=int, default=3)
+    p.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    p.add_argument("--workload", default="large", choices=list(W.CONFIG_ORDER))
+    p.add_argument("--states", type=int, default=0, help="override the number of states per GPU (0 = the config's)")
+    p.add_argument("--chunk", type=int, default=0, help="tdh_set_chunk_states (0 = library default)")
+    p.add_argument("--no-sweep", action="store_true", help="skip the other configs / propagate legs")
+    p.add_argument("--no-e2e", action="store_true")
+    p.add_argument("--no-cpu-baseline", action="store_true")
+    p.add_argument("--cpu-sample-states", type=int, default=0, help="states in the cpu_baseline sample (0 = auto)")
+    return p.parse_args()
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# helpers
+# ----------------------------------------------------------------------------------------------------------------
+def host_states(cfg, s0, s1, pinned=True):
+    """States [s0, s1) of the config as a (pinned) host torch tensor; generated per state (seeded) on a thread pool."""
+    import torch
+    t = torch.empty((s1 - s0,) + tuple(cfg.n), dtype=torch.complex128, pin_memory=pinned)
+    a = t.numpy()
+
+    def fill(s):
+        a[s - s0] = W.state(cfg, s)
+
+    with cf.ThreadPoolExecutor(max_workers=min(16, os.cpu_count() or 1)) as ex:
+        list(ex.map(fill, range(s0, s1)))
+    return t
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while a timed region runs."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); smax.append(float(f[2])); power.append(float(f[3]))
+            except ValueError:
+                continue
+            for name, val in zip(names, f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class Dist:
+    """torch.distributed plumbing: barrier and max-over-ranks only (no data-path collective)."""
+
+    def __init__(self, want_gpus):
+        import torch
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.local = int(os.environ.get("LOCAL_RANK", "0"))
+        self.torch = torch
+        if self.world > 1:
+            import torch.distributed as dist
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            os.environ.setdefault("MASTER_PORT", "29500")
+            torch.cuda.set_device(self.local)
+            dist.init_process_group("nccl", device_id=torch.device("cuda", self.local))
+            self.dist = dist
+        else:
+            self.dist = None
+            if torch.cuda.is_available():
+                torch.cuda.set_device(0)
+        if want_gpus != self.world and self.rank == 0:
+            sys.stderr.write(f"bench.py: --gpus {want_gpus} but WORLD_SIZE={self.world}; using WORLD_SIZE\n")
+
+    def barrier(self):
+        if self.dist is not None:
+            self.dist.barrier()
+
+    def max(self, x):
+        if self.dist is None:
+            return float(x)
+        t = self.torch.tensor([x], dtype=self.torch.float64, device="cuda")
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def close(self):
+        if self.dist is not None:
+            self.dist.destroy_process_group()
+
+
+def timed_device(D, fn, steps, warmup):
+    """`warmup` untimed calls, then exactly `steps` calls between CUDA events on torch's current stream (the handle's
+    stream), barrier + synchronize on both sides; returns max-over-ranks seconds for the `steps` calls."""
+    torch = D.torch
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    D.barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(steps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    D.barrier()
+    return D.max(e0.elapsed_time(e1) * 1e-3)
+
+
+def timed_each(torch, fn, reps, flush=None):
+    """Per-call device times (s); `flush` (a big tensor) is overwritten before each call to evict L2."""
+    out = []
+    for _ in range(reps):
+        if flush is not None:
+            flush.add_(1.0)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        fn()
+        e1.record()
+        torch.cuda.synchronize()
+        out.append(e0.elapsed_time(e1) * 1e-3)
+    return out
+
+
+def upload_states(torch, cfg, s0, nst, keep_host):
+    """Device block of states [s0, s0+nst); returns (device tensor, pinned host tensor of the first keep_host states)."""
+    dev = torch.empty((nst,) + tuple(cfg.n), dtype=torch.complex128, device="cuda")
+    step = max(1, min(nst, (1 << 30) // (cfg.npts * 16)))
+    host_keep = None
+    if keep_host > 0:
+        host_keep = host_states(cfg, s0, s0 + keep_host)
+        dev[:keep_host].copy_(host_keep, non_blocking=True)
+    for a in range(keep_host, nst, step):
+        b = min(nst, a + step)
+        h = host_states(cfg, s0 + a, s0 + b)
+        dev[a:b].copy_(h, non_blocking=True)
+        torch.cuda.synchronize()
+    torch.cuda.synchronize()
+    return dev, host_keep
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# legs
+# ----------------------------------------------------------------------------------------------------------------
+def kernel_breakdown(torch, g, fn, steps):
+    """Per-family device seconds per step from the library's own CUDA events on its stream (profiling pass)."""
+    g.set_profiling(True)
+    tot, launches = {}, 0
+    for _ in range(steps):
+        fn()
+        torch.cuda.synchronize()
+        launches = g.last_launch_count()
+        for k, v in g.last_kernel_seconds().items():
+            tot[k] = tot.get(k, 0.0) + v
+    g.set_profiling(False)
+    return {k: v / steps for k, v in tot.items()}, launches
+
+
+def roofline_of(kern_s, units, peak_gbs, peak_src):
+    """Roofline object for the dominant kernel family (largest share of the step)."""
+    cand = {k: v for k, v in kern_s.items() if ALG_BYTES.get(k) and v > 0}
+    if not cand:
+        return None
+    top = max(cand, key=cand.get)
+    achieved = ALG_BYTES[top] * units / cand[top] * 1e-9
+    return {"kernel": top, "bound": "hbm", "achieved": round(achieved, 1), "peak": peak_gbs, "unit": "GB/s",
+            "frac": round(achieved / peak_gbs, 4), "traffic": None, "peak_source": peak_src,
+            "algorithmic_bytes_per_unit": ALG_BYTES[top], "units_per_step": units,
+            "share_of_step": round(cand[top] / sum(kern_s.values()), 4),
+            "note": "achieved = algorithmic bytes of all launches of this family in one step / their summed CUDA-event "
+                    "time (separate profiling pass of the same steps); traffic (ncu dram bytes) is in profiles/"}
+
+
+def cpu_baseline(cfg, wl, sample_states):
+    """The CPU oracle as it stands on a bounded sample of the same workload (states [0, S))."""
+    from oracle import ref
+    cores = ref.num_threads()
+    cal = W.states(cfg, 0, min(cfg.nst, cores))
+    t0 = time.perf_counter()
+    ref.apply_workload(wl, cal, ref.NAIVE_FFT)
+    rate = cal.shape[0] * cfg.npts / (time.perf_counter() - t0)
+    S = sample_states or int(min(cfg.nst, max(cores, cores * round(rate * 12.0 / cfg.npts / cores))))
+    S = max(1, min(S, cfg.nst))
+    psi = W.states(cfg, 0, S)
+    t0 = time.perf_counter()
+    ref.apply_workload(wl, psi, ref.NAIVE_FFT)
+    dt = time.perf_counter() - t0
+    return {"value": S * cfg.npts / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"states [0,{S}) of '{cfg.name}' ({S} x {cfg.n[0]}^3 points), one ref_apply_hamiltonian call "
+                      f"(naive radix-2/3 FFT back-end, OpenMP over states), {dt:.2f} s"}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the host cores; each step a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import ref
+    cfg = W.CONFIGS[args.workload]
+    wl = W.make(cfg)
+    cores = ref.num_threads()
+    S = args.cpu_sample_states or min(cfg.nst, 4 * cores)
+    psi = W.states(cfg, 0, S)
+    for _ in range(args.warmup):
+        ref.apply_workload(wl, psi, ref.NAIVE_FFT)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        ref.apply_workload(wl, psi, ref.NAIVE_FFT)
+    dt = time.perf_counter() - t0
+    val = args.steps * S * cfg.npts / dt
+    sample = f"each step = states [0,{S}) of '{cfg.name}' through ref_apply_hamiltonian (naive FFT back-end)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "grid": list(cfg.n), "states_per_step": S, "atoms": cfg.natoms},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def sweep_leg(torch, B, name, flush, reps=7):
+    """One of the non-headline configs at its full size: apply_hamiltonian cold (L2 flushed) and L2-hot."""
+    cfg = W.CONFIGS[name]
+    wl = W.make(cfg)
+    psi, _ = upload_states(torch, cfg, 0, cfg.nst, 0)
+    out = torch.empty_like(psi)
+    units = cfg.nst * cfg.npts
+    with B.grid_for(wl) as g:
+        fn = lambda: g.apply_hamiltonian(psi, out=out)
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        cold = statistics.median(timed_each(torch, fn, reps, flush))
+        hot = statistics.median(timed_each(torch, fn, reps, None))
+        res = {"states": cfg.nst, "grid": cfg.n[0], "value": units / cold, "ms": cold * 1e3,
+               "value_l2_hot": units / hot, "ms_l2_hot": hot * 1e3, "launches": g.last_launch_count()}
+        if name == "tddft":
+            # row a7: the config's 20 Taylor-4 steps (80 H applications + fused axpys) in one tdh_propagate call
+            work = psi.clone()
+            g.propagate(work, cfg.dt, 1)
+            torch.cuda.synchronize()
+            work.copy_(psi)
+            ts = timed_each(torch, lambda: g.propagate(work, cfg.dt, cfg.nsteps), 1, flush)
+            t = ts[0]
+            res["propagate"] = {"steps": cfg.nsteps, "dt": cfg.dt, "seconds": t, "steps_per_s": cfg.nsteps / t,
+                                "h_application_equivalents_per_s": units * 4 * cfg.nsteps / t, "unit": UNIT,
+                                "launches": g.last_launch_count()}
+    del psi, out
+    torch.cuda.empty_cache()
+    return res
+
+
+def block_sweep(torch, g, psi, out, cfg, blocks=(32, 128, 512, 1024)):
+    """Config 4's sweep: the whole block submitted as consecutive sub-blocks of b states (PAPER.md:456 batching claim)."""
+    res = {}
+    nst = psi.shape[0]
+    for b in blocks:
+        if b > nst:
+            continue
+
+        def fn():
+            for s0 in range(0, nst, b):
+                g.apply_hamiltonian(psi[s0:s0 + b], out=out[s0:s0 + b])
+
+        fn()
+        torch.cuda.synchronize()
+        t = statistics.median(timed_each(torch, fn, 3, None))
+        res[str(b)] = nst * cfg.npts / t
+    return res
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+    import torch
+    from paper_2106_03872_b200 import binding as B
+    B.lib()                                            # fails loudly if libtdh.so is missing (no fallback)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback (use --impl reference for the oracle)")
+    D = Dist(args.gpus)
+    cfg = W.CONFIGS[args.workload]
+    nst = args.states or cfg.nst
+    wl = W.make(cfg)
+    units = nst * cfg.npts                              # per GPU and step
+    s_first = D.rank * nst                              # weak scaling: every rank its own states (distinct seeds)
+    # e2e host buffers: the whole block when it fits the host comfortably, else a bounded part (stated in the output)
+    e2e_states = 0 if args.no_e2e else (nst if D.world <= 2 else min(nst, 256))
+    psi, host_in = upload_states(torch, cfg, s_first, nst, e2e_states)
+    hpsi = torch.empty_like(psi)
+    g = B.grid_for(wl, max_states=nst)
+    if args.chunk:
+        g.set_chunk_states(args.chunk)
+    fn = lambda: g.apply_hamiltonian(psi, out=hpsi)
+
+    # ---- headline: device-resident, K steps
+    sampler = ClockSampler(D.local)
+    fn(); torch.cuda.synchronize()
+    sampler.start()
+    t = timed_device(D, fn, args.steps, args.warmup)
+    clocks = sampler.stop()
+    launches = g.last_launch_count() * args.steps
+    value = D.world * units * args.steps / t
+
+    # ---- per-kernel times (same steps, library events on the launching stream) -> roofline of the dominant family
+    kern_s, _ = kernel_breakdown(torch, g, fn, max(1, min(args.steps, 5)))
+    peak, peak_src = measured_peaks()
+    roof = roofline_of(kern_s, units, peak, peak_src)
+
+    # ---- end to end through the host-buffer entry point (pinned host in/out, copies inside the timed region)
+    e2e = None
+    if e2e_states > 0:
+        host_out = torch.empty_like(host_in).pin_memory()
+        efn = lambda: g.apply_hamiltonian_host(host_in, host_out)
+        for _ in range(min(args.warmup, 2)):
+            efn()
+        torch.cuda.synchronize(); D.barrier()
+        esteps = max(1, min(args.steps, 5))
+        t0 = time.perf_counter()
+        for _ in range(esteps):
+            efn()                                        # returns when host_out is complete
+        torch.cuda.synchronize()
+        te = D.max(time.perf_counter() - t0)
+        D.barrier()
+        nbytes = e2e_states * cfg.npts * 16
+        e2e = {"value": D.world * e2e_states * cfg.npts * esteps / te, "unit": UNIT, "h2d_bytes_per_step": nbytes,
+               "d2h_bytes_per_step": nbytes, "steps": esteps, "states_per_gpu": e2e_states,
+               "ms_per_step": te / esteps * 1e3,
+               "timer": "host perf_counter around the blocking tdh_apply_hamiltonian_host calls, max over ranks"}
+        del host_out
+    host_in = None
+
+    extra = {}
+    if D.rank == 0 and D.world == 1 and not args.no_sweep:
+        flush = torch.zeros(64 * 1024 * 1024, dtype=torch.float32, device="cuda")       # 256 MB > 126 MB L2
+        if args.workload == "large":
+            extra["block_sweep_states_per_call"] = block_sweep(torch, g, psi, hpsi, cfg)
+        g.close()
+        del psi, hpsi
+        torch.cuda.empty_cache()
+        wls = {}
+        for name in W.CONFIG_ORDER:
+            if name != args.workload:
+                wls[name] = sweep_leg(torch, B, name, flush)
+        extra["workloads"] = wls
+        if "tddft" in wls and "propagate" in wls["tddft"]:
+            extra["propagate"] = wls["tddft"].pop("propagate")
+    else:
+        g.close()
+
+    cpu = None
+    if D.rank == 0 and D.world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_baseline(cfg, wl, args.cpu_sample_states)
+
+    if D.rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": D.world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": t / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{cfg.name}: {cfg.n[0]}^3 grid, {nst} states/GPU complex128, {cfg.natoms} atoms, "
+                                   f"{cfg.nchan_per_atom} KB channels/atom, rc={cfg.rc}",
+                       "call": "tdh_apply_hamiltonian on the whole block", "states_per_gpu": nst,
+                       "l2": "inputs larger than L2 (block of %.1f GB per GPU), no flush" % (units * 16 / 1e9)
+                             if units * 16 > 512e6 else "L2-resident block, no flush (use the 'large' workload)",
+                       "parallelism": f"states sharded over {D.world} GPU(s), no collective"},
+            "e2e": e2e, "gpu_launches": launches, "clocks": clocks, "roofline": roof, "cpu_baseline": cpu,
+            "kernels_s_per_step": kern_s,
+            "strict_roofline": {"bytes_per_unit": 32.0, "achieved_gbs": 32.0 * units * args.steps / t * 1e-9,
+                                "frac_of_peak": 32.0 * units * args.steps / t * 1e-9 / peak,
+                                "note": "compulsory traffic of H|psi> (read psi + write Hpsi) x throughput / HBM peak"},
+        }
+        line.update(extra)
+        print(json.dumps(line))
+    D.close()
+
+
+if __name__ == "__main__":
+    main()

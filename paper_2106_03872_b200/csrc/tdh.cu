@@ -134,12 +134,9 @@ static void free_projectors(tdh_grid* g) {
 }
 
 static int default_chunk(const tdh_grid* g) {
-    // Keep work (+ in + out) L2-resident: aim at ~24 MB of workspace, but never fewer states than fill the GPU once.
-    const double state_bytes = (double)g->np * sizeof(cd);
-    int c = (int)std::floor(24.0 * 1048576.0 / state_bytes);
-    const int ctas_per_state = g->n[0] / g->pl.ppc;
-    const int fill = (2 * 148 + ctas_per_state - 1) / ctas_per_state;
-    c = std::max(c, fill);
+    // Measured on B200 (profiles/r01_chunk_sweep.md): every kernel gets faster with more states per launch and the
+    // L2-resident small-chunk variant never wins, so the default is the largest chunk the workspace holds.
+    int c = g->chunk_cap;
     if (const char* e = getenv("TDH_CHUNK_STATES")) { int v = atoi(e); if (v > 0) c = v; }
     return std::max(1, std::min(c, g->chunk_cap));
 }
