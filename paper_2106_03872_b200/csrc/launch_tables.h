@@ -4,27 +4,30 @@
 
 namespace tdh {
 
-struct PlaneLaunch {
-    const void* fwd;   // plane_fwd_kernel<NY,NZ>
-    const void* inv;   // plane_inv_kernel<NY,NZ>
+struct TileLaunch {
+    const void* fwd;   // tile_fwd_kernel<NY,NZ>
+    const void* inv;   // tile_inv_kernel<NY,NZ>
     int threads;
-    int ppc;           // planes per CTA
+    int ppc;           // plane parts per CTA
+    int s;             // y-split: a plane is s parts (rows y = s*m + r)
+    int r1y, r2y;      // factorisation of the y transform of length NY/s (row order inside a tile)
+    int r1z;           // NZ / 8 (cell rotation inside a tile)
     size_t smem;       // dynamic shared memory per CTA
 };
 
 struct XLaunch {
-    const void* fused;  // xpencil_kernel<NX,0>
-    const void* fwd;    // xpencil_kernel<NX,1>
-    const void* inv;    // xpencil_kernel<NX,2>
+    const void* fused;  // xpencil_kernel<NX,S,0>
+    const void* fwd;    // xpencil_kernel<NX,S,1>
+    const void* inv;    // xpencil_kernel<NX,S,2>
     int threads;
 };
 
-// defined in plane_nz<NZ>.cu / xpencil_inst.cu; return false for an unsupported size
-bool plane_launch_nz16(int ny, PlaneLaunch* out);
-bool plane_launch_nz32(int ny, PlaneLaunch* out);
-bool plane_launch_nz48(int ny, PlaneLaunch* out);
-bool plane_launch_nz64(int ny, PlaneLaunch* out);
-bool plane_launch_nz96(int ny, PlaneLaunch* out);
-bool xpencil_launch(int nx, XLaunch* out);
+// defined in tile_nz<NZ>.cu / xpencil_inst.cu; return false for an unsupported size
+bool tile_launch_nz16(int ny, TileLaunch* out);
+bool tile_launch_nz32(int ny, TileLaunch* out);
+bool tile_launch_nz48(int ny, TileLaunch* out);
+bool tile_launch_nz64(int ny, TileLaunch* out);
+bool tile_launch_nz96(int ny, TileLaunch* out);
+bool xpencil_launch(int nx, int s, XLaunch* out);
 
 }  // namespace tdh

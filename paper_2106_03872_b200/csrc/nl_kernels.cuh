@@ -2,12 +2,13 @@
 //
 // For atom I and state s:   dpi[s][c] = D_{I,c} dV sum_q beta_{I,c}[q] e^{+ik.d_q} psi_s[S_I[q]]
 // This is a real (C_I x P_I) matrix times a complex (P_I x n_st) block, gathered from the sphere's grid points.
-// One warp owns 8 states; per step of 4 sphere points it issues, for each tile of 8 channels,
+// A CTA owns one atom and 8 states; its NLP_WARPS warps split the sphere's points in blocks of 32.  Per block a lane
+// issues 8 independent 16-byte gathers (8 k-steps of 4 points), then for each tile of 8 channels
 //     mma.sync.m8n8k4.f64   D(8 chan x 8 states) += A(8 chan x 4 points) * B(4 points x 8 states)
-// twice (real and imaginary parts of psi).  Fragment layout of m8n8k4 (PTX ISA): lane l holds A[l/4][l%4],
-// B[l%4][l/4] and C[l/4][2*(l%4) + {0,1}].  So lane l gathers ONE complex value psi_{s0 + l/4}[S[q0 + l%4]] with a
-// 16-byte load and that is both B fragments.  The sum over q is sequential inside the warp: deterministic, no atomics.
-// The second half of Eq. 9 (back-projection and scatter) is fused into plane_inv's epilogue, point-centric.
+// twice per k-step (real and imaginary parts of psi).  Fragment layout of m8n8k4 (PTX ISA): lane l holds A[l/4][l%4],
+// B[l%4][l/4] and C[l/4][2*(l%4) + {0,1}].  So lane l gathers ONE complex value psi_{s0 + l/4}[S[q0 + l%4]] per k-step
+// and that is both B fragments.  The partial sums of the warps are combined through shared memory in warp order:
+// deterministic, no atomics.  The second half of Eq. 9 (back-projection) is fused into tile_inv's epilogue.
 #pragma once
 #include "fft_codelets.cuh"
 
@@ -27,64 +28,77 @@ __device__ __forceinline__ void dmma_m8n8k4(double (&c)[2], double a, double b) 
                  : "d"(a), "d"(b));
 }
 
-constexpr int NLP_WARPS = 8;            // warps per CTA
-constexpr int NLP_STATES = 8 * NLP_WARPS;  // states per CTA
+constexpr int NLP_WARPS = 8;     // warps per CTA, splitting the sphere
+constexpr int NLP_STATES = 8;    // states per CTA (the N of the MMA)
+constexpr int NLP_KSTEPS = 8;    // k-steps (of 4 points) per block: 32 points, 8 gathers in flight per lane
 
-// grid: (natoms, ceil(nst / NLP_STATES)); MT = number of 8-channel tiles (C_I <= 8*MT)
+// grid: (natoms, ceil(nst / 8)); MT = number of 8-channel tiles (C_I <= 8*MT)
 template <int MT>
 __global__ void __launch_bounds__(32 * NLP_WARPS)
 nl_project_kernel(const cd* __restrict__ psi, size_t npts, int nst, const AtomDesc* __restrict__ atoms,
                   const int* __restrict__ sidx, const double* __restrict__ sbeta, const cd* __restrict__ sphase,
                   const double* __restrict__ dscale, cd* __restrict__ dpi, int nchan_tot)
 {
+    __shared__ double part[NLP_WARPS][MT][4][32];
     const AtomDesc at = atoms[blockIdx.x];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int kq = lane & 3, r8 = lane >> 2;
-    const int s = blockIdx.y * NLP_STATES + warp * 8 + r8;      // this lane's state (B fragment column)
-    if (blockIdx.y * NLP_STATES + warp * 8 >= nst) return;      // whole warp idle (warp-uniform)
+    const int s0 = blockIdx.y * NLP_STATES;
+    const int s = s0 + r8;                                      // this lane's state (B fragment column)
     const bool s_ok = s < nst;
     const cd* ps = psi + (size_t)(s_ok ? s : 0) * npts;
     const int* idx = sidx + at.q0;
     const cd* phs = sphase ? sphase + at.q0 : nullptr;
 
-    // two accumulator sets (even / odd k-steps) to keep two independent MMA chains in flight
-    double cre[2][MT][2], cim[2][MT][2];
+    double cre[MT][2], cim[MT][2];
 #pragma unroll
-    for (int u = 0; u < 2; ++u)
-#pragma unroll
-        for (int m = 0; m < MT; ++m) cre[u][m][0] = cre[u][m][1] = cim[u][m][0] = cim[u][m][1] = 0.0;
+    for (int m = 0; m < MT; ++m) cre[m][0] = cre[m][1] = cim[m][0] = cim[m][1] = 0.0;
 
-    for (int q0 = 0; q0 < at.np; q0 += 8) {
+    for (int q0 = warp * 4 * NLP_KSTEPS; q0 < at.np; q0 += NLP_WARPS * 4 * NLP_KSTEPS) {
+        cd b[NLP_KSTEPS];
 #pragma unroll
-        for (int u = 0; u < 2; ++u) {
+        for (int u = 0; u < NLP_KSTEPS; ++u) {
+            const int q = q0 + 4 * u + kq;
+            b[u] = make_double2(0.0, 0.0);
+            if (q < at.np && s_ok) b[u] = __ldcs(ps + __ldg(idx + q));
+        }
+#pragma unroll
+        for (int u = 0; u < NLP_KSTEPS; ++u) {
             const int q = q0 + 4 * u + kq;
             const bool q_ok = q < at.np;
-            cd b = make_double2(0.0, 0.0);
-            if (q_ok && s_ok) {
-                b = __ldg(ps + __ldg(idx + q));
-                if (phs) b = cmul(b, __ldg(phs + q));
-            }
+            cd bv = b[u];
+            if (phs != nullptr && q_ok) bv = cmul(bv, __ldg(phs + q));
 #pragma unroll
             for (int m = 0; m < MT; ++m) {
                 const int c = 8 * m + r8;                                   // A fragment row = channel
                 const double a = (q_ok && c < at.nchan) ? __ldg(sbeta + at.boff + (size_t)c * at.np + q) : 0.0;
-                dmma_m8n8k4(cre[u][m], a, b.x);
-                dmma_m8n8k4(cim[u][m], a, b.y);
+                dmma_m8n8k4(cre[m], a, bv.x);
+                dmma_m8n8k4(cim[m], a, bv.y);
             }
         }
     }
-    // C fragment: row = channel 8m + lane/4, columns = states 2*(lane%4) + {0,1} of this warp
 #pragma unroll
     for (int m = 0; m < MT; ++m) {
+        part[warp][m][0][lane] = cre[m][0];
+        part[warp][m][1][lane] = cre[m][1];
+        part[warp][m][2][lane] = cim[m][0];
+        part[warp][m][3][lane] = cim[m][1];
+    }
+    __syncthreads();
+    // C fragment: row = channel 8m + lane/4, columns = states 2*(lane%4) + {0,1}.  Warp m < MT sums tile m.
+    if (warp < MT) {
+        const int m = warp;
+        double acc[4] = {0.0, 0.0, 0.0, 0.0};
+        for (int w = 0; w < NLP_WARPS; ++w)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) acc[j] += part[w][m][j][lane];
         const int c = 8 * m + r8;
         if (c < at.nchan) {
             const double d = __ldg(dscale + at.chan0 + c);
 #pragma unroll
             for (int j = 0; j < 2; ++j) {
-                const int so = blockIdx.y * NLP_STATES + warp * 8 + 2 * kq + j;
-                if (so < nst)
-                    dpi[(size_t)so * nchan_tot + at.chan0 + c] =
-                        make_double2(d * (cre[0][m][j] + cre[1][m][j]), d * (cim[0][m][j] + cim[1][m][j]));
+                const int so = s0 + 2 * kq + j;
+                if (so < nst) dpi[(size_t)so * nchan_tot + at.chan0 + c] = make_double2(d * acc[j], d * acc[2 + j]);
             }
         }
     }

@@ -2,11 +2,11 @@
 //
 // One Hamiltonian application on a chunk of states is four launches:
 //     nl_project  (gather + FP64-MMA projection, only with projectors)
-//     plane_fwd   (z,y forward FFT per (state,x) plane)            in  -> work
-//     xpencil     (x forward, 1/2|G+k|^2 scale + mask, x inverse)   work in place
-//     plane_inv   (y,z inverse FFT + epilogue alpha*(T+V+Vnl)phi + y)  work -> out
-// States are independent, so a block is pushed through this chain chunk by chunk; the chunk is sized
-// so that `work` (and, for propagate, the two Horner buffers) stay resident in the 126 MB L2 between kernels.
+//     plane_fwd   (tile_fwd: z,y forward FFT per tile of a (state,x) plane)   in  -> work
+//     xpencil     (x forward, 1/2|G+k|^2 scale + mask, x inverse)             work in place
+//     plane_inv   (tile_inv: y,z inverse FFT + epilogue alpha*(T+V+Vnl)phi + y)  work -> out
+// States are independent, so a block is pushed through this chain chunk by chunk; a chunk is as many
+// states as the 1 GiB workspace holds (measured: L2-resident small chunks never win, profiles/r01a_chunk_sweep.md).
 // propagate runs ALL steps of one chunk before moving to the next chunk (H is fixed: readings R10, R16), evaluating
 // Eq. 8 in Horner form  psi + a1 H(psi + a2 H(psi + a3 H(psi + a4 H psi))),  a_k = -i dt / k,  so that every
 // application's epilogue is a single fused axpy and no accumulator is read-modified-written.
@@ -22,9 +22,10 @@
 #include <vector>
 
 #include "../../include/tdh.h"
-#include "fft_kernels.cuh"
 #include "launch_tables.h"
 #include "nl_kernels.cuh"
+#include "tile_kernels.cuh"
+#include "xpencil_kernel.cuh"
 
 using tdh::cd;
 
@@ -78,7 +79,7 @@ struct tdh_grid {
     cd* d_work;
     cd* d_phi[2];
 
-    tdh::PlaneLaunch pl;
+    tdh::TileLaunch tl;
     tdh::XLaunch xl;
 
     // projectors
@@ -89,9 +90,12 @@ struct tdh_grid {
     cd* d_sphase;
     double* d_dscale;
     cd* d_dpi;
-    int* d_nl_start;
-    int4* d_nl_ent;
+    // back-projection records, grouped by tile (x, r) and layer (tile_kernels.cuh, struct Epilogue)
+    int* d_nl_off;
+    unsigned* d_nl_cc;
+    double* d_nl_beta;
     cd* d_nl_phase;
+    int nl_layers, nl_nrec, nl_cmax;
 
     // host-buffer path
     int host_chunk;
@@ -127,14 +131,15 @@ static int freq_index(int a, int n) {
 
 static void free_projectors(tdh_grid* g) {
     cudaFree(g->d_atoms); cudaFree(g->d_sidx); cudaFree(g->d_sbeta); cudaFree(g->d_sphase); cudaFree(g->d_dscale);
-    cudaFree(g->d_dpi); cudaFree(g->d_nl_start); cudaFree(g->d_nl_ent); cudaFree(g->d_nl_phase);
+    cudaFree(g->d_dpi); cudaFree(g->d_nl_off); cudaFree(g->d_nl_cc); cudaFree(g->d_nl_beta); cudaFree(g->d_nl_phase);
     g->d_atoms = nullptr; g->d_sidx = nullptr; g->d_sbeta = nullptr; g->d_sphase = nullptr; g->d_dscale = nullptr;
-    g->d_dpi = nullptr; g->d_nl_start = nullptr; g->d_nl_ent = nullptr; g->d_nl_phase = nullptr;
+    g->d_dpi = nullptr; g->d_nl_off = nullptr; g->d_nl_cc = nullptr; g->d_nl_beta = nullptr; g->d_nl_phase = nullptr;
     g->natoms = 0; g->nchan_tot = 0; g->mt = 1;
+    g->nl_layers = 0; g->nl_nrec = 0; g->nl_cmax = 0;
 }
 
 static int default_chunk(const tdh_grid* g) {
-    // Measured on B200 (profiles/r01_chunk_sweep.md): every kernel gets faster with more states per launch and the
+    // Measured on B200 (profiles/r01a_chunk_sweep.md): every kernel gets faster with more states per launch and the
     // L2-resident small-chunk variant never wins, so the default is the largest chunk the workspace holds.
     int c = g->chunk_cap;
     if (const char* e = getenv("TDH_CHUNK_STATES")) { int v = atoi(e); if (v > 0) c = v; }
@@ -168,19 +173,23 @@ extern "C" int tdh_create_grid(const int n[3], const double len[3], const double
 
     bool ok = false;
     switch (n[2]) {
-        case 16: ok = tdh::plane_launch_nz16(n[1], &g->pl); break;
-        case 32: ok = tdh::plane_launch_nz32(n[1], &g->pl); break;
-        case 48: ok = tdh::plane_launch_nz48(n[1], &g->pl); break;
-        case 64: ok = tdh::plane_launch_nz64(n[1], &g->pl); break;
-        case 96: ok = tdh::plane_launch_nz96(n[1], &g->pl); break;
+        case 16: ok = tdh::tile_launch_nz16(n[1], &g->tl); break;
+        case 32: ok = tdh::tile_launch_nz32(n[1], &g->tl); break;
+        case 48: ok = tdh::tile_launch_nz48(n[1], &g->tl); break;
+        case 64: ok = tdh::tile_launch_nz64(n[1], &g->tl); break;
+        case 96: ok = tdh::tile_launch_nz96(n[1], &g->tl); break;
     }
-    ok = ok && tdh::xpencil_launch(n[0], &g->xl);
+    ok = ok && tdh::xpencil_launch(n[0], g->tl.s, &g->xl);
     if (!ok) { delete g; return fail(TDH_EUNSUPPORTED, "tdh_create_grid: no kernel for this grid"); }
 
     int rc = TDH_OK;
     auto body = [&]() -> int {
-        CU(cudaFuncSetAttribute(g->pl.fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g->pl.smem));
-        CU(cudaFuncSetAttribute(g->pl.inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g->pl.smem));
+        CU(cudaFuncSetAttribute(g->tl.fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g->tl.smem));
+        CU(cudaFuncSetAttribute(g->tl.inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g->tl.smem));
+        // ask for the largest shared-memory carve-out so that the resident-CTA counts of the launch bounds are reached
+        const void* fs[5] = {g->tl.fwd, g->tl.inv, g->xl.fused, g->xl.fwd, g->xl.inv};
+        for (const void* f : fs)
+            CU(cudaFuncSetAttribute(f, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
         // tables: built on the host exactly as the oracle builds its G vectors (two_pi * m / L + k, then squared)
         const double two_pi = 6.283185307179586476925286766559;
         for (int a = 0; a < 3; ++a) {
@@ -316,25 +325,59 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
         atoms[a].q0 = (int)q0; atoms[a].np = pn; atoms[a].boff = (int)boff; atoms[a].chan0 = c0; atoms[a].nchan = nc;
         boff += (size_t)nc * pn;
     }
-    // ---- point-centric inverse map for the atomic-free scatter
-    std::vector<int> nl_start(g->np, -1);
+    // ---- back-projection records: one per (atom, sphere point), grouped by tile (x, r) and by layer.  The layer of a
+    //      record is the number of earlier atoms covering the same grid point, so no two records of one (tile, layer)
+    //      share a shared-memory cell and the scatter needs no atomics.  The cell address follows tile_kernels.cuh.
+    if (ctot >= 65536) return fail(TDH_EUNSUPPORTED, "tdh_set_projectors: more than 65535 channels");
+    const int ny = g->n[1], nz = g->n[2];
+    const int S = g->tl.s, r1y = g->tl.r1y, r2y = g->tl.r2y, r1z = g->tl.r1z;
+    int nlayers = 0;
+    for (size_t p = 0; p < g->np; ++p) nlayers = std::max(nlayers, cover[p]);
+    const int ntiles = g->n[0] * S;
+    std::vector<int> nl_off((size_t)ntiles * (nlayers + 1) + 1, 0);
+    std::vector<int> rec_slot(ptot);                       // (tile*(nlayers) + layer) of each (atom, point)
+    std::vector<unsigned> rec_cell(ptot);
     {
+        std::vector<int> fill(g->np, 0);
+        std::vector<int> count((size_t)ntiles * nlayers, 0);
+        for (int a = 0; a < natoms; ++a) {
+            const tdh::AtomDesc& at = atoms[a];
+            for (int j = 0; j < at.np; ++j) {
+                const int p = sidx[at.q0 + j];
+                const int x = p / (ny * nz), y = (p / nz) % ny, z = p % nz;
+                const int r = y % S, m = y / S;
+                const int rho = (m % r1y) * r2y + m / r1y;
+                const int grp = rho * r1z + z % r1z;
+                const int cell = 8 * grp + ((z / r1z + grp) & 7);
+                const int layer = fill[p]++;
+                const int slot = (x * S + r) * nlayers + layer;
+                rec_slot[at.q0 + j] = slot;
+                rec_cell[at.q0 + j] = (unsigned)cell | ((unsigned)at.chan0 << 16);
+                count[slot] += 1;
+            }
+        }
+        // offsets: tile t, layer l at nl_off[t*(nlayers+1) + l]; the end of the tile's last layer in [.. + nlayers]
         int run = 0;
-        for (size_t p = 0; p < g->np; ++p)
-            if (cover[p] > 0) { nl_start[p] = run; run += cover[p]; }
+        for (int t = 0; t < ntiles; ++t) {
+            for (int l = 0; l < nlayers; ++l) { nl_off[(size_t)t * (nlayers + 1) + l] = run; run += count[(size_t)t * nlayers + l]; }
+            nl_off[(size_t)t * (nlayers + 1) + nlayers] = run;
+        }
     }
-    std::vector<int4> ent(ptot);
-    std::vector<cd> ent_phase(g->have_k ? ptot : 0);
-    std::vector<int> fill(g->np, 0);
-    for (int a = 0; a < natoms; ++a) {
-        const tdh::AtomDesc& at = atoms[a];
-        for (int j = 0; j < at.np; ++j) {
-            const int p = sidx[at.q0 + j];
-            const int e = nl_start[p] + fill[p];
-            fill[p] += 1;
-            const int last = fill[p] == cover[p] ? 1 : 0;
-            ent[e] = make_int4(at.boff + j, at.np, at.chan0, at.nchan | (last << 16));
-            if (g->have_k) ent_phase[e] = sphase[at.q0 + j];
+    std::vector<unsigned> rec_cc(ptot);
+    std::vector<double> rec_beta((size_t)cmax * ptot, 0.0);
+    std::vector<cd> rec_phase(g->have_k ? ptot : 0);
+    {
+        std::vector<int> cursor((size_t)ntiles * nlayers);
+        for (int t = 0; t < ntiles; ++t)
+            for (int l = 0; l < nlayers; ++l) cursor[(size_t)t * nlayers + l] = nl_off[(size_t)t * (nlayers + 1) + l];
+        for (int a = 0; a < natoms; ++a) {
+            const tdh::AtomDesc& at = atoms[a];
+            for (int j = 0; j < at.np; ++j) {
+                const int i = cursor[rec_slot[at.q0 + j]]++;
+                rec_cc[i] = rec_cell[at.q0 + j];
+                for (int c = 0; c < at.nchan; ++c) rec_beta[(size_t)c * ptot + i] = sbeta[at.boff + (size_t)c * at.np + j];
+                if (g->have_k) rec_phase[i] = sphase[at.q0 + j];
+            }
         }
     }
 
@@ -347,15 +390,22 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
     };
     int rc;
     if ((rc = up(&g->d_atoms, atoms)) || (rc = up(&g->d_sidx, sidx)) || (rc = up(&g->d_sbeta, sbeta)) ||
-        (rc = up(&g->d_sphase, sphase)) || (rc = up(&g->d_dscale, dscale)) || (rc = up(&g->d_nl_start, nl_start)) ||
-        (rc = up(&g->d_nl_ent, ent)) || (rc = up(&g->d_nl_phase, ent_phase))) {
+        (rc = up(&g->d_sphase, sphase)) || (rc = up(&g->d_dscale, dscale)) || (rc = up(&g->d_nl_off, nl_off)) ||
+        (rc = up(&g->d_nl_cc, rec_cc)) || (rc = up(&g->d_nl_beta, rec_beta)) || (rc = up(&g->d_nl_phase, rec_phase))) {
         free_projectors(g);
         return rc;
     }
-    cudaError_t e = cudaMalloc(&g->d_dpi, sizeof(cd) * (size_t)g->chunk_cap * ctot);
+    // dpi: [chunk_cap][ctot] plus cmax zeroed entries (records of atoms with fewer than cmax channels read past their
+    // own channels with a zero projector value)
+    const size_t ndpi = (size_t)g->chunk_cap * ctot + cmax;
+    cudaError_t e = cudaMalloc(&g->d_dpi, sizeof(cd) * ndpi);
+    if (e == cudaSuccess) e = cudaMemset(g->d_dpi, 0, sizeof(cd) * ndpi);
     if (e != cudaSuccess) { free_projectors(g); return fail(TDH_ENOMEM, "tdh_set_projectors: %s", cudaGetErrorString(e)); }
     g->natoms = natoms;
     g->nchan_tot = ctot;
+    g->nl_layers = nlayers;
+    g->nl_nrec = (int)ptot;
+    g->nl_cmax = cmax;
     g->mt = cmax <= 8 ? 1 : 2;
     return TDH_OK;
 }
@@ -413,20 +463,22 @@ static int launch_plane_fwd(tdh_grid* g, int nst, const cd* in, cd* out) {
     const cd* twy = g->d_tw[1];
     const cd* twz = g->d_tw[2];
     void* args[] = {(void*)&in, (void*)&out, (void*)&twy, (void*)&twz};
-    const unsigned grid = (unsigned)((size_t)nst * g->n[0] / g->pl.ppc);
-    LAUNCH(K_PLANE_FWD, g->pl.fwd, dim3(grid), dim3(g->pl.threads), g->pl.smem, args);
+    const unsigned grid = (unsigned)((size_t)nst * g->n[0] * g->tl.s / g->tl.ppc);
+    LAUNCH(K_PLANE_FWD, g->tl.fwd, dim3(grid), dim3(g->tl.threads), g->tl.smem, args);
     return TDH_OK;
 }
 
-static int launch_xpencil(tdh_grid* g, int nst, cd* w, int mode) {
+static int launch_xpencil(tdh_grid* g, int nst, const cd* in, cd* out, int mode) {
     tdh::Kinetic kin;
     kin.g2x = g->d_g2[0]; kin.g2y = g->d_g2[1]; kin.g2z = g->d_g2[2];
     kin.ecut = g->ecut;
     kin.scale = 1.0 / (double)g->np;
     kin.nz = g->n[2];
+    kin.nys = g->n[1] / g->tl.s;
     int nynz = g->n[1] * g->n[2];
     const cd* twx = g->d_tw[0];
-    void* args[] = {(void*)&w, (void*)&nynz, (void*)&twx, (void*)&kin};
+    const cd* twy = g->d_tw[1];
+    void* args[] = {(void*)&in, (void*)&out, (void*)&nynz, (void*)&twx, (void*)&twy, (void*)&kin};
     const void* f = mode == 0 ? g->xl.fused : (mode == 1 ? g->xl.fwd : g->xl.inv);
     LAUNCH(K_XPENCIL, f, dim3(nynz / tdh::XP_LPC, nst), dim3(g->xl.threads), 0, args);
     return TDH_OK;
@@ -436,8 +488,8 @@ static int launch_plane_inv(tdh_grid* g, int nst, const cd* in, cd* out, const t
     const cd* twy = g->d_tw[1];
     const cd* twz = g->d_tw[2];
     void* args[] = {(void*)&in, (void*)&out, (void*)&twy, (void*)&twz, (void*)&ep};
-    const unsigned grid = (unsigned)((size_t)nst * g->n[0] / g->pl.ppc);
-    LAUNCH(K_PLANE_INV, g->pl.inv, dim3(grid), dim3(g->pl.threads), g->pl.smem, args);
+    const unsigned grid = (unsigned)((size_t)nst * g->n[0] * g->tl.s / g->tl.ppc);
+    LAUNCH(K_PLANE_INV, g->tl.inv, dim3(grid), dim3(g->tl.threads), g->tl.smem, args);
     return TDH_OK;
 }
 
@@ -454,7 +506,7 @@ static int launch_nl_project(tdh_grid* g, int nst, const cd* in) {
                     (void*)&sphase, (void*)&dscale, (void*)&dpi, (void*)&nct};
     const void* f = g->mt == 1 ? reinterpret_cast<const void*>(&tdh::nl_project_kernel<1>)
                                : reinterpret_cast<const void*>(&tdh::nl_project_kernel<2>);
-    dim3 grid(g->natoms, (nst + tdh::NLP_STATES - 1) / tdh::NLP_STATES);
+    dim3 grid(g->natoms, (nst + tdh::NLP_STATES - 1) / tdh::NLP_STATES);   // y <= 65535: nst <= 524280 per chunk
     LAUNCH(K_NLPROJ, f, grid, dim3(32 * tdh::NLP_WARPS), 0, args);
     return TDH_OK;
 }
@@ -464,19 +516,25 @@ static int apply_chunk(tdh_grid* g, int nst, const cd* in, cd* out, cd alpha, co
     int rc;
     if (g->natoms > 0 && (rc = launch_nl_project(g, nst, in))) return rc;
     if ((rc = launch_plane_fwd(g, nst, in, g->d_work))) return rc;
-    if ((rc = launch_xpencil(g, nst, g->d_work, 0))) return rc;
+    if ((rc = launch_xpencil(g, nst, g->d_work, g->d_work, 0))) return rc;
     tdh::Epilogue ep;
+    memset(&ep, 0, sizeof(ep));
     ep.phi = in;
     ep.v = g->have_v ? g->d_v : nullptr;
     ep.yv = yv;
     ep.alpha = alpha;
     ep.nx = g->n[0];
-    ep.nl_start = g->natoms > 0 ? g->d_nl_start : nullptr;
-    ep.nl_ent = g->d_nl_ent;
-    ep.nl_phase = g->d_nl_phase;
-    ep.nl_beta = g->d_sbeta;
-    ep.dpi = g->d_dpi;
-    ep.nchan_tot = g->nchan_tot;
+    if (g->natoms > 0) {
+        ep.nl_off = g->d_nl_off;
+        ep.nl_layers = g->nl_layers;
+        ep.nl_cc = g->d_nl_cc;
+        ep.nl_beta = g->d_nl_beta;
+        ep.nl_phase = g->d_nl_phase;
+        ep.dpi = g->d_dpi;
+        ep.nrec = g->nl_nrec;
+        ep.cmax = g->nl_cmax;
+        ep.nchan_tot = g->nchan_tot;
+    }
     return launch_plane_inv(g, nst, g->d_work, out, ep);
 }
 
@@ -546,21 +604,21 @@ extern "C" int tdh_fft3d(tdh_grid* g, int nst, tdh_c128* psi_dev, int sign) {
     if (sign != 1 && sign != -1) return fail(TDH_EINVAL, "tdh_fft3d: sign must be -1 or +1");
     stats_reset(g);
     cd* p = (cd*)psi_dev;
-    // the launch grid's y dimension is limited to 65535 states per call
-    for (int s0 = 0; s0 < nst; s0 += 32768) {
-        const int c = std::min(32768, nst - s0);
+    // through the workspace, chunk by chunk (the tile kernels do not work in place when the planes are split)
+    for (int s0 = 0; s0 < nst; s0 += g->chunk_cap) {
+        const int c = std::min(g->chunk_cap, nst - s0);
         cd* q = p + (size_t)s0 * g->np;
         int rc;
         if (sign < 0) {
-            if ((rc = launch_plane_fwd(g, c, q, q))) return rc;
-            if ((rc = launch_xpencil(g, c, q, 1))) return rc;
+            if ((rc = launch_plane_fwd(g, c, q, g->d_work))) return rc;
+            if ((rc = launch_xpencil(g, c, g->d_work, q, 1))) return rc;
         } else {
-            if ((rc = launch_xpencil(g, c, q, 2))) return rc;
+            if ((rc = launch_xpencil(g, c, q, g->d_work, 2))) return rc;
             tdh::Epilogue ep;
             memset(&ep, 0, sizeof(ep));
             ep.alpha = make_double2(1.0, 0.0);
             ep.nx = g->n[0];
-            if ((rc = launch_plane_inv(g, c, q, q, ep))) return rc;
+            if ((rc = launch_plane_inv(g, c, g->d_work, q, ep))) return rc;
         }
     }
     return prof_collect(g);
