@@ -11,8 +11,9 @@ struct TileLaunch {
     int ppc;           // plane parts per CTA
     int s;             // y-split: a plane is s parts (rows y = s*m + r)
     int r1y, r2y;      // factorisation of the y transform of length NY/s (row order inside a tile)
-    int r1z;           // NZ / 8 (cell rotation inside a tile)
-    size_t smem;       // dynamic shared memory per CTA
+    int r1z;           // NZ / 8 (128-byte lines per row)
+    size_t smem_fwd;   // dynamic shared memory per CTA of tile_fwd (ring of tiles)
+    size_t smem_inv;   // dynamic shared memory per CTA of tile_inv (two spectrum buffers + one phi buffer)
 };
 
 struct XLaunch {
@@ -20,6 +21,7 @@ struct XLaunch {
     const void* fwd;    // xpencil_kernel<NX,S,1>
     const void* inv;    // xpencil_kernel<NX,S,2>
     int threads;
+    size_t smem;        // dynamic shared memory per CTA (ring of tiles)
 };
 
 // defined in tile_nz<NZ>.cu / xpencil_inst.cu; return false for an unsupported size

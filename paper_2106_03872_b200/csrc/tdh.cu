@@ -5,6 +5,9 @@
 //     plane_fwd   (tile_fwd: z,y forward FFT per tile of a (state,x) plane)   in  -> work
 //     xpencil     (x forward, 1/2|G+k|^2 scale + mask, x inverse)             work in place
 //     plane_inv   (tile_inv: y,z inverse FFT + epilogue alpha*(T+V+Vnl)phi + y)  work -> out
+// The three FFT kernels are persistent (one CTA per SM, or as many as fit) and fed by TMA: the host encodes a
+// CUtensorMap per launch (tensor_maps.h) and the kernels stream tiles through a shared-memory ring.  `work` holds the
+// spectrum in the digit-permuted order the in-place transforms produce (xpencil_kernel.cuh, WORK LAYOUT).
 // States are independent, so a block is pushed through this chain chunk by chunk; a chunk is as many
 // states as the 1 GiB workspace holds (measured: L2-resident small chunks never win, profiles/r01a_chunk_sweep.md).
 // propagate runs ALL steps of one chunk before moving to the next chunk (H is fixed: readings R10, R16), evaluating
@@ -24,6 +27,7 @@
 #include "../../include/tdh.h"
 #include "launch_tables.h"
 #include "nl_kernels.cuh"
+#include "tensor_maps.h"
 #include "tile_kernels.cuh"
 #include "xpencil_kernel.cuh"
 
@@ -73,6 +77,12 @@ struct tdh_grid {
     bool have_v;
     double* d_g2[3];      // (G_a + k_a)^2
     cd* d_tw[3];          // exp(+2 pi i m / N_a)
+    double* d_g2y_w;      // (G_y + k_y)^2 per plane row of the work layout
+    double* d_g2z_w;      // (G_z + k_z)^2 per column of the work layout
+    cd* d_twy_w;          // exp(+2 pi i k / NY) per row pair of the work layout (y-split grids)
+    int* d_rowmap;        // natural ky -> plane row of the work layout
+    int* d_colmap;        // natural kz -> column of the work layout
+    int ctas_fwd, ctas_inv, ctas_x[3];   // persistent grid sizes (SM count x resident CTAs)
 
     int chunk_cap;        // states the workspace can hold
     int chunk;            // states pushed through the chain together
@@ -184,12 +194,26 @@ extern "C" int tdh_create_grid(const int n[3], const double len[3], const double
 
     int rc = TDH_OK;
     auto body = [&]() -> int {
-        CU(cudaFuncSetAttribute(g->tl.fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g->tl.smem));
-        CU(cudaFuncSetAttribute(g->tl.inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g->tl.smem));
-        // ask for the largest shared-memory carve-out so that the resident-CTA counts of the launch bounds are reached
+        if (!tdh::encode_tiled_fn()) return fail(TDH_ECUDA, "tdh_create_grid: cuTensorMapEncodeTiled not available from the driver");
+        // persistent grids: SM count x the number of CTAs of each kernel that fit on one SM
+        int dev = 0, nsm = 0;
+        CU(cudaGetDevice(&dev));
+        CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
         const void* fs[5] = {g->tl.fwd, g->tl.inv, g->xl.fused, g->xl.fwd, g->xl.inv};
-        for (const void* f : fs)
-            CU(cudaFuncSetAttribute(f, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
+        const size_t sm[5] = {g->tl.smem_fwd, g->tl.smem_inv, g->xl.smem, g->xl.smem, g->xl.smem};
+        const int th[5] = {g->tl.threads, g->tl.threads, g->xl.threads, g->xl.threads, g->xl.threads};
+        int ctas[5];
+        for (int i = 0; i < 5; ++i) {
+            CU(cudaFuncSetAttribute(fs[i], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm[i]));
+            CU(cudaFuncSetAttribute(fs[i], cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
+            int occ = 0;
+            CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fs[i], th[i], sm[i]));
+            if (occ < 1) return fail(TDH_ECUDA, "tdh_create_grid: kernel %d does not fit on an SM", i);
+            if (const char* e = getenv("TDH_MAX_CTAS_PER_SM")) { int v = atoi(e); if (v > 0) occ = std::min(occ, v); }
+            ctas[i] = nsm * occ;
+        }
+        g->ctas_fwd = ctas[0]; g->ctas_inv = ctas[1];
+        g->ctas_x[0] = ctas[2]; g->ctas_x[1] = ctas[3]; g->ctas_x[2] = ctas[4];
         // tables: built on the host exactly as the oracle builds its G vectors (two_pi * m / L + k, then squared)
         const double two_pi = 6.283185307179586476925286766559;
         for (int a = 0; a < 3; ++a) {
@@ -205,6 +229,41 @@ extern "C" int tdh_create_grid(const int n[3], const double len[3], const double
             CU(cudaMalloc(&g->d_tw[a], sizeof(cd) * n[a]));
             CU(cudaMemcpy(g->d_g2[a], g2.data(), sizeof(double) * n[a], cudaMemcpyHostToDevice));
             CU(cudaMemcpy(g->d_tw[a], tw.data(), sizeof(cd) * n[a], cudaMemcpyHostToDevice));
+        }
+        // the same tables in the order of the work layout (xpencil_kernel.cuh): plane row Y = S*rho + r with
+        // rho = k1y*R2Y + k2y <-> k = k1y + R1Y*k2y and ky = k + r*NY/S; column z' = 8*k1 + k2 <-> kz = k1 + (NZ/8)*k2
+        {
+            const int ny = n[1], nz = n[2], S = g->tl.s, nys = ny / S, r1y = g->tl.r1y, r2y = g->tl.r2y, r1z = g->tl.r1z;
+            std::vector<int> rowmap(ny), colmap(nz);
+            std::vector<double> g2y_w(ny), g2z_w(nz);
+            std::vector<cd> twy_w(ny / 2);
+            for (int ky = 0; ky < ny; ++ky) {
+                const int h = ky / nys, k = ky % nys;
+                const int rho = (k % r1y) * r2y + k / r1y;
+                rowmap[ky] = S * rho + h;
+                const double ga = two_pi * freq_index(ky, ny) / len[1] + kpt[1];
+                g2y_w[rowmap[ky]] = ga * ga;
+                if (S == 2 && h == 0) {
+                    const long double ang = 6.283185307179586476925286766559005768L * (long double)k / (long double)ny;
+                    twy_w[rho] = make_double2((double)cosl(ang), (double)sinl(ang));
+                }
+            }
+            if (S == 1) for (auto& w : twy_w) w = make_double2(1.0, 0.0);
+            for (int kz = 0; kz < nz; ++kz) {
+                colmap[kz] = 8 * (kz % r1z) + kz / r1z;
+                const double ga = two_pi * freq_index(kz, nz) / len[2] + kpt[2];
+                g2z_w[colmap[kz]] = ga * ga;
+            }
+            CU(cudaMalloc(&g->d_g2y_w, sizeof(double) * ny));
+            CU(cudaMalloc(&g->d_g2z_w, sizeof(double) * nz));
+            CU(cudaMalloc(&g->d_twy_w, sizeof(cd) * (ny / 2)));
+            CU(cudaMalloc(&g->d_rowmap, sizeof(int) * ny));
+            CU(cudaMalloc(&g->d_colmap, sizeof(int) * nz));
+            CU(cudaMemcpy(g->d_g2y_w, g2y_w.data(), sizeof(double) * ny, cudaMemcpyHostToDevice));
+            CU(cudaMemcpy(g->d_g2z_w, g2z_w.data(), sizeof(double) * nz, cudaMemcpyHostToDevice));
+            CU(cudaMemcpy(g->d_twy_w, twy_w.data(), sizeof(cd) * (ny / 2), cudaMemcpyHostToDevice));
+            CU(cudaMemcpy(g->d_rowmap, rowmap.data(), sizeof(int) * ny, cudaMemcpyHostToDevice));
+            CU(cudaMemcpy(g->d_colmap, colmap.data(), sizeof(int) * nz, cudaMemcpyHostToDevice));
         }
         CU(cudaMalloc(&g->d_v, sizeof(double) * g->np));
         CU(cudaMemset(g->d_v, 0, sizeof(double) * g->np));
@@ -231,6 +290,7 @@ extern "C" int tdh_destroy_grid(tdh_grid* g) {
     free_projectors(g);
     cudaFree(g->d_v);
     for (int a = 0; a < 3; ++a) { cudaFree(g->d_g2[a]); cudaFree(g->d_tw[a]); }
+    cudaFree(g->d_g2y_w); cudaFree(g->d_g2z_w); cudaFree(g->d_twy_w); cudaFree(g->d_rowmap); cudaFree(g->d_colmap);
     cudaFree(g->d_work); cudaFree(g->d_phi[0]); cudaFree(g->d_phi[1]);
     for (int i = 0; i < 2; ++i) {
         cudaFree(g->d_hin[i]); cudaFree(g->d_hout[i]);
@@ -330,7 +390,7 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
     //      share a shared-memory cell and the scatter needs no atomics.  The cell address follows tile_kernels.cuh.
     if (ctot >= 65536) return fail(TDH_EUNSUPPORTED, "tdh_set_projectors: more than 65535 channels");
     const int ny = g->n[1], nz = g->n[2];
-    const int S = g->tl.s, r1y = g->tl.r1y, r2y = g->tl.r2y, r1z = g->tl.r1z;
+    const int S = g->tl.s, r1z = g->tl.r1z;
     int nlayers = 0;
     for (size_t p = 0; p < g->np; ++p) nlayers = std::max(nlayers, cover[p]);
     const int ntiles = g->n[0] * S;
@@ -346,9 +406,8 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
                 const int p = sidx[at.q0 + j];
                 const int x = p / (ny * nz), y = (p / nz) % ny, z = p % nz;
                 const int r = y % S, m = y / S;
-                const int rho = (m % r1y) * r2y + m / r1y;
-                const int grp = rho * r1z + z % r1z;
-                const int cell = 8 * grp + ((z / r1z + grp) & 7);
+                const int line = m * r1z + (z >> 3);                 // natural order after the inverse transforms
+                const int cell = 8 * line + ((z & 7) ^ (line & 7));  // tile_kernels.cuh, swz()
                 const int layer = fill[p]++;
                 const int slot = (x * S + r) * nlayers + layer;
                 rec_slot[at.q0 + j] = slot;
@@ -459,37 +518,78 @@ static void stats_reset(tdh_grid* g) {
         if (rc_) return rc_;                                                                       \
     } while (0)
 
+// CUtensorMap of a chunk of nst states starting at `base` as the tile kernels see it
+static int tile_map(tdh_grid* g, const cd* base, int nst, CUtensorMap* m) {
+    if (!tdh::encode_tile_map(m, base, (size_t)nst * g->n[0], g->n[1], g->n[2], g->tl.s, g->tl.ppc))
+        return fail(TDH_ECUDA, "cuTensorMapEncodeTiled failed (tile map)");
+    return TDH_OK;
+}
+
 static int launch_plane_fwd(tdh_grid* g, int nst, const cd* in, cd* out) {
+    CUtensorMap map;
+    int rc = tile_map(g, in, nst, &map);
+    if (rc) return rc;
     const cd* twy = g->d_tw[1];
     const cd* twz = g->d_tw[2];
-    void* args[] = {(void*)&in, (void*)&out, (void*)&twy, (void*)&twz};
-    const unsigned grid = (unsigned)((size_t)nst * g->n[0] * g->tl.s / g->tl.ppc);
-    LAUNCH(K_PLANE_FWD, g->tl.fwd, dim3(grid), dim3(g->tl.threads), g->tl.smem, args);
+    int ntiles = (int)((size_t)nst * g->n[0] * g->tl.s / g->tl.ppc);
+    void* args[] = {(void*)&map, (void*)&out, (void*)&ntiles, (void*)&twy, (void*)&twz};
+    const unsigned grid = (unsigned)std::min(ntiles, g->ctas_fwd);
+    LAUNCH(K_PLANE_FWD, g->tl.fwd, dim3(grid), dim3(g->tl.threads), g->tl.smem_fwd, args);
     return TDH_OK;
 }
 
 static int launch_xpencil(tdh_grid* g, int nst, const cd* in, cd* out, int mode) {
+    CUtensorMap map;
+    if (!tdh::encode_line_map(&map, in, (size_t)nst * g->n[0], g->n[0], g->n[1], g->n[2]))
+        return fail(TDH_ECUDA, "cuTensorMapEncodeTiled failed (line map)");
     tdh::Kinetic kin;
-    kin.g2x = g->d_g2[0]; kin.g2y = g->d_g2[1]; kin.g2z = g->d_g2[2];
+    kin.g2x = g->d_g2[0]; kin.g2y_w = g->d_g2y_w; kin.g2z_w = g->d_g2z_w; kin.twy_w = g->d_twy_w;
     kin.ecut = g->ecut;
     kin.scale = 1.0 / (double)g->np;
     kin.nz = g->n[2];
-    kin.nys = g->n[1] / g->tl.s;
-    int nynz = g->n[1] * g->n[2];
+    kin.ny = g->n[1];
+    int ntiles = nst * (g->n[1] / 2) * (g->n[2] / 16);
     const cd* twx = g->d_tw[0];
-    const cd* twy = g->d_tw[1];
-    void* args[] = {(void*)&in, (void*)&out, (void*)&nynz, (void*)&twx, (void*)&twy, (void*)&kin};
+    void* args[] = {(void*)&map, (void*)&out, (void*)&ntiles, (void*)&twx, (void*)&kin};
     const void* f = mode == 0 ? g->xl.fused : (mode == 1 ? g->xl.fwd : g->xl.inv);
-    LAUNCH(K_XPENCIL, f, dim3(nynz / tdh::XP_LPC, nst), dim3(g->xl.threads), 0, args);
+    const unsigned grid = (unsigned)std::min(ntiles, g->ctas_x[mode]);
+    LAUNCH(K_XPENCIL, f, dim3(grid), dim3(g->xl.threads), g->xl.smem, args);
     return TDH_OK;
 }
 
-static int launch_plane_inv(tdh_grid* g, int nst, const cd* in, cd* out, const tdh::Epilogue& ep) {
+// in: work block (spectrum), phi: input block of this application (read only when the epilogue has V or projectors)
+static int launch_plane_inv(tdh_grid* g, int nst, const cd* in, const cd* phi, cd* out, const tdh::Epilogue& ep) {
+    CUtensorMap map_spec, map_phi;
+    int rc = tile_map(g, in, nst, &map_spec);
+    if (rc) return rc;
+    if ((rc = tile_map(g, phi ? phi : in, nst, &map_phi))) return rc;
     const cd* twy = g->d_tw[1];
     const cd* twz = g->d_tw[2];
-    void* args[] = {(void*)&in, (void*)&out, (void*)&twy, (void*)&twz, (void*)&ep};
-    const unsigned grid = (unsigned)((size_t)nst * g->n[0] * g->tl.s / g->tl.ppc);
-    LAUNCH(K_PLANE_INV, g->tl.inv, dim3(grid), dim3(g->tl.threads), g->tl.smem, args);
+    int ntiles = (int)((size_t)nst * g->n[0] * g->tl.s / g->tl.ppc);
+    void* args[] = {(void*)&map_spec, (void*)&map_phi, (void*)&out, (void*)&ntiles, (void*)&twy, (void*)&twz, (void*)&ep};
+    const unsigned grid = (unsigned)std::min(ntiles, g->ctas_inv);
+    LAUNCH(K_PLANE_INV, g->tl.inv, dim3(grid), dim3(g->tl.threads), g->tl.smem_inv, args);
+    return TDH_OK;
+}
+
+// natural (ky, kz) order <-> work layout, for tdh_fft3d only.  dir 0: out[plane][ky][kz] = in[plane][rowmap[ky]][colmap[kz]];
+// dir 1: the inverse permutation.
+__global__ void reorder_kernel(const cd* __restrict__ in, cd* __restrict__ out, size_t nplanes, int ny, int nz,
+                               const int* __restrict__ rowmap, const int* __restrict__ colmap, int dir) {
+    const size_t total = nplanes * ny * nz;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const int kz = (int)(i % nz), ky = (int)((i / nz) % ny);
+        const size_t plane = i / ((size_t)ny * nz);
+        const size_t j = (plane * ny + rowmap[ky]) * nz + colmap[kz];
+        if (dir == 0) out[i] = in[j]; else out[j] = in[i];
+    }
+}
+
+static int launch_reorder(tdh_grid* g, int nst, const cd* in, cd* out, int dir) {
+    const size_t nplanes = (size_t)nst * g->n[0];
+    reorder_kernel<<<1184, 256, 0, g->stream>>>(in, out, nplanes, g->n[1], g->n[2], g->d_rowmap, g->d_colmap, dir);
+    CU(cudaGetLastError());
+    g->launch_count += 1;
     return TDH_OK;
 }
 
@@ -519,8 +619,7 @@ static int apply_chunk(tdh_grid* g, int nst, const cd* in, cd* out, cd alpha, co
     if ((rc = launch_xpencil(g, nst, g->d_work, g->d_work, 0))) return rc;
     tdh::Epilogue ep;
     memset(&ep, 0, sizeof(ep));
-    ep.phi = in;
-    ep.v = g->have_v ? g->d_v : nullptr;
+    ep.v = (g->have_v || g->natoms > 0) ? g->d_v : nullptr;   // zero-filled until set; required with projectors
     ep.yv = yv;
     ep.alpha = alpha;
     ep.nx = g->n[0];
@@ -535,7 +634,7 @@ static int apply_chunk(tdh_grid* g, int nst, const cd* in, cd* out, cd alpha, co
         ep.cmax = g->nl_cmax;
         ep.nchan_tot = g->nchan_tot;
     }
-    return launch_plane_inv(g, nst, g->d_work, out, ep);
+    return launch_plane_inv(g, nst, g->d_work, in, out, ep);
 }
 
 static int apply_block(tdh_grid* g, int nst, const cd* psi, cd* hpsi) {
@@ -611,14 +710,16 @@ extern "C" int tdh_fft3d(tdh_grid* g, int nst, tdh_c128* psi_dev, int sign) {
         int rc;
         if (sign < 0) {
             if ((rc = launch_plane_fwd(g, c, q, g->d_work))) return rc;
-            if ((rc = launch_xpencil(g, c, g->d_work, q, 1))) return rc;
+            if ((rc = launch_xpencil(g, c, g->d_work, g->d_work, 1))) return rc;
+            if ((rc = launch_reorder(g, c, g->d_work, q, 0))) return rc;
         } else {
-            if ((rc = launch_xpencil(g, c, q, g->d_work, 2))) return rc;
+            if ((rc = launch_reorder(g, c, q, g->d_work, 1))) return rc;
+            if ((rc = launch_xpencil(g, c, g->d_work, g->d_work, 2))) return rc;
             tdh::Epilogue ep;
             memset(&ep, 0, sizeof(ep));
             ep.alpha = make_double2(1.0, 0.0);
             ep.nx = g->n[0];
-            if ((rc = launch_plane_inv(g, c, g->d_work, q, ep))) return rc;
+            if ((rc = launch_plane_inv(g, c, g->d_work, nullptr, q, ep))) return rc;
         }
     }
     return prof_collect(g);

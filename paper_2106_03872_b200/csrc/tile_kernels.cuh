@@ -1,31 +1,31 @@
-// tile_kernels.cuh -- the two (y,z)-transform kernels of one Hamiltonian application.
+// tile_kernels.cuh -- the two (y,z)-transform kernels of one Hamiltonian application (persistent, TMA-fed).
 //
 //   tile_fwd : per tile: forward FFT along z then y                                   (row a1 of the scope table)
 //   tile_inv : per tile: inverse FFT along y then z, then the fused epilogue
 //              out = alpha * (T psi + V psi + V_nl psi) + y           (rows a3, a4, a5 back-projection, a6, a7 axpy)
 //
 // TILE.  Global layout is [state][x][y][z], z fastest.  A tile is the set of rows y = S*m + r (m = 0..NY/S-1) of one
-// (state, x) plane: the whole plane when S = 1, the even or the odd rows when S = 2.  S = 2 is used for the large
-// planes (96x96, 96x64, 64x96) so that a tile is at most 73,728 bytes and three CTAs fit in the 227 KB of one SM
-// (a 96x96 plane is 147 KB: one CTA per SM and no overlap of the load, FFT and store phases).  With S = 2 the tile
-// transforms only length-NY/2 sequences along y; the remaining radix-2 butterfly of the y transform commutes with the
-// x transform and is done in registers by the x-pencil kernel (xpencil_kernel.cuh), which sees both halves of a line
-// pair in one warp.  The spectrum halves are stored at rows r*(NY/2) + k.
+// (state, x) plane: the whole plane when S = 1 (PPC consecutive planes when they are small), the even or the odd rows
+// when S = 2.  S = 2 is used for the large planes (96x96, 96x64, 64x96) so that a tile is at most 73,728 bytes and a
+// ring of three tiles fits in the 227 KB of one SM.  With S = 2 the tile transforms only length-NY/2 sequences along
+// y; the remaining radix-2 butterfly of the y transform commutes with the x transform and is done in registers by the
+// x-pencil kernel (xpencil_kernel.cuh), which sees both parts of a row pair in one warp.
 //
-// SHARED-MEMORY LAYOUT.  One complex128 is a 16-byte cell; a quarter-warp (8 lanes) of a 128-bit access is
-// conflict free when its 8 cells are distinct modulo 8.  A row of NZ cells is NZ/8 groups of 8 cells; group index
-// g = row*(NZ/8) + k1, cell address 8*g + ((p + g) & 7): the position p inside a group is rotated by g.  Then
-//   * the first z stage (radix NZ/8 across groups, fixed p) touches 8 consecutive p of one group per quarter-warp,
-//   * the second z stage (radix 8 inside a group) runs over consecutive g with a fixed p,
-//   * the y stages run over the 8 positions of one group of one row,
-// and all of them are conflict free WITHOUT padding: a 48x96 tile is exactly 73,728 bytes.  Only the final sweep in
-// natural z order (8 consecutive z straddle two rotation offsets for NZ = 48, 96) has some 2-way conflicts.
-// Every stage overwrites exactly the cells it has read, so one barrier per stage suffices.
+// TMA + SWIZZLE.  A tile is one 4-D box {16 doubles, NZ/8, NY/S, PPC} of a tensor map with 128-byte swizzling
+// (tensor_maps.h): the 128-byte line Ln = row*(NZ/8) + (z >> 3) lands at byte 128*Ln of a 1024-byte aligned buffer
+// and complex value p = z & 7 of the line at chunk p ^ (Ln & 7).  With that hardware XOR swizzle every stage below is
+// free of bank conflicts without padding: a quarter-warp always touches 8 distinct 16-byte chunks modulo 128 bytes
+// (8 positions of one line, or one position of 8 consecutive lines).  CTAs are persistent; one elected thread keeps a
+// ring of buffers filled with cp.async.bulk.tensor, so the next tiles stream in while this one is transformed.
 //
-// 1-D transforms: length N = R1*R2 in two register stages (radix R1 on stride R2, twiddle, radix R2), with
-// z: R2 = 8, R1 = NZ/8;  y (length NY/S): 16 = 4x4, 32 = 8x4, 48 = 8x6, 64 = 8x8.
+// ORDER.  1-D transforms of length N = R1*R2 run as two in-place register stages.  Forward (natural in): radix R1 over
+// j1 (stride R2), twiddle, radix R2 over j2; position k1*R2 + k2 then holds index k1 + R1*k2.  The inverse takes
+// exactly that digit-permuted order as input (radix R2 over k2, twiddle, radix R1 over k1) and ends in natural order,
+// so no reordering pass exists anywhere: the x-pencil kernel works on permuted lines.  z: R2 = 8, R1 = NZ/8;
+// y (length NY/S): 16 = 4x4, 32 = 8x4, 48 = 8x6, 64 = 8x8.
 #pragma once
 #include "fft_codelets.cuh"
+#include "tma.cuh"
 
 namespace tdh {
 
@@ -43,6 +43,8 @@ template <> struct FactY<64> { static constexpr int R1 = 8, R2 = 8; };
 template <> struct FactY<96> { static constexpr int R1 = 12, R2 = 8; };
 
 constexpr int tile_round_up(int a, int b) { return (a + b - 1) / b * b; }
+constexpr int TILE_MAX_CELLS = 4608;
+constexpr int TILE_HEADER = 1024;      // barriers; keeps the buffers 1024-byte aligned
 
 template <int NY, int NZ> struct TileCfg {
     static constexpr int S = (NY * NZ >= 6144) ? 2 : 1;            // y-split (96x96, 96x64, 64x96)
@@ -50,130 +52,182 @@ template <int NY, int NZ> struct TileCfg {
     static constexpr int R1Z = NZ / 8, R2Z = 8;
     static constexpr int R1Y = FactY<NYS>::R1, R2Y = FactY<NYS>::R2;
     static constexpr int PART = NYS * NZ;                           // cells of one plane part
-    static constexpr int PPC = PART <= 1152 ? 4 : (PART <= 2304 ? 2 : 1);   // parts per CTA: at most 4608 cells
+    static constexpr int pick_ppc() {
+        if (S == 2) return 1;
+        int p = 1;
+        while (p < 16 && 2 * p * PART <= TILE_MAX_CELLS) p *= 2;
+        return p;
+    }
+    static constexpr int PPC = pick_ppc();                          // plane parts per tile (divides NX: NX % 16 == 0)
     static constexpr int ROWS = PPC * NYS;
     static constexpr int CELLS = ROWS * NZ;
-    static constexpr size_t SMEM = (size_t)CELLS * sizeof(cd);
+    static constexpr size_t TILE_BYTES = (size_t)CELLS * sizeof(cd);
+    static constexpr int NB_FWD = 3;                                // ring depth of tile_fwd
+    static constexpr size_t SMEM_FWD = TILE_HEADER + NB_FWD * TILE_BYTES;
+    static constexpr size_t SMEM_INV = TILE_HEADER + 3 * TILE_BYTES;   // two spectrum buffers + one phi buffer
     // work items of the four stages
     static constexpr int I_ZA = ROWS * 8, I_ZB = ROWS * R1Z, I_YA = PPC * NZ * R2Y, I_YB = PPC * NZ * R1Y;
     static constexpr int cost(int t) {
         return tile_round_up(I_ZA, t) + tile_round_up(I_ZB, t) + tile_round_up(I_YA, t) + tile_round_up(I_YB, t);
     }
     static constexpr int pick_t() {
-        int best = 64;
-        const int cand[5] = {64, 96, 128, 192, 256};
+        int best = 256;
+        const int cand[5] = {256, 320, 384, 448, 512};
         for (int i = 0; i < 5; ++i)
-            if (cand[i] * 2 <= I_ZA && cost(cand[i]) <= cost(best)) best = cand[i];
+            if (cost(cand[i]) <= cost(best)) best = cand[i];
         return best;
     }
+#ifdef TDH_TILE_THREADS
+    static constexpr int T = TDH_TILE_THREADS;
+#else
     static constexpr int T = pick_t();
-    // resident CTAs per SM the launch bounds ask for: limited by shared memory (227 KB, 1 KB reserved per CTA) and by
-    // a register budget of >= 80 per thread (>= 104 when the first z stage holds 12 values + 11 twiddles)
-    static constexpr int REGS = R1Z > 8 ? 104 : 80;
-    static constexpr int by_smem = (int)(232448 / (SMEM + 1024));
-    static constexpr int by_regs = 65536 / (T * REGS);
-    static constexpr int MINB = by_smem < by_regs ? (by_smem < 1 ? 1 : by_smem) : (by_regs < 1 ? 1 : by_regs);
-    static_assert(NZ % 8 == 0 && T % 8 == 0, "z stage mapping");
-    static_assert((NYS * R1Z) % 8 == 0, "group rotation must not depend on the plane part");
+#endif
+    static_assert(NZ % 16 == 0 && T % 8 == 0, "z stage mapping");
+    static_assert(PART % 64 == 0, "plane parts must keep the 1024-byte swizzle phase");
+    static_assert(CELLS <= TILE_MAX_CELLS, "tile too large");
 };
 
-// cell address of (row lr of the tile, group k1, position p): 8*g + ((p + g) & 7), g = lr*R1Z + k1
-template <int R1Z> __device__ __forceinline__ int cell_addr(int lr, int k1, int p) {
-    const int g = lr * R1Z + k1;
-    return 8 * g + ((p + g) & 7);
-}
+// cell (in complex values) of position p of 128-byte line ln in a swizzled tile buffer
+__device__ __forceinline__ int swz(int ln, int p) { return 8 * ln + (p ^ (ln & 7)); }
 
 // ------------------------------------------------------------------------------------------------------------
-// forward: in -> out (must not alias when S = 2).  Grid: nst * NX * S / PPC tiles.
+// forward: `map_in` describes the input block, `out` is the work block (same geometry, digit-permuted spectrum).
+// Persistent grid; ntiles = nst * NX * S / PPC.
 // ------------------------------------------------------------------------------------------------------------
 template <int NY, int NZ>
-__global__ void __launch_bounds__(TileCfg<NY, NZ>::T, TileCfg<NY, NZ>::MINB)
-tile_fwd_kernel(const cd* __restrict__ in, cd* __restrict__ out, const cd* __restrict__ tw_y,
-                const cd* __restrict__ tw_z)
+__global__ void __launch_bounds__(TileCfg<NY, NZ>::T, 1)
+tile_fwd_kernel(const __grid_constant__ CUtensorMap map_in, cd* __restrict__ out, int ntiles,
+                const cd* __restrict__ tw_y, const cd* __restrict__ tw_z)
 {
     using C = TileCfg<NY, NZ>;
-    constexpr int S = C::S, NYS = C::NYS, R1Z = C::R1Z, R1Y = C::R1Y, R2Y = C::R2Y, T = C::T;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    cd* sm = reinterpret_cast<cd*>(smem_raw);
+    constexpr int S = C::S, NYS = C::NYS, R1Z = C::R1Z, R1Y = C::R1Y, R2Y = C::R2Y, T = C::T, NB = C::NB_FWD;
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);
+    cd* ring = reinterpret_cast<cd*>(smem_raw + TILE_HEADER);
     const int tid = threadIdx.x;
-    const int part0 = blockIdx.x * C::PPC;
 
-    // ---- z stage A: global -> registers, radix R1Z over j1 (stride 8 cells), twiddle w^(k1*j2) -> cell (lr, k1, j2)
+    uint64_t pol = 0;
+    if (tid == 0) {
+        tma_prefetch_desc(&map_in);
+        pol = policy_evict_first();
+        for (int b = 0; b < NB; ++b) mbar_init(full + b, 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    auto issue = [&](int t, int b) {                    // thread 0 only
+        const int part0 = t * C::PPC, plane = part0 / S, r = part0 % S;
+        mbar_arrive_expect_tx(full + b, (uint32_t)C::TILE_BYTES);
+        tma_load_4d(ring + (size_t)b * C::CELLS, &map_in, full + b, 0, r * R1Z, 0, plane, pol);
+    };
+    if (tid == 0)
+        for (int b = 0; b < NB; ++b) {
+            const int t = blockIdx.x + b * gridDim.x;
+            if (t < ntiles) issue(t, b);
+        }
+
+    // z stage A twiddles of this thread's column j2 = tid & 7: w_NZ^(k1*j2)
+    cd twz[R1Z];
     {
         const int j2 = tid & 7;
-        cd tw[R1Z];
 #pragma unroll
-        for (int k1 = 1; k1 < R1Z; ++k1) tw[k1] = ldg_cd(tw_z + k1 * j2);
-        for (int lr = tid >> 3; lr < C::ROWS; lr += T / 8) {
-            const int lp = lr / NYS, m = lr % NYS;
-            const int part = part0 + lp, plane = part / S, r = part % S;
-            const cd* src = in + (size_t)plane * NY * NZ + (size_t)(S * m + r) * NZ + j2;
-            cd x[R1Z];
+        for (int k1 = 1; k1 < R1Z; ++k1) twz[k1] = ldg_cd(tw_z + k1 * j2);
+    }
+
+    int it = 0;
+    for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++it) {
+        const int b = it % NB;
+        cd* sm = ring + (size_t)b * C::CELLS;
+        const int part0 = t * C::PPC;
+        mbar_wait(full + b, (uint32_t)(it / NB) & 1u);
+
+        // ---- z stage A, in place: radix R1Z over j1 (lines lr*R1Z + j1, position j2), twiddle w^(k1*j2)
+        {
+            const int j2 = tid & 7;
+            for (int lr = tid >> 3; lr < C::ROWS; lr += T / 8) {
+                const int l0 = lr * R1Z;
+                cd x[R1Z];
 #pragma unroll
-            for (int j1 = 0; j1 < R1Z; ++j1) x[j1] = lds_cd(src + j1 * 8);
-            Dft<R1Z, -1>::run(x);
-            sm[cell_addr<R1Z>(lr, 0, j2)] = x[0];
+                for (int j1 = 0; j1 < R1Z; ++j1) x[j1] = sm[swz(l0 + j1, j2)];
+                Dft<R1Z, -1>::run(x);
+                sm[swz(l0, j2)] = x[0];
 #pragma unroll
-            for (int k1 = 1; k1 < R1Z; ++k1) sm[cell_addr<R1Z>(lr, k1, j2)] = cmulc(x[k1], tw[k1]);
+                for (int k1 = 1; k1 < R1Z; ++k1) sm[swz(l0 + k1, j2)] = cmulc(x[k1], twz[k1]);
+            }
         }
-    }
-    __syncthreads();
-    // ---- z stage B, in place inside group g: position k2 then holds kz = k1 + R1Z*k2
-    for (int g = tid; g < C::I_ZB; g += T) {
-        cd* p = sm + 8 * g;
-        const int s = g & 7;
-        cd t[8];
+        __syncthreads();
+        // ---- z stage B, in place inside line g: position k2 then holds kz = k1 + R1Z*k2
+        for (int g = tid; g < C::I_ZB; g += T) {
+            cd* p = sm + 8 * g;
+            const int s = g & 7;
+            cd v[8];
 #pragma unroll
-        for (int j2 = 0; j2 < 8; ++j2) t[j2] = p[(j2 + s) & 7];
-        Dft<8, -1>::run(t);
+            for (int j2 = 0; j2 < 8; ++j2) v[j2] = p[j2 ^ s];
+            Dft<8, -1>::run(v);
 #pragma unroll
-        for (int k2 = 0; k2 < 8; ++k2) p[(k2 + s) & 7] = t[k2];
-    }
-    __syncthreads();
-    // ---- y stage A, in place: rows j1*R2Y + j2 of column c = (k1, k2) -> rows k1y*R2Y + j2
-    for (int item = tid; item < C::I_YA; item += T) {
-        const int c = item % NZ, rr = item / NZ, j2 = rr % R2Y, lp = rr / R2Y;
-        const int k1 = c >> 3, k2 = c & 7;
-        const int row0 = lp * NYS + j2;
-        cd x[R1Y];
+            for (int k2 = 0; k2 < 8; ++k2) p[k2 ^ s] = v[k2];
+        }
+        __syncthreads();
+        // ---- y stage A, in place: rows j1*R2Y + j2 of column c = (k1, k2) -> rows k1y*R2Y + j2
+        for (int item = tid; item < C::I_YA; item += T) {
+            const int c = item % NZ, rr = item / NZ, j2 = rr % R2Y, lp = rr / R2Y;
+            const int k1 = c >> 3, k2 = c & 7;
+            const int row0 = lp * NYS + j2;
+            cd x[R1Y];
 #pragma unroll
-        for (int j1 = 0; j1 < R1Y; ++j1) x[j1] = sm[cell_addr<R1Z>(row0 + j1 * R2Y, k1, k2)];
-        Dft<R1Y, -1>::run(x);
-        sm[cell_addr<R1Z>(row0, k1, k2)] = x[0];
+            for (int j1 = 0; j1 < R1Y; ++j1) x[j1] = sm[swz((row0 + j1 * R2Y) * R1Z + k1, k2)];
+            Dft<R1Y, -1>::run(x);
+            sm[swz(row0 * R1Z + k1, k2)] = x[0];
 #pragma unroll
-        for (int k1y = 1; k1y < R1Y; ++k1y)
-            sm[cell_addr<R1Z>(row0 + k1y * R2Y, k1, k2)] = cmulc(x[k1y], ldg_cd(tw_y + S * k1y * j2));
-    }
-    __syncthreads();
-    // ---- y stage B -> global, natural kz order; spectrum half r goes to rows r*NYS + ky
-    for (int item = tid; item < C::I_YB; item += T) {
-        const int kz = item % NZ, rr = item / NZ, k1y = rr % R1Y, lp = rr / R1Y;
-        const int k1 = kz % R1Z, k2 = kz / R1Z;
-        const int row0 = lp * NYS + k1y * R2Y;
-        cd t[R2Y];
+            for (int k1y = 1; k1y < R1Y; ++k1y)
+                sm[swz((row0 + k1y * R2Y) * R1Z + k1, k2)] = cmulc(x[k1y], ldg_cd(tw_y + S * k1y * j2));
+        }
+        __syncthreads();
+        // ---- y stage B -> global at the in-place position: row rho = k1y*R2Y + k2y (plane row S*rho + r), column c
+        constexpr int RB = (C::I_YB + T - 1) / T;
+        cd res[RB][R2Y];
 #pragma unroll
-        for (int j2 = 0; j2 < R2Y; ++j2) t[j2] = sm[cell_addr<R1Z>(row0 + j2, k1, k2)];
-        Dft<R2Y, -1>::run(t);
-        const int part = part0 + lp, plane = part / S, r = part % S;
-        cd* dst = out + (size_t)plane * NY * NZ + (size_t)(r * NYS) * NZ + kz;
+        for (int u = 0; u < RB; ++u) {
+            const int item = tid + u * T;
+            if (item < C::I_YB) {
+                const int c = item % NZ, rr = item / NZ, k1y = rr % R1Y, lp = rr / R1Y;
+                const int k1 = c >> 3, k2 = c & 7;
+                const int row0 = lp * NYS + k1y * R2Y;
 #pragma unroll
-        for (int k2y = 0; k2y < R2Y; ++k2y) dst[(size_t)(k1y + R1Y * k2y) * NZ] = t[k2y];
+                for (int j2 = 0; j2 < R2Y; ++j2) res[u][j2] = sm[swz((row0 + j2) * R1Z + k1, k2)];
+            }
+        }
+        // every read of this buffer is done: hand it back to the TMA before the butterflies and the stores
+        fence_proxy_async();
+        __syncthreads();
+        if (tid == 0 && t + NB * (int)gridDim.x < ntiles) issue(t + NB * gridDim.x, b);
+#pragma unroll
+        for (int u = 0; u < RB; ++u) {
+            const int item = tid + u * T;
+            if (item < C::I_YB) {
+                const int c = item % NZ, rr = item / NZ, k1y = rr % R1Y, lp = rr / R1Y;
+                Dft<R2Y, -1>::run(res[u]);
+                const int part = part0 + lp, plane = part / S, r = part % S;
+                cd* dst = out + (size_t)plane * NY * NZ + (size_t)(S * (k1y * R2Y) + r) * NZ + c;
+#pragma unroll
+                for (int k2y = 0; k2y < R2Y; ++k2y) sts_cd(dst + (size_t)(S * k2y) * NZ, res[u][k2y]);
+            }
+        }
     }
 }
 
 // Arguments of the fused epilogue of tile_inv.
 struct Epilogue {
-    const cd* phi;          // input block of this application (for V*phi); used only when v != NULL
-    const double* v;        // V(r), n0*n1*n2; NULL: no local term
+    const double* v;        // V(r), n0*n1*n2; NULL: no local term (then map_phi is not used, unless nl_off != NULL)
     const cd* yv;           // optional addend y (same block layout as out); NULL: none
     cd alpha;               // out = alpha * (T + V + Vnl) phi + y
     int nx;                 // planes per state
     // Kleinman-Bylander back-projection (second half of Eq. 9), as per-tile record lists; nl_off == NULL: none.
     // Tile (x, r) owns records nl_off[(x*S + r)*(nl_layers+1) + l] .. [.. + l + 1) of layer l; within one layer every
-    // grid point appears at most once, so the shared-memory read-modify-write needs no atomics.
+    // grid point appears at most once, so the shared-memory read-modify-write needs no atomics.  With projectors, v must
+    // not be NULL (the handle passes its zero-filled potential when none was set).
     const int* nl_off;
     int nl_layers;
-    const unsigned* nl_cc;  // per record: cell address inside the plane part | first channel << 16
+    const unsigned* nl_cc;  // per record: swizzled cell inside the plane part | first channel << 16
     const double* nl_beta;  // [cmax][nrec] projector values, zero padded above the atom's channel count
     const cd* nl_phase;     // per record e^{+ik.d}; NULL at Gamma
     const cd* dpi;          // [state][nchan_tot] D * dV * <beta|phi>  (+ cmax zeroed entries of padding)
@@ -183,126 +237,198 @@ struct Epilogue {
 };
 
 // ------------------------------------------------------------------------------------------------------------
-// inverse + epilogue: in -> out (must not alias when S = 2)
+// inverse + epilogue: `map_spec` describes the work block (digit-permuted spectrum), `map_phi` the input block of this
+// Hamiltonian application (same geometry), `out` the output block.  Shared memory: two spectrum buffers X0, X1 (tile
+// i in X[i & 1], tile i+1 streaming into the other) and one buffer Y for phi of the current tile, which becomes
+// V*phi + V_nl phi when there are projectors.  Persistent grid; ntiles = nst * NX * S / PPC.
 // ------------------------------------------------------------------------------------------------------------
 template <int NY, int NZ>
-__global__ void __launch_bounds__(TileCfg<NY, NZ>::T, TileCfg<NY, NZ>::MINB)
-tile_inv_kernel(const cd* __restrict__ in, cd* __restrict__ out, const cd* __restrict__ tw_y,
-                const cd* __restrict__ tw_z, const Epilogue ep)
+__global__ void __launch_bounds__(TileCfg<NY, NZ>::T, 1)
+tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_constant__ CUtensorMap map_phi,
+                cd* __restrict__ out, int ntiles, const cd* __restrict__ tw_y, const cd* __restrict__ tw_z,
+                const Epilogue ep)
 {
     using C = TileCfg<NY, NZ>;
     constexpr int S = C::S, NYS = C::NYS, R1Z = C::R1Z, R1Y = C::R1Y, R2Y = C::R2Y, T = C::T;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    cd* sm = reinterpret_cast<cd*>(smem_raw);
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);             // [0], [1]: X buffers; [2]: Y
+    cd* xbuf = reinterpret_cast<cd*>(smem_raw + TILE_HEADER);
+    cd* ybuf = xbuf + 2 * (size_t)C::CELLS;
     const int tid = threadIdx.x;
-    const int part0 = blockIdx.x * C::PPC;
+    const bool have_nl = ep.nl_off != nullptr;
+    const bool have_phi = have_nl || ep.v != nullptr;
 
-    // ---- y stage A: global rows r*NYS + n1*R2Y + n2 -> registers, radix R1Y, twiddle -> rows m1*R2Y + n2
-    for (int item = tid; item < C::I_YA; item += T) {
-        const int kz = item % NZ, rr = item / NZ, n2 = rr % R2Y, lp = rr / R2Y;
-        const int part = part0 + lp, plane = part / S, r = part % S;
-        const cd* src = in + (size_t)plane * NY * NZ + (size_t)(r * NYS + n2) * NZ + kz;
-        cd x[R1Y];
-#pragma unroll
-        for (int n1 = 0; n1 < R1Y; ++n1) x[n1] = lds_cd(src + (size_t)n1 * R2Y * NZ);
-        Dft<R1Y, +1>::run(x);
-        const int row0 = lp * NYS + n2, grp = kz >> 3, pos = kz & 7;
-        sm[cell_addr<R1Z>(row0, grp, pos)] = x[0];
-#pragma unroll
-        for (int m1 = 1; m1 < R1Y; ++m1)
-            sm[cell_addr<R1Z>(row0 + m1 * R2Y, grp, pos)] = cmul(x[m1], ldg_cd(tw_y + S * m1 * n2));
+    uint64_t pol = 0;
+    if (tid == 0) {
+        tma_prefetch_desc(&map_spec);
+        tma_prefetch_desc(&map_phi);
+        pol = policy_evict_first();
+        for (int b = 0; b < 3; ++b) mbar_init(full + b, 1);
+        mbar_fence_init();
     }
     __syncthreads();
-    // ---- y stage B, in place: row m1*R2Y + m2 then holds m = m1 + R1Y*m2, i.e. y = S*m + r
-    for (int item = tid; item < C::I_YB; item += T) {
-        const int c = item % NZ, rr = item / NZ, m1 = rr % R1Y, lp = rr / R1Y;
-        const int grp = c >> 3, pos = c & 7;
-        const int row0 = lp * NYS + m1 * R2Y;
-        cd t[R2Y];
-#pragma unroll
-        for (int n2 = 0; n2 < R2Y; ++n2) t[n2] = sm[cell_addr<R1Z>(row0 + n2, grp, pos)];
-        Dft<R2Y, +1>::run(t);
-#pragma unroll
-        for (int m2 = 0; m2 < R2Y; ++m2) sm[cell_addr<R1Z>(row0 + m2, grp, pos)] = t[m2];
-    }
-    __syncthreads();
-    // ---- z stage A, in place: input kz = 8*n1 + n2 sits at (group n1, position n2); radix R1Z over n1, twiddle
-    {
-        const int n2 = tid & 7;
-        cd tw[R1Z];
-#pragma unroll
-        for (int m1 = 1; m1 < R1Z; ++m1) tw[m1] = ldg_cd(tw_z + m1 * n2);
-        for (int lr = tid >> 3; lr < C::ROWS; lr += T / 8) {
-            cd x[R1Z];
-#pragma unroll
-            for (int n1 = 0; n1 < R1Z; ++n1) x[n1] = sm[cell_addr<R1Z>(lr, n1, n2)];
-            Dft<R1Z, +1>::run(x);
-            sm[cell_addr<R1Z>(lr, 0, n2)] = x[0];
-#pragma unroll
-            for (int m1 = 1; m1 < R1Z; ++m1) sm[cell_addr<R1Z>(lr, m1, n2)] = cmul(x[m1], tw[m1]);
+    auto issue = [&](const CUtensorMap* map, int t, cd* dst, uint64_t* bar) {      // thread 0 only
+        const int part0 = t * C::PPC, plane = part0 / S, r = part0 % S;
+        mbar_arrive_expect_tx(bar, (uint32_t)C::TILE_BYTES);
+        tma_load_4d(dst, map, bar, 0, r * R1Z, 0, plane, pol);
+    };
+    if (tid == 0) {
+        const int t0 = blockIdx.x, t1 = blockIdx.x + gridDim.x;
+        if (t0 < ntiles) {
+            issue(&map_spec, t0, xbuf, full + 0);
+            if (have_phi) issue(&map_phi, t0, ybuf, full + 2);
         }
+        if (t1 < ntiles) issue(&map_spec, t1, xbuf + C::CELLS, full + 1);
     }
-    __syncthreads();
-    // ---- z stage B, in place: (group m1, position m2) then holds z = m1 + R1Z*m2 of the kinetic term
-    for (int g = tid; g < C::I_ZB; g += T) {
-        cd* p = sm + 8 * g;
-        const int s = g & 7;
-        cd t[8];
+
+    // last z stage twiddles of this thread's column j2 = tid & 7: w_NZ^(-k1*j2)
+    cd twz[R1Z];
+    {
+        const int j2 = tid & 7;
 #pragma unroll
-        for (int n2 = 0; n2 < 8; ++n2) t[n2] = p[(n2 + s) & 7];
-        Dft<8, +1>::run(t);
-#pragma unroll
-        for (int m2 = 0; m2 < 8; ++m2) p[(m2 + s) & 7] = t[m2];
+        for (int k1 = 1; k1 < R1Z; ++k1) twz[k1] = ldg_cd(tw_z + k1 * j2);
     }
-    __syncthreads();
-    // ---- Kleinman-Bylander back-projection into the tile (layer by layer: no two records of a layer share a cell)
-    if (ep.nl_off != nullptr) {
-        for (int layer = 0; layer < ep.nl_layers; ++layer) {
+
+    int it = 0;
+    for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++it) {
+        const int cur = it & 1;
+        cd* sm = xbuf + (size_t)cur * C::CELLS;
+        const int part0 = t * C::PPC;
+        mbar_wait(full + cur, (uint32_t)(it >> 1) & 1u);
+
+        // ---- y stage A', in place: rows k1y*R2Y + k2y (contiguous) hold k = k1y + R1Y*k2y; radix R2Y over k2y -> j2,
+        //      twiddle w^(-j2*k1y)
+        for (int item = tid; item < C::I_YB; item += T) {
+            const int c = item % NZ, rr = item / NZ, k1y = rr % R1Y, lp = rr / R1Y;
+            const int k1 = c >> 3, k2 = c & 7;
+            const int row0 = lp * NYS + k1y * R2Y;
+            cd v[R2Y];
 #pragma unroll
-            for (int lp = 0; lp < C::PPC; ++lp) {
+            for (int k2y = 0; k2y < R2Y; ++k2y) v[k2y] = sm[swz((row0 + k2y) * R1Z + k1, k2)];
+            Dft<R2Y, +1>::run(v);
+            sm[swz(row0 * R1Z + k1, k2)] = v[0];
+#pragma unroll
+            for (int j2 = 1; j2 < R2Y; ++j2)
+                sm[swz((row0 + j2) * R1Z + k1, k2)] = cmul(v[j2], ldg_cd(tw_y + S * j2 * k1y));
+        }
+        __syncthreads();
+        // ---- y stage B', in place: rows k1y*R2Y + j2, radix R1Y over k1y -> j1: row j1*R2Y + j2 = m, y = S*m + r
+        for (int item = tid; item < C::I_YA; item += T) {
+            const int c = item % NZ, rr = item / NZ, j2 = rr % R2Y, lp = rr / R2Y;
+            const int k1 = c >> 3, k2 = c & 7;
+            const int row0 = lp * NYS + j2;
+            cd x[R1Y];
+#pragma unroll
+            for (int k1y = 0; k1y < R1Y; ++k1y) x[k1y] = sm[swz((row0 + k1y * R2Y) * R1Z + k1, k2)];
+            Dft<R1Y, +1>::run(x);
+#pragma unroll
+            for (int j1 = 0; j1 < R1Y; ++j1) sm[swz((row0 + j1 * R2Y) * R1Z + k1, k2)] = x[j1];
+        }
+        __syncthreads();
+        // ---- z stage A', in place inside line g = (row, k1): positions k2 hold kz = k1 + R1Z*k2; radix 8 -> j2
+        for (int g = tid; g < C::I_ZB; g += T) {
+            cd* p = sm + 8 * g;
+            const int s = g & 7;
+            cd v[8];
+#pragma unroll
+            for (int k2 = 0; k2 < 8; ++k2) v[k2] = p[k2 ^ s];
+            Dft<8, +1>::run(v);
+#pragma unroll
+            for (int j2 = 0; j2 < 8; ++j2) p[j2 ^ s] = v[j2];
+        }
+        // ---- with projectors: Y = V * phi, then the back-projection adds V_nl phi into Y layer by layer
+        if (have_nl) {
+            mbar_wait(full + 2, (uint32_t)it & 1u);
+            const int j2 = tid & 7;
+            for (int lr = tid >> 3; lr < C::ROWS; lr += T / 8) {
+                const int lp = lr / NYS, m = lr % NYS;
                 const int part = part0 + lp, plane = part / S, r = part % S;
-                const int st = plane / ep.nx, x = plane % ep.nx;
-                const int* off = ep.nl_off + (size_t)(x * S + r) * (ep.nl_layers + 1) + layer;
-                const int i1 = __ldg(off + 1);
-                const cd* dp = ep.dpi + (size_t)st * ep.nchan_tot;
-                cd* base = sm + lp * C::PART;
-                for (int i = __ldg(off) + tid; i < i1; i += T) {
-                    const unsigned cc = __ldg(ep.nl_cc + i);
-                    const cd* d = dp + (cc >> 16);
-                    const double* b = ep.nl_beta + i;
-                    cd s = make_double2(0.0, 0.0);
-                    for (int c = 0; c < ep.cmax; ++c) {
-                        const double bv = __ldg(b + (size_t)c * ep.nrec);
-                        const cd dv = ldg_cd(d + c);
-                        s.x = fma(bv, dv.x, s.x);
-                        s.y = fma(bv, dv.y, s.y);
-                    }
-                    if (ep.nl_phase != nullptr) s = cmulc(s, ldg_cd(ep.nl_phase + i));
-                    cd* cell = base + (cc & 0xffffu);
-                    *cell = cadd(*cell, s);
+                const double* vrow = ep.v + ((size_t)(plane % ep.nx) * NY + (S * m + r)) * NZ + j2;
+#pragma unroll
+                for (int j1 = 0; j1 < R1Z; ++j1) {
+                    const int cell = swz(lr * R1Z + j1, j2);
+                    const double vv = __ldg(vrow + 8 * j1);
+                    const cd ph = ybuf[cell];
+                    ybuf[cell] = make_double2(vv * ph.x, vv * ph.y);
                 }
             }
             __syncthreads();
+            for (int layer = 0; layer < ep.nl_layers; ++layer) {
+#pragma unroll
+                for (int lp = 0; lp < C::PPC; ++lp) {
+                    const int part = part0 + lp, plane = part / S, r = part % S;
+                    const int st = plane / ep.nx, x = plane % ep.nx;
+                    const int* off = ep.nl_off + (size_t)(x * S + r) * (ep.nl_layers + 1) + layer;
+                    const int i1 = __ldg(off + 1);
+                    const cd* dp = ep.dpi + (size_t)st * ep.nchan_tot;
+                    cd* base = ybuf + lp * C::PART;
+                    for (int i = __ldg(off) + tid; i < i1; i += T) {
+                        const unsigned cc = __ldg(ep.nl_cc + i);
+                        const cd* d = dp + (cc >> 16);
+                        const double* bq = ep.nl_beta + i;
+                        cd sacc = make_double2(0.0, 0.0);
+                        for (int c = 0; c < ep.cmax; ++c) {
+                            const double bv = __ldg(bq + (size_t)c * ep.nrec);
+                            const cd dv = ldg_cd(d + c);
+                            sacc.x = fma(bv, dv.x, sacc.x);
+                            sacc.y = fma(bv, dv.y, sacc.y);
+                        }
+                        if (ep.nl_phase != nullptr) sacc = cmulc(sacc, ldg_cd(ep.nl_phase + i));
+                        cd* cell = base + (cc & 0xffffu);
+                        *cell = cadd(*cell, sacc);
+                    }
+                }
+                __syncthreads();
+            }
+        } else {
+            if (have_phi) mbar_wait(full + 2, (uint32_t)it & 1u);
+            __syncthreads();
         }
-    }
-    // ---- sweep in natural z order: out = alpha * (T phi + V phi + Vnl phi) + y
-    for (int item = tid; item < C::CELLS; item += T) {
-        const int z = item % NZ, lr = item / NZ;
-        const int lp = lr / NYS, rho = lr % NYS;
-        const int part = part0 + lp, plane = part / S, r = part % S;
-        const int y = S * (rho / R2Y + R1Y * (rho % R2Y)) + r;
-        cd acc = sm[cell_addr<R1Z>(lr, z % R1Z, z / R1Z)];
-        const size_t gi = (size_t)plane * NY * NZ + (size_t)y * NZ + z;                    // index in the block
-        if (ep.v != nullptr) {
-            const size_t q = ((size_t)(plane % ep.nx) * NY + y) * NZ + z;                 // index in the state
-            const cd ph = lds_cd(ep.phi + gi);
-            const double vv = __ldg(ep.v + q);
-            acc.x = fma(vv, ph.x, acc.x);
-            acc.y = fma(vv, ph.y, acc.y);
+        // ---- z stage B' + epilogue: thread (row lr, j2): twiddle, radix R1Z over k1 -> z = 8*j1 + j2;
+        //      out = alpha * (T phi + V phi + Vnl phi) + y, straight from registers
+        {
+            const int j2 = tid & 7;
+            for (int lr = tid >> 3; lr < C::ROWS; lr += T / 8) {
+                const int l0 = lr * R1Z;
+                cd x[R1Z];
+                x[0] = sm[swz(l0, j2)];
+#pragma unroll
+                for (int k1 = 1; k1 < R1Z; ++k1) x[k1] = cmul(sm[swz(l0 + k1, j2)], twz[k1]);
+                Dft<R1Z, +1>::run(x);
+                const int lp = lr / NYS, m = lr % NYS;
+                const int part = part0 + lp, plane = part / S, r = part % S;
+                const int y = S * m + r;
+                const size_t gi = (size_t)plane * NY * NZ + (size_t)y * NZ + j2;               // index in the block
+                if (have_nl) {
+#pragma unroll
+                    for (int j1 = 0; j1 < R1Z; ++j1) x[j1] = cadd(x[j1], ybuf[swz(l0 + j1, j2)]);
+                } else if (ep.v != nullptr) {
+                    const double* vrow = ep.v + ((size_t)(plane % ep.nx) * NY + y) * NZ + j2;
+#pragma unroll
+                    for (int j1 = 0; j1 < R1Z; ++j1) {
+                        const double vv = __ldg(vrow + 8 * j1);
+                        const cd ph = ybuf[swz(l0 + j1, j2)];
+                        x[j1].x = fma(vv, ph.x, x[j1].x);
+                        x[j1].y = fma(vv, ph.y, x[j1].y);
+                    }
+                }
+                if (ep.yv != nullptr) {
+#pragma unroll
+                    for (int j1 = 0; j1 < R1Z; ++j1) sts_cd(out + gi + 8 * j1, cadd(cmul(ep.alpha, x[j1]), lds_cd(ep.yv + gi + 8 * j1)));
+                } else {
+#pragma unroll
+                    for (int j1 = 0; j1 < R1Z; ++j1) sts_cd(out + gi + 8 * j1, cmul(ep.alpha, x[j1]));
+                }
+            }
         }
-        cd o = cmul(ep.alpha, acc);
-        if (ep.yv != nullptr) o = cadd(o, lds_cd(ep.yv + gi));
-        sts_cd(out + gi, o);
+        // every read of X[cur] and Y is done: stream in the spectrum of tile i+2 and phi of tile i+1
+        fence_proxy_async();
+        __syncthreads();
+        if (tid == 0) {
+            const int t1 = t + gridDim.x, t2 = t + 2 * gridDim.x;
+            if (t2 < ntiles) issue(&map_spec, t2, sm, full + cur);
+            if (have_phi && t1 < ntiles) issue(&map_phi, t1, ybuf, full + 2);
+        }
     }
 }
 
