@@ -21,7 +21,7 @@ INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-         "-Xcompiler", "-fPIC,-O2", "-I", INCLUDE]
+         "-Xcompiler", "-fPIC,-O2", "-I", INCLUDE] + os.environ.get("TDH_NVCC_FLAGS", "").split()
 
 
 def _sources():

@@ -83,6 +83,7 @@ struct tdh_grid {
     int* d_rowmap;        // natural ky -> plane row of the work layout
     int* d_colmap;        // natural kz -> column of the work layout
     int ctas_fwd, ctas_inv, ctas_x[3];   // persistent grid sizes (SM count x resident CTAs)
+    size_t smem_inv_max;                 // dynamic shared memory tile_inv may use (tile buffers + staged dpi)
 
     int chunk_cap;        // states the workspace can hold
     int chunk;            // states pushed through the chain together
@@ -200,7 +201,9 @@ extern "C" int tdh_create_grid(const int n[3], const double len[3], const double
         CU(cudaGetDevice(&dev));
         CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
         const void* fs[5] = {g->tl.fwd, g->tl.inv, g->xl.fused, g->xl.fwd, g->xl.inv};
-        const size_t sm[5] = {g->tl.smem_fwd, g->tl.smem_inv, g->xl.smem, g->xl.smem, g->xl.smem};
+        // tile_inv may stage up to 16 KB of projection coefficients behind its tile buffers (launch_plane_inv)
+        g->smem_inv_max = std::min<size_t>(232448, g->tl.smem_inv + 16384);
+        const size_t sm[5] = {g->tl.smem_fwd, g->smem_inv_max, g->xl.smem, g->xl.smem, g->xl.smem};
         const int th[5] = {g->tl.threads, g->tl.threads, g->xl.threads, g->xl.threads, g->xl.threads};
         int ctas[5];
         for (int i = 0; i < 5; ++i) {
@@ -422,8 +425,9 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
             nl_off[(size_t)t * (nlayers + 1) + nlayers] = run;
         }
     }
+    const int cpad = tdh::nl_pad_cmax(cmax);               // channel count the record loop is compiled for
     std::vector<unsigned> rec_cc(ptot);
-    std::vector<double> rec_beta((size_t)cmax * ptot, 0.0);
+    std::vector<double> rec_beta((size_t)cpad * ptot, 0.0);
     std::vector<cd> rec_phase(g->have_k ? ptot : 0);
     {
         std::vector<int> cursor((size_t)ntiles * nlayers);
@@ -454,9 +458,9 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
         free_projectors(g);
         return rc;
     }
-    // dpi: [chunk_cap][ctot] plus cmax zeroed entries (records of atoms with fewer than cmax channels read past their
+    // dpi: [chunk_cap][ctot] plus cpad zeroed entries (records of atoms with fewer than cpad channels read past their
     // own channels with a zero projector value)
-    const size_t ndpi = (size_t)g->chunk_cap * ctot + cmax;
+    const size_t ndpi = (size_t)g->chunk_cap * ctot + cpad;
     cudaError_t e = cudaMalloc(&g->d_dpi, sizeof(cd) * ndpi);
     if (e == cudaSuccess) e = cudaMemset(g->d_dpi, 0, sizeof(cd) * ndpi);
     if (e != cudaSuccess) { free_projectors(g); return fail(TDH_ENOMEM, "tdh_set_projectors: %s", cudaGetErrorString(e)); }
@@ -464,7 +468,7 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
     g->nchan_tot = ctot;
     g->nl_layers = nlayers;
     g->nl_nrec = (int)ptot;
-    g->nl_cmax = cmax;
+    g->nl_cmax = cpad;
     g->mt = cmax <= 8 ? 1 : 2;
     return TDH_OK;
 }
@@ -563,12 +567,21 @@ static int launch_plane_inv(tdh_grid* g, int nst, const cd* in, const cd* phi, c
     int rc = tile_map(g, in, nst, &map_spec);
     if (rc) return rc;
     if ((rc = tile_map(g, phi ? phi : in, nst, &map_phi))) return rc;
+    CUtensorMap map_yv;
+    if ((rc = tile_map(g, ep.yv ? ep.yv : in, nst, &map_yv))) return rc;
     const cd* twy = g->d_tw[1];
     const cd* twz = g->d_tw[2];
     int ntiles = (int)((size_t)nst * g->n[0] * g->tl.s / g->tl.ppc);
-    void* args[] = {(void*)&map_spec, (void*)&map_phi, (void*)&out, (void*)&ntiles, (void*)&twy, (void*)&twz, (void*)&ep};
+    tdh::Epilogue epl = ep;
+    size_t smem = g->tl.smem_inv;
+    if (epl.nl_off != nullptr) {
+        // dpi of the current state is staged behind the tile buffers when it fits
+        const size_t extra = sizeof(cd) * (size_t)(epl.nchan_tot + epl.cmax);
+        if (smem + extra <= g->smem_inv_max) { epl.dpi_smem = 1; smem += extra; }
+    }
+    void* args[] = {(void*)&map_spec, (void*)&map_phi, (void*)&map_yv, (void*)&out, (void*)&ntiles, (void*)&twy, (void*)&twz, (void*)&epl};
     const unsigned grid = (unsigned)std::min(ntiles, g->ctas_inv);
-    LAUNCH(K_PLANE_INV, g->tl.inv, dim3(grid), dim3(g->tl.threads), g->tl.smem_inv, args);
+    LAUNCH(K_PLANE_INV, g->tl.inv, dim3(grid), dim3(g->tl.threads), smem, args);
     return TDH_OK;
 }
 

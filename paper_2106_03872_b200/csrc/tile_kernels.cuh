@@ -232,20 +232,65 @@ struct Epilogue {
     const cd* nl_phase;     // per record e^{+ik.d}; NULL at Gamma
     const cd* dpi;          // [state][nchan_tot] D * dV * <beta|phi>  (+ cmax zeroed entries of padding)
     int nrec;
-    int cmax;
+    int cmax;               // padded channel count of a record: 1, 4, 9 or 16 (nl_pad_cmax)
     int nchan_tot;
+    int dpi_smem;           // 1: the CTA stages dpi of the current state in shared memory behind the tile buffers
 };
+
+// channel counts the record loop is compiled for; the host pads nl_beta (zeros) and dpi (zeros) to this
+__host__ __device__ constexpr int nl_pad_cmax(int c) { return c <= 1 ? 1 : (c <= 4 ? 4 : (c <= 9 ? 9 : 16)); }
+
+// One layer of the back-projection of one plane part: records [i0, i1) add  e^{-ik.d} sum_c beta_c[i] * dpi[chan0 + c]
+// into cell (cc & 0xffff) of `base`.  U records per thread are in flight together: the loop is bound by the latency of
+// the record loads (L2), not by arithmetic.  dp points at dpi of this state (shared or global memory).
+template <int CM, int U>
+__device__ __forceinline__ void nl_scatter_layer(cd* base, const cd* dp, const unsigned* __restrict__ nl_cc,
+                                                 const double* __restrict__ nl_beta, const cd* __restrict__ nl_phase,
+                                                 size_t nrec, int i0, int i1, int tid, int nthreads)
+{
+    for (int ib = i0 + tid; ib < i1; ib += U * nthreads) {
+        unsigned cc[U];
+        double bv[U][CM];
+        cd ph[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int i = ib + u * nthreads;
+            const bool ok = i < i1;
+            cc[u] = ok ? __ldg(nl_cc + i) : 0u;
+#pragma unroll
+            for (int c = 0; c < CM; ++c) bv[u][c] = ok ? __ldg(nl_beta + (size_t)c * nrec + i) : 0.0;
+            if (nl_phase != nullptr) ph[u] = ok ? __ldg(nl_phase + i) : make_double2(1.0, 0.0);
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            if (ib + u * nthreads < i1) {
+                const cd* d = dp + (cc[u] >> 16);
+                cd sacc = make_double2(0.0, 0.0);
+#pragma unroll
+                for (int c = 0; c < CM; ++c) {
+                    const cd dv = d[c];
+                    sacc.x = fma(bv[u][c], dv.x, sacc.x);
+                    sacc.y = fma(bv[u][c], dv.y, sacc.y);
+                }
+                if (nl_phase != nullptr) sacc = cmulc(sacc, ph[u]);
+                cd* cell = base + (cc[u] & 0xffffu);
+                *cell = cadd(*cell, sacc);
+            }
+        }
+    }
+}
 
 // ------------------------------------------------------------------------------------------------------------
 // inverse + epilogue: `map_spec` describes the work block (digit-permuted spectrum), `map_phi` the input block of this
-// Hamiltonian application (same geometry), `out` the output block.  Shared memory: two spectrum buffers X0, X1 (tile
+// Hamiltonian application, `map_yv` the addend block ep.yv (both same geometry; map_yv is only used to prefetch the
+// addend tile into L2), `out` the output block.  Shared memory: two spectrum buffers X0, X1 (tile
 // i in X[i & 1], tile i+1 streaming into the other) and one buffer Y for phi of the current tile, which becomes
 // V*phi + V_nl phi when there are projectors.  Persistent grid; ntiles = nst * NX * S / PPC.
 // ------------------------------------------------------------------------------------------------------------
 template <int NY, int NZ>
 __global__ void __launch_bounds__(TileCfg<NY, NZ>::T, 1)
 tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_constant__ CUtensorMap map_phi,
-                cd* __restrict__ out, int ntiles, const cd* __restrict__ tw_y, const cd* __restrict__ tw_z,
+                const __grid_constant__ CUtensorMap map_yv, cd* __restrict__ out, int ntiles, const cd* __restrict__ tw_y, const cd* __restrict__ tw_z,
                 const Epilogue ep)
 {
     using C = TileCfg<NY, NZ>;
@@ -254,6 +299,7 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);             // [0], [1]: X buffers; [2]: Y
     cd* xbuf = reinterpret_cast<cd*>(smem_raw + TILE_HEADER);
     cd* ybuf = xbuf + 2 * (size_t)C::CELLS;
+    cd* sdpi = ybuf + (size_t)C::CELLS;                                   // [nchan_tot + cmax], only with ep.dpi_smem
     const int tid = threadIdx.x;
     const bool have_nl = ep.nl_off != nullptr;
     const bool have_phi = have_nl || ep.v != nullptr;
@@ -272,28 +318,39 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
         mbar_arrive_expect_tx(bar, (uint32_t)C::TILE_BYTES);
         tma_load_4d(dst, map, bar, 0, r * R1Z, 0, plane, pol);
     };
+    // this CTA's tiles: the contiguous range [t_begin, t_end) -- consecutive x of one state, so that the state (and its
+    // dpi in shared memory) changes once per NX*S/PPC tiles
+#ifdef TDH_INV_CONTIG
+    const int t_begin = (int)((long long)ntiles * blockIdx.x / gridDim.x);
+    const int t_end = (int)((long long)ntiles * (blockIdx.x + 1) / gridDim.x);
+    constexpr int t_step_c = 1; const int t_step = t_step_c;
+#else
+    const int t_begin = blockIdx.x, t_end = ntiles, t_step = gridDim.x;
+#endif
     if (tid == 0) {
-        const int t0 = blockIdx.x, t1 = blockIdx.x + gridDim.x;
-        if (t0 < ntiles) {
-            issue(&map_spec, t0, xbuf, full + 0);
-            if (have_phi) issue(&map_phi, t0, ybuf, full + 2);
+        if (t_begin < t_end) {
+            issue(&map_spec, t_begin, xbuf, full + 0);
+            if (have_phi) issue(&map_phi, t_begin, ybuf, full + 2);
         }
-        if (t1 < ntiles) issue(&map_spec, t1, xbuf + C::CELLS, full + 1);
+        if (t_begin + t_step < t_end) issue(&map_spec, t_begin + t_step, xbuf + C::CELLS, full + 1);
     }
-
-    // last z stage twiddles of this thread's column j2 = tid & 7: w_NZ^(-k1*j2)
-    cd twz[R1Z];
-    {
-        const int j2 = tid & 7;
-#pragma unroll
-        for (int k1 = 1; k1 < R1Z; ++k1) twz[k1] = ldg_cd(tw_z + k1 * j2);
-    }
+    int st_smem = -1;                                                     // state whose dpi is in sdpi
 
     int it = 0;
-    for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++it) {
+    for (int t = t_begin; t < t_end; t += t_step, ++it) {
         const int cur = it & 1;
         cd* sm = xbuf + (size_t)cur * C::CELLS;
         const int part0 = t * C::PPC;
+        const int st = (part0 / S) / ep.nx;                               // PPC divides NX: one state per tile
+        if (have_nl && ep.dpi_smem && st != st_smem) {
+            // read by the record loop below, after at least one barrier; the previous tile ended with a barrier
+            const cd* src = ep.dpi + (size_t)st * ep.nchan_tot;
+            for (int i = tid; i < ep.nchan_tot + ep.cmax; i += T)
+                sdpi[i] = i < ep.nchan_tot ? ldg_cd(src + i) : make_double2(0.0, 0.0);
+            st_smem = st;
+        }
+        // the addend tile is read straight from global memory by the epilogue: start it towards L2 now
+        if (tid == 0 && ep.yv != nullptr) tma_prefetch_l2_4d(&map_yv, 0, (part0 % S) * R1Z, 0, part0 / S);
         mbar_wait(full + cur, (uint32_t)(it >> 1) & 1u);
 
         // ---- y stage A', in place: rows k1y*R2Y + k2y (contiguous) hold k = k1y + R1Y*k2y; radix R2Y over k2y -> j2,
@@ -353,29 +410,20 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
                 }
             }
             __syncthreads();
+            const cd* dp = ep.dpi_smem ? sdpi : ep.dpi + (size_t)st * ep.nchan_tot;
             for (int layer = 0; layer < ep.nl_layers; ++layer) {
 #pragma unroll
                 for (int lp = 0; lp < C::PPC; ++lp) {
                     const int part = part0 + lp, plane = part / S, r = part % S;
-                    const int st = plane / ep.nx, x = plane % ep.nx;
+                    const int x = plane % ep.nx;
                     const int* off = ep.nl_off + (size_t)(x * S + r) * (ep.nl_layers + 1) + layer;
-                    const int i1 = __ldg(off + 1);
-                    const cd* dp = ep.dpi + (size_t)st * ep.nchan_tot;
+                    const int i0 = __ldg(off), i1 = __ldg(off + 1);
                     cd* base = ybuf + lp * C::PART;
-                    for (int i = __ldg(off) + tid; i < i1; i += T) {
-                        const unsigned cc = __ldg(ep.nl_cc + i);
-                        const cd* d = dp + (cc >> 16);
-                        const double* bq = ep.nl_beta + i;
-                        cd sacc = make_double2(0.0, 0.0);
-                        for (int c = 0; c < ep.cmax; ++c) {
-                            const double bv = __ldg(bq + (size_t)c * ep.nrec);
-                            const cd dv = ldg_cd(d + c);
-                            sacc.x = fma(bv, dv.x, sacc.x);
-                            sacc.y = fma(bv, dv.y, sacc.y);
-                        }
-                        if (ep.nl_phase != nullptr) sacc = cmulc(sacc, ldg_cd(ep.nl_phase + i));
-                        cd* cell = base + (cc & 0xffffu);
-                        *cell = cadd(*cell, sacc);
+                    switch (ep.cmax) {
+                        case 1: nl_scatter_layer<1, 4>(base, dp, ep.nl_cc, ep.nl_beta, ep.nl_phase, ep.nrec, i0, i1, tid, T); break;
+                        case 4: nl_scatter_layer<4, 4>(base, dp, ep.nl_cc, ep.nl_beta, ep.nl_phase, ep.nrec, i0, i1, tid, T); break;
+                        case 9: nl_scatter_layer<9, 2>(base, dp, ep.nl_cc, ep.nl_beta, ep.nl_phase, ep.nrec, i0, i1, tid, T); break;
+                        default: nl_scatter_layer<16, 1>(base, dp, ep.nl_cc, ep.nl_beta, ep.nl_phase, ep.nrec, i0, i1, tid, T); break;
                     }
                 }
                 __syncthreads();
@@ -390,15 +438,15 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
             const int j2 = tid & 7;
             for (int lr = tid >> 3; lr < C::ROWS; lr += T / 8) {
                 const int l0 = lr * R1Z;
-                cd x[R1Z];
-                x[0] = sm[swz(l0, j2)];
-#pragma unroll
-                for (int k1 = 1; k1 < R1Z; ++k1) x[k1] = cmul(sm[swz(l0 + k1, j2)], twz[k1]);
-                Dft<R1Z, +1>::run(x);
                 const int lp = lr / NYS, m = lr % NYS;
                 const int part = part0 + lp, plane = part / S, r = part % S;
                 const int y = S * m + r;
                 const size_t gi = (size_t)plane * NY * NZ + (size_t)y * NZ + j2;               // index in the block
+                cd x[R1Z];
+                x[0] = sm[swz(l0, j2)];
+#pragma unroll
+                for (int k1 = 1; k1 < R1Z; ++k1) x[k1] = cmul(sm[swz(l0 + k1, j2)], ldg_cd(tw_z + k1 * j2));   // w_NZ^(-k1*j2)
+                Dft<R1Z, +1>::run(x);
                 if (have_nl) {
 #pragma unroll
                     for (int j1 = 0; j1 < R1Z; ++j1) x[j1] = cadd(x[j1], ybuf[swz(l0 + j1, j2)]);
@@ -413,8 +461,13 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
                     }
                 }
                 if (ep.yv != nullptr) {
+                    // all loads of the addend before the first store: out may alias yv, so the compiler cannot reorder
+                    // them itself.  The tile of yv was prefetched into L2 when this tile's turn began.
+                    cd ya[R1Z];
 #pragma unroll
-                    for (int j1 = 0; j1 < R1Z; ++j1) sts_cd(out + gi + 8 * j1, cadd(cmul(ep.alpha, x[j1]), lds_cd(ep.yv + gi + 8 * j1)));
+                    for (int j1 = 0; j1 < R1Z; ++j1) ya[j1] = lds_cd(ep.yv + gi + 8 * j1);
+#pragma unroll
+                    for (int j1 = 0; j1 < R1Z; ++j1) sts_cd(out + gi + 8 * j1, cadd(cmul(ep.alpha, x[j1]), ya[j1]));
                 } else {
 #pragma unroll
                     for (int j1 = 0; j1 < R1Z; ++j1) sts_cd(out + gi + 8 * j1, cmul(ep.alpha, x[j1]));
@@ -425,9 +478,8 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
         fence_proxy_async();
         __syncthreads();
         if (tid == 0) {
-            const int t1 = t + gridDim.x, t2 = t + 2 * gridDim.x;
-            if (t2 < ntiles) issue(&map_spec, t2, sm, full + cur);
-            if (have_phi && t1 < ntiles) issue(&map_phi, t1, ybuf, full + 2);
+            if (t + 2 * t_step < t_end) issue(&map_spec, t + 2 * t_step, sm, full + cur);
+            if (have_phi && t + t_step < t_end) issue(&map_phi, t + t_step, ybuf, full + 2);
         }
     }
 }

@@ -15,6 +15,12 @@
 // walks tiles blockIdx.x, blockIdx.x + gridDim.x, ... through a ring of NB buffers that one elected thread keeps
 // filled with cp.async.bulk.tensor, so the loads of the next tiles are in flight while this one is transformed.
 //
+// THREADS.  NX = R1*R2 (R1 >= R2).  A CTA has TPL threads per line (TPL >= R2): the R2 radix-R1 transforms of a line
+// (first forward stage, last inverse stage) take one round, the R1 radix-R2 transforms in between take
+// ceil(R1/TPL) rounds.  The kernel is compiled for CPS resident CTAs per SM (<= 128 registers per thread): the
+// barrier-separated stages of one CTA alternate between shared-memory, FP64 and store phases, and the second CTA
+// fills the gaps.  Twiddles and (G_x+k_x)^2 sit in shared memory behind the ring.
+//
 // S = 2 (see tile_kernels.cuh): the tile kernels leave/expect half-length y transforms E_r[k] / F_r[k], r = 0, 1, at
 // rows Y = 2*rho + r -- lanes l and l ^ 16 of a warp.  The missing radix-2 step of the y transform commutes with the x
 // transform.  With A_h = FFT_x(E_h), w = e^{-2 pi i k / NY} and f_h the kinetic factor of ky = k + h NY/2:
@@ -47,28 +53,44 @@ __device__ __forceinline__ cd shfl16(cd v) {
 
 template <int NX> struct XCfg {
     static constexpr int R1 = Fact<NX>::R1, R2 = Fact<NX>::R2;
-    static constexpr int T = XP_LPC * R1;
+    static constexpr int TPL = NX >= 48 ? 8 : 4;                    // threads per line
+    static constexpr int T = XP_LPC * TPL;
+    static constexpr int CPS = NX >= 48 ? 2 : 4;                    // resident CTAs per SM the kernel is built for
+    static constexpr int ROUNDS_B = (R1 + TPL - 1) / TPL;           // rounds of the radix-R2 stage
     static constexpr int TILE_CELLS = NX * XP_LPC;
     static constexpr size_t TILE_BYTES = (size_t)TILE_CELLS * sizeof(cd);
-    // ring depth: as many tiles as fit beside the barriers, at most 4
-    static constexpr int NB = (int)((232448 - 1024) / TILE_BYTES) < 4 ? (int)((232448 - 1024) / TILE_BYTES) : 4;
-    static constexpr size_t SMEM = NB * TILE_BYTES + 1024;
+    static constexpr size_t TABLE_BYTES = (size_t)NX * (sizeof(cd) + sizeof(double));
+    // ring depth: what fits in 1/CPS of the SM's 228 KB beside the barriers, the tables and the 1 KB the system
+    // reserves per CTA; between 2 and 4 tiles
+    static constexpr int fit() { return (int)((233472 / CPS - 2048 - TABLE_BYTES) / TILE_BYTES); }
+    static constexpr int NB = fit() < 2 ? 2 : (fit() > 4 ? 4 : fit());
+    static constexpr size_t SMEM = 1024 + NB * TILE_BYTES + TABLE_BYTES;
+    static_assert(R2 <= TPL, "the radix-R1 stages must fit one round");
 };
+
+// the kinetic factor t = 0.5*((gx^2 + gy^2) + gz^2) in the oracle's operation order (no contraction), masked, times
+// the 1/N_p of the inverse transform
+__device__ __forceinline__ double kin_factor(double gx2, double gy2, double gz2, double ecut, double scale) {
+    const double tk = __dmul_rn(0.5, __dadd_rn(__dadd_rn(gx2, gy2), gz2));
+    return (ecut > 0.0 && !(tk <= ecut)) ? 0.0 : tk * scale;
+}
 
 // grid: persistent CTAs; ntiles = nst * (NY/2) * (NZ/16).  in (through `map`) and out may be the same buffer: a tile
 // is read completely before any of its lines is written.
 template <int NX, int S, int MODE>
-__global__ void __launch_bounds__(XCfg<NX>::T, 1)
+__global__ void __launch_bounds__(XCfg<NX>::T, XCfg<NX>::CPS)
 xpencil_kernel(const __grid_constant__ CUtensorMap map, cd* __restrict__ out, int ntiles,
                const cd* __restrict__ tw_x, const Kinetic kin)
 {
     using C = XCfg<NX>;
-    constexpr int R1 = C::R1, R2 = C::R2, L = XP_LPC, NB = C::NB;
+    constexpr int R1 = C::R1, R2 = C::R2, L = XP_LPC, NB = C::NB, TPL = C::TPL, RB = C::ROUNDS_B;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);            // NB barriers in the first 1024 bytes
     cd* ring = reinterpret_cast<cd*>(smem_raw + 1024);
+    cd* stw = ring + (size_t)NB * C::TILE_CELLS;                        // e^{+2 pi i m / NX}
+    double* sg2x = reinterpret_cast<double*>(stw + NX);                 // (G_x + k_x)^2
     const int tid = threadIdx.x;
-    const int l = tid % L, hi = tid / L;               // hi < R1
+    const int l = tid % L, hi = tid / L;               // hi < TPL, warp-uniform
     const int half = l >> 4;
     const int zc = kin.nz >> 4;                         // 16-column chunks per plane row
     const int tiles_per_state = (kin.ny >> 1) * zc;
@@ -80,6 +102,10 @@ xpencil_kernel(const __grid_constant__ CUtensorMap map, cd* __restrict__ out, in
         pol = policy_evict_first();
         for (int b = 0; b < NB; ++b) mbar_init(full + b, 1);
         mbar_fence_init();
+    }
+    for (int i = tid; i < NX; i += C::T) {
+        stw[i] = __ldg(tw_x + i);
+        sg2x[i] = (MODE == 0) ? __ldg(kin.g2x + i) : 0.0;
     }
     __syncthreads();
     auto issue = [&](int t, int b) {                    // thread 0 only
@@ -94,11 +120,6 @@ xpencil_kernel(const __grid_constant__ CUtensorMap map, cd* __restrict__ out, in
             if (t < ntiles) issue(t, b);
         }
 
-    // per-thread constants: x-direction twiddles and (G_x + k_x)^2 of the spectrum rows this thread owns
-    double gx2[R2];
-#pragma unroll
-    for (int k2 = 0; k2 < R2; ++k2) gx2[k2] = (MODE == 0) ? __ldg(kin.g2x + hi + R1 * k2) : 0.0;
-
     int it = 0;
     for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++it) {
         const int b = it % NB;
@@ -108,11 +129,19 @@ xpencil_kernel(const __grid_constant__ CUtensorMap map, cd* __restrict__ out, in
         const int rho2 = rem / zc, ch = rem % zc;
         const int Y = 2 * rho2 + half, zp = ch * 16 + (l & 15);
         cd* gcol = out + (size_t)st * NX * nynz + (size_t)Y * kin.nz + zp;   // element x at gcol + x * nynz
+        // per-line constants of this tile (in flight while the tile arrives)
+        double gy2a = 0.0, gy2b = 0.0, gz2 = 0.0;
+        cd w = make_double2(1.0, 0.0);
+        if (MODE == 0) {
+            gz2 = __ldg(kin.g2z_w + zp);
+            gy2a = __ldg(kin.g2y_w + (S == 2 ? 2 * rho2 : Y));
+            if (S == 2) gy2b = __ldg(kin.g2y_w + 2 * rho2 + 1);
+        }
+        if (S == 2) w = __ldg(kin.twy_w + rho2);                 // e^{+2 pi i k / NY} = conj(w of the header comment)
         mbar_wait(full + b, parity);
 
-        cd xr[R2];                                                 // stage-B registers: X[hi + R1*k2]
         if (MODE != 2) {
-            // ---- forward stage A (threads with hi < R2): radix R1 over x = j1*R2 + j2, j2 = hi, in place
+            // ---- forward stage A: radix R1 over x = j1*R2 + j2, one transform per thread with hi = j2 < R2, in place
             if (hi < R2) {
                 const int j2 = hi;
                 cd x[R1];
@@ -121,102 +150,117 @@ xpencil_kernel(const __grid_constant__ CUtensorMap map, cd* __restrict__ out, in
                 Dft<R1, -1>::run(x);
                 sm[j2 * L + l] = x[0];
 #pragma unroll
-                for (int k1 = 1; k1 < R1; ++k1) sm[(k1 * R2 + j2) * L + l] = cmulc(x[k1], __ldg(tw_x + k1 * j2));
+                for (int k1 = 1; k1 < R1; ++k1) sm[(k1 * R2 + j2) * L + l] = cmulc(x[k1], stw[k1 * j2]);
             }
             __syncthreads();
-            // ---- forward stage B: thread (l, k1 = hi) -> X[k1 + R1*k2]
-#pragma unroll
-            for (int j2 = 0; j2 < R2; ++j2) xr[j2] = sm[(hi * R2 + j2) * L + l];
-            Dft<R2, -1>::run(xr);
-        } else {
-#pragma unroll
-            for (int k2 = 0; k2 < R2; ++k2) xr[k2] = sm[(hi + R1 * k2) * L + l];
         }
 
-        // ---- kinetic factor t = 0.5*((gx^2 + gy^2) + gz^2) in the oracle's operation order, no contraction;
-        //      with S = 2 also the radix-2 step of the y transform (header comment)
-        if (S == 1) {
-            if (MODE == 0) {
-                const double gy2 = __ldg(kin.g2y_w + Y), gz2 = __ldg(kin.g2z_w + zp);
+        if (MODE == 2) {
+            // ---- inverse only: X[k1 + R1*k2] sits in slot k1 + R1*k2; every thread reads all its inputs, then the
+            //      intermediate values go to slots k1*R2 + n2 (other threads' inputs: barrier in between)
+            cd xr[RB][R2];
 #pragma unroll
-                for (int k2 = 0; k2 < R2; ++k2) {
-                    const double tk = __dmul_rn(0.5, __dadd_rn(__dadd_rn(gx2[k2], gy2), gz2));
-                    const double f = (kin.ecut > 0.0 && !(tk <= kin.ecut)) ? 0.0 : tk * kin.scale;
-                    xr[k2] = cscale(xr[k2], f);
+            for (int rd = 0; rd < RB; ++rd) {
+                const int k1 = hi + rd * TPL;
+                if (k1 < R1) {
+#pragma unroll
+                    for (int k2 = 0; k2 < R2; ++k2) xr[rd][k2] = sm[(k1 + R1 * k2) * L + l];
                 }
-            } else if (MODE == 2) {
+            }
+            __syncthreads();
 #pragma unroll
-                for (int k2 = 0; k2 < R2; ++k2) xr[k2] = cscale(xr[k2], kin.scale);
+            for (int rd = 0; rd < RB; ++rd) {
+                const int k1 = hi + rd * TPL;
+                if (k1 < R1) {
+#pragma unroll
+                    for (int k2 = 0; k2 < R2; ++k2) {
+                        if (S == 2) {
+                            // F_0 = X_0 + X_1,  F_1 = conj(w) (X_0 - X_1), conj(w) = twy_w[rho]; then the 1/N_p
+                            const cd other = shfl16(xr[rd][k2]);
+                            const cd v = half ? cmul(w, csub(other, xr[rd][k2])) : cadd(xr[rd][k2], other);
+                            xr[rd][k2] = cscale(v, kin.scale);
+                        } else {
+                            xr[rd][k2] = cscale(xr[rd][k2], kin.scale);
+                        }
+                    }
+                    Dft<R2, +1>::run(xr[rd]);
+                    sm[(k1 * R2) * L + l] = xr[rd][0];
+#pragma unroll
+                    for (int n2 = 1; n2 < R2; ++n2) sm[(k1 * R2 + n2) * L + l] = cmul(xr[rd][n2], stw[n2 * k1]);
+                }
             }
         } else {
-            const cd w = __ldg(kin.twy_w + rho2);            // e^{+2 pi i k / NY} = conj(w of the header comment)
-            if (MODE == 0) {
-                const double gy2a = __ldg(kin.g2y_w + 2 * rho2), gy2b = __ldg(kin.g2y_w + 2 * rho2 + 1);
-                const double gz2 = __ldg(kin.g2z_w + zp);
-                const cd wh = half ? w : make_double2(w.x, -w.y);
+            // ---- forward stage B: the transform of slots k1*R2 + j2 gives X[k1 + R1*k2]; MODE 0 continues in registers
+            //      with the kinetic factor and the first inverse stage, whose output n2 goes back to slot k1*R2 + n2 --
+            //      a slot this thread read itself, so no barrier is needed inside the stage
 #pragma unroll
-                for (int k2 = 0; k2 < R2; ++k2) {
-                    const double ta = __dmul_rn(0.5, __dadd_rn(__dadd_rn(gx2[k2], gy2a), gz2));
-                    const double tb = __dmul_rn(0.5, __dadd_rn(__dadd_rn(gx2[k2], gy2b), gz2));
-                    const double fa = (kin.ecut > 0.0 && !(ta <= kin.ecut)) ? 0.0 : ta * kin.scale;
-                    const double fb = (kin.ecut > 0.0 && !(tb <= kin.ecut)) ? 0.0 : tb * kin.scale;
-                    const cd other = shfl16(xr[k2]);
-                    const cd wo = cmul(wh, other);
-                    const double fs = fa + fb, fd = fa - fb;
-                    xr[k2] = make_double2(fma(fs, xr[k2].x, fd * wo.x), fma(fs, xr[k2].y, fd * wo.y));
-                }
-            } else if (MODE == 1) {
-                // X_0 = A_0 + w A_1 (lane of half 0), X_1 = A_0 - w A_1 (lane of half 1), w = conj(twy_w[rho])
+            for (int rd = 0; rd < RB; ++rd) {
+                const int k1 = hi + rd * TPL;
+                if (k1 < R1) {                                             // warp-uniform
+                    cd xr[R2];
 #pragma unroll
-                for (int k2 = 0; k2 < R2; ++k2) {
-                    const cd mine = half ? cmulc(xr[k2], w) : xr[k2];      // half 1 sends w A_1, half 0 sends A_0
-                    const cd other = shfl16(mine);
-                    xr[k2] = half ? csub(other, mine) : cadd(mine, other);
-                }
-            } else {
-                // F_0 = X_0 + X_1,  F_1 = conj(w) (X_0 - X_1), conj(w) = twy_w[rho]; then the 1/N_p
+                    for (int j2 = 0; j2 < R2; ++j2) xr[j2] = sm[(k1 * R2 + j2) * L + l];
+                    Dft<R2, -1>::run(xr);
+                    if (MODE == 0) {
 #pragma unroll
-                for (int k2 = 0; k2 < R2; ++k2) {
-                    const cd other = shfl16(xr[k2]);
-                    const cd v = half ? cmul(w, csub(other, xr[k2])) : cadd(xr[k2], other);
-                    xr[k2] = cscale(v, kin.scale);
+                        for (int k2 = 0; k2 < R2; ++k2) {
+                            const double gx2 = sg2x[k1 + R1 * k2];
+                            if (S == 1) {
+                                xr[k2] = cscale(xr[k2], kin_factor(gx2, gy2a, gz2, kin.ecut, kin.scale));
+                            } else {
+                                // the radix-2 step of the y transform folded into the factor (header comment)
+                                const double fa = kin_factor(gx2, gy2a, gz2, kin.ecut, kin.scale);
+                                const double fb = kin_factor(gx2, gy2b, gz2, kin.ecut, kin.scale);
+                                const cd wh = half ? w : make_double2(w.x, -w.y);
+                                const cd other = shfl16(xr[k2]);
+                                const cd wo = cmul(wh, other);
+                                const double fs = fa + fb, fd = fa - fb;
+                                xr[k2] = make_double2(fma(fs, xr[k2].x, fd * wo.x), fma(fs, xr[k2].y, fd * wo.y));
+                            }
+                        }
+                        Dft<R2, +1>::run(xr);
+                        sm[(k1 * R2) * L + l] = xr[0];
+#pragma unroll
+                        for (int n2 = 1; n2 < R2; ++n2) sm[(k1 * R2 + n2) * L + l] = cmul(xr[n2], stw[n2 * k1]);
+                    } else {
+                        if (S == 2) {
+                            // X_0 = A_0 + w A_1 (lane of half 0), X_1 = A_0 - w A_1 (lane of half 1), w = conj(twy_w[rho])
+#pragma unroll
+                            for (int k2 = 0; k2 < R2; ++k2) {
+                                const cd mine = half ? cmulc(xr[k2], w) : xr[k2];  // half 1 sends w A_1, half 0 sends A_0
+                                const cd other = shfl16(mine);
+                                xr[k2] = half ? csub(other, mine) : cadd(mine, other);
+                            }
+                        }
+#pragma unroll
+                        for (int k2 = 0; k2 < R2; ++k2) __stcs(gcol + (size_t)(k1 + R1 * k2) * nynz, xr[k2]);
+                    }
                 }
             }
         }
 
         if (MODE == 1) {
-            // all reads of the buffer are done: hand it back to the TMA, then store from registers
+            // all reads of the buffer are done: hand it back to the TMA
             fence_proxy_async();
             __syncthreads();
             if (tid == 0 && t + NB * (int)gridDim.x < ntiles) issue(t + NB * gridDim.x, b);
-#pragma unroll
-            for (int k2 = 0; k2 < R2; ++k2) __stcs(gcol + (size_t)(hi + R1 * k2) * nynz, xr[k2]);
             continue;
         }
 
-        // ---- inverse with the mirrored factorisation (first radix R2 on stride R1): the registers of stage B are
-        //      exactly the inputs of its first stage, n = k2*R1 + hi.  Intermediate value k1 of thread hi goes to slot
-        //      hi*R2 + k1 -- one of the slots this thread itself read in stage B, so no barrier is needed before it.
-        Dft<R2, +1>::run(xr);
-        if (MODE == 2) __syncthreads();   // MODE 2 read slots hi + R1*k2: other threads' slots
-        sm[(hi * R2) * L + l] = xr[0];
-#pragma unroll
-        for (int k1 = 1; k1 < R2; ++k1) sm[(hi * R2 + k1) * L + l] = cmul(xr[k1], __ldg(tw_x + k1 * hi));
+        // ---- last inverse stage: thread hi = n2 < R2 transforms slots k1*R2 + n2 over k1 -> x = n2 + R2*n1
         __syncthreads();
         cd x[R1];
         if (hi < R2) {
-            const int k1 = hi;
 #pragma unroll
-            for (int j2 = 0; j2 < R1; ++j2) x[j2] = sm[(j2 * R2 + k1) * L + l];
+            for (int k1 = 0; k1 < R1; ++k1) x[k1] = sm[(k1 * R2 + hi) * L + l];
         }
         fence_proxy_async();
         __syncthreads();                  // every read of this buffer is done: refill it
         if (tid == 0 && t + NB * (int)gridDim.x < ntiles) issue(t + NB * gridDim.x, b);
         if (hi < R2) {
-            const int k1 = hi;
             Dft<R1, +1>::run(x);
 #pragma unroll
-            for (int k2 = 0; k2 < R1; ++k2) __stcs(gcol + (size_t)(k1 + R2 * k2) * nynz, x[k2]);
+            for (int n1 = 0; n1 < R1; ++n1) __stcs(gcol + (size_t)(hi + R2 * n1) * nynz, x[n1]);
         }
     }
 }
