@@ -44,7 +44,9 @@ template <> struct FactY<96> { static constexpr int R1 = 12, R2 = 8; };
 
 constexpr int tile_round_up(int a, int b) { return (a + b - 1) / b * b; }
 constexpr int TILE_MAX_CELLS = 4608;
-constexpr int TILE_HEADER = 1024;      // barriers; keeps the buffers 1024-byte aligned
+constexpr int TILE_HEADER = 1024;      // tile_inv: barriers; keeps the buffers 1024-byte aligned
+constexpr int TILE_HEADER_FWD = 4096;  // tile_fwd: barriers (64 bytes), then the z and y twiddle tables
+constexpr int TILE_TW_OFF = 64;
 
 template <int NY, int NZ> struct TileCfg {
     static constexpr int S = (NY * NZ >= 6144) ? 2 : 1;            // y-split (96x96, 96x64, 64x96)
@@ -63,7 +65,7 @@ template <int NY, int NZ> struct TileCfg {
     static constexpr int CELLS = ROWS * NZ;
     static constexpr size_t TILE_BYTES = (size_t)CELLS * sizeof(cd);
     static constexpr int NB_FWD = 3;                                // ring depth of tile_fwd
-    static constexpr size_t SMEM_FWD = TILE_HEADER + NB_FWD * TILE_BYTES;
+    static constexpr size_t SMEM_FWD = TILE_HEADER_FWD + NB_FWD * TILE_BYTES;
     static constexpr size_t SMEM_INV = TILE_HEADER + 3 * TILE_BYTES;   // two spectrum buffers + one phi buffer
     // work items of the four stages
     static constexpr int I_ZA = ROWS * 8, I_ZB = ROWS * R1Z, I_YA = PPC * NZ * R2Y, I_YB = PPC * NZ * R1Y;
@@ -85,14 +87,26 @@ template <int NY, int NZ> struct TileCfg {
     static_assert(NZ % 16 == 0 && T % 8 == 0, "z stage mapping");
     static_assert(PART % 64 == 0, "plane parts must keep the 1024-byte swizzle phase");
     static_assert(CELLS <= TILE_MAX_CELLS, "tile too large");
+    static_assert(TILE_TW_OFF + (NY + NZ) * sizeof(cd) <= TILE_HEADER_FWD, "twiddle tables must fit in the header");
 };
 
 // cell (in complex values) of position p of 128-byte line ln in a swizzled tile buffer
 __device__ __forceinline__ int swz(int ln, int p) { return 8 * ln + (p ^ (ln & 7)); }
 
+// named barrier of one warp group (ids 1, 2; id 0 is __syncthreads)
+template <int NTHREADS>
+__device__ __forceinline__ void group_sync(int grp) {
+    asm volatile("bar.sync %0, %1;" ::"r"(grp + 1), "n"(NTHREADS) : "memory");
+}
+
 // ------------------------------------------------------------------------------------------------------------
 // forward: `map_in` describes the input block, `out` is the work block (same geometry, digit-permuted spectrum).
 // Persistent grid; ntiles = nst * NX * S / PPC.
+//
+// WARP GROUPS.  The CTA is two independent groups of TG = T/2 threads that share the ring of NB = 3 tile buffers: the
+// CTA's k-th tile (tile blockIdx.x + k*gridDim.x) lives in buffer k % 3 and is transformed by group k % 2, whose thread 0
+// refills the buffer with tile k + 3 when the group is done with it.  The groups only meet at the mbarriers of the
+// ring, so while one group sits in a shared-memory-bound or store-bound stage the other one keeps the FP64 pipe busy.
 // ------------------------------------------------------------------------------------------------------------
 template <int NY, int NZ>
 __global__ void __launch_bounds__(TileCfg<NY, NZ>::T, 1)
@@ -101,49 +115,47 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap map_in, cd* __restrict__ out
 {
     using C = TileCfg<NY, NZ>;
     constexpr int S = C::S, NYS = C::NYS, R1Z = C::R1Z, R1Y = C::R1Y, R2Y = C::R2Y, T = C::T, NB = C::NB_FWD;
+    constexpr int TG = T / 2;
+    static_assert(NB == 3 && TG % 32 == 0, "ring of three buffers shared by two warp groups");
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);
-    cd* ring = reinterpret_cast<cd*>(smem_raw + TILE_HEADER);
-    const int tid = threadIdx.x;
+    cd* stw_z = reinterpret_cast<cd*>(smem_raw + TILE_TW_OFF);          // e^{+2 pi i m / NZ}
+    cd* stw_y = stw_z + NZ;                                             // e^{+2 pi i m / NY}
+    cd* ring = reinterpret_cast<cd*>(smem_raw + TILE_HEADER_FWD);
+    const int grp = threadIdx.x / TG, tid = threadIdx.x % TG;           // tid: index inside the group
 
-    uint64_t pol = 0;
-    if (tid == 0) {
+    uint64_t pol = policy_evict_first();
+    if (threadIdx.x == 0) {
         tma_prefetch_desc(&map_in);
-        pol = policy_evict_first();
         for (int b = 0; b < NB; ++b) mbar_init(full + b, 1);
         mbar_fence_init();
     }
+    for (int i = threadIdx.x; i < NZ; i += T) stw_z[i] = ldg_cd(tw_z + i);
+    for (int i = threadIdx.x; i < NY; i += T) stw_y[i] = ldg_cd(tw_y + i);
     __syncthreads();
-    auto issue = [&](int t, int b) {                    // thread 0 only
+    auto issue = [&](int k) {                            // one thread; tile k of this CTA into buffer k % NB
+        const int t = blockIdx.x + k * gridDim.x;
+        if (t >= ntiles) return;
+        const int b = k % NB;
         const int part0 = t * C::PPC, plane = part0 / S, r = part0 % S;
         mbar_arrive_expect_tx(full + b, (uint32_t)C::TILE_BYTES);
         tma_load_4d(ring + (size_t)b * C::CELLS, &map_in, full + b, 0, r * R1Z, 0, plane, pol);
     };
-    if (tid == 0)
-        for (int b = 0; b < NB; ++b) {
-            const int t = blockIdx.x + b * gridDim.x;
-            if (t < ntiles) issue(t, b);
-        }
+    if (threadIdx.x == 0)
+        for (int k = 0; k < NB; ++k) issue(k);
 
-    // z stage A twiddles of this thread's column j2 = tid & 7: w_NZ^(k1*j2)
-    cd twz[R1Z];
-    {
-        const int j2 = tid & 7;
-#pragma unroll
-        for (int k1 = 1; k1 < R1Z; ++k1) twz[k1] = ldg_cd(tw_z + k1 * j2);
-    }
-
-    int it = 0;
-    for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++it) {
-        const int b = it % NB;
+    for (int k = grp;; k += 2) {
+        const int t = blockIdx.x + k * gridDim.x;
+        if (t >= ntiles) break;
+        const int b = k % NB;
         cd* sm = ring + (size_t)b * C::CELLS;
         const int part0 = t * C::PPC;
-        mbar_wait(full + b, (uint32_t)(it / NB) & 1u);
+        mbar_wait(full + b, (uint32_t)(k / NB) & 1u);
 
         // ---- z stage A, in place: radix R1Z over j1 (lines lr*R1Z + j1, position j2), twiddle w^(k1*j2)
         {
             const int j2 = tid & 7;
-            for (int lr = tid >> 3; lr < C::ROWS; lr += T / 8) {
+            for (int lr = tid >> 3; lr < C::ROWS; lr += TG / 8) {
                 const int l0 = lr * R1Z;
                 cd x[R1Z];
 #pragma unroll
@@ -151,12 +163,12 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap map_in, cd* __restrict__ out
                 Dft<R1Z, -1>::run(x);
                 sm[swz(l0, j2)] = x[0];
 #pragma unroll
-                for (int k1 = 1; k1 < R1Z; ++k1) sm[swz(l0 + k1, j2)] = cmulc(x[k1], twz[k1]);
+                for (int k1 = 1; k1 < R1Z; ++k1) sm[swz(l0 + k1, j2)] = cmulc(x[k1], stw_z[k1 * j2]);
             }
         }
-        __syncthreads();
+        group_sync<TG>(grp);
         // ---- z stage B, in place inside line g: position k2 then holds kz = k1 + R1Z*k2
-        for (int g = tid; g < C::I_ZB; g += T) {
+        for (int g = tid; g < C::I_ZB; g += TG) {
             cd* p = sm + 8 * g;
             const int s = g & 7;
             cd v[8];
@@ -166,9 +178,9 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap map_in, cd* __restrict__ out
 #pragma unroll
             for (int k2 = 0; k2 < 8; ++k2) p[k2 ^ s] = v[k2];
         }
-        __syncthreads();
+        group_sync<TG>(grp);
         // ---- y stage A, in place: rows j1*R2Y + j2 of column c = (k1, k2) -> rows k1y*R2Y + j2
-        for (int item = tid; item < C::I_YA; item += T) {
+        for (int item = tid; item < C::I_YA; item += TG) {
             const int c = item % NZ, rr = item / NZ, j2 = rr % R2Y, lp = rr / R2Y;
             const int k1 = c >> 3, k2 = c & 7;
             const int row0 = lp * NYS + j2;
@@ -179,39 +191,27 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap map_in, cd* __restrict__ out
             sm[swz(row0 * R1Z + k1, k2)] = x[0];
 #pragma unroll
             for (int k1y = 1; k1y < R1Y; ++k1y)
-                sm[swz((row0 + k1y * R2Y) * R1Z + k1, k2)] = cmulc(x[k1y], ldg_cd(tw_y + S * k1y * j2));
+                sm[swz((row0 + k1y * R2Y) * R1Z + k1, k2)] = cmulc(x[k1y], stw_y[S * k1y * j2]);
         }
-        __syncthreads();
+        group_sync<TG>(grp);
         // ---- y stage B -> global at the in-place position: row rho = k1y*R2Y + k2y (plane row S*rho + r), column c
-        constexpr int RB = (C::I_YB + T - 1) / T;
-        cd res[RB][R2Y];
+        for (int item = tid; item < C::I_YB; item += TG) {
+            const int c = item % NZ, rr = item / NZ, k1y = rr % R1Y, lp = rr / R1Y;
+            const int k1 = c >> 3, k2 = c & 7;
+            const int row0 = lp * NYS + k1y * R2Y;
+            cd res[R2Y];
 #pragma unroll
-        for (int u = 0; u < RB; ++u) {
-            const int item = tid + u * T;
-            if (item < C::I_YB) {
-                const int c = item % NZ, rr = item / NZ, k1y = rr % R1Y, lp = rr / R1Y;
-                const int k1 = c >> 3, k2 = c & 7;
-                const int row0 = lp * NYS + k1y * R2Y;
+            for (int j2 = 0; j2 < R2Y; ++j2) res[j2] = sm[swz((row0 + j2) * R1Z + k1, k2)];
+            Dft<R2Y, -1>::run(res);
+            const int part = part0 + lp, plane = part / S, r = part % S;
+            cd* dst = out + (size_t)plane * NY * NZ + (size_t)(S * (k1y * R2Y) + r) * NZ + c;
 #pragma unroll
-                for (int j2 = 0; j2 < R2Y; ++j2) res[u][j2] = sm[swz((row0 + j2) * R1Z + k1, k2)];
-            }
+            for (int k2y = 0; k2y < R2Y; ++k2y) sts_cd(dst + (size_t)(S * k2y) * NZ, res[k2y]);
         }
-        // every read of this buffer is done: hand it back to the TMA before the butterflies and the stores
+        // every read of this buffer is done: hand it back to the TMA
         fence_proxy_async();
-        __syncthreads();
-        if (tid == 0 && t + NB * (int)gridDim.x < ntiles) issue(t + NB * gridDim.x, b);
-#pragma unroll
-        for (int u = 0; u < RB; ++u) {
-            const int item = tid + u * T;
-            if (item < C::I_YB) {
-                const int c = item % NZ, rr = item / NZ, k1y = rr % R1Y, lp = rr / R1Y;
-                Dft<R2Y, -1>::run(res[u]);
-                const int part = part0 + lp, plane = part / S, r = part % S;
-                cd* dst = out + (size_t)plane * NY * NZ + (size_t)(S * (k1y * R2Y) + r) * NZ + c;
-#pragma unroll
-                for (int k2y = 0; k2y < R2Y; ++k2y) sts_cd(dst + (size_t)(S * k2y) * NZ, res[u][k2y]);
-            }
-        }
+        group_sync<TG>(grp);
+        if (tid == 0) issue(k + NB);
     }
 }
 
