@@ -6,14 +6,14 @@ namespace tdh {
 
 struct TileLaunch {
     const void* fwd;   // tile_fwd_kernel<NY,NZ>
-    const void* inv;   // tile_inv_kernel<NY,NZ>
+    const void* inv[5];  // tile_inv_kernel<NY,NZ,CM>, CM = 0 (no projectors), 1, 4, 9, 16 (tile_kernels.cuh, nl_cm_index)
     int threads;
     int ppc;           // plane parts per CTA
     int s;             // y-split: a plane is s parts (rows y = s*m + r)
     int r1y, r2y;      // factorisation of the y transform of length NY/s (row order inside a tile)
     int r1z;           // NZ / 8 (128-byte lines per row)
     size_t smem_fwd;   // dynamic shared memory per CTA of tile_fwd (ring of tiles)
-    size_t smem_inv;   // dynamic shared memory per CTA of tile_inv (two spectrum buffers + one phi buffer)
+    size_t smem_inv;   // dynamic shared memory per CTA of tile_inv (the same ring)
 };
 
 struct XLaunch {

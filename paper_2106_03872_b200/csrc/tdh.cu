@@ -82,8 +82,7 @@ struct tdh_grid {
     cd* d_twy_w;          // exp(+2 pi i k / NY) per row pair of the work layout (y-split grids)
     int* d_rowmap;        // natural ky -> plane row of the work layout
     int* d_colmap;        // natural kz -> column of the work layout
-    int ctas_fwd, ctas_inv, ctas_x[3];   // persistent grid sizes (SM count x resident CTAs)
-    size_t smem_inv_max;                 // dynamic shared memory tile_inv may use (tile buffers + staged dpi)
+    int ctas_fwd, ctas_inv[tdh::NL_NCM], ctas_x[3];   // persistent grid sizes (SM count x resident CTAs)
 
     int chunk_cap;        // states the workspace can hold
     int chunk;            // states pushed through the chain together
@@ -200,13 +199,13 @@ extern "C" int tdh_create_grid(const int n[3], const double len[3], const double
         int dev = 0, nsm = 0;
         CU(cudaGetDevice(&dev));
         CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
-        const void* fs[5] = {g->tl.fwd, g->tl.inv, g->xl.fused, g->xl.fwd, g->xl.inv};
-        // tile_inv may stage up to 16 KB of projection coefficients behind its tile buffers (launch_plane_inv)
-        g->smem_inv_max = std::min<size_t>(232448, g->tl.smem_inv + 16384);
-        const size_t sm[5] = {g->tl.smem_fwd, g->smem_inv_max, g->xl.smem, g->xl.smem, g->xl.smem};
-        const int th[5] = {g->tl.threads, g->tl.threads, g->xl.threads, g->xl.threads, g->xl.threads};
-        int ctas[5];
-        for (int i = 0; i < 5; ++i) {
+        constexpr int NK = 4 + tdh::NL_NCM;
+        const void* fs[NK] = {g->tl.fwd, g->xl.fused, g->xl.fwd, g->xl.inv};
+        size_t sm[NK] = {g->tl.smem_fwd, g->xl.smem, g->xl.smem, g->xl.smem};
+        int th[NK] = {g->tl.threads, g->xl.threads, g->xl.threads, g->xl.threads};
+        for (int i = 0; i < tdh::NL_NCM; ++i) { fs[4 + i] = g->tl.inv[i]; sm[4 + i] = g->tl.smem_inv; th[4 + i] = g->tl.threads; }
+        int ctas[NK];
+        for (int i = 0; i < NK; ++i) {
             CU(cudaFuncSetAttribute(fs[i], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm[i]));
             CU(cudaFuncSetAttribute(fs[i], cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
             int occ = 0;
@@ -215,8 +214,9 @@ extern "C" int tdh_create_grid(const int n[3], const double len[3], const double
             if (const char* e = getenv("TDH_MAX_CTAS_PER_SM")) { int v = atoi(e); if (v > 0) occ = std::min(occ, v); }
             ctas[i] = nsm * occ;
         }
-        g->ctas_fwd = ctas[0]; g->ctas_inv = ctas[1];
-        g->ctas_x[0] = ctas[2]; g->ctas_x[1] = ctas[3]; g->ctas_x[2] = ctas[4];
+        g->ctas_fwd = ctas[0];
+        g->ctas_x[0] = ctas[1]; g->ctas_x[1] = ctas[2]; g->ctas_x[2] = ctas[3];
+        for (int i = 0; i < tdh::NL_NCM; ++i) g->ctas_inv[i] = ctas[4 + i];
         // tables: built on the host exactly as the oracle builds its G vectors (two_pi * m / L + k, then squared)
         const double two_pi = 6.283185307179586476925286766559;
         for (int a = 0; a < 3; ++a) {
@@ -561,6 +561,23 @@ static int launch_xpencil(tdh_grid* g, int nst, const cd* in, cd* out, int mode)
     return TDH_OK;
 }
 
+#ifdef TDH_PHASE_CLOCKS
+// debug builds only (not part of include/tdh.h): clock ticks per phase of tile_inv, summed over warp groups; reading
+// resets them
+static unsigned long long* g_ticks = nullptr;
+static unsigned long long* phase_ticks_buffer() {
+    if (!g_ticks && cudaMalloc(&g_ticks, 16 * sizeof(unsigned long long)) == cudaSuccess)
+        cudaMemset(g_ticks, 0, 16 * sizeof(unsigned long long));
+    return g_ticks;
+}
+extern "C" int tdh_debug_phase_ticks(unsigned long long out[16]) {
+    if (!phase_ticks_buffer() || cudaDeviceSynchronize() != cudaSuccess) return TDH_ECUDA;
+    if (cudaMemcpy(out, g_ticks, 16 * sizeof(unsigned long long), cudaMemcpyDeviceToHost) != cudaSuccess) return TDH_ECUDA;
+    if (cudaMemset(g_ticks, 0, 16 * sizeof(unsigned long long)) != cudaSuccess) return TDH_ECUDA;
+    return TDH_OK;
+}
+#endif
+
 // in: work block (spectrum), phi: input block of this application (read only when the epilogue has V or projectors)
 static int launch_plane_inv(tdh_grid* g, int nst, const cd* in, const cd* phi, cd* out, const tdh::Epilogue& ep) {
     CUtensorMap map_spec, map_phi;
@@ -573,15 +590,14 @@ static int launch_plane_inv(tdh_grid* g, int nst, const cd* in, const cd* phi, c
     const cd* twz = g->d_tw[2];
     int ntiles = (int)((size_t)nst * g->n[0] * g->tl.s / g->tl.ppc);
     tdh::Epilogue epl = ep;
-    size_t smem = g->tl.smem_inv;
-    if (epl.nl_off != nullptr) {
-        // dpi of the current state is staged behind the tile buffers when it fits
-        const size_t extra = sizeof(cd) * (size_t)(epl.nchan_tot + epl.cmax);
-        if (smem + extra <= g->smem_inv_max) { epl.dpi_smem = 1; smem += extra; }
-    }
+    epl.phi = phi;
+#ifdef TDH_PHASE_CLOCKS
+    epl.ticks = phase_ticks_buffer();
+#endif
     void* args[] = {(void*)&map_spec, (void*)&map_phi, (void*)&map_yv, (void*)&out, (void*)&ntiles, (void*)&twy, (void*)&twz, (void*)&epl};
-    const unsigned grid = (unsigned)std::min(ntiles, g->ctas_inv);
-    LAUNCH(K_PLANE_INV, g->tl.inv, dim3(grid), dim3(g->tl.threads), smem, args);
+    const int cmi = tdh::nl_cm_index(epl.nl_off != nullptr ? epl.cmax : 0);
+    const unsigned grid = (unsigned)std::min(ntiles, g->ctas_inv[cmi]);
+    LAUNCH(K_PLANE_INV, g->tl.inv[cmi], dim3(grid), dim3(g->tl.threads), g->tl.smem_inv, args);
     return TDH_OK;
 }
 

@@ -44,8 +44,7 @@ template <> struct FactY<96> { static constexpr int R1 = 12, R2 = 8; };
 
 constexpr int tile_round_up(int a, int b) { return (a + b - 1) / b * b; }
 constexpr int TILE_MAX_CELLS = 4608;
-constexpr int TILE_HEADER = 1024;      // tile_inv: barriers; keeps the buffers 1024-byte aligned
-constexpr int TILE_HEADER_FWD = 4096;  // tile_fwd: barriers (64 bytes), then the z and y twiddle tables
+constexpr int TILE_HEADER_FWD = 4096;  // barriers (64 bytes), then the z and y twiddle tables; keeps the buffers 1024-byte aligned
 constexpr int TILE_TW_OFF = 64;
 
 template <int NY, int NZ> struct TileCfg {
@@ -66,7 +65,7 @@ template <int NY, int NZ> struct TileCfg {
     static constexpr size_t TILE_BYTES = (size_t)CELLS * sizeof(cd);
     static constexpr int NB_FWD = 3;                                // ring depth of tile_fwd
     static constexpr size_t SMEM_FWD = TILE_HEADER_FWD + NB_FWD * TILE_BYTES;
-    static constexpr size_t SMEM_INV = TILE_HEADER + 3 * TILE_BYTES;   // two spectrum buffers + one phi buffer
+    static constexpr size_t SMEM_INV = SMEM_FWD;                       // tile_inv: the same ring of three tiles
     // work items of the four stages
     static constexpr int I_ZA = ROWS * 8, I_ZB = ROWS * R1Z, I_YA = PPC * NZ * R2Y, I_YB = PPC * NZ * R1Y;
     static constexpr int cost(int t) {
@@ -217,7 +216,8 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap map_in, cd* __restrict__ out
 
 // Arguments of the fused epilogue of tile_inv.
 struct Epilogue {
-    const double* v;        // V(r), n0*n1*n2; NULL: no local term (then map_phi is not used, unless nl_off != NULL)
+    const double* v;        // V(r), n0*n1*n2; NULL: no local term (then phi is not read, unless nl_off != NULL)
+    const cd* phi;          // input block of this Hamiltonian application (read with V and with projectors)
     const cd* yv;           // optional addend y (same block layout as out); NULL: none
     cd alpha;               // out = alpha * (T + V + Vnl) phi + y
     int nx;                 // planes per state
@@ -232,25 +232,33 @@ struct Epilogue {
     const cd* nl_phase;     // per record e^{+ik.d}; NULL at Gamma
     const cd* dpi;          // [state][nchan_tot] D * dV * <beta|phi>  (+ cmax zeroed entries of padding)
     int nrec;
-    int cmax;               // padded channel count of a record: 1, 4, 9 or 16 (nl_pad_cmax)
+    int cmax;               // padded channel count of a record: 1, 4, 9 or 16 (nl_pad_cmax) = the kernel's CM
     int nchan_tot;
-    int dpi_smem;           // 1: the CTA stages dpi of the current state in shared memory behind the tile buffers
+#ifdef TDH_PHASE_CLOCKS
+    unsigned long long* ticks;   // [16] phase timers (debug builds)
+#endif
 };
 
 // channel counts the record loop is compiled for; the host pads nl_beta (zeros) and dpi (zeros) to this
 __host__ __device__ constexpr int nl_pad_cmax(int c) { return c <= 1 ? 1 : (c <= 4 ? 4 : (c <= 9 ? 9 : 16)); }
+// index of a padded channel count in the table of tile_inv instantiations (0: no projectors)
+__host__ __device__ constexpr int nl_cm_index(int cm) { return cm == 0 ? 0 : (cm == 1 ? 1 : (cm == 4 ? 2 : (cm == 9 ? 3 : 4))); }
+constexpr int NL_NCM = 5;
+// records of one thread in flight together
+template <int CM> struct NlUnroll { static constexpr int U = CM <= 1 ? 8 : (CM <= 4 ? 6 : (CM <= 9 ? 3 : 2)); };
 
 // One layer of the back-projection of one plane part: records [i0, i1) add  e^{-ik.d} sum_c beta_c[i] * dpi[chan0 + c]
 // into cell (cc & 0xffff) of `base`.  U records per thread are in flight together: the loop is bound by the latency of
-// the record loads (L2), not by arithmetic.  dp points at dpi of this state (shared or global memory).
+// the record loads (L2), not by arithmetic.  dp points at dpi of this state (global memory; the few hundred bytes a
+// tile touches stay in L1).
 template <int CM, int U>
-__device__ __forceinline__ void nl_scatter_layer(cd* base, const cd* dp, const unsigned* __restrict__ nl_cc,
+__device__ __forceinline__ void nl_scatter_layer(cd* base, const cd* __restrict__ dp, const unsigned* __restrict__ nl_cc,
                                                  const double* __restrict__ nl_beta, const cd* __restrict__ nl_phase,
                                                  size_t nrec, int i0, int i1, int tid, int nthreads)
 {
     for (int ib = i0 + tid; ib < i1; ib += U * nthreads) {
         unsigned cc[U];
-        double bv[U][CM];
+        double bv[U][CM > 0 ? CM : 1];
         cd ph[U];
 #pragma unroll
         for (int u = 0; u < U; ++u) {
@@ -268,7 +276,7 @@ __device__ __forceinline__ void nl_scatter_layer(cd* base, const cd* dp, const u
                 cd sacc = make_double2(0.0, 0.0);
 #pragma unroll
                 for (int c = 0; c < CM; ++c) {
-                    const cd dv = d[c];
+                    const cd dv = ldg_cd(d + c);
                     sacc.x = fma(bv[u][c], dv.x, sacc.x);
                     sacc.y = fma(bv[u][c], dv.y, sacc.y);
                 }
@@ -280,82 +288,97 @@ __device__ __forceinline__ void nl_scatter_layer(cd* base, const cd* dp, const u
     }
 }
 
+// Optional phase timing of tile_inv (build with -DTDH_PHASE_CLOCKS): thread 0 of every warp group accumulates the
+// clock64() ticks between the marks below into ep.ticks[16], read back by tdh_debug_phase_ticks (tdh.cu).
+#ifdef TDH_PHASE_CLOCKS
+#define TDH_MARK(k)                                                                     \
+    do {                                                                                \
+        if (tid == 0) {                                                                 \
+            const long long now_ = clock64();                                           \
+            atomicAdd(ep.ticks + (k), (unsigned long long)(now_ - mark_t_));            \
+            mark_t_ = now_;                                                             \
+        }                                                                               \
+    } while (0)
+#define TDH_MARK_INIT long long mark_t_ = clock64()
+#else
+#define TDH_MARK(k) do {} while (0)
+#define TDH_MARK_INIT do {} while (0)
+#endif
+
 // ------------------------------------------------------------------------------------------------------------
-// inverse + epilogue: `map_spec` describes the work block (digit-permuted spectrum), `map_phi` the input block of this
-// Hamiltonian application, `map_yv` the addend block ep.yv (both same geometry; map_yv is only used to prefetch the
-// addend tile into L2), `out` the output block.  Shared memory: two spectrum buffers X0, X1 (tile
-// i in X[i & 1], tile i+1 streaming into the other) and one buffer Y for phi of the current tile, which becomes
-// V*phi + V_nl phi when there are projectors.  Persistent grid; ntiles = nst * NX * S / PPC.
+// inverse + epilogue: `map_spec` describes the work block (digit-permuted spectrum), `out` the output block; `map_phi`
+// and `map_yv` describe the input block ep.phi of this Hamiltonian application and the addend block ep.yv (same
+// geometry) and are only used to start their tiles towards L2 when a tile's turn begins -- the epilogue reads both
+// straight from global memory.  CM = padded channel count of the projector records (0: no projectors; ep.cmax == CM).
+// Persistent grid; ntiles = nst * NX * S / PPC.
+//
+// WARP GROUPS as in tile_fwd: two groups of TG = T/2 threads, a ring of three spectrum buffers, the CTA's k-th tile in
+// buffer k % 3 handled by group k % 2.  Per tile: inverse y (two stages), inverse z (two stages), then
+//   without projectors: the last z stage ends in registers, out = alpha * (x + V phi) + y goes straight to global;
+//   with projectors:    the last z stage is written back in place (natural order), the record lists add V_nl phi into
+//                       the tile layer by layer, and a final pass forms out = alpha * (tile + V phi) + y.
+// A stage of one group that waits on L2 (records, phi, V, y) or on the store queue overlaps with the other group's
+// butterflies.
 // ------------------------------------------------------------------------------------------------------------
-template <int NY, int NZ>
+template <int NY, int NZ, int CM>
 __global__ void __launch_bounds__(TileCfg<NY, NZ>::T, 1)
 tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_constant__ CUtensorMap map_phi,
-                const __grid_constant__ CUtensorMap map_yv, cd* __restrict__ out, int ntiles, const cd* __restrict__ tw_y, const cd* __restrict__ tw_z,
-                const Epilogue ep)
+                const __grid_constant__ CUtensorMap map_yv, cd* __restrict__ out, int ntiles,
+                const cd* __restrict__ tw_y, const cd* __restrict__ tw_z, const Epilogue ep)
 {
     using C = TileCfg<NY, NZ>;
-    constexpr int S = C::S, NYS = C::NYS, R1Z = C::R1Z, R1Y = C::R1Y, R2Y = C::R2Y, T = C::T;
+    constexpr int S = C::S, NYS = C::NYS, R1Z = C::R1Z, R1Y = C::R1Y, R2Y = C::R2Y, T = C::T, NB = C::NB_FWD;
+    constexpr int TG = T / 2;
+    constexpr bool HAVE_NL = CM > 0;
+    static_assert(NB == 3 && TG % 32 == 0, "ring of three buffers shared by two warp groups");
     extern __shared__ __align__(1024) unsigned char smem_raw[];
-    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);             // [0], [1]: X buffers; [2]: Y
-    cd* xbuf = reinterpret_cast<cd*>(smem_raw + TILE_HEADER);
-    cd* ybuf = xbuf + 2 * (size_t)C::CELLS;
-    cd* sdpi = ybuf + (size_t)C::CELLS;                                   // [nchan_tot + cmax], only with ep.dpi_smem
-    const int tid = threadIdx.x;
-    const bool have_nl = ep.nl_off != nullptr;
-    const bool have_phi = have_nl || ep.v != nullptr;
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);
+    cd* stw_z = reinterpret_cast<cd*>(smem_raw + TILE_TW_OFF);          // e^{+2 pi i m / NZ}
+    cd* stw_y = stw_z + NZ;                                             // e^{+2 pi i m / NY}
+    cd* ring = reinterpret_cast<cd*>(smem_raw + TILE_HEADER_FWD);
+    const int grp = threadIdx.x / TG, tid = threadIdx.x % TG;           // tid: index inside the group
+    const bool have_v = HAVE_NL || ep.v != nullptr;
 
-    uint64_t pol = 0;
-    if (tid == 0) {
+    uint64_t pol = policy_evict_first();
+    if (threadIdx.x == 0) {
         tma_prefetch_desc(&map_spec);
-        tma_prefetch_desc(&map_phi);
-        pol = policy_evict_first();
-        for (int b = 0; b < 3; ++b) mbar_init(full + b, 1);
+        if (have_v) tma_prefetch_desc(&map_phi);
+        if (ep.yv != nullptr) tma_prefetch_desc(&map_yv);
+        for (int b = 0; b < NB; ++b) mbar_init(full + b, 1);
         mbar_fence_init();
     }
+    for (int i = threadIdx.x; i < NZ; i += T) stw_z[i] = ldg_cd(tw_z + i);
+    for (int i = threadIdx.x; i < NY; i += T) stw_y[i] = ldg_cd(tw_y + i);
     __syncthreads();
-    auto issue = [&](const CUtensorMap* map, int t, cd* dst, uint64_t* bar) {      // thread 0 only
+    auto issue = [&](int k) {                            // one thread; tile k of this CTA into buffer k % NB
+        const int t = blockIdx.x + k * gridDim.x;
+        if (t >= ntiles) return;
+        const int b = k % NB;
         const int part0 = t * C::PPC, plane = part0 / S, r = part0 % S;
-        mbar_arrive_expect_tx(bar, (uint32_t)C::TILE_BYTES);
-        tma_load_4d(dst, map, bar, 0, r * R1Z, 0, plane, pol);
+        mbar_arrive_expect_tx(full + b, (uint32_t)C::TILE_BYTES);
+        tma_load_4d(ring + (size_t)b * C::CELLS, &map_spec, full + b, 0, r * R1Z, 0, plane, pol);
     };
-    // this CTA's tiles: the contiguous range [t_begin, t_end) -- consecutive x of one state, so that the state (and its
-    // dpi in shared memory) changes once per NX*S/PPC tiles
-#ifdef TDH_INV_CONTIG
-    const int t_begin = (int)((long long)ntiles * blockIdx.x / gridDim.x);
-    const int t_end = (int)((long long)ntiles * (blockIdx.x + 1) / gridDim.x);
-    constexpr int t_step_c = 1; const int t_step = t_step_c;
-#else
-    const int t_begin = blockIdx.x, t_end = ntiles, t_step = gridDim.x;
-#endif
-    if (tid == 0) {
-        if (t_begin < t_end) {
-            issue(&map_spec, t_begin, xbuf, full + 0);
-            if (have_phi) issue(&map_phi, t_begin, ybuf, full + 2);
-        }
-        if (t_begin + t_step < t_end) issue(&map_spec, t_begin + t_step, xbuf + C::CELLS, full + 1);
-    }
-    int st_smem = -1;                                                     // state whose dpi is in sdpi
+    if (threadIdx.x == 0)
+        for (int k = 0; k < NB; ++k) issue(k);
 
-    int it = 0;
-    for (int t = t_begin; t < t_end; t += t_step, ++it) {
-        const int cur = it & 1;
-        cd* sm = xbuf + (size_t)cur * C::CELLS;
+    TDH_MARK_INIT;
+    for (int k = grp;; k += 2) {
+        const int t = blockIdx.x + k * gridDim.x;
+        if (t >= ntiles) break;
+        const int b = k % NB;
+        cd* sm = ring + (size_t)b * C::CELLS;
         const int part0 = t * C::PPC;
-        const int st = (part0 / S) / ep.nx;                               // PPC divides NX: one state per tile
-        if (have_nl && ep.dpi_smem && st != st_smem) {
-            // read by the record loop below, after at least one barrier; the previous tile ended with a barrier
-            const cd* src = ep.dpi + (size_t)st * ep.nchan_tot;
-            for (int i = tid; i < ep.nchan_tot + ep.cmax; i += T)
-                sdpi[i] = i < ep.nchan_tot ? ldg_cd(src + i) : make_double2(0.0, 0.0);
-            st_smem = st;
+        // the tiles of phi and of the addend that the epilogue will read: start them towards L2 now
+        if (tid == 0) {
+            if (have_v) tma_prefetch_l2_4d(&map_phi, 0, (part0 % S) * R1Z, 0, part0 / S);
+            if (ep.yv != nullptr) tma_prefetch_l2_4d(&map_yv, 0, (part0 % S) * R1Z, 0, part0 / S);
         }
-        // the addend tile is read straight from global memory by the epilogue: start it towards L2 now
-        if (tid == 0 && ep.yv != nullptr) tma_prefetch_l2_4d(&map_yv, 0, (part0 % S) * R1Z, 0, part0 / S);
-        mbar_wait(full + cur, (uint32_t)(it >> 1) & 1u);
+        mbar_wait(full + b, (uint32_t)(k / NB) & 1u);
+        TDH_MARK(0);
 
         // ---- y stage A', in place: rows k1y*R2Y + k2y (contiguous) hold k = k1y + R1Y*k2y; radix R2Y over k2y -> j2,
         //      twiddle w^(-j2*k1y)
-        for (int item = tid; item < C::I_YB; item += T) {
+        for (int item = tid; item < C::I_YB; item += TG) {
             const int c = item % NZ, rr = item / NZ, k1y = rr % R1Y, lp = rr / R1Y;
             const int k1 = c >> 3, k2 = c & 7;
             const int row0 = lp * NYS + k1y * R2Y;
@@ -365,12 +388,12 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
             Dft<R2Y, +1>::run(v);
             sm[swz(row0 * R1Z + k1, k2)] = v[0];
 #pragma unroll
-            for (int j2 = 1; j2 < R2Y; ++j2)
-                sm[swz((row0 + j2) * R1Z + k1, k2)] = cmul(v[j2], ldg_cd(tw_y + S * j2 * k1y));
+            for (int j2 = 1; j2 < R2Y; ++j2) sm[swz((row0 + j2) * R1Z + k1, k2)] = cmul(v[j2], stw_y[S * j2 * k1y]);
         }
-        __syncthreads();
+        group_sync<TG>(grp);
+        TDH_MARK(1);
         // ---- y stage B', in place: rows k1y*R2Y + j2, radix R1Y over k1y -> j1: row j1*R2Y + j2 = m, y = S*m + r
-        for (int item = tid; item < C::I_YA; item += T) {
+        for (int item = tid; item < C::I_YA; item += TG) {
             const int c = item % NZ, rr = item / NZ, j2 = rr % R2Y, lp = rr / R2Y;
             const int k1 = c >> 3, k2 = c & 7;
             const int row0 = lp * NYS + j2;
@@ -381,9 +404,10 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
 #pragma unroll
             for (int j1 = 0; j1 < R1Y; ++j1) sm[swz((row0 + j1 * R2Y) * R1Z + k1, k2)] = x[j1];
         }
-        __syncthreads();
+        group_sync<TG>(grp);
+        TDH_MARK(2);
         // ---- z stage A', in place inside line g = (row, k1): positions k2 hold kz = k1 + R1Z*k2; radix 8 -> j2
-        for (int g = tid; g < C::I_ZB; g += T) {
+        for (int g = tid; g < C::I_ZB; g += TG) {
             cd* p = sm + 8 * g;
             const int s = g & 7;
             cd v[8];
@@ -393,94 +417,92 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
 #pragma unroll
             for (int j2 = 0; j2 < 8; ++j2) p[j2 ^ s] = v[j2];
         }
-        // ---- with projectors: Y = V * phi, then the back-projection adds V_nl phi into Y layer by layer
-        if (have_nl) {
-            mbar_wait(full + 2, (uint32_t)it & 1u);
-            const int j2 = tid & 7;
-            for (int lr = tid >> 3; lr < C::ROWS; lr += T / 8) {
-                const int lp = lr / NYS, m = lr % NYS;
-                const int part = part0 + lp, plane = part / S, r = part % S;
-                const double* vrow = ep.v + ((size_t)(plane % ep.nx) * NY + (S * m + r)) * NZ + j2;
+        group_sync<TG>(grp);
+        TDH_MARK(3);
+        const int j2 = tid & 7;
+        if (HAVE_NL) {
+            // ---- z stage B', in place: thread (row lr, j2): twiddle w^(-k1*j2), radix R1Z over k1 -> cell (lr, 8*j1 + j2)
+            for (int lr = tid >> 3; lr < C::ROWS; lr += TG / 8) {
+                const int l0 = lr * R1Z;
+                cd x[R1Z];
+                x[0] = sm[swz(l0, j2)];
 #pragma unroll
-                for (int j1 = 0; j1 < R1Z; ++j1) {
-                    const int cell = swz(lr * R1Z + j1, j2);
-                    const double vv = __ldg(vrow + 8 * j1);
-                    const cd ph = ybuf[cell];
-                    ybuf[cell] = make_double2(vv * ph.x, vv * ph.y);
-                }
+                for (int k1 = 1; k1 < R1Z; ++k1) x[k1] = cmul(sm[swz(l0 + k1, j2)], stw_z[k1 * j2]);
+                Dft<R1Z, +1>::run(x);
+#pragma unroll
+                for (int j1 = 0; j1 < R1Z; ++j1) sm[swz(l0 + j1, j2)] = x[j1];
             }
-            __syncthreads();
-            const cd* dp = ep.dpi_smem ? sdpi : ep.dpi + (size_t)st * ep.nchan_tot;
+            group_sync<TG>(grp);
+            TDH_MARK(4);
+            // ---- back-projection: the tile now holds T phi in natural order; add V_nl phi layer by layer
+            const int st = (part0 / S) / ep.nx;                           // PPC divides NX: one state per tile
+            const cd* dp = ep.dpi + (size_t)st * ep.nchan_tot;
             for (int layer = 0; layer < ep.nl_layers; ++layer) {
 #pragma unroll
                 for (int lp = 0; lp < C::PPC; ++lp) {
                     const int part = part0 + lp, plane = part / S, r = part % S;
                     const int x = plane % ep.nx;
                     const int* off = ep.nl_off + (size_t)(x * S + r) * (ep.nl_layers + 1) + layer;
-                    const int i0 = __ldg(off), i1 = __ldg(off + 1);
-                    cd* base = ybuf + lp * C::PART;
-                    switch (ep.cmax) {
-                        case 1: nl_scatter_layer<1, 4>(base, dp, ep.nl_cc, ep.nl_beta, ep.nl_phase, ep.nrec, i0, i1, tid, T); break;
-                        case 4: nl_scatter_layer<4, 4>(base, dp, ep.nl_cc, ep.nl_beta, ep.nl_phase, ep.nrec, i0, i1, tid, T); break;
-                        case 9: nl_scatter_layer<9, 2>(base, dp, ep.nl_cc, ep.nl_beta, ep.nl_phase, ep.nrec, i0, i1, tid, T); break;
-                        default: nl_scatter_layer<16, 1>(base, dp, ep.nl_cc, ep.nl_beta, ep.nl_phase, ep.nrec, i0, i1, tid, T); break;
-                    }
+                    nl_scatter_layer<CM, NlUnroll<CM>::U>(sm + lp * C::PART, dp, ep.nl_cc, ep.nl_beta, ep.nl_phase,
+                                                          (size_t)ep.nrec, __ldg(off), __ldg(off + 1), tid, TG);
                 }
-                __syncthreads();
+                group_sync<TG>(grp);
             }
-        } else {
-            if (have_phi) mbar_wait(full + 2, (uint32_t)it & 1u);
-            __syncthreads();
+            TDH_MARK(5);
         }
-        // ---- z stage B' + epilogue: thread (row lr, j2): twiddle, radix R1Z over k1 -> z = 8*j1 + j2;
-        //      out = alpha * (T phi + V phi + Vnl phi) + y, straight from registers
-        {
-            const int j2 = tid & 7;
-            for (int lr = tid >> 3; lr < C::ROWS; lr += T / 8) {
-                const int l0 = lr * R1Z;
-                const int lp = lr / NYS, m = lr % NYS;
-                const int part = part0 + lp, plane = part / S, r = part % S;
-                const int y = S * m + r;
-                const size_t gi = (size_t)plane * NY * NZ + (size_t)y * NZ + j2;               // index in the block
-                cd x[R1Z];
+        // ---- epilogue, thread (row lr, j2), cells z = 8*j1 + j2:  out = alpha * (T phi [+ V_nl phi] + V phi) + y.
+        //      phi, V and y come straight from global memory (their tiles were started towards L2 above); all their
+        //      loads are issued before the first store because out may alias y.
+        for (int lr = tid >> 3; lr < C::ROWS; lr += TG / 8) {
+            const int l0 = lr * R1Z;
+            const int lp = lr / NYS, m = lr % NYS;
+            const int part = part0 + lp, plane = part / S, r = part % S;
+            const int y = S * m + r;
+            const size_t gi = (size_t)plane * NY * NZ + (size_t)y * NZ + j2;               // index in the block
+            double vv[R1Z];
+            cd ph[R1Z];
+            if (have_v) {
+                const double* vrow = ep.v + ((size_t)(plane % ep.nx) * NY + y) * NZ + j2;
+#pragma unroll
+                for (int j1 = 0; j1 < R1Z; ++j1) {
+                    vv[j1] = __ldg(vrow + 8 * j1);
+                    ph[j1] = lds_cd(ep.phi + gi + 8 * j1);
+                }
+            }
+            cd x[R1Z];
+            if (HAVE_NL) {
+#pragma unroll
+                for (int j1 = 0; j1 < R1Z; ++j1) x[j1] = sm[swz(l0 + j1, j2)];
+            } else {
                 x[0] = sm[swz(l0, j2)];
 #pragma unroll
-                for (int k1 = 1; k1 < R1Z; ++k1) x[k1] = cmul(sm[swz(l0 + k1, j2)], ldg_cd(tw_z + k1 * j2));   // w_NZ^(-k1*j2)
+                for (int k1 = 1; k1 < R1Z; ++k1) x[k1] = cmul(sm[swz(l0 + k1, j2)], stw_z[k1 * j2]);   // w_NZ^(-k1*j2)
                 Dft<R1Z, +1>::run(x);
-                if (have_nl) {
+            }
+            if (have_v) {
 #pragma unroll
-                    for (int j1 = 0; j1 < R1Z; ++j1) x[j1] = cadd(x[j1], ybuf[swz(l0 + j1, j2)]);
-                } else if (ep.v != nullptr) {
-                    const double* vrow = ep.v + ((size_t)(plane % ep.nx) * NY + y) * NZ + j2;
-#pragma unroll
-                    for (int j1 = 0; j1 < R1Z; ++j1) {
-                        const double vv = __ldg(vrow + 8 * j1);
-                        const cd ph = ybuf[swz(l0 + j1, j2)];
-                        x[j1].x = fma(vv, ph.x, x[j1].x);
-                        x[j1].y = fma(vv, ph.y, x[j1].y);
-                    }
-                }
-                if (ep.yv != nullptr) {
-                    // all loads of the addend before the first store: out may alias yv, so the compiler cannot reorder
-                    // them itself.  The tile of yv was prefetched into L2 when this tile's turn began.
-                    cd ya[R1Z];
-#pragma unroll
-                    for (int j1 = 0; j1 < R1Z; ++j1) ya[j1] = lds_cd(ep.yv + gi + 8 * j1);
-#pragma unroll
-                    for (int j1 = 0; j1 < R1Z; ++j1) sts_cd(out + gi + 8 * j1, cadd(cmul(ep.alpha, x[j1]), ya[j1]));
-                } else {
-#pragma unroll
-                    for (int j1 = 0; j1 < R1Z; ++j1) sts_cd(out + gi + 8 * j1, cmul(ep.alpha, x[j1]));
+                for (int j1 = 0; j1 < R1Z; ++j1) {
+                    x[j1].x = fma(vv[j1], ph[j1].x, x[j1].x);
+                    x[j1].y = fma(vv[j1], ph[j1].y, x[j1].y);
                 }
             }
+            if (ep.yv != nullptr) {
+                cd ya[R1Z];
+#pragma unroll
+                for (int j1 = 0; j1 < R1Z; ++j1) ya[j1] = lds_cd(ep.yv + gi + 8 * j1);
+#pragma unroll
+                for (int j1 = 0; j1 < R1Z; ++j1) sts_cd(out + gi + 8 * j1, cadd(cmul(ep.alpha, x[j1]), ya[j1]));
+            } else {
+#pragma unroll
+                for (int j1 = 0; j1 < R1Z; ++j1) sts_cd(out + gi + 8 * j1, cmul(ep.alpha, x[j1]));
+            }
         }
-        // every read of X[cur] and Y is done: stream in the spectrum of tile i+2 and phi of tile i+1
+        TDH_MARK(6);
+        // every read of this buffer is done: hand it back to the TMA
         fence_proxy_async();
-        __syncthreads();
-        if (tid == 0) {
-            if (t + 2 * t_step < t_end) issue(&map_spec, t + 2 * t_step, sm, full + cur);
-            if (have_phi && t + t_step < t_end) issue(&map_phi, t + t_step, ybuf, full + 2);
-        }
+        group_sync<TG>(grp);
+        if (tid == 0) issue(k + NB);
+        TDH_MARK(7);
     }
 }
 
