@@ -1,0 +1,151 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (whole block in one call, default
+chunking), on sampled states the oracle can compute one by one; and the projector shapes the configs do not reach
+(more than 9 channels per atom, three spheres on one grid point).
+
+The blocks are filled on the device with seeded noise; the sampled states are the configs' own seeded states
+(workloads.state), placed at the first, a middle and the last position of the block.
+"""
+import numpy as np
+import pytest
+
+from paper_2106_03872_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU test selected but no CUDA device: the product has no CPU fallback")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2106_03872_b200 import binding
+    binding.lib()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def oracle():
+    from oracle import build, ref
+    build.build()
+    return ref
+
+
+def per_state_rel(a, b):
+    a = a.reshape(a.shape[0], -1)
+    b = b.reshape(b.shape[0], -1)
+    return np.linalg.norm(a - b, axis=1) / np.linalg.norm(b, axis=1)
+
+
+def device_block(torch, cfg, nst, sample):
+    """(nst, n) complex128 block of seeded device noise scaled like the config's states; states `sample` are W.state."""
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(W.BASE_SEED + cfg.cid)
+    psi = torch.empty((nst,) + tuple(cfg.n), dtype=torch.complex128, device="cuda")
+    scale = 1.0 / np.sqrt(2.0 * cfg.npts * cfg.dv)
+    for s0 in range(0, nst, 64):
+        s1 = min(nst, s0 + 64)
+        v = torch.view_as_real(psi[s0:s1])
+        v.copy_(torch.randn(v.shape, dtype=torch.float64, device="cuda", generator=gen))
+        v.mul_(scale)
+    host = np.stack([W.state(cfg, s) for s in sample])
+    for j, s in enumerate(sample):
+        psi[s].copy_(torch.from_numpy(host[j]))
+    return psi, host
+
+
+def test_large_full_block_sampled_states(torch_cuda, B, oracle):
+    """Config 4 (96^3, 1024 states, 128 atoms): one tdh_apply_hamiltonian call on the whole block, as bench.py times it."""
+    torch = torch_cuda
+    cfg = W.CONFIGS["large"]
+    free, _ = torch.cuda.mem_get_info()
+    nst = cfg.nst if free > 36 * 2 ** 30 else 256           # smaller boxes: same launch configuration, fewer states
+    sample = [0, nst // 2 - 1, nst - 1]
+    wl = W.make(cfg)
+    psi, host = device_block(torch, cfg, nst, sample)
+    with B.grid_for(wl, max_states=nst) as g:
+        out = g.apply_hamiltonian(psi)
+        torch.cuda.synchronize()
+        got = np.stack([out[s].cpu().numpy() for s in sample])
+        # the block around the sampled states was processed too: no state is left unwritten or non-finite
+        assert bool(torch.isfinite(torch.view_as_real(out[nst // 3])).all())
+    ref = oracle.apply_workload(wl, host, oracle.NAIVE_FFT)
+    err = per_state_rel(got, ref)
+    assert err.max() < TOL, err
+    del psi, out
+    torch.cuda.empty_cache()
+
+
+def test_tddft_full_block_sampled_states(torch_cuda, B, oracle):
+    """Config 5 (64^3, 512 states, 64 atoms, 20 Taylor-4 steps of dt = 0.02): propagate the whole block in place."""
+    torch = torch_cuda
+    cfg = W.CONFIGS["tddft"]
+    nst = cfg.nst
+    sample = [0, 255, nst - 1]
+    wl = W.make(cfg)
+    psi, host = device_block(torch, cfg, nst, sample)
+    with B.grid_for(wl, max_states=nst) as g:
+        g.propagate(psi, cfg.dt, cfg.nsteps)
+        torch.cuda.synchronize()
+        got = np.stack([psi[s].cpu().numpy() for s in sample])
+    ref = oracle.propagate_workload(wl, host, backend=oracle.NAIVE_FFT)
+    err = per_state_rel(got, ref)
+    assert err.max() < TOL, err
+    # norm after 20 steps equals the oracle's (reading R15: Taylor-4 is not unitary for white-noise states)
+    n_got = cfg.dv * np.sum(np.abs(got.reshape(len(sample), -1)) ** 2, axis=1)
+    n_ref = cfg.dv * np.sum(np.abs(ref.reshape(len(sample), -1)) ** 2, axis=1)
+    assert np.abs(n_got - n_ref).max() < 1e-11
+    del psi
+    torch.cuda.empty_cache()
+
+
+def synthetic_projectors(cfg, centers, nchan, rng):
+    """Random real projector tables with `nchan` channels on spheres around `centers` (any channel count, any overlap)."""
+    sph_off, chan_off = [0], [0]
+    idx_all, disp_all, beta_all, d_all = [], [], [], []
+    for c in centers:
+        idx, disp = W.sphere_points(cfg, np.asarray(c, dtype=np.float64))
+        idx_all.append(idx)
+        disp_all.append(disp)
+        beta_all.append(rng.standard_normal((nchan, len(idx))).ravel())
+        d_all.append(rng.uniform(-1.0, 2.0, nchan))
+        sph_off.append(sph_off[-1] + len(idx))
+        chan_off.append(chan_off[-1] + nchan)
+    return W.Projectors(natoms=len(centers), sph_off=np.asarray(sph_off, dtype=np.int64),
+                        sph_idx=np.concatenate(idx_all).astype(np.int32), sph_disp=np.concatenate(disp_all),
+                        chan_off=np.asarray(chan_off, dtype=np.int32), beta=np.concatenate(beta_all),
+                        dcoef=np.concatenate(d_all))
+
+
+@pytest.mark.parametrize("n,nchan,kfrac", [((48, 48, 48), 12, (0.0, 0.0, 0.0)), ((16, 32, 16), 16, (0.25, 0.0, -0.1)),
+                                           ((96, 96, 16), 5, (0.0, 0.0, 0.0)), ((32, 32, 32), 1, (0.0, 0.3, 0.0))])
+def test_many_channels_and_three_overlapping_spheres(torch_cuda, B, oracle, n, nchan, kfrac):
+    """Channel counts that pad to 16 / 9 / 1, and grid points covered by three and four spheres (layers >= 3)."""
+    torch = torch_cuda
+    length = tuple(0.4 * m for m in n)
+    cfg = W.test_config(230 + nchan, n, length, nst=6, natoms=1, lmax=0, rc=2.2, dl=(1.0,), kfrac=kfrac)
+    rng = np.random.default_rng([W.BASE_SEED, 230, nchan])
+    mid = [0.5 * l for l in length]
+    centers = [mid, [mid[0] + 0.3, mid[1], mid[2]], [mid[0], mid[1] - 0.4, mid[2] + 0.2], [mid[0] + 0.1, mid[1] + 0.1, mid[2]],
+               [0.1, 0.2, length[2] - 0.1]]                  # the last sphere wraps around the cell corner
+    proj = synthetic_projectors(cfg, centers, nchan, rng)
+    v = rng.uniform(-1.0, 1.0, n)
+    psi = W.states(cfg)
+    ref = oracle.apply_hamiltonian(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, v, proj, psi, oracle.NAIVE_FFT)
+    nl = oracle.nonlocal_(cfg.n, cfg.length, cfg.kpt, proj, psi)
+    assert np.linalg.norm(nl) > 1e-2 * np.linalg.norm(ref)   # the non-local term is a visible part of the result
+    with B.Grid(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, cfg.nst) as g:
+        g.set_potential(torch.from_numpy(v).cuda())
+        g.set_projectors(proj)
+        out = g.apply_hamiltonian(torch.from_numpy(psi).cuda()).cpu().numpy()
+        assert per_state_rel(out, ref).max() < TOL
+        d = torch.from_numpy(psi).cuda()
+        g.propagate(d, 0.01, 2)
+        ref_p = oracle.propagate(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, v, proj, psi, 0.01, 2, 4, oracle.NAIVE_FFT)
+        assert per_state_rel(d.cpu().numpy(), ref_p).max() < TOL
