@@ -242,17 +242,28 @@ def kernel_breakdown(torch, g, fn, steps):
     return {k: v / steps for k, v in tot.items()}, launches
 
 
-def roofline_of(kern_s, units, peak_gbs, peak_src):
-    """Roofline object for the dominant kernel family (largest share of the step)."""
-    cand = {k: v for k, v in kern_s.items() if ALG_BYTES.get(k) and v > 0}
+def alg_bytes(wl):
+    """ALG_BYTES with the gather of the projection kernel filled in: 16 bytes per sphere point and state."""
+    b = dict(ALG_BYTES)
+    b["nl_project"] = 16.0 * float(wl.proj.sph_off[-1]) / wl.cfg.npts if wl.proj.natoms else None
+    return b
+
+
+def roofline_of(kern_s, units, peak_gbs, peak_src, bytes_per_unit):
+    """Roofline object for the dominant kernel family (largest share of the step) + the fractions of the others."""
+    cand = {k: v for k, v in kern_s.items() if bytes_per_unit.get(k) and v > 0}
     if not cand:
         return None
     top = max(cand, key=cand.get)
-    achieved = ALG_BYTES[top] * units / cand[top] * 1e-9
+    achieved = bytes_per_unit[top] * units / cand[top] * 1e-9
+    others = {k: {"achieved": round(bytes_per_unit[k] * units / v * 1e-9, 1),
+                  "frac": round(bytes_per_unit[k] * units / v * 1e-9 / peak_gbs, 4),
+                  "algorithmic_bytes_per_unit": round(bytes_per_unit[k], 3),
+                  "share_of_step": round(v / sum(kern_s.values()), 4)} for k, v in cand.items()}
     return {"kernel": top, "bound": "hbm", "achieved": round(achieved, 1), "peak": peak_gbs, "unit": "GB/s",
             "frac": round(achieved / peak_gbs, 4), "traffic": None, "peak_source": peak_src,
-            "algorithmic_bytes_per_unit": ALG_BYTES[top], "units_per_step": units,
-            "share_of_step": round(cand[top] / sum(kern_s.values()), 4),
+            "algorithmic_bytes_per_unit": bytes_per_unit[top], "units_per_step": units,
+            "share_of_step": round(cand[top] / sum(kern_s.values()), 4), "all_kernels": others,
             "note": "achieved = algorithmic bytes of all launches of this family in one step / their summed CUDA-event "
                     "time (separate profiling pass of the same steps); traffic (ncu dram bytes) is in profiles/"}
 
@@ -394,7 +405,7 @@ def main():
     # ---- per-kernel times (same steps, library events on the launching stream) -> roofline of the dominant family
     kern_s, _ = kernel_breakdown(torch, g, fn, max(1, min(args.steps, 5)))
     peak, peak_src = measured_peaks()
-    roof = roofline_of(kern_s, units, peak, peak_src)
+    roof = roofline_of(kern_s, units, peak, peak_src, alg_bytes(wl))
 
     # ---- end to end through the host-buffer entry point (pinned host in/out, copies inside the timed region)
     e2e = None

@@ -118,7 +118,8 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap map_in, cd* __restrict__ out
     static_assert(NB == 3 && TG % 32 == 0, "ring of three buffers shared by two warp groups");
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);
-    cd* stw_z = reinterpret_cast<cd*>(smem_raw + TILE_TW_OFF);          // e^{+2 pi i m / NZ}
+    cd* stw_z = reinterpret_cast<cd*>(smem_raw + TILE_TW_OFF);          // [k1][j2] = e^{+2 pi i k1 j2 / NZ}: a quarter-warp
+                                                                        // reads 8 consecutive entries (no bank conflict)
     cd* stw_y = stw_z + NZ;                                             // e^{+2 pi i m / NY}
     cd* ring = reinterpret_cast<cd*>(smem_raw + TILE_HEADER_FWD);
     const int grp = threadIdx.x / TG, tid = threadIdx.x % TG;           // tid: index inside the group
@@ -129,7 +130,7 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap map_in, cd* __restrict__ out
         for (int b = 0; b < NB; ++b) mbar_init(full + b, 1);
         mbar_fence_init();
     }
-    for (int i = threadIdx.x; i < NZ; i += T) stw_z[i] = ldg_cd(tw_z + i);
+    for (int i = threadIdx.x; i < NZ; i += T) stw_z[i] = ldg_cd(tw_z + (i >> 3) * (i & 7));   // [k1][j2]: w^(k1*j2)
     for (int i = threadIdx.x; i < NY; i += T) stw_y[i] = ldg_cd(tw_y + i);
     __syncthreads();
     auto issue = [&](int k) {                            // one thread; tile k of this CTA into buffer k % NB
@@ -162,7 +163,7 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap map_in, cd* __restrict__ out
                 Dft<R1Z, -1>::run(x);
                 sm[swz(l0, j2)] = x[0];
 #pragma unroll
-                for (int k1 = 1; k1 < R1Z; ++k1) sm[swz(l0 + k1, j2)] = cmulc(x[k1], stw_z[k1 * j2]);
+                for (int k1 = 1; k1 < R1Z; ++k1) sm[swz(l0 + k1, j2)] = cmulc(x[k1], stw_z[8 * k1 + j2]);
             }
         }
         group_sync<TG>(grp);
@@ -333,7 +334,8 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
     static_assert(NB == 3 && TG % 32 == 0, "ring of three buffers shared by two warp groups");
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);
-    cd* stw_z = reinterpret_cast<cd*>(smem_raw + TILE_TW_OFF);          // e^{+2 pi i m / NZ}
+    cd* stw_z = reinterpret_cast<cd*>(smem_raw + TILE_TW_OFF);          // [k1][j2] = e^{+2 pi i k1 j2 / NZ}: a quarter-warp
+                                                                        // reads 8 consecutive entries (no bank conflict)
     cd* stw_y = stw_z + NZ;                                             // e^{+2 pi i m / NY}
     cd* ring = reinterpret_cast<cd*>(smem_raw + TILE_HEADER_FWD);
     const int grp = threadIdx.x / TG, tid = threadIdx.x % TG;           // tid: index inside the group
@@ -347,7 +349,7 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
         for (int b = 0; b < NB; ++b) mbar_init(full + b, 1);
         mbar_fence_init();
     }
-    for (int i = threadIdx.x; i < NZ; i += T) stw_z[i] = ldg_cd(tw_z + i);
+    for (int i = threadIdx.x; i < NZ; i += T) stw_z[i] = ldg_cd(tw_z + (i >> 3) * (i & 7));   // [k1][j2]: w^(k1*j2)
     for (int i = threadIdx.x; i < NY; i += T) stw_y[i] = ldg_cd(tw_y + i);
     __syncthreads();
     auto issue = [&](int k) {                            // one thread; tile k of this CTA into buffer k % NB
@@ -427,7 +429,7 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
                 cd x[R1Z];
                 x[0] = sm[swz(l0, j2)];
 #pragma unroll
-                for (int k1 = 1; k1 < R1Z; ++k1) x[k1] = cmul(sm[swz(l0 + k1, j2)], stw_z[k1 * j2]);
+                for (int k1 = 1; k1 < R1Z; ++k1) x[k1] = cmul(sm[swz(l0 + k1, j2)], stw_z[8 * k1 + j2]);
                 Dft<R1Z, +1>::run(x);
 #pragma unroll
                 for (int j1 = 0; j1 < R1Z; ++j1) sm[swz(l0 + j1, j2)] = x[j1];
@@ -476,7 +478,7 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
             } else {
                 x[0] = sm[swz(l0, j2)];
 #pragma unroll
-                for (int k1 = 1; k1 < R1Z; ++k1) x[k1] = cmul(sm[swz(l0 + k1, j2)], stw_z[k1 * j2]);   // w_NZ^(-k1*j2)
+                for (int k1 = 1; k1 < R1Z; ++k1) x[k1] = cmul(sm[swz(l0 + k1, j2)], stw_z[8 * k1 + j2]);   // w_NZ^(-k1*j2)
                 Dft<R1Z, +1>::run(x);
             }
             if (have_v) {
