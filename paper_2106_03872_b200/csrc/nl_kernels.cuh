@@ -54,27 +54,52 @@ nl_project_kernel(const cd* __restrict__ psi, size_t npts, int nst, const AtomDe
 #pragma unroll
     for (int m = 0; m < MT; ++m) cre[m][0] = cre[m][1] = cim[m][0] = cim[m][1] = 0.0;
 
-    for (int q0 = warp * 4 * NLP_KSTEPS; q0 < at.np; q0 += NLP_WARPS * 4 * NLP_KSTEPS) {
-        cd b[NLP_KSTEPS];
-#pragma unroll
-        for (int u = 0; u < NLP_KSTEPS; ++u) {
-            const int q = q0 + 4 * u + kq;
-            b[u] = make_double2(0.0, 0.0);
-            if (q < at.np && s_ok) b[u] = __ldcs(ps + __ldg(idx + q));
-        }
+    // Software pipeline over the warp's blocks of 32 points: the sphere indices and the projector values (A fragments)
+    // of block i+1 are requested while the gathers of block i are in flight, so a block costs one DRAM round trip
+    // instead of three dependent ones (index -> psi, beta).
+    constexpr int STRIDE = NLP_WARPS * 4 * NLP_KSTEPS;
+    int ix[NLP_KSTEPS];
+    double af[NLP_KSTEPS][MT];
+    auto load_meta = [&](int q0, int (&ixo)[NLP_KSTEPS], double (&afo)[NLP_KSTEPS][MT]) {
 #pragma unroll
         for (int u = 0; u < NLP_KSTEPS; ++u) {
             const int q = q0 + 4 * u + kq;
             const bool q_ok = q < at.np;
-            cd bv = b[u];
-            if (phs != nullptr && q_ok) bv = cmul(bv, __ldg(phs + q));
+            ixo[u] = q_ok ? __ldg(idx + q) : -1;
 #pragma unroll
             for (int m = 0; m < MT; ++m) {
                 const int c = 8 * m + r8;                                   // A fragment row = channel
-                const double a = (q_ok && c < at.nchan) ? __ldg(sbeta + at.boff + (size_t)c * at.np + q) : 0.0;
-                dmma_m8n8k4(cre[m], a, bv.x);
-                dmma_m8n8k4(cim[m], a, bv.y);
+                afo[u][m] = (q_ok && c < at.nchan) ? __ldg(sbeta + at.boff + (size_t)c * at.np + q) : 0.0;
             }
+        }
+    };
+    int q0 = warp * 4 * NLP_KSTEPS;
+    if (q0 < at.np) load_meta(q0, ix, af);
+    for (; q0 < at.np; q0 += STRIDE) {
+        cd b[NLP_KSTEPS];
+#pragma unroll
+        for (int u = 0; u < NLP_KSTEPS; ++u) {
+            b[u] = make_double2(0.0, 0.0);
+            if (ix[u] >= 0 && s_ok) b[u] = __ldcs(ps + ix[u]);
+        }
+        int ixn[NLP_KSTEPS];
+        double afn[NLP_KSTEPS][MT];
+        if (q0 + STRIDE < at.np) load_meta(q0 + STRIDE, ixn, afn);
+#pragma unroll
+        for (int u = 0; u < NLP_KSTEPS; ++u) {
+            cd bv = b[u];
+            if (phs != nullptr && ix[u] >= 0) bv = cmul(bv, __ldg(phs + q0 + 4 * u + kq));
+#pragma unroll
+            for (int m = 0; m < MT; ++m) {
+                dmma_m8n8k4(cre[m], af[u][m], bv.x);
+                dmma_m8n8k4(cim[m], af[u][m], bv.y);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < NLP_KSTEPS; ++u) {
+            ix[u] = ixn[u];
+#pragma unroll
+            for (int m = 0; m < MT; ++m) af[u][m] = afn[u][m];
         }
     }
 #pragma unroll
