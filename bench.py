@@ -44,7 +44,8 @@ UNIT = "states*gridpoints/s"
 
 # Algorithmic bytes per state*gridpoint of each kernel family: what the launch must read and
 # write if nothing were cached.  plane_inv: spectrum in (16) + phi for V*phi (16) + out (16); +16 with an axpy addend.
-ALG_BYTES = {"nl_project": None, "plane_fwd": 32.0, "xpencil": 32.0, "plane_inv": 48.0}
+# nl_project / nl_scatter: 16 / 32 bytes per sphere point and state (filled in per workload by alg_bytes).
+ALG_BYTES = {"nl_project": None, "plane_fwd": 32.0, "xpencil": 32.0, "plane_inv": 48.0, "nl_scatter": None}
 
 
 def parse_args():
@@ -242,14 +243,21 @@ def kernel_breakdown(torch, g, fn, steps):
     return {k: v / steps for k, v in tot.items()}, launches
 
 
+# DRAM bytes per state*gridpoint measured by ncu (dram__bytes_read.sum + dram__bytes_write.sum of one launch of each
+# kernel / the units of that launch), `large` config: profiles/r01d_summary.md.  Used for roofline.traffic only.
+NCU_DRAM_BYTES_PER_UNIT = {"large": {"nl_project": 13.56, "plane_fwd": 31.01, "xpencil": 30.96, "plane_inv": 50.89}}
+
+
 def alg_bytes(wl):
     """ALG_BYTES with the gather of the projection kernel filled in: 16 bytes per sphere point and state."""
     b = dict(ALG_BYTES)
     b["nl_project"] = 16.0 * float(wl.proj.sph_off[-1]) / wl.cfg.npts if wl.proj.natoms else None
+    # back-projection kernel (large grids): read-modify-write of the same points of the output block
+    b["nl_scatter"] = 32.0 * float(wl.proj.sph_off[-1]) / wl.cfg.npts if wl.proj.natoms else None
     return b
 
 
-def roofline_of(kern_s, units, peak_gbs, peak_src, bytes_per_unit):
+def roofline_of(kern_s, units, peak_gbs, peak_src, bytes_per_unit, workload=None, units_per_launch=None):
     """Roofline object for the dominant kernel family (largest share of the step) + the fractions of the others."""
     cand = {k: v for k, v in kern_s.items() if bytes_per_unit.get(k) and v > 0}
     if not cand:
@@ -260,12 +268,19 @@ def roofline_of(kern_s, units, peak_gbs, peak_src, bytes_per_unit):
                   "frac": round(bytes_per_unit[k] * units / v * 1e-9 / peak_gbs, 4),
                   "algorithmic_bytes_per_unit": round(bytes_per_unit[k], 3),
                   "share_of_step": round(v / sum(kern_s.values()), 4)} for k, v in cand.items()}
+    traffic = None
+    per_unit = NCU_DRAM_BYTES_PER_UNIT.get(workload, {}).get(top)
+    if per_unit and units_per_launch:
+        traffic = {"bytes_per_launch": per_unit * units_per_launch, "algorithmic_bytes_per_launch":
+                   bytes_per_unit[top] * units_per_launch, "units_per_launch": units_per_launch,
+                   "source": "profiles/r01d_summary.md (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum per "
+                             "state*gridpoint of one launch, scaled to this run's launch size)"}
     return {"kernel": top, "bound": "hbm", "achieved": round(achieved, 1), "peak": peak_gbs, "unit": "GB/s",
-            "frac": round(achieved / peak_gbs, 4), "traffic": None, "peak_source": peak_src,
+            "frac": round(achieved / peak_gbs, 4), "traffic": traffic, "peak_source": peak_src,
             "algorithmic_bytes_per_unit": bytes_per_unit[top], "units_per_step": units,
             "share_of_step": round(cand[top] / sum(kern_s.values()), 4), "all_kernels": others,
             "note": "achieved = algorithmic bytes of all launches of this family in one step / their summed CUDA-event "
-                    "time (separate profiling pass of the same steps); traffic (ncu dram bytes) is in profiles/"}
+                    "time (separate profiling pass of the same steps)"}
 
 
 def cpu_baseline(cfg, wl, sample_states):
@@ -405,7 +420,8 @@ def main():
     # ---- per-kernel times (same steps, library events on the launching stream) -> roofline of the dominant family
     kern_s, _ = kernel_breakdown(torch, g, fn, max(1, min(args.steps, 5)))
     peak, peak_src = measured_peaks()
-    roof = roofline_of(kern_s, units, peak, peak_src, alg_bytes(wl))
+    states_per_launch = args.chunk or max(1, min(nst, (1 << 30) // (cfg.npts * 16)))   # the library's default chunk
+    roof = roofline_of(kern_s, units, peak, peak_src, alg_bytes(wl), args.workload, states_per_launch * cfg.npts)
 
     # ---- end to end through the host-buffer entry point (pinned host in/out, copies inside the timed region)
     e2e = None

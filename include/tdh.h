@@ -113,7 +113,7 @@ int tdh_last_launch_count(const tdh_grid* g);
 /* Seconds (device time, CUDA events on the handle's stream) spent in each kernel family during the last call, when
  * profiling was switched on with tdh_set_profiling(g, 1); profiling inserts events and synchronises at the end.
  * out[0..TDH_NKERNELS-1]; order given by tdh_kernel_name(i).  Off by default. */
-#define TDH_NKERNELS 4
+#define TDH_NKERNELS 5
 int tdh_set_profiling(tdh_grid* g, int on);
 int tdh_last_kernel_seconds(const tdh_grid* g, double out[TDH_NKERNELS]);
 const char* tdh_kernel_name(int i);

@@ -28,7 +28,7 @@ SYMBOLS = (
     "tdh_propagate", "tdh_apply_hamiltonian_host", "tdh_propagate_host", "tdh_fft3d", "tdh_last_launch_count",
     "tdh_set_profiling", "tdh_last_kernel_seconds", "tdh_kernel_name", "tdh_set_chunk_states", "tdh_last_error",
 )
-NKERNELS = 4
+NKERNELS = 5
 
 TDH_OK, TDH_EINVAL, TDH_EUNSUPPORTED, TDH_ENOMEM, TDH_ECUDA, TDH_EINDEX = 0, -1, -2, -3, -4, -5
 

@@ -129,4 +129,106 @@ nl_project_kernel(const cd* __restrict__ psi, size_t npts, int nst, const AtomDe
     }
 }
 
+
+// ------------------------------------------------------------------------------------------------------------
+// Back-projection (second half of Eq. 9):   out_s[S_I[q]] += alpha e^{-ik.d_q} sum_c beta_{I,c}[q] dpi[s][c]
+// The mirror image of the projection: a real (P_I x C_I) matrix times the complex (C_I x n_st) coefficients, added
+// into the sphere's grid points of the output block.  A CTA owns one atom and 8 states, its warps split the sphere in
+// blocks of 8 points; per block and per tile of 4 channels
+//     mma.sync.m8n8k4.f64   D(8 points x 8 states) += A(8 points x 4 chan) * B(4 chan x 8 states)
+// twice (real and imaginary parts of dpi; B is loop invariant and stays in registers).  Lane l then holds the sums of
+// point q0 + l/4 for the two states s0 + 2*(l%4) + {0,1} and read-modify-writes those two values: for one state the 8
+// lanes l/4 = 0..7 touch 8 consecutive sphere points = up to 128 contiguous bytes (a sphere is z-runs of grid points).
+// NLS_BLOCKS blocks are in flight per warp, and the indices / projector values of the next iteration are requested
+// while this iteration's loads travel (one DRAM round trip per iteration).
+// ATOMIC FREE: one launch covers a set of atoms whose spheres share no grid point (the host colours the atoms), a
+// point appears once per sphere, CTAs of one atom own different states -- plain loads and stores, deterministic.
+// ------------------------------------------------------------------------------------------------------------
+constexpr int NLS_WARPS = 8;
+constexpr int NLS_BLOCKS = 4;
+
+// grid: (atoms of this colour, ceil(nst / 8)); KT = number of 4-channel tiles (C_I <= 4*KT)
+template <int KT>
+__global__ void __launch_bounds__(32 * NLS_WARPS)
+nl_scatter_kernel(cd* __restrict__ out, size_t npts, int nst, const AtomDesc* __restrict__ atoms,
+                  const int* __restrict__ sidx, const double* __restrict__ sbeta, const cd* __restrict__ sphase,
+                  const cd* __restrict__ dpi, int nchan_tot, cd alpha)
+{
+    const AtomDesc at = atoms[blockIdx.x];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int kq = lane & 3, r8 = lane >> 2;
+    const int s0 = blockIdx.y * NLP_STATES;
+    // B fragments: B[k = kq][n = r8] = alpha * dpi[s0 + r8][chan0 + 4*kt + kq]
+    double bre[KT], bim[KT];
+#pragma unroll
+    for (int kt = 0; kt < KT; ++kt) {
+        const int c = 4 * kt + kq, s = s0 + r8;
+        cd v = make_double2(0.0, 0.0);
+        if (c < at.nchan && s < nst) v = cmul(alpha, __ldg(dpi + (size_t)s * nchan_tot + at.chan0 + c));
+        bre[kt] = v.x;
+        bim[kt] = v.y;
+    }
+    // C fragment: row = point q0 + 8u + r8, columns = states sa, sa + 1
+    const int sa = s0 + 2 * kq;
+    const bool ok0 = sa < nst, ok1 = sa + 1 < nst;
+    cd* o0 = out + (size_t)(ok0 ? sa : 0) * npts;
+    cd* o1 = out + (size_t)(ok1 ? sa + 1 : 0) * npts;
+    const int* idx = sidx + at.q0;
+    const cd* phs = sphase ? sphase + at.q0 : nullptr;
+
+    constexpr int STRIDE = NLS_WARPS * 8 * NLS_BLOCKS;
+    int ix[NLS_BLOCKS];
+    double af[NLS_BLOCKS][KT];
+    auto load_meta = [&](int q0, int (&ixo)[NLS_BLOCKS], double (&afo)[NLS_BLOCKS][KT]) {
+#pragma unroll
+        for (int u = 0; u < NLS_BLOCKS; ++u) {
+            const int q = q0 + 8 * u + r8;
+            const bool q_ok = q < at.np;
+            ixo[u] = q_ok ? __ldg(idx + q) : -1;
+#pragma unroll
+            for (int kt = 0; kt < KT; ++kt) {
+                const int c = 4 * kt + kq;                                  // A fragment column = channel
+                afo[u][kt] = (q_ok && c < at.nchan) ? __ldg(sbeta + at.boff + (size_t)c * at.np + q) : 0.0;
+            }
+        }
+    };
+    int q0 = warp * 8 * NLS_BLOCKS;
+    if (q0 < at.np) load_meta(q0, ix, af);
+    for (; q0 < at.np; q0 += STRIDE) {
+        cd v0[NLS_BLOCKS], v1[NLS_BLOCKS];
+#pragma unroll
+        for (int u = 0; u < NLS_BLOCKS; ++u) {
+            v0[u] = v1[u] = make_double2(0.0, 0.0);
+            if (ix[u] >= 0 && ok0) v0[u] = o0[ix[u]];
+            if (ix[u] >= 0 && ok1) v1[u] = o1[ix[u]];
+        }
+        int ixn[NLS_BLOCKS];
+        double afn[NLS_BLOCKS][KT];
+        if (q0 + STRIDE < at.np) load_meta(q0 + STRIDE, ixn, afn);
+#pragma unroll
+        for (int u = 0; u < NLS_BLOCKS; ++u) {
+            double cre[2] = {0.0, 0.0}, cim[2] = {0.0, 0.0};
+#pragma unroll
+            for (int kt = 0; kt < KT; ++kt) {
+                dmma_m8n8k4(cre, af[u][kt], bre[kt]);
+                dmma_m8n8k4(cim, af[u][kt], bim[kt]);
+            }
+            cd a0 = make_double2(cre[0], cim[0]), a1 = make_double2(cre[1], cim[1]);
+            if (phs != nullptr && ix[u] >= 0) {
+                const cd ph = __ldg(phs + q0 + 8 * u + r8);
+                a0 = cmulc(a0, ph);
+                a1 = cmulc(a1, ph);
+            }
+            if (ix[u] >= 0 && ok0) o0[ix[u]] = cadd(v0[u], a0);
+            if (ix[u] >= 0 && ok1) o1[ix[u]] = cadd(v1[u], a1);
+        }
+#pragma unroll
+        for (int u = 0; u < NLS_BLOCKS; ++u) {
+            ix[u] = ixn[u];
+#pragma unroll
+            for (int kt = 0; kt < KT; ++kt) af[u][kt] = afn[u][kt];
+        }
+    }
+}
+
 }  // namespace tdh

@@ -59,8 +59,8 @@ extern "C" const char* tdh_last_error(void) { return g_err; }
 // ------------------------------------------------------------------------------------------------------------
 // handle
 // ------------------------------------------------------------------------------------------------------------
-enum { K_NLPROJ = 0, K_PLANE_FWD = 1, K_XPENCIL = 2, K_PLANE_INV = 3 };
-static const char* const kKernelNames[TDH_NKERNELS] = {"nl_project", "plane_fwd", "xpencil", "plane_inv"};
+enum { K_NLPROJ = 0, K_PLANE_FWD = 1, K_XPENCIL = 2, K_PLANE_INV = 3, K_NLSCATTER = 4 };
+static const char* const kKernelNames[TDH_NKERNELS] = {"nl_project", "plane_fwd", "xpencil", "plane_inv", "nl_scatter"};
 
 struct ProfRec { cudaEvent_t a, b; int k; };
 
@@ -106,6 +106,11 @@ struct tdh_grid {
     double* d_nl_beta;
     cd* d_nl_phase;
     int nl_layers, nl_nrec, nl_cmax;
+    // separate back-projection kernel: atoms grouped by colour (spheres of one colour share no grid point)
+    int nl_mode;                       // 1: nl_scatter kernel per colour after plane_inv; 0: records inside plane_inv
+    tdh::AtomDesc* d_atoms_col;        // atoms sorted by colour
+    std::vector<int> col_off;          // [ncolours + 1] offsets into d_atoms_col
+    int kt;                            // 4-channel tiles of the back-projection MMA
 
     // host-buffer path
     int host_chunk;
@@ -141,6 +146,7 @@ static int freq_index(int a, int n) {
 
 static void free_projectors(tdh_grid* g) {
     cudaFree(g->d_atoms); cudaFree(g->d_sidx); cudaFree(g->d_sbeta); cudaFree(g->d_sphase); cudaFree(g->d_dscale);
+    cudaFree(g->d_atoms_col); g->d_atoms_col = nullptr; g->col_off.clear();
     cudaFree(g->d_dpi); cudaFree(g->d_nl_off); cudaFree(g->d_nl_cc); cudaFree(g->d_nl_beta); cudaFree(g->d_nl_phase);
     g->d_atoms = nullptr; g->d_sidx = nullptr; g->d_sbeta = nullptr; g->d_sphase = nullptr; g->d_dscale = nullptr;
     g->d_dpi = nullptr; g->d_nl_off = nullptr; g->d_nl_cc = nullptr; g->d_nl_beta = nullptr; g->d_nl_phase = nullptr;
@@ -388,6 +394,32 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
         atoms[a].q0 = (int)q0; atoms[a].np = pn; atoms[a].boff = (int)boff; atoms[a].chan0 = c0; atoms[a].nchan = nc;
         boff += (size_t)nc * pn;
     }
+    // ---- colours for the separate back-projection kernel: greedy, an atom takes the lowest colour that no atom sharing
+    //      a grid point with it has taken (per-point bit mask of the colours already present)
+    std::vector<tdh::AtomDesc> atoms_col;
+    std::vector<int> col_off;
+    {
+        std::vector<unsigned> pmask(g->np, 0u);
+        std::vector<int> colour(natoms, 0);
+        int ncol = 0;
+        for (int a = 0; a < natoms; ++a) {
+            unsigned used = 0u;
+            for (int j = 0; j < atoms[a].np; ++j) used |= pmask[sidx[atoms[a].q0 + j]];
+            int c = 0;
+            while (c < 32 && (used >> c & 1u)) ++c;
+            if (c == 32) return fail(TDH_EUNSUPPORTED, "tdh_set_projectors: more than 32 spheres overlap transitively at atom %d", a);
+            colour[a] = c;
+            ncol = std::max(ncol, c + 1);
+            for (int j = 0; j < atoms[a].np; ++j) pmask[sidx[atoms[a].q0 + j]] |= 1u << c;
+        }
+        col_off.assign(ncol + 1, 0);
+        for (int c = 0; c < ncol; ++c) {
+            col_off[c] = (int)atoms_col.size();
+            for (int a = 0; a < natoms; ++a)
+                if (colour[a] == c) atoms_col.push_back(atoms[a]);
+        }
+        col_off[ncol] = (int)atoms_col.size();
+    }
     // ---- back-projection records: one per (atom, sphere point), grouped by tile (x, r) and by layer.  The layer of a
     //      record is the number of earlier atoms covering the same grid point, so no two records of one (tile, layer)
     //      share a shared-memory cell and the scatter needs no atomics.  The cell address follows tile_kernels.cuh.
@@ -452,7 +484,7 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
         return TDH_OK;
     };
     int rc;
-    if ((rc = up(&g->d_atoms, atoms)) || (rc = up(&g->d_sidx, sidx)) || (rc = up(&g->d_sbeta, sbeta)) ||
+    if ((rc = up(&g->d_atoms_col, atoms_col)) || (rc = up(&g->d_atoms, atoms)) || (rc = up(&g->d_sidx, sidx)) || (rc = up(&g->d_sbeta, sbeta)) ||
         (rc = up(&g->d_sphase, sphase)) || (rc = up(&g->d_dscale, dscale)) || (rc = up(&g->d_nl_off, nl_off)) ||
         (rc = up(&g->d_nl_cc, rec_cc)) || (rc = up(&g->d_nl_beta, rec_beta)) || (rc = up(&g->d_nl_phase, rec_phase))) {
         free_projectors(g);
@@ -470,6 +502,12 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
     g->nl_nrec = (int)ptot;
     g->nl_cmax = cpad;
     g->mt = cmax <= 8 ? 1 : 2;
+    g->kt = (cmax + 3) / 4;
+    g->col_off = col_off;
+    // Measured on B200 (profiles/r01e_summary.md): the separate kernel wins on the split (half-plane) tiles of the large
+    // grids, the records inside plane_inv win on whole-plane tiles.  TDH_NL_MODE=0/1 overrides (tests run both).
+    g->nl_mode = g->tl.s == 2 ? 1 : 0;
+    if (const char* e = getenv("TDH_NL_MODE")) g->nl_mode = atoi(e) != 0;
     return TDH_OK;
 }
 
@@ -640,6 +678,26 @@ static int launch_nl_project(tdh_grid* g, int nst, const cd* in) {
     return TDH_OK;
 }
 
+// out += alpha * V_nl phi from the coefficients nl_project left in d_dpi: one launch per colour
+static int launch_nl_scatter(tdh_grid* g, int nst, cd* out, cd alpha) {
+    size_t npts = g->np;
+    const int* sidx = g->d_sidx;
+    const double* sbeta = g->d_sbeta;
+    const cd* sphase = g->d_sphase;
+    const cd* dpi = g->d_dpi;
+    int nct = g->nchan_tot;
+    const void* fs[4] = {reinterpret_cast<const void*>(&tdh::nl_scatter_kernel<1>), reinterpret_cast<const void*>(&tdh::nl_scatter_kernel<2>),
+                         reinterpret_cast<const void*>(&tdh::nl_scatter_kernel<3>), reinterpret_cast<const void*>(&tdh::nl_scatter_kernel<4>)};
+    for (size_t c = 0; c + 1 < g->col_off.size(); ++c) {
+        const tdh::AtomDesc* atoms = g->d_atoms_col + g->col_off[c];
+        void* args[] = {(void*)&out, (void*)&npts, (void*)&nst, (void*)&atoms, (void*)&sidx, (void*)&sbeta,
+                        (void*)&sphase, (void*)&dpi, (void*)&nct, (void*)&alpha};
+        dim3 grid(g->col_off[c + 1] - g->col_off[c], (nst + tdh::NLP_STATES - 1) / tdh::NLP_STATES);
+        LAUNCH(K_NLSCATTER, fs[g->kt - 1], grid, dim3(32 * tdh::NLS_WARPS), 0, args);
+    }
+    return TDH_OK;
+}
+
 // out = alpha * H in + yv   for one chunk (nst <= chunk_cap); in/out/yv point at the chunk's first state
 static int apply_chunk(tdh_grid* g, int nst, const cd* in, cd* out, cd alpha, const cd* yv) {
     int rc;
@@ -648,11 +706,12 @@ static int apply_chunk(tdh_grid* g, int nst, const cd* in, cd* out, cd alpha, co
     if ((rc = launch_xpencil(g, nst, g->d_work, g->d_work, 0))) return rc;
     tdh::Epilogue ep;
     memset(&ep, 0, sizeof(ep));
-    ep.v = (g->have_v || g->natoms > 0) ? g->d_v : nullptr;   // zero-filled until set; required with projectors
+    const bool fused_nl = g->natoms > 0 && g->nl_mode == 0;
+    ep.v = (g->have_v || fused_nl) ? g->d_v : nullptr;        // zero-filled until set; required with the fused records
     ep.yv = yv;
     ep.alpha = alpha;
     ep.nx = g->n[0];
-    if (g->natoms > 0) {
+    if (fused_nl) {
         ep.nl_off = g->d_nl_off;
         ep.nl_layers = g->nl_layers;
         ep.nl_cc = g->d_nl_cc;
@@ -663,7 +722,9 @@ static int apply_chunk(tdh_grid* g, int nst, const cd* in, cd* out, cd alpha, co
         ep.cmax = g->nl_cmax;
         ep.nchan_tot = g->nchan_tot;
     }
-    return launch_plane_inv(g, nst, g->d_work, in, out, ep);
+    if ((rc = launch_plane_inv(g, nst, g->d_work, in, out, ep))) return rc;
+    if (g->natoms > 0 && !fused_nl) return launch_nl_scatter(g, nst, out, alpha);
+    return TDH_OK;
 }
 
 static int apply_block(tdh_grid* g, int nst, const cd* psi, cd* hpsi) {

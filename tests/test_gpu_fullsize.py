@@ -149,3 +149,26 @@ def test_many_channels_and_three_overlapping_spheres(torch_cuda, B, oracle, n, n
         g.propagate(d, 0.01, 2)
         ref_p = oracle.propagate(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, v, proj, psi, 0.01, 2, 4, oracle.NAIVE_FFT)
         assert per_state_rel(d.cpu().numpy(), ref_p).max() < TOL
+
+
+@pytest.mark.parametrize("mode", ["0", "1"])
+def test_both_back_projection_paths(torch_cuda, B, oracle, monkeypatch, mode):
+    """The back-projection exists as records fused into plane_inv (TDH_NL_MODE=0) and as the coloured nl_scatter kernel
+    (TDH_NL_MODE=1); the library picks one per grid.  Both must match the oracle on split and whole-plane tiles."""
+    torch = torch_cuda
+    monkeypatch.setenv("TDH_NL_MODE", mode)
+    for cid, n, natoms, lmax in [(260, (32, 96, 96), 6, 1), (261, (48, 48, 32), 7, 2), (262, (16, 16, 16), 3, 0)]:
+        cfg = W.test_config(cid, n, tuple(0.42 * m for m in n), nst=11, natoms=natoms, lmax=lmax, rc=2.9,
+                            dl=(2.0, -0.8, 0.3)[: lmax + 1], kfrac=(0.1, 0.0, -0.2) if cid == 261 else (0.0, 0.0, 0.0))
+        wl = W.make(cfg)
+        psi = W.states(cfg)
+        ref = oracle.apply_workload(wl, psi, oracle.NAIVE_FFT)
+        with B.grid_for(wl) as g:
+            d = torch.from_numpy(psi).cuda()
+            out = g.apply_hamiltonian(d)
+            n_launch = g.last_launch_count()
+            assert per_state_rel(out.cpu().numpy(), ref).max() < TOL
+            assert (n_launch > 4) == (mode == "1")
+            g.propagate(d, 0.01, 1)
+            ref_p = oracle.propagate_workload(wl, psi, dt=0.01, nsteps=1, backend=oracle.NAIVE_FFT)
+            assert per_state_rel(d.cpu().numpy(), ref_p).max() < TOL
