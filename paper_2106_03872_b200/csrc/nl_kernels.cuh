@@ -32,7 +32,8 @@ constexpr int NLP_WARPS = 8;     // warps per CTA, splitting the sphere
 constexpr int NLP_STATES = 8;    // states per CTA (the N of the MMA)
 constexpr int NLP_KSTEPS = 8;    // k-steps (of 4 points) per block: 32 points, 8 gathers in flight per lane
 
-// grid: (natoms, ceil(nst / 8)); MT = number of 8-channel tiles (C_I <= 8*MT)
+// grid: (ceil(nst / 8), natoms) -- the state groups of one atom are neighbours in launch order, run together and share
+// the atom's index and projector tables through L2; MT = number of 8-channel tiles (C_I <= 8*MT)
 template <int MT>
 __global__ void __launch_bounds__(32 * NLP_WARPS)
 nl_project_kernel(const cd* __restrict__ psi, size_t npts, int nst, const AtomDesc* __restrict__ atoms,
@@ -40,10 +41,10 @@ nl_project_kernel(const cd* __restrict__ psi, size_t npts, int nst, const AtomDe
                   const double* __restrict__ dscale, cd* __restrict__ dpi, int nchan_tot)
 {
     __shared__ double part[NLP_WARPS][MT][4][32];
-    const AtomDesc at = atoms[blockIdx.x];
+    const AtomDesc at = atoms[blockIdx.y];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int kq = lane & 3, r8 = lane >> 2;
-    const int s0 = blockIdx.y * NLP_STATES;
+    const int s0 = blockIdx.x * NLP_STATES;
     const int s = s0 + r8;                                      // this lane's state (B fragment column)
     const bool s_ok = s < nst;
     const cd* ps = psi + (size_t)(s_ok ? s : 0) * npts;
@@ -147,17 +148,17 @@ nl_project_kernel(const cd* __restrict__ psi, size_t npts, int nst, const AtomDe
 constexpr int NLS_WARPS = 8;
 constexpr int NLS_BLOCKS = 4;
 
-// grid: (atoms of this colour, ceil(nst / 8)); KT = number of 4-channel tiles (C_I <= 4*KT)
+// grid: (ceil(nst / 8), atoms of this colour); KT = number of 4-channel tiles (C_I <= 4*KT)
 template <int KT>
 __global__ void __launch_bounds__(32 * NLS_WARPS)
 nl_scatter_kernel(cd* __restrict__ out, size_t npts, int nst, const AtomDesc* __restrict__ atoms,
                   const int* __restrict__ sidx, const double* __restrict__ sbeta, const cd* __restrict__ sphase,
                   const cd* __restrict__ dpi, int nchan_tot, cd alpha)
 {
-    const AtomDesc at = atoms[blockIdx.x];
+    const AtomDesc at = atoms[blockIdx.y];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int kq = lane & 3, r8 = lane >> 2;
-    const int s0 = blockIdx.y * NLP_STATES;
+    const int s0 = blockIdx.x * NLP_STATES;
     // B fragments: B[k = kq][n = r8] = alpha * dpi[s0 + r8][chan0 + 4*kt + kq]
     double bre[KT], bim[KT];
 #pragma unroll

@@ -157,7 +157,9 @@ static void free_projectors(tdh_grid* g) {
 static int default_chunk(const tdh_grid* g) {
     // Measured on B200 (profiles/r01a_chunk_sweep.md): every kernel gets faster with more states per launch and the
     // L2-resident small-chunk variant never wins, so the default is the largest chunk the workspace holds.
-    int c = g->chunk_cap;
+    // When a block has to be split anyway: a multiple of 8 states (the N of the projector MMAs), so that no state group
+    // of the non-local kernels is ragged.
+    int c = (g->chunk_cap < g->max_states && g->chunk_cap >= 8) ? g->chunk_cap / 8 * 8 : g->chunk_cap;
     if (const char* e = getenv("TDH_CHUNK_STATES")) { int v = atoi(e); if (v > 0) c = v; }
     return std::max(1, std::min(c, g->chunk_cap));
 }
@@ -335,6 +337,7 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
     CU(cudaStreamSynchronize(g->stream));
     free_projectors(g);
     if (natoms == 0) return TDH_OK;
+    if (natoms > 65535) return fail(TDH_EUNSUPPORTED, "tdh_set_projectors: more than 65535 atoms");
     if (!sph_off || !sph_idx || !chan_off || !beta || !dcoef)
         return fail(TDH_EINVAL, "tdh_set_projectors: null table with natoms > 0");
     if (g->have_k && !sph_disp) return fail(TDH_EINVAL, "tdh_set_projectors: sph_disp is required when k != 0");
@@ -673,7 +676,7 @@ static int launch_nl_project(tdh_grid* g, int nst, const cd* in) {
                     (void*)&sphase, (void*)&dscale, (void*)&dpi, (void*)&nct};
     const void* f = g->mt == 1 ? reinterpret_cast<const void*>(&tdh::nl_project_kernel<1>)
                                : reinterpret_cast<const void*>(&tdh::nl_project_kernel<2>);
-    dim3 grid(g->natoms, (nst + tdh::NLP_STATES - 1) / tdh::NLP_STATES);   // y <= 65535: nst <= 524280 per chunk
+    dim3 grid((nst + tdh::NLP_STATES - 1) / tdh::NLP_STATES, g->natoms);   // y <= 65535 atoms
     LAUNCH(K_NLPROJ, f, grid, dim3(32 * tdh::NLP_WARPS), 0, args);
     return TDH_OK;
 }
@@ -692,7 +695,7 @@ static int launch_nl_scatter(tdh_grid* g, int nst, cd* out, cd alpha) {
         const tdh::AtomDesc* atoms = g->d_atoms_col + g->col_off[c];
         void* args[] = {(void*)&out, (void*)&npts, (void*)&nst, (void*)&atoms, (void*)&sidx, (void*)&sbeta,
                         (void*)&sphase, (void*)&dpi, (void*)&nct, (void*)&alpha};
-        dim3 grid(g->col_off[c + 1] - g->col_off[c], (nst + tdh::NLP_STATES - 1) / tdh::NLP_STATES);
+        dim3 grid((nst + tdh::NLP_STATES - 1) / tdh::NLP_STATES, g->col_off[c + 1] - g->col_off[c]);
         LAUNCH(K_NLSCATTER, fs[g->kt - 1], grid, dim3(32 * tdh::NLS_WARPS), 0, args);
     }
     return TDH_OK;
