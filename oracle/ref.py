@@ -26,7 +26,7 @@ def lib() -> C.CDLL:
     if _lib is None:
         _lib = C.CDLL(_build.build())
         for name in ("ref_dft3d", "ref_kinetic", "ref_local", "ref_nonlocal", "ref_apply_hamiltonian",
-                     "ref_propagate", "ref_num_threads"):
+                     "ref_propagate", "ref_taylor_pair", "ref_etrs_step", "ref_num_threads"):
             getattr(_lib, name).restype = C.c_int
     return _lib
 
@@ -134,6 +134,31 @@ def propagate(n, length, kpt, ecut, v, proj, psi, dt: float, nsteps: int, order:
                                _ptr(psi), C.c_double(dt), C.c_int(nsteps), C.c_int(order), C.c_int(backend)),
            "propagate")
     return psi
+
+
+def taylor_pair(n, length, kpt, ecut, v, proj, psi, dt: float, order: int = 4, backend: int = NAIVE_FFT):
+    """(exp(-i dt/2 H) psi, exp(-i dt H) psi) from one chain of powers H^k psi.  Returns new arrays."""
+    psi = _c128(psi)
+    half, full = np.empty_like(psi), np.empty_like(psi)
+    nst = 1 if psi.ndim == 3 else psi.shape[0]
+    v = None if v is None else np.ascontiguousarray(v, dtype=np.float64)
+    p = _Proj(proj)
+    _check(lib().ref_taylor_pair(_i3(n), _d3(length), _d3(kpt), C.c_double(ecut), _ptr(v), *p.args, C.c_int(nst), _ptr(psi),
+                                 _ptr(half), _ptr(full), C.c_double(dt), C.c_int(order), C.c_int(backend)), "taylor_pair")
+    return half, full
+
+
+def etrs_step(n, length, kpt, ecut, v, v_next, proj, psi, dt: float, backend: int = NAIVE_FFT):
+    """One ETRS step (Eq. 6-7) with V(t+dt) = v_next supplied.  Returns (psi(t+dt), approx = exp(-i dt H(t)) psi(t))."""
+    out = _c128(psi).copy()
+    approx = np.empty_like(out)
+    nst = 1 if out.ndim == 3 else out.shape[0]
+    v = None if v is None else np.ascontiguousarray(v, dtype=np.float64)
+    v_next = None if v_next is None else np.ascontiguousarray(v_next, dtype=np.float64)
+    p = _Proj(proj)
+    _check(lib().ref_etrs_step(_i3(n), _d3(length), _d3(kpt), C.c_double(ecut), _ptr(v), _ptr(v_next), *p.args, C.c_int(nst),
+                               _ptr(out), _ptr(approx), C.c_double(dt), C.c_int(backend)), "etrs_step")
+    return out, approx
 
 
 def apply_workload(wl, psi, backend: int = NAIVE_FFT) -> np.ndarray:

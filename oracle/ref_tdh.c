@@ -16,6 +16,7 @@
  *     V_nl psi = sum_I sum_c beta_Ic(r-R_I) D_Ic dV sum_{r' in sphere} beta_Ic(r'-R_I) psi(r')
  *                                                                      Eq. 9; readings R2-R5
  *   exp(-i dt H) psi ~= sum_{k=0..4} (-i dt)^k / k!  H^k psi           Eq. 8
+ *   ETRS step (Eq. 6-7) from two such sums sharing H^k psi, V(t+dt) supplied
  *
  * Two DFT back-ends: backend 0 = direct O(N^2)-per-pencil sum (the definition), backend 1 = a separately
  * written recursive radix-2/3 decimation-in-time FFT (only to make the large configs affordable; it is
@@ -24,7 +25,8 @@
  * Pins (tests/test_oracle_pins.py): P1 brute-force 3-D DFT / round trip / Parseval, P2 plane waves are
  * kinetic eigenvectors incl. Nyquist and mask, P3 constant potential = shift, P4 rank / closed form of one
  * projector, P5 Hermiticity and dense-matrix spectrum, P6 Bloch-phase identity and translation covariance,
- * P7 closed-form Taylor propagation of kinetic-only H, P8 independence of batching.  The paper prints no
+ * P7 closed-form Taylor propagation of kinetic-only H, P8 independence of batching, P9 ETRS against dense
+ * matrix polynomials and the kinetic-only closed form.  The paper prints no
  * worked H.psi example, so beyond P1-P8 parity is unpinned by the paper (stated in DESIGN.md).
  *
  * Build: gcc -O2 -std=c99 -fopenmp -shared -fPIC ref_tdh.c -o libref_tdh.so -lm   (oracle/build.py)
@@ -406,6 +408,90 @@ int ref_propagate(const int n[3], const double len[3], const double kpt[3], doub
         }
     }
     return err;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * exported (NEXT-1): the two exponentials of one ETRS step that share their powers H^k psi.
+ * "we can evaluate this expression for several values of lambda for almost the same cost
+ * of a single value, since lambda only appears as a multiplicative coefficient".  Eq. 8 for
+ * lambda_1 = -i dt/2 and lambda_2 = -i dt, literally:
+ *   half = full = psi;  phi_0 = psi;  for k = 1..order:  phi_k = H phi_{k-1};
+ *       half += (-i dt/2)^k / k! phi_k;   full += (-i dt)^k / k! phi_k.
+ * psi is not modified.
+ * ------------------------------------------------------------------------------------------------ */
+int ref_taylor_pair(const int n[3], const double len[3], const double kpt[3], double ecut, const double *v, int natoms,
+                    const int64_t *sph_off, const int32_t *sph_idx, const double *sph_disp, const int32_t *chan_off,
+                    const double *beta, const double *dcoef, int nst, const cplx *psi, cplx *half, cplx *full, double dt,
+                    int order, int backend)
+{
+    if (check_geometry(n, len) || !kpt || !psi || !half || !full || nst < 0 || order < 1 || order > 16) return REF_EINVAL;
+    if (check_projectors(n, natoms, sph_off, sph_idx, chan_off, beta, dcoef)) return REF_EINVAL;
+    const size_t np_ = npoints(n);
+    int err = REF_OK;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int s = 0; s < nst; ++s) {
+        const cplx *x = psi + (size_t)s * np_;
+        cplx *h = half + (size_t)s * np_, *f = full + (size_t)s * np_;
+        cplx *phi = (cplx *)malloc(sizeof(cplx) * np_);
+        cplx *hphi = (cplx *)malloc(sizeof(cplx) * np_);
+        int e = (phi && hphi) ? REF_OK : REF_ENOMEM;
+        if (e == REF_OK) {
+            memcpy(phi, x, sizeof(cplx) * np_);
+            memcpy(h, x, sizeof(cplx) * np_);
+            memcpy(f, x, sizeof(cplx) * np_);
+        }
+        cplx ch = 1.0, cf = 1.0;
+        for (int k = 1; k <= order && e == REF_OK; ++k) {
+            e = hamiltonian_one(n, len, kpt, ecut, v, natoms, sph_off, sph_idx, sph_disp, chan_off, beta, dcoef, phi, hphi,
+                                backend);
+            ch *= (-I * (0.5 * dt)) / (double)k; /* (-i dt/2)^k / k! */
+            cf *= (-I * dt) / (double)k;         /* (-i dt)^k / k!   */
+            for (size_t p = 0; p < np_; ++p) {
+                h[p] += ch * hphi[p];
+                f[p] += cf * hphi[p];
+            }
+            cplx *t = phi; phi = hphi; hphi = t;
+        }
+        free(phi);
+        free(hphi);
+        if (e != REF_OK) {
+#pragma omp critical
+            err = e;
+        }
+    }
+    return err;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * exported (NEXT-1): one ETRS step, Eq. 6-7, with the potential at t+dt supplied by the
+ * caller (the density -> potential map needs the XC functional, which is outside this path):
+ *   approx = exp(-i dt H(t)) psi          Eq. 7  (returned; the caller derives V(t+dt) from it BEFORE calling
+ *                                                 when V(t+dt) depends on it -- here v_next is an input)
+ *   psi   <- exp(-i dt/2 H(t+dt)) exp(-i dt/2 H(t)) psi        Eq. 6
+ * Every exponential is the order-4 Taylor sum of Eq. 8.  H(t) uses v, H(t+dt) uses v_next; the projectors
+ * are the same in both (fixed ions).  approx may be NULL.
+ * ------------------------------------------------------------------------------------------------ */
+int ref_etrs_step(const int n[3], const double len[3], const double kpt[3], double ecut, const double *v,
+                  const double *v_next, int natoms, const int64_t *sph_off, const int32_t *sph_idx, const double *sph_disp,
+                  const int32_t *chan_off, const double *beta, const double *dcoef, int nst, cplx *psi, cplx *approx,
+                  double dt, int backend)
+{
+    if (!psi || nst < 0) return REF_EINVAL;
+    const size_t np_ = npoints(n);
+    cplx *half = (cplx *)malloc(sizeof(cplx) * np_ * (size_t)(nst > 0 ? nst : 1));
+    cplx *full = approx ? approx : (cplx *)malloc(sizeof(cplx) * np_ * (size_t)(nst > 0 ? nst : 1));
+    int e = (half && full) ? REF_OK : REF_ENOMEM;
+    if (e == REF_OK)
+        e = ref_taylor_pair(n, len, kpt, ecut, v, natoms, sph_off, sph_idx, sph_disp, chan_off, beta, dcoef, nst, psi, half,
+                            full, dt, 4, backend);
+    if (e == REF_OK) {
+        memcpy(psi, half, sizeof(cplx) * np_ * (size_t)nst);
+        e = ref_propagate(n, len, kpt, ecut, v_next, natoms, sph_off, sph_idx, sph_disp, chan_off, beta, dcoef, nst, psi,
+                          0.5 * dt, 1, 4, backend);
+    }
+    free(half);
+    if (!approx) free(full);
+    return e;
 }
 
 /* number of OpenMP threads the block loops will use (reported by bench.py's cpu_baseline) */

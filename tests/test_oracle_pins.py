@@ -329,6 +329,67 @@ def test_p7_propagate_is_literal_eq8(oracle):
     assert rel(two, oracle.propagate_workload(wl, acc, dt=dt, nsteps=1, backend=0)) < 1e-13
 
 
+# --------------------------------------------------------------------------------------------- P9 (NEXT-1: ETRS)
+def poly4(m, lam):
+    """sum_{k=0..4} (lam m)^k / k! of a dense matrix m, by explicit matrix powers (numpy, independent of the oracle's loop)."""
+    a = lam * m
+    a2 = a @ a
+    return np.eye(m.shape[0], dtype=np.complex128) + a + a2 / 2.0 + (a2 @ a) / 6.0 + (a2 @ a2) / 24.0
+
+
+def test_p9_taylor_pair_against_dense_matrix_polynomials(oracle):
+    """both exponentials from one chain.  half = P4(-i dt/2 H) psi, full = P4(-i dt H) psi, with H the
+    dense small-grid matrix (pinned by P1-P6) and the polynomials formed by matrix products."""
+    cfg = small_cfg(111, n=(4, 5, 6), length=(4.4, 5.0, 5.5), natoms=2, lmax=1, rc=1.9, kfrac=(0.0, 0.2, -0.1))
+    wl = W.make(cfg)
+    h = dense_matrix(oracle, cfg, wl)
+    psi = W.states(cfg)
+    dt = 0.06
+    half, full = oracle.taylor_pair(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, wl.v, wl.proj, psi, dt, 4, 0)
+    flat = psi.reshape(psi.shape[0], -1).T
+    assert rel(half.reshape(psi.shape[0], -1).T, poly4(h, -0.5j * dt) @ flat) < 1e-13
+    assert rel(full.reshape(psi.shape[0], -1).T, poly4(h, -1j * dt) @ flat) < 1e-13
+    # and the two agree with the single-lambda routine pinned by P7
+    assert rel(half, oracle.propagate_workload(wl, psi, dt=0.5 * dt, nsteps=1, backend=0)) < 1e-14
+    assert rel(full, oracle.propagate_workload(wl, psi, dt=dt, nsteps=1, backend=0)) < 1e-14
+
+
+def test_p9_etrs_step_against_dense_matrices_with_two_potentials(oracle):
+    """Eq. 6-7: psi(t+dt) = P4(-i dt/2 H(t+dt)) P4(-i dt/2 H(t)) psi, approx = P4(-i dt H(t)) psi, H(t+dt) from a second V."""
+    cfg = small_cfg(112, n=(5, 4, 6), length=(5.0, 4.2, 5.6), natoms=2, lmax=1, rc=1.9)
+    wl = W.make(cfg)
+    rng = np.random.default_rng(112)
+    v2 = wl.v + rng.uniform(-0.3, 0.3, wl.v.shape)
+    wl2 = W.Workload(cfg=cfg, pos=wl.pos, v=v2, proj=wl.proj)
+    h1, h2 = dense_matrix(oracle, cfg, wl), dense_matrix(oracle, cfg, wl2)
+    psi = W.states(cfg)
+    dt = 0.05
+    out, approx = oracle.etrs_step(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, wl.v, v2, wl.proj, psi, dt, 0)
+    flat = psi.reshape(psi.shape[0], -1).T
+    expect = poly4(h2, -0.5j * dt) @ (poly4(h1, -0.5j * dt) @ flat)
+    assert rel(out.reshape(psi.shape[0], -1).T, expect) < 1e-13
+    assert rel(approx.reshape(psi.shape[0], -1).T, poly4(h1, -1j * dt) @ flat) < 1e-13
+    # the order of the two half steps matters when the potentials differ (a transposed operand would pass otherwise)
+    swapped = poly4(h1, -0.5j * dt) @ (poly4(h2, -0.5j * dt) @ flat)
+    assert rel(swapped, expect) > 1e-8
+
+
+def test_p9_etrs_kinetic_only_closed_form(oracle):
+    """V = 0, no atoms, fixed H: every plane wave is multiplied by P(t dt/2)^2 per ETRS step and approx by P(t dt)."""
+    n, length = (6, 8, 4), (4.0, 5.0, 3.0)
+    kpt = [TWO_PI * 0.2 / length[0], 0.0, 0.0]
+    rng = np.random.default_rng(9)
+    psi0 = rand_c(rng, (2,) + n)
+    dt = 0.08
+    g = [TWO_PI * np.fft.fftfreq(n[a], d=1.0 / n[a]) / length[a] + kpt[a] for a in range(3)]
+    t = 0.5 * (g[0][:, None, None] ** 2 + g[1][None, :, None] ** 2 + g[2][None, None, :] ** 2)
+    for backend in (0, 1):
+        out, approx = oracle.etrs_step(n, length, kpt, -1.0, None, None, None, psi0, dt, backend)
+        f0 = np.fft.fftn(psi0, axes=(1, 2, 3))
+        assert rel(out, np.fft.ifftn(taylor4(0.5 * t * dt) ** 2 * f0, axes=(1, 2, 3))) < 1e-12
+        assert rel(approx, np.fft.ifftn(taylor4(t * dt) * f0, axes=(1, 2, 3))) < 1e-12
+
+
 # --------------------------------------------------------------------------------------------- P8
 def test_p8_independent_of_batching(oracle):
     cfg = W.CONFIGS["tiny"]
