@@ -359,6 +359,22 @@ def sweep_leg(torch, B, name, flush, reps=7):
             res["propagate"] = {"steps": cfg.nsteps, "dt": cfg.dt, "seconds": t, "steps_per_s": cfg.nsteps / t,
                                 "h_application_equivalents_per_s": units * 4 * cfg.nsteps / t, "unit": UNIT,
                                 "launches": g.last_launch_count()}
+            # NEXT-1: ETRS steps (Eq. 6-7) with the shared-powers pair: 8 H applications per step
+            # instead of the 12 of three separate exponentials
+            work.copy_(psi)
+            vdev = torch.from_numpy(wl.v).cuda()
+            g.etrs_step(work, cfg.dt, vdev, approx=out)
+            torch.cuda.synchronize()
+            work.copy_(psi)
+            nsteps_e = 5
+
+            def etrs():
+                for _ in range(nsteps_e):
+                    g.etrs_step(work, cfg.dt, vdev, approx=out)
+            te = timed_each(torch, etrs, 1, flush)[0]
+            res["etrs"] = {"steps": nsteps_e, "dt": cfg.dt, "seconds_per_step": te / nsteps_e,
+                           "h_applications_per_step": 8, "h_application_equivalents_per_s": units * 8 * nsteps_e / te,
+                           "unit": UNIT, "note": "tdh_etrs_step: taylor pair (4 H) + potential switch + half step (4 H)"}
     del psi, out
     torch.cuda.empty_cache()
     return res
@@ -462,6 +478,7 @@ def main():
         extra["workloads"] = wls
         if "tddft" in wls and "propagate" in wls["tddft"]:
             extra["propagate"] = wls["tddft"].pop("propagate")
+            extra["etrs"] = wls["tddft"].pop("etrs")
     else:
         g.close()
 

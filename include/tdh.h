@@ -97,6 +97,22 @@ int tdh_apply_hamiltonian(tdh_grid* g, int nst, const tdh_c128* psi_dev, tdh_c12
  * psi_dev: DEVICE, nst*n0*n1*n2 complex128.  order must be 4.  nsteps >= 0.  Asynchronous on the handle's stream. */
 int tdh_propagate(tdh_grid* g, int nst, tdh_c128* psi_dev, double dt, int nsteps, int order);
 
+/* The two exponentials of an ETRS step that share their powers H^k psi (Eq. 8 for two lambdas):
+ *     full <- sum_{k=0..4} (-i dt)^k/k!   H^k psi        (Eq. 7: the approximate psi(t+dt) from which H(t+dt) is built)
+ *     psi  <- sum_{k=0..4} (-i dt/2)^k/k! H^k psi        (the first factor of Eq. 6), in place
+ * from four H applications instead of eight.  psi_dev, full_dev: DEVICE, nst*n0*n1*n2 complex128 each, must not overlap.
+ * order must be 4.  Asynchronous on the handle's stream; allocates nothing. */
+int tdh_taylor_pair(tdh_grid* g, int nst, tdh_c128* psi_dev, tdh_c128* full_dev, double dt, int order);
+
+/* One ETRS step, Eq. 6-7, with the local potential at t+dt supplied by the caller:
+ *     approx <- exp(-i dt H(t)) psi;   psi <- exp(-i dt/2 H(t+dt)) exp(-i dt/2 H(t)) psi      (Taylor order 4 each)
+ * H(t) uses the handle's current potential, H(t+dt) uses v_next_dev (DEVICE, n0*n1*n2 doubles, or NULL for V = 0),
+ * which becomes the handle's potential (as after tdh_set_potential); the projectors are the same in both.  This is
+ * tdh_taylor_pair, a potential switch and tdh_propagate(dt/2, 1 step): 8 H applications.  When V(t+dt) has to be
+ * derived from approx (self-consistent propagation), call those three yourself with your update in between.
+ * approx_dev: DEVICE work/output block of the size of psi_dev, must not overlap it. */
+int tdh_etrs_step(tdh_grid* g, int nst, tdh_c128* psi_dev, tdh_c128* approx_dev, double dt, const double* v_next_dev);
+
 /* The same two operations with HOST buffers (pageable or pinned): the library stages state chunks through its own
  * pinned buffers, overlapping host<->device copies with the kernels, and returns when hpsi_host / psi_host is complete.
  * nst is not limited by max_states here (chunks are).  These are the end-to-end entry points timed by bench.py. */

@@ -25,7 +25,7 @@ LIB_PATH = os.path.join(_HERE, "libtdh.so")
 #: every symbol include/tdh.h declares
 SYMBOLS = (
     "tdh_create_grid", "tdh_destroy_grid", "tdh_set_potential", "tdh_set_projectors", "tdh_apply_hamiltonian",
-    "tdh_propagate", "tdh_apply_hamiltonian_host", "tdh_propagate_host", "tdh_fft3d", "tdh_last_launch_count",
+    "tdh_propagate", "tdh_taylor_pair", "tdh_etrs_step", "tdh_apply_hamiltonian_host", "tdh_propagate_host", "tdh_fft3d", "tdh_last_launch_count",
     "tdh_set_profiling", "tdh_last_kernel_seconds", "tdh_kernel_name", "tdh_set_chunk_states", "tdh_last_error",
 )
 NKERNELS = 5
@@ -58,6 +58,8 @@ def lib() -> C.CDLL:
     l.tdh_set_projectors.argtypes = [vp, i, vp, vp, vp, vp, vp, vp]
     l.tdh_apply_hamiltonian.argtypes = [vp, i, vp, vp]
     l.tdh_propagate.argtypes = [vp, i, vp, d, i, i]
+    l.tdh_taylor_pair.argtypes = [vp, i, vp, vp, d, i]
+    l.tdh_etrs_step.argtypes = [vp, i, vp, vp, d, vp]
     l.tdh_apply_hamiltonian_host.argtypes = [vp, i, vp, vp]
     l.tdh_propagate_host.argtypes = [vp, i, vp, d, i, i]
     l.tdh_fft3d.argtypes = [vp, i, vp, i]
@@ -171,6 +173,30 @@ class Grid:
         nst = self._block(psi)
         _check(lib().tdh_propagate(self._h, nst, C.c_void_p(psi.data_ptr()), float(dt), int(nsteps), int(order)))
         return psi
+
+    def taylor_pair(self, psi, dt: float, full=None, order: int = 4):
+        """psi <- exp(-i dt/2 H) psi in place; returns full = exp(-i dt H) psi (both Taylor order 4, one chain of powers)."""
+        import torch
+        nst = self._block(psi)
+        if full is None:
+            full = torch.empty_like(psi)
+        assert self._block(full) == nst
+        _check(lib().tdh_taylor_pair(self._h, nst, C.c_void_p(psi.data_ptr()), C.c_void_p(full.data_ptr()), float(dt), int(order)))
+        return full
+
+    def etrs_step(self, psi, dt: float, v_next, approx=None):
+        """One ETRS step in place with V(t+dt) = v_next (device float64 tensor or None); returns approx = exp(-i dt H(t)) psi."""
+        import torch
+        nst = self._block(psi)
+        if approx is None:
+            approx = torch.empty_like(psi)
+        assert self._block(approx) == nst
+        vp_ = None
+        if v_next is not None:
+            assert v_next.is_cuda and v_next.dtype == torch.float64 and v_next.is_contiguous() and v_next.numel() == self.npts
+            vp_ = C.c_void_p(v_next.data_ptr())
+        _check(lib().tdh_etrs_step(self._h, nst, C.c_void_p(psi.data_ptr()), C.c_void_p(approx.data_ptr()), float(dt), vp_))
+        return approx
 
     def fft3d(self, psi, sign: int):
         nst = self._block(psi)

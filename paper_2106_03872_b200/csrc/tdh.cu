@@ -284,8 +284,9 @@ extern "C" int tdh_create_grid(const int n[3], const double len[3], const double
         size_t cap = std::max<size_t>(1, ((size_t)1 << 30) / state_bytes);
         g->chunk_cap = (int)std::min<size_t>(cap, (size_t)max_states);
         CU(cudaMalloc(&g->d_work, state_bytes * g->chunk_cap));
-        CU(cudaMalloc(&g->d_phi[0], state_bytes * g->chunk_cap));
-        CU(cudaMalloc(&g->d_phi[1], state_bytes * g->chunk_cap));
+        // at least two states each: tdh_taylor_pair keeps phi_2 and phi_3 in the two halves of d_phi[0]
+        CU(cudaMalloc(&g->d_phi[0], state_bytes * std::max(2, g->chunk_cap)));
+        CU(cudaMalloc(&g->d_phi[1], state_bytes * std::max(2, g->chunk_cap)));
         g->chunk = default_chunk(g);
         return TDH_OK;
     };
@@ -753,6 +754,52 @@ static int propagate_chunk(tdh_grid* g, int nst, cd* psi, double dt, int nsteps)
     return TDH_OK;
 }
 
+// half = psi + sum_k a_k phi_k (written over psi), full = psi + sum_k b_k phi_k (written over phi_1), k = 1..4, elementwise
+__global__ void taylor_pair_combine_kernel(cd* __restrict__ psi, cd* __restrict__ f1, const cd* __restrict__ p2,
+                                           const cd* __restrict__ p3, const cd* __restrict__ p4, size_t n, cd a1, cd a2,
+                                           cd a3, cd a4, cd b1, cd b2, cd b3, cd b4) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const cd x = __ldcs(psi + i), y1 = __ldcs(f1 + i), y2 = __ldcs(p2 + i), y3 = __ldcs(p3 + i), y4 = __ldcs(p4 + i);
+        cd h = tdh::cfma(a1, y1, x), f = tdh::cfma(b1, y1, x);
+        h = tdh::cfma(a2, y2, h); f = tdh::cfma(b2, y2, f);
+        h = tdh::cfma(a3, y3, h); f = tdh::cfma(b3, y3, f);
+        h = tdh::cfma(a4, y4, h); f = tdh::cfma(b4, y4, f);
+        __stcs(psi + i, h);
+        __stcs(f1 + i, f);
+    }
+}
+
+// phi_k = H phi_{k-1} once, both Taylor sums from the same four vectors.  Runs in half chunks so that
+// phi_2, phi_3 (halves of d_phi[0]) and phi_4 (d_phi[1]) fit the handle's workspace; phi_1 lives in the caller's `full`.
+static int taylor_pair_block(tdh_grid* g, int nst, cd* psi, cd* full, double dt) {
+    const int hc = std::max(1, g->chunk / 2);
+    const cd one = make_double2(1.0, 0.0);
+    // (-i dt)^k / k!  and  (-i dt/2)^k / k!
+    const double d = dt, e = 0.5 * dt;
+    const cd b1 = make_double2(0.0, -d), b2 = make_double2(-d * d / 2.0, 0.0), b3 = make_double2(0.0, d * d * d / 6.0),
+             b4 = make_double2(d * d * d * d / 24.0, 0.0);
+    const cd a1 = make_double2(0.0, -e), a2 = make_double2(-e * e / 2.0, 0.0), a3 = make_double2(0.0, e * e * e / 6.0),
+             a4 = make_double2(e * e * e * e / 24.0, 0.0);
+    for (int s0 = 0; s0 < nst; s0 += hc) {
+        const int c = std::min(hc, nst - s0);
+        cd* x = psi + (size_t)s0 * g->np;
+        cd* f1 = full + (size_t)s0 * g->np;
+        cd* p2 = g->d_phi[0];
+        cd* p3 = g->d_phi[0] + (size_t)hc * g->np;
+        cd* p4 = g->d_phi[1];
+        int rc;
+        if ((rc = apply_chunk(g, c, x, f1, one, nullptr))) return rc;
+        if ((rc = apply_chunk(g, c, f1, p2, one, nullptr))) return rc;
+        if ((rc = apply_chunk(g, c, p2, p3, one, nullptr))) return rc;
+        if ((rc = apply_chunk(g, c, p3, p4, one, nullptr))) return rc;
+        const size_t n = (size_t)c * g->np;
+        taylor_pair_combine_kernel<<<148 * 8, 256, 0, g->stream>>>(x, f1, p2, p3, p4, n, a1, a2, a3, a4, b1, b2, b3, b4);
+        CU(cudaGetLastError());
+        g->launch_count += 1;
+    }
+    return TDH_OK;
+}
+
 static int propagate_block(tdh_grid* g, int nst, cd* psi, double dt, int nsteps) {
     for (int s0 = 0; s0 < nst; s0 += g->chunk) {
         const int c = std::min(g->chunk, nst - s0);
@@ -787,6 +834,43 @@ extern "C" int tdh_propagate(tdh_grid* g, int nst, tdh_c128* psi_dev, double dt,
     stats_reset(g);
     int rc = propagate_block(g, nst, (cd*)psi_dev, dt, nsteps);
     if (rc) return rc;
+    return prof_collect(g);
+}
+
+extern "C" int tdh_taylor_pair(tdh_grid* g, int nst, tdh_c128* psi_dev, tdh_c128* full_dev, double dt, int order) {
+    if (!g || !psi_dev || !full_dev) return fail(TDH_EINVAL, "tdh_taylor_pair: null argument");
+    if (nst < 1 || nst > g->max_states) return fail(TDH_EINVAL, "tdh_taylor_pair: nst = %d outside [1, %d]", nst, g->max_states);
+    if (order != 4) return fail(TDH_EINVAL, "tdh_taylor_pair: order must be 4");
+    if (!std::isfinite(dt)) return fail(TDH_EINVAL, "tdh_taylor_pair: bad dt");
+    if (overlaps(psi_dev, full_dev, (size_t)nst * g->np * sizeof(cd)))
+        return fail(TDH_EINVAL, "tdh_taylor_pair: psi and full overlap");
+    stats_reset(g);
+    int rc = taylor_pair_block(g, nst, (cd*)psi_dev, (cd*)full_dev, dt);
+    if (rc) return rc;
+    return prof_collect(g);
+}
+
+extern "C" int tdh_etrs_step(tdh_grid* g, int nst, tdh_c128* psi_dev, tdh_c128* approx_dev, double dt,
+                             const double* v_next_dev) {
+    if (!g || !psi_dev || !approx_dev) return fail(TDH_EINVAL, "tdh_etrs_step: null argument");
+    if (nst < 1 || nst > g->max_states) return fail(TDH_EINVAL, "tdh_etrs_step: nst = %d outside [1, %d]", nst, g->max_states);
+    if (!std::isfinite(dt)) return fail(TDH_EINVAL, "tdh_etrs_step: bad dt");
+    if (overlaps(psi_dev, approx_dev, (size_t)nst * g->np * sizeof(cd)))
+        return fail(TDH_EINVAL, "tdh_etrs_step: psi and approx overlap");
+    stats_reset(g);
+    int rc = taylor_pair_block(g, nst, (cd*)psi_dev, (cd*)approx_dev, dt);          // Eq. 7 and the first factor of Eq. 6
+    if (rc) return rc;
+    // H(t+dt): stream-ordered switch of the potential
+    if (v_next_dev) {
+        CU(cudaMemcpyAsync(g->d_v, v_next_dev, sizeof(double) * g->np, cudaMemcpyDeviceToDevice, g->stream));
+        g->have_v = true;
+    } else {
+        CU(cudaMemsetAsync(g->d_v, 0, sizeof(double) * g->np, g->stream));
+        g->have_v = false;
+    }
+    const int launches = g->launch_count;
+    if ((rc = propagate_block(g, nst, (cd*)psi_dev, 0.5 * dt, 1))) return rc;      // the second factor of Eq. 6
+    (void)launches;
     return prof_collect(g);
 }
 

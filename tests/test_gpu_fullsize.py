@@ -172,3 +172,53 @@ def test_both_back_projection_paths(torch_cuda, B, oracle, monkeypatch, mode):
             g.propagate(d, 0.01, 1)
             ref_p = oracle.propagate_workload(wl, psi, dt=0.01, nsteps=1, backend=oracle.NAIVE_FFT)
             assert per_state_rel(d.cpu().numpy(), ref_p).max() < TOL
+
+
+# ------------------------------------------------------------------------------------------------ NEXT-1: ETRS
+@pytest.mark.parametrize("name,nst,backend", [("tiny", 8, 0), ("small", 24, 1), ("medium", 10, 1)])
+def test_taylor_pair_and_etrs_match_oracle(torch_cuda, B, oracle, name, nst, backend):
+    """tdh_taylor_pair and tdh_etrs_step (Eq. 6-7, V(t+dt) supplied) against the oracle."""
+    torch = torch_cuda
+    cfg = W.CONFIGS[name]
+    wl = W.make(cfg)
+    psi = W.states(cfg, 0, nst)
+    rng = np.random.default_rng([W.BASE_SEED + cfg.cid, 7])
+    v_next = wl.v + rng.uniform(-0.2, 0.2, wl.v.shape)
+    dt = 0.02
+    half_ref, full_ref = oracle.taylor_pair(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, wl.v, wl.proj, psi, dt, 4, backend)
+    out_ref, approx_ref = oracle.etrs_step(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, wl.v, v_next, wl.proj, psi, dt, backend)
+    with B.grid_for(wl, max_states=nst) as g:
+        for chunk in (None, 3):
+            if chunk:
+                g.set_chunk_states(chunk)
+            g.set_potential(torch.from_numpy(wl.v).cuda())
+            d = torch.from_numpy(psi).cuda()
+            full = g.taylor_pair(d, dt)
+            assert per_state_rel(d.cpu().numpy(), half_ref).max() < TOL
+            assert per_state_rel(full.cpu().numpy(), full_ref).max() < TOL
+            d = torch.from_numpy(psi).cuda()
+            approx = g.etrs_step(d, dt, torch.from_numpy(v_next).cuda())
+            assert per_state_rel(d.cpu().numpy(), out_ref).max() < TOL
+            assert per_state_rel(approx.cpu().numpy(), approx_ref).max() < TOL
+        # the handle now holds V(t+dt): a plain application uses it
+        wl2 = W.Workload(cfg=cfg, pos=wl.pos, v=v_next, proj=wl.proj)
+        h = g.apply_hamiltonian(torch.from_numpy(psi).cuda()).cpu().numpy()
+        assert per_state_rel(h, oracle.apply_workload(wl2, psi, backend)).max() < TOL
+
+
+def test_etrs_single_state_handle_and_errors(torch_cuda, B, oracle):
+    """max_states = 1 (workspace of one state) still has room for the four powers; overlapping buffers are refused."""
+    torch = torch_cuda
+    cfg = W.CONFIGS["tiny"]
+    wl = W.make(cfg)
+    psi = W.states(cfg, 0, 1)
+    out_ref, _ = oracle.etrs_step(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, wl.v, None, wl.proj, psi, 0.03, 0)
+    with B.grid_for(wl, max_states=1) as g:
+        d = torch.from_numpy(psi).cuda()
+        g.etrs_step(d, 0.03, None)
+        assert per_state_rel(d.cpu().numpy(), out_ref).max() < TOL
+        with pytest.raises(B.TdhError) as e:
+            g.taylor_pair(d, 0.03, full=d)
+        assert e.value.code == B.TDH_EINVAL
+        with pytest.raises(B.TdhError):
+            g.taylor_pair(d, 0.03, order=2)
