@@ -15,11 +15,13 @@
 // walks tiles blockIdx.x, blockIdx.x + gridDim.x, ... through a ring of NB buffers that one elected thread keeps
 // filled with cp.async.bulk.tensor, so the loads of the next tiles are in flight while this one is transformed.
 //
-// THREADS.  NX = R1*R2 (R1 >= R2).  A CTA has TPL threads per line (TPL >= R2): the R2 radix-R1 transforms of a line
-// (first forward stage, last inverse stage) take one round, the R1 radix-R2 transforms in between take
-// ceil(R1/TPL) rounds.  The kernel is compiled for CPS resident CTAs per SM (<= 128 registers per thread): the
-// barrier-separated stages of one CTA alternate between shared-memory, FP64 and store phases, and the second CTA
-// fills the gaps.  Twiddles and (G_x+k_x)^2 sit in shared memory behind the ring.
+// THREADS.  NX = R1*R2 (R1 >= R2).  A CTA has TPL = 4 threads per line (128 threads): the R2 radix-R1 transforms of a
+// line (first forward stage, last inverse stage) take ceil(R2/4) rounds, the R1 radix-R2 transforms in between
+// ceil(R1/4) rounds -- for NX = 96 (12 x 8) that is 2, 3, 2 rounds with every thread busy in each.  The kernel is compiled
+// for four resident CTAs per SM (<= 128 registers per thread): the barrier-separated stages of one CTA alternate between
+// TMA wait, shared-memory, FP64 and store phases, and the other three fill the gaps (measured on Large: 8 threads per
+// line and two CTAs 0.79 ms per 128 states, this layout 0.69 ms).  Twiddles and (G_x+k_x)^2 sit in shared memory
+// behind the ring.
 //
 // S = 2 (see tile_kernels.cuh): the tile kernels leave/expect half-length y transforms E_r[k] / F_r[k], r = 0, 1, at
 // rows Y = 2*rho + r -- lanes l and l ^ 16 of a warp.  The missing radix-2 step of the y transform commutes with the x
@@ -53,9 +55,10 @@ __device__ __forceinline__ cd shfl16(cd v) {
 
 template <int NX> struct XCfg {
     static constexpr int R1 = Fact<NX>::R1, R2 = Fact<NX>::R2;
-    static constexpr int TPL = NX >= 48 ? 8 : 4;                    // threads per line
+    static constexpr int TPL = 4;                                   // threads per line
     static constexpr int T = XP_LPC * TPL;
-    static constexpr int CPS = NX >= 48 ? 2 : 4;                    // resident CTAs per SM the kernel is built for
+    static constexpr int CPS = 512 / T;                             // resident CTAs per SM the kernel is built for
+    static constexpr int ROUNDS_A = (R2 + TPL - 1) / TPL;           // rounds of the radix-R1 stages
     static constexpr int ROUNDS_B = (R1 + TPL - 1) / TPL;           // rounds of the radix-R2 stage
     static constexpr int TILE_CELLS = NX * XP_LPC;
     static constexpr size_t TILE_BYTES = (size_t)TILE_CELLS * sizeof(cd);
@@ -63,9 +66,8 @@ template <int NX> struct XCfg {
     // ring depth: what fits in 1/CPS of the SM's 228 KB beside the barriers, the tables and the 1 KB the system
     // reserves per CTA; between 2 and 4 tiles
     static constexpr int fit() { return (int)((233472 / CPS - 2048 - TABLE_BYTES) / TILE_BYTES); }
-    static constexpr int NB = fit() < 2 ? 2 : (fit() > 4 ? 4 : fit());
+    static constexpr int NB = fit() < 1 ? 1 : (fit() > 4 ? 4 : fit());
     static constexpr size_t SMEM = 1024 + NB * TILE_BYTES + TABLE_BYTES;
-    static_assert(R2 <= TPL, "the radix-R1 stages must fit one round");
 };
 
 // the kinetic factor t = 0.5*((gx^2 + gy^2) + gz^2) in the oracle's operation order (no contraction), masked, times
@@ -83,7 +85,7 @@ xpencil_kernel(const __grid_constant__ CUtensorMap map, cd* __restrict__ out, in
                const cd* __restrict__ tw_x, const Kinetic kin)
 {
     using C = XCfg<NX>;
-    constexpr int R1 = C::R1, R2 = C::R2, L = XP_LPC, NB = C::NB, TPL = C::TPL, RB = C::ROUNDS_B;
+    constexpr int R1 = C::R1, R2 = C::R2, L = XP_LPC, NB = C::NB, TPL = C::TPL, RA = C::ROUNDS_A, RB = C::ROUNDS_B;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);            // NB barriers in the first 1024 bytes
     cd* ring = reinterpret_cast<cd*>(smem_raw + 1024);
@@ -138,19 +140,28 @@ xpencil_kernel(const __grid_constant__ CUtensorMap map, cd* __restrict__ out, in
             if (S == 2) gy2b = __ldg(kin.g2y_w + 2 * rho2 + 1);
         }
         if (S == 2) w = __ldg(kin.twy_w + rho2);                 // e^{+2 pi i k / NY} = conj(w of the header comment)
+        // a ring of one buffer cannot prefetch into shared memory: start the CTA's next tile towards L2 instead
+        // (measured: +3 % for the 48 KB tiles of NX = 96, -4 % for the 32 KB tiles of NX = 64, so only the former)
+        if (NB == 1 && NX >= 96 && tid == 0 && t + (int)gridDim.x < ntiles) {
+            const int tn = t + gridDim.x, stn = tn / tiles_per_state, remn = tn % tiles_per_state;
+            tma_prefetch_l2_4d(&map, 0, remn % zc, 2 * (remn / zc), stn * NX);
+        }
         mbar_wait(full + b, parity);
 
         if (MODE != 2) {
-            // ---- forward stage A: radix R1 over x = j1*R2 + j2, one transform per thread with hi = j2 < R2, in place
-            if (hi < R2) {
-                const int j2 = hi;
-                cd x[R1];
+            // ---- forward stage A: radix R1 over x = j1*R2 + j2, transforms j2 = hi, hi + TPL, ... < R2, in place
 #pragma unroll
-                for (int j1 = 0; j1 < R1; ++j1) x[j1] = sm[(j1 * R2 + j2) * L + l];
-                Dft<R1, -1>::run(x);
-                sm[j2 * L + l] = x[0];
+            for (int ra = 0; ra < RA; ++ra) {
+                const int j2 = hi + ra * TPL;
+                if (j2 < R2) {
+                    cd x[R1];
 #pragma unroll
-                for (int k1 = 1; k1 < R1; ++k1) sm[(k1 * R2 + j2) * L + l] = cmulc(x[k1], stw[k1 * j2]);
+                    for (int j1 = 0; j1 < R1; ++j1) x[j1] = sm[(j1 * R2 + j2) * L + l];
+                    Dft<R1, -1>::run(x);
+                    sm[j2 * L + l] = x[0];
+#pragma unroll
+                    for (int k1 = 1; k1 < R1; ++k1) sm[(k1 * R2 + j2) * L + l] = cmulc(x[k1], stw[k1 * j2]);
+                }
             }
             __syncthreads();
         }
@@ -247,20 +258,34 @@ xpencil_kernel(const __grid_constant__ CUtensorMap map, cd* __restrict__ out, in
             continue;
         }
 
-        // ---- last inverse stage: thread hi = n2 < R2 transforms slots k1*R2 + n2 over k1 -> x = n2 + R2*n1
+        // ---- last inverse stage: transforms n2 = hi, hi + TPL, ... < R2 over the slots k1*R2 + n2 -> x = n2 + R2*n1.
+        //      The buffer is handed back to the TMA as soon as the inputs of the last round are in registers.
         __syncthreads();
-        cd x[R1];
-        if (hi < R2) {
 #pragma unroll
-            for (int k1 = 0; k1 < R1; ++k1) x[k1] = sm[(k1 * R2 + hi) * L + l];
+        for (int ra = 0; ra + 1 < RA; ++ra) {
+            const int n2 = hi + ra * TPL;
+            if (n2 < R2) {
+                cd x[R1];
+#pragma unroll
+                for (int k1 = 0; k1 < R1; ++k1) x[k1] = sm[(k1 * R2 + n2) * L + l];
+                Dft<R1, +1>::run(x);
+#pragma unroll
+                for (int n1 = 0; n1 < R1; ++n1) __stcs(gcol + (size_t)(n2 + R2 * n1) * nynz, x[n1]);
+            }
+        }
+        const int n2 = hi + (RA - 1) * TPL;
+        cd x[R1];
+        if (n2 < R2) {
+#pragma unroll
+            for (int k1 = 0; k1 < R1; ++k1) x[k1] = sm[(k1 * R2 + n2) * L + l];
         }
         fence_proxy_async();
         __syncthreads();                  // every read of this buffer is done: refill it
         if (tid == 0 && t + NB * (int)gridDim.x < ntiles) issue(t + NB * gridDim.x, b);
-        if (hi < R2) {
+        if (n2 < R2) {
             Dft<R1, +1>::run(x);
 #pragma unroll
-            for (int n1 = 0; n1 < R1; ++n1) __stcs(gcol + (size_t)(hi + R2 * n1) * nynz, x[n1]);
+            for (int n1 = 0; n1 < R1; ++n1) __stcs(gcol + (size_t)(n2 + R2 * n1) * nynz, x[n1]);
         }
     }
 }
