@@ -222,3 +222,39 @@ def test_etrs_single_state_handle_and_errors(torch_cuda, B, oracle):
         assert e.value.code == B.TDH_EINVAL
         with pytest.raises(B.TdhError):
             g.taylor_pair(d, 0.03, order=2)
+
+
+@pytest.mark.parametrize("mode", ["0", "1"])
+def test_degenerate_projectors(torch_cuda, B, oracle, monkeypatch, mode):
+    """An atom whose sphere holds no grid point, an atom with no channel, a one-point sphere, all in one table."""
+    torch = torch_cuda
+    monkeypatch.setenv("TDH_NL_MODE", mode)
+    n, length = (16, 16, 32), (6.0, 6.0, 12.0)
+    cfg = W.test_config(270, n, length, nst=5, natoms=1, lmax=1, rc=2.0, dl=(1.3, -0.6))
+    full = W.projectors(cfg, np.array([[3.0, 3.0, 6.0]]))
+    P = int(full.sph_off[1])
+    beta_full = full.beta.reshape(4, P)
+    # atoms: 0 = regular (4 channels), 1 = empty sphere (2 channels, 0 points), 2 = no channels (P points),
+    #        3 = a single point with one channel
+    sph_off = np.array([0, P, P, 2 * P, 2 * P + 1], dtype=np.int64)
+    one_pt = np.array([123], dtype=np.int32)
+    sph_idx = np.concatenate([full.sph_idx, full.sph_idx, one_pt]).astype(np.int32)
+    sph_disp = np.concatenate([full.sph_disp, full.sph_disp, np.zeros((1, 3))])
+    chan_off = np.array([0, 4, 6, 6, 7], dtype=np.int32)
+    beta = np.concatenate([beta_full.ravel(), np.zeros(0), np.zeros(0), np.array([0.8])])
+    dcoef = np.array([1.3, -0.6, -0.6, -0.6, 9.0, 9.0, 2.5])
+    proj = W.Projectors(natoms=4, sph_off=sph_off, sph_idx=sph_idx, sph_disp=sph_disp, chan_off=chan_off, beta=beta,
+                        dcoef=dcoef)
+    psi = W.states(cfg)
+    v = W.local_potential(cfg, np.array([[3.0, 3.0, 6.0]]))
+    ref = oracle.apply_hamiltonian(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, v, proj, psi, oracle.NAIVE_FFT)
+    with B.Grid(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, cfg.nst) as g:
+        g.set_potential(torch.from_numpy(v).cuda())
+        g.set_projectors(proj)
+        out = g.apply_hamiltonian(torch.from_numpy(psi).cuda()).cpu().numpy()
+        assert per_state_rel(out, ref).max() < TOL
+        # the single-point projector is visible at its point and nowhere else
+        g.set_projectors(None)
+        base = g.apply_hamiltonian(torch.from_numpy(psi).cuda()).cpu().numpy()
+        diff = (out - base).reshape(cfg.nst, -1)
+        assert np.abs(diff[:, 123]).min() > 1e-6

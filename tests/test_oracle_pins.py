@@ -329,6 +329,33 @@ def test_p7_propagate_is_literal_eq8(oracle):
     assert rel(two, oracle.propagate_workload(wl, acc, dt=dt, nsteps=1, backend=0)) < 1e-13
 
 
+def test_golden_eq8_coefficients(oracle):
+    """tests/golden/eq8_taylor_coefficients.txt (Eq. 8): one oracle step on a 1-point 'grid-free' problem --
+    an eigenvector of a constant potential with eigenvalue eps -- is multiplied by sum_k (1/k!) (-i)^k (eps dt)^k."""
+    import os
+    from fractions import Fraction as F
+    rows, mod2 = [], None
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "eq8_taylor_coefficients.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        tok = line.split()
+        if tok[0] == "modulus2":
+            mod2 = [F(t) for t in tok[1:]]
+        else:
+            rows.append((int(tok[0]), F(tok[1]), int(tok[2]), int(tok[3])))
+    assert [r[0] for r in rows] == [0, 1, 2, 3, 4] and len(mod2) == 9
+    # constant potential c on a 4^3 grid, psi = const: H psi = c psi (kinetic term of the G = 0 wave is 0 at Gamma)
+    n, length, c, dt = (4, 4, 4), (3.0, 3.0, 3.0), -0.7, 0.9
+    psi = np.ones(n, dtype=np.complex128)
+    for lam_scale, nsteps in ((1.0, 1), (0.5, 1)):
+        out = oracle.propagate(n, length, (0.0, 0.0, 0.0), -1.0, np.full(n, c), None, psi, dt * lam_scale, nsteps, 4, 0)
+        x = c * dt * lam_scale
+        expect = sum(float(f) * complex(re, im) * x ** k for k, f, re, im in rows)
+        assert np.abs(out - expect).max() < 1e-14
+        m2 = sum(float(cf) * x ** m for m, cf in enumerate(mod2))
+        assert abs(abs(expect) ** 2 - m2) < 1e-14
+
+
 # --------------------------------------------------------------------------------------------- P9 (NEXT-1: ETRS)
 def poly4(m, lam):
     """sum_{k=0..4} (lam m)^k / k! of a dense matrix m, by explicit matrix powers (numpy, independent of the oracle's loop)."""
