@@ -26,7 +26,7 @@ def lib() -> C.CDLL:
     if _lib is None:
         _lib = C.CDLL(_build.build())
         for name in ("ref_dft3d", "ref_kinetic", "ref_local", "ref_nonlocal", "ref_apply_hamiltonian",
-                     "ref_propagate", "ref_taylor_pair", "ref_etrs_step", "ref_num_threads"):
+                     "ref_propagate", "ref_taylor_pair", "ref_etrs_step", "ref_density", "ref_hartree", "ref_num_threads"):
             getattr(_lib, name).restype = C.c_int
     return _lib
 
@@ -159,6 +159,26 @@ def etrs_step(n, length, kpt, ecut, v, v_next, proj, psi, dt: float, backend: in
     _check(lib().ref_etrs_step(_i3(n), _d3(length), _d3(kpt), C.c_double(ecut), _ptr(v), _ptr(v_next), *p.args, C.c_int(nst),
                                _ptr(out), _ptr(approx), C.c_double(dt), C.c_int(backend)), "etrs_step")
     return out, approx
+
+
+def density(n, psi, occ=None, accumulate_into=None) -> np.ndarray:
+    """n(r) = sum_s occ[s] |psi_s(r)|^2 (Eq. 1); occ None: all 1.  accumulate_into: float64 array (n) that is added to."""
+    psi = _c128(psi)
+    nst = 1 if psi.ndim == 3 else psi.shape[0]
+    occ = None if occ is None else np.ascontiguousarray(occ, dtype=np.float64)
+    out = np.zeros(tuple(n), dtype=np.float64) if accumulate_into is None else accumulate_into
+    assert out.flags["C_CONTIGUOUS"] and out.dtype == np.float64
+    _check(lib().ref_density(_i3(n), C.c_int(nst), _ptr(psi), _ptr(occ), _ptr(out),
+                             C.c_int(0 if accumulate_into is None else 1)), "density")
+    return out
+
+
+def hartree(n, length, dens, backend: int = NAIVE_FFT) -> np.ndarray:
+    """Periodic Hartree potential: v_hat(G) = 4 pi n_hat(G) / |G|^2, G = 0 dropped."""
+    dens = np.ascontiguousarray(dens, dtype=np.float64)
+    out = np.empty_like(dens)
+    _check(lib().ref_hartree(_i3(n), _d3(length), _ptr(dens), _ptr(out), C.c_int(backend)), "hartree")
+    return out
 
 
 def apply_workload(wl, psi, backend: int = NAIVE_FFT) -> np.ndarray:

@@ -17,6 +17,7 @@
  *                                                                      Eq. 9; readings R2-R5
  *   exp(-i dt H) psi ~= sum_{k=0..4} (-i dt)^k / k!  H^k psi           Eq. 8
  *   ETRS step (Eq. 6-7) from two such sums sharing H^k psi, V(t+dt) supplied
+ *   n(r) = sum_s f_s |psi_s(r)|^2  (Eq. 1);  v_H from the periodic Poisson equation in Fourier space
  *
  * Two DFT back-ends: backend 0 = direct O(N^2)-per-pencil sum (the definition), backend 1 = a separately
  * written recursive radix-2/3 decimation-in-time FFT (only to make the large configs affordable; it is
@@ -26,7 +27,7 @@
  * kinetic eigenvectors incl. Nyquist and mask, P3 constant potential = shift, P4 rank / closed form of one
  * projector, P5 Hermiticity and dense-matrix spectrum, P6 Bloch-phase identity and translation covariance,
  * P7 closed-form Taylor propagation of kinetic-only H, P8 independence of batching, P9 ETRS against dense
- * matrix polynomials and the kinetic-only closed form.  The paper prints no
+ * matrix polynomials and the kinetic-only closed form, P10 density / Poisson closed forms.  The paper prints no
  * worked H.psi example, so beyond P1-P8 parity is unpinned by the paper (stated in DESIGN.md).
  *
  * Build: gcc -O2 -std=c99 -fopenmp -shared -fPIC ref_tdh.c -o libref_tdh.so -lm   (oracle/build.py)
@@ -491,6 +492,67 @@ int ref_etrs_step(const int n[3], const double len[3], const double kpt[3], doub
     }
     free(half);
     if (!approx) free(full);
+    return e;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * exported (NEXT-2): the density, Eq. 1:  n(r) = sum_k |phi_k(r)|^2, here with optional
+ * occupations f_s (occ == NULL: all 1, Eq. 1 as printed).  "trivially parallelizable in RS points but requires a
+ * parallel reduction over states": literal loop over points, inner loop over states in order.
+ * accumulate != 0 adds to dens (partial sums of a block processed in pieces / shards).
+ * ------------------------------------------------------------------------------------------------ */
+int ref_density(const int n[3], int nst, const cplx *psi, const double *occ, double *dens, int accumulate)
+{
+    if (!n || !psi || !dens || nst < 0) return REF_EINVAL;
+    const size_t np_ = npoints(n);
+#pragma omp parallel for schedule(static)
+    for (long long p = 0; p < (long long)np_; ++p) {
+        double acc = accumulate ? dens[p] : 0.0;
+        for (int s = 0; s < nst; ++s) {
+            const cplx z = psi[(size_t)s * np_ + (size_t)p];
+            const double a = creal(z) * creal(z) + cimag(z) * cimag(z);
+            acc += (occ ? occ[s] : 1.0) * a;
+        }
+        dens[p] = acc;
+    }
+    return REF_OK;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * exported (NEXT-2): Hartree potential of a periodic density, PAPER.md:504 ("We solve the equation in FS, where the
+ * Poisson equation becomes a simple algebraic equation ... two FFTs are needed to go to FS and back"):
+ *   nabla^2 v = -4 pi n   =>   v_hat(G) = 4 pi n_hat(G) / |G|^2  for G != 0,   v_hat(0) = 0
+ * (the G = 0 component of a periodic charge is compensated by the ionic background; periodic boundary conditions
+ * only -- the paper's free-boundary kernel is out of scope).  G_a = 2 pi m(a) / L_a with the frequency convention R7;
+ * no Bloch vector enters: the density is periodic.  The result is the real part of the inverse transform.
+ * ------------------------------------------------------------------------------------------------ */
+int ref_hartree(const int n[3], const double len[3], const double *dens, double *vh, int backend)
+{
+    if (check_geometry(n, len) || !dens || !vh) return REF_EINVAL;
+    const size_t np_ = npoints(n);
+    const double two_pi = 6.283185307179586476925286766559;
+    cplx *a = (cplx *)malloc(sizeof(cplx) * np_);
+    if (!a) return REF_ENOMEM;
+    for (size_t p = 0; p < np_; ++p) a[p] = dens[p];
+    int e = dft3d_one(n, a, -1, backend);
+    if (e == REF_OK) {
+        for (int i = 0; i < n[0]; ++i) {
+            const double gx = two_pi * freq_index(i, n[0]) / len[0];
+            for (int j = 0; j < n[1]; ++j) {
+                const double gy = two_pi * freq_index(j, n[1]) / len[1];
+                for (int k = 0; k < n[2]; ++k) {
+                    const double gz = two_pi * freq_index(k, n[2]) / len[2];
+                    const double g2 = (gx * gx + gy * gy) + gz * gz;
+                    const size_t p = ((size_t)i * n[1] + j) * n[2] + k;
+                    a[p] = (g2 > 0.0) ? a[p] * (2.0 * two_pi / g2) : 0.0;
+                }
+            }
+        }
+        e = dft3d_one(n, a, +1, backend);
+    }
+    if (e == REF_OK)
+        for (size_t p = 0; p < np_; ++p) vh[p] = creal(a[p]);
+    free(a);
     return e;
 }
 

@@ -417,6 +417,54 @@ def test_p9_etrs_kinetic_only_closed_form(oracle):
         assert rel(approx, np.fft.ifftn(taylor4(t * dt) * f0, axes=(1, 2, 3))) < 1e-12
 
 
+# --------------------------------------------------------------------------------------------- P10 (NEXT-2)
+def test_p10_density_definition_and_integral(oracle):
+    """Eq. 1 by hand on a tiny grid; integral = sum of occupations for normalised states; accumulation in two pieces."""
+    cfg = small_cfg(113, n=(4, 3, 5), length=(4.0, 3.3, 5.5), natoms=0, lmax=0)
+    psi = W.states(cfg)                                    # 3 normalised states
+    occ = np.array([2.0, 1.0, 0.25])
+    d = oracle.density(cfg.n, psi, occ)
+    assert np.abs(d - np.einsum("s,sxyz->xyz", occ, np.abs(psi) ** 2)).max() < 1e-15 * d.max()
+    assert abs(cfg.dv * d.sum() - occ.sum()) < 1e-13
+    assert np.abs(oracle.density(cfg.n, psi) - np.sum(np.abs(psi) ** 2, axis=0)).max() < 1e-15 * d.max()
+    part = oracle.density(cfg.n, psi[:2], occ[:2])
+    both = oracle.density(cfg.n, psi[2:], occ[2:], accumulate_into=part)
+    assert np.abs(both - d).max() < 1e-15 * d.max()
+
+
+@pytest.mark.parametrize("n,length", [((8, 6, 4), (5.0, 4.0, 3.0)), ((6, 6, 9), (4.0, 4.5, 7.0))])
+def test_p10_hartree_plane_wave_closed_form(oracle, n, length):
+    """n = cos(G0.r) is an eigenfunction of the periodic Poisson operator: v = 4 pi / |G0|^2 cos(G0.r); a constant gives 0
+    (G = 0 dropped); the Nyquist wave of an even axis; linearity."""
+    ii = np.meshgrid(*[np.arange(m) for m in n], indexing="ij")
+    for backend in (0, 1):
+        total, expect = np.zeros(n), np.zeros(n)
+        for w, m in [(1.0, (1, 0, 0)), (-0.5, (0, 2, 1)), (0.3, (-1, 1, -2)), (0.7, (n[0] // 2, 0, 0))]:
+            phase = TWO_PI * sum(m[a] * ii[a] / n[a] for a in range(3))
+            g2 = sum((TWO_PI * m[a] / length[a]) ** 2 for a in range(3))
+            dens = np.cos(phase)
+            v = oracle.hartree(n, length, dens, backend)
+            assert rel(v, 4 * np.pi / g2 * dens) < 1e-13
+            total += w * dens
+            expect += w * 4 * np.pi / g2 * dens
+        assert rel(oracle.hartree(n, length, total + 3.7, backend), expect) < 1e-13
+        assert np.abs(oracle.hartree(n, length, np.full(n, 2.5), backend)).max() < 1e-13
+
+
+def test_p10_hartree_satisfies_the_poisson_equation(oracle):
+    """Spectral Laplacian of v_H (numpy FFT, independent of the oracle's DFT) equals -4 pi (n - mean n); v_H has zero mean."""
+    n, length = (6, 8, 5), (5.0, 6.0, 4.5)
+    rng = np.random.default_rng(10)
+    dens = rng.uniform(0.0, 1.0, n)
+    v = oracle.hartree(n, length, dens, 0)
+    g = [TWO_PI * np.fft.fftfreq(n[a], d=1.0 / n[a]) / length[a] for a in range(3)]
+    g2 = g[0][:, None, None] ** 2 + g[1][None, :, None] ** 2 + g[2][None, None, :] ** 2
+    lap = np.real(np.fft.ifftn(-g2 * np.fft.fftn(v)))
+    assert rel(lap, -4 * np.pi * (dens - dens.mean())) < 1e-12
+    assert abs(v.mean()) < 1e-13
+    assert rel(oracle.hartree(n, length, dens, 1), v) < 1e-13
+
+
 # --------------------------------------------------------------------------------------------- P8
 def test_p8_independent_of_batching(oracle):
     cfg = W.CONFIGS["tiny"]
