@@ -376,6 +376,29 @@ def sweep_leg(torch, B, name, flush, reps=7):
             res["etrs"] = {"steps": nsteps_e, "dt": cfg.dt, "seconds_per_step": te / nsteps_e,
                            "h_applications_per_step": 8, "h_application_equivalents_per_s": units * 8 * nsteps_e / te,
                            "unit": UNIT, "note": "tdh_etrs_step: taylor pair (4 H) + potential switch + half step (4 H)"}
+            # NEXT-2: density (Eq. 1) of the whole block, Hartree solve, and the self-consistent (Hartree-only) ETRS step
+            dens = g.density(psi)
+            vh = g.hartree(dens)
+            torch.cuda.synchronize()
+            td = statistics.median(timed_each(torch, lambda: g.density(psi, out=dens), 5, flush))
+            th = statistics.median(timed_each(torch, lambda: g.hartree(dens, out=vh), 5, None))
+            work.copy_(psi)
+
+            def scf_step():
+                g.set_potential(vdev + g.hartree(g.density(work)))
+                approx = g.taylor_pair(work, cfg.dt, full=out)
+                g.set_potential(vdev + g.hartree(g.density(approx)))
+                g.propagate(work, 0.5 * cfg.dt, 1)
+            scf_step()
+            torch.cuda.synchronize()
+            work.copy_(psi)
+            ts = timed_each(torch, scf_step, 1, flush)[0]
+            res["density_hartree"] = {
+                "density_seconds": td, "density_gbs": units * 16 / td * 1e-9, "hartree_seconds": th,
+                "self_consistent_etrs_seconds_per_step": ts,
+                "note": "tdh_density over the whole block (16 B per state*gridpoint read), tdh_hartree (one-state FFT pair, "
+                        "launch bound), and one ETRS step with V(t+dt) = V_ext + v_H[n(t+dt)] rebuilt from Eq. 7's states"}
+            g.set_potential(vdev)
     del psi, out
     torch.cuda.empty_cache()
     return res
@@ -480,6 +503,7 @@ def main():
         if "tddft" in wls and "propagate" in wls["tddft"]:
             extra["propagate"] = wls["tddft"].pop("propagate")
             extra["etrs"] = wls["tddft"].pop("etrs")
+            extra["density_hartree"] = wls["tddft"].pop("density_hartree")
     else:
         g.close()
 

@@ -113,6 +113,19 @@ int tdh_taylor_pair(tdh_grid* g, int nst, tdh_c128* psi_dev, tdh_c128* full_dev,
  * approx_dev: DEVICE work/output block of the size of psi_dev, must not overlap it. */
 int tdh_etrs_step(tdh_grid* g, int nst, tdh_c128* psi_dev, tdh_c128* approx_dev, double dt, const double* v_next_dev);
 
+/* Density, Eq. 1:  n[p] = sum_s occ[s] |psi_s[p]|^2  over the nst states of the block ("a parallel
+ * reduction over states"; with states sharded over GPUs the caller all-reduces n_dev afterwards).
+ *   psi_dev   DEVICE  nst*n0*n1*n2 complex128         occ_host  HOST [nst] occupations, or NULL for all 1
+ *   n_dev     DEVICE  n0*n1*n2 doubles                accumulate != 0: added to n_dev (blocks processed in pieces)
+ * States are summed in order (deterministic).  Asynchronous on the handle's stream (synchronises once if occ_host). */
+int tdh_density(tdh_grid* g, int nst, const tdh_c128* psi_dev, const double* occ_host, double* n_dev, int accumulate);
+
+/* Hartree potential of a periodic density (the Poisson equation solved in Fourier space):
+ *   v_hat(G) = 4 pi n_hat(G) / |G|^2 for G != 0, v_hat(0) = 0;  periodic boundary conditions only.
+ * n_dev, vh_dev: DEVICE, n0*n1*n2 doubles each (may be the same array).  Uses the handle's workspace: do not run
+ * concurrently with other calls on the same handle.  Asynchronous on the handle's stream. */
+int tdh_hartree(tdh_grid* g, const double* n_dev, double* vh_dev);
+
 /* The same two operations with HOST buffers (pageable or pinned): the library stages state chunks through its own
  * pinned buffers, overlapping host<->device copies with the kernels, and returns when hpsi_host / psi_host is complete.
  * nst is not limited by max_states here (chunks are).  These are the end-to-end entry points timed by bench.py. */

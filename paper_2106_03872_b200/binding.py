@@ -25,7 +25,7 @@ LIB_PATH = os.path.join(_HERE, "libtdh.so")
 #: every symbol include/tdh.h declares
 SYMBOLS = (
     "tdh_create_grid", "tdh_destroy_grid", "tdh_set_potential", "tdh_set_projectors", "tdh_apply_hamiltonian",
-    "tdh_propagate", "tdh_taylor_pair", "tdh_etrs_step", "tdh_apply_hamiltonian_host", "tdh_propagate_host", "tdh_fft3d", "tdh_last_launch_count",
+    "tdh_propagate", "tdh_taylor_pair", "tdh_etrs_step", "tdh_density", "tdh_hartree", "tdh_apply_hamiltonian_host", "tdh_propagate_host", "tdh_fft3d", "tdh_last_launch_count",
     "tdh_set_profiling", "tdh_last_kernel_seconds", "tdh_kernel_name", "tdh_set_chunk_states", "tdh_last_error",
 )
 NKERNELS = 5
@@ -60,6 +60,8 @@ def lib() -> C.CDLL:
     l.tdh_propagate.argtypes = [vp, i, vp, d, i, i]
     l.tdh_taylor_pair.argtypes = [vp, i, vp, vp, d, i]
     l.tdh_etrs_step.argtypes = [vp, i, vp, vp, d, vp]
+    l.tdh_density.argtypes = [vp, i, vp, vp, vp, i]
+    l.tdh_hartree.argtypes = [vp, vp, vp]
     l.tdh_apply_hamiltonian_host.argtypes = [vp, i, vp, vp]
     l.tdh_propagate_host.argtypes = [vp, i, vp, d, i, i]
     l.tdh_fft3d.argtypes = [vp, i, vp, i]
@@ -197,6 +199,30 @@ class Grid:
             vp_ = C.c_void_p(v_next.data_ptr())
         _check(lib().tdh_etrs_step(self._h, nst, C.c_void_p(psi.data_ptr()), C.c_void_p(approx.data_ptr()), float(dt), vp_))
         return approx
+
+    def density(self, psi, occ=None, out=None, accumulate: bool = False):
+        """n(r) = sum_s occ[s] |psi_s(r)|^2 (Eq. 1) of the block on this device; occ: host numpy array or None (all 1)."""
+        import torch
+        nst = self._block(psi)
+        if out is None:
+            assert not accumulate
+            out = torch.empty(self.n, dtype=torch.float64, device=psi.device)
+        assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == self.npts
+        occ_arr = None if occ is None else np.ascontiguousarray(occ, dtype=np.float64)
+        assert occ_arr is None or occ_arr.size == nst
+        _check(lib().tdh_density(self._h, nst, C.c_void_p(psi.data_ptr()),
+                                 None if occ_arr is None else C.c_void_p(occ_arr.ctypes.data),
+                                 C.c_void_p(out.data_ptr()), 1 if accumulate else 0))
+        return out
+
+    def hartree(self, dens, out=None):
+        """Periodic Hartree potential of a density (device float64 tensor of the grid's shape)."""
+        import torch
+        assert dens.is_cuda and dens.dtype == torch.float64 and dens.is_contiguous() and dens.numel() == self.npts
+        if out is None:
+            out = torch.empty_like(dens)
+        _check(lib().tdh_hartree(self._h, C.c_void_p(dens.data_ptr()), C.c_void_p(out.data_ptr())))
+        return out
 
     def fft3d(self, psi, sign: int):
         nst = self._block(psi)

@@ -20,6 +20,7 @@ struct XLaunch {
     const void* fused;  // xpencil_kernel<NX,S,0>
     const void* fwd;    // xpencil_kernel<NX,S,1>
     const void* inv;    // xpencil_kernel<NX,S,2>
+    const void* poisson;  // xpencil_kernel<NX,S,3>
     int threads;
     size_t smem;        // dynamic shared memory per CTA (ring of tiles)
 };

@@ -82,7 +82,11 @@ struct tdh_grid {
     cd* d_twy_w;          // exp(+2 pi i k / NY) per row pair of the work layout (y-split grids)
     int* d_rowmap;        // natural ky -> plane row of the work layout
     int* d_colmap;        // natural kz -> column of the work layout
-    int ctas_fwd, ctas_inv[tdh::NL_NCM], ctas_x[3];   // persistent grid sizes (SM count x resident CTAs)
+    double* d_p2x;        // |G_x|^2 (no Bloch vector): Poisson solver, natural x order
+    double* d_p2y_w;      // |G_y|^2, work-layout order
+    double* d_p2z_w;      // |G_z|^2, work-layout order
+    double* d_occ;        // [max_states] occupations of the last tdh_density call
+    int ctas_fwd, ctas_inv[tdh::NL_NCM], ctas_x[4];   // persistent grid sizes (SM count x resident CTAs)
 
     int chunk_cap;        // states the workspace can hold
     int chunk;            // states pushed through the chain together
@@ -207,11 +211,11 @@ extern "C" int tdh_create_grid(const int n[3], const double len[3], const double
         int dev = 0, nsm = 0;
         CU(cudaGetDevice(&dev));
         CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
-        constexpr int NK = 4 + tdh::NL_NCM;
-        const void* fs[NK] = {g->tl.fwd, g->xl.fused, g->xl.fwd, g->xl.inv};
-        size_t sm[NK] = {g->tl.smem_fwd, g->xl.smem, g->xl.smem, g->xl.smem};
-        int th[NK] = {g->tl.threads, g->xl.threads, g->xl.threads, g->xl.threads};
-        for (int i = 0; i < tdh::NL_NCM; ++i) { fs[4 + i] = g->tl.inv[i]; sm[4 + i] = g->tl.smem_inv; th[4 + i] = g->tl.threads; }
+        constexpr int NK = 5 + tdh::NL_NCM;
+        const void* fs[NK] = {g->tl.fwd, g->xl.fused, g->xl.fwd, g->xl.inv, g->xl.poisson};
+        size_t sm[NK] = {g->tl.smem_fwd, g->xl.smem, g->xl.smem, g->xl.smem, g->xl.smem};
+        int th[NK] = {g->tl.threads, g->xl.threads, g->xl.threads, g->xl.threads, g->xl.threads};
+        for (int i = 0; i < tdh::NL_NCM; ++i) { fs[5 + i] = g->tl.inv[i]; sm[5 + i] = g->tl.smem_inv; th[5 + i] = g->tl.threads; }
         int ctas[NK];
         for (int i = 0; i < NK; ++i) {
             CU(cudaFuncSetAttribute(fs[i], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm[i]));
@@ -223,8 +227,8 @@ extern "C" int tdh_create_grid(const int n[3], const double len[3], const double
             ctas[i] = nsm * occ;
         }
         g->ctas_fwd = ctas[0];
-        g->ctas_x[0] = ctas[1]; g->ctas_x[1] = ctas[2]; g->ctas_x[2] = ctas[3];
-        for (int i = 0; i < tdh::NL_NCM; ++i) g->ctas_inv[i] = ctas[4 + i];
+        g->ctas_x[0] = ctas[1]; g->ctas_x[1] = ctas[2]; g->ctas_x[2] = ctas[3]; g->ctas_x[3] = ctas[4];
+        for (int i = 0; i < tdh::NL_NCM; ++i) g->ctas_inv[i] = ctas[5 + i];
         // tables: built on the host exactly as the oracle builds its G vectors (two_pi * m / L + k, then squared)
         const double two_pi = 6.283185307179586476925286766559;
         for (int a = 0; a < 3; ++a) {
@@ -275,6 +279,18 @@ extern "C" int tdh_create_grid(const int n[3], const double len[3], const double
             CU(cudaMemcpy(g->d_twy_w, twy_w.data(), sizeof(cd) * (ny / 2), cudaMemcpyHostToDevice));
             CU(cudaMemcpy(g->d_rowmap, rowmap.data(), sizeof(int) * ny, cudaMemcpyHostToDevice));
             CU(cudaMemcpy(g->d_colmap, colmap.data(), sizeof(int) * nz, cudaMemcpyHostToDevice));
+            // |G|^2 tables of the Poisson solver (tdh_hartree): the same orders, without the Bloch vector
+            std::vector<double> p2x(n[0]), p2y_w(ny), p2z_w(nz);
+            for (int kx = 0; kx < n[0]; ++kx) { const double ga = two_pi * freq_index(kx, n[0]) / len[0]; p2x[kx] = ga * ga; }
+            for (int ky = 0; ky < ny; ++ky) { const double ga = two_pi * freq_index(ky, ny) / len[1]; p2y_w[rowmap[ky]] = ga * ga; }
+            for (int kz = 0; kz < nz; ++kz) { const double ga = two_pi * freq_index(kz, nz) / len[2]; p2z_w[colmap[kz]] = ga * ga; }
+            CU(cudaMalloc(&g->d_p2x, sizeof(double) * n[0]));
+            CU(cudaMalloc(&g->d_p2y_w, sizeof(double) * ny));
+            CU(cudaMalloc(&g->d_p2z_w, sizeof(double) * nz));
+            CU(cudaMemcpy(g->d_p2x, p2x.data(), sizeof(double) * n[0], cudaMemcpyHostToDevice));
+            CU(cudaMemcpy(g->d_p2y_w, p2y_w.data(), sizeof(double) * ny, cudaMemcpyHostToDevice));
+            CU(cudaMemcpy(g->d_p2z_w, p2z_w.data(), sizeof(double) * nz, cudaMemcpyHostToDevice));
+            CU(cudaMalloc(&g->d_occ, sizeof(double) * max_states));
         }
         CU(cudaMalloc(&g->d_v, sizeof(double) * g->np));
         CU(cudaMemset(g->d_v, 0, sizeof(double) * g->np));
@@ -303,6 +319,7 @@ extern "C" int tdh_destroy_grid(tdh_grid* g) {
     cudaFree(g->d_v);
     for (int a = 0; a < 3; ++a) { cudaFree(g->d_g2[a]); cudaFree(g->d_tw[a]); }
     cudaFree(g->d_g2y_w); cudaFree(g->d_g2z_w); cudaFree(g->d_twy_w); cudaFree(g->d_rowmap); cudaFree(g->d_colmap);
+    cudaFree(g->d_p2x); cudaFree(g->d_p2y_w); cudaFree(g->d_p2z_w); cudaFree(g->d_occ);
     cudaFree(g->d_work); cudaFree(g->d_phi[0]); cudaFree(g->d_phi[1]);
     for (int i = 0; i < 2; ++i) {
         cudaFree(g->d_hin[i]); cudaFree(g->d_hout[i]);
@@ -590,6 +607,7 @@ static int launch_xpencil(tdh_grid* g, int nst, const cd* in, cd* out, int mode)
         return fail(TDH_ECUDA, "cuTensorMapEncodeTiled failed (line map)");
     tdh::Kinetic kin;
     kin.g2x = g->d_g2[0]; kin.g2y_w = g->d_g2y_w; kin.g2z_w = g->d_g2z_w; kin.twy_w = g->d_twy_w;
+    if (mode == 3) { kin.g2x = g->d_p2x; kin.g2y_w = g->d_p2y_w; kin.g2z_w = g->d_p2z_w; }     // Poisson: pure |G|^2
     kin.ecut = g->ecut;
     kin.scale = 1.0 / (double)g->np;
     kin.nz = g->n[2];
@@ -597,7 +615,7 @@ static int launch_xpencil(tdh_grid* g, int nst, const cd* in, cd* out, int mode)
     int ntiles = nst * (g->n[1] / 2) * (g->n[2] / 16);
     const cd* twx = g->d_tw[0];
     void* args[] = {(void*)&map, (void*)&out, (void*)&ntiles, (void*)&twx, (void*)&kin};
-    const void* f = mode == 0 ? g->xl.fused : (mode == 1 ? g->xl.fwd : g->xl.inv);
+    const void* f = mode == 0 ? g->xl.fused : (mode == 1 ? g->xl.fwd : (mode == 2 ? g->xl.inv : g->xl.poisson));
     const unsigned grid = (unsigned)std::min(ntiles, g->ctas_x[mode]);
     LAUNCH(K_XPENCIL, f, dim3(grid), dim3(g->xl.threads), g->xl.smem, args);
     return TDH_OK;
@@ -871,6 +889,86 @@ extern "C" int tdh_etrs_step(tdh_grid* g, int nst, tdh_c128* psi_dev, tdh_c128* 
     const int launches = g->launch_count;
     if ((rc = propagate_block(g, nst, (cd*)psi_dev, 0.5 * dt, 1))) return rc;      // the second factor of Eq. 6
     (void)launches;
+    return prof_collect(g);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// NEXT-2: density (Eq. 1) and periodic Hartree potential
+// ------------------------------------------------------------------------------------------------------------
+// n[p] (+)= sum_s occ[s] |psi_s[p]|^2.  One thread per grid point (consecutive threads read consecutive 16-byte values of
+// one state), states summed in order: deterministic, the order of the oracle.  Eight loads in flight per thread.
+__global__ void density_kernel(const cd* __restrict__ psi, size_t npts, int nst, const double* __restrict__ occ,
+                               double* __restrict__ dens, int accumulate) {
+    const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= npts) return;
+    double acc = accumulate ? dens[p] : 0.0;
+    int s = 0;
+    for (; s + 8 <= nst; s += 8) {
+        cd v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) v[u] = __ldcs(psi + (size_t)(s + u) * npts + p);
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const double a = __dadd_rn(__dmul_rn(v[u].x, v[u].x), __dmul_rn(v[u].y, v[u].y));
+            acc = __dadd_rn(acc, __dmul_rn(occ ? occ[s + u] : 1.0, a));
+        }
+    }
+    for (; s < nst; ++s) {
+        const cd v = __ldcs(psi + (size_t)s * npts + p);
+        const double a = __dadd_rn(__dmul_rn(v.x, v.x), __dmul_rn(v.y, v.y));
+        acc = __dadd_rn(acc, __dmul_rn(occ ? occ[s] : 1.0, a));
+    }
+    dens[p] = acc;
+}
+
+__global__ void real_to_complex_kernel(const double* __restrict__ in, cd* __restrict__ out, size_t n) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+        out[i] = make_double2(in[i], 0.0);
+}
+__global__ void complex_to_real_kernel(const cd* __restrict__ in, double* __restrict__ out, size_t n) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+        out[i] = in[i].x;
+}
+
+extern "C" int tdh_density(tdh_grid* g, int nst, const tdh_c128* psi_dev, const double* occ_host, double* n_dev,
+                           int accumulate) {
+    if (!g || !psi_dev || !n_dev) return fail(TDH_EINVAL, "tdh_density: null argument");
+    if (nst < 1 || nst > g->max_states) return fail(TDH_EINVAL, "tdh_density: nst = %d outside [1, %d]", nst, g->max_states);
+    stats_reset(g);
+    const double* occ = nullptr;
+    if (occ_host) {
+        // stream-ordered after the kernels that may still read the previous occupations
+        CU(cudaMemcpyAsync(g->d_occ, occ_host, sizeof(double) * nst, cudaMemcpyHostToDevice, g->stream));
+        CU(cudaStreamSynchronize(g->stream));             // occ_host may be pageable and reused by the caller
+        occ = g->d_occ;
+    }
+    const unsigned blocks = (unsigned)((g->np + 255) / 256);
+    density_kernel<<<blocks, 256, 0, g->stream>>>((const cd*)psi_dev, g->np, nst, occ, n_dev, accumulate);
+    CU(cudaGetLastError());
+    g->launch_count += 1;
+    return TDH_OK;
+}
+
+// v_H: real -> complex, forward (z,y), x-pencil pass with the Poisson factor, inverse (y,z), real part.  One state's
+// worth of work through the same three FFT kernels as H; uses the work buffer and the first Horner buffer.
+extern "C" int tdh_hartree(tdh_grid* g, const double* n_dev, double* vh_dev) {
+    if (!g || !n_dev || !vh_dev) return fail(TDH_EINVAL, "tdh_hartree: null argument");
+    stats_reset(g);
+    cd* a = g->d_phi[0];
+    real_to_complex_kernel<<<296, 256, 0, g->stream>>>(n_dev, a, g->np);
+    CU(cudaGetLastError());
+    g->launch_count += 1;
+    int rc;
+    if ((rc = launch_plane_fwd(g, 1, a, g->d_work))) return rc;
+    if ((rc = launch_xpencil(g, 1, g->d_work, g->d_work, 3))) return rc;
+    tdh::Epilogue ep;
+    memset(&ep, 0, sizeof(ep));
+    ep.alpha = make_double2(1.0, 0.0);
+    ep.nx = g->n[0];
+    if ((rc = launch_plane_inv(g, 1, g->d_work, nullptr, a, ep))) return rc;
+    complex_to_real_kernel<<<296, 256, 0, g->stream>>>(a, vh_dev, g->np);
+    CU(cudaGetLastError());
+    g->launch_count += 1;
     return prof_collect(g);
 }
 

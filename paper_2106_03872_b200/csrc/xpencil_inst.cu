@@ -9,6 +9,7 @@ template <int NX, int S> static XLaunch make_x_launch() {
     x.fused = reinterpret_cast<const void*>(&xpencil_kernel<NX, S, 0>);
     x.fwd = reinterpret_cast<const void*>(&xpencil_kernel<NX, S, 1>);
     x.inv = reinterpret_cast<const void*>(&xpencil_kernel<NX, S, 2>);
+    x.poisson = reinterpret_cast<const void*>(&xpencil_kernel<NX, S, 3>);
     x.threads = XCfg<NX>::T;
     x.smem = XCfg<NX>::SMEM;
     return x;

@@ -29,6 +29,8 @@
 //   X_0 = A_0 + w A_1,  X_1 = A_0 - w A_1,   F_0 = f_0 X_0 + f_1 X_1,  F_1 = conj(w) (f_0 X_0 - f_1 X_1)
 //   =>  F_h = (f_0 + f_1) A_h + (f_0 - f_1) w_h A_(1-h),   w_0 = w, w_1 = conj(w):  one register exchange per value.
 // MODE 0: forward x, kinetic, inverse x.   MODE 1: forward x only (spectrum out, work layout).
+// MODE 3: as MODE 0 with the Poisson factor 4 pi / |G|^2 (G = 0 dropped) in place of the kinetic one (tdh_hartree;
+//         the tables in `Kinetic` are then those of the pure reciprocal vectors, without the Bloch vector).
 // MODE 2: inverse x only, times `scale` (spectrum in, work layout).
 #pragma once
 #include "fft_codelets.cuh"
@@ -76,6 +78,15 @@ __device__ __forceinline__ double kin_factor(double gx2, double gy2, double gz2,
     const double tk = __dmul_rn(0.5, __dadd_rn(__dadd_rn(gx2, gy2), gz2));
     return (ecut > 0.0 && !(tk <= ecut)) ? 0.0 : tk * scale;
 }
+// the Poisson factor 4 pi / |G|^2, 0 for G = 0, times 1/N_p; |G|^2 summed in the oracle's order
+__device__ __forceinline__ double poisson_factor(double gx2, double gy2, double gz2, double scale) {
+    const double g2 = __dadd_rn(__dadd_rn(gx2, gy2), gz2);
+    return g2 > 0.0 ? __ddiv_rn(12.566370614359172953850573533118, g2) * scale : 0.0;
+}
+template <int MODE>
+__device__ __forceinline__ double diag_factor(double gx2, double gy2, double gz2, double ecut, double scale) {
+    return MODE == 3 ? poisson_factor(gx2, gy2, gz2, scale) : kin_factor(gx2, gy2, gz2, ecut, scale);
+}
 
 // grid: persistent CTAs; ntiles = nst * (NY/2) * (NZ/16).  in (through `map`) and out may be the same buffer: a tile
 // is read completely before any of its lines is written.
@@ -107,7 +118,7 @@ xpencil_kernel(const __grid_constant__ CUtensorMap map, cd* __restrict__ out, in
     }
     for (int i = tid; i < NX; i += C::T) {
         stw[i] = __ldg(tw_x + i);
-        sg2x[i] = (MODE == 0) ? __ldg(kin.g2x + i) : 0.0;
+        sg2x[i] = (MODE == 0 || MODE == 3) ? __ldg(kin.g2x + i) : 0.0;
     }
     __syncthreads();
     auto issue = [&](int t, int b) {                    // thread 0 only
@@ -134,7 +145,7 @@ xpencil_kernel(const __grid_constant__ CUtensorMap map, cd* __restrict__ out, in
         // per-line constants of this tile (in flight while the tile arrives)
         double gy2a = 0.0, gy2b = 0.0, gz2 = 0.0;
         cd w = make_double2(1.0, 0.0);
-        if (MODE == 0) {
+        if (MODE == 0 || MODE == 3) {
             gz2 = __ldg(kin.g2z_w + zp);
             gy2a = __ldg(kin.g2y_w + (S == 2 ? 2 * rho2 : Y));
             if (S == 2) gy2b = __ldg(kin.g2y_w + 2 * rho2 + 1);
@@ -212,16 +223,16 @@ xpencil_kernel(const __grid_constant__ CUtensorMap map, cd* __restrict__ out, in
 #pragma unroll
                     for (int j2 = 0; j2 < R2; ++j2) xr[j2] = sm[(k1 * R2 + j2) * L + l];
                     Dft<R2, -1>::run(xr);
-                    if (MODE == 0) {
+                    if (MODE == 0 || MODE == 3) {
 #pragma unroll
                         for (int k2 = 0; k2 < R2; ++k2) {
                             const double gx2 = sg2x[k1 + R1 * k2];
                             if (S == 1) {
-                                xr[k2] = cscale(xr[k2], kin_factor(gx2, gy2a, gz2, kin.ecut, kin.scale));
+                                xr[k2] = cscale(xr[k2], diag_factor<MODE>(gx2, gy2a, gz2, kin.ecut, kin.scale));
                             } else {
                                 // the radix-2 step of the y transform folded into the factor (header comment)
-                                const double fa = kin_factor(gx2, gy2a, gz2, kin.ecut, kin.scale);
-                                const double fb = kin_factor(gx2, gy2b, gz2, kin.ecut, kin.scale);
+                                const double fa = diag_factor<MODE>(gx2, gy2a, gz2, kin.ecut, kin.scale);
+                                const double fb = diag_factor<MODE>(gx2, gy2b, gz2, kin.ecut, kin.scale);
                                 const cd wh = half ? w : make_double2(w.x, -w.y);
                                 const cd other = shfl16(xr[k2]);
                                 const cd wo = cmul(wh, other);

@@ -1,8 +1,10 @@
 """State sharding for multi-GPU runs (Fig. 7).
 
 Each state's H psi and each Taylor chain is independent of every other state, so a block is split into contiguous
-state ranges, one per rank, with V and the projector tables replicated.  There is no collective on the data path;
-torch.distributed is used only for the barrier and the max-over-ranks timing in bench.py.
+state ranges, one per rank, with V and the projector tables replicated.  There is no collective on the path of H|psi> and
+of the Taylor steps; torch.distributed supplies the barrier and the max-over-ranks timing in bench.py, and the one real
+exchange step of a self-consistent propagation: the sum of the per-shard densities (Eq. 1, "requires a parallel reduction
+over states") -- one all-reduce of N_p doubles per step (NCCL over NVLink on GPUs, gloo in the CPU tests).
 """
 from __future__ import annotations
 
@@ -28,3 +30,14 @@ def max_over_ranks(seconds: float) -> float:
     t = torch.tensor([seconds], dtype=torch.float64, device=dev)
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return float(t.item())
+
+
+def allreduce_density(dens):
+    """Sum the per-rank partial densities (tdh_density of each rank's states) in place; no-op without a process group.
+
+    `dens` is a float64 tensor of the grid's shape, on the GPU under NCCL, on the CPU under gloo.
+    """
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(dens, op=dist.ReduceOp.SUM)
+    return dens

@@ -258,3 +258,71 @@ def test_degenerate_projectors(torch_cuda, B, oracle, monkeypatch, mode):
         base = g.apply_hamiltonian(torch.from_numpy(psi).cuda()).cpu().numpy()
         diff = (out - base).reshape(cfg.nst, -1)
         assert np.abs(diff[:, 123]).min() > 1e-6
+
+
+# ------------------------------------------------------------------------------------------------ NEXT-2: density, Hartree
+@pytest.mark.parametrize("name,nst", [("tiny", 8), ("small", 37), ("medium", 19)])
+def test_density_matches_oracle(torch_cuda, B, oracle, name, nst):
+    """tdh_density (Eq. 1) with and without occupations, in one piece and accumulated over two pieces (the sharded form)."""
+    torch = torch_cuda
+    cfg = W.CONFIGS[name]
+    psi = W.states(cfg, 0, nst)
+    rng = np.random.default_rng([W.BASE_SEED + cfg.cid, 8])
+    occ = rng.uniform(0.0, 2.0, nst)
+    with B.Grid(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, nst) as g:
+        d = torch.from_numpy(psi).cuda()
+        for o in (None, occ):
+            ref = oracle.density(cfg.n, psi, o)
+            got = g.density(d, o).cpu().numpy()
+            assert np.abs(got - ref).max() <= 1e-13 * np.abs(ref).max()
+        cut = nst // 3 + 1
+        part = g.density(d[:cut], occ[:cut])
+        g.density(d[cut:], occ[cut:], out=part, accumulate=True)
+        assert np.abs(part.cpu().numpy() - ref).max() <= 1e-13 * np.abs(ref).max()
+
+
+@pytest.mark.parametrize("n,length", [((16, 16, 16), (10.0, 10.0, 10.0)), ((32, 48, 16), (9.0, 14.0, 5.0)),
+                                      ((96, 96, 32), (30.0, 30.0, 10.0)), ((64, 64, 64), (25.0, 25.0, 25.0))])
+def test_hartree_matches_oracle_and_closed_form(torch_cuda, B, oracle, n, length):
+    """tdh_hartree against the oracle on a seeded density, and against 4 pi / |G|^2 cos(G.r) directly."""
+    torch = torch_cuda
+    rng = np.random.default_rng([W.BASE_SEED, 9, n[0], n[1]])
+    dens = rng.uniform(0.0, 1.0, n)
+    ref = oracle.hartree(n, length, dens, oracle.NAIVE_FFT)
+    # a Bloch vector on the handle must not enter the Poisson solve
+    with B.Grid(n, length, (0.1, -0.2, 0.05), -1.0, 1) as g:
+        got = g.hartree(torch.from_numpy(dens).cuda()).cpu().numpy()
+        assert np.linalg.norm(got - ref) <= TOL * np.linalg.norm(ref)
+        ii = np.meshgrid(*[np.arange(m) for m in n], indexing="ij")
+        for m in [(1, 0, 0), (0, -2, 3), (n[0] // 2, 1, 0), (3, 5, -7)]:
+            wave = np.cos(2 * np.pi * sum(m[a] * ii[a] / n[a] for a in range(3)))
+            g2 = sum((2 * np.pi * m[a] / length[a]) ** 2 for a in range(3))
+            v = g.hartree(torch.from_numpy(wave + 0.3).cuda()).cpu().numpy()
+            assert np.abs(v - 4 * np.pi / g2 * wave).max() < 1e-11 * 4 * np.pi / g2
+        d = torch.from_numpy(dens).cuda()
+        g.hartree(d, out=d)                                 # in place
+        assert np.linalg.norm(d.cpu().numpy() - ref) <= TOL * np.linalg.norm(ref)
+
+
+def test_self_consistent_etrs_step_with_hartree(torch_cuda, B, oracle):
+    """The paper's loop (Eq. 6-7) closed with the Hartree term: approx -> n(t+dt) -> v_H -> H(t+dt) -> second half step,
+    composed from tdh_taylor_pair, tdh_density, tdh_hartree, tdh_set_potential, tdh_propagate; same composition of the oracle."""
+    torch = torch_cuda
+    cfg = W.CONFIGS["small"]
+    wl = W.make(cfg)
+    nst = 12
+    psi = W.states(cfg, 0, nst)
+    occ = np.full(nst, 2.0)
+    dt = 0.02
+    v0 = wl.v + oracle.hartree(cfg.n, cfg.length, oracle.density(cfg.n, psi, occ))
+    half_ref, approx_ref = oracle.taylor_pair(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, v0, wl.proj, psi, dt)
+    v1 = wl.v + oracle.hartree(cfg.n, cfg.length, oracle.density(cfg.n, approx_ref, occ))
+    out_ref = oracle.propagate(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, v1, wl.proj, half_ref, 0.5 * dt, 1)
+    with B.grid_for(wl, max_states=nst) as g:
+        vext = torch.from_numpy(wl.v).cuda()
+        d = torch.from_numpy(psi).cuda()
+        g.set_potential(vext + g.hartree(g.density(d, occ)))
+        approx = g.taylor_pair(d, dt)
+        g.set_potential(vext + g.hartree(g.density(approx, occ)))
+        g.propagate(d, 0.5 * dt, 1)
+        assert per_state_rel(d.cpu().numpy(), out_ref).max() < TOL

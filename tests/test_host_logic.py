@@ -126,6 +126,16 @@ dist.all_gather_object(got, (s0, s1))
 assert got == [(0, 5), (5, 9)], got
 t = shard.max_over_ranks(1.0 + rank)
 assert t == 2.0, t
+# NEXT-2: the density of a state block is the all-reduced sum of the shard densities (Eq. 1, PAPER.md:474)
+import numpy as np
+from paper_2106_03872_b200 import workloads as W
+cfg = W.test_config(150, (4, 3, 5), (4.0, 3.0, 5.0), nst=9, natoms=0)
+psi = W.states(cfg)
+occ = np.linspace(0.5, 2.0, 9)
+part = torch.from_numpy(np.einsum("s,sxyz->xyz", occ[s0:s1], np.abs(psi[s0:s1]) ** 2))
+shard.allreduce_density(part)
+full = np.einsum("s,sxyz->xyz", occ, np.abs(psi) ** 2)
+assert np.abs(part.numpy() - full).max() < 1e-14 * full.max()
 dist.barrier()
 dist.destroy_process_group()
 print("ok", rank)
