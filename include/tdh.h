@@ -11,6 +11,8 @@
  *       local potential: pointwise product in real space
  *       non-local Kleinman-Bylander projectors on spheres in real space                     Eq. 9
  *     exp(-i dt H) psi ~= sum_{k=0..4} (-i dt)^k / k! H^k psi          Eq. 8
+ *     ETRS step from two such sums sharing H^k psi                       Eq. 6-7
+ *     n(r) = sum_s f_s |psi_s(r)|^2;  v_H from the periodic Poisson equation in Fourier space   Eq. 1
  *
  * Conventions (readings R1-R16 of DESIGN.md): orthorhombic periodic cell, atomic units (Hartree, bohr).
  * Grid point (i,j,k) sits at r = (i h_x, j h_y, k h_z), h_a = len[a]/n[a]; flat index p = (i*n[1] + j)*n[2] + k.
