@@ -224,19 +224,34 @@ xpencil_kernel(const __grid_constant__ CUtensorMap map, cd* __restrict__ out, in
                     for (int j2 = 0; j2 < R2; ++j2) xr[j2] = sm[(k1 * R2 + j2) * L + l];
                     Dft<R2, -1>::run(xr);
                     if (MODE == 0 || MODE == 3) {
+                        // Without a cutoff mask no decision hangs on the bits of t, and the kinetic factor is affine in
+                        // (G_x+k_x)^2: f = fx * gx2 + f0 with per-line constants (one FMA per value instead of the
+                        // masked evaluation in the oracle's order); for the split y transform f_0 + f_1 is affine in
+                        // gx2 as well and f_0 - f_1 does not depend on it.
+                        const bool affine = MODE == 0 && !(kin.ecut > 0.0);
+                        const double hs = 0.5 * kin.scale;
+                        const double f0a = hs * (gy2a + gz2), f0b = hs * (gy2b + gz2);
+                        const cd wh = half ? w : make_double2(w.x, -w.y);
 #pragma unroll
                         for (int k2 = 0; k2 < R2; ++k2) {
                             const double gx2 = sg2x[k1 + R1 * k2];
                             if (S == 1) {
-                                xr[k2] = cscale(xr[k2], diag_factor<MODE>(gx2, gy2a, gz2, kin.ecut, kin.scale));
+                                const double f = affine ? fma(hs, gx2, f0a) : diag_factor<MODE>(gx2, gy2a, gz2, kin.ecut, kin.scale);
+                                xr[k2] = cscale(xr[k2], f);
                             } else {
                                 // the radix-2 step of the y transform folded into the factor (header comment)
-                                const double fa = diag_factor<MODE>(gx2, gy2a, gz2, kin.ecut, kin.scale);
-                                const double fb = diag_factor<MODE>(gx2, gy2b, gz2, kin.ecut, kin.scale);
-                                const cd wh = half ? w : make_double2(w.x, -w.y);
+                                double fs, fd;
+                                if (affine) {
+                                    fs = fma(kin.scale, gx2, f0a + f0b);
+                                    fd = f0a - f0b;
+                                } else {
+                                    const double fa = diag_factor<MODE>(gx2, gy2a, gz2, kin.ecut, kin.scale);
+                                    const double fb = diag_factor<MODE>(gx2, gy2b, gz2, kin.ecut, kin.scale);
+                                    fs = fa + fb;
+                                    fd = fa - fb;
+                                }
                                 const cd other = shfl16(xr[k2]);
                                 const cd wo = cmul(wh, other);
-                                const double fs = fa + fb, fd = fa - fb;
                                 xr[k2] = make_double2(fma(fs, xr[k2].x, fd * wo.x), fma(fs, xr[k2].y, fd * wo.y));
                             }
                         }
