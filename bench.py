@@ -244,9 +244,9 @@ def kernel_breakdown(torch, g, fn, steps):
 
 
 # DRAM bytes per state*gridpoint measured by ncu (dram__bytes_read.sum + dram__bytes_write.sum of one launch of each
-# kernel / the units of that launch), `large` config: profiles/r01e_summary.md.  Used for roofline.traffic only.
-NCU_DRAM_BYTES_PER_UNIT = {"large": {"nl_project": 12.98, "plane_fwd": 31.01, "xpencil": 30.97, "plane_inv": 47.35,
-                                     "nl_scatter": 22.01}}
+# kernel / the units of that launch), `large` config: profiles/r01f_summary.md.  Used for roofline.traffic only.
+NCU_DRAM_BYTES_PER_UNIT = {"large": {"nl_project": 12.97, "plane_fwd": 31.00, "xpencil": 31.17, "plane_inv": 47.39,
+                                     "nl_scatter": 21.99}}
 
 
 def alg_bytes(wl):
@@ -274,7 +274,7 @@ def roofline_of(kern_s, units, peak_gbs, peak_src, bytes_per_unit, workload=None
     if per_unit and units_per_launch:
         traffic = {"bytes_per_launch": per_unit * units_per_launch, "algorithmic_bytes_per_launch":
                    bytes_per_unit[top] * units_per_launch, "units_per_launch": units_per_launch,
-                   "source": "profiles/r01e_summary.md (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum per "
+                   "source": "profiles/r01f_summary.md (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum per "
                              "state*gridpoint of one launch, scaled to this run's launch size)"}
     return {"kernel": top, "bound": "hbm", "achieved": round(achieved, 1), "peak": peak_gbs, "unit": "GB/s",
             "frac": round(achieved / peak_gbs, 4), "traffic": traffic, "peak_source": peak_src,
