@@ -1,11 +1,15 @@
 // tdh.cu -- C ABI of libtdh.so (include/tdh.h): handle, tables, projector re-indexing, launch orchestration.
 //
-// One Hamiltonian application on a chunk of states is four launches:
+// One Hamiltonian application on a chunk of states is four launches, plus one per atom colour on split-tile grids:
 //     nl_project  (gather + FP64-MMA projection, only with projectors)
 //     plane_fwd   (tile_fwd: z,y forward FFT per tile of a (state,x) plane)   in  -> work
 //     xpencil     (x forward, 1/2|G+k|^2 scale + mask, x inverse)             work in place
-//     plane_inv   (tile_inv: y,z inverse FFT + epilogue alpha*(T+V+Vnl)phi + y)  work -> out
-// The three FFT kernels are persistent (one CTA per SM, or as many as fit) and fed by TMA: the host encodes a
+//     plane_inv   (tile_inv: y,z inverse FFT + epilogue alpha*(T+V[+Vnl])phi + y)  work -> out
+//     nl_scatter  (FP64-MMA back-projection added into out; nl_mode 1 -- otherwise the back-projection runs inside
+//                  plane_inv from per-tile record lists)
+// tdh_taylor_pair / tdh_etrs_step (NEXT-1) and tdh_density / tdh_hartree (NEXT-2) are compositions of the same
+// launches plus three elementwise kernels.
+// The three FFT kernels are persistent (one or several CTAs per SM, as many as fit) and fed by TMA: the host encodes a
 // CUtensorMap per launch (tensor_maps.h) and the kernels stream tiles through a shared-memory ring.  `work` holds the
 // spectrum in the digit-permuted order the in-place transforms produce (xpencil_kernel.cuh, WORK LAYOUT).
 // States are independent, so a block is pushed through this chain chunk by chunk; a chunk is as many

@@ -2,7 +2,8 @@
 //
 //   tile_fwd : per tile: forward FFT along z then y                                   (row a1 of the scope table)
 //   tile_inv : per tile: inverse FFT along y then z, then the fused epilogue
-//              out = alpha * (T psi + V psi + V_nl psi) + y           (rows a3, a4, a5 back-projection, a6, a7 axpy)
+//              out = alpha * (T psi + V psi [+ V_nl psi]) + y         (rows a3, a4, a5 back-projection, a6, a7 axpy)
+// Both kernels run two independent warp groups per CTA on a ring of three tiles (see tile_fwd_kernel).
 //
 // TILE.  Global layout is [state][x][y][z], z fastest.  A tile is the set of rows y = S*m + r (m = 0..NY/S-1) of one
 // (state, x) plane: the whole plane when S = 1 (PPC consecutive planes when they are small), the even or the odd rows
@@ -15,8 +16,8 @@
 // (tensor_maps.h): the 128-byte line Ln = row*(NZ/8) + (z >> 3) lands at byte 128*Ln of a 1024-byte aligned buffer
 // and complex value p = z & 7 of the line at chunk p ^ (Ln & 7).  With that hardware XOR swizzle every stage below is
 // free of bank conflicts without padding: a quarter-warp always touches 8 distinct 16-byte chunks modulo 128 bytes
-// (8 positions of one line, or one position of 8 consecutive lines).  CTAs are persistent; one elected thread keeps a
-// ring of buffers filled with cp.async.bulk.tensor, so the next tiles stream in while this one is transformed.
+// (8 positions of one line, or one position of 8 consecutive lines).  CTAs are persistent; the thread that releases a
+// buffer refills it with cp.async.bulk.tensor, so the next tiles stream in while this one is transformed.
 //
 // ORDER.  1-D transforms of length N = R1*R2 run as two in-place register stages.  Forward (natural in): radix R1 over
 // j1 (stride R2), twiddle, radix R2 over j2; position k1*R2 + k2 then holds index k1 + R1*k2.  The inverse takes
