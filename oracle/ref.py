@@ -26,7 +26,7 @@ def lib() -> C.CDLL:
     if _lib is None:
         _lib = C.CDLL(_build.build())
         for name in ("ref_dft3d", "ref_kinetic", "ref_local", "ref_nonlocal", "ref_apply_hamiltonian",
-                     "ref_propagate", "ref_taylor_pair", "ref_etrs_step", "ref_density", "ref_hartree", "ref_num_threads"):
+                     "ref_propagate", "ref_taylor_pair", "ref_etrs_step", "ref_density", "ref_hartree", "ref_overlap", "ref_num_threads"):
             getattr(_lib, name).restype = C.c_int
     return _lib
 
@@ -179,6 +179,15 @@ def hartree(n, length, dens, backend: int = NAIVE_FFT) -> np.ndarray:
     out = np.empty_like(dens)
     _check(lib().ref_hartree(_i3(n), _d3(length), _ptr(dens), _ptr(out), C.c_int(backend)), "hartree")
     return out
+
+
+def overlap(n, dv: float, a, b) -> np.ndarray:
+    """S[i][j] = dV sum_p conj(a_i[p]) b_j[p] for two state blocks (na, n0, n1, n2), (nb, n0, n1, n2)."""
+    a, b = _c128(a), _c128(b)
+    na, nb = a.shape[0], b.shape[0]
+    s = np.empty((na, nb), dtype=np.complex128)
+    _check(lib().ref_overlap(_i3(n), C.c_double(dv), C.c_int(na), _ptr(a), C.c_int(nb), _ptr(b), _ptr(s)), "overlap")
+    return s
 
 
 def apply_workload(wl, psi, backend: int = NAIVE_FFT) -> np.ndarray:

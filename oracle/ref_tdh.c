@@ -27,7 +27,7 @@
  * kinetic eigenvectors incl. Nyquist and mask, P3 constant potential = shift, P4 rank / closed form of one
  * projector, P5 Hermiticity and dense-matrix spectrum, P6 Bloch-phase identity and translation covariance,
  * P7 closed-form Taylor propagation of kinetic-only H, P8 independence of batching, P9 ETRS against dense
- * matrix polynomials and the kinetic-only closed form, P10 density / Poisson closed forms.  The paper prints no
+ * matrix polynomials and the kinetic-only closed form, P10 density / Poisson closed forms, P11 overlap matrix.  The paper prints no
  * worked H.psi example, so beyond P1-P8 parity is unpinned by the paper (stated in DESIGN.md).
  *
  * Build: gcc -O2 -std=c99 -fopenmp -shared -fPIC ref_tdh.c -o libref_tdh.so -lm   (oracle/build.py)
@@ -554,6 +554,27 @@ int ref_hartree(const int n[3], const double len[3], const double *dens, double 
         for (size_t p = 0; p < np_; ++p) vh[p] = creal(a[p]);
     free(a);
     return e;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * exported (first building block of NEXT-3): overlap / subspace matrix of two state blocks,
+ *   S[i][j] = <a_i | b_j> = dV sum_p conj(a_i[p]) b_j[p],   i < na, j < nb   (row-major [na][nb])
+ * -- the matrix behind "orthogonalization and subspace diagonalization" ("rotations in the space of
+ * eigenvectors ... dominated by linear algebra operations") and behind the statement that real-time propagation
+ * "conserves orthogonality of the KS states mathematically and also numerically".  Literal loops.
+ * ------------------------------------------------------------------------------------------------ */
+int ref_overlap(const int n[3], double dv, int na, const cplx *a, int nb, const cplx *b, cplx *s)
+{
+    if (!n || !a || !b || !s || na < 0 || nb < 0) return REF_EINVAL;
+    const size_t np_ = npoints(n);
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int i = 0; i < na; ++i)
+        for (int j = 0; j < nb; ++j) {
+            cplx acc = 0.0;
+            for (size_t p = 0; p < np_; ++p) acc += conj(a[(size_t)i * np_ + p]) * b[(size_t)j * np_ + p];
+            s[(size_t)i * nb + j] = dv * acc;
+        }
+    return REF_OK;
 }
 
 /* number of OpenMP threads the block loops will use (reported by bench.py's cpu_baseline) */

@@ -465,6 +465,46 @@ def test_p10_hartree_satisfies_the_poisson_equation(oracle):
     assert rel(oracle.hartree(n, length, dens, 1), v) < 1e-13
 
 
+# --------------------------------------------------------------------------------------------- P11 (overlap matrix)
+def test_p11_overlap_plane_waves_and_hand_values(oracle):
+    """Distinct plane waves are orthogonal with norm^2 = cell volume; a 2-point hand example; conjugation on the left."""
+    n, length = (4, 6, 5), (3.0, 4.0, 5.0)
+    dv = np.prod([length[a] / n[a] for a in range(3)])
+    ii = np.meshgrid(*[np.arange(m) for m in n], indexing="ij")
+    ms = [(0, 0, 0), (1, 0, 0), (0, 2, 1), (-1, 1, 2), (1, 2, -2)]
+    pw = np.array([np.exp(2j * np.pi * sum(m[a] * ii[a] / n[a] for a in range(3))) for m in ms])
+    s = oracle.overlap(n, dv, pw, pw)
+    assert np.abs(s - np.prod(length) * np.eye(len(ms))).max() < 1e-12
+    a = np.zeros((1,) + n, dtype=np.complex128)
+    b = np.zeros((2,) + n, dtype=np.complex128)
+    a[0, 0, 0, 0], a[0, 1, 2, 3] = 1 + 2j, -1j
+    b[0, 0, 0, 0], b[1, 1, 2, 3], b[1, 0, 0, 0] = 3 - 1j, 2.0, 1j
+    s = oracle.overlap(n, 0.5, a, b)
+    assert s.shape == (1, 2)
+    assert abs(s[0, 0] - 0.5 * (1 - 2j) * (3 - 1j)) < 1e-15 and abs(s[0, 1] - 0.5 * ((1 - 2j) * 1j + 1j * 2.0)) < 1e-15
+
+
+def test_p11_overlap_is_sesquilinear_and_hermitian(oracle):
+    cfg = small_cfg(114, n=(5, 4, 6), length=(5.0, 4.4, 6.0), natoms=0, lmax=0)
+    rng = np.random.default_rng(114)
+    a, b = rand_c(rng, (3,) + cfg.n), rand_c(rng, (4,) + cfg.n)
+    s = oracle.overlap(cfg.n, cfg.dv, a, b)
+    assert np.abs(s - cfg.dv * np.einsum("ixyz,jxyz->ij", a.conj(), b)).max() < 1e-13 * np.abs(s).max()
+    assert np.abs(oracle.overlap(cfg.n, cfg.dv, b, a) - s.conj().T).max() < 1e-13 * np.abs(s).max()
+    saa = oracle.overlap(cfg.n, cfg.dv, a, a)
+    assert np.abs(saa - saa.conj().T).max() < 1e-14 * np.abs(saa).max() and np.all(np.linalg.eigvalsh(saa) > 0)
+    # normalised states of the generator have unit diagonal
+    psi = W.states(cfg)
+    assert np.abs(np.diag(oracle.overlap(cfg.n, cfg.dv, psi, psi)) - 1).max() < 1e-13
+    # Hermiticity of H as a statement about overlaps: <a|Hb> = <Ha|b> (P5 in matrix form)
+    cfgp = small_cfg(115, n=(4, 5, 6), length=(4.4, 5.0, 5.5), natoms=2, lmax=1, rc=1.9)
+    wl = W.make(cfgp)
+    x = W.states(cfgp)
+    hx = oracle.apply_workload(wl, x, 0)
+    m = oracle.overlap(cfgp.n, cfgp.dv, x, hx)
+    assert np.abs(m - m.conj().T).max() < 1e-12 * np.abs(m).max()
+
+
 # --------------------------------------------------------------------------------------------- P8
 def test_p8_independent_of_batching(oracle):
     cfg = W.CONFIGS["tiny"]
