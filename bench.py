@@ -136,6 +136,19 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def fp64_tensor_peak():
+    """FP64 tensor-core peak for the contraction legs: no FP64 GEMM was measured on this pool, so it is the measured bf16
+    peak times the nominal FP64 / bf16 ratio of B200 (45 / 2250 dense TFLOP/s, blackwell_cuda_programming.md)."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    ratio = 45.0 / 2250.0
+    if os.path.exists(path):
+        try:
+            return float(json.load(open(path))["bf16_tflops"]) * ratio, "measured bf16_tflops x 45/2250 (nominal FP64/bf16 ratio)"
+        except Exception:
+            pass
+    return 45.0, "nominal 45 TFLOP/s (no MEASURED_PEAKS.json)"
+
+
 class Dist:
     """torch.distributed plumbing: barrier and max-over-ranks only (no data-path collective)."""
 
@@ -399,6 +412,16 @@ def sweep_leg(torch, B, name, flush, reps=7):
                 "note": "tdh_density over the whole block (16 B per state*gridpoint read), tdh_hartree (one-state FFT pair, "
                         "launch bound), and one ETRS step with V(t+dt) = V_ext + v_H[n(t+dt)] rebuilt from Eq. 7's states"}
             g.set_potential(vdev)
+            # overlap matrix S = dV psi^H psi of the whole block: the one flop-bound contraction (FP64 tensor cores)
+            smat = g.overlap(psi)
+            torch.cuda.synchronize()
+            to = statistics.median(timed_each(torch, lambda: g.overlap(psi, out=smat), 5, flush))
+            peak_tf, peak_src = fp64_tensor_peak()
+            tf = 8.0 * cfg.nst * cfg.nst * cfg.npts / to * 1e-12
+            res["overlap"] = {"seconds": to, "bound": "tensor", "achieved": round(tf, 2), "peak": round(peak_tf, 2),
+                              "unit": "TFLOP/s", "frac": round(tf / peak_tf, 4), "peak_source": peak_src,
+                              "flops": "8 * nst^2 * N_p (complex128 GEMM, K = N_p)",
+                              "note": "tdh_overlap: mma.sync.m8n8k4.f64, 64x64 tiles, split-K with ordered reduction"}
     del psi, out
     torch.cuda.empty_cache()
     return res
@@ -504,6 +527,7 @@ def main():
             extra["propagate"] = wls["tddft"].pop("propagate")
             extra["etrs"] = wls["tddft"].pop("etrs")
             extra["density_hartree"] = wls["tddft"].pop("density_hartree")
+            extra["overlap"] = wls["tddft"].pop("overlap")
     else:
         g.close()
 

@@ -128,6 +128,14 @@ int tdh_density(tdh_grid* g, int nst, const tdh_c128* psi_dev, const double* occ
  * concurrently with other calls on the same handle.  Asynchronous on the handle's stream. */
 int tdh_hartree(tdh_grid* g, const double* n_dev, double* vh_dev);
 
+/* Overlap / subspace matrix of two state blocks (first building block of the ground-state rotations, PAPER.md:393;
+ * also the check that propagation keeps the states orthonormal):
+ *     S[i][j] = dV sum_p conj(a_i[p]) b_j[p],   i < na, j < nb,   row-major [na][nb] complex128
+ * a_dev, b_dev: DEVICE blocks of na / nb states (may be the same block); s_dev: DEVICE, na*nb complex128.
+ * A flop-bound complex GEMM on FP64 tensor cores, split over K with a deterministic reduction.  Uses the handle's
+ * workspace (na, nb rounded up to 64 must satisfy na*nb <= workspace / 16 bytes).  Asynchronous on the handle's stream. */
+int tdh_overlap(tdh_grid* g, int na, const tdh_c128* a_dev, int nb, const tdh_c128* b_dev, tdh_c128* s_dev);
+
 /* The same two operations with HOST buffers (pageable or pinned): the library stages state chunks through its own
  * pinned buffers, overlapping host<->device copies with the kernels, and returns when hpsi_host / psi_host is complete.
  * nst is not limited by max_states here (chunks are).  These are the end-to-end entry points timed by bench.py. */

@@ -25,7 +25,7 @@ LIB_PATH = os.path.join(_HERE, "libtdh.so")
 #: every symbol include/tdh.h declares
 SYMBOLS = (
     "tdh_create_grid", "tdh_destroy_grid", "tdh_set_potential", "tdh_set_projectors", "tdh_apply_hamiltonian",
-    "tdh_propagate", "tdh_taylor_pair", "tdh_etrs_step", "tdh_density", "tdh_hartree", "tdh_apply_hamiltonian_host", "tdh_propagate_host", "tdh_fft3d", "tdh_last_launch_count",
+    "tdh_propagate", "tdh_taylor_pair", "tdh_etrs_step", "tdh_density", "tdh_hartree", "tdh_overlap", "tdh_apply_hamiltonian_host", "tdh_propagate_host", "tdh_fft3d", "tdh_last_launch_count",
     "tdh_set_profiling", "tdh_last_kernel_seconds", "tdh_kernel_name", "tdh_set_chunk_states", "tdh_last_error",
 )
 NKERNELS = 5
@@ -62,6 +62,7 @@ def lib() -> C.CDLL:
     l.tdh_etrs_step.argtypes = [vp, i, vp, vp, d, vp]
     l.tdh_density.argtypes = [vp, i, vp, vp, vp, i]
     l.tdh_hartree.argtypes = [vp, vp, vp]
+    l.tdh_overlap.argtypes = [vp, i, vp, i, vp, vp]
     l.tdh_apply_hamiltonian_host.argtypes = [vp, i, vp, vp]
     l.tdh_propagate_host.argtypes = [vp, i, vp, d, i, i]
     l.tdh_fft3d.argtypes = [vp, i, vp, i]
@@ -222,6 +223,19 @@ class Grid:
         if out is None:
             out = torch.empty_like(dens)
         _check(lib().tdh_hartree(self._h, C.c_void_p(dens.data_ptr()), C.c_void_p(out.data_ptr())))
+        return out
+
+    def overlap(self, a, b=None, out=None):
+        """S[i][j] = dV sum_p conj(a_i[p]) b_j[p] (b = a if omitted); returns a (na, nb) complex128 device tensor."""
+        import torch
+        if b is None:
+            b = a
+        na, nb = self._block(a), self._block(b)
+        if out is None:
+            out = torch.empty((na, nb), dtype=torch.complex128, device=a.device)
+        assert out.is_cuda and out.dtype == torch.complex128 and out.is_contiguous() and out.numel() == na * nb
+        _check(lib().tdh_overlap(self._h, na, C.c_void_p(a.data_ptr()), nb, C.c_void_p(b.data_ptr()),
+                                 C.c_void_p(out.data_ptr())))
         return out
 
     def fft3d(self, psi, sign: int):

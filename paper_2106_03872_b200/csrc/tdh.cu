@@ -31,6 +31,7 @@
 #include "../../include/tdh.h"
 #include "launch_tables.h"
 #include "nl_kernels.cuh"
+#include "overlap_kernels.cuh"
 #include "tensor_maps.h"
 #include "tile_kernels.cuh"
 #include "xpencil_kernel.cuh"
@@ -974,6 +975,45 @@ extern "C" int tdh_hartree(tdh_grid* g, const double* n_dev, double* vh_dev) {
     CU(cudaGetLastError());
     g->launch_count += 1;
     return prof_collect(g);
+}
+
+// S = dV a^H b on FP64 tensor cores, split-K partials in the work buffer (overlap_kernels.cuh)
+extern "C" int tdh_overlap(tdh_grid* g, int na, const tdh_c128* a_dev, int nb, const tdh_c128* b_dev, tdh_c128* s_dev) {
+    if (!g || !a_dev || !b_dev || !s_dev) return fail(TDH_EINVAL, "tdh_overlap: null argument");
+    if (na < 1 || nb < 1) return fail(TDH_EINVAL, "tdh_overlap: na, nb must be >= 1");
+    stats_reset(g);
+    const int ti = (na + tdh::OV_T - 1) / tdh::OV_T, tj = (nb + tdh::OV_T - 1) / tdh::OV_T;
+    const size_t tile_cells = (size_t)ti * tj * tdh::OV_T * tdh::OV_T;
+    const size_t cap = (size_t)g->chunk_cap * g->np;                       // complex values the work buffer holds
+    if (tile_cells > cap) return fail(TDH_EUNSUPPORTED, "tdh_overlap: %d x %d does not fit the workspace", na, nb);
+    const size_t nchunks = g->np / tdh::OV_KC;
+    // enough slices of K for about four waves of CTAs, bounded by the workspace and by 8 chunks per slice
+    int dev = 0, nsm = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+    size_t ksplit = std::max<size_t>(1, ((size_t)8 * nsm + (size_t)ti * tj - 1) / ((size_t)ti * tj));
+    ksplit = std::min(ksplit, std::max<size_t>(1, nchunks / 8));
+    ksplit = std::min(ksplit, cap / tile_cells);
+    ksplit = std::min<size_t>(ksplit, 65535);
+    int cps = (int)((nchunks + ksplit - 1) / ksplit);
+    ksplit = (nchunks + cps - 1) / cps;
+    size_t npts = g->np;
+    int tjv = tj;
+    cd* part = g->d_work;
+    const cd* a = (const cd*)a_dev;
+    const cd* b = (const cd*)b_dev;
+    {
+        void* args[] = {(void*)&a, (void*)&na, (void*)&b, (void*)&nb, (void*)&npts, (void*)&tjv, (void*)&cps, (void*)&part};
+        CU(cudaLaunchKernel(reinterpret_cast<const void*>(&tdh::overlap_kernel), dim3(ti * tj, (unsigned)ksplit),
+                            dim3(tdh::OV_THREADS), args, 0, g->stream));
+        g->launch_count += 1;
+    }
+    const int na_pad = ti * tdh::OV_T, nb_pad = tj * tdh::OV_T, ks = (int)ksplit;
+    tdh::overlap_reduce_kernel<<<(na * nb + 255) / 256, 256, 0, g->stream>>>(part, ks, na, nb, na_pad, nb_pad, g->dv,
+                                                                            (cd*)s_dev);
+    CU(cudaGetLastError());
+    g->launch_count += 1;
+    return TDH_OK;
 }
 
 extern "C" int tdh_fft3d(tdh_grid* g, int nst, tdh_c128* psi_dev, int sign) {
