@@ -190,6 +190,26 @@ def overlap(n, dv: float, a, b) -> np.ndarray:
     return s
 
 
+def rotate(psi, m) -> np.ndarray:
+    """Rotation in the space of states: out_j = sum_i psi_i m[i][j]; psi (n_in, n0, n1, n2), m (n_in, n_out)."""
+    psi = _c128(psi)
+    m = _c128(m)
+    out = np.zeros((m.shape[1],) + psi.shape[1:], dtype=np.complex128)
+    for j in range(m.shape[1]):                 # literal loops over the two state indices
+        for i in range(m.shape[0]):
+            out[j] += psi[i] * m[i, j]
+    return out
+
+
+def orthonormalize(n, dv: float, psi) -> np.ndarray:
+    """Cholesky orthonormalisation ("orthogonalization"): S = dV psi^H psi = L L^H (library Cholesky as one
+    step), psi' = psi L^{-H}, so that dV psi'^H psi' = 1 and psi'_j only mixes psi_0..psi_j (the Gram-Schmidt order)."""
+    s = overlap(n, dv, psi, psi)
+    l = np.linalg.cholesky(0.5 * (s + s.conj().T))
+    w = np.linalg.inv(l)                         # lower triangular L^{-1}
+    return rotate(psi, w.conj().T)
+
+
 def apply_workload(wl, psi, backend: int = NAIVE_FFT) -> np.ndarray:
     """Convenience: H psi with a workloads.Workload."""
     c = wl.cfg

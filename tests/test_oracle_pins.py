@@ -505,6 +505,34 @@ def test_p11_overlap_is_sesquilinear_and_hermitian(oracle):
     assert np.abs(m - m.conj().T).max() < 1e-12 * np.abs(m).max()
 
 
+def test_p11_orthonormalize_equals_gram_schmidt(oracle):
+    """Cholesky orthonormalisation = modified Gram-Schmidt with positive normalisation (explicit loops here): unit overlap,
+    psi'_j in span(psi_0..psi_j), and the same vectors; a rotation by a unitary keeps the overlap (rotate pin)."""
+    cfg = small_cfg(116, n=(5, 6, 4), length=(5.0, 6.0, 4.0), natoms=0, lmax=0)
+    rng = np.random.default_rng(116)
+    psi = rand_c(rng, (5,) + cfg.n)
+    psi[3] = 0.7 * psi[1] + 0.3 * psi[3]                       # some correlation between the inputs
+    out = oracle.orthonormalize(cfg.n, cfg.dv, psi)
+    s = oracle.overlap(cfg.n, cfg.dv, out, out)
+    assert np.abs(s - np.eye(5)).max() < 1e-12
+    q = []
+    for j in range(5):                                         # modified Gram-Schmidt
+        v = psi[j].copy()
+        for u in q:
+            v -= u * (cfg.dv * np.vdot(u, v))
+        q.append(v / np.sqrt(cfg.dv * np.vdot(v, v).real))
+    assert rel(out, np.array(q)) < 1e-11
+    # triangular structure: <psi_i | out_j> dV is upper triangular ... equivalently out_j has no component outside span(psi_0..j)
+    c = np.linalg.lstsq(psi.reshape(5, -1).T, out.reshape(5, -1).T, rcond=None)[0]     # out = psi c
+    assert np.abs(np.tril(c, -1)).max() < 1e-10
+    # rotate: a unitary rotation of an orthonormal block stays orthonormal; a single-column rotation is a linear combination
+    u, _ = np.linalg.qr(rand_c(rng, (5, 5)))
+    r = oracle.rotate(out, u)
+    assert np.abs(oracle.overlap(cfg.n, cfg.dv, r, r) - np.eye(5)).max() < 1e-12
+    col = rand_c(rng, (5, 1))
+    assert rel(oracle.rotate(psi, col)[0], np.tensordot(col[:, 0], psi, axes=(0, 0))) < 1e-14
+
+
 # --------------------------------------------------------------------------------------------- P8
 def test_p8_independent_of_batching(oracle):
     cfg = W.CONFIGS["tiny"]
