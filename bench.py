@@ -422,6 +422,11 @@ def sweep_leg(torch, B, name, flush, reps=7):
                               "unit": "TFLOP/s", "frac": round(tf / peak_tf, 4), "peak_source": peak_src,
                               "flops": "8 * nst^2 * N_p (complex128 GEMM, K = N_p)",
                               "note": "tdh_overlap: mma.sync.m8n8k4.f64, 64x64 tiles, split-K with ordered reduction"}
+            tor = statistics.median(timed_each(torch, lambda: g.orthonormalize(psi, out=out), 3, flush))
+            res["orthonormalize"] = {"seconds": tor, "launches": g.last_launch_count(),
+                                     "effective_tflops": round(12.0 * cfg.nst * cfg.nst * cfg.npts / tor * 1e-12, 2),
+                                     "note": "tdh_orthonormalize: overlap (8 n^2 N_p flop) + cooperative Cholesky + triangular "
+                                             "inverse + upper-triangular rotation (4 n^2 N_p flop)"}
     del psi, out
     torch.cuda.empty_cache()
     return res
@@ -528,6 +533,7 @@ def main():
             extra["etrs"] = wls["tddft"].pop("etrs")
             extra["density_hartree"] = wls["tddft"].pop("density_hartree")
             extra["overlap"] = wls["tddft"].pop("overlap")
+            extra["orthonormalize"] = wls["tddft"].pop("orthonormalize")
     else:
         g.close()
 

@@ -136,6 +136,19 @@ int tdh_hartree(tdh_grid* g, const double* n_dev, double* vh_dev);
  * workspace (na, nb rounded up to 64 must satisfy na*nb <= workspace / 16 bytes).  Asynchronous on the handle's stream. */
 int tdh_overlap(tdh_grid* g, int na, const tdh_c128* a_dev, int nb, const tdh_c128* b_dev, tdh_c128* s_dev);
 
+/* Rotation in the space of states ("rotations in the space of eigenvectors"):
+ *     out_j[p] = sum_i psi_i[p] m[i][j],   i < n_in, j < n_out
+ * psi_dev: DEVICE block of n_in states; m_dev: DEVICE, row-major [n_in][n_out] complex128; out_dev: DEVICE block of
+ * n_out states, must not overlap psi_dev.  A flop-bound complex GEMM on FP64 tensor cores.  Asynchronous. */
+int tdh_rotate(tdh_grid* g, int n_in, const tdh_c128* psi_dev, int n_out, const tdh_c128* m_dev, tdh_c128* out_dev);
+
+/* Cholesky orthonormalisation ("orthogonalization"): S = dV psi^H psi = L L^H, out = psi L^{-H}, so that
+ * dV out^H out = 1 and out_j mixes psi_0..psi_j only (the Gram-Schmidt order).  tdh_overlap, a cooperative Cholesky and
+ * a triangular inverse of the nst x nst matrix, tdh_rotate.  1 <= nst <= 1024; psi_dev, out_dev: DEVICE blocks of nst
+ * states, must not overlap.  The first call (or a larger nst) allocates two nst x nst scratch matrices.
+ * Synchronises the stream; returns TDH_EINVAL when the states are linearly dependent (out is then undefined). */
+int tdh_orthonormalize(tdh_grid* g, int nst, const tdh_c128* psi_dev, tdh_c128* out_dev);
+
 /* The same two operations with HOST buffers (pageable or pinned): the library stages state chunks through its own
  * pinned buffers, overlapping host<->device copies with the kernels, and returns when hpsi_host / psi_host is complete.
  * nst is not limited by max_states here (chunks are).  These are the end-to-end entry points timed by bench.py. */

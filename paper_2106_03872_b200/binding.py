@@ -25,7 +25,7 @@ LIB_PATH = os.path.join(_HERE, "libtdh.so")
 #: every symbol include/tdh.h declares
 SYMBOLS = (
     "tdh_create_grid", "tdh_destroy_grid", "tdh_set_potential", "tdh_set_projectors", "tdh_apply_hamiltonian",
-    "tdh_propagate", "tdh_taylor_pair", "tdh_etrs_step", "tdh_density", "tdh_hartree", "tdh_overlap", "tdh_apply_hamiltonian_host", "tdh_propagate_host", "tdh_fft3d", "tdh_last_launch_count",
+    "tdh_propagate", "tdh_taylor_pair", "tdh_etrs_step", "tdh_density", "tdh_hartree", "tdh_overlap", "tdh_rotate", "tdh_orthonormalize", "tdh_apply_hamiltonian_host", "tdh_propagate_host", "tdh_fft3d", "tdh_last_launch_count",
     "tdh_set_profiling", "tdh_last_kernel_seconds", "tdh_kernel_name", "tdh_set_chunk_states", "tdh_last_error",
 )
 NKERNELS = 5
@@ -63,6 +63,8 @@ def lib() -> C.CDLL:
     l.tdh_density.argtypes = [vp, i, vp, vp, vp, i]
     l.tdh_hartree.argtypes = [vp, vp, vp]
     l.tdh_overlap.argtypes = [vp, i, vp, i, vp, vp]
+    l.tdh_rotate.argtypes = [vp, i, vp, i, vp, vp]
+    l.tdh_orthonormalize.argtypes = [vp, i, vp, vp]
     l.tdh_apply_hamiltonian_host.argtypes = [vp, i, vp, vp]
     l.tdh_propagate_host.argtypes = [vp, i, vp, d, i, i]
     l.tdh_fft3d.argtypes = [vp, i, vp, i]
@@ -236,6 +238,28 @@ class Grid:
         assert out.is_cuda and out.dtype == torch.complex128 and out.is_contiguous() and out.numel() == na * nb
         _check(lib().tdh_overlap(self._h, na, C.c_void_p(a.data_ptr()), nb, C.c_void_p(b.data_ptr()),
                                  C.c_void_p(out.data_ptr())))
+        return out
+
+    def rotate(self, psi, m, out=None):
+        """out_j = sum_i psi_i m[i][j]; m: (n_in, n_out) complex128 device tensor."""
+        import torch
+        n_in = self._block(psi)
+        assert m.is_cuda and m.dtype == torch.complex128 and m.is_contiguous() and m.dim() == 2 and m.shape[0] == n_in
+        n_out = int(m.shape[1])
+        if out is None:
+            out = torch.empty((n_out,) + self.n, dtype=torch.complex128, device=psi.device)
+        assert self._block(out) == n_out
+        _check(lib().tdh_rotate(self._h, n_in, C.c_void_p(psi.data_ptr()), n_out, C.c_void_p(m.data_ptr()),
+                                C.c_void_p(out.data_ptr())))
+        return out
+
+    def orthonormalize(self, psi, out=None):
+        """Cholesky orthonormalisation of a block (out-of-place)."""
+        import torch
+        nst = self._block(psi)
+        if out is None:
+            out = torch.empty_like(psi)
+        _check(lib().tdh_orthonormalize(self._h, nst, C.c_void_p(psi.data_ptr()), C.c_void_p(out.data_ptr())))
         return out
 
     def fft3d(self, psi, sign: int):

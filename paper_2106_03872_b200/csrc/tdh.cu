@@ -91,6 +91,9 @@ struct tdh_grid {
     double* d_p2y_w;      // |G_y|^2, work-layout order
     double* d_p2z_w;      // |G_z|^2, work-layout order
     double* d_occ;        // [max_states] occupations of the last tdh_density call
+    cd* d_small[3];       // n x n scratch of tdh_orthonormalize ([0] overlap / Cholesky factor, [2] rotation), grown on demand
+    int small_n;
+    int* d_status;        // Cholesky status word
     int ctas_fwd, ctas_inv[tdh::NL_NCM], ctas_x[4];   // persistent grid sizes (SM count x resident CTAs)
 
     int chunk_cap;        // states the workspace can hold
@@ -325,6 +328,8 @@ extern "C" int tdh_destroy_grid(tdh_grid* g) {
     for (int a = 0; a < 3; ++a) { cudaFree(g->d_g2[a]); cudaFree(g->d_tw[a]); }
     cudaFree(g->d_g2y_w); cudaFree(g->d_g2z_w); cudaFree(g->d_twy_w); cudaFree(g->d_rowmap); cudaFree(g->d_colmap);
     cudaFree(g->d_p2x); cudaFree(g->d_p2y_w); cudaFree(g->d_p2z_w); cudaFree(g->d_occ);
+    for (int i = 0; i < 3; ++i) cudaFree(g->d_small[i]);
+    cudaFree(g->d_status);
     cudaFree(g->d_work); cudaFree(g->d_phi[0]); cudaFree(g->d_phi[1]);
     for (int i = 0; i < 2; ++i) {
         cudaFree(g->d_hin[i]); cudaFree(g->d_hout[i]);
@@ -1013,6 +1018,75 @@ extern "C" int tdh_overlap(tdh_grid* g, int na, const tdh_c128* a_dev, int nb, c
                                                                             (cd*)s_dev);
     CU(cudaGetLastError());
     g->launch_count += 1;
+    return TDH_OK;
+}
+
+static int launch_rotate(tdh_grid* g, int n_in, const cd* in, int n_out, const cd* m, cd* out, int upper) {
+    size_t npts = g->np;
+    void* args[] = {(void*)&in, (void*)&n_in, (void*)&m, (void*)&n_out, (void*)&npts, (void*)&upper, (void*)&out};
+    dim3 grid((unsigned)(g->np / tdh::RT_P), (n_out + tdh::RT_J - 1) / tdh::RT_J);
+    CU(cudaLaunchKernel(reinterpret_cast<const void*>(&tdh::rotate_kernel), grid, dim3(tdh::OV_THREADS), args, 0, g->stream));
+    g->launch_count += 1;
+    return TDH_OK;
+}
+
+// out_j = sum_i psi_i m[i][j]: rotation in the space of states on FP64 tensor cores (overlap_kernels.cuh)
+extern "C" int tdh_rotate(tdh_grid* g, int n_in, const tdh_c128* psi_dev, int n_out, const tdh_c128* m_dev,
+                          tdh_c128* out_dev) {
+    if (!g || !psi_dev || !m_dev || !out_dev) return fail(TDH_EINVAL, "tdh_rotate: null argument");
+    if (n_in < 1 || n_out < 1 || n_out > 65535 * tdh::RT_J) return fail(TDH_EINVAL, "tdh_rotate: bad n_in / n_out");
+    if (overlaps(psi_dev, out_dev, (size_t)std::min(n_in, n_out) * g->np * sizeof(cd)))
+        return fail(TDH_EINVAL, "tdh_rotate: psi and out overlap");
+    stats_reset(g);
+    return launch_rotate(g, n_in, (const cd*)psi_dev, n_out, (const cd*)m_dev, (cd*)out_dev, 0);
+}
+
+// Cholesky orthonormalisation: S = dV psi^H psi = L L^H, out = psi L^{-H}
+extern "C" int tdh_orthonormalize(tdh_grid* g, int nst, const tdh_c128* psi_dev, tdh_c128* out_dev) {
+    if (!g || !psi_dev || !out_dev) return fail(TDH_EINVAL, "tdh_orthonormalize: null argument");
+    if (nst < 1 || nst > 1024) return fail(nst < 1 ? TDH_EINVAL : TDH_EUNSUPPORTED, "tdh_orthonormalize: nst = %d outside [1, 1024]", nst);
+    if (overlaps(psi_dev, out_dev, (size_t)nst * g->np * sizeof(cd)))
+        return fail(TDH_EINVAL, "tdh_orthonormalize: psi and out overlap");
+    if (g->small_n < nst) {                       // first use (or a larger block): n x n scratch
+        CU(cudaStreamSynchronize(g->stream));
+        for (int i = 0; i < 3; ++i) { cudaFree(g->d_small[i]); g->d_small[i] = nullptr; }
+        g->small_n = 0;
+        for (int i = 0; i < 3; i += 2) CU(cudaMalloc(&g->d_small[i], sizeof(cd) * (size_t)nst * nst));   // [0] S / L, [2] L^{-H}
+        if (!g->d_status) CU(cudaMalloc(&g->d_status, 2 * sizeof(int)));       // [0] status, [1] grid-barrier counter
+        g->small_n = nst;
+    }
+    int rc = tdh_overlap(g, nst, psi_dev, nst, psi_dev, (tdh_c128*)g->d_small[0]);
+    if (rc) return rc;
+    {
+        // cooperative launch: as many CTAs as are resident at once, at most one warp per row
+        int dev = 0, nsm = 0, occ = 0;
+        CU(cudaGetDevice(&dev));
+        CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tdh::cholesky_kernel, 256, 0));
+        const int ctas = std::max(1, std::min(nsm * std::min(occ, 2), (nst + 7) / 8));
+        CU(cudaMemsetAsync(g->d_status + 1, 0, sizeof(unsigned), g->stream));
+        cd* sm = g->d_small[0];
+        int n = nst;
+        int* status = g->d_status;
+        unsigned* barrier = reinterpret_cast<unsigned*>(g->d_status + 1);
+        void* args[] = {(void*)&sm, (void*)&n, (void*)&status, (void*)&barrier};
+        CU(cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(&tdh::cholesky_kernel), dim3(ctas), dim3(256), args, 0,
+                                       g->stream));
+    }
+    {
+        const int warps = 4;
+        const size_t smem = (size_t)warps * nst * sizeof(cd);
+        CU(cudaFuncSetAttribute(tdh::inverse_lower_conjtrans_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        tdh::inverse_lower_conjtrans_kernel<<<(nst + warps - 1) / warps, 32 * warps, smem, g->stream>>>(g->d_small[0], nst,
+                                                                                                     g->d_small[2]);
+        CU(cudaGetLastError());
+    }
+    g->launch_count += 2;
+    if ((rc = launch_rotate(g, nst, (const cd*)psi_dev, nst, g->d_small[2], (cd*)out_dev, 1))) return rc;
+    int status = 0;
+    CU(cudaMemcpyAsync(&status, g->d_status, sizeof(int), cudaMemcpyDeviceToHost, g->stream));
+    CU(cudaStreamSynchronize(g->stream));
+    if (status != 0) return fail(TDH_EINVAL, "tdh_orthonormalize: the states are linearly dependent (pivot %d of the overlap matrix is not positive)", status - 1);
     return TDH_OK;
 }
 

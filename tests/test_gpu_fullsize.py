@@ -371,3 +371,37 @@ def test_propagation_keeps_orthonormality(torch_cuda, B, oracle):
         ref = oracle.propagate_workload(wl, psi, dt=0.01, nsteps=10)
         assert np.abs(s1 - oracle.overlap(cfg.n, cfg.dv, ref, ref)).max() < 1e-11
         assert np.abs(s1 - np.eye(nst)).max() < 1e-6            # orthonormal up to the Taylor truncation
+
+
+@pytest.mark.parametrize("n,n_in,n_out", [((16, 16, 16), 8, 8), ((32, 16, 48), 70, 5), ((48, 48, 16), 33, 130), ((16, 32, 16), 1, 1)])
+def test_rotate_matches_oracle(torch_cuda, B, oracle, n, n_in, n_out):
+    """tdh_rotate (FP64 tensor-core GEMM over the state index) against the literal loops, ragged edges included."""
+    torch = torch_cuda
+    rng = np.random.default_rng([W.BASE_SEED, 12, n_in, n_out])
+    psi = rng.standard_normal((n_in,) + n) + 1j * rng.standard_normal((n_in,) + n)
+    m = rng.standard_normal((n_in, n_out)) + 1j * rng.standard_normal((n_in, n_out))
+    ref = oracle.rotate(psi, m)
+    with B.Grid(n, tuple(0.5 * k for k in n), (0.0, 0.0, 0.0), -1.0, max(n_in, n_out)) as g:
+        got = g.rotate(torch.from_numpy(psi).cuda(), torch.from_numpy(m).cuda()).cpu().numpy()
+        assert per_state_rel(got, ref).max() < 1e-13
+
+
+@pytest.mark.parametrize("name,nst", [("tiny", 8), ("small", 64), ("medium", 37)])
+def test_orthonormalize_matches_oracle(torch_cuda, B, oracle, name, nst):
+    """tdh_orthonormalize = overlap + Cholesky + triangular inverse + rotation, against the oracle's composition; the
+    result has unit overlap (measured with tdh_overlap); linearly dependent input is refused."""
+    torch = torch_cuda
+    cfg = W.CONFIGS[name]
+    psi = W.states(cfg, 0, nst)
+    psi[1] = 0.6 * psi[0] + 0.8 * psi[1]                       # correlated inputs
+    ref = oracle.orthonormalize(cfg.n, cfg.dv, psi)
+    with B.Grid(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, nst) as g:
+        d = torch.from_numpy(psi).cuda()
+        out = g.orthonormalize(d)
+        assert g.last_launch_count() == 5
+        assert per_state_rel(out.cpu().numpy(), ref).max() < 1e-11
+        s = g.overlap(out).cpu().numpy()
+        assert np.abs(s - np.eye(nst)).max() < 1e-12
+        d[2] = d[0] - 2.0 * d[1]
+        with pytest.raises(B.TdhError):
+            g.orthonormalize(d)
