@@ -27,10 +27,12 @@ constexpr int OV_THREADS = 256;
 
 // grid: (tiles_i * tiles_j, ksplit).  part: [ksplit][na_pad][nb_pad] complex, na_pad = tiles_i*64, nb_pad = tiles_j*64.
 // Slice ks covers the chunks [ks*chunks_per_slice, (ks+1)*chunks_per_slice) of the N_p/16 chunks.
+// hermitian != 0 (a and b are the same block): tiles below the diagonal are skipped, the reduction mirrors them.
 __global__ void __launch_bounds__(OV_THREADS)
 overlap_kernel(const cd* __restrict__ a, int na, const cd* __restrict__ b, int nb, size_t npts, int tiles_j,
-               int chunks_per_slice, cd* __restrict__ part)
+               int chunks_per_slice, cd* __restrict__ part, int hermitian)
 {
+    if (hermitian && (int)(blockIdx.x % tiles_j) < (int)(blockIdx.x / tiles_j)) return;
     __shared__ double sre[2 * OV_T][OV_KCP];     // rows 0..63: A tile (states of a), rows 64..127: B tile (states of b)
     __shared__ double sim[2 * OV_T][OV_KCP];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -113,20 +115,23 @@ overlap_kernel(const cd* __restrict__ a, int na, const cd* __restrict__ b, int n
         }
 }
 
-// s[i][j] = dv * sum over slices (in order) of part[ks][i][j]
+// s[i][j] = dv * sum over slices (in order) of part[ks][i][j]; hermitian: elements in tiles below the diagonal are the
+// conjugates of their mirror images (which were computed)
 __global__ void overlap_reduce_kernel(const cd* __restrict__ part, int ksplit, int na, int nb, int na_pad, int nb_pad,
-                                      double dv, cd* __restrict__ s)
+                                      double dv, cd* __restrict__ s, int hermitian)
 {
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= na * nb) return;
-    const int i = idx / nb, j = idx % nb;
+    int i = idx / nb, j = idx % nb;
+    const bool mirror = hermitian && (j / OV_T) < (i / OV_T);
+    if (mirror) { const int t = i; i = j; j = t; }
     double re = 0.0, im = 0.0;
     for (int ks = 0; ks < ksplit; ++ks) {
         const cd v = part[((size_t)ks * na_pad + i) * nb_pad + j];
         re += v.x;
         im += v.y;
     }
-    s[idx] = make_double2(dv * re, dv * im);
+    s[idx] = make_double2(dv * re, mirror ? -dv * im : dv * im);
 }
 
 // ------------------------------------------------------------------------------------------------------------

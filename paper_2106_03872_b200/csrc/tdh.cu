@@ -1007,15 +1007,17 @@ extern "C" int tdh_overlap(tdh_grid* g, int na, const tdh_c128* a_dev, int nb, c
     cd* part = g->d_work;
     const cd* a = (const cd*)a_dev;
     const cd* b = (const cd*)b_dev;
+    int hermitian = (a_dev == b_dev && na == nb) ? 1 : 0;      // Gram matrix of one block: upper tiles only
     {
-        void* args[] = {(void*)&a, (void*)&na, (void*)&b, (void*)&nb, (void*)&npts, (void*)&tjv, (void*)&cps, (void*)&part};
+        void* args[] = {(void*)&a, (void*)&na, (void*)&b, (void*)&nb, (void*)&npts, (void*)&tjv, (void*)&cps, (void*)&part,
+                        (void*)&hermitian};
         CU(cudaLaunchKernel(reinterpret_cast<const void*>(&tdh::overlap_kernel), dim3(ti * tj, (unsigned)ksplit),
                             dim3(tdh::OV_THREADS), args, 0, g->stream));
         g->launch_count += 1;
     }
     const int na_pad = ti * tdh::OV_T, nb_pad = tj * tdh::OV_T, ks = (int)ksplit;
     tdh::overlap_reduce_kernel<<<(na * nb + 255) / 256, 256, 0, g->stream>>>(part, ks, na, nb, na_pad, nb_pad, g->dv,
-                                                                            (cd*)s_dev);
+                                                                            (cd*)s_dev, hermitian);
     CU(cudaGetLastError());
     g->launch_count += 1;
     return TDH_OK;
