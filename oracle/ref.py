@@ -26,7 +26,7 @@ def lib() -> C.CDLL:
     if _lib is None:
         _lib = C.CDLL(_build.build())
         for name in ("ref_dft3d", "ref_kinetic", "ref_local", "ref_nonlocal", "ref_apply_hamiltonian",
-                     "ref_propagate", "ref_taylor_pair", "ref_etrs_step", "ref_density", "ref_hartree", "ref_overlap", "ref_num_threads"):
+                     "ref_propagate", "ref_taylor_pair", "ref_etrs_step", "ref_density", "ref_hartree", "ref_overlap", "ref_sd_step", "ref_num_threads"):
             getattr(_lib, name).restype = C.c_int
     return _lib
 
@@ -208,6 +208,18 @@ def orthonormalize(n, dv: float, psi) -> np.ndarray:
     l = np.linalg.cholesky(0.5 * (s + s.conj().T))
     w = np.linalg.inv(l)                         # lower triangular L^{-1}
     return rotate(psi, w.conj().T)
+
+
+def sd_step(n, length, kpt, ecut, v, proj, psi, lam: float, backend: int = NAIVE_FFT):
+    """One Teter-preconditioned steepest-descent update of every state (fixed step lam).  Returns (new psi, eps before)."""
+    out = _c128(psi).copy()
+    nst = 1 if out.ndim == 3 else out.shape[0]
+    v = None if v is None else np.ascontiguousarray(v, dtype=np.float64)
+    eig = np.empty(nst, dtype=np.float64)
+    p = _Proj(proj)
+    _check(lib().ref_sd_step(_i3(n), _d3(length), _d3(kpt), C.c_double(ecut), _ptr(v), *p.args, C.c_int(nst), _ptr(out),
+                             C.c_double(lam), _ptr(eig), C.c_int(backend)), "sd_step")
+    return out, eig
 
 
 def apply_workload(wl, psi, backend: int = NAIVE_FFT) -> np.ndarray:

@@ -577,6 +577,80 @@ int ref_overlap(const int n[3], double dv, int na, const cplx *a, int nb, const 
     return REF_OK;
 }
 
+/* ------------------------------------------------------------------------------------------------
+ * exported (NEXT-3): one preconditioned steepest-descent update of every state, independently ("the
+ * preconditioned steepest (SD) descent algorithm ... can work simultaneously and independently on all eigenvectors.
+ * For preconditioning we use the method of Teter et al. that is applied in Fourier space").  The paper gives no
+ * formulas; the reading (R19) is the textbook one:
+ *   eps_s = <psi|H psi> / <psi|psi>,   T_s = <psi|T psi> / <psi|psi>       (sums over grid points, dV cancels)
+ *   r = H psi - eps_s psi
+ *   p_hat(G) = K(x) r_hat(G),  x = t(G) / T_s,  t = 1/2 |G+k|^2,
+ *       K(x) = (27 + 18x + 12x^2 + 8x^3) / (27 + 18x + 12x^2 + 8x^3 + 16x^4)         (Teter, Payne, Allan 1989)
+ *   psi <- psi - lambda p                                             (fixed step; no orthogonalisation here)
+ * eig[s] receives eps_s (the Rayleigh quotient BEFORE the update).  The cutoff mask acts in T as in H.
+ * ------------------------------------------------------------------------------------------------ */
+static double teter(double x)
+{
+    const double num = 27.0 + x * (18.0 + x * (12.0 + x * 8.0));
+    return num / (num + 16.0 * x * x * x * x);
+}
+
+int ref_sd_step(const int n[3], const double len[3], const double kpt[3], double ecut, const double *v, int natoms,
+                const int64_t *sph_off, const int32_t *sph_idx, const double *sph_disp, const int32_t *chan_off,
+                const double *beta, const double *dcoef, int nst, cplx *psi, double lambda, double *eig, int backend)
+{
+    if (check_geometry(n, len) || !kpt || !psi || nst < 0) return REF_EINVAL;
+    if (check_projectors(n, natoms, sph_off, sph_idx, chan_off, beta, dcoef)) return REF_EINVAL;
+    const size_t np_ = npoints(n);
+    const double two_pi = 6.283185307179586476925286766559;
+    int err = REF_OK;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int s = 0; s < nst; ++s) {
+        cplx *x = psi + (size_t)s * np_;
+        cplx *h = (cplx *)malloc(sizeof(cplx) * np_);
+        cplx *t = (cplx *)calloc(np_, sizeof(cplx));
+        int e = (h && t) ? REF_OK : REF_ENOMEM;
+        if (e == REF_OK)
+            e = hamiltonian_one(n, len, kpt, ecut, v, natoms, sph_off, sph_idx, sph_disp, chan_off, beta, dcoef, x, h, backend);
+        if (e == REF_OK) e = kinetic_one(n, len, kpt, ecut, x, t, backend);          /* t += T psi (t was zero) */
+        if (e == REF_OK) {
+            double nn = 0.0, eh = 0.0, et = 0.0;
+            for (size_t p = 0; p < np_; ++p) {
+                nn += creal(x[p]) * creal(x[p]) + cimag(x[p]) * cimag(x[p]);
+                eh += creal(conj(x[p]) * h[p]);
+                et += creal(conj(x[p]) * t[p]);
+            }
+            const double eps = eh / nn, ts = et / nn;
+            if (eig) eig[s] = eps;
+            for (size_t p = 0; p < np_; ++p) h[p] -= eps * x[p];                    /* residual */
+            e = dft3d_one(n, h, -1, backend);
+            if (e == REF_OK) {
+                for (int i = 0; i < n[0]; ++i) {
+                    const double gx = two_pi * freq_index(i, n[0]) / len[0] + kpt[0];
+                    for (int j = 0; j < n[1]; ++j) {
+                        const double gy = two_pi * freq_index(j, n[1]) / len[1] + kpt[1];
+                        for (int k = 0; k < n[2]; ++k) {
+                            const double gz = two_pi * freq_index(k, n[2]) / len[2] + kpt[2];
+                            const double tk = 0.5 * ((gx * gx + gy * gy) + gz * gz);
+                            h[((size_t)i * n[1] + j) * n[2] + k] *= teter(tk / ts);
+                        }
+                    }
+                }
+                e = dft3d_one(n, h, +1, backend);
+            }
+            if (e == REF_OK)
+                for (size_t p = 0; p < np_; ++p) x[p] -= lambda * h[p];
+        }
+        free(h);
+        free(t);
+        if (e != REF_OK) {
+#pragma omp critical
+            err = e;
+        }
+    }
+    return err;
+}
+
 /* number of OpenMP threads the block loops will use (reported by bench.py's cpu_baseline) */
 int ref_num_threads(void)
 {

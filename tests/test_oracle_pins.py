@@ -533,6 +533,60 @@ def test_p11_orthonormalize_equals_gram_schmidt(oracle):
     assert rel(oracle.rotate(psi, col)[0], np.tensordot(col[:, 0], psi, axes=(0, 0))) < 1e-14
 
 
+# --------------------------------------------------------------------------------------------- P12 (NEXT-3: SD step)
+def teter_k(x):
+    num = 27 + 18 * x + 12 * x ** 2 + 8 * x ** 3
+    return num / (num + 16 * x ** 4)
+
+
+def test_p12_sd_step_two_plane_waves_closed_form(oracle):
+    """Kinetic-only H, psi = a e^{iG1.r} + b e^{iG2.r}: eps = T = (|a|^2 t1 + |b|^2 t2)/(|a|^2 + |b|^2) and the update
+    multiplies coefficient c_m by 1 - lambda K(t_m / T)(t_m - eps).  Also K(0) = 1, K(x) -> 1/(2x)."""
+    assert teter_k(0.0) == 1.0 and abs(teter_k(1e6) * 2e6 - 1.0) < 1e-5
+    n, length = (6, 4, 8), (5.0, 3.0, 7.0)
+    kpt = [0.0, TWO_PI * 0.1 / length[1], 0.0]
+    ii = np.meshgrid(*[np.arange(m) for m in n], indexing="ij")
+    m1, m2 = (1, 0, -2), (-2, 1, 3)
+    w = [np.exp(2j * np.pi * sum(m[a] * ii[a] / n[a] for a in range(3))) for m in (m1, m2)]
+    t = [0.5 * sum((TWO_PI * m[a] / length[a] + kpt[a]) ** 2 for a in range(3)) for m in (m1, m2)]
+    a, b, lam = 0.8 - 0.3j, 0.5j, 0.21
+    psi = (a * w[0] + b * w[1])[None]
+    for backend in (0, 1):
+        out, eig = oracle.sd_step(n, length, kpt, -1.0, None, None, psi, lam, backend)
+        eps = (abs(a) ** 2 * t[0] + abs(b) ** 2 * t[1]) / (abs(a) ** 2 + abs(b) ** 2)
+        assert abs(eig[0] - eps) < 1e-12 * eps
+        expect = sum(c * (1 - lam * teter_k(tm / eps) * (tm - eps)) * wm for c, tm, wm in ((a, t[0], w[0]), (b, t[1], w[1])))
+        assert rel(out[0], expect) < 1e-12
+
+
+def test_p12_sd_step_fixed_points_and_descent(oracle):
+    """An eigenvector of the dense small-grid H is a fixed point (zero residual) with eig = its eigenvalue; for a random
+    state a small step lowers the Rayleigh quotient; the update equals the explicit formula built from H, T and numpy FFTs."""
+    cfg = small_cfg(117, n=(4, 5, 6), length=(4.4, 5.0, 5.5), natoms=2, lmax=1, rc=1.9)
+    wl = W.make(cfg)
+    h = dense_matrix(oracle, cfg, wl)
+    ev, vec = np.linalg.eigh(0.5 * (h + h.conj().T))
+    v0 = vec[:, 3].reshape((1,) + cfg.n)
+    out, eig = oracle.sd_step(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, wl.v, wl.proj, v0, 0.3, 0)
+    assert abs(eig[0] - ev[3]) < 1e-12 and rel(out, v0) < 1e-11
+    psi = W.states(cfg)
+    lam = 0.05
+    out, eig = oracle.sd_step(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, wl.v, wl.proj, psi, lam, 0)
+    hpsi = oracle.apply_workload(wl, psi, 0)
+    tpsi = oracle.kinetic(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, psi, 0)
+    g = [TWO_PI * np.fft.fftfreq(cfg.n[a], d=1.0 / cfg.n[a]) / cfg.length[a] + cfg.kpt[a] for a in range(3)]
+    tg = 0.5 * (g[0][:, None, None] ** 2 + g[1][None, :, None] ** 2 + g[2][None, None, :] ** 2)
+    for s in range(psi.shape[0]):
+        nn = np.vdot(psi[s], psi[s]).real
+        eps, ts = np.vdot(psi[s], hpsi[s]).real / nn, np.vdot(psi[s], tpsi[s]).real / nn
+        assert abs(eig[s] - eps) < 1e-12 * abs(eps)
+        r = hpsi[s] - eps * psi[s]
+        p = np.fft.ifftn(teter_k(tg / ts) * np.fft.fftn(r))
+        assert rel(out[s], psi[s] - lam * p) < 1e-12
+        hn = oracle.apply_workload(wl, out[s:s + 1], 0)[0]
+        assert np.vdot(out[s], hn).real / np.vdot(out[s], out[s]).real < eps
+
+
 # --------------------------------------------------------------------------------------------- P8
 def test_p8_independent_of_batching(oracle):
     cfg = W.CONFIGS["tiny"]
