@@ -424,6 +424,11 @@ def sweep_leg(torch, B, name, flush, reps=7):
                               "flops": "8 * nst^2 * N_p (complex128 GEMM, K = N_p)", "gram_seconds": tg,
                               "note": "tdh_overlap of two blocks: mma.sync.m8n8k4.f64, 64x64 tiles, split-K with ordered reduction; "
                                       "gram_seconds: one block with itself (tiles below the diagonal mirrored)"}
+            work.copy_(psi)
+            tsd = statistics.median(timed_each(torch, lambda: g.sd_step(work, 0.05, work=out, want_eig=False), 3, flush))
+            res["sd_step"] = {"seconds": tsd, "launches": g.last_launch_count(),
+                              "note": "tdh_sd_step on the whole block: H psi, T psi, Rayleigh quotients, residual, Teter "
+                                      "preconditioner pass with the fused update (about 2.7 H-application equivalents)"}
             tor = statistics.median(timed_each(torch, lambda: g.orthonormalize(psi, out=out), 3, flush))
             res["orthonormalize"] = {"seconds": tor, "launches": g.last_launch_count(),
                                      "effective_tflops": round(12.0 * cfg.nst * cfg.nst * cfg.npts / tor * 1e-12, 2),
@@ -536,6 +541,7 @@ def main():
             extra["density_hartree"] = wls["tddft"].pop("density_hartree")
             extra["overlap"] = wls["tddft"].pop("overlap")
             extra["orthonormalize"] = wls["tddft"].pop("orthonormalize")
+            extra["sd_step"] = wls["tddft"].pop("sd_step")
     else:
         g.close()
 

@@ -149,6 +149,15 @@ int tdh_rotate(tdh_grid* g, int n_in, const tdh_c128* psi_dev, int n_out, const 
  * Synchronises the stream; returns TDH_EINVAL when the states are linearly dependent (out is then undefined). */
 int tdh_orthonormalize(tdh_grid* g, int nst, const tdh_c128* psi_dev, tdh_c128* out_dev);
 
+/* One Teter-preconditioned steepest-descent update of every state, independently (reading R19):
+ *     eps_s = <psi|H psi>/<psi|psi>,  T_s = <psi|T psi>/<psi|psi>,  r = H psi - eps_s psi,
+ *     p_hat(G) = K(t(G)/T_s) r_hat(G),  K(x) = (27+18x+12x^2+8x^3)/(27+18x+12x^2+8x^3+16x^4),  psi <- psi - lambda p
+ * psi_dev: DEVICE block, updated in place; work_dev: DEVICE scratch block of the same size (holds the residuals
+ * afterwards), must not overlap psi_dev; eig_host: HOST [nst], receives eps_s (before the update), or NULL.
+ * One H application, one kinetic-only application and one preconditioner pass per state; no orthogonalisation
+ * (tdh_orthonormalize).  Asynchronous unless eig_host is given. */
+int tdh_sd_step(tdh_grid* g, int nst, tdh_c128* psi_dev, tdh_c128* work_dev, double lambda, double* eig_host);
+
 /* The same two operations with HOST buffers (pageable or pinned): the library stages state chunks through its own
  * pinned buffers, overlapping host<->device copies with the kernels, and returns when hpsi_host / psi_host is complete.
  * nst is not limited by max_states here (chunks are).  These are the end-to-end entry points timed by bench.py. */

@@ -21,6 +21,7 @@ struct XLaunch {
     const void* fwd;    // xpencil_kernel<NX,S,1>
     const void* inv;    // xpencil_kernel<NX,S,2>
     const void* poisson;  // xpencil_kernel<NX,S,3>
+    const void* teter;    // xpencil_kernel<NX,S,4>
     int threads;
     size_t smem;        // dynamic shared memory per CTA (ring of tiles)
 };

@@ -94,7 +94,8 @@ struct tdh_grid {
     cd* d_small[3];       // n x n scratch of tdh_orthonormalize ([0] overlap / Cholesky factor, [2] rotation), grown on demand
     int small_n;
     int* d_status;        // Cholesky status word
-    int ctas_fwd, ctas_inv[tdh::NL_NCM], ctas_x[4];   // persistent grid sizes (SM count x resident CTAs)
+    double* d_sd;         // tdh_sd_step: [max_states] eps, [max_states] T, [max_states * 3 * SD_SLICES] partial sums
+    int ctas_fwd, ctas_inv[tdh::NL_NCM], ctas_x[5];   // persistent grid sizes (SM count x resident CTAs)
 
     int chunk_cap;        // states the workspace can hold
     int chunk;            // states pushed through the chain together
@@ -219,11 +220,11 @@ extern "C" int tdh_create_grid(const int n[3], const double len[3], const double
         int dev = 0, nsm = 0;
         CU(cudaGetDevice(&dev));
         CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
-        constexpr int NK = 5 + tdh::NL_NCM;
-        const void* fs[NK] = {g->tl.fwd, g->xl.fused, g->xl.fwd, g->xl.inv, g->xl.poisson};
-        size_t sm[NK] = {g->tl.smem_fwd, g->xl.smem, g->xl.smem, g->xl.smem, g->xl.smem};
-        int th[NK] = {g->tl.threads, g->xl.threads, g->xl.threads, g->xl.threads, g->xl.threads};
-        for (int i = 0; i < tdh::NL_NCM; ++i) { fs[5 + i] = g->tl.inv[i]; sm[5 + i] = g->tl.smem_inv; th[5 + i] = g->tl.threads; }
+        constexpr int NK = 6 + tdh::NL_NCM;
+        const void* fs[NK] = {g->tl.fwd, g->xl.fused, g->xl.fwd, g->xl.inv, g->xl.poisson, g->xl.teter};
+        size_t sm[NK] = {g->tl.smem_fwd, g->xl.smem, g->xl.smem, g->xl.smem, g->xl.smem, g->xl.smem};
+        int th[NK] = {g->tl.threads, g->xl.threads, g->xl.threads, g->xl.threads, g->xl.threads, g->xl.threads};
+        for (int i = 0; i < tdh::NL_NCM; ++i) { fs[6 + i] = g->tl.inv[i]; sm[6 + i] = g->tl.smem_inv; th[6 + i] = g->tl.threads; }
         int ctas[NK];
         for (int i = 0; i < NK; ++i) {
             CU(cudaFuncSetAttribute(fs[i], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm[i]));
@@ -235,8 +236,8 @@ extern "C" int tdh_create_grid(const int n[3], const double len[3], const double
             ctas[i] = nsm * occ;
         }
         g->ctas_fwd = ctas[0];
-        g->ctas_x[0] = ctas[1]; g->ctas_x[1] = ctas[2]; g->ctas_x[2] = ctas[3]; g->ctas_x[3] = ctas[4];
-        for (int i = 0; i < tdh::NL_NCM; ++i) g->ctas_inv[i] = ctas[5 + i];
+        g->ctas_x[0] = ctas[1]; g->ctas_x[1] = ctas[2]; g->ctas_x[2] = ctas[3]; g->ctas_x[3] = ctas[4]; g->ctas_x[4] = ctas[5];
+        for (int i = 0; i < tdh::NL_NCM; ++i) g->ctas_inv[i] = ctas[6 + i];
         // tables: built on the host exactly as the oracle builds its G vectors (two_pi * m / L + k, then squared)
         const double two_pi = 6.283185307179586476925286766559;
         for (int a = 0; a < 3; ++a) {
@@ -329,7 +330,7 @@ extern "C" int tdh_destroy_grid(tdh_grid* g) {
     cudaFree(g->d_g2y_w); cudaFree(g->d_g2z_w); cudaFree(g->d_twy_w); cudaFree(g->d_rowmap); cudaFree(g->d_colmap);
     cudaFree(g->d_p2x); cudaFree(g->d_p2y_w); cudaFree(g->d_p2z_w); cudaFree(g->d_occ);
     for (int i = 0; i < 3; ++i) cudaFree(g->d_small[i]);
-    cudaFree(g->d_status);
+    cudaFree(g->d_status); cudaFree(g->d_sd);
     cudaFree(g->d_work); cudaFree(g->d_phi[0]); cudaFree(g->d_phi[1]);
     for (int i = 0; i < 2; ++i) {
         cudaFree(g->d_hin[i]); cudaFree(g->d_hout[i]);
@@ -611,13 +612,14 @@ static int launch_plane_fwd(tdh_grid* g, int nst, const cd* in, cd* out) {
     return TDH_OK;
 }
 
-static int launch_xpencil(tdh_grid* g, int nst, const cd* in, cd* out, int mode) {
+static int launch_xpencil(tdh_grid* g, int nst, const cd* in, cd* out, int mode, const double* tstate = nullptr) {
     CUtensorMap map;
     if (!tdh::encode_line_map(&map, in, (size_t)nst * g->n[0], g->n[0], g->n[1], g->n[2]))
         return fail(TDH_ECUDA, "cuTensorMapEncodeTiled failed (line map)");
     tdh::Kinetic kin;
     kin.g2x = g->d_g2[0]; kin.g2y_w = g->d_g2y_w; kin.g2z_w = g->d_g2z_w; kin.twy_w = g->d_twy_w;
     if (mode == 3) { kin.g2x = g->d_p2x; kin.g2y_w = g->d_p2y_w; kin.g2z_w = g->d_p2z_w; }     // Poisson: pure |G|^2
+    kin.tstate = tstate;
     kin.ecut = g->ecut;
     kin.scale = 1.0 / (double)g->np;
     kin.nz = g->n[2];
@@ -625,7 +627,7 @@ static int launch_xpencil(tdh_grid* g, int nst, const cd* in, cd* out, int mode)
     int ntiles = nst * (g->n[1] / 2) * (g->n[2] / 16);
     const cd* twx = g->d_tw[0];
     void* args[] = {(void*)&map, (void*)&out, (void*)&ntiles, (void*)&twx, (void*)&kin};
-    const void* f = mode == 0 ? g->xl.fused : (mode == 1 ? g->xl.fwd : (mode == 2 ? g->xl.inv : g->xl.poisson));
+    const void* f = mode == 0 ? g->xl.fused : (mode == 1 ? g->xl.fwd : (mode == 2 ? g->xl.inv : (mode == 3 ? g->xl.poisson : g->xl.teter)));
     const unsigned grid = (unsigned)std::min(ntiles, g->ctas_x[mode]);
     LAUNCH(K_XPENCIL, f, dim3(grid), dim3(g->xl.threads), g->xl.smem, args);
     return TDH_OK;
@@ -731,8 +733,18 @@ static int launch_nl_scatter(tdh_grid* g, int nst, cd* out, cd alpha) {
 }
 
 // out = alpha * H in + yv   for one chunk (nst <= chunk_cap); in/out/yv point at the chunk's first state
-static int apply_chunk(tdh_grid* g, int nst, const cd* in, cd* out, cd alpha, const cd* yv) {
+static int apply_chunk(tdh_grid* g, int nst, const cd* in, cd* out, cd alpha, const cd* yv, bool kinetic_only = false) {
     int rc;
+    if (kinetic_only) {                                   // out = alpha * T in + yv
+        if ((rc = launch_plane_fwd(g, nst, in, g->d_work))) return rc;
+        if ((rc = launch_xpencil(g, nst, g->d_work, g->d_work, 0))) return rc;
+        tdh::Epilogue ek;
+        memset(&ek, 0, sizeof(ek));
+        ek.yv = yv;
+        ek.alpha = alpha;
+        ek.nx = g->n[0];
+        return launch_plane_inv(g, nst, g->d_work, nullptr, out, ek);
+    }
     if (g->natoms > 0 && (rc = launch_nl_project(g, nst, in))) return rc;
     if ((rc = launch_plane_fwd(g, nst, in, g->d_work))) return rc;
     if ((rc = launch_xpencil(g, nst, g->d_work, g->d_work, 0))) return rc;
@@ -979,6 +991,116 @@ extern "C" int tdh_hartree(tdh_grid* g, const double* n_dev, double* vh_dev) {
     complex_to_real_kernel<<<296, 256, 0, g->stream>>>(a, vh_dev, g->np);
     CU(cudaGetLastError());
     g->launch_count += 1;
+    return prof_collect(g);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// NEXT-3: Teter-preconditioned steepest-descent update (reading R19)
+// ------------------------------------------------------------------------------------------------------------
+constexpr int SD_SLICES = 32;
+
+// partial[(s*SD_SLICES + slice)*3 + {0,1,2}] = sums over the slice's points of |psi|^2, Re conj(psi) h, Re conj(psi) t.
+// grid (SD_SLICES, nst), 256 threads; fixed summation order (thread-strided, warp shuffles, warps in order).
+__global__ void sd_dots_kernel(const cd* __restrict__ psi, const cd* __restrict__ h, const cd* __restrict__ t, size_t npts,
+                               double* __restrict__ partial) {
+    __shared__ double red[8][3];
+    const int s = blockIdx.y, slice = blockIdx.x;
+    const size_t per = (npts + SD_SLICES - 1) / SD_SLICES, p0 = (size_t)slice * per, p1 = p0 + per < npts ? p0 + per : npts;
+    const cd* a = psi + (size_t)s * npts;
+    const cd* b = h + (size_t)s * npts;
+    const cd* c = t + (size_t)s * npts;
+    double nn = 0.0, eh = 0.0, et = 0.0;
+    for (size_t p = p0 + threadIdx.x; p < p1; p += blockDim.x) {
+        const cd x = __ldcs(a + p), y = __ldcs(b + p), z = __ldcs(c + p);
+        nn += x.x * x.x + x.y * x.y;
+        eh += x.x * y.x + x.y * y.y;
+        et += x.x * z.x + x.y * z.y;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        nn += __shfl_xor_sync(0xffffffffu, nn, o);
+        eh += __shfl_xor_sync(0xffffffffu, eh, o);
+        et += __shfl_xor_sync(0xffffffffu, et, o);
+    }
+    if ((threadIdx.x & 31) == 0) { red[threadIdx.x >> 5][0] = nn; red[threadIdx.x >> 5][1] = eh; red[threadIdx.x >> 5][2] = et; }
+    __syncthreads();
+    if (threadIdx.x < 3) {
+        double v = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) v += red[w][threadIdx.x];
+        partial[((size_t)s * SD_SLICES + slice) * 3 + threadIdx.x] = v;
+    }
+}
+
+// eps[s] = <psi|H psi>/<psi|psi>, ts[s] = <psi|T psi>/<psi|psi> from the slice sums, in slice order
+__global__ void sd_finalize_kernel(const double* __restrict__ partial, int nst, double* __restrict__ eps, double* __restrict__ ts) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= nst) return;
+    double nn = 0.0, eh = 0.0, et = 0.0;
+    for (int k = 0; k < SD_SLICES; ++k) {
+        nn += partial[((size_t)s * SD_SLICES + k) * 3 + 0];
+        eh += partial[((size_t)s * SD_SLICES + k) * 3 + 1];
+        et += partial[((size_t)s * SD_SLICES + k) * 3 + 2];
+    }
+    eps[s] = eh / nn;
+    ts[s] = et / nn;
+}
+
+// h <- h - eps[s] psi   (the residual)
+__global__ void sd_residual_kernel(const cd* __restrict__ psi, cd* __restrict__ h, size_t npts, const double* __restrict__ eps) {
+    const int s = blockIdx.y;
+    const double e = eps[s];
+    const cd* a = psi + (size_t)s * npts;
+    cd* b = h + (size_t)s * npts;
+    for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < npts; p += (size_t)gridDim.x * blockDim.x) {
+        const cd x = __ldcs(a + p);
+        cd y = __ldcs(b + p);
+        y.x -= e * x.x;
+        y.y -= e * x.y;
+        __stcs(b + p, y);
+    }
+}
+
+extern "C" int tdh_sd_step(tdh_grid* g, int nst, tdh_c128* psi_dev, tdh_c128* work_dev, double lambda, double* eig_host) {
+    if (!g || !psi_dev || !work_dev) return fail(TDH_EINVAL, "tdh_sd_step: null argument");
+    if (nst < 1 || nst > g->max_states) return fail(TDH_EINVAL, "tdh_sd_step: nst = %d outside [1, %d]", nst, g->max_states);
+    if (!std::isfinite(lambda)) return fail(TDH_EINVAL, "tdh_sd_step: bad lambda");
+    if (overlaps(psi_dev, work_dev, (size_t)nst * g->np * sizeof(cd)))
+        return fail(TDH_EINVAL, "tdh_sd_step: psi and work overlap");
+    if (!g->d_sd) CU(cudaMalloc(&g->d_sd, sizeof(double) * (size_t)g->max_states * (2 + 3 * SD_SLICES)));   // first use
+    stats_reset(g);
+    double* eps = g->d_sd;
+    double* ts = g->d_sd + g->max_states;
+    double* partial = g->d_sd + 2 * (size_t)g->max_states;
+    const cd one = make_double2(1.0, 0.0);
+    for (int s0 = 0; s0 < nst; s0 += g->chunk) {
+        const int c = std::min(g->chunk, nst - s0);
+        cd* x = (cd*)psi_dev + (size_t)s0 * g->np;
+        cd* h = (cd*)work_dev + (size_t)s0 * g->np;
+        cd* t = g->d_phi[0];
+        int rc;
+        if ((rc = apply_chunk(g, c, x, h, one, nullptr))) return rc;                 // h = H psi
+        if ((rc = apply_chunk(g, c, x, t, one, nullptr, true))) return rc;           // t = T psi
+        sd_dots_kernel<<<dim3(SD_SLICES, c), 256, 0, g->stream>>>(x, h, t, g->np, partial);
+        CU(cudaGetLastError());
+        sd_finalize_kernel<<<(c + 127) / 128, 128, 0, g->stream>>>(partial, c, eps + s0, ts + s0);
+        CU(cudaGetLastError());
+        sd_residual_kernel<<<dim3(64, c), 256, 0, g->stream>>>(x, h, g->np, eps + s0);
+        CU(cudaGetLastError());
+        g->launch_count += 3;
+        // psi <- psi - lambda K r : forward (z,y), x pass with the Teter factor, inverse (y,z) with the axpy epilogue
+        if ((rc = launch_plane_fwd(g, c, h, g->d_work))) return rc;
+        if ((rc = launch_xpencil(g, c, g->d_work, g->d_work, 4, ts + s0))) return rc;
+        tdh::Epilogue ep;
+        memset(&ep, 0, sizeof(ep));
+        ep.yv = x;
+        ep.alpha = make_double2(-lambda, 0.0);
+        ep.nx = g->n[0];
+        if ((rc = launch_plane_inv(g, c, g->d_work, nullptr, x, ep))) return rc;
+    }
+    if (eig_host) {
+        CU(cudaMemcpyAsync(eig_host, eps, sizeof(double) * nst, cudaMemcpyDeviceToHost, g->stream));
+        CU(cudaStreamSynchronize(g->stream));
+    }
     return prof_collect(g);
 }
 

@@ -10,6 +10,7 @@ template <int NX, int S> static XLaunch make_x_launch() {
     x.fwd = reinterpret_cast<const void*>(&xpencil_kernel<NX, S, 1>);
     x.inv = reinterpret_cast<const void*>(&xpencil_kernel<NX, S, 2>);
     x.poisson = reinterpret_cast<const void*>(&xpencil_kernel<NX, S, 3>);
+    x.teter = reinterpret_cast<const void*>(&xpencil_kernel<NX, S, 4>);
     x.threads = XCfg<NX>::T;
     x.smem = XCfg<NX>::SMEM;
     return x;

@@ -31,6 +31,7 @@
 // MODE 0: forward x, kinetic, inverse x.   MODE 1: forward x only (spectrum out, work layout).
 // MODE 3: as MODE 0 with the Poisson factor 4 pi / |G|^2 (G = 0 dropped) in place of the kinetic one (tdh_hartree;
 //         the tables in `Kinetic` are then those of the pure reciprocal vectors, without the Bloch vector).
+// MODE 4: as MODE 0 with the Teter preconditioner K(t / T_s), t = 1/2|G+k|^2, T_s = kin.tstate[state] (tdh_sd_step).
 // MODE 2: inverse x only, times `scale` (spectrum in, work layout).
 #pragma once
 #include "fft_codelets.cuh"
@@ -45,6 +46,7 @@ struct Kinetic {
     const double* g2y_w;   // [NY] (G_y + k_y)^2 of the ky that plane row Y stands for (work-layout order)
     const double* g2z_w;   // [NZ] (G_z + k_z)^2 of the kz that column z' stands for
     const cd* twy_w;       // [NY/2] e^{+2 pi i k / NY} of row pair rho (S = 2 only)
+    const double* tstate;  // MODE 4: kinetic energy T_s per state of this launch
     double ecut;           // <= 0: no mask
     double scale;          // 1 / N_p (MODE 0 and 2); unused in MODE 1
     int nz;
@@ -83,9 +85,18 @@ __device__ __forceinline__ double poisson_factor(double gx2, double gy2, double 
     const double g2 = __dadd_rn(__dadd_rn(gx2, gy2), gz2);
     return g2 > 0.0 ? __ddiv_rn(12.566370614359172953850573533118, g2) * scale : 0.0;
 }
+// the Teter-Payne-Allan preconditioner K(x), x = t / T_s (reading R19), times 1/N_p
+__device__ __forceinline__ double teter_factor(double gx2, double gy2, double gz2, double ts, double scale) {
+    const double tk = __dmul_rn(0.5, __dadd_rn(__dadd_rn(gx2, gy2), gz2));
+    const double x = tk / ts;
+    const double num = 27.0 + x * (18.0 + x * (12.0 + x * 8.0));
+    const double x2 = x * x;
+    return num / (num + 16.0 * x2 * x2) * scale;
+}
 template <int MODE>
-__device__ __forceinline__ double diag_factor(double gx2, double gy2, double gz2, double ecut, double scale) {
-    return MODE == 3 ? poisson_factor(gx2, gy2, gz2, scale) : kin_factor(gx2, gy2, gz2, ecut, scale);
+__device__ __forceinline__ double diag_factor(double gx2, double gy2, double gz2, double ecut, double scale, double ts) {
+    return MODE == 3 ? poisson_factor(gx2, gy2, gz2, scale)
+                     : (MODE == 4 ? teter_factor(gx2, gy2, gz2, ts, scale) : kin_factor(gx2, gy2, gz2, ecut, scale));
 }
 
 // grid: persistent CTAs; ntiles = nst * (NY/2) * (NZ/16).  in (through `map`) and out may be the same buffer: a tile
@@ -118,7 +129,7 @@ xpencil_kernel(const __grid_constant__ CUtensorMap map, cd* __restrict__ out, in
     }
     for (int i = tid; i < NX; i += C::T) {
         stw[i] = __ldg(tw_x + i);
-        sg2x[i] = (MODE == 0 || MODE == 3) ? __ldg(kin.g2x + i) : 0.0;
+        sg2x[i] = (MODE == 0 || MODE >= 3) ? __ldg(kin.g2x + i) : 0.0;
     }
     __syncthreads();
     auto issue = [&](int t, int b) {                    // thread 0 only
@@ -145,12 +156,13 @@ xpencil_kernel(const __grid_constant__ CUtensorMap map, cd* __restrict__ out, in
         // per-line constants of this tile (in flight while the tile arrives)
         double gy2a = 0.0, gy2b = 0.0, gz2 = 0.0;
         cd w = make_double2(1.0, 0.0);
-        if (MODE == 0 || MODE == 3) {
+        if (MODE == 0 || MODE >= 3) {
             gz2 = __ldg(kin.g2z_w + zp);
             gy2a = __ldg(kin.g2y_w + (S == 2 ? 2 * rho2 : Y));
             if (S == 2) gy2b = __ldg(kin.g2y_w + 2 * rho2 + 1);
         }
         if (S == 2) w = __ldg(kin.twy_w + rho2);                 // e^{+2 pi i k / NY} = conj(w of the header comment)
+        const double ts = MODE == 4 ? __ldg(kin.tstate + st) : 1.0;
         // a ring of one buffer cannot prefetch into shared memory: start the CTA's next tile towards L2 instead
         // (measured: +3 % for the 48 KB tiles of NX = 96, -4 % for the 32 KB tiles of NX = 64, so only the former)
         if (NB == 1 && NX >= 96 && tid == 0 && t + (int)gridDim.x < ntiles) {
@@ -223,7 +235,7 @@ xpencil_kernel(const __grid_constant__ CUtensorMap map, cd* __restrict__ out, in
 #pragma unroll
                     for (int j2 = 0; j2 < R2; ++j2) xr[j2] = sm[(k1 * R2 + j2) * L + l];
                     Dft<R2, -1>::run(xr);
-                    if (MODE == 0 || MODE == 3) {
+                    if (MODE == 0 || MODE >= 3) {
                         // Without a cutoff mask no decision hangs on the bits of t, and the kinetic factor is affine in
                         // (G_x+k_x)^2: f = fx * gx2 + f0 with per-line constants (one FMA per value instead of the
                         // masked evaluation in the oracle's order); for the split y transform f_0 + f_1 is affine in
@@ -236,7 +248,7 @@ xpencil_kernel(const __grid_constant__ CUtensorMap map, cd* __restrict__ out, in
                         for (int k2 = 0; k2 < R2; ++k2) {
                             const double gx2 = sg2x[k1 + R1 * k2];
                             if (S == 1) {
-                                const double f = affine ? fma(hs, gx2, f0a) : diag_factor<MODE>(gx2, gy2a, gz2, kin.ecut, kin.scale);
+                                const double f = affine ? fma(hs, gx2, f0a) : diag_factor<MODE>(gx2, gy2a, gz2, kin.ecut, kin.scale, ts);
                                 xr[k2] = cscale(xr[k2], f);
                             } else {
                                 // the radix-2 step of the y transform folded into the factor (header comment)
@@ -245,8 +257,8 @@ xpencil_kernel(const __grid_constant__ CUtensorMap map, cd* __restrict__ out, in
                                     fs = fma(kin.scale, gx2, f0a + f0b);
                                     fd = f0a - f0b;
                                 } else {
-                                    const double fa = diag_factor<MODE>(gx2, gy2a, gz2, kin.ecut, kin.scale);
-                                    const double fb = diag_factor<MODE>(gx2, gy2b, gz2, kin.ecut, kin.scale);
+                                    const double fa = diag_factor<MODE>(gx2, gy2a, gz2, kin.ecut, kin.scale, ts);
+                                    const double fb = diag_factor<MODE>(gx2, gy2b, gz2, kin.ecut, kin.scale, ts);
                                     fs = fa + fb;
                                     fd = fa - fb;
                                 }

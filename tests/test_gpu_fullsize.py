@@ -405,3 +405,46 @@ def test_orthonormalize_matches_oracle(torch_cuda, B, oracle, name, nst):
         d[2] = d[0] - 2.0 * d[1]
         with pytest.raises(B.TdhError):
             g.orthonormalize(d)
+
+
+# ------------------------------------------------------------------------------------------------ NEXT-3: SD step
+@pytest.mark.parametrize("name,nst,backend", [("tiny", 8, 0), ("small", 21, 1), ("medium", 9, 1)])
+def test_sd_step_matches_oracle(torch_cuda, B, oracle, name, nst, backend):
+    """tdh_sd_step (Teter-preconditioned steepest descent, reading R19) against the oracle, chunked and not."""
+    torch = torch_cuda
+    cfg = W.CONFIGS[name]
+    wl = W.make(cfg)
+    psi = W.states(cfg, 0, nst)
+    lam = 0.1
+    ref, eig_ref = oracle.sd_step(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, wl.v, wl.proj, psi, lam, backend)
+    with B.grid_for(wl, max_states=nst) as g:
+        for chunk in (None, 4):
+            if chunk:
+                g.set_chunk_states(chunk)
+            d = torch.from_numpy(psi).cuda()
+            eig = g.sd_step(d, lam)
+            assert np.abs(eig - eig_ref).max() < 1e-11 * np.abs(eig_ref).max()
+            assert per_state_rel(d.cpu().numpy(), ref).max() < TOL
+
+
+def test_sd_sweeps_with_orthonormalisation_lower_the_energy(torch_cuda, B, oracle):
+    """A few ground-state iterations composed from the C-ABI calls (SD update + Cholesky orthonormalisation): the sum of the
+    Rayleigh quotients decreases monotonically and the block stays orthonormal; the same sequence of the oracle agrees."""
+    torch = torch_cuda
+    cfg = W.CONFIGS["tiny"]
+    wl = W.make(cfg)
+    psi = oracle.orthonormalize(cfg.n, cfg.dv, W.states(cfg))
+    ref = psi.copy()
+    with B.grid_for(wl) as g:
+        d = torch.from_numpy(psi).cuda()
+        sums = []
+        for it in range(4):
+            eig = g.sd_step(d, 0.3)
+            d = g.orthonormalize(d)
+            ref, eig_ref = oracle.sd_step(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, wl.v, wl.proj, ref, 0.3, 0)
+            ref = oracle.orthonormalize(cfg.n, cfg.dv, ref)
+            assert np.abs(eig - eig_ref).max() < 1e-10
+            sums.append(eig.sum())
+        assert all(b < a for a, b in zip(sums, sums[1:]))
+        assert per_state_rel(d.cpu().numpy(), ref).max() < 1e-9          # four compounded iterations
+        assert np.abs(g.overlap(d).cpu().numpy() - np.eye(cfg.nst)).max() < 1e-12
