@@ -222,6 +222,15 @@ def sd_step(n, length, kpt, ecut, v, proj, psi, lam: float, backend: int = NAIVE
     return out, eig
 
 
+def subspace_diag(n, dv: float, psi, hpsi):
+    """Subspace diagonalisation of an orthonormal block: M = dV psi^H (H psi), M = V diag(w) V^H (library
+    Hermitian eigensolver as one step, w ascending), psi' = psi V.  Returns (w, psi', V); V's columns are unique only up
+    to a phase (and within degenerate eigenspaces)."""
+    m = overlap(n, dv, psi, hpsi)
+    w, v = np.linalg.eigh(0.5 * (m + m.conj().T))
+    return w, rotate(psi, v), v
+
+
 def apply_workload(wl, psi, backend: int = NAIVE_FFT) -> np.ndarray:
     """Convenience: H psi with a workloads.Workload."""
     c = wl.cfg

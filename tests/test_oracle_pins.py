@@ -587,6 +587,34 @@ def test_p12_sd_step_fixed_points_and_descent(oracle):
         assert np.vdot(out[s], hn).real / np.vdot(out[s], out[s]).real < eps
 
 
+# --------------------------------------------------------------------------------------------- P13 (NEXT-3: subspace diagonalisation)
+def test_p13_subspace_diag_recovers_mixed_eigenvectors_and_cauchy_bounds(oracle):
+    """A block spanned by exact eigenvectors of the dense small-grid H, mixed by a random unitary: the Ritz values are those
+    eigenvalues and the Ritz vectors the eigenvectors up to a phase.  For a random orthonormal block: the Ritz vectors are
+    orthonormal, psi'^H H psi' is diagonal with the Ritz values, the trace is kept, and Cauchy interlacing holds."""
+    cfg = small_cfg(118, n=(4, 5, 6), length=(4.4, 5.0, 5.5), natoms=2, lmax=1, rc=1.9)
+    wl = W.make(cfg)
+    h = dense_matrix(oracle, cfg, wl)
+    ev, vec = np.linalg.eigh(0.5 * (h + h.conj().T))
+    pick = [0, 2, 5, 9]
+    basis = vec[:, pick].T.reshape((4,) + cfg.n) / np.sqrt(cfg.dv)             # dV-orthonormal eigenvectors
+    rng = np.random.default_rng(118)
+    u, _ = np.linalg.qr(rand_c(rng, (4, 4)))
+    psi = oracle.rotate(basis, u)
+    w, out, _ = oracle.subspace_diag(cfg.n, cfg.dv, psi, oracle.apply_workload(wl, psi, 0))
+    assert np.abs(w - ev[pick]).max() < 1e-12
+    s = oracle.overlap(cfg.n, cfg.dv, basis, out)
+    assert np.abs(np.abs(s) - np.eye(4)).max() < 1e-10                          # same vectors up to a phase
+    psi = oracle.orthonormalize(cfg.n, cfg.dv, W.states(cfg))
+    hp = oracle.apply_workload(wl, psi, 0)
+    w, out, v = oracle.subspace_diag(cfg.n, cfg.dv, psi, hp)
+    assert np.abs(oracle.overlap(cfg.n, cfg.dv, out, out) - np.eye(3)).max() < 1e-12
+    m2 = oracle.overlap(cfg.n, cfg.dv, out, oracle.apply_workload(wl, out, 0))
+    assert np.abs(m2 - np.diag(w)).max() < 1e-12
+    assert abs(w.sum() - np.trace(oracle.overlap(cfg.n, cfg.dv, psi, hp)).real) < 1e-12
+    assert all(w[i] >= ev[i] - 1e-12 for i in range(3)) and all(w[2 - i] <= ev[-1 - i] + 1e-12 for i in range(3))
+
+
 # --------------------------------------------------------------------------------------------- P8
 def test_p8_independent_of_batching(oracle):
     cfg = W.CONFIGS["tiny"]
