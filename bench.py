@@ -429,6 +429,12 @@ def sweep_leg(torch, B, name, flush, reps=7):
             res["sd_step"] = {"seconds": tsd, "launches": g.last_launch_count(),
                               "note": "tdh_sd_step on the whole block: H psi, T psi, Rayleigh quotients, residual, Teter "
                                       "preconditioner pass with the fused update (about 2.7 H-application equivalents)"}
+            hps = g.apply_hamiltonian(work)
+            tsub = statistics.median(timed_each(torch, lambda: g.subspace_diag(work, hps, out=out), 3, flush))
+            res["subspace_diag"] = {"seconds": tsub, "launches": g.last_launch_count(),
+                                    "note": "tdh_subspace_diag: overlap psi^H (H psi), cooperative parallel Jacobi eigensolver of "
+                                            "the nst x nst matrix, rotation psi V (host timer incl. the eigenvalue copy)"}
+            del hps
             tor = statistics.median(timed_each(torch, lambda: g.orthonormalize(psi, out=out), 3, flush))
             res["orthonormalize"] = {"seconds": tor, "launches": g.last_launch_count(),
                                      "effective_tflops": round(12.0 * cfg.nst * cfg.nst * cfg.npts / tor * 1e-12, 2),
@@ -542,6 +548,7 @@ def main():
             extra["overlap"] = wls["tddft"].pop("overlap")
             extra["orthonormalize"] = wls["tddft"].pop("orthonormalize")
             extra["sd_step"] = wls["tddft"].pop("sd_step")
+            extra["subspace_diag"] = wls["tddft"].pop("subspace_diag")
     else:
         g.close()
 

@@ -149,6 +149,15 @@ int tdh_rotate(tdh_grid* g, int n_in, const tdh_c128* psi_dev, int n_out, const 
  * Synchronises the stream; returns TDH_EINVAL when the states are linearly dependent (out is then undefined). */
 int tdh_orthonormalize(tdh_grid* g, int nst, const tdh_c128* psi_dev, tdh_c128* out_dev);
 
+/* Subspace diagonalisation of an ORTHONORMAL block: M = dV psi^H (H psi) = V diag(w) V^H, out = psi V,
+ * so that dV out^H H out = diag(w), w ascending.  hpsi_dev holds H psi (tdh_apply_hamiltonian).  tdh_overlap, a
+ * cooperative parallel Jacobi eigensolver of the nst x nst Hermitian matrix, tdh_rotate.  1 <= nst <= 1024.
+ * psi_dev, hpsi_dev, out_dev: DEVICE blocks of nst states, out must not overlap psi; eig_host: HOST [nst] or NULL
+ * (the call synchronises when it is given).  The Ritz vectors are unique up to a phase and within degenerate
+ * eigenspaces. */
+int tdh_subspace_diag(tdh_grid* g, int nst, const tdh_c128* psi_dev, const tdh_c128* hpsi_dev, tdh_c128* out_dev,
+                      double* eig_host);
+
 /* One Teter-preconditioned steepest-descent update of every state, independently (reading R19):
  *     eps_s = <psi|H psi>/<psi|psi>,  T_s = <psi|T psi>/<psi|psi>,  r = H psi - eps_s psi,
  *     p_hat(G) = K(t(G)/T_s) r_hat(G),  K(x) = (27+18x+12x^2+8x^3)/(27+18x+12x^2+8x^3+16x^4),  psi <- psi - lambda p

@@ -25,7 +25,7 @@ LIB_PATH = os.path.join(_HERE, "libtdh.so")
 #: every symbol include/tdh.h declares
 SYMBOLS = (
     "tdh_create_grid", "tdh_destroy_grid", "tdh_set_potential", "tdh_set_projectors", "tdh_apply_hamiltonian",
-    "tdh_propagate", "tdh_taylor_pair", "tdh_etrs_step", "tdh_density", "tdh_hartree", "tdh_overlap", "tdh_rotate", "tdh_orthonormalize", "tdh_sd_step", "tdh_apply_hamiltonian_host", "tdh_propagate_host", "tdh_fft3d", "tdh_last_launch_count",
+    "tdh_propagate", "tdh_taylor_pair", "tdh_etrs_step", "tdh_density", "tdh_hartree", "tdh_overlap", "tdh_rotate", "tdh_orthonormalize", "tdh_subspace_diag", "tdh_sd_step", "tdh_apply_hamiltonian_host", "tdh_propagate_host", "tdh_fft3d", "tdh_last_launch_count",
     "tdh_set_profiling", "tdh_last_kernel_seconds", "tdh_kernel_name", "tdh_set_chunk_states", "tdh_last_error",
 )
 NKERNELS = 5
@@ -66,6 +66,7 @@ def lib() -> C.CDLL:
     l.tdh_rotate.argtypes = [vp, i, vp, i, vp, vp]
     l.tdh_orthonormalize.argtypes = [vp, i, vp, vp]
     l.tdh_sd_step.argtypes = [vp, i, vp, vp, d, vp]
+    l.tdh_subspace_diag.argtypes = [vp, i, vp, vp, vp, vp]
     l.tdh_apply_hamiltonian_host.argtypes = [vp, i, vp, vp]
     l.tdh_propagate_host.argtypes = [vp, i, vp, d, i, i]
     l.tdh_fft3d.argtypes = [vp, i, vp, i]
@@ -262,6 +263,18 @@ class Grid:
             out = torch.empty_like(psi)
         _check(lib().tdh_orthonormalize(self._h, nst, C.c_void_p(psi.data_ptr()), C.c_void_p(out.data_ptr())))
         return out
+
+    def subspace_diag(self, psi, hpsi, out=None):
+        """Ritz values (ascending, host numpy) and Ritz vectors out = psi V of an orthonormal block; hpsi = H psi."""
+        import torch
+        nst = self._block(psi)
+        assert self._block(hpsi) == nst
+        if out is None:
+            out = torch.empty_like(psi)
+        eig = np.empty(nst, dtype=np.float64)
+        _check(lib().tdh_subspace_diag(self._h, nst, C.c_void_p(psi.data_ptr()), C.c_void_p(hpsi.data_ptr()),
+                                       C.c_void_p(out.data_ptr()), C.c_void_p(eig.ctypes.data)))
+        return eig, out
 
     def sd_step(self, psi, lam: float, work=None, want_eig: bool = True):
         """One Teter-preconditioned steepest-descent update in place; returns the Rayleigh quotients before the update."""

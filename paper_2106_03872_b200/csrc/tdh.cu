@@ -32,6 +32,7 @@
 #include "launch_tables.h"
 #include "nl_kernels.cuh"
 #include "overlap_kernels.cuh"
+#include "eigh_kernels.cuh"
 #include "tensor_maps.h"
 #include "tile_kernels.cuh"
 #include "xpencil_kernel.cuh"
@@ -94,6 +95,9 @@ struct tdh_grid {
     cd* d_small[3];       // n x n scratch of tdh_orthonormalize ([0] overlap / Cholesky factor, [2] rotation), grown on demand
     int small_n;
     int* d_status;        // Cholesky status word
+    tdh::JacobiRot* d_rot;  // tdh_subspace_diag: rotations of one Jacobi step
+    unsigned* d_ctl;      // tdh_subspace_diag: barrier counter, sweep maximum, sweeps used
+    double* d_w;          // tdh_subspace_diag: eigenvalues
     double* d_sd;         // tdh_sd_step: [max_states] eps, [max_states] T, [max_states * 3 * SD_SLICES] partial sums
     int ctas_fwd, ctas_inv[tdh::NL_NCM], ctas_x[5];   // persistent grid sizes (SM count x resident CTAs)
 
@@ -330,7 +334,7 @@ extern "C" int tdh_destroy_grid(tdh_grid* g) {
     cudaFree(g->d_g2y_w); cudaFree(g->d_g2z_w); cudaFree(g->d_twy_w); cudaFree(g->d_rowmap); cudaFree(g->d_colmap);
     cudaFree(g->d_p2x); cudaFree(g->d_p2y_w); cudaFree(g->d_p2z_w); cudaFree(g->d_occ);
     for (int i = 0; i < 3; ++i) cudaFree(g->d_small[i]);
-    cudaFree(g->d_status); cudaFree(g->d_sd);
+    cudaFree(g->d_status); cudaFree(g->d_sd); cudaFree(g->d_rot); cudaFree(g->d_ctl); cudaFree(g->d_w);
     cudaFree(g->d_work); cudaFree(g->d_phi[0]); cudaFree(g->d_phi[1]);
     for (int i = 0; i < 2; ++i) {
         cudaFree(g->d_hin[i]); cudaFree(g->d_hout[i]);
@@ -1165,21 +1169,72 @@ extern "C" int tdh_rotate(tdh_grid* g, int n_in, const tdh_c128* psi_dev, int n_
     return launch_rotate(g, n_in, (const cd*)psi_dev, n_out, (const cd*)m_dev, (cd*)out_dev, 0);
 }
 
+// n x n scratch matrices of the rotations in the space of states: allocated at first use, grown for a larger block
+static int small_scratch(tdh_grid* g, int nst) {
+    if (g->small_n >= nst) return TDH_OK;
+    CU(cudaStreamSynchronize(g->stream));
+    for (int i = 0; i < 3; ++i) { cudaFree(g->d_small[i]); g->d_small[i] = nullptr; }
+    cudaFree(g->d_rot); g->d_rot = nullptr;
+    cudaFree(g->d_w); g->d_w = nullptr;
+    g->small_n = 0;
+    for (int i = 0; i < 3; ++i) CU(cudaMalloc(&g->d_small[i], sizeof(cd) * (size_t)nst * nst));
+    CU(cudaMalloc(&g->d_rot, sizeof(tdh::JacobiRot) * (size_t)(nst / 2 + 1)));
+    CU(cudaMalloc(&g->d_w, sizeof(double) * (size_t)nst));
+    if (!g->d_status) CU(cudaMalloc(&g->d_status, 2 * sizeof(int)));       // [0] status, [1] grid-barrier counter
+    if (!g->d_ctl) CU(cudaMalloc(&g->d_ctl, 8 * sizeof(unsigned)));
+    g->small_n = nst;
+    return TDH_OK;
+}
+
+// Subspace diagonalisation of an orthonormal block: M = dV psi^H (H psi) = V diag(w) V^H, out = psi V
+extern "C" int tdh_subspace_diag(tdh_grid* g, int nst, const tdh_c128* psi_dev, const tdh_c128* hpsi_dev, tdh_c128* out_dev,
+                                 double* eig_host) {
+    if (!g || !psi_dev || !hpsi_dev || !out_dev) return fail(TDH_EINVAL, "tdh_subspace_diag: null argument");
+    if (nst < 1 || nst > 1024) return fail(nst < 1 ? TDH_EINVAL : TDH_EUNSUPPORTED, "tdh_subspace_diag: nst = %d outside [1, 1024]", nst);
+    if (overlaps(psi_dev, out_dev, (size_t)nst * g->np * sizeof(cd)))
+        return fail(TDH_EINVAL, "tdh_subspace_diag: psi and out overlap");
+    int rc = small_scratch(g, nst);
+    if (rc) return rc;
+    if ((rc = tdh_overlap(g, nst, psi_dev, nst, hpsi_dev, (tdh_c128*)g->d_small[1]))) return rc;
+    tdh::symmetrize_kernel<<<296, 256, 0, g->stream>>>(g->d_small[1], nst, g->d_small[0]);
+    CU(cudaGetLastError());
+    {
+        int dev = 0, nsm = 0, occ = 0;
+        CU(cudaGetDevice(&dev));
+        CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tdh::jacobi_eigh_kernel, 256, 0));
+        const int want = (int)(((size_t)nst * (nst / 2 + 1) + 255) / 256);
+        const int ctas = std::max(1, std::min(nsm * std::min(occ, 2), want));
+        CU(cudaMemsetAsync(g->d_ctl, 0, 8 * sizeof(unsigned), g->stream));
+        cd* a = g->d_small[0];
+        cd* v = g->d_small[1];
+        int n = nst;
+        tdh::JacobiRot* rot = g->d_rot;
+        unsigned* ctl = g->d_ctl;
+        void* args[] = {(void*)&a, (void*)&v, (void*)&n, (void*)&rot, (void*)&ctl};
+        CU(cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(&tdh::jacobi_eigh_kernel), dim3(ctas), dim3(256), args,
+                                       0, g->stream));
+    }
+    tdh::eigh_sort_kernel<<<1, 256, sizeof(double) * nst, g->stream>>>(g->d_small[0], g->d_small[1], nst, g->d_w, g->d_small[2]);
+    CU(cudaGetLastError());
+    g->launch_count += 3;
+    if ((rc = launch_rotate(g, nst, (const cd*)psi_dev, nst, g->d_small[2], (cd*)out_dev, 0))) return rc;
+    if (eig_host) {
+        CU(cudaMemcpyAsync(eig_host, g->d_w, sizeof(double) * nst, cudaMemcpyDeviceToHost, g->stream));
+        CU(cudaStreamSynchronize(g->stream));
+    }
+    return TDH_OK;
+}
+
 // Cholesky orthonormalisation: S = dV psi^H psi = L L^H, out = psi L^{-H}
 extern "C" int tdh_orthonormalize(tdh_grid* g, int nst, const tdh_c128* psi_dev, tdh_c128* out_dev) {
     if (!g || !psi_dev || !out_dev) return fail(TDH_EINVAL, "tdh_orthonormalize: null argument");
     if (nst < 1 || nst > 1024) return fail(nst < 1 ? TDH_EINVAL : TDH_EUNSUPPORTED, "tdh_orthonormalize: nst = %d outside [1, 1024]", nst);
     if (overlaps(psi_dev, out_dev, (size_t)nst * g->np * sizeof(cd)))
         return fail(TDH_EINVAL, "tdh_orthonormalize: psi and out overlap");
-    if (g->small_n < nst) {                       // first use (or a larger block): n x n scratch
-        CU(cudaStreamSynchronize(g->stream));
-        for (int i = 0; i < 3; ++i) { cudaFree(g->d_small[i]); g->d_small[i] = nullptr; }
-        g->small_n = 0;
-        for (int i = 0; i < 3; i += 2) CU(cudaMalloc(&g->d_small[i], sizeof(cd) * (size_t)nst * nst));   // [0] S / L, [2] L^{-H}
-        if (!g->d_status) CU(cudaMalloc(&g->d_status, 2 * sizeof(int)));       // [0] status, [1] grid-barrier counter
-        g->small_n = nst;
-    }
-    int rc = tdh_overlap(g, nst, psi_dev, nst, psi_dev, (tdh_c128*)g->d_small[0]);
+    int rc = small_scratch(g, nst);
+    if (rc) return rc;
+    rc = tdh_overlap(g, nst, psi_dev, nst, psi_dev, (tdh_c128*)g->d_small[0]);
     if (rc) return rc;
     {
         // cooperative launch: as many CTAs as are resident at once, at most one warp per row
