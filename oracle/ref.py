@@ -26,7 +26,7 @@ def lib() -> C.CDLL:
     if _lib is None:
         _lib = C.CDLL(_build.build())
         for name in ("ref_dft3d", "ref_kinetic", "ref_local", "ref_nonlocal", "ref_apply_hamiltonian",
-                     "ref_propagate", "ref_taylor_pair", "ref_etrs_step", "ref_density", "ref_hartree", "ref_overlap", "ref_sd_step", "ref_num_threads"):
+                     "ref_propagate", "ref_taylor_pair", "ref_etrs_step", "ref_density", "ref_hartree", "ref_overlap", "ref_sd_step", "ref_gradient", "ref_forces", "ref_num_threads"):
             getattr(_lib, name).restype = C.c_int
     return _lib
 
@@ -229,6 +229,29 @@ def subspace_diag(n, dv: float, psi, hpsi):
     m = overlap(n, dv, psi, hpsi)
     w, v = np.linalg.eigh(0.5 * (m + m.conj().T))
     return w, rotate(psi, v), v
+
+
+def gradient(n, length, kpt, axis: int, psi, backend: int = NAIVE_FFT) -> np.ndarray:
+    """d_axis psi = DFT^-1(i (G_a + k_a) DFT psi) for a block or a single state."""
+    psi = _c128(psi)
+    out = np.empty_like(psi)
+    nst = 1 if psi.ndim == 3 else psi.shape[0]
+    _check(lib().ref_gradient(_i3(n), _d3(length), _d3(kpt), C.c_int(axis), C.c_int(nst), _ptr(psi), _ptr(out),
+                              C.c_int(backend)), "gradient")
+    return out
+
+
+def forces(n, length, kpt, proj, psi, occ=None, vloc_atoms=None, backend: int = NAIVE_FFT) -> np.ndarray:
+    """Eq. 11: F[I][a] = sum_s f_s (<d_a psi_s|v_I|psi_s> + c.c.); vloc_atoms: (natoms, n0, n1, n2) float64 or None."""
+    psi = _c128(psi)
+    nst = 1 if psi.ndim == 3 else psi.shape[0]
+    p = _Proj(proj)
+    occ = None if occ is None else np.ascontiguousarray(occ, dtype=np.float64)
+    vl = None if vloc_atoms is None else np.ascontiguousarray(vloc_atoms, dtype=np.float64)
+    out = np.zeros((p.natoms, 3), dtype=np.float64)
+    _check(lib().ref_forces(_i3(n), _d3(length), _d3(kpt), *p.args, _ptr(vl), C.c_int(nst), _ptr(psi), _ptr(occ), _ptr(out),
+                            C.c_int(backend)), "forces")
+    return out
 
 
 def apply_workload(wl, psi, backend: int = NAIVE_FFT) -> np.ndarray:

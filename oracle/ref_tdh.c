@@ -651,6 +651,92 @@ int ref_sd_step(const int n[3], const double len[3], const double kpt[3], double
     return err;
 }
 
+/* ------------------------------------------------------------------------------------------------
+ * exported (NEXT-4): gradient of a block, "just like the Laplacian, a local operation in Fourier space":
+ *   (d_a psi)[p] = DFT^-1( i (G_a + k_a) DFT(psi) ),  a = axis (0, 1, 2);  frequencies as in the kinetic term (R7), no mask.
+ * ------------------------------------------------------------------------------------------------ */
+static int gradient_one(const int n[3], const double len[3], const double kpt[3], int axis, const cplx *psi, cplx *out,
+                        int backend)
+{
+    const size_t np_ = npoints(n);
+    const double two_pi = 6.283185307179586476925286766559;
+    memcpy(out, psi, sizeof(cplx) * np_);
+    int e = dft3d_one(n, out, -1, backend);
+    if (e != REF_OK) return e;
+    for (int i = 0; i < n[0]; ++i)
+        for (int j = 0; j < n[1]; ++j)
+            for (int k = 0; k < n[2]; ++k) {
+                const int idx[3] = {i, j, k};
+                const double ga = two_pi * freq_index(idx[axis], n[axis]) / len[axis] + kpt[axis];
+                out[((size_t)i * n[1] + j) * n[2] + k] *= I * ga;
+            }
+    return dft3d_one(n, out, +1, backend);
+}
+
+int ref_gradient(const int n[3], const double len[3], const double kpt[3], int axis, int nst, const cplx *psi, cplx *out,
+                 int backend)
+{
+    if (check_geometry(n, len) || !kpt || !psi || !out || nst < 0 || axis < 0 || axis > 2) return REF_EINVAL;
+    const size_t np_ = npoints(n);
+    int err = REF_OK;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int s = 0; s < nst; ++s) {
+        int e = gradient_one(n, len, kpt, axis, psi + (size_t)s * np_, out + (size_t)s * np_, backend);
+        if (e != REF_OK) {
+#pragma omp critical
+            err = e;
+        }
+    }
+    return err;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * exported (NEXT-4): Eq. 11 literally, per atom I and axis a:
+ *   F[I][a] = sum_s f_s ( <d_a psi_s | v_I | psi_s> + c.c. ) = sum_s f_s 2 Re( dV sum_p conj(d_a psi_s[p]) (v_I psi_s)[p] )
+ * v_I = the Kleinman-Bylander projectors of atom I (Eq. 9 restricted to that atom) plus, when vloc_atoms != NULL, the
+ * atom's own local potential vloc_atoms[I][p].  occ == NULL: all f_s = 1.  forces: [natoms][3].
+ * ------------------------------------------------------------------------------------------------ */
+int ref_forces(const int n[3], const double len[3], const double kpt[3], int natoms, const int64_t *sph_off,
+               const int32_t *sph_idx, const double *sph_disp, const int32_t *chan_off, const double *beta,
+               const double *dcoef, const double *vloc_atoms, int nst, const cplx *psi, const double *occ, double *forces,
+               int backend)
+{
+    if (check_geometry(n, len) || !kpt || !psi || !forces || nst < 0 || natoms < 0) return REF_EINVAL;
+    if (check_projectors(n, natoms, sph_off, sph_idx, chan_off, beta, dcoef)) return REF_EINVAL;
+    const size_t np_ = npoints(n);
+    const double dv = (len[0] / n[0]) * (len[1] / n[1]) * (len[2] / n[2]);
+    for (int i = 0; i < 3 * natoms; ++i) forces[i] = 0.0;
+    cplx *grad = (cplx *)malloc(sizeof(cplx) * np_);
+    cplx *w = (cplx *)malloc(sizeof(cplx) * np_);
+    int e = (grad && w) ? REF_OK : REF_ENOMEM;
+    for (int s = 0; s < nst && e == REF_OK; ++s) {
+        const cplx *x = psi + (size_t)s * np_;
+        const double f = occ ? occ[s] : 1.0;
+        for (int a = 0; a < 3 && e == REF_OK; ++a) {
+            e = gradient_one(n, len, kpt, a, x, grad, backend);
+            size_t boff = 0;
+            for (int ia = 0; ia < natoms && e == REF_OK; ++ia) {
+                const int64_t pn = sph_off[ia + 1] - sph_off[ia];
+                const int nc = chan_off[ia + 1] - chan_off[ia];
+                /* w = v_I psi: this atom's projectors (nonlocal_one on a one-atom table), plus its local potential */
+                memset(w, 0, sizeof(cplx) * np_);
+                const int64_t so[2] = {sph_off[ia], sph_off[ia + 1]};
+                const int32_t co[2] = {chan_off[ia], chan_off[ia + 1]};
+                nonlocal_one(dv, kpt, 1, so, sph_idx, sph_disp, co, beta + boff, dcoef, x, w);
+                if (vloc_atoms)
+                    for (size_t p = 0; p < np_; ++p) w[p] += vloc_atoms[(size_t)ia * np_ + p] * x[p];
+                cplx acc = 0.0;
+                for (size_t p = 0; p < np_; ++p) acc += conj(grad[p]) * w[p];
+                forces[3 * ia + a] += f * 2.0 * creal(dv * acc);
+                boff += (size_t)nc * (size_t)pn;
+            }
+        }
+    }
+    free(grad);
+    free(w);
+    return e;
+}
+
 /* number of OpenMP threads the block loops will use (reported by bench.py's cpu_baseline) */
 int ref_num_threads(void)
 {

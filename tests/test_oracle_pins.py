@@ -6,6 +6,7 @@ a brute-force triple sum, a closed form, an invariant, a library routine used as
 import math
 
 import numpy as np
+from dataclasses import replace as dataclasses_replace
 import pytest
 
 from paper_2106_03872_b200 import workloads as W
@@ -613,6 +614,66 @@ def test_p13_subspace_diag_recovers_mixed_eigenvectors_and_cauchy_bounds(oracle)
     assert np.abs(m2 - np.diag(w)).max() < 1e-12
     assert abs(w.sum() - np.trace(oracle.overlap(cfg.n, cfg.dv, psi, hp)).real) < 1e-12
     assert all(w[i] >= ev[i] - 1e-12 for i in range(3)) and all(w[2 - i] <= ev[-1 - i] + 1e-12 for i in range(3))
+
+
+# --------------------------------------------------------------------------------------------- P14 (NEXT-4: gradient, forces)
+def test_p14_gradient_of_plane_waves(oracle):
+    """d_a e^{iG.r} = i (G_a + k_a) e^{iG.r} (psi is the periodic part u_k, so the Bloch vector enters as in the kinetic term)."""
+    n, length = (6, 8, 5), (5.0, 7.0, 4.0)
+    kpt = [TWO_PI * 0.2 / length[0], 0.0, -TWO_PI * 0.1 / length[2]]
+    ii = np.meshgrid(*[np.arange(m) for m in n], indexing="ij")
+    ms = [(0, 0, 0), (1, -2, 2), (-2, 3, -1), (2, 1, 0)]
+    psi = np.array([np.exp(2j * np.pi * sum(m[a] * ii[a] / n[a] for a in range(3))) for m in ms])
+    for backend in (0, 1):
+        for a in range(3):
+            g = oracle.gradient(n, length, kpt, a, psi, backend)
+            for s, m in enumerate(ms):
+                assert rel(g[s], 1j * (TWO_PI * m[a] / length[a] + kpt[a]) * psi[s]) < 1e-12 or np.abs(g[s]).max() < 1e-12
+
+
+def test_p14_forces_are_the_derivative_of_the_ionic_energy_at_fixed_orbitals(oracle):
+    """Eq. 11 equals d/dR_I of E_I(R) = sum_s f_s <psi_s| v_I(r - R_I) |psi_s> at fixed orbitals (translate the atom, rebuild
+    its projector table and its local well, central differences) -- for smooth band-limited orbitals and projectors that
+    are negligible at the cutoff sphere.  Checks sign, the factor 2 Re, occupations, the per-atom split, both terms."""
+    cfg = W.test_config(119, (12, 12, 12), (6.0, 6.0, 6.0), nst=3, natoms=2, lmax=1, rc=2.9, dl=(1.5, -0.7), proj_sigma=0.5,
+                        well_z=1.2, well_sigma=0.7)
+    pos = np.array([[2.1, 3.3, 2.7], [4.0, 1.6, 3.9]])
+    ii = np.meshgrid(*[np.arange(m) for m in cfg.n], indexing="ij")
+    rng = np.random.default_rng(119)
+    ms = [(a, b, c) for a in (0, 1, -1) for b in (0, 1, -1) for c in (0, 1, -1)]
+    pw = np.array([np.exp(2j * np.pi * sum(m[k] * ii[k] / cfg.n[k] for k in range(3))) for m in ms])
+    psi = np.tensordot(rand_c(rng, (3, len(ms))), pw, axes=(1, 0))                    # band-limited, not normalised
+    occ = np.array([2.0, 1.0, 0.5])
+
+    def well(center):
+        return W.local_potential(dataclasses_replace(cfg, natoms=1), np.array([center]))
+
+    def energy(atom, center):
+        one = W.projectors(dataclasses_replace(cfg, natoms=1), np.array([center]))
+        e = 0.0
+        v = well(center)
+        for s in range(3):
+            nl = oracle.nonlocal_(cfg.n, cfg.length, cfg.kpt, one, psi[s])
+            e += occ[s] * cfg.dv * (np.vdot(psi[s], nl).real + np.sum(v * np.abs(psi[s]) ** 2))
+        return e
+
+    proj = W.projectors(cfg, pos)
+    vloc = np.array([well(pos[0]), well(pos[1])])
+    f = oracle.forces(cfg.n, cfg.length, cfg.kpt, proj, psi, occ, vloc, 0)
+    f_nl = oracle.forces(cfg.n, cfg.length, cfg.kpt, proj, psi, occ, None, 0)
+    assert np.abs(f - f_nl).max() > 1e-3 * np.abs(f).max()                            # the local term is visible
+    delta = 1e-3
+    for atom in range(2):
+        for a in range(3):
+            d = np.zeros(3); d[a] = delta
+            fd = (energy(atom, pos[atom] + d) - energy(atom, pos[atom] - d)) / (2 * delta)
+            # equality holds in the band-limited limit; on this grid (h = 0.5, sigma = 0.5) aliasing of the projectors
+            # leaves a few 1e-4 relative -- a dropped term, a wrong sign or a missing factor 2 is an O(1) error
+            assert abs(f[atom, a] - fd) < 2e-3 * np.abs(f).max(), (atom, a, f[atom, a], fd)
+    # occupations enter linearly; a constant orbital at Gamma has no gradient, hence no force
+    assert np.abs(oracle.forces(cfg.n, cfg.length, cfg.kpt, proj, psi, 2 * occ, vloc, 0) - 2 * f).max() < 1e-12 * np.abs(f).max()
+    const = np.ones((1,) + cfg.n, dtype=np.complex128)
+    assert np.abs(oracle.forces(cfg.n, cfg.length, cfg.kpt, proj, const, None, vloc, 0)).max() < 1e-12
 
 
 # --------------------------------------------------------------------------------------------- P8
