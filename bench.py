@@ -429,6 +429,10 @@ def sweep_leg(torch, B, name, flush, reps=7):
             res["sd_step"] = {"seconds": tsd, "launches": g.last_launch_count(),
                               "note": "tdh_sd_step on the whole block: H psi, T psi, Rayleigh quotients, residual, Teter "
                                       "preconditioner pass with the fused update (about 2.7 H-application equivalents)"}
+            tfo = statistics.median(timed_each(torch, lambda: g.forces(psi, cfg.natoms), 3, flush))
+            res["forces"] = {"seconds": tfo, "launches": g.last_launch_count(),
+                             "note": "tdh_forces (Eq. 11, non-local part) of the whole block: forward transform, three gradient "
+                                     "chains, four projector gathers per state (host timer incl. the result copy)"}
             hps = g.apply_hamiltonian(work)
             tsub = statistics.median(timed_each(torch, lambda: g.subspace_diag(work, hps, out=out), 3, flush))
             res["subspace_diag"] = {"seconds": tsub, "launches": g.last_launch_count(),
@@ -549,6 +553,7 @@ def main():
             extra["orthonormalize"] = wls["tddft"].pop("orthonormalize")
             extra["sd_step"] = wls["tddft"].pop("sd_step")
             extra["subspace_diag"] = wls["tddft"].pop("subspace_diag")
+            extra["forces"] = wls["tddft"].pop("forces")
     else:
         g.close()
 

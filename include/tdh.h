@@ -167,6 +167,21 @@ int tdh_subspace_diag(tdh_grid* g, int nst, const tdh_c128* psi_dev, const tdh_c
  * (tdh_orthonormalize).  Asynchronous unless eig_host is given. */
 int tdh_sd_step(tdh_grid* g, int nst, tdh_c128* psi_dev, tdh_c128* work_dev, double lambda, double* eig_host);
 
+/* Gradient along one axis, "a local operation in Fourier space":
+ *     out = FFT^-1( i (G_a + k_a) FFT(psi) ),   axis a = 0, 1, 2   (frequency convention as in the kinetic term, no mask)
+ * psi_dev, out_dev: DEVICE blocks of nst states, must not overlap.  Asynchronous on the handle's stream. */
+int tdh_gradient(tdh_grid* g, int nst, const tdh_c128* psi_dev, int axis, tdh_c128* out_dev);
+
+/* Eq. 11, per atom I of the projector table and axis a:
+ *     F[I][a] = sum_s f_s ( <d_a psi_s | v_I | psi_s> + c.c. )
+ * with v_I = the atom's Kleinman-Bylander projectors plus, if vloc_atoms_dev != NULL, its own local potential
+ * vloc_atoms_dev[I][p] (DEVICE, natoms*n0*n1*n2 doubles).  occ_host: HOST [nst] or NULL (all 1).
+ * forces_host: HOST [natoms][3].  This is +dE_I/dR_I of E_I = sum_s f_s <psi_s|v_I(r - R_I)|psi_s> at fixed orbitals
+ * (reading R20).  One forward transform, three gradient chains and four projector gathers per state;
+ * the non-local part is 2 Re of the projection coefficients of d_a psi against those of psi.  Synchronises. */
+int tdh_forces(tdh_grid* g, int nst, const tdh_c128* psi_dev, const double* occ_host, const double* vloc_atoms_dev,
+               double* forces_host);
+
 /* The same two operations with HOST buffers (pageable or pinned): the library stages state chunks through its own
  * pinned buffers, overlapping host<->device copies with the kernels, and returns when hpsi_host / psi_host is complete.
  * nst is not limited by max_states here (chunks are).  These are the end-to-end entry points timed by bench.py. */

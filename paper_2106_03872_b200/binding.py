@@ -25,7 +25,7 @@ LIB_PATH = os.path.join(_HERE, "libtdh.so")
 #: every symbol include/tdh.h declares
 SYMBOLS = (
     "tdh_create_grid", "tdh_destroy_grid", "tdh_set_potential", "tdh_set_projectors", "tdh_apply_hamiltonian",
-    "tdh_propagate", "tdh_taylor_pair", "tdh_etrs_step", "tdh_density", "tdh_hartree", "tdh_overlap", "tdh_rotate", "tdh_orthonormalize", "tdh_subspace_diag", "tdh_sd_step", "tdh_apply_hamiltonian_host", "tdh_propagate_host", "tdh_fft3d", "tdh_last_launch_count",
+    "tdh_propagate", "tdh_taylor_pair", "tdh_etrs_step", "tdh_density", "tdh_hartree", "tdh_overlap", "tdh_rotate", "tdh_orthonormalize", "tdh_subspace_diag", "tdh_sd_step", "tdh_gradient", "tdh_forces", "tdh_apply_hamiltonian_host", "tdh_propagate_host", "tdh_fft3d", "tdh_last_launch_count",
     "tdh_set_profiling", "tdh_last_kernel_seconds", "tdh_kernel_name", "tdh_set_chunk_states", "tdh_last_error",
 )
 NKERNELS = 5
@@ -67,6 +67,8 @@ def lib() -> C.CDLL:
     l.tdh_orthonormalize.argtypes = [vp, i, vp, vp]
     l.tdh_sd_step.argtypes = [vp, i, vp, vp, d, vp]
     l.tdh_subspace_diag.argtypes = [vp, i, vp, vp, vp, vp]
+    l.tdh_gradient.argtypes = [vp, i, vp, i, vp]
+    l.tdh_forces.argtypes = [vp, i, vp, vp, vp, vp]
     l.tdh_apply_hamiltonian_host.argtypes = [vp, i, vp, vp]
     l.tdh_propagate_host.argtypes = [vp, i, vp, d, i, i]
     l.tdh_fft3d.argtypes = [vp, i, vp, i]
@@ -262,6 +264,31 @@ class Grid:
         if out is None:
             out = torch.empty_like(psi)
         _check(lib().tdh_orthonormalize(self._h, nst, C.c_void_p(psi.data_ptr()), C.c_void_p(out.data_ptr())))
+        return out
+
+    def gradient(self, psi, axis: int, out=None):
+        """d_axis psi through Fourier space."""
+        import torch
+        nst = self._block(psi)
+        if out is None:
+            out = torch.empty_like(psi)
+        _check(lib().tdh_gradient(self._h, nst, C.c_void_p(psi.data_ptr()), int(axis), C.c_void_p(out.data_ptr())))
+        return out
+
+    def forces(self, psi, natoms: int, occ=None, vloc_atoms=None):
+        """Eq. 11 per atom and axis -> (natoms, 3) host numpy; vloc_atoms: device float64 (natoms, n0, n1, n2) or None."""
+        import torch
+        nst = self._block(psi)
+        occ_arr = None if occ is None else np.ascontiguousarray(occ, dtype=np.float64)
+        assert occ_arr is None or occ_arr.size == nst
+        if vloc_atoms is not None:
+            assert vloc_atoms.is_cuda and vloc_atoms.dtype == torch.float64 and vloc_atoms.is_contiguous()
+            assert vloc_atoms.numel() == natoms * self.npts
+        out = np.zeros((natoms, 3), dtype=np.float64)
+        _check(lib().tdh_forces(self._h, nst, C.c_void_p(psi.data_ptr()),
+                                None if occ_arr is None else C.c_void_p(occ_arr.ctypes.data),
+                                None if vloc_atoms is None else C.c_void_p(vloc_atoms.data_ptr()),
+                                C.c_void_p(out.ctypes.data)))
         return out
 
     def subspace_diag(self, psi, hpsi, out=None):

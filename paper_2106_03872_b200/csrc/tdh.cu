@@ -92,6 +92,11 @@ struct tdh_grid {
     double* d_p2y_w;      // |G_y|^2, work-layout order
     double* d_p2z_w;      // |G_z|^2, work-layout order
     double* d_occ;        // [max_states] occupations of the last tdh_density call
+    double* d_gs[3];      // signed G_a + k_a: x in natural order, y and z in work-layout order (gradient, forces)
+    double* d_dvscale;    // [nchan_tot] dV: projections without the KB coefficient (forces)
+    cd* d_dpig;           // [chunk_cap][nchan_tot] dV <beta|d_a psi> (forces)
+    double* d_gd;         // [3][N_p] sum_s f_s 2 Re conj(d_a psi_s) psi_s (forces, local term)
+    double* d_force;      // [natoms][3] + reduction scratch (forces)
     cd* d_small[3];       // n x n scratch of tdh_orthonormalize ([0] overlap / Cholesky factor, [2] rotation), grown on demand
     int small_n;
     int* d_status;        // Cholesky status word
@@ -164,6 +169,8 @@ static int freq_index(int a, int n) {
 static void free_projectors(tdh_grid* g) {
     cudaFree(g->d_atoms); cudaFree(g->d_sidx); cudaFree(g->d_sbeta); cudaFree(g->d_sphase); cudaFree(g->d_dscale);
     cudaFree(g->d_atoms_col); g->d_atoms_col = nullptr; g->col_off.clear();
+    cudaFree(g->d_dvscale); g->d_dvscale = nullptr; cudaFree(g->d_dpig); g->d_dpig = nullptr;
+    cudaFree(g->d_force); g->d_force = nullptr;
     cudaFree(g->d_dpi); cudaFree(g->d_nl_off); cudaFree(g->d_nl_cc); cudaFree(g->d_nl_beta); cudaFree(g->d_nl_phase);
     g->d_atoms = nullptr; g->d_sidx = nullptr; g->d_sbeta = nullptr; g->d_sphase = nullptr; g->d_dscale = nullptr;
     g->d_dpi = nullptr; g->d_nl_off = nullptr; g->d_nl_cc = nullptr; g->d_nl_beta = nullptr; g->d_nl_phase = nullptr;
@@ -304,6 +311,16 @@ extern "C" int tdh_create_grid(const int n[3], const double len[3], const double
             CU(cudaMemcpy(g->d_p2y_w, p2y_w.data(), sizeof(double) * ny, cudaMemcpyHostToDevice));
             CU(cudaMemcpy(g->d_p2z_w, p2z_w.data(), sizeof(double) * nz, cudaMemcpyHostToDevice));
             CU(cudaMalloc(&g->d_occ, sizeof(double) * max_states));
+            // signed G_a + k_a (gradient): x natural, y and z in work-layout order
+            std::vector<double> gsx(n[0]), gsy(ny), gsz(nz);
+            for (int kx = 0; kx < n[0]; ++kx) gsx[kx] = two_pi * freq_index(kx, n[0]) / len[0] + kpt[0];
+            for (int ky = 0; ky < ny; ++ky) gsy[rowmap[ky]] = two_pi * freq_index(ky, ny) / len[1] + kpt[1];
+            for (int kz = 0; kz < nz; ++kz) gsz[colmap[kz]] = two_pi * freq_index(kz, nz) / len[2] + kpt[2];
+            const std::vector<double>* gsv[3] = {&gsx, &gsy, &gsz};
+            for (int a = 0; a < 3; ++a) {
+                CU(cudaMalloc(&g->d_gs[a], sizeof(double) * n[a]));
+                CU(cudaMemcpy(g->d_gs[a], gsv[a]->data(), sizeof(double) * n[a], cudaMemcpyHostToDevice));
+            }
         }
         CU(cudaMalloc(&g->d_v, sizeof(double) * g->np));
         CU(cudaMemset(g->d_v, 0, sizeof(double) * g->np));
@@ -333,6 +350,8 @@ extern "C" int tdh_destroy_grid(tdh_grid* g) {
     for (int a = 0; a < 3; ++a) { cudaFree(g->d_g2[a]); cudaFree(g->d_tw[a]); }
     cudaFree(g->d_g2y_w); cudaFree(g->d_g2z_w); cudaFree(g->d_twy_w); cudaFree(g->d_rowmap); cudaFree(g->d_colmap);
     cudaFree(g->d_p2x); cudaFree(g->d_p2y_w); cudaFree(g->d_p2z_w); cudaFree(g->d_occ);
+    for (int a = 0; a < 3; ++a) cudaFree(g->d_gs[a]);
+    cudaFree(g->d_gd);
     for (int i = 0; i < 3; ++i) cudaFree(g->d_small[i]);
     cudaFree(g->d_status); cudaFree(g->d_sd); cudaFree(g->d_rot); cudaFree(g->d_ctl); cudaFree(g->d_w);
     cudaFree(g->d_work); cudaFree(g->d_phi[0]); cudaFree(g->d_phi[1]);
@@ -532,6 +551,13 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
     cudaError_t e = cudaMalloc(&g->d_dpi, sizeof(cd) * ndpi);
     if (e == cudaSuccess) e = cudaMemset(g->d_dpi, 0, sizeof(cd) * ndpi);
     if (e != cudaSuccess) { free_projectors(g); return fail(TDH_ENOMEM, "tdh_set_projectors: %s", cudaGetErrorString(e)); }
+    {
+        std::vector<double> dvs(ctot, g->dv);
+        if ((rc = up(&g->d_dvscale, dvs))) { free_projectors(g); return rc; }
+        e = cudaMalloc(&g->d_dpig, sizeof(cd) * (size_t)g->chunk_cap * ctot);
+        if (e == cudaSuccess) e = cudaMalloc(&g->d_force, sizeof(double) * (size_t)natoms * 3 * (1 + 64));
+        if (e != cudaSuccess) { free_projectors(g); return fail(TDH_ENOMEM, "tdh_set_projectors: %s", cudaGetErrorString(e)); }
+    }
     g->natoms = natoms;
     g->nchan_tot = ctot;
     g->nl_layers = nlayers;
@@ -698,14 +724,14 @@ static int launch_reorder(tdh_grid* g, int nst, const cd* in, cd* out, int dir) 
     return TDH_OK;
 }
 
-static int launch_nl_project(tdh_grid* g, int nst, const cd* in) {
+static int launch_nl_project(tdh_grid* g, int nst, const cd* in, const double* dscale_in = nullptr, cd* dpi_out = nullptr) {
     size_t npts = g->np;
     const tdh::AtomDesc* atoms = g->d_atoms;
     const int* sidx = g->d_sidx;
     const double* sbeta = g->d_sbeta;
     const cd* sphase = g->d_sphase;
-    const double* dscale = g->d_dscale;
-    cd* dpi = g->d_dpi;
+    const double* dscale = dscale_in ? dscale_in : g->d_dscale;
+    cd* dpi = dpi_out ? dpi_out : g->d_dpi;
     int nct = g->nchan_tot;
     void* args[] = {(void*)&in, (void*)&npts, (void*)&nst, (void*)&atoms, (void*)&sidx, (void*)&sbeta,
                     (void*)&sphase, (void*)&dscale, (void*)&dpi, (void*)&nct};
@@ -995,6 +1021,166 @@ extern "C" int tdh_hartree(tdh_grid* g, const double* n_dev, double* vh_dev) {
     complex_to_real_kernel<<<296, 256, 0, g->stream>>>(a, vh_dev, g->np);
     CU(cudaGetLastError());
     g->launch_count += 1;
+    return prof_collect(g);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// NEXT-4: gradient in Fourier space and the forces of Eq. 11 (reading R20)
+// ------------------------------------------------------------------------------------------------------------
+// out = i (G_a + k_a) in on a spectrum in work layout [state][x][Y][z'] (x natural, Y and z' permuted: the tables are in
+// the same orders)
+__global__ void grad_scale_kernel(const cd* __restrict__ in, cd* __restrict__ out, size_t total, int nx, int ny, int nz,
+                                  const double* __restrict__ gs, int axis) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const int z = (int)(i % nz), y = (int)((i / nz) % ny), x = (int)((i / ((size_t)nz * ny)) % nx);
+        const double ga = gs[axis == 0 ? x : (axis == 1 ? y : z)];
+        const cd v = __ldcs(in + i);
+        __stcs(out + i, make_double2(-ga * v.y, ga * v.x));
+    }
+}
+
+// gd[p] (+)= sum_s occ[s] 2 Re( conj(grad_s[p]) psi_s[p] ), states in order
+__global__ void grad_density_kernel(const cd* __restrict__ grad, const cd* __restrict__ psi, size_t npts, int nst,
+                                    const double* __restrict__ occ, double* __restrict__ gd, int accumulate) {
+    const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= npts) return;
+    double acc = accumulate ? gd[p] : 0.0;
+    for (int s = 0; s < nst; ++s) {
+        const cd a = __ldcs(grad + (size_t)s * npts + p), b = __ldcs(psi + (size_t)s * npts + p);
+        acc += (occ ? occ[s] : 1.0) * 2.0 * (a.x * b.x + a.y * b.y);
+    }
+    gd[p] = acc;
+}
+
+// f[I][axis] += sum_s occ[s] 2 Re sum_{c in I} conj(dpig[s][c]) dpi[s][c]   (one thread per atom, fixed order)
+__global__ void force_nl_kernel(const tdh::AtomDesc* __restrict__ atoms, int natoms, int nst, int nct, const cd* __restrict__ dpig,
+                                const cd* __restrict__ dpi, const double* __restrict__ occ, int axis, double* __restrict__ f) {
+    const int ia = blockIdx.x * blockDim.x + threadIdx.x;
+    if (ia >= natoms) return;
+    const tdh::AtomDesc at = atoms[ia];
+    double acc = 0.0;
+    for (int s = 0; s < nst; ++s) {
+        double t = 0.0;
+        for (int c = 0; c < at.nchan; ++c) {
+            const cd a = dpig[(size_t)s * nct + at.chan0 + c], b = dpi[(size_t)s * nct + at.chan0 + c];
+            t += a.x * b.x + a.y * b.y;
+        }
+        acc += (occ ? occ[s] : 1.0) * 2.0 * t;
+    }
+    f[3 * ia + axis] += acc;
+}
+
+// partial[(I*3 + a)*64 + slice] = sum over the slice's points of v_I[p] gd_a[p]; grid (64, natoms*3), 256 threads
+__global__ void force_loc_partial_kernel(const double* __restrict__ vloc, const double* __restrict__ gd, size_t npts,
+                                         double* __restrict__ partial) {
+    __shared__ double red[8];
+    const int ia = blockIdx.y / 3, a = blockIdx.y % 3, slice = blockIdx.x;
+    const size_t per = (npts + 63) / 64, p0 = (size_t)slice * per, p1 = p0 + per < npts ? p0 + per : npts;
+    const double* v = vloc + (size_t)ia * npts;
+    const double* d = gd + (size_t)a * npts;
+    double acc = 0.0;
+    for (size_t p = p0 + threadIdx.x; p < p1; p += blockDim.x) acc += v[p] * d[p];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < 8; ++w) t += red[w];
+        partial[(size_t)blockIdx.y * 64 + slice] = t;
+    }
+}
+__global__ void force_loc_final_kernel(const double* __restrict__ partial, int n3, double dv, double* __restrict__ f) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n3) return;
+    double t = 0.0;
+    for (int k = 0; k < 64; ++k) t += partial[(size_t)i * 64 + k];
+    f[i] += dv * t;
+}
+
+// spectrum of a chunk in work layout into d_work (forward (z,y), forward x)
+static int forward_spectrum(tdh_grid* g, int nst, const cd* in) {
+    int rc;
+    if ((rc = launch_plane_fwd(g, nst, in, g->d_work))) return rc;
+    return launch_xpencil(g, nst, g->d_work, g->d_work, 1);
+}
+// out = d_axis of the states whose spectrum is in d_work; uses d_phi[1] as the second spectrum buffer
+static int gradient_from_spectrum(tdh_grid* g, int nst, int axis, cd* out) {
+    const size_t total = (size_t)nst * g->np;
+    grad_scale_kernel<<<1184, 256, 0, g->stream>>>(g->d_work, g->d_phi[1], total, g->n[0], g->n[1], g->n[2], g->d_gs[axis], axis);
+    CU(cudaGetLastError());
+    g->launch_count += 1;
+    int rc;
+    if ((rc = launch_xpencil(g, nst, g->d_phi[1], g->d_phi[1], 2))) return rc;
+    tdh::Epilogue ep;
+    memset(&ep, 0, sizeof(ep));
+    ep.alpha = make_double2(1.0, 0.0);
+    ep.nx = g->n[0];
+    return launch_plane_inv(g, nst, g->d_phi[1], nullptr, out, ep);
+}
+
+extern "C" int tdh_gradient(tdh_grid* g, int nst, const tdh_c128* psi_dev, int axis, tdh_c128* out_dev) {
+    if (!g || !psi_dev || !out_dev) return fail(TDH_EINVAL, "tdh_gradient: null argument");
+    if (nst < 1 || nst > g->max_states) return fail(TDH_EINVAL, "tdh_gradient: nst = %d outside [1, %d]", nst, g->max_states);
+    if (axis < 0 || axis > 2) return fail(TDH_EINVAL, "tdh_gradient: axis must be 0, 1 or 2");
+    if (overlaps(psi_dev, out_dev, (size_t)nst * g->np * sizeof(cd))) return fail(TDH_EINVAL, "tdh_gradient: psi and out overlap");
+    stats_reset(g);
+    for (int s0 = 0; s0 < nst; s0 += g->chunk) {
+        const int c = std::min(g->chunk, nst - s0);
+        int rc;
+        if ((rc = forward_spectrum(g, c, (const cd*)psi_dev + (size_t)s0 * g->np))) return rc;
+        if ((rc = gradient_from_spectrum(g, c, axis, (cd*)out_dev + (size_t)s0 * g->np))) return rc;
+    }
+    return prof_collect(g);
+}
+
+extern "C" int tdh_forces(tdh_grid* g, int nst, const tdh_c128* psi_dev, const double* occ_host, const double* vloc_atoms_dev,
+                          double* forces_host) {
+    if (!g || !psi_dev || !forces_host) return fail(TDH_EINVAL, "tdh_forces: null argument");
+    if (nst < 1 || nst > g->max_states) return fail(TDH_EINVAL, "tdh_forces: nst = %d outside [1, %d]", nst, g->max_states);
+    if (g->natoms < 1) return fail(TDH_EINVAL, "tdh_forces: no atoms (tdh_set_projectors)");
+    stats_reset(g);
+    const double* occ = nullptr;
+    if (occ_host) {
+        CU(cudaMemcpyAsync(g->d_occ, occ_host, sizeof(double) * nst, cudaMemcpyHostToDevice, g->stream));
+        CU(cudaStreamSynchronize(g->stream));
+        occ = g->d_occ;
+    }
+    if (vloc_atoms_dev && !g->d_gd) CU(cudaMalloc(&g->d_gd, sizeof(double) * 3 * g->np));     // first use
+    const int n3 = 3 * g->natoms;
+    CU(cudaMemsetAsync(g->d_force, 0, sizeof(double) * n3, g->stream));
+    cd* grad = g->d_phi[0];
+    for (int s0 = 0; s0 < nst; s0 += g->chunk) {
+        const int c = std::min(g->chunk, nst - s0);
+        const cd* x = (const cd*)psi_dev + (size_t)s0 * g->np;
+        int rc;
+        if ((rc = launch_nl_project(g, c, x))) return rc;                               // D dV <beta|psi>
+        if ((rc = forward_spectrum(g, c, x))) return rc;
+        for (int a = 0; a < 3; ++a) {
+            if ((rc = gradient_from_spectrum(g, c, a, grad))) return rc;
+            if ((rc = launch_nl_project(g, c, grad, g->d_dvscale, g->d_dpig))) return rc;  // dV <beta|d_a psi>
+            force_nl_kernel<<<(g->natoms + 63) / 64, 64, 0, g->stream>>>(g->d_atoms, g->natoms, c, g->nchan_tot, g->d_dpig,
+                                                                          g->d_dpi, occ ? occ + s0 : nullptr, a, g->d_force);
+            CU(cudaGetLastError());
+            g->launch_count += 1;
+            if (vloc_atoms_dev) {
+                grad_density_kernel<<<(unsigned)((g->np + 255) / 256), 256, 0, g->stream>>>(
+                    grad, x, g->np, c, occ ? occ + s0 : nullptr, g->d_gd + (size_t)a * g->np, s0 > 0 ? 1 : 0);
+                CU(cudaGetLastError());
+                g->launch_count += 1;
+            }
+        }
+    }
+    if (vloc_atoms_dev) {
+        double* partial = g->d_force + n3;
+        force_loc_partial_kernel<<<dim3(64, n3), 256, 0, g->stream>>>(vloc_atoms_dev, g->d_gd, g->np, partial);
+        CU(cudaGetLastError());
+        force_loc_final_kernel<<<(n3 + 127) / 128, 128, 0, g->stream>>>(partial, n3, g->dv, g->d_force);
+        CU(cudaGetLastError());
+        g->launch_count += 2;
+    }
+    CU(cudaMemcpyAsync(forces_host, g->d_force, sizeof(double) * n3, cudaMemcpyDeviceToHost, g->stream));
+    CU(cudaStreamSynchronize(g->stream));
     return prof_collect(g);
 }
 

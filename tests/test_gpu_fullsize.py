@@ -503,3 +503,46 @@ def test_ground_state_iterations_converge_towards_the_lowest_eigenvalues(torch_c
     ev = np.sort(eigsh(op, k=4, which="SA", tol=1e-10, return_eigenvectors=False))
     assert np.all(hist[-1] >= ev - 1e-8)                           # variational bound (Cauchy interlacing)
     assert hist[-1, 0] - ev[0] < 0.05 * (hist[0, 0] - ev[0])       # and the iteration has closed most of the gap
+
+
+# ------------------------------------------------------------------------------------------------ NEXT-4: gradient, forces
+@pytest.mark.parametrize("name,nst", [("tiny", 8), ("small", 11), ("medium", 5)])
+def test_gradient_matches_oracle(torch_cuda, B, oracle, name, nst):
+    """tdh_gradient (i (G_a + k_a) in Fourier space) for the three axes, whole and split planes, k != 0."""
+    torch = torch_cuda
+    cfg = W.CONFIGS[name]
+    psi = W.states(cfg, 0, nst)
+    with B.Grid(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, nst) as g:
+        d = torch.from_numpy(psi).cuda()
+        for a in range(3):
+            ref = oracle.gradient(cfg.n, cfg.length, cfg.kpt, a, psi)
+            assert per_state_rel(g.gradient(d, a).cpu().numpy(), ref).max() < TOL
+    n = (16, 96, 96)
+    cfg2 = W.test_config(290, n, (5.0, 30.0, 30.0), nst=2, natoms=0)
+    psi = W.states(cfg2)
+    with B.Grid(cfg2.n, cfg2.length, cfg2.kpt, -1.0, 2) as g:
+        d = torch.from_numpy(psi).cuda()
+        for a in range(3):
+            assert per_state_rel(g.gradient(d, a).cpu().numpy(), oracle.gradient(cfg2.n, cfg2.length, cfg2.kpt, a, psi)).max() < TOL
+
+
+@pytest.mark.parametrize("name,nst,chunk", [("tiny", 8, None), ("small", 13, 4), ("medium", 6, None)])
+def test_forces_match_oracle(torch_cuda, B, oracle, name, nst, chunk):
+    """tdh_forces (Eq. 11) against the oracle: non-local part alone and with per-atom local potentials, occupations."""
+    torch = torch_cuda
+    cfg = W.CONFIGS[name]
+    wl = W.make(cfg)
+    psi = W.states(cfg, 0, nst)
+    rng = np.random.default_rng([W.BASE_SEED + cfg.cid, 14])
+    occ = rng.uniform(0.2, 2.0, nst)
+    import dataclasses
+    one = dataclasses.replace(cfg, natoms=1)
+    vloc = np.array([W.local_potential(one, wl.pos[i:i + 1]) for i in range(cfg.natoms)])
+    with B.grid_for(wl, max_states=nst) as g:
+        if chunk:
+            g.set_chunk_states(chunk)
+        d = torch.from_numpy(psi).cuda()
+        for o, v in ((None, None), (occ, vloc)):
+            ref = oracle.forces(cfg.n, cfg.length, cfg.kpt, wl.proj, psi, o, v)
+            got = g.forces(d, cfg.natoms, o, None if v is None else torch.from_numpy(v).cuda())
+            assert np.abs(got - ref).max() < 1e-10 * np.abs(ref).max(), (got, ref)
