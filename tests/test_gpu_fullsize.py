@@ -546,3 +546,31 @@ def test_forces_match_oracle(torch_cuda, B, oracle, name, nst, chunk):
             ref = oracle.forces(cfg.n, cfg.length, cfg.kpt, wl.proj, psi, o, v)
             got = g.forces(d, cfg.natoms, o, None if v is None else torch.from_numpy(v).cuda())
             assert np.abs(got - ref).max() < 1e-10 * np.abs(ref).max(), (got, ref)
+
+
+def test_new_entry_points_are_deterministic(torch_cuda, B):
+    """No atomics on any data path (split-K partials, coloured scatter, ordered reductions, grid barriers): two runs of every
+    NEXT entry point give bit-identical results."""
+    torch = torch_cuda
+    cfg = W.CONFIGS["small"]
+    wl = W.make(cfg)
+    nst = 24
+    psi = torch.from_numpy(W.states(cfg, 0, nst)).cuda()
+
+    def run():
+        with B.grid_for(wl, max_states=nst) as g:
+            q = g.orthonormalize(psi)
+            h = g.apply_hamiltonian(q)
+            w, r = g.subspace_diag(q, h)
+            d = q.clone()
+            eig = g.sd_step(d, 0.1)
+            f = g.forces(q, cfg.natoms)
+            n = g.density(q)
+            vh = g.hartree(n)
+            full = g.taylor_pair(d, 0.02)
+            return [q.cpu().numpy(), g.overlap(q, h).cpu().numpy(), w, r.cpu().numpy(), eig, d.cpu().numpy(), f,
+                    n.cpu().numpy(), vh.cpu().numpy(), full.cpu().numpy()]
+
+    a, b = run(), run()
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
