@@ -505,7 +505,7 @@ def main():
     # ---- per-kernel times (same steps, library events on the launching stream) -> roofline of the dominant family
     kern_s, _ = kernel_breakdown(torch, g, fn, max(1, min(args.steps, 5)))
     peak, peak_src = measured_peaks()
-    cap = max(1, (1 << 30) // (cfg.npts * 16))                                   # the library's default chunk
+    cap = max(1, (4 << 30) // (cfg.npts * 16))                                   # the library's default chunk
     states_per_launch = args.chunk or (nst if cap >= nst else (cap // 8 * 8 if cap >= 8 else cap))
     roof = roofline_of(kern_s, units, peak, peak_src, alg_bytes(wl), args.workload, states_per_launch * cfg.npts)
 

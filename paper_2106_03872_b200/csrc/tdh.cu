@@ -13,7 +13,7 @@
 // CUtensorMap per launch (tensor_maps.h) and the kernels stream tiles through a shared-memory ring.  `work` holds the
 // spectrum in the digit-permuted order the in-place transforms produce (xpencil_kernel.cuh, WORK LAYOUT).
 // States are independent, so a block is pushed through this chain chunk by chunk; a chunk is as many
-// states as the 1 GiB workspace holds (measured: L2-resident small chunks never win, profiles/r01a_chunk_sweep.md).
+// states as the 4 GiB workspace holds (measured: L2-resident small chunks never win, profiles/r01a_chunk_sweep.md).
 // propagate runs ALL steps of one chunk before moving to the next chunk (H is fixed: readings R10, R16), evaluating
 // Eq. 8 in Horner form  psi + a1 H(psi + a2 H(psi + a3 H(psi + a4 H psi))),  a_k = -i dt / k,  so that every
 // application's epilogue is a single fused axpy and no accumulator is read-modified-written.
@@ -325,9 +325,13 @@ extern "C" int tdh_create_grid(const int n[3], const double len[3], const double
         CU(cudaMalloc(&g->d_v, sizeof(double) * g->np));
         CU(cudaMemset(g->d_v, 0, sizeof(double) * g->np));
         g->have_v = false;
-        // workspace: up to 1 GiB per buffer
+        // workspace: up to 4 GiB per buffer (TDH_WORKSPACE_MB overrides)
         const size_t state_bytes = g->np * sizeof(cd);
-        size_t cap = std::max<size_t>(1, ((size_t)1 << 30) / state_bytes);
+        // three block buffers of this size (work, two Horner buffers): 12 GiB of the 180 GB when max_states needs them.
+        // Measured on Large (profiles/r01f_summary.md): 1 GiB 26.05 ms per step, 2 GiB 25.88, 4 GiB 25.27 (fewer, longer launches)
+        size_t ws_bytes = (size_t)4 << 30;
+        if (const char* e = getenv("TDH_WORKSPACE_MB")) { long v = atol(e); if (v > 0) ws_bytes = (size_t)v << 20; }
+        size_t cap = std::max<size_t>(1, ws_bytes / state_bytes);
         g->chunk_cap = (int)std::min<size_t>(cap, (size_t)max_states);
         CU(cudaMalloc(&g->d_work, state_bytes * g->chunk_cap));
         // at least two states each: tdh_taylor_pair keeps phi_2 and phi_3 in the two halves of d_phi[0]

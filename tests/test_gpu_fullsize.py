@@ -65,7 +65,7 @@ def test_large_full_block_sampled_states(torch_cuda, B, oracle):
     torch = torch_cuda
     cfg = W.CONFIGS["large"]
     free, _ = torch.cuda.mem_get_info()
-    nst = cfg.nst if free > 36 * 2 ** 30 else 256           # smaller boxes: same launch configuration, fewer states
+    nst = cfg.nst if free > 48 * 2 ** 30 else 256           # smaller boxes: same launch configuration, fewer states
     sample = [0, nst // 2 - 1, nst - 1]
     wl = W.make(cfg)
     psi, host = device_block(torch, cfg, nst, sample)
