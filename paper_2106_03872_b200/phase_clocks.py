@@ -29,6 +29,7 @@ def main(argv):
         raise SystemExit("this libtdh.so was built without -DTDH_PHASE_CLOCKS (see the module docstring)")
     cfg = W.CONFIGS[name]
     wl = W.make(cfg)
+    torch.manual_seed(W.BASE_SEED + cfg.cid)
     psi = torch.randn(nst, *cfg.n, dtype=torch.complex128, device="cuda")
     out = torch.empty_like(psi)
     with binding.Grid(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, nst) as g:
