@@ -574,3 +574,27 @@ def test_new_entry_points_are_deterministic(torch_cuda, B):
     a, b = run(), run()
     for x, y in zip(a, b):
         assert np.array_equal(x, y)
+
+
+def test_rotations_at_full_grid_size_sampled(torch_cuda, B, oracle):
+    """Large grid (96^3), 256 states: sampled entries of the overlap matrix against the oracle's literal sums, unit overlap
+    after tdh_orthonormalize, and sampled states of a rotation against the oracle."""
+    torch = torch_cuda
+    cfg = W.CONFIGS["large"]
+    nst = 256
+    sample = [0, 77, 255]
+    psi, host = device_block(torch, cfg, nst, sample)
+    with B.Grid(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, nst) as g:
+        s = g.overlap(psi).cpu().numpy()
+        ref = oracle.overlap(cfg.n, cfg.dv, host, host)
+        assert np.abs(s[np.ix_(sample, sample)] - ref).max() < 1e-12
+        q = g.orthonormalize(psi)
+        assert np.abs(g.overlap(q).cpu().numpy() - np.eye(nst)).max() < 1e-12
+        # a rotation that only mixes the sampled states into three output states
+        rng = np.random.default_rng(31)
+        m = np.zeros((nst, 3), dtype=np.complex128)
+        m[sample, :] = rng.standard_normal((3, 3)) + 1j * rng.standard_normal((3, 3))
+        r = g.rotate(psi, torch.from_numpy(m).cuda()).cpu().numpy()
+        assert per_state_rel(r, oracle.rotate(host, m[sample, :])).max() < 1e-13
+    del psi, q
+    torch.cuda.empty_cache()
