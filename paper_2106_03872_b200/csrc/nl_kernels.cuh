@@ -8,7 +8,9 @@
 // twice per k-step (real and imaginary parts of psi).  Fragment layout of m8n8k4 (PTX ISA): lane l holds A[l/4][l%4],
 // B[l%4][l/4] and C[l/4][2*(l%4) + {0,1}].  So lane l gathers ONE complex value psi_{s0 + l/4}[S[q0 + l%4]] per k-step
 // and that is both B fragments.  The partial sums of the warps are combined through shared memory in warp order:
-// deterministic, no atomics.  The second half of Eq. 9 (back-projection) is fused into tile_inv's epilogue.
+// deterministic, no atomics.  The second half of Eq. 9 (back-projection) is nl_scatter_kernel below, or, on whole-plane
+// tiles, the record lists inside tile_inv (tile_kernels.cuh).  The indices and projector values of the next block are
+// requested while the gathers of the current one are in flight.
 #pragma once
 #include "fft_codelets.cuh"
 
