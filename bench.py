@@ -136,9 +136,29 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def fp64_gemm_ceiling(torch, n=8192, reps=3):
+    """Measured FP64 ceiling of this GPU in the same run: cuBLAS DGEMM n^3 through torch.matmul (a measurement of the
+    hardware, not part of the product path).  Returns TFLOP/s."""
+    a = torch.randn(n, n, dtype=torch.float64, device="cuda")
+    b = torch.randn(n, n, dtype=torch.float64, device="cuda")
+    c = torch.matmul(a, b)
+    torch.cuda.synchronize()
+    best = float("inf")
+    for _ in range(reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        torch.matmul(a, b, out=c)
+        e1.record()
+        torch.cuda.synchronize()
+        best = min(best, e0.elapsed_time(e1) * 1e-3)
+    del a, b, c
+    return 2.0 * n ** 3 / best * 1e-12
+
+
 def fp64_tensor_peak():
-    """FP64 tensor-core peak for the contraction legs: no FP64 GEMM was measured on this pool, so it is the measured bf16
-    peak times the nominal FP64 / bf16 ratio of B200 (45 / 2250 dense TFLOP/s, blackwell_cuda_programming.md)."""
+    """FP64 tensor-core peak for the contraction legs: no FP64 GEMM is in MEASURED_PEAKS.json, so it is the measured bf16
+    peak times the nominal FP64 / bf16 ratio of B200 (45 / 2250 dense TFLOP/s, blackwell_cuda_programming.md); the cuBLAS
+    DGEMM rate measured in the same run is reported beside it (fp64_gemm_ceiling)."""
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     ratio = 45.0 / 2250.0
     if os.path.exists(path):
@@ -362,6 +382,15 @@ def sweep_leg(torch, B, name, flush, reps=7):
         hot = statistics.median(timed_each(torch, fn, reps, None))
         res = {"states": cfg.nst, "grid": cfg.n[0], "value": units / cold, "ms": cold * 1e3,
                "value_l2_hot": units / hot, "ms_l2_hot": hot * 1e3, "launches": g.last_launch_count()}
+        if name in ("tiny", "small"):
+            # launch-latency regime: 100 back-to-back calls, one pair of events around the loop
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(100):
+                fn()
+            e1.record()
+            torch.cuda.synchronize()
+            res["ms_per_call_in_a_100_call_loop"] = e0.elapsed_time(e1) / 100
         if name == "tddft":
             # row a7: the config's 20 Taylor-4 steps (80 H applications + fused axpys) in one tdh_propagate call
             work = psi.clone()
@@ -418,10 +447,13 @@ def sweep_leg(torch, B, name, flush, reps=7):
             to = statistics.median(timed_each(torch, lambda: g.overlap(psi, out, out=smat), 5, flush))
             tg = statistics.median(timed_each(torch, lambda: g.overlap(psi, out=smat), 5, flush))
             peak_tf, peak_src = fp64_tensor_peak()
+            dgemm_tf = fp64_gemm_ceiling(torch)
             tf = 8.0 * cfg.nst * cfg.nst * cfg.npts / to * 1e-12
             res["overlap"] = {"seconds": to, "bound": "tensor", "achieved": round(tf, 2), "peak": round(peak_tf, 2),
                               "unit": "TFLOP/s", "frac": round(tf / peak_tf, 4), "peak_source": peak_src,
                               "flops": "8 * nst^2 * N_p (complex128 GEMM, K = N_p)", "gram_seconds": tg,
+                              "cublas_dgemm_8192_tflops_same_run": round(dgemm_tf, 2),
+                              "frac_of_cublas_dgemm": round(tf / dgemm_tf, 4),
                               "note": "tdh_overlap of two blocks: mma.sync.m8n8k4.f64, 64x64 tiles, split-K with ordered reduction; "
                                       "gram_seconds: one block with itself (tiles below the diagonal mirrored)"}
             work.copy_(psi)
