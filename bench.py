@@ -291,7 +291,16 @@ def alg_bytes(wl):
     return b
 
 
-def roofline_of(kern_s, units, peak_gbs, peak_src, bytes_per_unit, workload=None, units_per_launch=None):
+def nl_flops_per_unit(wl):
+    """Useful flop per state*gridpoint of each projector kernel: 8 * sum_I C_I P_I / N_p (real matrix x complex block)."""
+    pr = wl.proj
+    if not pr.natoms:
+        return 0.0
+    cp = sum(int(pr.chan_off[i + 1] - pr.chan_off[i]) * int(pr.sph_off[i + 1] - pr.sph_off[i]) for i in range(pr.natoms))
+    return 8.0 * cp / wl.cfg.npts
+
+
+def roofline_of(kern_s, units, peak_gbs, peak_src, bytes_per_unit, workload=None, units_per_launch=None, nl_flops=0.0):
     """Roofline object for the dominant kernel family (largest share of the step) + the fractions of the others."""
     cand = {k: v for k, v in kern_s.items() if bytes_per_unit.get(k) and v > 0}
     if not cand:
@@ -302,6 +311,10 @@ def roofline_of(kern_s, units, peak_gbs, peak_src, bytes_per_unit, workload=None
                   "frac": round(bytes_per_unit[k] * units / v * 1e-9 / peak_gbs, 4),
                   "algorithmic_bytes_per_unit": round(bytes_per_unit[k], 3),
                   "share_of_step": round(v / sum(kern_s.values()), 4)} for k, v in cand.items()}
+    for k in ("nl_project", "nl_scatter"):
+        if k in others and nl_flops > 0:
+            # the contraction is byte bound: its useful FP64 rate is reported, the bytes govern
+            others[k]["useful_tflops"] = round(nl_flops * units / cand[k] * 1e-12, 2)
     traffic = None
     per_unit = NCU_DRAM_BYTES_PER_UNIT.get(workload, {}).get(top)
     if per_unit and units_per_launch:
@@ -539,7 +552,8 @@ def main():
     peak, peak_src = measured_peaks()
     cap = max(1, (4 << 30) // (cfg.npts * 16))                                   # the library's default chunk
     states_per_launch = args.chunk or (nst if cap >= nst else (cap // 8 * 8 if cap >= 8 else cap))
-    roof = roofline_of(kern_s, units, peak, peak_src, alg_bytes(wl), args.workload, states_per_launch * cfg.npts)
+    roof = roofline_of(kern_s, units, peak, peak_src, alg_bytes(wl), args.workload, states_per_launch * cfg.npts,
+                       nl_flops_per_unit(wl))
 
     # ---- end to end through the host-buffer entry point (pinned host in/out, copies inside the timed region)
     e2e = None
