@@ -598,3 +598,39 @@ def test_rotations_at_full_grid_size_sampled(torch_cuda, B, oracle):
         assert per_state_rel(r, oracle.rotate(host, m[sample, :])).max() < 1e-13
     del psi, q
     torch.cuda.empty_cache()
+
+
+def test_seeded_sweep_over_grid_shapes_and_options(torch_cuda, B, oracle, monkeypatch):
+    """Sixteen seeded combinations of grid shape (every supported size on every axis), state count, atoms, channel set,
+    Bloch vector, cutoff, chunking and back-projection path: apply and two Taylor steps against the oracle."""
+    torch = torch_cuda
+    rng = np.random.default_rng(20260501)
+    sizes = [16, 32, 48, 64, 96]
+    done = 0
+    while done < 16:
+        n = tuple(int(rng.choice(sizes)) for _ in range(3))
+        if n[0] * n[1] * n[2] > 64 * 64 * 64:
+            continue
+        h = rng.uniform(0.3, 0.5)
+        length = tuple(float(h * m * rng.uniform(0.9, 1.1)) for m in n)
+        nst = int(rng.integers(1, 10))
+        natoms = int(rng.integers(0, 5))
+        lmax = int(rng.integers(0, 3))
+        kw = dict(nst=nst, natoms=natoms, lmax=lmax, rc=float(min(2.6, 0.45 * min(length))), dl=(2.0, -0.8, 0.3)[: lmax + 1],
+                  kfrac=tuple(float(rng.choice([0.0, 0.0, 0.25, -0.1])) for _ in range(3)))
+        if rng.random() < 0.4:
+            kw["ecut"] = float(rng.choice([15.0, 40.0]))
+        cfg = W.test_config(500 + done, n, length, **kw)
+        wl = W.make(cfg)
+        psi = W.states(cfg)
+        ref_h = oracle.apply_workload(wl, psi, oracle.NAIVE_FFT)
+        ref_p = oracle.propagate_workload(wl, psi, dt=0.01, nsteps=2)
+        monkeypatch.setenv("TDH_NL_MODE", str(done % 2))
+        with B.grid_for(wl) as g:
+            if rng.random() < 0.5:
+                g.set_chunk_states(int(rng.integers(1, nst + 1)))
+            d = torch.from_numpy(psi).cuda()
+            assert per_state_rel(g.apply_hamiltonian(d).cpu().numpy(), ref_h).max() < TOL, (done, n, kw)
+            g.propagate(d, 0.01, 2)
+            assert per_state_rel(d.cpu().numpy(), ref_p).max() < TOL, (done, n, kw)
+        done += 1
