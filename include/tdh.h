@@ -203,8 +203,9 @@ int tdh_set_profiling(tdh_grid* g, int on);
 int tdh_last_kernel_seconds(const tdh_grid* g, double out[TDH_NKERNELS]);
 const char* tdh_kernel_name(int i);
 
-/* Tuning knob: how many states are pushed through the kernel chain together (0 = library default, chosen so that
- * the inter-kernel workspace stays resident in the 126 MB L2). */
+/* Tuning knob: how many states are pushed through the kernel chain together (0 = library default: as many as the
+ * handle's workspace of at most 4 GiB per buffer holds, a multiple of 8 when a block has to be split -- measured on
+ * B200, longer launches are never slower than L2-resident small chunks). */
 int tdh_set_chunk_states(tdh_grid* g, int chunk);
 
 const char* tdh_last_error(void);                 /* thread-local, static storage; never NULL */

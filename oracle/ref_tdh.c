@@ -632,7 +632,9 @@ int ref_sd_step(const int n[3], const double len[3], const double kpt[3], double
                         for (int k = 0; k < n[2]; ++k) {
                             const double gz = two_pi * freq_index(k, n[2]) / len[2] + kpt[2];
                             const double tk = 0.5 * ((gx * gx + gy * gy) + gz * gz);
-                            h[((size_t)i * n[1] + j) * n[2] + k] *= teter(tk / ts);
+                            /* T_s <= 0 (a constant state at Gamma, up to rounding): x = t / T_s is undefined; reading
+                             * R19 takes the limit x -> infinity: K = 1 at t = 0, K = 0 elsewhere */
+                            h[((size_t)i * n[1] + j) * n[2] + k] *= ts > 0.0 ? teter(tk / ts) : (tk == 0.0 ? 1.0 : 0.0);
                         }
                     }
                 }

@@ -115,6 +115,7 @@ class Grid:
         self.n = tuple(int(x) for x in n)
         self.npts = self.n[0] * self.n[1] * self.n[2]
         self.max_states = int(max_states)
+        self.natoms = 0
         self._h = C.c_void_p()
         _check(l.tdh_create_grid((C.c_int * 3)(*self.n), (C.c_double * 3)(*[float(x) for x in length]),
                                  (C.c_double * 3)(*[float(x) for x in kpt]), float(ecut), int(max_states),
@@ -151,6 +152,7 @@ class Grid:
         """proj: workloads.Projectors-like object with host numpy tables, or None to clear."""
         if proj is None or proj.natoms == 0:
             _check(lib().tdh_set_projectors(self._h, 0, None, None, None, None, None, None))
+            self.natoms = 0
             return
         sph_off = np.ascontiguousarray(proj.sph_off, dtype=np.int64)
         sph_idx = np.ascontiguousarray(proj.sph_idx, dtype=np.int32)
@@ -161,6 +163,8 @@ class Grid:
         p = lambda a: None if a is None else C.c_void_p(a.ctypes.data)
         _check(lib().tdh_set_projectors(self._h, int(proj.natoms), p(sph_off), p(sph_idx), p(sph_disp), p(chan_off),
                                         p(beta), p(dcoef)))
+        # the handle's atom count sizes the result of tdh_forces; a table without any channel clears the projectors
+        self.natoms = int(proj.natoms) if int(chan_off[-1]) > 0 else 0
 
     # -- device entry points
     def _block(self, psi):
@@ -275,10 +279,15 @@ class Grid:
         _check(lib().tdh_gradient(self._h, nst, C.c_void_p(psi.data_ptr()), int(axis), C.c_void_p(out.data_ptr())))
         return out
 
-    def forces(self, psi, natoms: int, occ=None, vloc_atoms=None):
-        """Eq. 11 per atom and axis -> (natoms, 3) host numpy; vloc_atoms: device float64 (natoms, n0, n1, n2) or None."""
+    def forces(self, psi, natoms: Optional[int] = None, occ=None, vloc_atoms=None):
+        """Eq. 11 per atom and axis -> (natoms, 3) host numpy; vloc_atoms: device float64 (natoms, n0, n1, n2) or None.
+        natoms is the atom count of the installed projector table (checked when given: it sizes the result buffer)."""
         import torch
         nst = self._block(psi)
+        if natoms is None:
+            natoms = self.natoms
+        if natoms != self.natoms:
+            raise TdhError(TDH_EINVAL, f"forces: natoms = {natoms} but the installed projector table has {self.natoms} atoms")
         occ_arr = None if occ is None else np.ascontiguousarray(occ, dtype=np.float64)
         assert occ_arr is None or occ_arr.size == nst
         if vloc_atoms is not None:

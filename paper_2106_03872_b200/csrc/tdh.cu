@@ -390,9 +390,13 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
                                   const double* dcoef) {
     if (!g) return fail(TDH_EINVAL, "tdh_set_projectors: null handle");
     if (natoms < 0) return fail(TDH_EINVAL, "tdh_set_projectors: natoms < 0");
-    CU(cudaStreamSynchronize(g->stream));
-    free_projectors(g);
-    if (natoms == 0) return TDH_OK;
+    if (natoms == 0) {
+        CU(cudaStreamSynchronize(g->stream));
+        free_projectors(g);
+        return TDH_OK;
+    }
+    // The new tables are validated and built first (host vectors, then device arrays of the staging handle `nw`); the
+    // installed ones are replaced only when everything succeeded, so a rejected table leaves the handle as it was.
     if (natoms > 65535) return fail(TDH_EUNSUPPORTED, "tdh_set_projectors: more than 65535 atoms");
     if (!sph_off || !sph_idx || !chan_off || !beta || !dcoef)
         return fail(TDH_EINVAL, "tdh_set_projectors: null table with natoms > 0");
@@ -403,6 +407,11 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
             return fail(TDH_EINVAL, "tdh_set_projectors: offsets must be non-decreasing");
     const int64_t ptot = sph_off[natoms];
     const int ctot = chan_off[natoms];
+    if (ctot == 0) {                       // atoms without any channel: V_nl = 0, the same as no projectors
+        CU(cudaStreamSynchronize(g->stream));
+        free_projectors(g);
+        return TDH_OK;
+    }
     if (ptot >= (int64_t)1 << 30) return fail(TDH_EUNSUPPORTED, "tdh_set_projectors: too many sphere points");
 
     // ---- validate, sort each sphere by flat grid index (coalesced gathers), re-index beta, build phases
@@ -543,25 +552,34 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
         return TDH_OK;
     };
     int rc;
-    if ((rc = up(&g->d_atoms_col, atoms_col)) || (rc = up(&g->d_atoms, atoms)) || (rc = up(&g->d_sidx, sidx)) || (rc = up(&g->d_sbeta, sbeta)) ||
-        (rc = up(&g->d_sphase, sphase)) || (rc = up(&g->d_dscale, dscale)) || (rc = up(&g->d_nl_off, nl_off)) ||
-        (rc = up(&g->d_nl_cc, rec_cc)) || (rc = up(&g->d_nl_beta, rec_beta)) || (rc = up(&g->d_nl_phase, rec_phase))) {
-        free_projectors(g);
+    tdh_grid stage{};                                      // only its projector fields are used
+    tdh_grid* nw = &stage;
+    if ((rc = up(&nw->d_atoms_col, atoms_col)) || (rc = up(&nw->d_atoms, atoms)) || (rc = up(&nw->d_sidx, sidx)) || (rc = up(&nw->d_sbeta, sbeta)) ||
+        (rc = up(&nw->d_sphase, sphase)) || (rc = up(&nw->d_dscale, dscale)) || (rc = up(&nw->d_nl_off, nl_off)) ||
+        (rc = up(&nw->d_nl_cc, rec_cc)) || (rc = up(&nw->d_nl_beta, rec_beta)) || (rc = up(&nw->d_nl_phase, rec_phase))) {
+        free_projectors(nw);
         return rc;
     }
     // dpi: [chunk_cap][ctot] plus cpad zeroed entries (records of atoms with fewer than cpad channels read past their
     // own channels with a zero projector value)
     const size_t ndpi = (size_t)g->chunk_cap * ctot + cpad;
-    cudaError_t e = cudaMalloc(&g->d_dpi, sizeof(cd) * ndpi);
-    if (e == cudaSuccess) e = cudaMemset(g->d_dpi, 0, sizeof(cd) * ndpi);
-    if (e != cudaSuccess) { free_projectors(g); return fail(TDH_ENOMEM, "tdh_set_projectors: %s", cudaGetErrorString(e)); }
+    cudaError_t e = cudaMalloc(&nw->d_dpi, sizeof(cd) * ndpi);
+    if (e == cudaSuccess) e = cudaMemset(nw->d_dpi, 0, sizeof(cd) * ndpi);
+    if (e != cudaSuccess) { free_projectors(nw); return fail(TDH_ENOMEM, "tdh_set_projectors: %s", cudaGetErrorString(e)); }
     {
         std::vector<double> dvs(ctot, g->dv);
-        if ((rc = up(&g->d_dvscale, dvs))) { free_projectors(g); return rc; }
-        e = cudaMalloc(&g->d_dpig, sizeof(cd) * (size_t)g->chunk_cap * ctot);
-        if (e == cudaSuccess) e = cudaMalloc(&g->d_force, sizeof(double) * (size_t)natoms * 3 * (1 + 64));
-        if (e != cudaSuccess) { free_projectors(g); return fail(TDH_ENOMEM, "tdh_set_projectors: %s", cudaGetErrorString(e)); }
+        if ((rc = up(&nw->d_dvscale, dvs))) { free_projectors(nw); return rc; }
+        e = cudaMalloc(&nw->d_dpig, sizeof(cd) * (size_t)g->chunk_cap * ctot);
+        if (e == cudaSuccess) e = cudaMalloc(&nw->d_force, sizeof(double) * (size_t)natoms * 3 * (1 + 64));
+        if (e != cudaSuccess) { free_projectors(nw); return fail(TDH_ENOMEM, "tdh_set_projectors: %s", cudaGetErrorString(e)); }
     }
+    // success: replace the installed tables
+    if (cudaStreamSynchronize(g->stream) != cudaSuccess) { free_projectors(nw); return fail(TDH_ECUDA, "tdh_set_projectors: stream synchronisation failed"); }
+    free_projectors(g);
+    g->d_atoms_col = nw->d_atoms_col; g->d_atoms = nw->d_atoms; g->d_sidx = nw->d_sidx; g->d_sbeta = nw->d_sbeta;
+    g->d_sphase = nw->d_sphase; g->d_dscale = nw->d_dscale; g->d_nl_off = nw->d_nl_off; g->d_nl_cc = nw->d_nl_cc;
+    g->d_nl_beta = nw->d_nl_beta; g->d_nl_phase = nw->d_nl_phase; g->d_dpi = nw->d_dpi; g->d_dvscale = nw->d_dvscale;
+    g->d_dpig = nw->d_dpig; g->d_force = nw->d_force;
     g->natoms = natoms;
     g->nchan_tot = ctot;
     g->nl_layers = nlayers;
@@ -667,23 +685,6 @@ static int launch_xpencil(tdh_grid* g, int nst, const cd* in, cd* out, int mode,
     return TDH_OK;
 }
 
-#ifdef TDH_PHASE_CLOCKS
-// debug builds only (not part of include/tdh.h): clock ticks per phase of tile_inv, summed over warp groups; reading
-// resets them
-static unsigned long long* g_ticks = nullptr;
-static unsigned long long* phase_ticks_buffer() {
-    if (!g_ticks && cudaMalloc(&g_ticks, 16 * sizeof(unsigned long long)) == cudaSuccess)
-        cudaMemset(g_ticks, 0, 16 * sizeof(unsigned long long));
-    return g_ticks;
-}
-extern "C" int tdh_debug_phase_ticks(unsigned long long out[16]) {
-    if (!phase_ticks_buffer() || cudaDeviceSynchronize() != cudaSuccess) return TDH_ECUDA;
-    if (cudaMemcpy(out, g_ticks, 16 * sizeof(unsigned long long), cudaMemcpyDeviceToHost) != cudaSuccess) return TDH_ECUDA;
-    if (cudaMemset(g_ticks, 0, 16 * sizeof(unsigned long long)) != cudaSuccess) return TDH_ECUDA;
-    return TDH_OK;
-}
-#endif
-
 // in: work block (spectrum), phi: input block of this application (read only when the epilogue has V or projectors)
 static int launch_plane_inv(tdh_grid* g, int nst, const cd* in, const cd* phi, cd* out, const tdh::Epilogue& ep) {
     CUtensorMap map_spec, map_phi;
@@ -697,9 +698,6 @@ static int launch_plane_inv(tdh_grid* g, int nst, const cd* in, const cd* phi, c
     int ntiles = (int)((size_t)nst * g->n[0] * g->tl.s / g->tl.ppc);
     tdh::Epilogue epl = ep;
     epl.phi = phi;
-#ifdef TDH_PHASE_CLOCKS
-    epl.ticks = phase_ticks_buffer();
-#endif
     void* args[] = {(void*)&map_spec, (void*)&map_phi, (void*)&map_yv, (void*)&out, (void*)&ntiles, (void*)&twy, (void*)&twz, (void*)&epl};
     const int cmi = tdh::nl_cm_index(epl.nl_off != nullptr ? epl.cmax : 0);
     const unsigned grid = (unsigned)std::min(ntiles, g->ctas_inv[cmi]);
@@ -756,6 +754,7 @@ static int launch_nl_scatter(tdh_grid* g, int nst, cd* out, cd alpha) {
     int nct = g->nchan_tot;
     const void* fs[4] = {reinterpret_cast<const void*>(&tdh::nl_scatter_kernel<1>), reinterpret_cast<const void*>(&tdh::nl_scatter_kernel<2>),
                          reinterpret_cast<const void*>(&tdh::nl_scatter_kernel<3>), reinterpret_cast<const void*>(&tdh::nl_scatter_kernel<4>)};
+    if (g->kt < 1) return TDH_OK;                          // no channel anywhere: nothing to add
     for (size_t c = 0; c + 1 < g->col_off.size(); ++c) {
         const tdh::AtomDesc* atoms = g->d_atoms_col + g->col_off[c];
         void* args[] = {(void*)&out, (void*)&npts, (void*)&nst, (void*)&atoms, (void*)&sidx, (void*)&sbeta,
@@ -1353,8 +1352,12 @@ extern "C" int tdh_rotate(tdh_grid* g, int n_in, const tdh_c128* psi_dev, int n_
                           tdh_c128* out_dev) {
     if (!g || !psi_dev || !m_dev || !out_dev) return fail(TDH_EINVAL, "tdh_rotate: null argument");
     if (n_in < 1 || n_out < 1 || n_out > 65535 * tdh::RT_J) return fail(TDH_EINVAL, "tdh_rotate: bad n_in / n_out");
-    if (overlaps(psi_dev, out_dev, (size_t)std::min(n_in, n_out) * g->np * sizeof(cd)))
-        return fail(TDH_EINVAL, "tdh_rotate: psi and out overlap");
+    {
+        const char* x = (const char*)psi_dev;
+        const char* y = (const char*)out_dev;
+        const size_t bx = (size_t)n_in * g->np * sizeof(cd), by = (size_t)n_out * g->np * sizeof(cd);
+        if (x < y + by && y < x + bx) return fail(TDH_EINVAL, "tdh_rotate: psi and out overlap");
+    }
     stats_reset(g);
     return launch_rotate(g, n_in, (const cd*)psi_dev, n_out, (const cd*)m_dev, (cd*)out_dev, 0);
 }

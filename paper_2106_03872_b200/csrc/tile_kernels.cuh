@@ -236,9 +236,6 @@ struct Epilogue {
     int nrec;
     int cmax;               // padded channel count of a record: 1, 4, 9 or 16 (nl_pad_cmax) = the kernel's CM
     int nchan_tot;
-#ifdef TDH_PHASE_CLOCKS
-    unsigned long long* ticks;   // [16] phase timers (debug builds)
-#endif
 };
 
 // channel counts the record loop is compiled for; the host pads nl_beta (zeros) and dpi (zeros) to this
@@ -289,23 +286,6 @@ __device__ __forceinline__ void nl_scatter_layer(cd* base, const cd* __restrict_
         }
     }
 }
-
-// Optional phase timing of tile_inv (build with -DTDH_PHASE_CLOCKS): thread 0 of every warp group accumulates the
-// clock64() ticks between the marks below into ep.ticks[16], read back by tdh_debug_phase_ticks (tdh.cu).
-#ifdef TDH_PHASE_CLOCKS
-#define TDH_MARK(k)                                                                     \
-    do {                                                                                \
-        if (tid == 0) {                                                                 \
-            const long long now_ = clock64();                                           \
-            atomicAdd(ep.ticks + (k), (unsigned long long)(now_ - mark_t_));            \
-            mark_t_ = now_;                                                             \
-        }                                                                               \
-    } while (0)
-#define TDH_MARK_INIT long long mark_t_ = clock64()
-#else
-#define TDH_MARK(k) do {} while (0)
-#define TDH_MARK_INIT do {} while (0)
-#endif
 
 // ------------------------------------------------------------------------------------------------------------
 // inverse + epilogue: `map_spec` describes the work block (digit-permuted spectrum), `out` the output block; `map_phi`
@@ -363,8 +343,6 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
     };
     if (threadIdx.x == 0)
         for (int k = 0; k < NB; ++k) issue(k);
-
-    TDH_MARK_INIT;
     for (int k = grp;; k += 2) {
         const int t = blockIdx.x + k * gridDim.x;
         if (t >= ntiles) break;
@@ -377,7 +355,6 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
             if (ep.yv != nullptr) tma_prefetch_l2_4d(&map_yv, 0, (part0 % S) * R1Z, 0, part0 / S);
         }
         mbar_wait(full + b, (uint32_t)(k / NB) & 1u);
-        TDH_MARK(0);
 
         // ---- y stage A', in place: rows k1y*R2Y + k2y (contiguous) hold k = k1y + R1Y*k2y; radix R2Y over k2y -> j2,
         //      twiddle w^(-j2*k1y)
@@ -394,7 +371,6 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
             for (int j2 = 1; j2 < R2Y; ++j2) sm[swz((row0 + j2) * R1Z + k1, k2)] = cmul(v[j2], stw_y[S * j2 * k1y]);
         }
         group_sync<TG>(grp);
-        TDH_MARK(1);
         // ---- y stage B', in place: rows k1y*R2Y + j2, radix R1Y over k1y -> j1: row j1*R2Y + j2 = m, y = S*m + r
         for (int item = tid; item < C::I_YA; item += TG) {
             const int c = item % NZ, rr = item / NZ, j2 = rr % R2Y, lp = rr / R2Y;
@@ -408,7 +384,6 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
             for (int j1 = 0; j1 < R1Y; ++j1) sm[swz((row0 + j1 * R2Y) * R1Z + k1, k2)] = x[j1];
         }
         group_sync<TG>(grp);
-        TDH_MARK(2);
         // ---- z stage A', in place inside line g = (row, k1): positions k2 hold kz = k1 + R1Z*k2; radix 8 -> j2
         for (int g = tid; g < C::I_ZB; g += TG) {
             cd* p = sm + 8 * g;
@@ -421,7 +396,6 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
             for (int j2 = 0; j2 < 8; ++j2) p[j2 ^ s] = v[j2];
         }
         group_sync<TG>(grp);
-        TDH_MARK(3);
         const int j2 = tid & 7;
         if (HAVE_NL) {
             // ---- z stage B', in place: thread (row lr, j2): twiddle w^(-k1*j2), radix R1Z over k1 -> cell (lr, 8*j1 + j2)
@@ -436,7 +410,6 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
                 for (int j1 = 0; j1 < R1Z; ++j1) sm[swz(l0 + j1, j2)] = x[j1];
             }
             group_sync<TG>(grp);
-            TDH_MARK(4);
             // ---- back-projection: the tile now holds T phi in natural order; add V_nl phi layer by layer
             const int st = (part0 / S) / ep.nx;                           // PPC divides NX: one state per tile
             const cd* dp = ep.dpi + (size_t)st * ep.nchan_tot;
@@ -451,7 +424,6 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
                 }
                 group_sync<TG>(grp);
             }
-            TDH_MARK(5);
         }
         // ---- epilogue, thread (row lr, j2), cells z = 8*j1 + j2:  out = alpha * (T phi [+ V_nl phi] + V phi) + y.
         //      phi, V and y come straight from global memory (their tiles were started towards L2 above); all their
@@ -500,12 +472,10 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
                 for (int j1 = 0; j1 < R1Z; ++j1) sts_cd(out + gi + 8 * j1, cmul(ep.alpha, x[j1]));
             }
         }
-        TDH_MARK(6);
         // every read of this buffer is done: hand it back to the TMA
         fence_proxy_async();
         group_sync<TG>(grp);
         if (tid == 0) issue(k + NB);
-        TDH_MARK(7);
     }
 }
 

@@ -88,6 +88,8 @@ __device__ __forceinline__ double poisson_factor(double gx2, double gy2, double 
 // the Teter-Payne-Allan preconditioner K(x), x = t / T_s (reading R19), times 1/N_p
 __device__ __forceinline__ double teter_factor(double gx2, double gy2, double gz2, double ts, double scale) {
     const double tk = __dmul_rn(0.5, __dadd_rn(__dadd_rn(gx2, gy2), gz2));
+    // T_s <= 0 (a constant state at Gamma, up to rounding): the limit x -> infinity, K = 1 at t = 0 and 0 elsewhere (R19)
+    if (!(ts > 0.0)) return tk == 0.0 ? scale : 0.0;
     const double x = tk / ts;
     const double num = 27.0 + x * (18.0 + x * (12.0 + x * 8.0));
     const double x2 = x * x;

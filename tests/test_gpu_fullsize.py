@@ -60,26 +60,93 @@ def device_block(torch, cfg, nst, sample):
     return psi, host
 
 
-def test_large_full_block_sampled_states(torch_cuda, B, oracle):
-    """Config 4 (96^3, 1024 states, 128 atoms): one tdh_apply_hamiltonian call on the whole block, as bench.py times it."""
+def default_chunks(cfg, nst):
+    """State ranges of the launches tdh_apply_hamiltonian makes by default (as many states as a
+    4 GiB work buffer holds, a multiple of 8 when the block is split)."""
+    cap = min(nst, (4 << 30) // (cfg.npts * 16))
+    c = cap // 8 * 8 if (cap < nst and cap >= 8) else cap
+    return [(s0, min(nst, s0 + c)) for s0 in range(0, nst, c)]
+
+
+def test_large_full_block_every_chunk_and_sub_blocks(torch_cuda, B, oracle):
+    """Config 4 (96^3, 1024 states, 128 atoms): one tdh_apply_hamiltonian call on the whole block, as bench.py times it.
+    The first and the last state of EVERY default chunk (296 + 296 + 296 + 136 states) are compared with the oracle, the
+    whole output is finite, and the sub-blocks of bench.py's 32 / 128 / 512 sweep give bitwise the whole-block result."""
     torch = torch_cuda
     cfg = W.CONFIGS["large"]
     free, _ = torch.cuda.mem_get_info()
-    nst = cfg.nst if free > 48 * 2 ** 30 else 256           # smaller boxes: same launch configuration, fewer states
-    sample = [0, nst // 2 - 1, nst - 1]
+    nst = cfg.nst if free > 48 * 2 ** 30 else 320           # smaller boxes: same launch configuration, fewer states
+    chunks = default_chunks(cfg, nst)
+    assert len(chunks) >= 2
+    sample = sorted({s for a, b in chunks for s in (a, b - 1)})
     wl = W.make(cfg)
     psi, host = device_block(torch, cfg, nst, sample)
     with B.grid_for(wl, max_states=nst) as g:
         out = g.apply_hamiltonian(psi)
         torch.cuda.synchronize()
+        assert g.last_launch_count() == len(chunks) * (4 + 2)        # nl_project, 3 FFT kernels, nl_scatter x 2 colours
         got = np.stack([out[s].cpu().numpy() for s in sample])
-        # the block around the sampled states was processed too: no state is left unwritten or non-finite
-        assert bool(torch.isfinite(torch.view_as_real(out[nst // 3])).all())
-    ref = oracle.apply_workload(wl, host, oracle.NAIVE_FFT)
+        for a in range(0, nst, 64):                                     # no state is left unwritten or non-finite
+            assert bool(torch.isfinite(torch.view_as_real(out[a:a + 64])).all())
+        ref = oracle.apply_workload(wl, host, oracle.NAIVE_FFT)
+        err = per_state_rel(got, ref)
+        assert err.max() < TOL, err
+        # bench.py's block-size sweep (PAPER.md:456): a sub-block call gives bitwise the states of the whole-block call
+        sub = torch.empty_like(psi[:min(512, nst // 2)])
+        for b, s0 in ((32, nst // 2 + 96), (128, nst // 2), (min(512, nst // 2), nst // 2)):
+            g.apply_hamiltonian(psi[s0:s0 + b], out=sub[:b])
+            torch.cuda.synchronize()
+            assert torch.equal(sub[:b], out[s0:s0 + b]), (b, s0)
+    del psi, out, sub
+    torch.cuda.empty_cache()
+
+
+def test_large_propagate_default_chunking_sampled(torch_cuda, B, oracle):
+    """north_star: propagate on config 4.  Two Taylor-4 steps of the whole 1024-state block in place with the default
+    chunking (split tiles, coloured nl_scatter inside the Horner chain, the addend aliasing the output in the last
+    application); one state of every chunk against ref_propagate."""
+    torch = torch_cuda
+    cfg = W.CONFIGS["large"]
+    free, _ = torch.cuda.mem_get_info()
+    nst = cfg.nst if free > 48 * 2 ** 30 else 320
+    chunks = default_chunks(cfg, nst)
+    sample = sorted({(a + b) // 2 for a, b in chunks} | {0, nst - 1})
+    wl = W.make(cfg)
+    psi, host = device_block(torch, cfg, nst, sample)
+    nsteps, dt = 2, cfg.dt
+    with B.grid_for(wl, max_states=nst) as g:
+        g.propagate(psi, dt, nsteps)
+        torch.cuda.synchronize()
+        assert g.last_launch_count() == len(chunks) * nsteps * 4 * 6
+        got = np.stack([psi[s].cpu().numpy() for s in sample])
+    ref = oracle.propagate_workload(wl, host, dt=dt, nsteps=nsteps, backend=oracle.NAIVE_FFT)
     err = per_state_rel(got, ref)
     assert err.max() < TOL, err
-    del psi, out
+    del psi
     torch.cuda.empty_cache()
+
+
+def test_medium_full_block_apply_and_propagate(torch_cuda, B, oracle):
+    """north_star: config 3 (48^3, 256 states, k = (0.25,0,0) 2pi/L, 30 Ha mask, 9 channels per atom) on its FULL block:
+    apply compared for all 256 states, then three Taylor-4 steps of the resident block against ref_propagate on sampled
+    states."""
+    torch = torch_cuda
+    cfg = W.CONFIGS["medium"]
+    wl = W.make(cfg)
+    psi = W.states(cfg)
+    assert psi.shape[0] == 256
+    ref = oracle.apply_workload(wl, psi, oracle.NAIVE_FFT)
+    sample = [0, 1, 100, 254, 255]
+    ref_p = oracle.propagate_workload(wl, psi[sample], dt=cfg.dt, nsteps=3, backend=oracle.NAIVE_FFT)
+    with B.grid_for(wl) as g:
+        d = torch.from_numpy(psi).cuda()
+        out = g.apply_hamiltonian(d)
+        err = per_state_rel(out.cpu().numpy(), ref)
+        assert err.max() < TOL, err
+        g.propagate(d, cfg.dt, 3)
+        got = d.cpu().numpy()[sample]
+    err = per_state_rel(got, ref_p)
+    assert err.max() < TOL, err
 
 
 def test_tddft_full_block_sampled_states(torch_cuda, B, oracle):
@@ -634,3 +701,148 @@ def test_seeded_sweep_over_grid_shapes_and_options(torch_cuda, B, oracle, monkey
             g.propagate(d, 0.01, 2)
             assert per_state_rel(d.cpu().numpy(), ref_p).max() < TOL, (done, n, kw)
         done += 1
+
+
+# ------------------------------------------------------------------------------------------------ rotations at the sizes bench.py times
+def test_rotations_512_states_match_oracle(torch_cuda, B, oracle):
+    """tdh_orthonormalize and tdh_subspace_diag at nst = 512 (the cooperative Cholesky and the eigensolver at the size
+    bench.py times) against the oracle, all states, on a 32^3 grid (the oracle's literal loops stay affordable)."""
+    torch = torch_cuda
+    cfg = W.test_config(300, (32, 32, 32), (15.0, 15.0, 15.0), nst=512, natoms=6, lmax=1, rc=2.5, dl=(2.0, -0.8))
+    wl = W.make(cfg)
+    psi = W.states(cfg)
+    q_ref = oracle.orthonormalize(cfg.n, cfg.dv, psi)
+    h_ref = oracle.apply_workload(wl, q_ref, oracle.NAIVE_FFT)
+    w_ref, out_ref, _ = oracle.subspace_diag(cfg.n, cfg.dv, q_ref, h_ref)
+    with B.grid_for(wl) as g:
+        q = g.orthonormalize(torch.from_numpy(psi).cuda())
+        assert per_state_rel(q.cpu().numpy(), q_ref).max() < 1e-11
+        assert np.abs(g.overlap(q).cpu().numpy() - np.eye(512)).max() < 1e-12
+        qd = torch.from_numpy(q_ref).cuda()
+        w, out = g.subspace_diag(qd, g.apply_hamiltonian(qd))
+        assert np.abs(w - w_ref).max() < 1e-11 * max(1.0, np.abs(w_ref).max())
+        assert np.abs(g.overlap(out).cpu().numpy() - np.eye(512)).max() < 1e-11
+        ov = np.abs(np.diag(oracle.overlap(cfg.n, cfg.dv, out_ref, out.cpu().numpy())))
+        gap = np.minimum(np.diff(w_ref, prepend=-np.inf), np.diff(w_ref, append=np.inf))
+        sep = gap > 1e-4
+        assert sep.sum() >= 256 and np.abs(ov[sep] - 1).max() < 1e-7
+
+
+def test_rotations_tddft_block_properties(torch_cuda, B):
+    """The TDDFT block (512 x 64^3), exactly what bench.py times: unit overlap after tdh_orthonormalize to 1e-12, and the
+    Ritz values of tdh_subspace_diag equal LAPACK's eigenvalues of the same subspace matrix (read back with tdh_overlap)
+    to 1e-11; psi'^H H psi' is diagonal."""
+    torch = torch_cuda
+    cfg = W.CONFIGS["tddft"]
+    wl = W.make(cfg)
+    nst = cfg.nst
+    psi, _ = device_block(torch, cfg, nst, [0])
+    with B.grid_for(wl, max_states=nst) as g:
+        q = g.orthonormalize(psi)
+        assert np.abs(g.overlap(q).cpu().numpy() - np.eye(nst)).max() < 1e-12
+        h = g.apply_hamiltonian(q)
+        m = g.overlap(q, h).cpu().numpy()
+        w, out = g.subspace_diag(q, h, out=psi)
+        w_lapack = np.linalg.eigvalsh(0.5 * (m + m.conj().T))
+        assert np.abs(w - w_lapack).max() < 1e-11 * max(1.0, np.abs(w_lapack).max())
+        m2 = g.overlap(out, g.apply_hamiltonian(out, out=h)).cpu().numpy()
+        assert np.abs(m2 - np.diag(w)).max() < 1e-10 * max(1.0, np.abs(w).max())
+    del psi, q, h
+    torch.cuda.empty_cache()
+
+
+def test_rotations_1024_states_smoke(torch_cuda, B, oracle):
+    """The largest block the rotations accept (nst = 1024) on a 16^3 grid: orthonormalise, diagonalise, compare the Ritz
+    values with the oracle and the overlap with the identity."""
+    torch = torch_cuda
+    cfg = W.test_config(301, (16, 16, 16), (10.0, 10.0, 10.0), nst=1024, natoms=2, lmax=0, rc=2.0, dl=(1.5,))
+    wl = W.make(cfg)
+    psi = W.states(cfg)
+    q_ref = oracle.orthonormalize(cfg.n, cfg.dv, psi)
+    w_ref, _, _ = oracle.subspace_diag(cfg.n, cfg.dv, q_ref, oracle.apply_workload(wl, q_ref, oracle.NAIVE_FFT))
+    with B.grid_for(wl) as g:
+        q = g.orthonormalize(torch.from_numpy(psi).cuda())
+        assert np.abs(g.overlap(q).cpu().numpy() - np.eye(1024)).max() < 1e-12
+        assert per_state_rel(q.cpu().numpy(), q_ref).max() < 1e-10       # 1024 compounded Gram-Schmidt columns
+        w, out = g.subspace_diag(q, g.apply_hamiltonian(q))
+        assert np.abs(w - w_ref).max() < 1e-10 * max(1.0, np.abs(w_ref).max())
+        assert np.abs(g.overlap(out).cpu().numpy() - np.eye(1024)).max() < 1e-11
+        with pytest.raises(B.TdhError) as e:
+            g2 = B.Grid(cfg.n, cfg.length, max_states=1025)
+            g2.orthonormalize(torch.zeros((1025,) + cfg.n, dtype=torch.complex128, device="cuda"))
+        assert e.value.code == B.TDH_EUNSUPPORTED
+
+
+# ------------------------------------------------------------------------------------------------ advisor findings (round 1)
+def test_rejected_projector_table_keeps_the_installed_one(torch_cuda, B, oracle):
+    """tdh_set_projectors validates and builds before it replaces: after a rejected table (index out of range) the handle
+    still applies the previous projectors."""
+    torch = torch_cuda
+    cfg = W.CONFIGS["tiny"]
+    wl = W.make(cfg)
+    psi = W.states(cfg)
+    ref = oracle.apply_workload(wl, psi, oracle.DIRECT)
+    with B.grid_for(wl) as g:
+        bad = W.Projectors(**{**wl.proj.__dict__})
+        bad.sph_idx = wl.proj.sph_idx.copy()
+        bad.sph_idx[5] = cfg.npts
+        with pytest.raises(B.TdhError) as e:
+            g.set_projectors(bad)
+        assert e.value.code == B.TDH_EINDEX
+        out = g.apply_hamiltonian(torch.from_numpy(psi).cuda()).cpu().numpy()
+        assert per_state_rel(out, ref).max() < TOL
+        assert g.natoms == cfg.natoms
+        with pytest.raises(B.TdhError):
+            g.forces(torch.from_numpy(psi).cuda(), natoms=cfg.natoms - 1)
+
+
+@pytest.mark.parametrize("mode", ["0", "1"])
+def test_projector_table_without_any_channel(torch_cuda, B, oracle, monkeypatch, mode):
+    """Every atom has zero channels: V_nl = 0; on a split-tile grid (96 x 96 planes) the separate back-projection kernel
+    has no 4-channel tile to launch."""
+    torch = torch_cuda
+    monkeypatch.setenv("TDH_NL_MODE", mode)
+    n, length = (16, 96, 96), (5.0, 30.0, 30.0)
+    cfg = W.test_config(302, n, length, nst=3, natoms=2, lmax=0, rc=2.0, dl=(1.0,))
+    wl = W.make(cfg)
+    pr = wl.proj
+    empty = W.Projectors(natoms=2, sph_off=pr.sph_off, sph_idx=pr.sph_idx, sph_disp=pr.sph_disp,
+                         chan_off=np.zeros(3, dtype=np.int32), beta=np.zeros(0), dcoef=np.zeros(0))
+    psi = W.states(cfg)
+    ref = oracle.apply_hamiltonian(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, wl.v, None, psi, oracle.NAIVE_FFT)
+    with B.grid_for(wl) as g:
+        g.set_projectors(empty)
+        d = torch.from_numpy(psi).cuda()
+        assert per_state_rel(g.apply_hamiltonian(d).cpu().numpy(), ref).max() < TOL
+        g.propagate(d, 0.01, 1)
+        assert bool(torch.isfinite(torch.view_as_real(d)).all())
+
+
+def test_rotate_detects_partial_overlap(torch_cuda, B):
+    """out starting inside psi beyond the first min(n_in, n_out) states is an overlap too."""
+    torch = torch_cuda
+    n = (16, 16, 16)
+    with B.Grid(n, (8.0, 8.0, 8.0), max_states=10) as g:
+        psi = torch.zeros((10,) + n, dtype=torch.complex128, device="cuda")
+        m = torch.zeros((10, 1), dtype=torch.complex128, device="cuda")
+        with pytest.raises(B.TdhError) as e:
+            g.rotate(psi, m, out=psi[5:6])
+        assert e.value.code == B.TDH_EINVAL
+        out = torch.empty((1,) + n, dtype=torch.complex128, device="cuda")
+        g.rotate(psi, m, out=out)
+
+
+def test_sd_step_state_without_kinetic_energy(torch_cuda, B, oracle):
+    """Reading R19 for T_s <= 0 (a constant state at Gamma): finite, and equal to the oracle."""
+    torch = torch_cuda
+    cfg = W.test_config(303, (16, 32, 16), (6.0, 11.0, 6.0), nst=3, natoms=2, lmax=1, rc=2.0, dl=(1.3, -0.6))
+    wl = W.make(cfg)
+    psi = W.states(cfg)
+    psi[1] = 0.3 - 0.2j
+    ref, eig_ref = oracle.sd_step(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, wl.v, wl.proj, psi, 0.17, oracle.NAIVE_FFT)
+    with B.grid_for(wl) as g:
+        d = torch.from_numpy(psi).cuda()
+        eig = g.sd_step(d, 0.17)
+        out = d.cpu().numpy()
+    assert np.isfinite(out).all() and np.abs(eig - eig_ref).max() < 1e-11 * np.abs(eig_ref).max()
+    assert per_state_rel(out, ref).max() < TOL

@@ -588,6 +588,27 @@ def test_p12_sd_step_fixed_points_and_descent(oracle):
         assert np.vdot(out[s], hn).real / np.vdot(out[s], out[s]).real < eps
 
 
+def test_p12_sd_step_state_without_kinetic_energy(oracle):
+    """Reading R19, T_s <= 0: a constant state at Gamma has <psi|T psi> = 0 up to rounding, x = t / T_s is undefined and
+    the limit x -> infinity is taken (K = 1 at t = 0, K = 0 elsewhere) -- the same as a tiny positive T_s gives, so the
+    result cannot hang on the sign of the rounding noise: only the mean of the residual is stepped along, and the result
+    is finite.  With a constant potential and no atoms the constant state is an eigenvector and stays put."""
+    cfg = small_cfg(121, n=(4, 6, 5), length=(4.0, 5.5, 5.0), natoms=2, lmax=1, rc=1.9)
+    wl = W.make(cfg)
+    psi = np.full((1,) + cfg.n, 0.3 - 0.2j)
+    lam = 0.17
+    for backend in (0, 1):
+        out, eig = oracle.sd_step(cfg.n, cfg.length, (0.0, 0.0, 0.0), -1.0, wl.v, wl.proj, psi, lam, backend)
+        h = oracle.apply_hamiltonian(cfg.n, cfg.length, (0.0, 0.0, 0.0), -1.0, wl.v, wl.proj, psi, backend)
+        eps = np.vdot(psi[0], h[0]).real / np.vdot(psi[0], psi[0]).real
+        r = h[0] - eps * psi[0]
+        assert np.isfinite(out).all() and abs(eig[0] - eps) < 1e-12 * abs(eps)
+        assert np.abs(out[0] - (psi[0] - lam * r.mean())).max() < 1e-13
+    vc = np.full(cfg.n, -0.4)
+    out, eig = oracle.sd_step(cfg.n, cfg.length, (0.0, 0.0, 0.0), -1.0, vc, None, psi, lam, 0)
+    assert abs(eig[0] + 0.4) < 1e-13 and rel(out[0], psi[0]) < 1e-13
+
+
 # --------------------------------------------------------------------------------------------- P13 (NEXT-3: subspace diagonalisation)
 def test_p13_subspace_diag_recovers_mixed_eigenvectors_and_cauchy_bounds(oracle):
     """A block spanned by exact eigenvectors of the dense small-grid H, mixed by a random unitary: the Ritz values are those
@@ -631,16 +652,38 @@ def test_p14_gradient_of_plane_waves(oracle):
                 assert rel(g[s], 1j * (TWO_PI * m[a] / length[a] + kpt[a]) * psi[s]) < 1e-12 or np.abs(g[s]).max() < 1e-12
 
 
-@pytest.mark.parametrize("lmax,tol", [(0, 2e-4), (1, 3e-2)])
-def test_p14_forces_are_the_derivative_of_the_ionic_energy_at_fixed_orbitals(oracle, lmax, tol):
+def smooth_l1(proj):
+    """Test-only projector table: the l = 1 channels of workloads.projectors multiplied by |d|, i.e.
+    |d| exp(-d^2/2 sigma^2) Y_1m(d/|d|) = c exp(-d^2/2 sigma^2) (y, z, x): smooth at the atom, unlike the generator's."""
+    out = W.Projectors(**{**proj.__dict__})
+    out.beta = proj.beta.copy()
+    off = 0
+    for a in range(proj.natoms):
+        p0, p1 = int(proj.sph_off[a]), int(proj.sph_off[a + 1])
+        nc, npt = int(proj.chan_off[a + 1] - proj.chan_off[a]), p1 - p0
+        r = np.sqrt(np.sum(proj.sph_disp[p0:p1] ** 2, axis=1))
+        for c in range(1, nc):                                            # channel 0 is l = 0
+            out.beta[off + c * npt: off + (c + 1) * npt] *= r
+        off += nc * npt
+    return out
+
+
+@pytest.mark.parametrize("lmax,tol,smooth", [(0, 2e-4, False), (1, 3e-2, False), (1, 1e-5, True)])
+def test_p14_forces_are_the_derivative_of_the_ionic_energy_at_fixed_orbitals(oracle, lmax, tol, smooth):
     """Eq. 11 equals d/dR_I of E_I(R) = sum_s f_s <psi_s| v_I(r - R_I) |psi_s> at fixed orbitals (translate the atom, rebuild
-    its projector table and its local well, central differences).  Equality holds in the band-limited limit: smooth
+    its projector table and its local well, central differences).  The third case pins the l = 1 path tightly with a
+    projector that is smooth at the atom (smooth_l1, sigma = 0.7 on a 24^3 grid): 1e-5 (measured 2e-6).  Equality holds in the band-limited limit: smooth
     orbitals, projectors negligible at the cutoff sphere; the l = 0 Gaussian is smooth (tight tolerance), the generator's
     l = 1 projectors exp(-d^2/2 sigma^2) Y_1m(d/|d|) jump at the atom, so aliasing leaves about 1e-2 there -- a dropped
     term, a wrong sign or a missing factor 2 is an O(1) error in both.  Checks the factor 2 Re, occupations, the per-atom
     split and both terms of v_I."""
-    cfg = W.test_config(119 + lmax, (16, 16, 16), (6.0, 6.0, 6.0), nst=3, natoms=2, lmax=lmax, rc=2.9,
-                        dl=(1.5, -0.7)[: lmax + 1], proj_sigma=0.5, well_z=1.2, well_sigma=0.7)
+    if smooth:      # wider cell, so that sigma = 0.7 is negligible both at the grid's Nyquist frequency and at the sphere edge
+        cfg = W.test_config(122, (24, 24, 24), (9.0, 9.0, 9.0), nst=3, natoms=2, lmax=1, rc=4.0, dl=(1.5, -0.7),
+                            proj_sigma=0.7, well_z=1.2, well_sigma=0.7)
+    else:
+        cfg = W.test_config(119 + lmax, (16, 16, 16), (6.0, 6.0, 6.0), nst=3, natoms=2, lmax=lmax, rc=2.9,
+                            dl=(1.5, -0.7)[: lmax + 1], proj_sigma=0.5, well_z=1.2, well_sigma=0.7)
+    table = (lambda c, p: smooth_l1(W.projectors(c, p))) if smooth else W.projectors
     pos = np.array([[2.1, 3.3, 2.7], [4.0, 1.6, 3.9]])
     ii = np.meshgrid(*[np.arange(m) for m in cfg.n], indexing="ij")
     rng = np.random.default_rng(119)
@@ -654,7 +697,7 @@ def test_p14_forces_are_the_derivative_of_the_ionic_energy_at_fixed_orbitals(ora
         return W.local_potential(one_atom, np.array([center]))
 
     def energy(center):
-        one = W.projectors(one_atom, np.array([center]))
+        one = table(one_atom, np.array([center]))
         v = well(center)
         e = 0.0
         for s in range(3):
@@ -662,7 +705,7 @@ def test_p14_forces_are_the_derivative_of_the_ionic_energy_at_fixed_orbitals(ora
             e += occ[s] * cfg.dv * (np.vdot(psi[s], nl).real + np.sum(v * np.abs(psi[s]) ** 2))
         return e
 
-    proj = W.projectors(cfg, pos)
+    proj = table(cfg, pos)
     vloc = np.array([well(pos[0]), well(pos[1])])
     f = oracle.forces(cfg.n, cfg.length, cfg.kpt, proj, psi, occ, vloc, 1)
     f_nl = oracle.forces(cfg.n, cfg.length, cfg.kpt, proj, psi, occ, None, 1)
