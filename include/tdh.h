@@ -182,6 +182,54 @@ int tdh_gradient(tdh_grid* g, int nst, const tdh_c128* psi_dev, int axis, tdh_c1
 int tdh_forces(tdh_grid* g, int nst, const tdh_c128* psi_dev, const double* occ_host, const double* vloc_atoms_dev,
                double* forces_host);
 
+/* ---- Slab decomposition of the grid over `world` ranks (Fig. 6: "the real-space is divided along the x
+ * direction while the Fourier-space is split along" another one; "local transforms ... followed by a
+ * redistribution of the data ... and the transform in the last dimension").  Rank r holds, of every state,
+ *     real space:     planes x in [r n0/world, (r+1) n0/world), all y, z        block [nst][n0/world][n1][n2]
+ *     Fourier space:  all k_x, the n1/world rows r n1/world .. of the WORK LAYOUT (the digit-permuted (k_y, k_z) order
+ *                     the in-place transforms leave, see tdh_work_layout), all k_z            [nst][n0][n1/world][n2]
+ * DESIGN.md section 14 says why the Fourier-space split is along y here (the paper draws z).  The redistribution is
+ * not a separate copy: the kernel that produces a value stores it straight into the buffer of the rank that owns it
+ * (device pointers of the peers: NVLink peer memory between GPUs, plain device memory when several ranks are emulated
+ * on one device).  A Hamiltonian application of a rank is therefore four phases; the caller runs phase p on ALL ranks,
+ * then a barrier across the ranks' streams, then phase p + 1:
+ *     TDH_SLAB_PROJECT      partial Kleinman-Bylander projections over the rank's planes (nothing without projectors)
+ *     TDH_SLAB_PLANES_FWD   sum of all ranks' partial projections (read from the peers, in rank order); forward (z,y)
+ *                           transform of the rank's planes, every spectrum row stored to its owner
+ *     TDH_SLAB_PENCILS      forward x, kinetic factor, inverse x on the rank's rows; every plane value stored to its owner
+ *     TDH_SLAB_PLANES_INV   inverse (y,z) transform of the rank's planes, + V psi + V_nl psi, into hpsi
+ * tdh_create_slab_grid: n, len, kpt, ecut, max_states, cuda_stream as tdh_create_grid (n is the FULL grid); world in
+ * [2, 8] must divide n[0] and n[1]/2, and n[0]/world must be a multiple of the planes per tile (TDH_EUNSUPPORTED
+ * otherwise).  On a slab handle tdh_set_potential takes the rank's planes of V ([n0/world][n1][n2]) and
+ * tdh_set_projectors the sphere points inside the rank's planes with LOCAL flat indices ((x - x0) n1 + y) n2 + z and
+ * the SAME atoms and channels on every rank (an atom may have no point on a rank); nst of a phase call is at most the
+ * workspace chunk (max_states if that fits 4 GiB).  The other entry points that transform along x refuse slab handles. */
+enum { TDH_SLAB_PROJECT = 0, TDH_SLAB_PLANES_FWD = 1, TDH_SLAB_PENCILS = 2, TDH_SLAB_PLANES_INV = 3 };
+int tdh_create_slab_grid(const int n[3], const double len[3], const double kpt[3], double ecut, int max_states,
+                         int rank, int world, void* cuda_stream, tdh_grid** out);
+/* This rank's exchange buffers (DEVICE pointers owned by the handle): its Fourier-space slab, its real-space work
+ * block, its partial-projection buffer (NULL until tdh_set_projectors; it changes with every tdh_set_projectors). */
+int tdh_slab_buffers(tdh_grid* g, void** fs_dev, void** rs_dev, void** dpi_dev);
+/* The same three buffers of ALL ranks, in rank order: HOST arrays of `world` DEVICE pointers valid on this device
+ * (entry `rank` must be the handle's own).  dpi_dev may be NULL when no projectors are set.  Call after
+ * tdh_set_projectors. */
+int tdh_slab_set_peers(tdh_grid* g, void* const* fs_dev, void* const* rs_dev, void* const* dpi_dev);
+/* One phase of hpsi = H psi on the rank's planes (psi_dev, hpsi_dev: DEVICE, nst*(n0/world)*n1*n2 complex128; hpsi_dev is
+ * only used by TDH_SLAB_PLANES_INV).  Asynchronous on the handle's stream. */
+int tdh_slab_apply_phase(tdh_grid* g, int phase, int nst, const tdh_c128* psi_dev, tdh_c128* hpsi_dev);
+/* The distributed 3-D transform alone, two phases (barrier in between), in place on block_dev:
+ *   sign -1: rank's planes [nst][n0/world][n1][n2] -> rank's spectrum rows [nst][n0][n1/world][n2] in work layout
+ *   sign +1: the reverse, scaled by 1/(n0 n1 n2). */
+int tdh_slab_fft_phase(tdh_grid* g, int sign, int phase, int nst, tdh_c128* block_dev);
+/* CUDA IPC wrappers for one-process-per-GPU runs: export a handle-owned DEVICE buffer (tdh_slab_buffers) as a 64-byte
+ * token, open a peer's token as a DEVICE pointer valid in this process (peer access is enabled lazily), close it. */
+int tdh_ipc_export(void* dev_ptr, unsigned char handle[64]);
+int tdh_ipc_import(const unsigned char handle[64], void** dev_ptr);
+int tdh_ipc_close(void* dev_ptr);
+/* The work layout: row rowmap[ky] / column colmap[kz] of a spectrum plane holds frequency index ky / kz
+ * (HOST arrays of n1 and n2 ints). */
+int tdh_work_layout(const tdh_grid* g, int* rowmap_host, int* colmap_host);
+
 /* The same two operations with HOST buffers (pageable or pinned): the library stages state chunks through its own
  * pinned buffers, overlapping host<->device copies with the kernels, and returns when hpsi_host / psi_host is complete.
  * nst is not limited by max_states here (chunks are).  These are the end-to-end entry points timed by bench.py. */

@@ -26,6 +26,8 @@ LIB_PATH = os.path.join(_HERE, "libtdh.so")
 SYMBOLS = (
     "tdh_create_grid", "tdh_destroy_grid", "tdh_set_potential", "tdh_set_projectors", "tdh_apply_hamiltonian",
     "tdh_propagate", "tdh_taylor_pair", "tdh_etrs_step", "tdh_density", "tdh_hartree", "tdh_overlap", "tdh_rotate", "tdh_orthonormalize", "tdh_subspace_diag", "tdh_sd_step", "tdh_gradient", "tdh_forces", "tdh_apply_hamiltonian_host", "tdh_propagate_host", "tdh_fft3d", "tdh_last_launch_count",
+    "tdh_create_slab_grid", "tdh_slab_buffers", "tdh_slab_set_peers", "tdh_slab_apply_phase", "tdh_slab_fft_phase", "tdh_work_layout",
+    "tdh_ipc_export", "tdh_ipc_import", "tdh_ipc_close",
     "tdh_set_profiling", "tdh_last_kernel_seconds", "tdh_kernel_name", "tdh_set_chunk_states", "tdh_last_error",
 )
 NKERNELS = 5
@@ -73,6 +75,15 @@ def lib() -> C.CDLL:
     l.tdh_propagate_host.argtypes = [vp, i, vp, d, i, i]
     l.tdh_fft3d.argtypes = [vp, i, vp, i]
     l.tdh_last_launch_count.argtypes = [vp]
+    l.tdh_create_slab_grid.argtypes = [C.POINTER(i), C.POINTER(d), C.POINTER(d), d, i, i, i, vp, C.POINTER(vp)]
+    l.tdh_slab_buffers.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
+    l.tdh_slab_set_peers.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
+    l.tdh_slab_apply_phase.argtypes = [vp, i, i, vp, vp]
+    l.tdh_slab_fft_phase.argtypes = [vp, i, i, i, vp]
+    l.tdh_work_layout.argtypes = [vp, C.POINTER(i), C.POINTER(i)]
+    l.tdh_ipc_export.argtypes = [vp, C.c_char_p]
+    l.tdh_ipc_import.argtypes = [C.c_char_p, C.POINTER(vp)]
+    l.tdh_ipc_close.argtypes = [vp]
     l.tdh_set_profiling.argtypes = [vp, i]
     l.tdh_last_kernel_seconds.argtypes = [vp, C.POINTER(d)]
     l.tdh_kernel_name.argtypes = [i]
@@ -105,21 +116,29 @@ class Grid:
     """Owns one tdh_grid handle.  All tensors passed in must live on the device that was current at creation."""
 
     def __init__(self, n: Sequence[int], length: Sequence[float], kpt: Sequence[float] = (0.0, 0.0, 0.0),
-                 ecut: float = -1.0, max_states: int = 1, stream: Optional[int] = None):
+                 ecut: float = -1.0, max_states: int = 1, stream: Optional[int] = None,
+                 slab: Optional[Sequence[int]] = None):
+        """slab = (rank, world): the handle of one rank of a slab decomposition (tdh_create_slab_grid); self.n is then
+        the shape of the rank's real-space planes and self.n_full the whole grid."""
         import torch
         l = lib()
         if stream is None:
             if not torch.cuda.is_available():
                 raise TdhError(TDH_ECUDA, "no CUDA device available (there is no CPU fallback)")
             stream = torch.cuda.current_stream().cuda_stream
-        self.n = tuple(int(x) for x in n)
+        self.n_full = tuple(int(x) for x in n)
+        self.slab = None if slab is None else (int(slab[0]), int(slab[1]))
+        self.n = self.n_full if slab is None else (self.n_full[0] // self.slab[1],) + self.n_full[1:]
         self.npts = self.n[0] * self.n[1] * self.n[2]
         self.max_states = int(max_states)
         self.natoms = 0
         self._h = C.c_void_p()
-        _check(l.tdh_create_grid((C.c_int * 3)(*self.n), (C.c_double * 3)(*[float(x) for x in length]),
-                                 (C.c_double * 3)(*[float(x) for x in kpt]), float(ecut), int(max_states),
-                                 C.c_void_p(stream), C.byref(self._h)))
+        a3 = ((C.c_int * 3)(*self.n_full), (C.c_double * 3)(*[float(x) for x in length]),
+              (C.c_double * 3)(*[float(x) for x in kpt]), float(ecut), int(max_states))
+        if slab is None:
+            _check(l.tdh_create_grid(*a3, C.c_void_p(stream), C.byref(self._h)))
+        else:
+            _check(l.tdh_create_slab_grid(*a3, self.slab[0], self.slab[1], C.c_void_p(stream), C.byref(self._h)))
 
     # -- lifetime
     def close(self):
@@ -329,6 +348,34 @@ class Grid:
         _check(lib().tdh_fft3d(self._h, nst, C.c_void_p(psi.data_ptr()), int(sign)))
         return psi
 
+    # -- slab decomposition (one handle per rank; shard.SlabGroup drives the phases)
+    def slab_buffers(self):
+        """(fs, rs, dpi) device addresses of this rank's exchange buffers (dpi is 0 without projectors)."""
+        fs, rs, dp = C.c_void_p(), C.c_void_p(), C.c_void_p()
+        _check(lib().tdh_slab_buffers(self._h, C.byref(fs), C.byref(rs), C.byref(dp)))
+        return fs.value or 0, rs.value or 0, dp.value or 0
+
+    def slab_set_peers(self, fs: Sequence[int], rs: Sequence[int], dpi: Optional[Sequence[int]] = None):
+        w = len(fs)
+        arr = lambda xs: (C.c_void_p * w)(*[C.c_void_p(int(x)) for x in xs])
+        _check(lib().tdh_slab_set_peers(self._h, arr(fs), arr(rs), None if dpi is None else arr(dpi)))
+
+    def slab_apply_phase(self, phase: int, psi, out=None):
+        nst = self._block(psi)
+        _check(lib().tdh_slab_apply_phase(self._h, int(phase), nst, C.c_void_p(psi.data_ptr()),
+                                          None if out is None else C.c_void_p(out.data_ptr())))
+
+    def slab_fft_phase(self, sign: int, phase: int, block):
+        nst = self._block(block)
+        _check(lib().tdh_slab_fft_phase(self._h, int(sign), int(phase), nst, C.c_void_p(block.data_ptr())))
+
+    def work_layout(self):
+        """(rowmap, colmap): plane row rowmap[ky] / column colmap[kz] of the work layout holds frequency index ky / kz."""
+        ny, nz = self.n_full[1], self.n_full[2]
+        r, c = (C.c_int * ny)(), (C.c_int * nz)()
+        _check(lib().tdh_work_layout(self._h, r, c))
+        return np.array(r[:], dtype=np.int64), np.array(c[:], dtype=np.int64)
+
     # -- host entry points (end-to-end path)
     def apply_hamiltonian_host(self, psi_host, out_host):
         nst = psi_host.size // self.npts if isinstance(psi_host, np.ndarray) else psi_host.numel() // self.npts
@@ -356,6 +403,23 @@ class Grid:
 
     def set_chunk_states(self, chunk: int):
         _check(lib().tdh_set_chunk_states(self._h, int(chunk)))
+
+
+def ipc_export(dev_ptr: int) -> bytes:
+    """64-byte CUDA IPC token of a handle-owned device buffer."""
+    buf = C.create_string_buffer(64)
+    _check(lib().tdh_ipc_export(C.c_void_p(int(dev_ptr)), buf))
+    return buf.raw
+
+
+def ipc_import(token: bytes) -> int:
+    p = C.c_void_p()
+    _check(lib().tdh_ipc_import(C.create_string_buffer(token, 64), C.byref(p)))
+    return p.value
+
+
+def ipc_close(dev_ptr: int):
+    _check(lib().tdh_ipc_close(C.c_void_p(int(dev_ptr))))
 
 
 def grid_for(wl, max_states: Optional[int] = None, device_v=None) -> Grid:

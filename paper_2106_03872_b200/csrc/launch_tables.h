@@ -5,7 +5,8 @@
 namespace tdh {
 
 struct TileLaunch {
-    const void* fwd;   // tile_fwd_kernel<NY,NZ>
+    const void* fwd;   // tile_fwd_kernel<NY,NZ,false>
+    const void* fwd_slab;  // tile_fwd_kernel<NY,NZ,true>: spectrum rows stored into the ranks' Fourier-space slabs
     const void* inv[5];  // tile_inv_kernel<NY,NZ,CM>, CM = 0 (no projectors), 1, 4, 9, 16 (tile_kernels.cuh, nl_cm_index)
     int threads;
     int ppc;           // plane parts per CTA
@@ -22,6 +23,8 @@ struct XLaunch {
     const void* inv;    // xpencil_kernel<NX,S,2>
     const void* poisson;  // xpencil_kernel<NX,S,3>
     const void* teter;    // xpencil_kernel<NX,S,4>
+    const void* fused_slab;  // xpencil_kernel<NX,S,0,true>: pencils of a Fourier-space slab, x values stored to their owners
+    const void* inv_slab;    // xpencil_kernel<NX,S,2,true>
     int threads;
     size_t smem;        // dynamic shared memory per CTA (ring of tiles)
 };

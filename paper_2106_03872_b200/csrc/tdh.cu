@@ -105,6 +105,18 @@ struct tdh_grid {
     double* d_w;          // tdh_subspace_diag: eigenvalues
     double* d_sd;         // tdh_sd_step: [max_states] eps, [max_states] T, [max_states * 3 * SD_SLICES] partial sums
     int ctas_fwd, ctas_inv[tdh::NL_NCM], ctas_x[5];   // persistent grid sizes (SM count x resident CTAs)
+    int ctas_fwd_slab, ctas_x_slab[2];
+
+    // slab decomposition (tdh_create_slab_grid): n[0] is then the number of LOCAL planes, nx_fs the full NX
+    int nx_fs;            // planes the x transform spans (= n[0] unless this is a slab handle)
+    size_t np_total;      // grid points of the whole grid
+    int slab_world, slab_rank, ny_local;
+    cd* d_fs;             // Fourier-space slab [chunk][NX][ny_local][NZ]: target of the ranks' tile_fwd stores
+    cd* d_dpi_part;       // this rank's partial projections (summed over the ranks into d_dpi)
+    cd* peer_fs[tdh::SLAB_MAX_WORLD];
+    cd* peer_rs[tdh::SLAB_MAX_WORLD];
+    const cd* peer_dpi[tdh::SLAB_MAX_WORLD];
+    bool have_peers;
 
     int chunk_cap;        // states the workspace can hold
     int chunk;            // states pushed through the chain together
@@ -171,7 +183,7 @@ static void free_projectors(tdh_grid* g) {
     cudaFree(g->d_atoms_col); g->d_atoms_col = nullptr; g->col_off.clear();
     cudaFree(g->d_dvscale); g->d_dvscale = nullptr; cudaFree(g->d_dpig); g->d_dpig = nullptr;
     cudaFree(g->d_force); g->d_force = nullptr;
-    cudaFree(g->d_dpi); cudaFree(g->d_nl_off); cudaFree(g->d_nl_cc); cudaFree(g->d_nl_beta); cudaFree(g->d_nl_phase);
+    cudaFree(g->d_dpi); cudaFree(g->d_dpi_part); g->d_dpi_part = nullptr; cudaFree(g->d_nl_off); cudaFree(g->d_nl_cc); cudaFree(g->d_nl_beta); cudaFree(g->d_nl_phase);
     g->d_atoms = nullptr; g->d_sidx = nullptr; g->d_sbeta = nullptr; g->d_sphase = nullptr; g->d_dscale = nullptr;
     g->d_dpi = nullptr; g->d_nl_off = nullptr; g->d_nl_cc = nullptr; g->d_nl_beta = nullptr; g->d_nl_phase = nullptr;
     g->natoms = 0; g->nchan_tot = 0; g->mt = 1;
@@ -188,8 +200,10 @@ static int default_chunk(const tdh_grid* g) {
     return std::max(1, std::min(c, g->chunk_cap));
 }
 
-extern "C" int tdh_create_grid(const int n[3], const double len[3], const double kpt[3], double ecut, int max_states,
-                               void* cuda_stream, tdh_grid** out) {
+// n: the FULL grid.  world = 1: an ordinary handle.  world > 1: the handle of rank `rank` of a slab decomposition, which
+// owns planes rank * n[0]/world .. of every state in real space and rows rank * n[1]/world .. in Fourier space.
+static int create_impl(const int n[3], const double len[3], const double kpt[3], double ecut, int max_states,
+                       void* cuda_stream, int rank, int world, tdh_grid** out) {
     if (!n || !len || !kpt || !out) return fail(TDH_EINVAL, "tdh_create_grid: null argument");
     if (max_states < 1) return fail(TDH_EINVAL, "tdh_create_grid: max_states must be >= 1");
     for (int a = 0; a < 3; ++a) {
@@ -198,6 +212,10 @@ extern "C" int tdh_create_grid(const int n[3], const double len[3], const double
         if (size_index(n[a]) < 0)
             return fail(TDH_EUNSUPPORTED, "tdh_create_grid: n[%d] = %d unsupported (supported: 16, 32, 48, 64, 96)", a, n[a]);
     }
+    if (world < 1 || world > tdh::SLAB_MAX_WORLD || rank < 0 || rank >= world)
+        return fail(TDH_EINVAL, "tdh_create_slab_grid: rank %d / world %d (world <= %d)", rank, world, tdh::SLAB_MAX_WORLD);
+    if (world > 1 && (n[0] % world != 0 || n[1] % (2 * world) != 0))
+        return fail(TDH_EUNSUPPORTED, "tdh_create_slab_grid: world = %d must divide n[0] = %d and n[1] / 2 = %d", world, n[0], n[1] / 2);
     int ndev = 0;
     CU(cudaGetDeviceCount(&ndev));
     if (ndev < 1) return fail(TDH_ECUDA, "tdh_create_grid: no CUDA device (there is no CPU fallback)");
@@ -205,10 +223,16 @@ extern "C" int tdh_create_grid(const int n[3], const double len[3], const double
     tdh_grid* g = new (std::nothrow) tdh_grid();
     if (!g) return fail(TDH_ENOMEM, "tdh_create_grid: host allocation failed");
     for (int a = 0; a < 3; ++a) { g->n[a] = n[a]; g->len[a] = len[a]; g->kpt[a] = kpt[a]; }
+    g->nx_fs = n[0];
+    g->n[0] = n[0] / world;                                   // local planes
+    g->slab_world = world;
+    g->slab_rank = rank;
+    g->ny_local = n[1] / world;
     g->ecut = (ecut > 0.0 && std::isfinite(ecut)) ? ecut : -1.0;
     g->max_states = max_states;
     g->stream = (cudaStream_t)cuda_stream;
-    g->np = (size_t)n[0] * n[1] * n[2];
+    g->np_total = (size_t)n[0] * n[1] * n[2];
+    g->np = g->np_total / world;
     g->dv = (len[0] / n[0]) * (len[1] / n[1]) * (len[2] / n[2]);
     g->have_k = kpt[0] != 0.0 || kpt[1] != 0.0 || kpt[2] != 0.0;
     g->mt = 1;
@@ -223,6 +247,11 @@ extern "C" int tdh_create_grid(const int n[3], const double len[3], const double
     }
     ok = ok && tdh::xpencil_launch(n[0], g->tl.s, &g->xl);
     if (!ok) { delete g; return fail(TDH_EUNSUPPORTED, "tdh_create_grid: no kernel for this grid"); }
+    if (world > 1 && g->n[0] % g->tl.ppc != 0) {
+        const int ppc = g->tl.ppc;
+        delete g;
+        return fail(TDH_EUNSUPPORTED, "tdh_create_slab_grid: %d local planes are not a multiple of the %d planes of a tile", n[0] / world, ppc);
+    }
 
     int rc = TDH_OK;
     auto body = [&]() -> int {
@@ -231,13 +260,17 @@ extern "C" int tdh_create_grid(const int n[3], const double len[3], const double
         int dev = 0, nsm = 0;
         CU(cudaGetDevice(&dev));
         CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
-        constexpr int NK = 6 + tdh::NL_NCM;
-        const void* fs[NK] = {g->tl.fwd, g->xl.fused, g->xl.fwd, g->xl.inv, g->xl.poisson, g->xl.teter};
-        size_t sm[NK] = {g->tl.smem_fwd, g->xl.smem, g->xl.smem, g->xl.smem, g->xl.smem, g->xl.smem};
-        int th[NK] = {g->tl.threads, g->xl.threads, g->xl.threads, g->xl.threads, g->xl.threads, g->xl.threads};
-        for (int i = 0; i < tdh::NL_NCM; ++i) { fs[6 + i] = g->tl.inv[i]; sm[6 + i] = g->tl.smem_inv; th[6 + i] = g->tl.threads; }
+        constexpr int NK = 9 + tdh::NL_NCM;
+        const void* fs[NK] = {g->tl.fwd, g->xl.fused, g->xl.fwd, g->xl.inv, g->xl.poisson, g->xl.teter,
+                              g->tl.fwd_slab, g->xl.fused_slab, g->xl.inv_slab};
+        size_t sm[NK] = {g->tl.smem_fwd, g->xl.smem, g->xl.smem, g->xl.smem, g->xl.smem, g->xl.smem,
+                         g->tl.smem_fwd, g->xl.smem, g->xl.smem};
+        int th[NK] = {g->tl.threads, g->xl.threads, g->xl.threads, g->xl.threads, g->xl.threads, g->xl.threads,
+                      g->tl.threads, g->xl.threads, g->xl.threads};
+        for (int i = 0; i < tdh::NL_NCM; ++i) { fs[9 + i] = g->tl.inv[i]; sm[9 + i] = g->tl.smem_inv; th[9 + i] = g->tl.threads; }
         int ctas[NK];
         for (int i = 0; i < NK; ++i) {
+            if (world == 1 && i >= 6 && i < 9) { ctas[i] = 0; continue; }       // slab kernels: slab handles only
             CU(cudaFuncSetAttribute(fs[i], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm[i]));
             CU(cudaFuncSetAttribute(fs[i], cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
             int occ = 0;
@@ -248,7 +281,8 @@ extern "C" int tdh_create_grid(const int n[3], const double len[3], const double
         }
         g->ctas_fwd = ctas[0];
         g->ctas_x[0] = ctas[1]; g->ctas_x[1] = ctas[2]; g->ctas_x[2] = ctas[3]; g->ctas_x[3] = ctas[4]; g->ctas_x[4] = ctas[5];
-        for (int i = 0; i < tdh::NL_NCM; ++i) g->ctas_inv[i] = ctas[6 + i];
+        for (int i = 0; i < tdh::NL_NCM; ++i) g->ctas_inv[i] = ctas[9 + i];
+        g->ctas_fwd_slab = ctas[6]; g->ctas_x_slab[0] = ctas[7]; g->ctas_x_slab[1] = ctas[8];
         // tables: built on the host exactly as the oracle builds its G vectors (two_pi * m / L + k, then squared)
         const double two_pi = 6.283185307179586476925286766559;
         for (int a = 0; a < 3; ++a) {
@@ -337,6 +371,7 @@ extern "C" int tdh_create_grid(const int n[3], const double len[3], const double
         // at least two states each: tdh_taylor_pair keeps phi_2 and phi_3 in the two halves of d_phi[0]
         CU(cudaMalloc(&g->d_phi[0], state_bytes * std::max(2, g->chunk_cap)));
         CU(cudaMalloc(&g->d_phi[1], state_bytes * std::max(2, g->chunk_cap)));
+        if (world > 1) CU(cudaMalloc(&g->d_fs, state_bytes * g->chunk_cap));
         g->chunk = default_chunk(g);
         return TDH_OK;
     };
@@ -344,6 +379,17 @@ extern "C" int tdh_create_grid(const int n[3], const double len[3], const double
     if (rc != TDH_OK) { tdh_destroy_grid(g); return rc; }
     *out = g;
     return TDH_OK;
+}
+
+extern "C" int tdh_create_grid(const int n[3], const double len[3], const double kpt[3], double ecut, int max_states,
+                               void* cuda_stream, tdh_grid** out) {
+    return create_impl(n, len, kpt, ecut, max_states, cuda_stream, 0, 1, out);
+}
+
+extern "C" int tdh_create_slab_grid(const int n[3], const double len[3], const double kpt[3], double ecut, int max_states,
+                                    int rank, int world, void* cuda_stream, tdh_grid** out) {
+    if (world < 2) return fail(TDH_EINVAL, "tdh_create_slab_grid: world must be >= 2 (tdh_create_grid makes an undivided grid)");
+    return create_impl(n, len, kpt, ecut, max_states, cuda_stream, rank, world, out);
 }
 
 extern "C" int tdh_destroy_grid(tdh_grid* g) {
@@ -358,7 +404,7 @@ extern "C" int tdh_destroy_grid(tdh_grid* g) {
     cudaFree(g->d_gd);
     for (int i = 0; i < 3; ++i) cudaFree(g->d_small[i]);
     cudaFree(g->d_status); cudaFree(g->d_sd); cudaFree(g->d_rot); cudaFree(g->d_ctl); cudaFree(g->d_w);
-    cudaFree(g->d_work); cudaFree(g->d_phi[0]); cudaFree(g->d_phi[1]);
+    cudaFree(g->d_work); cudaFree(g->d_phi[0]); cudaFree(g->d_phi[1]); cudaFree(g->d_fs);
     for (int i = 0; i < 2; ++i) {
         cudaFree(g->d_hin[i]); cudaFree(g->d_hout[i]);
         if (g->ev_in[i]) cudaEventDestroy(g->ev_in[i]);
@@ -570,6 +616,7 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
         std::vector<double> dvs(ctot, g->dv);
         if ((rc = up(&nw->d_dvscale, dvs))) { free_projectors(nw); return rc; }
         e = cudaMalloc(&nw->d_dpig, sizeof(cd) * (size_t)g->chunk_cap * ctot);
+        if (e == cudaSuccess && g->slab_world > 1) e = cudaMalloc(&nw->d_dpi_part, sizeof(cd) * (size_t)g->chunk_cap * ctot);
         if (e == cudaSuccess) e = cudaMalloc(&nw->d_force, sizeof(double) * (size_t)natoms * 3 * (1 + 64));
         if (e != cudaSuccess) { free_projectors(nw); return fail(TDH_ENOMEM, "tdh_set_projectors: %s", cudaGetErrorString(e)); }
     }
@@ -579,7 +626,7 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
     g->d_atoms_col = nw->d_atoms_col; g->d_atoms = nw->d_atoms; g->d_sidx = nw->d_sidx; g->d_sbeta = nw->d_sbeta;
     g->d_sphase = nw->d_sphase; g->d_dscale = nw->d_dscale; g->d_nl_off = nw->d_nl_off; g->d_nl_cc = nw->d_nl_cc;
     g->d_nl_beta = nw->d_nl_beta; g->d_nl_phase = nw->d_nl_phase; g->d_dpi = nw->d_dpi; g->d_dvscale = nw->d_dvscale;
-    g->d_dpig = nw->d_dpig; g->d_force = nw->d_force;
+    g->d_dpig = nw->d_dpig; g->d_force = nw->d_force; g->d_dpi_part = nw->d_dpi_part;
     g->natoms = natoms;
     g->nchan_tot = ctot;
     g->nl_layers = nlayers;
@@ -651,36 +698,59 @@ static int tile_map(tdh_grid* g, const cd* base, int nst, CUtensorMap* m) {
     return TDH_OK;
 }
 
-static int launch_plane_fwd(tdh_grid* g, int nst, const cd* in, cd* out) {
+// to_peers (slab handles): every spectrum row is stored into the Fourier-space slab of the rank that owns it
+static int launch_plane_fwd(tdh_grid* g, int nst, const cd* in, cd* out, bool to_peers = false) {
     CUtensorMap map;
     int rc = tile_map(g, in, nst, &map);
     if (rc) return rc;
     const cd* twy = g->d_tw[1];
     const cd* twz = g->d_tw[2];
     int ntiles = (int)((size_t)nst * g->n[0] * g->tl.s / g->tl.ppc);
-    void* args[] = {(void*)&map, (void*)&out, (void*)&ntiles, (void*)&twy, (void*)&twz};
-    const unsigned grid = (unsigned)std::min(ntiles, g->ctas_fwd);
-    LAUNCH(K_PLANE_FWD, g->tl.fwd, dim3(grid), dim3(g->tl.threads), g->tl.smem_fwd, args);
+    tdh::SlabDst sd;
+    memset(&sd, 0, sizeof(sd));
+    if (to_peers) {
+        for (int q = 0; q < g->slab_world; ++q) sd.fs[q] = g->peer_fs[q];
+        sd.ny_local = g->ny_local; sd.nx_local = g->n[0]; sd.nx_total = g->nx_fs; sd.x0 = g->slab_rank * g->n[0];
+    }
+    void* args[] = {(void*)&map, (void*)&out, (void*)&ntiles, (void*)&twy, (void*)&twz, (void*)&sd};
+    const unsigned grid = (unsigned)std::min(ntiles, to_peers ? g->ctas_fwd_slab : g->ctas_fwd);
+    LAUNCH(K_PLANE_FWD, to_peers ? g->tl.fwd_slab : g->tl.fwd, dim3(grid), dim3(g->tl.threads), g->tl.smem_fwd, args);
     return TDH_OK;
 }
 
-static int launch_xpencil(tdh_grid* g, int nst, const cd* in, cd* out, int mode, const double* tstate = nullptr) {
+// On a slab handle `in` is this rank's Fourier-space slab [nst][NX][ny_local][NZ]; with to_peers (modes 0 and 2) the
+// values of plane x are stored into the real-space work buffer of the rank that owns x.
+static int launch_xpencil(tdh_grid* g, int nst, const cd* in, cd* out, int mode, const double* tstate = nullptr,
+                          bool to_peers = false) {
+    const bool slab = g->slab_world > 1;
+    const int ny = slab ? g->ny_local : g->n[1];                     // rows of the block this launch sees
+    const int y0 = slab ? g->slab_rank * g->ny_local : 0;
     CUtensorMap map;
-    if (!tdh::encode_line_map(&map, in, (size_t)nst * g->n[0], g->n[0], g->n[1], g->n[2]))
+    if (!tdh::encode_line_map(&map, in, (size_t)nst * g->nx_fs, g->nx_fs, ny, g->n[2]))
         return fail(TDH_ECUDA, "cuTensorMapEncodeTiled failed (line map)");
     tdh::Kinetic kin;
-    kin.g2x = g->d_g2[0]; kin.g2y_w = g->d_g2y_w; kin.g2z_w = g->d_g2z_w; kin.twy_w = g->d_twy_w;
-    if (mode == 3) { kin.g2x = g->d_p2x; kin.g2y_w = g->d_p2y_w; kin.g2z_w = g->d_p2z_w; }     // Poisson: pure |G|^2
+    kin.g2x = g->d_g2[0]; kin.g2y_w = g->d_g2y_w + y0; kin.g2z_w = g->d_g2z_w; kin.twy_w = g->d_twy_w + y0 / 2;
+    if (mode == 3) { kin.g2x = g->d_p2x; kin.g2y_w = g->d_p2y_w + y0; kin.g2z_w = g->d_p2z_w; }     // Poisson: pure |G|^2
     kin.tstate = tstate;
     kin.ecut = g->ecut;
-    kin.scale = 1.0 / (double)g->np;
+    kin.scale = 1.0 / (double)g->np_total;
     kin.nz = g->n[2];
-    kin.ny = g->n[1];
-    int ntiles = nst * (g->n[1] / 2) * (g->n[2] / 16);
+    kin.ny = ny;
+    int ntiles = nst * (ny / 2) * (g->n[2] / 16);
     const cd* twx = g->d_tw[0];
-    void* args[] = {(void*)&map, (void*)&out, (void*)&ntiles, (void*)&twx, (void*)&kin};
+    tdh::SlabSrc ss;
+    memset(&ss, 0, sizeof(ss));
     const void* f = mode == 0 ? g->xl.fused : (mode == 1 ? g->xl.fwd : (mode == 2 ? g->xl.inv : (mode == 3 ? g->xl.poisson : g->xl.teter)));
-    const unsigned grid = (unsigned)std::min(ntiles, g->ctas_x[mode]);
+    int ctas = g->ctas_x[mode];
+    if (to_peers) {
+        if (mode != 0 && mode != 2) return fail(TDH_EINVAL, "launch_xpencil: no slab stores for mode %d", mode);
+        for (int q = 0; q < g->slab_world; ++q) ss.rs[q] = g->peer_rs[q];
+        ss.nx_local = g->n[0]; ss.ny_total = g->n[1]; ss.y0 = y0;
+        f = mode == 0 ? g->xl.fused_slab : g->xl.inv_slab;
+        ctas = g->ctas_x_slab[mode == 0 ? 0 : 1];
+    }
+    void* args[] = {(void*)&map, (void*)&out, (void*)&ntiles, (void*)&twx, (void*)&kin, (void*)&ss};
+    const unsigned grid = (unsigned)std::min(ntiles, ctas);
     LAUNCH(K_XPENCIL, f, dim3(grid), dim3(g->xl.threads), g->xl.smem, args);
     return TDH_OK;
 }
@@ -733,7 +803,7 @@ static int launch_nl_project(tdh_grid* g, int nst, const cd* in, const double* d
     const double* sbeta = g->d_sbeta;
     const cd* sphase = g->d_sphase;
     const double* dscale = dscale_in ? dscale_in : g->d_dscale;
-    cd* dpi = dpi_out ? dpi_out : g->d_dpi;
+    cd* dpi = dpi_out ? dpi_out : (g->slab_world > 1 ? g->d_dpi_part : g->d_dpi);
     int nct = g->nchan_tot;
     void* args[] = {(void*)&in, (void*)&npts, (void*)&nst, (void*)&atoms, (void*)&sidx, (void*)&sbeta,
                     (void*)&sphase, (void*)&dscale, (void*)&dpi, (void*)&nct};
@@ -765,6 +835,8 @@ static int launch_nl_scatter(tdh_grid* g, int nst, cd* out, cd alpha) {
     return TDH_OK;
 }
 
+static int finish_chunk(tdh_grid* g, int nst, const cd* in, cd* out, cd alpha, const cd* yv);
+
 // out = alpha * H in + yv   for one chunk (nst <= chunk_cap); in/out/yv point at the chunk's first state
 static int apply_chunk(tdh_grid* g, int nst, const cd* in, cd* out, cd alpha, const cd* yv, bool kinetic_only = false) {
     int rc;
@@ -781,6 +853,12 @@ static int apply_chunk(tdh_grid* g, int nst, const cd* in, cd* out, cd alpha, co
     if (g->natoms > 0 && (rc = launch_nl_project(g, nst, in))) return rc;
     if ((rc = launch_plane_fwd(g, nst, in, g->d_work))) return rc;
     if ((rc = launch_xpencil(g, nst, g->d_work, g->d_work, 0))) return rc;
+    return finish_chunk(g, nst, in, out, alpha, yv);
+}
+
+// last part of one application: inverse (y,z) transform of the work block with the fused epilogue (+ back-projection)
+static int finish_chunk(tdh_grid* g, int nst, const cd* in, cd* out, cd alpha, const cd* yv) {
+    int rc;
     tdh::Epilogue ep;
     memset(&ep, 0, sizeof(ep));
     const bool fused_nl = g->natoms > 0 && g->nl_mode == 0;
@@ -882,6 +960,12 @@ static int propagate_block(tdh_grid* g, int nst, cd* psi, double dt, int nsteps)
     return TDH_OK;
 }
 
+// entry points that transform along x need the whole grid on one device: refused on the handles of a slab decomposition
+#define NOT_SLAB(name)                                                                                        \
+    do {                                                                                                      \
+        if (g->slab_world > 1) return fail(TDH_EINVAL, name ": not available on a slab handle (tdh_slab_*)"); \
+    } while (0)
+
 static bool overlaps(const void* a, const void* b, size_t bytes) {
     const char* x = (const char*)a;
     const char* y = (const char*)b;
@@ -890,6 +974,7 @@ static bool overlaps(const void* a, const void* b, size_t bytes) {
 
 extern "C" int tdh_apply_hamiltonian(tdh_grid* g, int nst, const tdh_c128* psi_dev, tdh_c128* hpsi_dev) {
     if (!g || !psi_dev || !hpsi_dev) return fail(TDH_EINVAL, "tdh_apply_hamiltonian: null argument");
+    NOT_SLAB("tdh_apply_hamiltonian");
     if (nst < 1 || nst > g->max_states) return fail(TDH_EINVAL, "tdh_apply_hamiltonian: nst = %d outside [1, %d]", nst, g->max_states);
     if (overlaps(psi_dev, hpsi_dev, (size_t)nst * g->np * sizeof(cd)))
         return fail(TDH_EINVAL, "tdh_apply_hamiltonian: psi and hpsi overlap");
@@ -901,6 +986,7 @@ extern "C" int tdh_apply_hamiltonian(tdh_grid* g, int nst, const tdh_c128* psi_d
 
 extern "C" int tdh_propagate(tdh_grid* g, int nst, tdh_c128* psi_dev, double dt, int nsteps, int order) {
     if (!g || !psi_dev) return fail(TDH_EINVAL, "tdh_propagate: null argument");
+    NOT_SLAB("tdh_propagate");
     if (nst < 1 || nst > g->max_states) return fail(TDH_EINVAL, "tdh_propagate: nst = %d outside [1, %d]", nst, g->max_states);
     if (order != 4) return fail(TDH_EINVAL, "tdh_propagate: order must be 4");
     if (nsteps < 0 || !std::isfinite(dt)) return fail(TDH_EINVAL, "tdh_propagate: bad dt / nsteps");
@@ -912,6 +998,7 @@ extern "C" int tdh_propagate(tdh_grid* g, int nst, tdh_c128* psi_dev, double dt,
 
 extern "C" int tdh_taylor_pair(tdh_grid* g, int nst, tdh_c128* psi_dev, tdh_c128* full_dev, double dt, int order) {
     if (!g || !psi_dev || !full_dev) return fail(TDH_EINVAL, "tdh_taylor_pair: null argument");
+    NOT_SLAB("tdh_taylor_pair");
     if (nst < 1 || nst > g->max_states) return fail(TDH_EINVAL, "tdh_taylor_pair: nst = %d outside [1, %d]", nst, g->max_states);
     if (order != 4) return fail(TDH_EINVAL, "tdh_taylor_pair: order must be 4");
     if (!std::isfinite(dt)) return fail(TDH_EINVAL, "tdh_taylor_pair: bad dt");
@@ -926,6 +1013,7 @@ extern "C" int tdh_taylor_pair(tdh_grid* g, int nst, tdh_c128* psi_dev, tdh_c128
 extern "C" int tdh_etrs_step(tdh_grid* g, int nst, tdh_c128* psi_dev, tdh_c128* approx_dev, double dt,
                              const double* v_next_dev) {
     if (!g || !psi_dev || !approx_dev) return fail(TDH_EINVAL, "tdh_etrs_step: null argument");
+    NOT_SLAB("tdh_etrs_step");
     if (nst < 1 || nst > g->max_states) return fail(TDH_EINVAL, "tdh_etrs_step: nst = %d outside [1, %d]", nst, g->max_states);
     if (!std::isfinite(dt)) return fail(TDH_EINVAL, "tdh_etrs_step: bad dt");
     if (overlaps(psi_dev, approx_dev, (size_t)nst * g->np * sizeof(cd)))
@@ -1008,6 +1096,7 @@ extern "C" int tdh_density(tdh_grid* g, int nst, const tdh_c128* psi_dev, const 
 // worth of work through the same three FFT kernels as H; uses the work buffer and the first Horner buffer.
 extern "C" int tdh_hartree(tdh_grid* g, const double* n_dev, double* vh_dev) {
     if (!g || !n_dev || !vh_dev) return fail(TDH_EINVAL, "tdh_hartree: null argument");
+    NOT_SLAB("tdh_hartree");
     stats_reset(g);
     cd* a = g->d_phi[0];
     real_to_complex_kernel<<<296, 256, 0, g->stream>>>(n_dev, a, g->np);
@@ -1124,6 +1213,7 @@ static int gradient_from_spectrum(tdh_grid* g, int nst, int axis, cd* out) {
 
 extern "C" int tdh_gradient(tdh_grid* g, int nst, const tdh_c128* psi_dev, int axis, tdh_c128* out_dev) {
     if (!g || !psi_dev || !out_dev) return fail(TDH_EINVAL, "tdh_gradient: null argument");
+    NOT_SLAB("tdh_gradient");
     if (nst < 1 || nst > g->max_states) return fail(TDH_EINVAL, "tdh_gradient: nst = %d outside [1, %d]", nst, g->max_states);
     if (axis < 0 || axis > 2) return fail(TDH_EINVAL, "tdh_gradient: axis must be 0, 1 or 2");
     if (overlaps(psi_dev, out_dev, (size_t)nst * g->np * sizeof(cd))) return fail(TDH_EINVAL, "tdh_gradient: psi and out overlap");
@@ -1140,6 +1230,7 @@ extern "C" int tdh_gradient(tdh_grid* g, int nst, const tdh_c128* psi_dev, int a
 extern "C" int tdh_forces(tdh_grid* g, int nst, const tdh_c128* psi_dev, const double* occ_host, const double* vloc_atoms_dev,
                           double* forces_host) {
     if (!g || !psi_dev || !forces_host) return fail(TDH_EINVAL, "tdh_forces: null argument");
+    NOT_SLAB("tdh_forces");
     if (nst < 1 || nst > g->max_states) return fail(TDH_EINVAL, "tdh_forces: nst = %d outside [1, %d]", nst, g->max_states);
     if (g->natoms < 1) return fail(TDH_EINVAL, "tdh_forces: no atoms (tdh_set_projectors)");
     stats_reset(g);
@@ -1255,6 +1346,7 @@ __global__ void sd_residual_kernel(const cd* __restrict__ psi, cd* __restrict__ 
 
 extern "C" int tdh_sd_step(tdh_grid* g, int nst, tdh_c128* psi_dev, tdh_c128* work_dev, double lambda, double* eig_host) {
     if (!g || !psi_dev || !work_dev) return fail(TDH_EINVAL, "tdh_sd_step: null argument");
+    NOT_SLAB("tdh_sd_step");
     if (nst < 1 || nst > g->max_states) return fail(TDH_EINVAL, "tdh_sd_step: nst = %d outside [1, %d]", nst, g->max_states);
     if (!std::isfinite(lambda)) return fail(TDH_EINVAL, "tdh_sd_step: bad lambda");
     if (overlaps(psi_dev, work_dev, (size_t)nst * g->np * sizeof(cd)))
@@ -1383,6 +1475,7 @@ static int small_scratch(tdh_grid* g, int nst) {
 extern "C" int tdh_subspace_diag(tdh_grid* g, int nst, const tdh_c128* psi_dev, const tdh_c128* hpsi_dev, tdh_c128* out_dev,
                                  double* eig_host) {
     if (!g || !psi_dev || !hpsi_dev || !out_dev) return fail(TDH_EINVAL, "tdh_subspace_diag: null argument");
+    NOT_SLAB("tdh_subspace_diag");
     if (nst < 1 || nst > 1024) return fail(nst < 1 ? TDH_EINVAL : TDH_EUNSUPPORTED, "tdh_subspace_diag: nst = %d outside [1, 1024]", nst);
     if (overlaps(psi_dev, out_dev, (size_t)nst * g->np * sizeof(cd)))
         return fail(TDH_EINVAL, "tdh_subspace_diag: psi and out overlap");
@@ -1422,6 +1515,7 @@ extern "C" int tdh_subspace_diag(tdh_grid* g, int nst, const tdh_c128* psi_dev, 
 // Cholesky orthonormalisation: S = dV psi^H psi = L L^H, out = psi L^{-H}
 extern "C" int tdh_orthonormalize(tdh_grid* g, int nst, const tdh_c128* psi_dev, tdh_c128* out_dev) {
     if (!g || !psi_dev || !out_dev) return fail(TDH_EINVAL, "tdh_orthonormalize: null argument");
+    NOT_SLAB("tdh_orthonormalize");
     if (nst < 1 || nst > 1024) return fail(nst < 1 ? TDH_EINVAL : TDH_EUNSUPPORTED, "tdh_orthonormalize: nst = %d outside [1, 1024]", nst);
     if (overlaps(psi_dev, out_dev, (size_t)nst * g->np * sizeof(cd)))
         return fail(TDH_EINVAL, "tdh_orthonormalize: psi and out overlap");
@@ -1464,6 +1558,7 @@ extern "C" int tdh_orthonormalize(tdh_grid* g, int nst, const tdh_c128* psi_dev,
 
 extern "C" int tdh_fft3d(tdh_grid* g, int nst, tdh_c128* psi_dev, int sign) {
     if (!g || !psi_dev) return fail(TDH_EINVAL, "tdh_fft3d: null argument");
+    NOT_SLAB("tdh_fft3d");
     if (nst < 1) return fail(TDH_EINVAL, "tdh_fft3d: nst < 1");
     if (sign != 1 && sign != -1) return fail(TDH_EINVAL, "tdh_fft3d: sign must be -1 or +1");
     stats_reset(g);
@@ -1488,6 +1583,148 @@ extern "C" int tdh_fft3d(tdh_grid* g, int nst, tdh_c128* psi_dev, int sign) {
         }
     }
     return prof_collect(g);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// NEXT-4: slab decomposition of the grid over ranks (Fig. 6).  The all-to-all of the
+// parallel 3-D transform is fused into the stores of the kernels that produce the data (tile_fwd: spectrum rows to
+// their owners' Fourier-space slabs; xpencil: plane values to their owners' real-space work buffers), so a rank's
+// Hamiltonian application is four stream-ordered phases with a cross-rank barrier between them and no copy kernels.
+// ------------------------------------------------------------------------------------------------------------
+// dpi[i] = sum over ranks (in rank order: every rank gets bitwise the same sum) of the partial projections
+__global__ void slab_reduce_dpi_kernel(cd* __restrict__ dpi, size_t n, int world, const cd* p0, const cd* p1, const cd* p2,
+                                       const cd* p3, const cd* p4, const cd* p5, const cd* p6, const cd* p7) {
+    const cd* ps[8] = {p0, p1, p2, p3, p4, p5, p6, p7};
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        cd acc = make_double2(0.0, 0.0);
+        for (int q = 0; q < world; ++q) {
+            const cd v = __ldcg(ps[q] + i);
+            acc.x += v.x;
+            acc.y += v.y;
+        }
+        dpi[i] = acc;
+    }
+}
+
+extern "C" int tdh_slab_buffers(tdh_grid* g, void** fs_dev, void** rs_dev, void** dpi_dev) {
+    if (!g) return fail(TDH_EINVAL, "tdh_slab_buffers: null handle");
+    if (g->slab_world < 2) return fail(TDH_EINVAL, "tdh_slab_buffers: not a slab handle");
+    if (fs_dev) *fs_dev = g->d_fs;
+    if (rs_dev) *rs_dev = g->d_work;
+    if (dpi_dev) *dpi_dev = g->d_dpi_part;
+    return TDH_OK;
+}
+
+extern "C" int tdh_slab_set_peers(tdh_grid* g, void* const* fs_dev, void* const* rs_dev, void* const* dpi_dev) {
+    if (!g || !fs_dev || !rs_dev) return fail(TDH_EINVAL, "tdh_slab_set_peers: null argument");
+    if (g->slab_world < 2) return fail(TDH_EINVAL, "tdh_slab_set_peers: not a slab handle");
+    for (int q = 0; q < g->slab_world; ++q) {
+        if (!fs_dev[q] || !rs_dev[q]) return fail(TDH_EINVAL, "tdh_slab_set_peers: null buffer of rank %d", q);
+        if (g->natoms > 0 && (!dpi_dev || !dpi_dev[q])) return fail(TDH_EINVAL, "tdh_slab_set_peers: projectors are set but rank %d has no projection buffer", q);
+    }
+    if (fs_dev[g->slab_rank] != g->d_fs || rs_dev[g->slab_rank] != g->d_work)
+        return fail(TDH_EINVAL, "tdh_slab_set_peers: entry %d must be this handle's own buffers (tdh_slab_buffers)", g->slab_rank);
+    CU(cudaStreamSynchronize(g->stream));
+    for (int q = 0; q < g->slab_world; ++q) {
+        g->peer_fs[q] = (cd*)fs_dev[q];
+        g->peer_rs[q] = (cd*)rs_dev[q];
+        g->peer_dpi[q] = dpi_dev ? (const cd*)dpi_dev[q] : nullptr;
+    }
+    g->have_peers = true;
+    return TDH_OK;
+}
+
+static int slab_check(tdh_grid* g, const char* name, int nst) {
+    if (!g) return fail(TDH_EINVAL, "%s: null handle", name);
+    if (g->slab_world < 2) return fail(TDH_EINVAL, "%s: not a slab handle (tdh_create_slab_grid)", name);
+    if (!g->have_peers) return fail(TDH_EINVAL, "%s: tdh_slab_set_peers has not been called", name);
+    if (nst < 1 || nst > g->chunk_cap) return fail(TDH_EINVAL, "%s: nst = %d outside [1, %d] (one chunk per call)", name, nst, g->chunk_cap);
+    return TDH_OK;
+}
+
+extern "C" int tdh_slab_apply_phase(tdh_grid* g, int phase, int nst, const tdh_c128* psi_dev, tdh_c128* hpsi_dev) {
+    int rc = slab_check(g, "tdh_slab_apply_phase", nst);
+    if (rc) return rc;
+    if (!psi_dev) return fail(TDH_EINVAL, "tdh_slab_apply_phase: null psi");
+    const cd* in = (const cd*)psi_dev;
+    if (phase == 0) stats_reset(g);
+    switch (phase) {
+        case TDH_SLAB_PROJECT:                      // partial projections over this rank's planes
+            if (g->natoms > 0 && (rc = launch_nl_project(g, nst, in))) return rc;
+            return TDH_OK;
+        case TDH_SLAB_PLANES_FWD: {                 // sum of the ranks' projections; (z,y) transform, rows to their owners
+            if (g->natoms > 0) {
+                for (int q = 0; q < g->slab_world; ++q)
+                    if (!g->peer_dpi[q]) return fail(TDH_EINVAL, "tdh_slab_apply_phase: projection buffer of rank %d not set", q);
+                const size_t n = (size_t)nst * g->nchan_tot;
+                const cd** pp = g->peer_dpi;
+                slab_reduce_dpi_kernel<<<(unsigned)std::min<size_t>(296, (n + 255) / 256), 256, 0, g->stream>>>(
+                    g->d_dpi, n, g->slab_world, pp[0], pp[1], pp[2], pp[3], pp[4], pp[5], pp[6], pp[7]);
+                CU(cudaGetLastError());
+                g->launch_count += 1;
+            }
+            return launch_plane_fwd(g, nst, in, nullptr, true);
+        }
+        case TDH_SLAB_PENCILS:                      // x transform, kinetic factor, inverse x: plane values to their owners
+            return launch_xpencil(g, nst, g->d_fs, nullptr, 0, nullptr, true);
+        case TDH_SLAB_PLANES_INV:                   // inverse (y,z) transform + epilogue on this rank's planes
+            if (!hpsi_dev) return fail(TDH_EINVAL, "tdh_slab_apply_phase: null hpsi");
+            if (overlaps(psi_dev, hpsi_dev, (size_t)nst * g->np * sizeof(cd)))
+                return fail(TDH_EINVAL, "tdh_slab_apply_phase: psi and hpsi overlap");
+            if ((rc = finish_chunk(g, nst, in, (cd*)hpsi_dev, make_double2(1.0, 0.0), nullptr))) return rc;
+            return prof_collect(g);
+        default:
+            return fail(TDH_EINVAL, "tdh_slab_apply_phase: phase %d", phase);
+    }
+}
+
+extern "C" int tdh_slab_fft_phase(tdh_grid* g, int sign, int phase, int nst, tdh_c128* block_dev) {
+    int rc = slab_check(g, "tdh_slab_fft_phase", nst);
+    if (rc) return rc;
+    if (!block_dev) return fail(TDH_EINVAL, "tdh_slab_fft_phase: null block");
+    if (sign != 1 && sign != -1) return fail(TDH_EINVAL, "tdh_slab_fft_phase: sign must be -1 or +1");
+    if (phase != 0 && phase != 1) return fail(TDH_EINVAL, "tdh_slab_fft_phase: phase %d", phase);
+    cd* blk = (cd*)block_dev;
+    if (phase == 0) stats_reset(g);
+    if (sign < 0) {
+        if (phase == 0) return launch_plane_fwd(g, nst, blk, nullptr, true);            // real-space slab -> owners' rows
+        return launch_xpencil(g, nst, g->d_fs, blk, 1);                                  // spectrum slab, work layout
+    }
+    if (phase == 0) return launch_xpencil(g, nst, blk, nullptr, 2, nullptr, true);      // spectrum slab -> owners' planes
+    tdh::Epilogue ep;
+    memset(&ep, 0, sizeof(ep));
+    ep.alpha = make_double2(1.0, 0.0);
+    ep.nx = g->n[0];
+    return launch_plane_inv(g, nst, g->d_work, nullptr, blk, ep);
+}
+
+// CUDA IPC wrappers so that one process per GPU can hand its exchange buffers to its peers (shard.SlabRank)
+extern "C" int tdh_ipc_export(void* dev_ptr, unsigned char handle[64]) {
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "IPC handle size");
+    if (!dev_ptr || !handle) return fail(TDH_EINVAL, "tdh_ipc_export: null argument");
+    cudaIpcMemHandle_t h;
+    CU(cudaIpcGetMemHandle(&h, dev_ptr));
+    memcpy(handle, &h, 64);
+    return TDH_OK;
+}
+extern "C" int tdh_ipc_import(const unsigned char handle[64], void** dev_ptr) {
+    if (!handle || !dev_ptr) return fail(TDH_EINVAL, "tdh_ipc_import: null argument");
+    cudaIpcMemHandle_t h;
+    memcpy(&h, handle, 64);
+    CU(cudaIpcOpenMemHandle(dev_ptr, h, cudaIpcMemLazyEnablePeerAccess));
+    return TDH_OK;
+}
+extern "C" int tdh_ipc_close(void* dev_ptr) {
+    if (!dev_ptr) return TDH_OK;
+    CU(cudaIpcCloseMemHandle(dev_ptr));
+    return TDH_OK;
+}
+
+extern "C" int tdh_work_layout(const tdh_grid* g, int* rowmap_host, int* colmap_host) {
+    if (!g || !rowmap_host || !colmap_host) return fail(TDH_EINVAL, "tdh_work_layout: null argument");
+    CU(cudaMemcpy(rowmap_host, g->d_rowmap, sizeof(int) * g->n[1], cudaMemcpyDeviceToHost));
+    CU(cudaMemcpy(colmap_host, g->d_colmap, sizeof(int) * g->n[2], cudaMemcpyDeviceToHost));
+    return TDH_OK;
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -1547,6 +1784,7 @@ static int host_pipeline(tdh_grid* g, int nst, const cd* in_host, cd* out_host, 
 
 extern "C" int tdh_apply_hamiltonian_host(tdh_grid* g, int nst, const tdh_c128* psi_host, tdh_c128* hpsi_host) {
     if (!g || !psi_host || !hpsi_host) return fail(TDH_EINVAL, "tdh_apply_hamiltonian_host: null argument");
+    NOT_SLAB("tdh_apply_hamiltonian_host");
     if (nst < 1) return fail(TDH_EINVAL, "tdh_apply_hamiltonian_host: nst < 1");
     if (overlaps(psi_host, hpsi_host, (size_t)nst * g->np * sizeof(cd)))
         return fail(TDH_EINVAL, "tdh_apply_hamiltonian_host: psi and hpsi overlap");
@@ -1555,6 +1793,7 @@ extern "C" int tdh_apply_hamiltonian_host(tdh_grid* g, int nst, const tdh_c128* 
 
 extern "C" int tdh_propagate_host(tdh_grid* g, int nst, tdh_c128* psi_host, double dt, int nsteps, int order) {
     if (!g || !psi_host) return fail(TDH_EINVAL, "tdh_propagate_host: null argument");
+    NOT_SLAB("tdh_propagate_host");
     if (nst < 1) return fail(TDH_EINVAL, "tdh_propagate_host: nst < 1");
     if (order != 4) return fail(TDH_EINVAL, "tdh_propagate_host: order must be 4");
     if (nsteps < 0 || !std::isfinite(dt)) return fail(TDH_EINVAL, "tdh_propagate_host: bad dt / nsteps");

@@ -99,6 +99,21 @@ __device__ __forceinline__ void group_sync(int grp) {
     asm volatile("bar.sync %0, %1;" ::"r"(grp + 1), "n"(NTHREADS) : "memory");
 }
 
+// Slab decomposition (Fig. 6): with the grid split over `world` ranks, a rank holds the planes
+// x0 .. x0 + nx_local - 1 of every state in real space and the rows y0 .. y0 + ny_local - 1 (work-layout order) of ALL
+// planes in Fourier space.  The redistribution between the two ("all-to-all") is fused into the stores of the producing
+// kernels: tile_fwd writes every spectrum row straight into the Fourier-space slab buffer of the rank that owns it
+// (fs[q] is that rank's buffer [state][NX][ny_local][NZ]: a peer pointer over NVLink, or another buffer of the same
+// device when the ranks are emulated on one GPU).
+constexpr int SLAB_MAX_WORLD = 8;
+struct SlabDst {
+    cd* fs[SLAB_MAX_WORLD];
+    int ny_local;           // rows per rank, NY / world (even)
+    int nx_local;           // planes per state on this rank, NX / world
+    int nx_total;           // NX
+    int x0;                 // first plane of this rank
+};
+
 // ------------------------------------------------------------------------------------------------------------
 // forward: `map_in` describes the input block, `out` is the work block (same geometry, digit-permuted spectrum).
 // Persistent grid; ntiles = nst * NX * S / PPC.
@@ -108,10 +123,10 @@ __device__ __forceinline__ void group_sync(int grp) {
 // refills the buffer with tile k + 3 when the group is done with it.  The groups only meet at the mbarriers of the
 // ring, so while one group sits in a shared-memory-bound or store-bound stage the other one keeps the FP64 pipe busy.
 // ------------------------------------------------------------------------------------------------------------
-template <int NY, int NZ>
+template <int NY, int NZ, bool SLAB>
 __global__ void __launch_bounds__(TileCfg<NY, NZ>::T, 1)
 tile_fwd_kernel(const __grid_constant__ CUtensorMap map_in, cd* __restrict__ out, int ntiles,
-                const cd* __restrict__ tw_y, const cd* __restrict__ tw_z)
+                const cd* __restrict__ tw_y, const cd* __restrict__ tw_z, const SlabDst slab)
 {
     using C = TileCfg<NY, NZ>;
     constexpr int S = C::S, NYS = C::NYS, R1Z = C::R1Z, R1Y = C::R1Y, R2Y = C::R2Y, T = C::T, NB = C::NB_FWD;
@@ -205,9 +220,21 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap map_in, cd* __restrict__ out
             for (int j2 = 0; j2 < R2Y; ++j2) res[j2] = sm[swz((row0 + j2) * R1Z + k1, k2)];
             Dft<R2Y, -1>::run(res);
             const int part = part0 + lp, plane = part / S, r = part % S;
-            cd* dst = out + (size_t)plane * NY * NZ + (size_t)(S * (k1y * R2Y) + r) * NZ + c;
+            if (SLAB) {
+                // row Y of plane (st, x0 + xl) belongs to rank q = Y / ny_local: local row Y - q * ny_local of its slab
+                const int st = plane / slab.nx_local, xl = plane - st * slab.nx_local;
+                const size_t prow = ((size_t)st * slab.nx_total + slab.x0 + xl) * slab.ny_local;
 #pragma unroll
-            for (int k2y = 0; k2y < R2Y; ++k2y) sts_cd(dst + (size_t)(S * k2y) * NZ, res[k2y]);
+                for (int k2y = 0; k2y < R2Y; ++k2y) {
+                    const int Y = S * (k1y * R2Y + k2y) + r;
+                    const int q = Y / slab.ny_local;
+                    sts_cd(slab.fs[q] + (prow + (Y - q * slab.ny_local)) * NZ + c, res[k2y]);
+                }
+            } else {
+                cd* dst = out + (size_t)plane * NY * NZ + (size_t)(S * (k1y * R2Y) + r) * NZ + c;
+#pragma unroll
+                for (int k2y = 0; k2y < R2Y; ++k2y) sts_cd(dst + (size_t)(S * k2y) * NZ, res[k2y]);
+            }
         }
         // every read of this buffer is done: hand it back to the TMA
         fence_proxy_async();

@@ -11,6 +11,8 @@ template <int NX, int S> static XLaunch make_x_launch() {
     x.inv = reinterpret_cast<const void*>(&xpencil_kernel<NX, S, 2>);
     x.poisson = reinterpret_cast<const void*>(&xpencil_kernel<NX, S, 3>);
     x.teter = reinterpret_cast<const void*>(&xpencil_kernel<NX, S, 4>);
+    x.fused_slab = reinterpret_cast<const void*>(&xpencil_kernel<NX, S, 0, true>);
+    x.inv_slab = reinterpret_cast<const void*>(&xpencil_kernel<NX, S, 2, true>);
     x.threads = XCfg<NX>::T;
     x.smem = XCfg<NX>::SMEM;
     return x;

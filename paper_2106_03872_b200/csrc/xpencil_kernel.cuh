@@ -53,6 +53,17 @@ struct Kinetic {
     int ny;
 };
 
+// Slab decomposition (tile_kernels.cuh, SlabDst): the pencils of this rank's Fourier-space slab (rows y0 .. y0 + ny_local - 1
+// of all NX planes; `Kinetic::ny` = ny_local and the y tables start at y0) end their inverse x transform with the value
+// of plane x, which belongs to rank p = x / nx_local: it is stored straight into that rank's real-space work buffer
+// rs[p] = [state][nx_local][NY][NZ] -- the way back of the all-to-all, fused into the stores (peer pointers over NVLink).
+struct SlabSrc {
+    cd* rs[8];
+    int nx_local;           // planes per state and rank
+    int ny_total;           // NY
+    int y0;                 // first row of this rank's Fourier-space slab
+};
+
 __device__ __forceinline__ cd shfl16(cd v) {
     return make_double2(__shfl_xor_sync(0xffffffffu, v.x, 16), __shfl_xor_sync(0xffffffffu, v.y, 16));
 }
@@ -103,11 +114,12 @@ __device__ __forceinline__ double diag_factor(double gx2, double gy2, double gz2
 
 // grid: persistent CTAs; ntiles = nst * (NY/2) * (NZ/16).  in (through `map`) and out may be the same buffer: a tile
 // is read completely before any of its lines is written.
-template <int NX, int S, int MODE>
+template <int NX, int S, int MODE, bool SLAB = false>
 __global__ void __launch_bounds__(XCfg<NX>::T, XCfg<NX>::CPS)
 xpencil_kernel(const __grid_constant__ CUtensorMap map, cd* __restrict__ out, int ntiles,
-               const cd* __restrict__ tw_x, const Kinetic kin)
+               const cd* __restrict__ tw_x, const Kinetic kin, const SlabSrc slab)
 {
+    static_assert(!SLAB || MODE == 0 || MODE == 2, "the slab stores exist for the modes that end in real space");
     using C = XCfg<NX>;
     constexpr int R1 = C::R1, R2 = C::R2, L = XP_LPC, NB = C::NB, TPL = C::TPL, RA = C::ROUNDS_A, RB = C::ROUNDS_B;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
@@ -155,6 +167,14 @@ xpencil_kernel(const __grid_constant__ CUtensorMap map, cd* __restrict__ out, in
         const int rho2 = rem / zc, ch = rem % zc;
         const int Y = 2 * rho2 + half, zp = ch * 16 + (l & 15);
         cd* gcol = out + (size_t)st * NX * nynz + (size_t)Y * kin.nz + zp;   // element x at gcol + x * nynz
+        // address of the value of plane x of this pencil
+        auto xdst = [&](int x) -> cd* {
+            if (SLAB) {
+                const int p = x / slab.nx_local;
+                return slab.rs[p] + (((size_t)st * slab.nx_local + (x - p * slab.nx_local)) * slab.ny_total + slab.y0 + Y) * kin.nz + zp;
+            }
+            return gcol + (size_t)x * nynz;
+        };
         // per-line constants of this tile (in flight while the tile arrives)
         double gy2a = 0.0, gy2b = 0.0, gz2 = 0.0;
         cd w = make_double2(1.0, 0.0);
@@ -310,7 +330,7 @@ xpencil_kernel(const __grid_constant__ CUtensorMap map, cd* __restrict__ out, in
                 for (int k1 = 0; k1 < R1; ++k1) x[k1] = sm[(k1 * R2 + n2) * L + l];
                 Dft<R1, +1>::run(x);
 #pragma unroll
-                for (int n1 = 0; n1 < R1; ++n1) __stcs(gcol + (size_t)(n2 + R2 * n1) * nynz, x[n1]);
+                for (int n1 = 0; n1 < R1; ++n1) __stcs(xdst(n2 + R2 * n1), x[n1]);
             }
         }
         const int n2 = hi + (RA - 1) * TPL;
@@ -325,7 +345,7 @@ xpencil_kernel(const __grid_constant__ CUtensorMap map, cd* __restrict__ out, in
         if (n2 < R2) {
             Dft<R1, +1>::run(x);
 #pragma unroll
-            for (int n1 = 0; n1 < R1; ++n1) __stcs(gcol + (size_t)(n2 + R2 * n1) * nynz, x[n1]);
+            for (int n1 = 0; n1 < R1; ++n1) __stcs(xdst(n2 + R2 * n1), x[n1]);
         }
     }
 }

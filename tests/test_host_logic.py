@@ -158,6 +158,115 @@ def test_world_size_2_gloo(tmp_path):
         assert p.returncode == 0 and f"ok {r}" in o, o
 
 
+_SLAB_WORKER = r"""
+import sys
+sys.path.insert(0, {root!r})
+import numpy as np
+import torch
+import torch.distributed as dist
+from paper_2106_03872_b200 import shard
+WORLD = 2
+dist.init_process_group("gloo", init_method="tcp://127.0.0.1:{port}", rank=int(sys.argv[1]), world_size=WORLD)
+rank = dist.get_rank()
+n, nst = (8, 12, 5), 3
+nxl, nyl = n[0] // WORLD, n[1] // WORLD
+# every element of the global block carries its own global index
+A = torch.arange(nst * n[0] * n[1] * n[2], dtype=torch.float64).reshape(nst, *n)
+x0, x1 = shard.slab_planes(n[0], rank, WORLD)
+y0, y1 = shard.slab_rows(n[1], rank, WORLD)
+mine = A[:, x0:x1].contiguous()
+
+
+def route(src, planes, rows_of, dest_fn, dest_shape):
+    # send every row of `src` to the rank and offset `dest_fn` names (grouped isend / irecv); returns the filled buffer
+    rows = [[] for _ in range(WORLD)]
+    offs = [[] for _ in range(WORLD)]
+    for s in range(nst):
+        for xi, x in enumerate(planes):
+            for ri, row in enumerate(rows_of):
+                q, off = dest_fn(n, WORLD, s, x, row)
+                rows[q].append(src[s, xi, ri])
+                offs[q].append(off)
+    send_d = [torch.stack(r) for r in rows]
+    send_o = [torch.tensor(o, dtype=torch.int64) for o in offs]
+    recv_d = [torch.empty_like(send_d[q]) for q in range(WORLD)]      # the partition is even: equal counts both ways
+    recv_o = [torch.empty_like(send_o[q]) for q in range(WORLD)]
+    ops = []
+    for q in range(WORLD):
+        if q == rank:
+            recv_d[q], recv_o[q] = send_d[q], send_o[q]
+            continue
+        ops += [dist.P2POp(dist.isend, send_d[q], q, tag=1), dist.P2POp(dist.irecv, recv_d[q], q, tag=1)]
+        ops += [dist.P2POp(dist.isend, send_o[q], q, tag=2), dist.P2POp(dist.irecv, recv_o[q], q, tag=2)]
+    for w in dist.batch_isend_irecv(ops):
+        w.wait()
+    buf = torch.full((int(np.prod(dest_shape)),), -1.0, dtype=torch.float64)
+    for q in range(WORLD):
+        for row, off in zip(recv_d[q], recv_o[q].tolist()):
+            assert (buf[off:off + n[2]] == -1.0).all(), "two rows landed on one address"
+            buf[off:off + n[2]] = row
+    assert (buf >= 0).all(), "a row of the slab was never written"
+    return buf.reshape(dest_shape)
+
+
+# forward exchange: my planes, all rows -> the owners of the rows
+fs = route(mine, range(x0, x1), range(n[1]), shard.fs_destination, (nst, n[0], nyl, n[2]))
+assert torch.equal(fs, A[:, :, y0:y1]), "Fourier-space slab is not rows [y0, y1) of all planes"
+# way back: my rows, all planes -> the owners of the planes
+rs = route(fs, range(n[0]), range(y0, y1), shard.rs_destination, (nst, nxl, n[1], n[2]))
+assert torch.equal(rs, mine), "the way back does not restore the real-space slab"
+
+# projector tables: the ranks' parts are a partition of the table, with local indices and the full channel list
+from paper_2106_03872_b200 import workloads as W
+cfg = W.test_config(160, (8, 12, 6), (4.0, 6.0, 3.0), nst=1, natoms=3, lmax=1, rc=1.4, dl=(1.0, -0.5))
+pr = W.projectors(cfg)
+part = shard.slab_projectors(pr, cfg.n, *shard.slab_planes(cfg.n[0], rank, WORLD))
+assert part.natoms == pr.natoms and np.array_equal(part.chan_off, pr.chan_off) and np.array_equal(part.dcoef, pr.dcoef)
+plane = cfg.n[1] * cfg.n[2]
+xs0 = shard.slab_planes(cfg.n[0], rank, WORLD)[0]
+counts = [int(part.sph_off[a + 1] - part.sph_off[a]) for a in range(pr.natoms)]
+allc = [None] * WORLD
+dist.all_gather_object(allc, counts)
+assert [sum(c[a] for c in allc) for a in range(pr.natoms)] == [int(pr.sph_off[a + 1] - pr.sph_off[a]) for a in range(pr.natoms)]
+boff_p = boff_f = 0
+for a in range(pr.natoms):
+    nc = int(pr.chan_off[a + 1] - pr.chan_off[a])
+    f0, f1 = int(pr.sph_off[a]), int(pr.sph_off[a + 1])
+    p0, p1 = int(part.sph_off[a]), int(part.sph_off[a + 1])
+    full_idx = pr.sph_idx[f0:f1].astype(np.int64)
+    keep = (full_idx // plane >= xs0) & (full_idx // plane < xs0 + cfg.n[0] // WORLD)
+    assert np.array_equal(part.sph_idx[p0:p1].astype(np.int64) + xs0 * plane, full_idx[keep])
+    assert np.array_equal(part.sph_disp[p0:p1], pr.sph_disp[f0:f1][keep])
+    bf = pr.beta[boff_f:boff_f + nc * (f1 - f0)].reshape(nc, f1 - f0)
+    bp = part.beta[boff_p:boff_p + nc * (p1 - p0)].reshape(nc, p1 - p0)
+    assert np.array_equal(bp, bf[:, keep])
+    boff_f += nc * (f1 - f0)
+    boff_p += nc * (p1 - p0)
+dist.barrier()
+dist.destroy_process_group()
+print("ok", rank)
+"""
+
+
+def test_slab_index_maps_world_size_2_gloo(tmp_path):
+    """NEXT-4: the two store-address maps of the slab decomposition (shard.fs_destination / rs_destination: the addresses
+    the tile_fwd and x-pencil kernels store to) route a block between two gloo ranks with grouped isend / irecv: every row
+    lands exactly once, the Fourier-space slab is rows [y0, y1) of all planes, the way back restores the planes; the ranks'
+    projector tables partition the full one."""
+    import socket
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    script = tmp_path / "slab_worker.py"
+    script.write_text(_SLAB_WORKER.format(root=ROOT, port=port))
+    procs = [subprocess.Popen([sys.executable, str(script), str(r)], stdout=subprocess.PIPE, stderr=subprocess.STDOUT)
+             for r in range(2)]
+    outs = [p.communicate(timeout=180)[0].decode() for p in procs]
+    for r, (p, o) in enumerate(zip(procs, outs)):
+        assert p.returncode == 0 and f"ok {r}" in o, o
+
+
 def test_bench_reference_arm_prints_the_contract_line():
     """bench.py --impl reference runs the oracle on the host cores and prints one JSON line with the contract's keys."""
     import json
