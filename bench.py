@@ -155,18 +155,22 @@ def fp64_gemm_ceiling(torch, n=8192, reps=3):
     return 2.0 * n ** 3 / best * 1e-12
 
 
-def fp64_tensor_peak():
-    """FP64 tensor-core peak for the contraction legs: no FP64 GEMM is in MEASURED_PEAKS.json, so it is the measured bf16
-    peak times the nominal FP64 / bf16 ratio of B200 (45 / 2250 dense TFLOP/s, blackwell_cuda_programming.md); the cuBLAS
-    DGEMM rate measured in the same run is reported beside it (fp64_gemm_ceiling)."""
+def fp64_tensor_peak(torch, B):
+    """FP64 tensor-core ceiling for the contraction legs, measured in this run two ways: a dependent-free
+    mma.sync.m8n8k4.f64 issue loop (tdh_measure_fp64_mma_peak, registers only) and cuBLAS DGEMM 8192^3 (torch.matmul).
+    The roofline denominator is the larger of the two; the bf16-scaled nominal figure is reported for context only."""
+    issue = B.measure_fp64_mma_peak()
+    dgemm = fp64_gemm_ceiling(torch)
+    out = {"mma_issue_loop_tflops": round(issue, 2), "cublas_dgemm_8192_tflops": round(dgemm, 2),
+           "peak": round(max(issue, dgemm), 2),
+           "peak_source": "larger of the mma.sync.m8n8k4.f64 issue loop and cuBLAS DGEMM 8192^3, both measured in this run"}
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    ratio = 45.0 / 2250.0
     if os.path.exists(path):
         try:
-            return float(json.load(open(path))["bf16_tflops"]) * ratio, "measured bf16_tflops x 45/2250 (nominal FP64/bf16 ratio)"
+            out["bf16_scaled_nominal_tflops"] = round(float(json.load(open(path))["bf16_tflops"]) * 45.0 / 2250.0, 2)
         except Exception:
             pass
-    return 45.0, "nominal 45 TFLOP/s (no MEASURED_PEAKS.json)"
+    return out
 
 
 class Dist:
@@ -276,10 +280,25 @@ def kernel_breakdown(torch, g, fn, steps):
     return {k: v / steps for k, v in tot.items()}, launches
 
 
-# DRAM bytes per state*gridpoint measured by ncu (dram__bytes_read.sum + dram__bytes_write.sum of one launch of each
-# kernel / the units of that launch), `large` config: profiles/r01f_summary.md.  Used for roofline.traffic only.
-NCU_DRAM_BYTES_PER_UNIT = {"large": {"nl_project": 12.97, "plane_fwd": 31.00, "xpencil": 31.17, "plane_inv": 47.39,
-                                     "nl_scatter": 21.99}}
+# DRAM bytes per launch measured by ncu (dram__bytes_read.sum + dram__bytes_write.sum, `ncu --set full`), one row per
+# kernel family and workload, written from the .ncu-rep of the command named in profiles/r02_ncu_dram.md.  Read at bench
+# time for roofline.traffic; a family without a row has traffic null (never a stale constant).
+NCU_DRAM_CSV = os.path.join(ROOT, "profiles", "r02_ncu_dram.csv")
+
+
+def ncu_dram_bytes_per_unit(workload):
+    """{family: DRAM bytes per state*gridpoint} for `workload` from the committed ncu table; {} if absent."""
+    out = {}
+    try:
+        with open(NCU_DRAM_CSV) as f:
+            head = f.readline().strip().split(",")
+            for line in f:
+                row = dict(zip(head, line.strip().split(",")))
+                if row.get("workload") == workload:
+                    out[row["family"]] = (float(row["dram_read_bytes"]) + float(row["dram_write_bytes"])) / float(row["units_per_launch"])
+    except (OSError, KeyError, ValueError, ZeroDivisionError):
+        return {}
+    return out
 
 
 def alg_bytes(wl):
@@ -300,53 +319,84 @@ def nl_flops_per_unit(wl):
     return 8.0 * cp / wl.cfg.npts
 
 
-def roofline_of(kern_s, units, peak_gbs, peak_src, bytes_per_unit, workload=None, units_per_launch=None, nl_flops=0.0):
-    """Roofline object for the dominant kernel family (largest share of the step) + the fractions of the others."""
+def roofline_of(kern_s, units, peak_gbs, peak_src, bytes_per_unit, workload=None, units_per_launch=None, nl_flops=0.0,
+                step_s=None):
+    """Roofline object for the dominant kernel family (largest share of the step) + the fractions of the others, the
+    step against its pass structure (sum of the families' algorithmic bytes) and against the 32 compulsory bytes."""
     cand = {k: v for k, v in kern_s.items() if bytes_per_unit.get(k) and v > 0}
     if not cand:
         return None
     top = max(cand, key=cand.get)
     achieved = bytes_per_unit[top] * units / cand[top] * 1e-9
+    tot = sum(kern_s.values())
     others = {k: {"achieved": round(bytes_per_unit[k] * units / v * 1e-9, 1),
                   "frac": round(bytes_per_unit[k] * units / v * 1e-9 / peak_gbs, 4),
                   "algorithmic_bytes_per_unit": round(bytes_per_unit[k], 3),
-                  "share_of_step": round(v / sum(kern_s.values()), 4)} for k, v in cand.items()}
+                  "share_of_step": round(v / tot, 4)} for k, v in cand.items()}
     for k in ("nl_project", "nl_scatter"):
         if k in others and nl_flops > 0:
             # the contraction is byte bound (SURVEY 8(d)): its useful FP64 rate is reported, the bytes govern
             others[k]["useful_tflops"] = round(nl_flops * units / cand[k] * 1e-12, 2)
     traffic = None
-    per_unit = NCU_DRAM_BYTES_PER_UNIT.get(workload, {}).get(top)
+    per_unit = ncu_dram_bytes_per_unit(workload).get(top)
     if per_unit and units_per_launch:
         traffic = {"bytes_per_launch": per_unit * units_per_launch, "algorithmic_bytes_per_launch":
                    bytes_per_unit[top] * units_per_launch, "units_per_launch": units_per_launch,
-                   "source": "profiles/r01f_summary.md (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum per "
-                             "state*gridpoint of one launch, scaled to this run's launch size)"}
+                   "source": "profiles/r02_ncu_dram.csv (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum of one "
+                             "launch per state*gridpoint, scaled to this run's launch size)"}
+    t = step_s if step_s else tot
+    pass_bytes = sum(bytes_per_unit[k] for k in cand)
     return {"kernel": top, "bound": "hbm", "achieved": round(achieved, 1), "peak": peak_gbs, "unit": "GB/s",
             "frac": round(achieved / peak_gbs, 4), "traffic": traffic, "peak_source": peak_src,
             "algorithmic_bytes_per_unit": bytes_per_unit[top], "units_per_step": units,
-            "share_of_step": round(cand[top] / sum(kern_s.values()), 4), "all_kernels": others,
+            "share_of_step": round(cand[top] / tot, 4), "all_kernels": others,
+            "pass_structure": {"bytes_per_unit": round(pass_bytes, 2),
+                               "frac": round(pass_bytes * units / t * 1e-9 / peak_gbs, 4),
+                               "note": "sum of the families' algorithmic bytes x units / step time / HBM peak"},
+            "strict_32B": {"frac": round(32.0 * units / t * 1e-9 / peak_gbs, 4),
+                           "note": "compulsory traffic (read psi + write H psi) x units / step time / HBM peak"},
             "note": "achieved = algorithmic bytes of all launches of this family in one step / their summed CUDA-event "
                     "time (separate profiling pass of the same steps)"}
 
 
-def cpu_baseline(cfg, wl, sample_states):
-    """The CPU oracle as it stands on a bounded sample of the same workload (states [0, S))."""
+def cpu_baseline(cfg, wl, sample_states, budget_s=12.0):
+    """The CPU oracle as it stands on a bounded sample of the same workload (states [0, S)); the whole block when that
+    takes less than `budget_s` seconds."""
     from oracle import ref
     cores = ref.num_threads()
     cal = W.states(cfg, 0, min(cfg.nst, cores))
     t0 = time.perf_counter()
     ref.apply_workload(wl, cal, ref.NAIVE_FFT)
     rate = cal.shape[0] * cfg.npts / (time.perf_counter() - t0)
-    S = sample_states or int(min(cfg.nst, max(cores, cores * round(rate * 12.0 / cfg.npts / cores))))
+    S = sample_states or int(min(cfg.nst, max(cores, cores * round(rate * budget_s / cfg.npts / cores))))
     S = max(1, min(S, cfg.nst))
     psi = W.states(cfg, 0, S)
     t0 = time.perf_counter()
     ref.apply_workload(wl, psi, ref.NAIVE_FFT)
     dt = time.perf_counter() - t0
     return {"value": S * cfg.npts / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"states [0,{S}) of '{cfg.name}' ({S} x {cfg.n[0]}^3 points), one ref_apply_hamiltonian call "
-                      f"(naive radix-2/3 FFT back-end, OpenMP over states), {dt:.2f} s"}
+            "sample": f"states [0,{S}) of '{cfg.name}' ({S} of {cfg.nst} states x {cfg.n[0]}^3 points), one "
+                      f"ref_apply_hamiltonian call (naive radix-2/3 FFT back-end, OpenMP over states), {dt:.2f} s"}
+
+
+def cpu_baseline_propagate(cfg, wl, budget_s=15.0):
+    """ref_propagate (Eq. 8 literally) on a bounded state sample of the TDDFT config, all of its steps."""
+    from oracle import ref
+    cores = ref.num_threads()
+    cal = W.states(cfg, 0, min(cfg.nst, cores))
+    t0 = time.perf_counter()
+    ref.propagate_workload(wl, cal, dt=cfg.dt, nsteps=1, backend=ref.NAIVE_FFT)
+    per_state_step = (time.perf_counter() - t0) / cal.shape[0]
+    S = int(max(cores, min(cfg.nst, cores * max(1, round(budget_s / (per_state_step * cfg.nsteps * cores))))))
+    S = min(S, cfg.nst)
+    psi = W.states(cfg, 0, S)
+    t0 = time.perf_counter()
+    ref.propagate_workload(wl, psi, dt=cfg.dt, nsteps=cfg.nsteps, backend=ref.NAIVE_FFT)
+    dt = time.perf_counter() - t0
+    return {"value": S * cfg.npts * 4 * cfg.nsteps / dt, "unit": UNIT + " (H-application equivalents)", "cores": cores,
+            "kind": "oracle", "steps_per_s": cfg.nsteps / dt * S / cfg.nst,
+            "sample": f"states [0,{S}) of '{cfg.name}' ({S} of {cfg.nst} states), one ref_propagate call of {cfg.nsteps} "
+                      f"Taylor-4 steps, {dt:.2f} s; steps_per_s scaled to the whole block"}
 
 
 def run_reference(args):
@@ -379,8 +429,9 @@ def run_reference(args):
     }))
 
 
-def sweep_leg(torch, B, name, flush, reps=7):
-    """One of the non-headline configs at its full size: apply_hamiltonian cold (L2 flushed) and L2-hot."""
+def sweep_leg(torch, B, name, flush, peak, peak_src, cpu, reps=7):
+    """One of the non-headline configs at its full size: apply_hamiltonian cold (L2 flushed) and L2-hot, its roofline
+    object (dominant family, pass-structure and strict fractions) and the CPU oracle beside it."""
     cfg = W.CONFIGS[name]
     wl = W.make(cfg)
     psi, _ = upload_states(torch, cfg, 0, cfg.nst, 0)
@@ -395,6 +446,24 @@ def sweep_leg(torch, B, name, flush, reps=7):
         hot = statistics.median(timed_each(torch, fn, reps, None))
         res = {"states": cfg.nst, "grid": cfg.n[0], "value": units / cold, "ms": cold * 1e3,
                "value_l2_hot": units / hot, "ms_l2_hot": hot * 1e3, "launches": g.last_launch_count()}
+        # per-family times (library events, L2 flushed before every call) -> this config's roofline object
+        g.set_profiling(True)
+        tot = {}
+        for _ in range(5):
+            flush.add_(1.0)
+            fn()
+            torch.cuda.synchronize()
+            for k, v in g.last_kernel_seconds().items():
+                tot[k] = tot.get(k, 0.0) + v / 5
+        g.set_profiling(False)
+        ab = alg_bytes(wl)                           # families that did not run (nl_scatter on whole-plane tiles) drop out
+        res["kernels_s_per_step"] = tot
+        res["roofline"] = roofline_of(tot, units, peak, peak_src, ab, name, units, nl_flops_per_unit(wl), step_s=cold)
+        if res["roofline"] and units * 32 < 100e6:
+            res["roofline"]["note"] += ("; the block and its output fit the 126 MB L2 several times over, the bytes of this "
+                                        "config are not the bound: launch latency is (see ms_per_call_in_a_100_call_loop)")
+        if cpu:
+            res["cpu_baseline"] = cpu_baseline(cfg, wl, 0)
         if name in ("tiny", "small"):
             # launch-latency regime: 100 back-to-back calls, one pair of events around the loop
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -414,7 +483,13 @@ def sweep_leg(torch, B, name, flush, reps=7):
             t = ts[0]
             res["propagate"] = {"steps": cfg.nsteps, "dt": cfg.dt, "seconds": t, "steps_per_s": cfg.nsteps / t,
                                 "h_application_equivalents_per_s": units * 4 * cfg.nsteps / t, "unit": UNIT,
-                                "launches": g.last_launch_count()}
+                                "launches": g.last_launch_count(),
+                                "pass_structure_frac": round((ALG_BYTES["plane_fwd"] + ALG_BYTES["xpencil"] + ALG_BYTES["plane_inv"]
+                                                              + 16.0 + (ab["nl_project"] or 0.0)) * units * 4 * cfg.nsteps / t
+                                                             * 1e-9 / peak, 4),
+                                "strict_32B_frac": round(32.0 * units * 4 * cfg.nsteps / t * 1e-9 / peak, 4)}
+            if cpu:
+                res["propagate"]["cpu_baseline"] = cpu_baseline_propagate(cfg, wl)
             # NEXT-1: ETRS steps (Eq. 6-7) with the shared-powers pair: 8 H applications per step
             # instead of the 12 of three separate exponentials
             work.copy_(psi)
@@ -459,14 +534,15 @@ def sweep_leg(torch, B, name, flush, reps=7):
             torch.cuda.synchronize()
             to = statistics.median(timed_each(torch, lambda: g.overlap(psi, out, out=smat), 5, flush))
             tg = statistics.median(timed_each(torch, lambda: g.overlap(psi, out=smat), 5, flush))
-            peak_tf, peak_src = fp64_tensor_peak()
-            dgemm_tf = fp64_gemm_ceiling(torch)
+            pk = fp64_tensor_peak(torch, B)
             tf = 8.0 * cfg.nst * cfg.nst * cfg.npts / to * 1e-12
-            res["overlap"] = {"seconds": to, "bound": "tensor", "achieved": round(tf, 2), "peak": round(peak_tf, 2),
-                              "unit": "TFLOP/s", "frac": round(tf / peak_tf, 4), "peak_source": peak_src,
+            res["overlap"] = {"seconds": to, "bound": "tensor", "achieved": round(tf, 2), "peak": pk["peak"],
+                              "unit": "TFLOP/s", "frac": round(tf / pk["peak"], 4), "peak_source": pk["peak_source"],
                               "flops": "8 * nst^2 * N_p (complex128 GEMM, K = N_p)", "gram_seconds": tg,
-                              "cublas_dgemm_8192_tflops_same_run": round(dgemm_tf, 2),
-                              "frac_of_cublas_dgemm": round(tf / dgemm_tf, 4),
+                              "fp64_peaks_same_run": pk,
+                              "frac_of_cublas_dgemm": round(tf / pk["cublas_dgemm_8192_tflops"], 4),
+                              "frac_of_mma_issue_loop": round(tf / pk["mma_issue_loop_tflops"], 4),
+                              "frac_of_nominal_45": round(tf / 45.0, 4),
                               "note": "tdh_overlap of two blocks: mma.sync.m8n8k4.f64, 64x64 tiles, split-K with ordered reduction; "
                                       "gram_seconds: one block with itself (tiles below the diagonal mirrored)"}
             work.copy_(psi)
@@ -552,8 +628,9 @@ def main():
     peak, peak_src = measured_peaks()
     cap = max(1, (4 << 30) // (cfg.npts * 16))                                   # the library's default chunk
     states_per_launch = args.chunk or (nst if cap >= nst else (cap // 8 * 8 if cap >= 8 else cap))
-    roof = roofline_of(kern_s, units, peak, peak_src, alg_bytes(wl), args.workload, states_per_launch * cfg.npts,
-                       nl_flops_per_unit(wl))
+    ab = alg_bytes(wl)
+    roof = roofline_of(kern_s, units, peak, peak_src, ab, args.workload, states_per_launch * cfg.npts,
+                       nl_flops_per_unit(wl), step_s=t / args.steps)
 
     # ---- end to end through the host-buffer entry point (pinned host in/out, copies inside the timed region)
     e2e = None
@@ -574,6 +651,9 @@ def main():
         e2e = {"value": D.world * e2e_states * cfg.npts * esteps / te, "unit": UNIT, "h2d_bytes_per_step": nbytes,
                "d2h_bytes_per_step": nbytes, "steps": esteps, "states_per_gpu": e2e_states,
                "ms_per_step": te / esteps * 1e3,
+               "pcie_gbs_per_direction": round(nbytes * esteps / te * 1e-9, 2),
+               "bound": "host link: the step moves the block in and out over PCIe (both directions overlap); the kernels "
+                        "take %.1f ms of the %.1f ms" % (t / args.steps * 1e3 * e2e_states / nst, te / esteps * 1e3),
                "timer": "host perf_counter around the blocking tdh_apply_hamiltonian_host calls, max over ranks"}
         del host_out
     host_in = None
@@ -609,7 +689,7 @@ def main():
         wls = {}
         for name in W.CONFIG_ORDER:
             if name != args.workload:
-                wls[name] = sweep_leg(torch, B, name, flush)
+                wls[name] = sweep_leg(torch, B, name, flush, peak, peak_src, not args.no_cpu_baseline)
         extra["workloads"] = wls
         if "tddft" in wls and "propagate" in wls["tddft"]:
             extra["propagate"] = wls["tddft"].pop("propagate")
@@ -640,9 +720,6 @@ def main():
                        "parallelism": f"states sharded over {D.world} GPU(s), no collective"},
             "e2e": e2e, "gpu_launches": launches, "clocks": clocks, "roofline": roof, "cpu_baseline": cpu,
             "kernels_s_per_step": kern_s,
-            "strict_roofline": {"bytes_per_unit": 32.0, "achieved_gbs": 32.0 * units * args.steps / t * 1e-9,
-                                "frac_of_peak": 32.0 * units * args.steps / t * 1e-9 / peak,
-                                "note": "compulsory traffic of H|psi> (read psi + write Hpsi) x throughput / HBM peak"},
         }
         line.update(extra)
         print(json.dumps(line))

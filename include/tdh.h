@@ -52,14 +52,18 @@ typedef struct { double re, im; } tdh_c128;      /* one complex128 value */
 enum {
     TDH_OK = 0,
     TDH_EINVAL = -1,        /* null pointer, nst < 1, nst > max_states, overlapping in/out, order != 4, ...       */
-    TDH_EUNSUPPORTED = -2,  /* grid size not supported: every n[a] must be one of 16, 32, 48, 64, 96              */
+    TDH_EUNSUPPORTED = -2,  /* grid size not supported: every n[a] must be 2^a 3^b with 4 <= n[a] <= 256; a size limit
+                               of one entry point (stated there)                                                   */
     TDH_ENOMEM = -3,        /* host or device allocation failed                                                   */
     TDH_ECUDA = -4,         /* CUDA runtime error (text in tdh_last_error)                                        */
     TDH_EINDEX = -5         /* sph_idx entry outside [0, n0*n1*n2), or a grid point listed twice for one atom     */
 };
 
 /* Create a grid handle.
- *   n[3]        HOST  grid points per axis; each must be in {16, 32, 48, 64, 96}   (else TDH_EUNSUPPORTED)
+ *   n[3]        HOST  grid points per axis; each must be 2^a 3^b with 4 <= n[a] <= 256 (else TDH_EUNSUPPORTED: a prime
+ *                     factor other than 2 or 3, n[a] < 4, or n[a] > 256).  Grids whose three lengths all lie in
+ *                     {16, 32, 48, 64, 96} (the BASELINE configs and their mixes) run the tuned TMA kernels; any other
+ *                     grid runs the general shared-memory Stockham path (five launches per application, same results)
  *   len[3]      HOST  cell lengths in bohr, > 0
  *   kpt[3]      HOST  Bloch vector k, Cartesian, 1/bohr (reading R1: psi is the periodic part u_k; kinetic 1/2|G+k|^2)
  *   ecut              plane-wave cutoff in Ha for the kinetic term: components with 1/2|G+k|^2 > ecut are zeroed in
@@ -133,7 +137,9 @@ int tdh_hartree(tdh_grid* g, const double* n_dev, double* vh_dev);
  *     S[i][j] = dV sum_p conj(a_i[p]) b_j[p],   i < na, j < nb,   row-major [na][nb] complex128
  * a_dev, b_dev: DEVICE blocks of na / nb states (may be the same block); s_dev: DEVICE, na*nb complex128.
  * A flop-bound complex GEMM on FP64 tensor cores, split over K with a deterministic reduction.  Uses the handle's
- * workspace (na, nb rounded up to 64 must satisfy na*nb <= workspace / 16 bytes).  Asynchronous on the handle's stream. */
+ * workspace (na, nb rounded up to 64 must satisfy na*nb <= workspace / 16 bytes).  n0*n1*n2 must be a multiple of 64
+ * (TDH_EUNSUPPORTED otherwise; this also holds for tdh_rotate and the two calls built on them).  Asynchronous on the
+ * handle's stream. */
 int tdh_overlap(tdh_grid* g, int na, const tdh_c128* a_dev, int nb, const tdh_c128* b_dev, tdh_c128* s_dev);
 
 /* Rotation in the space of states ("rotations in the space of eigenvectors"):
@@ -250,6 +256,11 @@ int tdh_last_launch_count(const tdh_grid* g);
 int tdh_set_profiling(tdh_grid* g, int on);
 int tdh_last_kernel_seconds(const tdh_grid* g, double out[TDH_NKERNELS]);
 const char* tdh_kernel_name(int i);
+
+/* Measurement, not product path: the FP64 tensor-core issue ceiling of the current device in TFLOP/s -- a full grid of
+ * warps issuing independent mma.sync.m8n8k4.f64 from registers; the denominator bench.py uses
+ * for the contraction kernels beside the cuBLAS DGEMM rate of the same run.  Synchronises the device. */
+int tdh_measure_fp64_mma_peak(double* tflops_out);
 
 /* Tuning knob: how many states are pushed through the kernel chain together (0 = library default: as many as the
  * handle's workspace of at most 4 GiB per buffer holds, a multiple of 8 when a block has to be split -- measured on

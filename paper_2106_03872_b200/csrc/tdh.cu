@@ -36,6 +36,7 @@
 #include "tensor_maps.h"
 #include "tile_kernels.cuh"
 #include "xpencil_kernel.cuh"
+#include "generic_fft.cuh"
 
 using tdh::cd;
 
@@ -106,6 +107,11 @@ struct tdh_grid {
     double* d_sd;         // tdh_sd_step: [max_states] eps, [max_states] T, [max_states * 3 * SD_SLICES] partial sums
     int ctas_fwd, ctas_inv[tdh::NL_NCM], ctas_x[5];   // persistent grid sizes (SM count x resident CTAs)
     int ctas_fwd_slab, ctas_x_slab[2];
+
+    // general axis lengths (generic_fft.cuh): any n[a] = 2^a 3^b in [4, 256] outside the tuned set {16, 32, 48, 64, 96}
+    bool generic;
+    tdh::GAxis gax[3];    // z, y, x transforms (index = axis)
+    int nsm;
 
     // slab decomposition (tdh_create_slab_grid): n[0] is then the number of LOCAL planes, nx_fs the full NX
     int nx_fs;            // planes the x transform spans (= n[0] unless this is a slab handle)
@@ -209,9 +215,13 @@ static int create_impl(const int n[3], const double len[3], const double kpt[3],
     for (int a = 0; a < 3; ++a) {
         if (!(len[a] > 0.0) || !std::isfinite(len[a])) return fail(TDH_EINVAL, "tdh_create_grid: len[%d] must be > 0", a);
         if (!std::isfinite(kpt[a])) return fail(TDH_EINVAL, "tdh_create_grid: kpt[%d] not finite", a);
-        if (size_index(n[a]) < 0)
-            return fail(TDH_EUNSUPPORTED, "tdh_create_grid: n[%d] = %d unsupported (supported: 16, 32, 48, 64, 96)", a, n[a]);
+        tdh::GAxis probe;
+        if (!tdh::gfft_factor(n[a], &probe))
+            return fail(TDH_EUNSUPPORTED, "tdh_create_grid: n[%d] = %d unsupported (every axis length must be 2^a 3^b in [4, 256])", a, n[a]);
     }
+    const bool generic = size_index(n[0]) < 0 || size_index(n[1]) < 0 || size_index(n[2]) < 0;
+    if (generic && world > 1)
+        return fail(TDH_EUNSUPPORTED, "tdh_create_slab_grid: slab handles exist for axis lengths 16, 32, 48, 64, 96 only");
     if (world < 1 || world > tdh::SLAB_MAX_WORLD || rank < 0 || rank >= world)
         return fail(TDH_EINVAL, "tdh_create_slab_grid: rank %d / world %d (world <= %d)", rank, world, tdh::SLAB_MAX_WORLD);
     if (world > 1 && (n[0] % world != 0 || n[1] % (2 * world) != 0))
@@ -237,15 +247,22 @@ static int create_impl(const int n[3], const double len[3], const double kpt[3],
     g->have_k = kpt[0] != 0.0 || kpt[1] != 0.0 || kpt[2] != 0.0;
     g->mt = 1;
 
-    bool ok = false;
-    switch (n[2]) {
+    g->generic = generic;
+    for (int a = 0; a < 3; ++a) tdh::gfft_factor(n[a], &g->gax[a]);
+    bool ok = generic;
+    if (generic) {                              // no tiles: whole planes, natural order (identity work layout)
+        memset(&g->tl, 0, sizeof(g->tl));
+        memset(&g->xl, 0, sizeof(g->xl));
+        g->tl.s = 1; g->tl.ppc = 1; g->tl.r1y = 1; g->tl.r2y = n[1]; g->tl.r1z = 1;
+    }
+    if (!generic) switch (n[2]) {
         case 16: ok = tdh::tile_launch_nz16(n[1], &g->tl); break;
         case 32: ok = tdh::tile_launch_nz32(n[1], &g->tl); break;
         case 48: ok = tdh::tile_launch_nz48(n[1], &g->tl); break;
         case 64: ok = tdh::tile_launch_nz64(n[1], &g->tl); break;
         case 96: ok = tdh::tile_launch_nz96(n[1], &g->tl); break;
     }
-    ok = ok && tdh::xpencil_launch(n[0], g->tl.s, &g->xl);
+    ok = ok && (generic || tdh::xpencil_launch(n[0], g->tl.s, &g->xl));
     if (!ok) { delete g; return fail(TDH_EUNSUPPORTED, "tdh_create_grid: no kernel for this grid"); }
     if (world > 1 && g->n[0] % g->tl.ppc != 0) {
         const int ppc = g->tl.ppc;
@@ -255,11 +272,21 @@ static int create_impl(const int n[3], const double len[3], const double kpt[3],
 
     int rc = TDH_OK;
     auto body = [&]() -> int {
-        if (!tdh::encode_tiled_fn()) return fail(TDH_ECUDA, "tdh_create_grid: cuTensorMapEncodeTiled not available from the driver");
-        // persistent grids: SM count x the number of CTAs of each kernel that fit on one SM
         int dev = 0, nsm = 0;
         CU(cudaGetDevice(&dev));
         CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+        g->nsm = nsm;
+        if (generic) {
+            size_t smx = 0;
+            for (int a = 0; a < 3; ++a) smx = std::max(smx, tdh::gfft_smem(g->gax[a]));
+            const void* gf[] = {(const void*)&tdh::gfft_axis_kernel<-1, -1>, (const void*)&tdh::gfft_axis_kernel<+1, -1>,
+                                (const void*)&tdh::gfft_axis_kernel<-1, 0>, (const void*)&tdh::gfft_axis_kernel<-1, 1>,
+                                (const void*)&tdh::gfft_axis_kernel<-1, 2>, (const void*)&tdh::gfft_axis_kernel<-1, 3>,
+                                (const void*)&tdh::gfft_axis_kernel<-1, 4>, (const void*)&tdh::gfft_zinv_epilogue_kernel};
+            for (const void* f : gf) CU(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smx));
+        }
+        if (!generic && !tdh::encode_tiled_fn()) return fail(TDH_ECUDA, "tdh_create_grid: cuTensorMapEncodeTiled not available from the driver");
+        // persistent grids: SM count x the number of CTAs of each kernel that fit on one SM
         constexpr int NK = 9 + tdh::NL_NCM;
         const void* fs[NK] = {g->tl.fwd, g->xl.fused, g->xl.fwd, g->xl.inv, g->xl.poisson, g->xl.teter,
                               g->tl.fwd_slab, g->xl.fused_slab, g->xl.inv_slab};
@@ -270,6 +297,7 @@ static int create_impl(const int n[3], const double len[3], const double kpt[3],
         for (int i = 0; i < tdh::NL_NCM; ++i) { fs[9 + i] = g->tl.inv[i]; sm[9 + i] = g->tl.smem_inv; th[9 + i] = g->tl.threads; }
         int ctas[NK];
         for (int i = 0; i < NK; ++i) {
+            if (generic) { ctas[i] = 0; continue; }
             if (world == 1 && i >= 6 && i < 9) { ctas[i] = 0; continue; }       // slab kernels: slab handles only
             CU(cudaFuncSetAttribute(fs[i], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm[i]));
             CU(cudaFuncSetAttribute(fs[i], cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
@@ -308,7 +336,7 @@ static int create_impl(const int n[3], const double len[3], const double kpt[3],
             std::vector<cd> twy_w(ny / 2);
             for (int ky = 0; ky < ny; ++ky) {
                 const int h = ky / nys, k = ky % nys;
-                const int rho = (k % r1y) * r2y + k / r1y;
+                const int rho = generic ? k : (k % r1y) * r2y + k / r1y;
                 rowmap[ky] = S * rho + h;
                 const double ga = two_pi * freq_index(ky, ny) / len[1] + kpt[1];
                 g2y_w[rowmap[ky]] = ga * ga;
@@ -319,7 +347,7 @@ static int create_impl(const int n[3], const double len[3], const double kpt[3],
             }
             if (S == 1) for (auto& w : twy_w) w = make_double2(1.0, 0.0);
             for (int kz = 0; kz < nz; ++kz) {
-                colmap[kz] = 8 * (kz % r1z) + kz / r1z;
+                colmap[kz] = generic ? kz : 8 * (kz % r1z) + kz / r1z;
                 const double ga = two_pi * freq_index(kz, nz) / len[2] + kpt[2];
                 g2z_w[colmap[kz]] = ga * ga;
             }
@@ -639,6 +667,7 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
     // grids, the records inside plane_inv win on whole-plane tiles.  TDH_NL_MODE=0/1 overrides (tests run both).
     g->nl_mode = g->tl.s == 2 ? 1 : 0;
     if (const char* e = getenv("TDH_NL_MODE")) g->nl_mode = atoi(e) != 0;
+    if (g->generic) g->nl_mode = 1;                 // the record lists address tile cells: tuned grids only
     return TDH_OK;
 }
 
@@ -698,8 +727,60 @@ static int tile_map(tdh_grid* g, const cd* base, int nst, CUtensorMap* m) {
     return TDH_OK;
 }
 
+// ---- general axis lengths (generic_fft.cuh): one batched 1-D transform per launch
+// axis 0 = x, 1 = y, 2 = z of a block of nst states; dir = -1 / +1 plain transform (mode -1), or the x-pencil modes 0..4
+static int launch_gaxis(tdh_grid* g, int kid, int nst, int axis, const cd* in, cd* out, int dir, int mode,
+                        const double* tstate = nullptr) {
+    tdh::GAxis ax = g->gax[axis];
+    const size_t nx = g->n[0], ny = g->n[1], nz = g->n[2];
+    if (axis == 2) { ax.stride = 1; ax.inner = 1; ax.outer = nz; ax.npencils = (size_t)nst * nx * ny; }
+    else if (axis == 1) { ax.stride = nz; ax.inner = nz; ax.outer = ny * nz; ax.npencils = (size_t)nst * nx * nz; }
+    else { ax.stride = ny * nz; ax.inner = ny * nz; ax.outer = nx * ny * nz; ax.npencils = (size_t)nst * ny * nz; }
+    tdh::Kinetic kin;
+    memset(&kin, 0, sizeof(kin));
+    kin.g2x = g->d_g2[0]; kin.g2y_w = g->d_g2y_w; kin.g2z_w = g->d_g2z_w;
+    if (mode == 3) { kin.g2x = g->d_p2x; kin.g2y_w = g->d_p2y_w; kin.g2z_w = g->d_p2z_w; }
+    kin.tstate = tstate;
+    kin.ecut = g->ecut;
+    kin.scale = 1.0 / (double)g->np_total;
+    kin.nz = g->n[2];
+    kin.ny = g->n[1];
+    const cd* tw = g->d_tw[axis];
+    int nxi = g->n[0];
+    const void* f = nullptr;
+    switch (mode) {
+        case -1: f = dir < 0 ? (const void*)&tdh::gfft_axis_kernel<-1, -1> : (const void*)&tdh::gfft_axis_kernel<+1, -1>; break;
+        case 0: f = (const void*)&tdh::gfft_axis_kernel<-1, 0>; break;
+        case 1: f = (const void*)&tdh::gfft_axis_kernel<-1, 1>; break;
+        case 2: f = (const void*)&tdh::gfft_axis_kernel<-1, 2>; break;
+        case 3: f = (const void*)&tdh::gfft_axis_kernel<-1, 3>; break;
+        default: f = (const void*)&tdh::gfft_axis_kernel<-1, 4>; break;
+    }
+    void* args[] = {(void*)&in, (void*)&out, (void*)&ax, (void*)&tw, (void*)&kin, (void*)&nxi};
+    const size_t tiles = (ax.npencils + ax.pt - 1) / ax.pt;
+    const unsigned grid = (unsigned)std::min<size_t>(tiles, (size_t)g->nsm * 8);
+    LAUNCH(kid, f, dim3(grid), dim3(tdh::GF_THREADS), tdh::gfft_smem(ax), args);
+    return TDH_OK;
+}
+
+static int launch_gzinv_epilogue(tdh_grid* g, int nst, const cd* in, cd* out, const tdh::Epilogue& ep) {
+    tdh::GAxis ax = g->gax[2];
+    ax.stride = 1; ax.inner = 1; ax.outer = g->n[2]; ax.npencils = (size_t)nst * g->n[0] * g->n[1];
+    const cd* tw = g->d_tw[2];
+    size_t npts = g->np;
+    void* args[] = {(void*)&in, (void*)&out, (void*)&ax, (void*)&tw, (void*)&ep, (void*)&npts};
+    const size_t tiles = (ax.npencils + ax.pt - 1) / ax.pt;
+    const unsigned grid = (unsigned)std::min<size_t>(tiles, (size_t)g->nsm * 8);
+    LAUNCH(K_PLANE_INV, (const void*)&tdh::gfft_zinv_epilogue_kernel, dim3(grid), dim3(tdh::GF_THREADS), tdh::gfft_smem(ax), args);
+    return TDH_OK;
+}
+
 // to_peers (slab handles): every spectrum row is stored into the Fourier-space slab of the rank that owns it
 static int launch_plane_fwd(tdh_grid* g, int nst, const cd* in, cd* out, bool to_peers = false) {
+    if (g->generic) {
+        int rc = launch_gaxis(g, K_PLANE_FWD, nst, 2, in, out, -1, -1);
+        return rc ? rc : launch_gaxis(g, K_PLANE_FWD, nst, 1, out, out, -1, -1);
+    }
     CUtensorMap map;
     int rc = tile_map(g, in, nst, &map);
     if (rc) return rc;
@@ -722,6 +803,7 @@ static int launch_plane_fwd(tdh_grid* g, int nst, const cd* in, cd* out, bool to
 // values of plane x are stored into the real-space work buffer of the rank that owns x.
 static int launch_xpencil(tdh_grid* g, int nst, const cd* in, cd* out, int mode, const double* tstate = nullptr,
                           bool to_peers = false) {
+    if (g->generic) return launch_gaxis(g, K_XPENCIL, nst, 0, in, out, -1, mode, tstate);
     const bool slab = g->slab_world > 1;
     const int ny = slab ? g->ny_local : g->n[1];                     // rows of the block this launch sees
     const int y0 = slab ? g->slab_rank * g->ny_local : 0;
@@ -757,6 +839,15 @@ static int launch_xpencil(tdh_grid* g, int nst, const cd* in, cd* out, int mode,
 
 // in: work block (spectrum), phi: input block of this application (read only when the epilogue has V or projectors)
 static int launch_plane_inv(tdh_grid* g, int nst, const cd* in, const cd* phi, cd* out, const tdh::Epilogue& ep) {
+    if (g->generic) {
+        // `in` is always one of the handle's scratch blocks: the y transform runs in place on it
+        cd* w = const_cast<cd*>(in);
+        int rc = launch_gaxis(g, K_PLANE_INV, nst, 1, w, w, +1, -1);
+        if (rc) return rc;
+        tdh::Epilogue epl = ep;
+        epl.phi = phi;
+        return launch_gzinv_epilogue(g, nst, w, out, epl);
+    }
     CUtensorMap map_spec, map_phi;
     int rc = tile_map(g, in, nst, &map_spec);
     if (rc) return rc;
@@ -1393,6 +1484,7 @@ extern "C" int tdh_sd_step(tdh_grid* g, int nst, tdh_c128* psi_dev, tdh_c128* wo
 extern "C" int tdh_overlap(tdh_grid* g, int na, const tdh_c128* a_dev, int nb, const tdh_c128* b_dev, tdh_c128* s_dev) {
     if (!g || !a_dev || !b_dev || !s_dev) return fail(TDH_EINVAL, "tdh_overlap: null argument");
     if (na < 1 || nb < 1) return fail(TDH_EINVAL, "tdh_overlap: na, nb must be >= 1");
+    if (g->np % tdh::RT_P != 0) return fail(TDH_EUNSUPPORTED, "tdh_overlap: the GEMM kernels need n0*n1*n2 to be a multiple of %d", tdh::RT_P);
     stats_reset(g);
     const int ti = (na + tdh::OV_T - 1) / tdh::OV_T, tj = (nb + tdh::OV_T - 1) / tdh::OV_T;
     const size_t tile_cells = (size_t)ti * tj * tdh::OV_T * tdh::OV_T;
@@ -1444,6 +1536,7 @@ extern "C" int tdh_rotate(tdh_grid* g, int n_in, const tdh_c128* psi_dev, int n_
                           tdh_c128* out_dev) {
     if (!g || !psi_dev || !m_dev || !out_dev) return fail(TDH_EINVAL, "tdh_rotate: null argument");
     if (n_in < 1 || n_out < 1 || n_out > 65535 * tdh::RT_J) return fail(TDH_EINVAL, "tdh_rotate: bad n_in / n_out");
+    if (g->np % tdh::RT_P != 0) return fail(TDH_EUNSUPPORTED, "tdh_rotate: the GEMM kernels need n0*n1*n2 to be a multiple of %d", tdh::RT_P);
     {
         const char* x = (const char*)psi_dev;
         const char* y = (const char*)out_dev;
