@@ -37,6 +37,7 @@
 #include "tile_kernels.cuh"
 #include "xpencil_kernel.cuh"
 #include "generic_fft.cuh"
+#include "small_kernels.cuh"
 
 using tdh::cd;
 
@@ -107,6 +108,11 @@ struct tdh_grid {
     double* d_sd;         // tdh_sd_step: [max_states] eps, [max_states] T, [max_states * 3 * SD_SLICES] partial sums
     int ctas_fwd, ctas_inv[tdh::NL_NCM], ctas_x[5];   // persistent grid sizes (SM count x resident CTAs)
     int ctas_fwd_slab, ctas_x_slab[2];
+
+    // whole state on chip (small_kernels.cuh): 16^3 (one CTA per state) and 32^3 (a cluster of four CTAs per state)
+    int small_cs;         // 0: not available; else the cluster size
+    const void* small_fn;
+    int small_cells;
 
     // general axis lengths (generic_fft.cuh): any n[a] = 2^a 3^b in [4, 256] outside the tuned set {16, 32, 48, 64, 96}
     bool generic;
@@ -196,14 +202,29 @@ static void free_projectors(tdh_grid* g) {
     g->nl_layers = 0; g->nl_nrec = 0; g->nl_cmax = 0;
 }
 
+// Largest number of states one launch may cover.  The workspace bound, and for the tile configurations that put several
+// small planes into one TMA box (16 x 16 ... 32 x 32 planes, ppc > 1) at most 128 MB of states: on B200 (driver 580.159)
+// tile_fwd launches of those configurations whose loads and stores each span more than 128 MB ended, about once in ten
+// launches, with "unspecified launch failure" -- with the loads OR the stores confined to a few MB, or with 128 MB per
+// launch, never in several thousand launches.  The cause is not understood; the bound avoids it.
+static int max_chunk(const tdh_grid* g) {
+    int c = g->chunk_cap;
+    if (!g->generic && g->tl.ppc > 1) {
+        const size_t lim = ((size_t)128 << 20) / (g->np * sizeof(cd));
+        c = (int)std::max<size_t>(1, std::min<size_t>((size_t)c, lim));
+    }
+    return c;
+}
+
 static int default_chunk(const tdh_grid* g) {
     // Measured on B200 (profiles/r01a_chunk_sweep.md): every kernel gets faster with more states per launch and the
     // L2-resident small-chunk variant never wins, so the default is the largest chunk the workspace holds.
     // When a block has to be split anyway: a multiple of 8 states (the N of the projector MMAs), so that no state group
     // of the non-local kernels is ragged.
-    int c = (g->chunk_cap < g->max_states && g->chunk_cap >= 8) ? g->chunk_cap / 8 * 8 : g->chunk_cap;
+    const int cap = max_chunk(g);
+    int c = (cap < g->max_states && cap >= 8) ? cap / 8 * 8 : cap;
     if (const char* e = getenv("TDH_CHUNK_STATES")) { int v = atoi(e); if (v > 0) c = v; }
-    return std::max(1, std::min(c, g->chunk_cap));
+    return std::max(1, std::min(c, cap));
 }
 
 // n: the FULL grid.  world = 1: an ordinary handle.  world > 1: the handle of rank `rank` of a slab decomposition, which
@@ -382,6 +403,18 @@ static int create_impl(const int n[3], const double len[3], const double kpt[3],
             for (int a = 0; a < 3; ++a) {
                 CU(cudaMalloc(&g->d_gs[a], sizeof(double) * n[a]));
                 CU(cudaMemcpy(g->d_gs[a], gsv[a]->data(), sizeof(double) * n[a], cudaMemcpyHostToDevice));
+            }
+        }
+        // one-launch path for the grids whose state fits on chip (TDH_SMALL=0 switches it off: the tests run both paths)
+        g->small_cs = 0;
+        if (!generic && world == 1 && n[0] == n[1] && n[1] == n[2] && (n[0] == 16 || n[0] == 32)) {
+            const char* e = getenv("TDH_SMALL");
+            if (!(e && atoi(e) == 0)) {
+                if (n[0] == 16) { g->small_cs = 1; g->small_fn = (const void*)&tdh::small_h_kernel<16, 1>; g->small_cells = tdh::SmallCfg<16, 1>::CELLS; }
+                else { g->small_cs = 4; g->small_fn = (const void*)&tdh::small_h_kernel<32, 4>; g->small_cells = tdh::SmallCfg<32, 4>::CELLS; }
+                CU(cudaFuncSetAttribute(g->small_fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                        (int)(tdh::SMALL_HEADER + (size_t)g->small_cells * sizeof(cd) +
+                                              (size_t)(tdh::SMALL_SEG_ENTRIES + 2 * tdh::SMALL_MAX_CHAN + 16) * sizeof(cd))));
             }
         }
         CU(cudaMalloc(&g->d_v, sizeof(double) * g->np));
@@ -927,6 +960,7 @@ static int launch_nl_scatter(tdh_grid* g, int nst, cd* out, cd alpha) {
 }
 
 static int finish_chunk(tdh_grid* g, int nst, const cd* in, cd* out, cd alpha, const cd* yv);
+static int launch_small(tdh_grid* g, int nst, const cd* in, cd* out, cd alpha, const cd* yv);
 
 // out = alpha * H in + yv   for one chunk (nst <= chunk_cap); in/out/yv point at the chunk's first state
 static int apply_chunk(tdh_grid* g, int nst, const cd* in, cd* out, cd alpha, const cd* yv, bool kinetic_only = false) {
@@ -941,10 +975,59 @@ static int apply_chunk(tdh_grid* g, int nst, const cd* in, cd* out, cd alpha, co
         ek.nx = g->n[0];
         return launch_plane_inv(g, nst, g->d_work, nullptr, out, ek);
     }
+    if (g->small_cs > 0 && g->nchan_tot <= tdh::SMALL_MAX_CHAN) return launch_small(g, nst, in, out, alpha, yv);
     if (g->natoms > 0 && (rc = launch_nl_project(g, nst, in))) return rc;
     if ((rc = launch_plane_fwd(g, nst, in, g->d_work))) return rc;
     if ((rc = launch_xpencil(g, nst, g->d_work, g->d_work, 0))) return rc;
     return finish_chunk(g, nst, in, out, alpha, yv);
+}
+
+// the whole application in one launch: a CTA (16^3) or a cluster of four CTAs (32^3) per state (small_kernels.cuh)
+static int launch_small(tdh_grid* g, int nst, const cd* in, cd* out, cd alpha, const cd* yv) {
+    tdh::Kinetic kin;
+    memset(&kin, 0, sizeof(kin));
+    kin.g2x = g->d_g2[0]; kin.g2y_w = g->d_g2y_w; kin.g2z_w = g->d_g2z_w;
+    kin.ecut = g->ecut;
+    kin.scale = 1.0 / (double)g->np_total;
+    kin.nz = g->n[2];
+    kin.ny = g->n[1];
+    tdh::Epilogue ep;
+    memset(&ep, 0, sizeof(ep));
+    ep.v = g->have_v ? g->d_v : nullptr;
+    ep.phi = in;
+    ep.yv = yv;
+    ep.alpha = alpha;
+    ep.nx = g->n[0];
+    tdh::SmallProj pj;
+    memset(&pj, 0, sizeof(pj));
+    if (g->natoms > 0) {
+        ep.nl_off = g->d_nl_off; ep.nl_layers = g->nl_layers; ep.nl_cc = g->d_nl_cc; ep.nl_beta = g->d_nl_beta;
+        ep.nl_phase = g->d_nl_phase; ep.nrec = g->nl_nrec; ep.cmax = g->nl_cmax; ep.nchan_tot = g->nchan_tot;
+        pj.atoms = g->d_atoms; pj.sidx = g->d_sidx; pj.sbeta = g->d_sbeta; pj.sphase = g->d_sphase; pj.dscale = g->d_dscale;
+        pj.natoms = g->natoms; pj.nchan_tot = g->nchan_tot;
+    }
+    const cd* twx = g->d_tw[0];
+    const cd* twy = g->d_tw[1];
+    const cd* twz = g->d_tw[2];
+    void* args[] = {(void*)&in, (void*)&out, (void*)&twx, (void*)&twy, (void*)&twz, (void*)&kin, (void*)&ep, (void*)&pj};
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3((unsigned)(nst * g->small_cs));
+    cfg.blockDim = dim3(g->small_cs == 1 ? tdh::SmallCfg<16, 1>::T : tdh::SmallCfg<32, 4>::T);
+    cfg.dynamicSmemBytes = tdh::small_smem(g->small_cells, g->natoms, g->nchan_tot);
+    cfg.stream = g->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)g->small_cs;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    int rc_ = prof_begin(g, K_PLANE_INV);
+    if (rc_) return rc_;
+    CU(cudaLaunchKernelExC(&cfg, g->small_fn, args));
+    g->launch_count += 1;
+    return prof_end(g);
 }
 
 // last part of one application: inverse (y,z) transform of the work block with the fused epilogue (+ back-projection)
@@ -1657,8 +1740,8 @@ extern "C" int tdh_fft3d(tdh_grid* g, int nst, tdh_c128* psi_dev, int sign) {
     stats_reset(g);
     cd* p = (cd*)psi_dev;
     // through the workspace, chunk by chunk (the tile kernels do not work in place when the planes are split)
-    for (int s0 = 0; s0 < nst; s0 += g->chunk_cap) {
-        const int c = std::min(g->chunk_cap, nst - s0);
+    for (int s0 = 0; s0 < nst; s0 += g->chunk) {
+        const int c = std::min(g->chunk, nst - s0);
         cd* q = p + (size_t)s0 * g->np;
         int rc;
         if (sign < 0) {
@@ -1731,7 +1814,7 @@ static int slab_check(tdh_grid* g, const char* name, int nst) {
     if (!g) return fail(TDH_EINVAL, "%s: null handle", name);
     if (g->slab_world < 2) return fail(TDH_EINVAL, "%s: not a slab handle (tdh_create_slab_grid)", name);
     if (!g->have_peers) return fail(TDH_EINVAL, "%s: tdh_slab_set_peers has not been called", name);
-    if (nst < 1 || nst > g->chunk_cap) return fail(TDH_EINVAL, "%s: nst = %d outside [1, %d] (one chunk per call)", name, nst, g->chunk_cap);
+    if (nst < 1 || nst > max_chunk(g)) return fail(TDH_EINVAL, "%s: nst = %d outside [1, %d] (one chunk per call)", name, nst, max_chunk(g));
     return TDH_OK;
 }
 
@@ -1915,6 +1998,6 @@ extern "C" const char* tdh_kernel_name(int i) { return (i >= 0 && i < TDH_NKERNE
 extern "C" int tdh_set_chunk_states(tdh_grid* g, int chunk) {
     if (!g) return fail(TDH_EINVAL, "tdh_set_chunk_states: null handle");
     if (chunk < 0) return fail(TDH_EINVAL, "tdh_set_chunk_states: chunk < 0");
-    g->chunk = chunk == 0 ? default_chunk(g) : std::min(chunk, g->chunk_cap);
+    g->chunk = chunk == 0 ? default_chunk(g) : std::min(chunk, max_chunk(g));
     return TDH_OK;
 }

@@ -98,7 +98,7 @@ def test_apply_matches_oracle_on_configs(torch_cuda, B, oracle, name, nst, backe
     ref = oracle.apply_workload(wl, psi, backend)
     err = per_state_rel(out, ref)
     assert err.max() < TOL, err
-    assert launches >= 4
+    assert launches >= (1 if cfg.n[0] <= 32 else 4)      # 16^3 and 32^3: the whole application is one launch
 
 
 def test_apply_terms_separately(torch_cuda, B, oracle):
@@ -188,7 +188,7 @@ def test_propagate_matches_oracle_tiny_and_small(torch_cuda, B, oracle):
             g.propagate(d, dt, nsteps)
             torch.cuda.synchronize()
             out = d.cpu().numpy()
-            assert g.last_launch_count() % (nsteps * 4 * 4) == 0     # 4 applications x 4 kernels per step and chunk
+            assert g.last_launch_count() == nsteps * 4              # 4 applications per step, one launch each (on-chip path)
         ref = oracle.propagate_workload(wl, psi, dt=dt, nsteps=nsteps, backend=1)
         assert per_state_rel(out, ref).max() < TOL
         # norms agree with the oracle's (R15: not with 1)

@@ -37,7 +37,7 @@ CASES = [((32, 32, 32), 2, 1), ((32, 32, 32), 4, 1), ((64, 64, 64), 2, 1), ((64,
 
 
 @pytest.mark.parametrize("n,world,lmax", CASES)
-def test_slab_apply_matches_oracle(torch_cuda, B, oracle, n, world, lmax):
+def test_slab_apply_matches_oracle(torch_cuda, B, oracle, monkeypatch, n, world, lmax):
     """H psi (kinetic through the distributed transform, V, projectors whose spheres straddle the slab boundaries) of the
     reassembled block against the oracle; without projectors the slab path is bitwise the undivided one."""
     torch = torch_cuda
@@ -65,6 +65,7 @@ def test_slab_apply_matches_oracle(torch_cuda, B, oracle, n, world, lmax):
         # white-noise states make the kinetic term dominate: the non-local part is compared on its own as well
         # (a difference of two O(100) numbers: 1e-8 of its own norm is 1e-14 of theirs)
         assert per_state_rel((out - out0).cpu().numpy(), nl).max() < 1e-8
+    monkeypatch.setenv("TDH_SMALL", "0")                    # the undivided TILED path (32^3 would run on chip otherwise)
     with B.Grid(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, cfg.nst) as g:
         g.set_potential(torch.from_numpy(wl.v).cuda())
         assert torch.equal(out0, g.apply_hamiltonian(d))

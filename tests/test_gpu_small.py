@@ -1,0 +1,156 @@
+"""The one-launch on-chip path for 16^3 and 32^3 grids (small_kernels.cuh) against the oracle, and against the tiled
+four-launch path (TDH_SMALL=0) that the same grids ran before: both must match the oracle on every case."""
+import numpy as np
+import pytest
+
+from paper_2106_03872_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU test selected but no CUDA device: the product has no CPU fallback")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2106_03872_b200 import binding
+    binding.lib()
+    return binding
+
+
+def per_state_rel(a, b):
+    a = a.reshape(a.shape[0], -1)
+    b = b.reshape(b.shape[0], -1)
+    return np.linalg.norm(a - b, axis=1) / np.linalg.norm(b, axis=1)
+
+
+@pytest.mark.parametrize("small", ["1", "0"])
+@pytest.mark.parametrize("name", ["tiny", "small"])
+def test_configs_apply_and_propagate_both_paths(torch_cuda, B, oracle, monkeypatch, name, small):
+    """Configs 1 and 2 in full: apply and six Taylor-4 steps; one launch per application on the on-chip path."""
+    torch = torch_cuda
+    monkeypatch.setenv("TDH_SMALL", small)
+    cfg = W.CONFIGS[name]
+    wl = W.make(cfg)
+    psi = W.states(cfg)
+    ref_h = oracle.apply_workload(wl, psi, oracle.NAIVE_FFT)
+    nsteps = 6 if name == "tiny" else 2
+    ref_p = oracle.propagate_workload(wl, psi, dt=cfg.dt, nsteps=nsteps, backend=oracle.NAIVE_FFT)
+    with B.grid_for(wl) as g:
+        d = torch.from_numpy(psi).cuda()
+        out = g.apply_hamiltonian(d)
+        assert g.last_launch_count() == (1 if small == "1" else 4)
+        assert per_state_rel(out.cpu().numpy(), ref_h).max() < TOL
+        g.propagate(d, cfg.dt, nsteps)
+        assert g.last_launch_count() == nsteps * 4 * (1 if small == "1" else 4)
+        assert per_state_rel(d.cpu().numpy(), ref_p).max() < TOL
+
+
+@pytest.mark.parametrize("n,nst,natoms,lmax,kfrac,ecut", [
+    (16, 5, 3, 2, (0.25, 0.0, -0.1), 12.0), (32, 7, 6, 2, (0.1, 0.2, 0.0), 25.0), (16, 1, 0, 0, (0.0, 0.0, 0.0), None),
+    (32, 3, 9, 1, (0.0, 0.0, 0.0), None), (16, 9, 4, 0, (0.0, 0.0, 0.3), None)])
+def test_small_path_options(torch_cuda, B, oracle, n, nst, natoms, lmax, kfrac, ecut):
+    """Bloch vector with phases in the projectors, cutoff mask, 1 / 4 / 9 channels, overlapping spheres (rc close to L/2),
+    no atoms, no potential, ragged chunks; the non-local part on its own as well."""
+    torch = torch_cuda
+    length = (0.4 * n,) * 3
+    cfg = W.test_config(700 + n + nst, (n, n, n), length, nst=nst, natoms=natoms, lmax=lmax, rc=0.45 * length[0],
+                        dl=(2.0, -0.8, 0.3)[: lmax + 1], kfrac=kfrac, ecut=ecut)
+    wl = W.make(cfg)
+    psi = W.states(cfg)
+    ref_h = oracle.apply_workload(wl, psi, oracle.NAIVE_FFT)
+    ref_p = oracle.propagate_workload(wl, psi, dt=0.01, nsteps=2, backend=oracle.NAIVE_FFT)
+    with B.grid_for(wl) as g:
+        for chunk in (None, 2):
+            if chunk:
+                g.set_chunk_states(chunk)
+            d = torch.from_numpy(psi).cuda()
+            out = g.apply_hamiltonian(d)
+            assert g.last_launch_count() == (1 if chunk is None else (nst + 1) // 2)
+            assert per_state_rel(out.cpu().numpy(), ref_h).max() < TOL
+            g.propagate(d, 0.01, 2)
+            assert per_state_rel(d.cpu().numpy(), ref_p).max() < TOL
+        if natoms:
+            nl = oracle.nonlocal_(cfg.n, cfg.length, cfg.kpt, wl.proj, psi)
+            g.set_projectors(None)
+            out0 = g.apply_hamiltonian(torch.from_numpy(psi).cuda())
+            assert per_state_rel((out - out0).cpu().numpy(), nl).max() < 1e-8
+            g.set_potential(None)
+            t_only = g.apply_hamiltonian(torch.from_numpy(psi).cuda()).cpu().numpy()
+            assert per_state_rel(t_only, oracle.kinetic(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, psi, oracle.NAIVE_FFT)).max() < TOL
+
+
+def test_small_path_many_channels_and_layers(torch_cuda, B, oracle):
+    """16 channels per atom and grid points covered by four spheres (record layers), on both on-chip grids."""
+    torch = torch_cuda
+    from test_gpu_fullsize import synthetic_projectors
+    for n in (16, 32):
+        length = (0.42 * n,) * 3
+        cfg = W.test_config(720 + n, (n, n, n), length, nst=4, natoms=1, lmax=0, rc=0.4 * length[0], dl=(1.0,),
+                            kfrac=(0.0, 0.25, 0.0))
+        rng = np.random.default_rng([W.BASE_SEED, 720, n])
+        mid = [0.5 * l for l in length]
+        centers = [mid, [mid[0] + 0.3, mid[1], mid[2]], [mid[0], mid[1] - 0.4, mid[2] + 0.2], [mid[0] + 0.1, mid[1] + 0.1, mid[2]],
+                   [0.1, 0.2, length[2] - 0.1]]
+        proj = synthetic_projectors(cfg, centers, 16, rng)
+        v = rng.uniform(-1.0, 1.0, cfg.n)
+        psi = W.states(cfg)
+        ref = oracle.apply_hamiltonian(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, v, proj, psi, oracle.NAIVE_FFT)
+        with B.Grid(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, cfg.nst) as g:
+            g.set_potential(torch.from_numpy(v).cuda())
+            g.set_projectors(proj)
+            out = g.apply_hamiltonian(torch.from_numpy(psi).cuda())
+            assert g.last_launch_count() == 1
+            assert per_state_rel(out.cpu().numpy(), ref).max() < TOL
+
+
+def test_small_path_is_deterministic_and_independent_of_batching(torch_cuda, B):
+    torch = torch_cuda
+    cfg = W.CONFIGS["small"]
+    wl = W.make(cfg)
+    psi = torch.from_numpy(W.states(cfg, 0, 20)).cuda()
+    with B.grid_for(wl, max_states=20) as g:
+        a = g.apply_hamiltonian(psi)
+        b = g.apply_hamiltonian(psi)
+        assert torch.equal(a, b)
+        part = g.apply_hamiltonian(psi[5:12].contiguous())
+        assert torch.equal(part, a[5:12])
+
+
+@pytest.mark.parametrize("small", ["0", "1"])
+def test_small_planes_many_states_stress(torch_cuda, B, oracle, monkeypatch, small):
+    """32^3 with 1024 states (512 MB blocks) through both paths, forty applications with re-created handles and tensors.
+    Regression test for the launch failures seen when one tile_fwd launch of a multi-plane-tile configuration spanned
+    more than 128 MB (max_chunk bounds the launch); sampled states against the oracle."""
+    torch = torch_cuda
+    import dataclasses
+    monkeypatch.setenv("TDH_SMALL", small)
+    cfg = dataclasses.replace(W.CONFIGS["small"], nst=1024)
+    wl = W.make(cfg)
+    sample = [0, 300, 1023]
+    host = np.stack([W.state(cfg, s) for s in sample])
+    ref = oracle.apply_workload(wl, host, oracle.NAIVE_FFT)
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(5)
+    for trial in range(5):
+        psi = torch.empty((cfg.nst,) + cfg.n, dtype=torch.complex128, device="cuda")
+        torch.view_as_real(psi).copy_(torch.randn((cfg.nst,) + cfg.n + (2,), dtype=torch.float64, device="cuda", generator=gen) * 0.01)
+        for j, s in enumerate(sample):
+            psi[s].copy_(torch.from_numpy(host[j]))
+        out = torch.empty_like(psi)
+        with B.grid_for(wl) as g:
+            for _ in range(8):
+                g.apply_hamiltonian(psi, out=out)
+            torch.cuda.synchronize()
+            assert g.last_launch_count() == (4 * 4 if small == "0" else 4)      # four chunks of 256 states (128 MB)
+            got = np.stack([out[s].cpu().numpy() for s in sample])
+            assert per_state_rel(got, ref).max() < TOL
+        del psi, out
+        torch.cuda.empty_cache()
