@@ -249,6 +249,9 @@ int tdh_fft3d(tdh_grid* g, int nst, tdh_c128* psi_dev, int sign);
 /* Number of kernel launches the last tdh_apply_hamiltonian / tdh_propagate / *_host call of this handle enqueued. */
 int tdh_last_launch_count(const tdh_grid* g);
 
+/* Jacobi sweeps the last tdh_subspace_diag call of this handle needed (when it was given eig_host). */
+int tdh_last_jacobi_sweeps(const tdh_grid* g);
+
 /* Seconds (device time, CUDA events on the handle's stream) spent in each kernel family during the last call, when
  * profiling was switched on with tdh_set_profiling(g, 1); profiling inserts events and synchronises at the end.
  * out[0..TDH_NKERNELS-1]; order given by tdh_kernel_name(i).  Off by default. */

@@ -27,7 +27,7 @@ SYMBOLS = (
     "tdh_create_grid", "tdh_destroy_grid", "tdh_set_potential", "tdh_set_projectors", "tdh_apply_hamiltonian",
     "tdh_propagate", "tdh_taylor_pair", "tdh_etrs_step", "tdh_density", "tdh_hartree", "tdh_overlap", "tdh_rotate", "tdh_orthonormalize", "tdh_subspace_diag", "tdh_sd_step", "tdh_gradient", "tdh_forces", "tdh_apply_hamiltonian_host", "tdh_propagate_host", "tdh_fft3d", "tdh_last_launch_count",
     "tdh_create_slab_grid", "tdh_slab_buffers", "tdh_slab_set_peers", "tdh_slab_apply_phase", "tdh_slab_fft_phase", "tdh_work_layout",
-    "tdh_ipc_export", "tdh_ipc_import", "tdh_ipc_close", "tdh_measure_fp64_mma_peak",
+    "tdh_ipc_export", "tdh_ipc_import", "tdh_ipc_close", "tdh_measure_fp64_mma_peak", "tdh_last_jacobi_sweeps",
     "tdh_set_profiling", "tdh_last_kernel_seconds", "tdh_kernel_name", "tdh_set_chunk_states", "tdh_last_error",
 )
 NKERNELS = 5
@@ -85,6 +85,7 @@ def lib() -> C.CDLL:
     l.tdh_ipc_import.argtypes = [C.c_char_p, C.POINTER(vp)]
     l.tdh_ipc_close.argtypes = [vp]
     l.tdh_measure_fp64_mma_peak.argtypes = [C.POINTER(d)]
+    l.tdh_last_jacobi_sweeps.argtypes = [vp]
     l.tdh_set_profiling.argtypes = [vp, i]
     l.tdh_last_kernel_seconds.argtypes = [vp, C.POINTER(d)]
     l.tdh_kernel_name.argtypes = [i]
@@ -391,6 +392,9 @@ class Grid:
         return psi_host
 
     # -- statistics / knobs
+    def last_jacobi_sweeps(self) -> int:
+        return int(lib().tdh_last_jacobi_sweeps(self._h))
+
     def last_launch_count(self) -> int:
         return int(lib().tdh_last_launch_count(self._h))
 

@@ -4,12 +4,19 @@
 // once, a sweep is n - 1 steps.  For a pair with a_pq = |a_pq| e^{i phi}, tau = (a_qq - a_pp) / (2 |a_pq|),
 // t = sign(tau) / (|tau| + sqrt(1 + tau^2)), c = 1 / sqrt(1 + t^2), s = t c, the unitary
 //     J_pp = c,  J_pq = s,  J_qp = -s e^{-i phi},  J_qq = c e^{-i phi}
-// zeroes a_pq in J^H A J.  One cooperative launch (every CTA resident) runs all sweeps; a step is three phases
-// separated by grid barriers: the rotation parameters of the step's pairs from the current matrix, the column update
-// A <- A J and V <- V J, the row update A <- J^H A.  The matrix (16 MB at n = 1024) lives in L2; every access that
-// crosses CTAs goes through ld.global.cg / st.global.cg.  Sweeps stop when the largest rotated |a_pq| of a sweep is
-// below 1e-15 of the largest matrix element (checked identically by every CTA), at most 40 sweeps.
-// The O(n^3) work of this kernel is small beside the O(n^2 N_p) of the GEMMs around it.
+// zeroes a_pq in J^H A J.  One cooperative launch (every CTA resident) runs all sweeps with ONE grid barrier per step:
+//   * every CTA computes the rotations of all n/2 pairs of the step itself (three matrix elements per pair, into shared
+//     memory) -- redundant arithmetic instead of a phase and a barrier of its own; the largest rotated |a_pq| of a sweep
+//     is therefore known to every CTA without any communication;
+//   * the two-sided update is done per 2 x 2 block (row pair P, column pair C): B' = J_P^H B J_C, read from one copy of
+//     the matrix and written to the other (ping-pong), so no CTA can read an element another CTA has already replaced;
+//     V <- V J in place (no CTA reads V).
+// The arithmetic per element (column rotation, then row rotation) is that of the three-phase version of round 1 (65 ms
+// for n = 512: three barriers per step).  The matrices (2 x 4 MB + 4 MB at n = 512) live in L2; every access that
+// crosses CTAs goes through ld.global.cg / st.global.cg.  Threshold Jacobi: elements below JACOBI_TOL of the largest
+// matrix element are not rotated, a step without any rotation costs no update and no barrier (the last, verifying sweep
+// is therefore cheap), and the sweeps stop after one in which nothing was rotated; at most JACOBI_MAX_SWEEPS sweeps;
+// ctl[4] receives the sweeps used and ctl[5] = 1 when the last sweep still rotated (the host reports that as an error).
 #pragma once
 #include "fft_codelets.cuh"
 
@@ -25,28 +32,24 @@ __device__ __forceinline__ void jacobi_pair(int m, int r, int k, int& p, int& q)
 }
 
 struct __align__(16) JacobiRot { double c, s, cph, sph; };      // e^{i phi} = cph + i sph
-// the rotations are written by one CTA and read by all others in the next phase: through L2
-__device__ __forceinline__ JacobiRot ld_rot(const JacobiRot* p) {
-    const double2 a = __ldcg(reinterpret_cast<const double2*>(p)), b = __ldcg(reinterpret_cast<const double2*>(p) + 1);
-    JacobiRot r;
-    r.c = a.x; r.s = a.y; r.cph = b.x; r.sph = b.y;
-    return r;
-}
-__device__ __forceinline__ void st_rot(JacobiRot* p, const JacobiRot& r) {
-    __stcg(reinterpret_cast<double2*>(p), make_double2(r.c, r.s));
-    __stcg(reinterpret_cast<double2*>(p) + 1, make_double2(r.cph, r.sph));
-}
+constexpr int JACOBI_MAX_SWEEPS = 40;
+constexpr int JACOBI_T = 512;
+constexpr double JACOBI_TOL = 1e-14;      // off-diagonal elements below JACOBI_TOL * max|a_ij| are not rotated
 
-// a: n x n Hermitian (row-major), overwritten; v: n x n, receives the eigenvectors as columns (not yet sorted);
-// rot: scratch [m/2]; ctl (8 words, zeroed): [0] grid-barrier counter, [2..3] (64-bit) largest |a_pq| of the sweep,
-// [4] sweeps used
-__global__ void __launch_bounds__(256)
-jacobi_eigh_kernel(cd* __restrict__ a, cd* __restrict__ v, int n, JacobiRot* __restrict__ rot, unsigned* __restrict__ ctl)
+// a: n x n Hermitian (row-major), overwritten; a2: second n x n buffer (ping-pong); v: n x n, receives the eigenvectors as
+// columns (not yet sorted); ctl (8 words, zeroed): [0] grid-barrier counter, [2..3] (64-bit) largest |a_ij| of the input,
+// [4] sweeps used, [5] not converged.  On return the diagonal of `a` holds the eigenvalues.
+// Dynamic shared memory: (n + 1) / 2 JacobiRot.
+__global__ void __launch_bounds__(JACOBI_T)
+jacobi_eigh_kernel(cd* __restrict__ a, cd* __restrict__ a2, cd* __restrict__ v, int n, unsigned* __restrict__ ctl)
 {
+    extern __shared__ __align__(16) unsigned char jsm[];
+    JacobiRot* srot = reinterpret_cast<JacobiRot*>(jsm);
+    __shared__ double red[JACOBI_T / 32];
     const int tid = threadIdx.x;
     const size_t gtid = (size_t)blockIdx.x * blockDim.x + tid, gsize = (size_t)gridDim.x * blockDim.x;
     const int m = n + (n & 1), half = m / 2;
-    unsigned long long* sweep_max = reinterpret_cast<unsigned long long*>(ctl + 2);
+    unsigned long long* scale_word = reinterpret_cast<unsigned long long*>(ctl + 2);
     unsigned epoch = 0;
     auto grid_barrier = [&]() {
         __syncthreads();
@@ -66,26 +69,30 @@ jacobi_eigh_kernel(cd* __restrict__ a, cd* __restrict__ v, int n, JacobiRot* __r
         const cd x = __ldcg(a + e);
         mx = fmax(mx, fmax(fabs(x.x), fabs(x.y)));
     }
-    atomicMax(sweep_max, (unsigned long long)__double_as_longlong(mx));
+    atomicMax(scale_word, (unsigned long long)__double_as_longlong(mx));
     grid_barrier();
-    const double scale = __longlong_as_double((long long)*((volatile unsigned long long*)sweep_max));
-    grid_barrier();
-    if (gtid == 0) *sweep_max = 0ull;
-    grid_barrier();
+    const double scale = __longlong_as_double((long long)*((volatile unsigned long long*)scale_word));
+    const double thr = JACOBI_TOL * scale;
+    cd* cur = a;
+    cd* nxt = a2;
     int sweep = 0;
-    for (; sweep < 40; ++sweep) {
+    bool converged = false;
+    for (; sweep < JACOBI_MAX_SWEEPS && !converged; ++sweep) {
+        double tmax = 0.0;                                   // this thread's largest rotated |a_pq| of the sweep
         for (int r = 0; r < m - 1; ++r) {
-            // ---- phase 0: rotation parameters of this step's pairs
-            for (size_t k = gtid; k < (size_t)half; k += gsize) {
+            // ---- rotations of this step's pairs, computed by every CTA from the current matrix
+            int any = 0;
+            for (int k = tid; k < half; k += JACOBI_T) {
                 int p, q;
-                jacobi_pair(m, r, (int)k, p, q);
+                jacobi_pair(m, r, k, p, q);
                 JacobiRot jr = {1.0, 0.0, 1.0, 0.0};
                 if (q < n) {
-                    const double app = __ldcg(a + (size_t)p * n + p).x, aqq = __ldcg(a + (size_t)q * n + q).x;
-                    const cd apq = __ldcg(a + (size_t)p * n + q);
-                    const double mag = hypot(apq.x, apq.y);
-                    if (mag > 0.0) {
-                        atomicMax(sweep_max, (unsigned long long)__double_as_longlong(mag));
+                    const double app = __ldcg(cur + (size_t)p * n + p).x, aqq = __ldcg(cur + (size_t)q * n + q).x;
+                    const cd apq = __ldcg(cur + (size_t)p * n + q);
+                    const double mag = sqrt(apq.x * apq.x + apq.y * apq.y);
+                    if (mag > thr) {                         // threshold Jacobi: smaller elements are left alone
+                        tmax = fmax(tmax, mag);
+                        any = 1;
                         const double tau = (aqq - app) / (2.0 * mag);
                         const double t = (tau >= 0.0 ? 1.0 : -1.0) / (fabs(tau) + sqrt(1.0 + tau * tau));
                         jr.c = 1.0 / sqrt(1.0 + t * t);
@@ -94,50 +101,90 @@ jacobi_eigh_kernel(cd* __restrict__ a, cd* __restrict__ v, int n, JacobiRot* __r
                         jr.sph = apq.y / mag;
                     }
                 }
-                st_rot(rot + k, jr);
+                srot[k] = jr;
             }
-            grid_barrier();
-            // ---- phase 1: columns p, q of A and of V:  [x, y] <- [c x - s e^{-i phi} y,  s x + c e^{-i phi} y]
-            for (size_t e = gtid; e < (size_t)n * half; e += gsize) {
-                const int row = (int)(e / half), k = (int)(e % half);
-                int p, q;
-                jacobi_pair(m, r, k, p, q);
-                if (q >= n) continue;
-                const JacobiRot jr = ld_rot(rot + k);
-                if (jr.s == 0.0) continue;
-#pragma unroll
-                for (int which = 0; which < 2; ++which) {
-                    cd* mat = which ? v : a;
-                    const cd x = __ldcg(mat + (size_t)row * n + p), y = __ldcg(mat + (size_t)row * n + q);
-                    const cd ey = make_double2(y.x * jr.cph + y.y * jr.sph, y.y * jr.cph - y.x * jr.sph);   // e^{-i phi} y
-                    __stcg(mat + (size_t)row * n + p, make_double2(jr.c * x.x - jr.s * ey.x, jr.c * x.y - jr.s * ey.y));
-                    __stcg(mat + (size_t)row * n + q, make_double2(jr.s * x.x + jr.c * ey.x, jr.s * x.y + jr.c * ey.y));
+            // a step without any rotation changes nothing: no update, no barrier (every CTA takes the same decision, it
+            // has computed the same rotations from the same matrix)
+            if (!__syncthreads_or(any)) continue;
+            // ---- one pass per thread over its items: 2 x 2 blocks of A (row pair kp, column pair kc), B' = J_P^H (B J_C),
+            //      cur -> nxt, and (row, column pair) items of V <- V J in place.  All loads of an item pair are issued
+            //      before the arithmetic (one L2 round trip per pass).
+            const int na_items = half * half, nv_items = n * half;         // n <= 1024: 32-bit index arithmetic
+            for (int e = (int)gtid; e < na_items || e < nv_items; e += (int)gsize) {
+                const bool do_a = e < na_items, do_v = e < nv_items;
+                int p = 0, q = 0, cr = 0, cs = 0, vp = 0, vq = 0, vrow = 0;
+                bool qv = false, sv = false;
+                JacobiRot jp = {1.0, 0.0, 1.0, 0.0}, jc = jp, jv = jp;
+                const cd z0 = make_double2(0.0, 0.0);
+                cd b11 = z0, b12 = z0, b21 = z0, b22 = z0, vx = z0, vy = z0;
+                if (do_a) {
+                    const int kp = e / half, kc = e % half;
+                    jacobi_pair(m, r, kp, p, q);
+                    jacobi_pair(m, r, kc, cr, cs);
+                    qv = q < n; sv = cs < n;
+                    jp = srot[kp]; jc = srot[kc];
+                    b11 = __ldcg(cur + (size_t)p * n + cr);
+                    if (sv) b12 = __ldcg(cur + (size_t)p * n + cs);
+                    if (qv) b21 = __ldcg(cur + (size_t)q * n + cr);
+                    if (qv && sv) b22 = __ldcg(cur + (size_t)q * n + cs);
+                }
+                bool v_on = false;
+                if (do_v) {
+                    vrow = e / half;
+                    const int k = e % half;
+                    jacobi_pair(m, r, k, vp, vq);
+                    jv = srot[k];
+                    v_on = vq < n && jv.s != 0.0;
+                    if (v_on) { vx = __ldcg(v + (size_t)vrow * n + vp); vy = __ldcg(v + (size_t)vrow * n + vq); }
+                }
+                if (do_a) {
+                    if (jc.s != 0.0) {       // columns: [x, y] <- [c x - s e^{-i phi} y,  s x + c e^{-i phi} y]
+                        const cd e1 = make_double2(b12.x * jc.cph + b12.y * jc.sph, b12.y * jc.cph - b12.x * jc.sph);
+                        const cd e2 = make_double2(b22.x * jc.cph + b22.y * jc.sph, b22.y * jc.cph - b22.x * jc.sph);
+                        const cd n11 = make_double2(jc.c * b11.x - jc.s * e1.x, jc.c * b11.y - jc.s * e1.y);
+                        const cd n12 = make_double2(jc.s * b11.x + jc.c * e1.x, jc.s * b11.y + jc.c * e1.y);
+                        const cd n21 = make_double2(jc.c * b21.x - jc.s * e2.x, jc.c * b21.y - jc.s * e2.y);
+                        const cd n22 = make_double2(jc.s * b21.x + jc.c * e2.x, jc.s * b21.y + jc.c * e2.y);
+                        b11 = n11; b12 = n12; b21 = n21; b22 = n22;
+                    }
+                    if (jp.s != 0.0) {       // rows: [x; y] <- [c x - s e^{+i phi} y;  s x + c e^{+i phi} y]
+                        const cd e1 = make_double2(b21.x * jp.cph - b21.y * jp.sph, b21.y * jp.cph + b21.x * jp.sph);
+                        const cd e2 = make_double2(b22.x * jp.cph - b22.y * jp.sph, b22.y * jp.cph + b22.x * jp.sph);
+                        const cd n11 = make_double2(jp.c * b11.x - jp.s * e1.x, jp.c * b11.y - jp.s * e1.y);
+                        const cd n21 = make_double2(jp.s * b11.x + jp.c * e1.x, jp.s * b11.y + jp.c * e1.y);
+                        const cd n12 = make_double2(jp.c * b12.x - jp.s * e2.x, jp.c * b12.y - jp.s * e2.y);
+                        const cd n22 = make_double2(jp.s * b12.x + jp.c * e2.x, jp.s * b12.y + jp.c * e2.y);
+                        b11 = n11; b21 = n21; b12 = n12; b22 = n22;
+                    }
+                    __stcg(nxt + (size_t)p * n + cr, b11);
+                    if (sv) __stcg(nxt + (size_t)p * n + cs, b12);
+                    if (qv) __stcg(nxt + (size_t)q * n + cr, b21);
+                    if (qv && sv) __stcg(nxt + (size_t)q * n + cs, b22);
+                }
+                if (v_on) {
+                    const cd ey = make_double2(vy.x * jv.cph + vy.y * jv.sph, vy.y * jv.cph - vy.x * jv.sph);   // e^{-i phi} y
+                    __stcg(v + (size_t)vrow * n + vp, make_double2(jv.c * vx.x - jv.s * ey.x, jv.c * vx.y - jv.s * ey.y));
+                    __stcg(v + (size_t)vrow * n + vq, make_double2(jv.s * vx.x + jv.c * ey.x, jv.s * vx.y + jv.c * ey.y));
                 }
             }
             grid_barrier();
-            // ---- phase 2: rows p, q of A:  [x; y] <- [c x - s e^{i phi} y;  s x + c e^{i phi} y]
-            for (size_t e = gtid; e < (size_t)half * n; e += gsize) {
-                const int k = (int)(e / n), col = (int)(e % n);
-                int p, q;
-                jacobi_pair(m, r, k, p, q);
-                if (q >= n) continue;
-                const JacobiRot jr = ld_rot(rot + k);
-                if (jr.s == 0.0) continue;
-                const cd x = __ldcg(a + (size_t)p * n + col), y = __ldcg(a + (size_t)q * n + col);
-                const cd ey = make_double2(y.x * jr.cph - y.y * jr.sph, y.y * jr.cph + y.x * jr.sph);       // e^{+i phi} y
-                __stcg(a + (size_t)p * n + col, make_double2(jr.c * x.x - jr.s * ey.x, jr.c * x.y - jr.s * ey.y));
-                __stcg(a + (size_t)q * n + col, make_double2(jr.s * x.x + jr.c * ey.x, jr.s * x.y + jr.c * ey.y));
-            }
-            grid_barrier();
+            cd* t = cur; cur = nxt; nxt = t;
         }
-        // ---- end of the sweep: every CTA reads the same maximum, then it is reset behind a barrier
-        const double big = __longlong_as_double((long long)*((volatile unsigned long long*)sweep_max));
-        grid_barrier();
-        if (gtid == 0) *sweep_max = 0ull;
-        grid_barrier();
-        if (big <= 1e-15 * scale) { ++sweep; break; }
+        // ---- end of the sweep: every CTA holds the same maximum (each computed every rotation)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) tmax = fmax(tmax, __shfl_xor_sync(0xffffffffu, tmax, o));
+        if ((tid & 31) == 0) red[tid >> 5] = tmax;
+        __syncthreads();
+        double big = 0.0;
+        for (int w = 0; w < JACOBI_T / 32; ++w) big = fmax(big, red[w]);
+        __syncthreads();
+        converged = big <= thr;                              // no element above the threshold was met in this sweep
     }
-    if (gtid == 0) ctl[4] = (unsigned)sweep;
+    // the eigenvalues are read from the diagonal of `a`
+    if (cur != a) {
+        for (size_t i = gtid; i < (size_t)n; i += gsize) a[i * n + i] = __ldcg(cur + i * n + i);
+    }
+    if (gtid == 0) { ctl[4] = (unsigned)sweep; ctl[5] = converged ? 0u : 1u; }
 }
 
 // eigenvalues ascending and the matching column permutation of v: w[rank] = a[i][i], vout[:, rank] = v[:, i]

@@ -102,8 +102,8 @@ struct tdh_grid {
     cd* d_small[3];       // n x n scratch of tdh_orthonormalize ([0] overlap / Cholesky factor, [2] rotation), grown on demand
     int small_n;
     int* d_status;        // Cholesky status word
-    tdh::JacobiRot* d_rot;  // tdh_subspace_diag: rotations of one Jacobi step
     unsigned* d_ctl;      // tdh_subspace_diag: barrier counter, sweep maximum, sweeps used
+    int jacobi_sweeps;    // sweeps of the last tdh_subspace_diag call that returned its eigenvalues
     double* d_w;          // tdh_subspace_diag: eigenvalues
     double* d_sd;         // tdh_sd_step: [max_states] eps, [max_states] T, [max_states * 3 * SD_SLICES] partial sums
     int ctas_fwd, ctas_inv[tdh::NL_NCM], ctas_x[5];   // persistent grid sizes (SM count x resident CTAs)
@@ -464,7 +464,7 @@ extern "C" int tdh_destroy_grid(tdh_grid* g) {
     for (int a = 0; a < 3; ++a) cudaFree(g->d_gs[a]);
     cudaFree(g->d_gd);
     for (int i = 0; i < 3; ++i) cudaFree(g->d_small[i]);
-    cudaFree(g->d_status); cudaFree(g->d_sd); cudaFree(g->d_rot); cudaFree(g->d_ctl); cudaFree(g->d_w);
+    cudaFree(g->d_status); cudaFree(g->d_sd); cudaFree(g->d_ctl); cudaFree(g->d_w);
     cudaFree(g->d_work); cudaFree(g->d_phi[0]); cudaFree(g->d_phi[1]); cudaFree(g->d_fs);
     for (int i = 0; i < 2; ++i) {
         cudaFree(g->d_hin[i]); cudaFree(g->d_hout[i]);
@@ -1564,7 +1564,17 @@ extern "C" int tdh_sd_step(tdh_grid* g, int nst, tdh_c128* psi_dev, tdh_c128* wo
 }
 
 // S = dV a^H b on FP64 tensor cores, split-K partials in the work buffer (overlap_kernels.cuh)
+static int overlap_impl(tdh_grid* g, int na, const tdh_c128* a_dev, int nb, const tdh_c128* b_dev, tdh_c128* s_dev,
+                        bool result_is_hermitian);
+
 extern "C" int tdh_overlap(tdh_grid* g, int na, const tdh_c128* a_dev, int nb, const tdh_c128* b_dev, tdh_c128* s_dev) {
+    return overlap_impl(g, na, a_dev, nb, b_dev, s_dev, false);
+}
+
+// result_is_hermitian: the caller knows that dV a^H b is Hermitian up to rounding (b = H a with a Hermitian H): only the
+// tiles on and above the diagonal are computed, the others are their conjugate transposes (as for the Gram matrix)
+static int overlap_impl(tdh_grid* g, int na, const tdh_c128* a_dev, int nb, const tdh_c128* b_dev, tdh_c128* s_dev,
+                        bool result_is_hermitian) {
     if (!g || !a_dev || !b_dev || !s_dev) return fail(TDH_EINVAL, "tdh_overlap: null argument");
     if (na < 1 || nb < 1) return fail(TDH_EINVAL, "tdh_overlap: na, nb must be >= 1");
     if (g->np % tdh::RT_P != 0) return fail(TDH_EUNSUPPORTED, "tdh_overlap: the GEMM kernels need n0*n1*n2 to be a multiple of %d", tdh::RT_P);
@@ -1589,7 +1599,7 @@ extern "C" int tdh_overlap(tdh_grid* g, int na, const tdh_c128* a_dev, int nb, c
     cd* part = g->d_work;
     const cd* a = (const cd*)a_dev;
     const cd* b = (const cd*)b_dev;
-    int hermitian = (a_dev == b_dev && na == nb) ? 1 : 0;      // Gram matrix of one block: upper tiles only
+    int hermitian = (na == nb && (a_dev == b_dev || result_is_hermitian)) ? 1 : 0;      // Gram matrix of one block: upper tiles only
     {
         void* args[] = {(void*)&a, (void*)&na, (void*)&b, (void*)&nb, (void*)&npts, (void*)&tjv, (void*)&cps, (void*)&part,
                         (void*)&hermitian};
@@ -1635,11 +1645,9 @@ static int small_scratch(tdh_grid* g, int nst) {
     if (g->small_n >= nst) return TDH_OK;
     CU(cudaStreamSynchronize(g->stream));
     for (int i = 0; i < 3; ++i) { cudaFree(g->d_small[i]); g->d_small[i] = nullptr; }
-    cudaFree(g->d_rot); g->d_rot = nullptr;
     cudaFree(g->d_w); g->d_w = nullptr;
     g->small_n = 0;
     for (int i = 0; i < 3; ++i) CU(cudaMalloc(&g->d_small[i], sizeof(cd) * (size_t)nst * nst));
-    CU(cudaMalloc(&g->d_rot, sizeof(tdh::JacobiRot) * (size_t)(nst / 2 + 1)));
     CU(cudaMalloc(&g->d_w, sizeof(double) * (size_t)nst));
     if (!g->d_status) CU(cudaMalloc(&g->d_status, 2 * sizeof(int)));       // [0] status, [1] grid-barrier counter
     if (!g->d_ctl) CU(cudaMalloc(&g->d_ctl, 8 * sizeof(unsigned)));
@@ -1657,33 +1665,44 @@ extern "C" int tdh_subspace_diag(tdh_grid* g, int nst, const tdh_c128* psi_dev, 
         return fail(TDH_EINVAL, "tdh_subspace_diag: psi and out overlap");
     int rc = small_scratch(g, nst);
     if (rc) return rc;
-    if ((rc = tdh_overlap(g, nst, psi_dev, nst, hpsi_dev, (tdh_c128*)g->d_small[1]))) return rc;
+    // M = dV psi^H (H psi) is Hermitian up to rounding: upper tiles only, then (M + M^H) / 2 inside the diagonal tiles
+    if ((rc = overlap_impl(g, nst, psi_dev, nst, hpsi_dev, (tdh_c128*)g->d_small[1], true))) return rc;
     tdh::symmetrize_kernel<<<296, 256, 0, g->stream>>>(g->d_small[1], nst, g->d_small[0]);
     CU(cudaGetLastError());
     {
         int dev = 0, nsm = 0, occ = 0;
         CU(cudaGetDevice(&dev));
         CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tdh::jacobi_eigh_kernel, 256, 0));
-        const int want = (int)(((size_t)nst * (nst / 2 + 1) + 255) / 256);
-        const int ctas = std::max(1, std::min(nsm * std::min(occ, 2), want));
+        const size_t smem = sizeof(tdh::JacobiRot) * (size_t)(nst / 2 + 1);
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tdh::jacobi_eigh_kernel, tdh::JACOBI_T, smem));
+        if (occ < 1) return fail(TDH_ECUDA, "tdh_subspace_diag: the eigensolver kernel does not fit on an SM");
+        const size_t blocks = (size_t)(nst / 2 + 1) * (nst / 2 + 1) + (size_t)nst * (nst / 2 + 1);
+        const int want = (int)((blocks + tdh::JACOBI_T - 1) / tdh::JACOBI_T);
+        int per_sm = 1;                                                 // one CTA per SM: the grid barrier is the cost
+        if (const char* e = getenv("TDH_JACOBI_CTAS_PER_SM")) per_sm = std::max(1, std::min(occ, atoi(e)));
+        const int ctas = std::max(1, std::min(nsm * per_sm, want));
         CU(cudaMemsetAsync(g->d_ctl, 0, 8 * sizeof(unsigned), g->stream));
         cd* a = g->d_small[0];
+        cd* a2 = g->d_small[2];
         cd* v = g->d_small[1];
         int n = nst;
-        tdh::JacobiRot* rot = g->d_rot;
         unsigned* ctl = g->d_ctl;
-        void* args[] = {(void*)&a, (void*)&v, (void*)&n, (void*)&rot, (void*)&ctl};
-        CU(cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(&tdh::jacobi_eigh_kernel), dim3(ctas), dim3(256), args,
-                                       0, g->stream));
+        void* args[] = {(void*)&a, (void*)&a2, (void*)&v, (void*)&n, (void*)&ctl};
+        CU(cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(&tdh::jacobi_eigh_kernel), dim3(ctas), dim3(tdh::JACOBI_T),
+                                       args, smem, g->stream));
     }
     tdh::eigh_sort_kernel<<<1, 256, sizeof(double) * nst, g->stream>>>(g->d_small[0], g->d_small[1], nst, g->d_w, g->d_small[2]);
     CU(cudaGetLastError());
     g->launch_count += 3;
     if ((rc = launch_rotate(g, nst, (const cd*)psi_dev, nst, g->d_small[2], (cd*)out_dev, 0))) return rc;
     if (eig_host) {
+        unsigned ctl_host[8] = {0};
         CU(cudaMemcpyAsync(eig_host, g->d_w, sizeof(double) * nst, cudaMemcpyDeviceToHost, g->stream));
+        CU(cudaMemcpyAsync(ctl_host, g->d_ctl, sizeof(ctl_host), cudaMemcpyDeviceToHost, g->stream));
         CU(cudaStreamSynchronize(g->stream));
+        g->jacobi_sweeps = (int)ctl_host[4];
+        if (ctl_host[5] != 0)
+            return fail(TDH_ECUDA, "tdh_subspace_diag: the Jacobi eigensolver did not converge in %u sweeps (non-finite input?)", ctl_host[4]);
     }
     return TDH_OK;
 }
@@ -1980,6 +1999,7 @@ extern "C" int tdh_propagate_host(tdh_grid* g, int nst, tdh_c128* psi_host, doub
 // statistics / knobs
 // ------------------------------------------------------------------------------------------------------------
 extern "C" int tdh_last_launch_count(const tdh_grid* g) { return g ? g->launch_count : 0; }
+extern "C" int tdh_last_jacobi_sweeps(const tdh_grid* g) { return g ? g->jacobi_sweeps : 0; }
 
 extern "C" int tdh_set_profiling(tdh_grid* g, int on) {
     if (!g) return fail(TDH_EINVAL, "tdh_set_profiling: null handle");
