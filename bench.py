@@ -473,6 +473,32 @@ def sweep_leg(torch, B, name, flush, peak, peak_src, cpu, reps=7):
             e1.record()
             torch.cuda.synchronize()
             res["ms_per_call_in_a_100_call_loop"] = e0.elapsed_time(e1) / 100
+            # row a7 in the launch-latency regime: 20 Taylor-4 steps in one tdh_propagate call, replayed as one CUDA graph
+            # (captured on the first call), and the same call as plain launches (a second handle with TDH_GRAPH=0)
+            nsteps_p = 20
+            work = psi.clone()
+
+            def prop_ms(gg):
+                gg.propagate(work, cfg.dt, nsteps_p)
+                torch.cuda.synchronize()
+                return statistics.median(timed_each(torch, lambda: gg.propagate(work, cfg.dt, nsteps_p), 5, None)) * 1e3
+            ms_graph = prop_ms(g)
+            launches = g.last_launch_count()
+            old_env = os.environ.get("TDH_GRAPH")
+            os.environ["TDH_GRAPH"] = "0"
+            try:
+                with B.grid_for(wl) as g2:
+                    work.copy_(psi)
+                    ms_plain = prop_ms(g2)
+            finally:
+                if old_env is None:
+                    del os.environ["TDH_GRAPH"]
+                else:
+                    os.environ["TDH_GRAPH"] = old_env
+            res["propagate"] = {"steps": nsteps_p, "dt": cfg.dt, "ms_cuda_graph": ms_graph, "ms_plain_launches": ms_plain,
+                                "launches": launches,
+                                "h_application_equivalents_per_s": units * 4 * nsteps_p / (ms_graph * 1e-3), "unit": UNIT}
+            del work
         if name == "tddft":
             # row a7: the config's 20 Taylor-4 steps (80 H applications + fused axpys) in one tdh_propagate call
             work = psi.clone()

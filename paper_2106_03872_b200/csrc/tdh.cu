@@ -165,6 +165,13 @@ struct tdh_grid {
     cudaStream_t s_h2d, s_d2h;
     cudaEvent_t ev_in[2], ev_k[2], ev_out[2];
 
+    // tdh_propagate on small blocks: the launches of one call captured once into a CUDA graph and replayed while the
+    // call's arguments and the handle's tables stay the same (`epoch` counts every change of the handle)
+    struct { cudaGraphExec_t exec; const void* psi; int nst, nsteps, launches; double dt; unsigned epoch; } pg;
+    unsigned epoch;
+    bool use_graph;
+    cudaStream_t s_cap;
+
     // statistics
     int launch_count;
     bool profiling;
@@ -434,6 +441,8 @@ static int create_impl(const int n[3], const double len[3], const double kpt[3],
         CU(cudaMalloc(&g->d_phi[1], state_bytes * std::max(2, g->chunk_cap)));
         if (world > 1) CU(cudaMalloc(&g->d_fs, state_bytes * g->chunk_cap));
         g->chunk = default_chunk(g);
+        g->use_graph = true;
+        if (const char* e = getenv("TDH_GRAPH")) g->use_graph = atoi(e) != 0;
         return TDH_OK;
     };
     rc = body();
@@ -472,6 +481,8 @@ extern "C" int tdh_destroy_grid(tdh_grid* g) {
         if (g->ev_k[i]) cudaEventDestroy(g->ev_k[i]);
         if (g->ev_out[i]) cudaEventDestroy(g->ev_out[i]);
     }
+    if (g->pg.exec) cudaGraphExecDestroy(g->pg.exec);
+    if (g->s_cap) cudaStreamDestroy(g->s_cap);
     if (g->s_h2d) cudaStreamDestroy(g->s_h2d);
     if (g->s_d2h) cudaStreamDestroy(g->s_d2h);
     for (auto& r : g->prof_pool) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
@@ -481,6 +492,7 @@ extern "C" int tdh_destroy_grid(tdh_grid* g) {
 
 extern "C" int tdh_set_potential(tdh_grid* g, const double* v_dev) {
     if (!g) return fail(TDH_EINVAL, "tdh_set_potential: null handle");
+    g->epoch += 1;
     if (v_dev) {
         CU(cudaMemcpyAsync(g->d_v, v_dev, sizeof(double) * g->np, cudaMemcpyDeviceToDevice, g->stream));
         g->have_v = true;
@@ -496,6 +508,7 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
                                   const double* sph_disp, const int32_t* chan_off, const double* beta,
                                   const double* dcoef) {
     if (!g) return fail(TDH_EINVAL, "tdh_set_projectors: null handle");
+    g->epoch += 1;
     if (natoms < 0) return fail(TDH_EINVAL, "tdh_set_projectors: natoms < 0");
     if (natoms == 0) {
         CU(cudaStreamSynchronize(g->stream));
@@ -1165,6 +1178,42 @@ extern "C" int tdh_propagate(tdh_grid* g, int nst, tdh_c128* psi_dev, double dt,
     if (order != 4) return fail(TDH_EINVAL, "tdh_propagate: order must be 4");
     if (nsteps < 0 || !std::isfinite(dt)) return fail(TDH_EINVAL, "tdh_propagate: bad dt / nsteps");
     stats_reset(g);
+    // Small blocks are bound by launch latency (Tiny: one 9 us kernel per application): replay the call as one CUDA graph.
+    // Captured on an internal stream (the caller's may be the legacy default stream, which cannot capture), launched on
+    // the caller's.  Kernel arguments, tensor maps included, are frozen in the graph, hence the key below.
+    const size_t block_bytes = (size_t)nst * g->np * sizeof(cd);
+    const long nodes = (long)nsteps * 4 * 6 * ((nst + g->chunk - 1) / g->chunk);
+    if (g->use_graph && !g->profiling && nsteps > 0 && block_bytes <= ((size_t)128 << 20) && nodes <= 8192) {
+        const bool hit = g->pg.exec && g->pg.psi == (const void*)psi_dev && g->pg.nst == nst && g->pg.nsteps == nsteps &&
+                         g->pg.dt == dt && g->pg.epoch == g->epoch;
+        if (!hit) {
+            if (g->pg.exec) { cudaGraphExecDestroy(g->pg.exec); g->pg.exec = nullptr; }
+            if (!g->s_cap) CU(cudaStreamCreateWithFlags(&g->s_cap, cudaStreamNonBlocking));
+            cudaStream_t user = g->stream;
+            g->stream = g->s_cap;
+            cudaGraph_t graph = nullptr;
+            cudaError_t e = cudaStreamBeginCapture(g->s_cap, cudaStreamCaptureModeThreadLocal);
+            int rc = e == cudaSuccess ? propagate_block(g, nst, (cd*)psi_dev, dt, nsteps) : TDH_ECUDA;
+            if (e == cudaSuccess) e = cudaStreamEndCapture(g->s_cap, &graph);
+            g->stream = user;
+            if (rc == TDH_OK && e == cudaSuccess && graph) e = cudaGraphInstantiate(&g->pg.exec, graph, 0);
+            if (graph) cudaGraphDestroy(graph);
+            if (rc != TDH_OK || e != cudaSuccess || !g->pg.exec) {
+                (void)cudaGetLastError();                 // capture is an optimisation: fall back to plain launches
+                g->pg.exec = nullptr;
+                g->use_graph = false;
+            } else {
+                g->pg.psi = psi_dev; g->pg.nst = nst; g->pg.nsteps = nsteps; g->pg.dt = dt; g->pg.epoch = g->epoch;
+                g->pg.launches = g->launch_count;
+            }
+        }
+        if (g->pg.exec) {
+            CU(cudaGraphLaunch(g->pg.exec, g->stream));
+            g->launch_count = g->pg.launches;
+            return TDH_OK;
+        }
+        stats_reset(g);
+    }
     int rc = propagate_block(g, nst, (cd*)psi_dev, dt, nsteps);
     if (rc) return rc;
     return prof_collect(g);
@@ -1196,6 +1245,7 @@ extern "C" int tdh_etrs_step(tdh_grid* g, int nst, tdh_c128* psi_dev, tdh_c128* 
     int rc = taylor_pair_block(g, nst, (cd*)psi_dev, (cd*)approx_dev, dt);          // Eq. 7 and the first factor of Eq. 6
     if (rc) return rc;
     // H(t+dt): stream-ordered switch of the potential
+    g->epoch += 1;
     if (v_next_dev) {
         CU(cudaMemcpyAsync(g->d_v, v_next_dev, sizeof(double) * g->np, cudaMemcpyDeviceToDevice, g->stream));
         g->have_v = true;
@@ -2004,6 +2054,7 @@ extern "C" int tdh_last_jacobi_sweeps(const tdh_grid* g) { return g ? g->jacobi_
 extern "C" int tdh_set_profiling(tdh_grid* g, int on) {
     if (!g) return fail(TDH_EINVAL, "tdh_set_profiling: null handle");
     g->profiling = on != 0;
+    g->epoch += 1;
     return TDH_OK;
 }
 
@@ -2019,5 +2070,6 @@ extern "C" int tdh_set_chunk_states(tdh_grid* g, int chunk) {
     if (!g) return fail(TDH_EINVAL, "tdh_set_chunk_states: null handle");
     if (chunk < 0) return fail(TDH_EINVAL, "tdh_set_chunk_states: chunk < 0");
     g->chunk = chunk == 0 ? default_chunk(g) : std::min(chunk, max_chunk(g));
+    g->epoch += 1;
     return TDH_OK;
 }

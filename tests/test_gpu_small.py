@@ -154,3 +154,44 @@ def test_small_planes_many_states_stress(torch_cuda, B, oracle, monkeypatch, sma
             assert per_state_rel(got, ref).max() < TOL
         del psi, out
         torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("name", ["tiny", "small"])
+def test_propagate_graph_replay_and_invalidation(torch_cuda, B, oracle, monkeypatch, name):
+    """tdh_propagate on small blocks replays a captured CUDA graph.  A replay (same buffer, same arguments) must continue the
+    propagation exactly as plain launches do, another buffer or step count must not reuse the frozen arguments, and a
+    new potential must invalidate the graph (the kernels' arguments are frozen at capture)."""
+    torch = torch_cuda
+    cfg = W.CONFIGS[name]
+    wl = W.make(cfg)
+    nst = cfg.nst if name == "tiny" else 6
+    psi = W.states(cfg, 0, nst)
+    dt = cfg.dt
+    rng = np.random.default_rng([W.BASE_SEED + cfg.cid, 11])
+    v2 = wl.v + rng.uniform(-0.3, 0.3, wl.v.shape)
+    wl2 = W.Workload(cfg=cfg, pos=wl.pos, v=v2, proj=wl.proj)
+    ref_a = oracle.propagate_workload(wl, psi, dt=dt, nsteps=2, backend=oracle.NAIVE_FFT)        # first call
+    ref_b = oracle.propagate_workload(wl, ref_a, dt=dt, nsteps=2, backend=oracle.NAIVE_FFT)      # replay
+    ref_c = oracle.propagate_workload(wl2, ref_b, dt=dt, nsteps=2, backend=oracle.NAIVE_FFT)     # new potential
+    ref_d = oracle.propagate_workload(wl2, psi, dt=dt, nsteps=1, backend=oracle.NAIVE_FFT)       # other buffer and count
+    results = {}
+    for graph in ("1", "0"):
+        monkeypatch.setenv("TDH_GRAPH", graph)
+        with B.grid_for(wl, max_states=nst) as g:
+            d = torch.from_numpy(psi).cuda()
+            g.propagate(d, dt, 2)
+            a = d.cpu().numpy()
+            g.propagate(d, dt, 2)
+            b = d.cpu().numpy()
+            g.set_potential(torch.from_numpy(v2).cuda())
+            g.propagate(d, dt, 2)
+            c = d.cpu().numpy()
+            e = torch.from_numpy(psi).cuda()
+            g.propagate(e, dt, 1)
+            dd = e.cpu().numpy()
+            assert g.last_launch_count() == 4 * (g.last_launch_count() // 4)
+        for got, ref in ((a, ref_a), (b, ref_b), (c, ref_c), (dd, ref_d)):
+            assert per_state_rel(got, ref).max() < TOL
+        results[graph] = (a, b, c, dd)
+    for x, y in zip(results["1"], results["0"]):
+        assert np.array_equal(x, y)                                  # the graph replays the same kernels: bitwise equal
