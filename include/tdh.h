@@ -100,7 +100,12 @@ int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_off, const in
 int tdh_apply_hamiltonian(tdh_grid* g, int nst, const tdh_c128* psi_dev, tdh_c128* hpsi_dev);
 
 /* nsteps steps of psi <- sum_{k=0..4} (-i dt)^k/k! H^k psi (Eq. 8 with lambda = -i dt; fixed H, reading R10), in place.
- * psi_dev: DEVICE, nst*n0*n1*n2 complex128.  order must be 4.  nsteps >= 0.  Asynchronous on the handle's stream. */
+ * psi_dev: DEVICE, nst*n0*n1*n2 complex128.  order must be 4.  nsteps >= 0.  Asynchronous on the handle's stream.
+ * Blocks of at most 128 MiB (the launch-latency regime) are replayed as one CUDA graph: the first call with a given
+ * (psi_dev, nst, dt, nsteps) captures the call's launches on an internal stream and instantiates the graph (host work
+ * only, nothing is allocated on the device), later calls with the same arguments launch that graph on the handle's
+ * stream; any tdh_set_* call, another buffer or another count captures anew.  The result is bitwise that of the plain
+ * launches.  TDH_GRAPH=0 in the environment at tdh_create_grid switches the graph off. */
 int tdh_propagate(tdh_grid* g, int nst, tdh_c128* psi_dev, double dt, int nsteps, int order);
 
 /* The two exponentials of an ETRS step that share their powers H^k psi (Eq. 8 for two lambdas):

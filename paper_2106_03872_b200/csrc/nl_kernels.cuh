@@ -43,10 +43,10 @@ nl_project_kernel(const cd* __restrict__ psi, size_t npts, int nst, const AtomDe
                   const double* __restrict__ dscale, cd* __restrict__ dpi, int nchan_tot)
 {
     __shared__ double part[NLP_WARPS][MT][4][32];
-    const AtomDesc at = atoms[blockIdx.y];
+    const AtomDesc at = atoms[blockIdx.x];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int kq = lane & 3, r8 = lane >> 2;
-    const int s0 = blockIdx.x * NLP_STATES;
+    const int s0 = blockIdx.y * NLP_STATES;
     const int s = s0 + r8;                                      // this lane's state (B fragment column)
     const bool s_ok = s < nst;
     const cd* ps = psi + (size_t)(s_ok ? s : 0) * npts;
@@ -157,10 +157,10 @@ nl_scatter_kernel(cd* __restrict__ out, size_t npts, int nst, const AtomDesc* __
                   const int* __restrict__ sidx, const double* __restrict__ sbeta, const cd* __restrict__ sphase,
                   const cd* __restrict__ dpi, int nchan_tot, cd alpha)
 {
-    const AtomDesc at = atoms[blockIdx.y];
+    const AtomDesc at = atoms[blockIdx.x];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int kq = lane & 3, r8 = lane >> 2;
-    const int s0 = blockIdx.x * NLP_STATES;
+    const int s0 = blockIdx.y * NLP_STATES;
     // B fragments: B[k = kq][n = r8] = alpha * dpi[s0 + r8][chan0 + 4*kt + kq]
     double bre[KT], bim[KT];
 #pragma unroll

@@ -210,14 +210,19 @@ static void free_projectors(tdh_grid* g) {
 }
 
 // Largest number of states one launch may cover.  The workspace bound, and for the tile configurations that put several
-// small planes into one TMA box (16 x 16 ... 32 x 32 planes, ppc > 1) at most 128 MB of states: on B200 (driver 580.159)
-// tile_fwd launches of those configurations whose loads and stores each span more than 128 MB ended, about once in ten
-// launches, with "unspecified launch failure" -- with the loads OR the stores confined to a few MB, or with 128 MB per
-// launch, never in several thousand launches.  The cause is not understood; the bound avoids it.
+// small planes into one tile of less than 72 KB (16 x 16 ... 32 x 48 planes; 48 x 48 planes, two to a 72 KB tile, are not
+// among them) at most 128 MB of states: on B200 (driver 580.159) tile_fwd launches of those configurations whose loads
+// and stores each span more than 128 MB end now and then with "unspecified launch failure" -- with the loads OR the
+// stores confined to a few MB, or with 128 MB per launch, never in several thousand launches; 48 x 48 planes ran 39,600
+// unbounded applications of 0.4 - 0.9 GB clean.  The cause is not understood; the bound avoids it.
+// TDH_MAX_LAUNCH_MB overrides the 128 (0: no bound) -- for the stress runs that watch this.
 static int max_chunk(const tdh_grid* g) {
     int c = g->chunk_cap;
-    if (!g->generic && g->tl.ppc > 1) {
-        const size_t lim = ((size_t)128 << 20) / (g->np * sizeof(cd));
+    const size_t tile_bytes = (size_t)g->tl.ppc * (g->n[1] / g->tl.s) * g->n[2] * sizeof(cd);
+    if (!g->generic && g->tl.ppc > 1 && tile_bytes < 73728) {
+        size_t lim_mb = 128;
+        if (const char* e = getenv("TDH_MAX_LAUNCH_MB")) { long v = atol(e); lim_mb = v > 0 ? (size_t)v : ((size_t)1 << 30); }
+        const size_t lim = (lim_mb << 20) / (g->np * sizeof(cd));
         c = (int)std::max<size_t>(1, std::min<size_t>((size_t)c, lim));
     }
     return c;
@@ -946,7 +951,7 @@ static int launch_nl_project(tdh_grid* g, int nst, const cd* in, const double* d
                     (void*)&sphase, (void*)&dscale, (void*)&dpi, (void*)&nct};
     const void* f = g->mt == 1 ? reinterpret_cast<const void*>(&tdh::nl_project_kernel<1>)
                                : reinterpret_cast<const void*>(&tdh::nl_project_kernel<2>);
-    dim3 grid((nst + tdh::NLP_STATES - 1) / tdh::NLP_STATES, g->natoms);   // y <= 65535 atoms
+    dim3 grid(g->natoms, (nst + tdh::NLP_STATES - 1) / tdh::NLP_STATES);
     LAUNCH(K_NLPROJ, f, grid, dim3(32 * tdh::NLP_WARPS), 0, args);
     return TDH_OK;
 }
@@ -966,7 +971,7 @@ static int launch_nl_scatter(tdh_grid* g, int nst, cd* out, cd alpha) {
         const tdh::AtomDesc* atoms = g->d_atoms_col + g->col_off[c];
         void* args[] = {(void*)&out, (void*)&npts, (void*)&nst, (void*)&atoms, (void*)&sidx, (void*)&sbeta,
                         (void*)&sphase, (void*)&dpi, (void*)&nct, (void*)&alpha};
-        dim3 grid((nst + tdh::NLP_STATES - 1) / tdh::NLP_STATES, g->col_off[c + 1] - g->col_off[c]);
+        dim3 grid(g->col_off[c + 1] - g->col_off[c], (nst + tdh::NLP_STATES - 1) / tdh::NLP_STATES);
         LAUNCH(K_NLSCATTER, fs[g->kt - 1], grid, dim3(32 * tdh::NLS_WARPS), 0, args);
     }
     return TDH_OK;
