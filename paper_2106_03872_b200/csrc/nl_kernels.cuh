@@ -22,6 +22,8 @@ struct AtomDesc {
     int boff;    // offset of beta_{I,0}[0]; channel c at boff + c*np
     int chan0;   // first channel in the global channel list
     int nchan;   // C_I
+    int sc0;     // first chunk of the atom in the chunk table of nl_scatter_bulk_kernel
+    int scn;     // number of chunks
 };
 
 __device__ __forceinline__ void dmma_m8n8k4(double (&c)[2], double a, double b) {
@@ -232,6 +234,120 @@ nl_scatter_kernel(cd* __restrict__ out, size_t npts, int nst, const AtomDesc* __
             for (int kt = 0; kt < KT; ++kt) af[u][kt] = afn[u][kt];
         }
     }
+}
+
+
+// ------------------------------------------------------------------------------------------------------------
+// The same back-projection with the read-modify-write done by the L2: cp.reduce.async.bulk ... .add.f64 (TMA, no tensor
+// map).  nl_scatter_kernel above loads every output value, adds and stores it, and waits on those loads (ncu,
+// profiles/r02_summary.md: 16 of 18 warp-cycles per issue on long_scoreboard, DRAM 56 % busy).  Here the kernel never
+// reads `out`: the contributions alpha e^{-ik.d} sum_c beta_c D pi_c of a chunk of the sphere go to shared memory, laid out
+// [state][point], and one bulk reduce-add per (z-run, state) adds them to the output block in the L2 -- a sphere is z-runs
+// of consecutive grid points, i.e. of consecutive addresses.  Measured on B200 (Large geometry, 296 states): plain RMW
+// 3.55 TB/s, bulk reduce-add 4.6 TB/s of the 32 B per point and state.
+// A chunk is up to SC_RC runs / SC_MAXPTS points (longer runs are cut); two chunk buffers: the TMA reads one while the warps
+// fill the other.  Rounding is that of one IEEE addition per point, as in the RMW kernel; the launches per colour keep the
+// order of the additions fixed where spheres overlap.
+// ------------------------------------------------------------------------------------------------------------
+constexpr int SC_RC = 32;          // runs per chunk: one bulk operation per (run, state) = 256 threads
+#ifndef TDH_SC_MAXPTS
+#define TDH_SC_MAXPTS 352
+#endif
+#ifndef TDH_SC_NBUF
+#define TDH_SC_NBUF 2
+#endif
+constexpr int SC_MAXPTS = TDH_SC_MAXPTS;     // points per chunk: two CTAs of 90 KB per SM
+constexpr int SC_NBUF = TDH_SC_NBUF;
+constexpr size_t SC_SMEM = (size_t)SC_NBUF * NLP_STATES * SC_MAXPTS * sizeof(cd);
+struct ScRun { int p0, len, off; };         // first grid point, points, offset (points) inside the chunk
+struct ScChunk { int r0, nr, q0, np; };     // first run, runs, first point in the atom's sorted list, points
+
+__device__ __forceinline__ void bulk_reduce_add_f64(void* gdst, const void* ssrc, unsigned bytes) {
+    asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f64 [%0], [%1], %2;" ::"l"(gdst),
+                 "r"((unsigned)__cvta_generic_to_shared(ssrc)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_commit_group() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void bulk_wait_group_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
+template <int N> __device__ __forceinline__ void bulk_wait_group() { asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory"); }
+
+// grid: (atoms of this colour, ceil(nst / 8)); KT = number of 4-channel tiles (C_I <= 4*KT)
+template <int KT>
+__global__ void __launch_bounds__(32 * NLS_WARPS)
+nl_scatter_bulk_kernel(cd* __restrict__ out, size_t npts, int nst, const AtomDesc* __restrict__ atoms,
+                       const ScRun* __restrict__ runs, const ScChunk* __restrict__ chunks, const double* __restrict__ sbeta,
+                       const cd* __restrict__ sphase, const cd* __restrict__ dpi, int nchan_tot, cd alpha)
+{
+    extern __shared__ __align__(128) unsigned char sc_smem[];
+    cd* buf = reinterpret_cast<cd*>(sc_smem);
+    const AtomDesc at = atoms[blockIdx.x];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int kq = lane & 3, r8 = lane >> 2;
+    const int s0 = blockIdx.y * NLP_STATES;
+    // B fragments: B[k = kq][n = r8] = alpha * dpi[s0 + r8][chan0 + 4*kt + kq]
+    double bre[KT], bim[KT];
+#pragma unroll
+    for (int kt = 0; kt < KT; ++kt) {
+        const int c = 4 * kt + kq, s = s0 + r8;
+        cd v = make_double2(0.0, 0.0);
+        if (c < at.nchan && s < nst) v = cmul(alpha, __ldg(dpi + (size_t)s * nchan_tot + at.chan0 + c));
+        bre[kt] = v.x;
+        bim[kt] = v.y;
+    }
+    const cd* phs = sphase ? sphase + at.q0 : nullptr;
+    const int prun = threadIdx.x >> 3, pst = threadIdx.x & 7;       // this thread's bulk operation: (run, state) of a chunk
+    cd* orow = out + (size_t)min(s0 + pst, nst - 1) * npts;
+    const bool pst_ok = s0 + pst < nst;
+    constexpr int U = 4;                                            // 8-point blocks of one warp in flight
+    for (int c = 0; c < at.scn; ++c) {
+        const ScChunk ch = chunks[at.sc0 + c];
+        cd* bb = buf + (size_t)(c % SC_NBUF) * NLP_STATES * SC_MAXPTS;
+        if (c >= SC_NBUF) bulk_wait_group_read<SC_NBUF - 1>();     // the TMA has read this buffer (chunk c - 2)
+        __syncthreads();
+        const int nblk = (ch.np + 7) >> 3;
+        for (int b0 = warp; b0 < nblk; b0 += U * NLS_WARPS) {
+            double af[U][KT];
+            cd ph[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int i = 8 * (b0 + u * NLS_WARPS) + r8;        // row of the MMA: point i of the chunk
+                const bool ok = i < ch.np;
+#pragma unroll
+                for (int kt = 0; kt < KT; ++kt) {
+                    const int cc = 4 * kt + kq;                     // column of the A fragment: channel
+                    af[u][kt] = (ok && cc < at.nchan) ? __ldg(sbeta + at.boff + (size_t)cc * at.np + ch.q0 + i) : 0.0;
+                }
+                if (phs != nullptr) ph[u] = ok ? __ldg(phs + ch.q0 + i) : make_double2(1.0, 0.0);
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int i = 8 * (b0 + u * NLS_WARPS) + r8;
+                double cre[2] = {0.0, 0.0}, cim[2] = {0.0, 0.0};
+#pragma unroll
+                for (int kt = 0; kt < KT; ++kt) {
+                    dmma_m8n8k4(cre, af[u][kt], bre[kt]);
+                    dmma_m8n8k4(cim, af[u][kt], bim[kt]);
+                }
+                cd a0 = make_double2(cre[0], cim[0]), a1 = make_double2(cre[1], cim[1]);
+                if (phs != nullptr) {
+                    a0 = cmulc(a0, ph[u]);
+                    a1 = cmulc(a1, ph[u]);
+                }
+                if (i < ch.np) {                                    // C fragment: point i, states 2*kq and 2*kq + 1
+                    bb[(size_t)(2 * kq) * SC_MAXPTS + i] = a0;
+                    bb[(size_t)(2 * kq + 1) * SC_MAXPTS + i] = a1;
+                }
+            }
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the generic-proxy writes above before the TMA's reads
+        __syncthreads();
+        if (prun < ch.nr && pst_ok) {
+            const ScRun ru = runs[ch.r0 + prun];
+            bulk_reduce_add_f64(orow + ru.p0, bb + (size_t)pst * SC_MAXPTS + ru.off, (unsigned)ru.len * 16u);
+        }
+        bulk_commit_group();
+    }
+    bulk_wait_group_read<0>();                                  // the buffers may be released; the kernel boundary completes the additions
 }
 
 }  // namespace tdh

@@ -155,6 +155,9 @@ struct tdh_grid {
     // separate back-projection kernel: atoms grouped by colour (spheres of one colour share no grid point)
     int nl_mode;                       // 1: nl_scatter kernel per colour after plane_inv; 0: records inside plane_inv
     tdh::AtomDesc* d_atoms_col;        // atoms sorted by colour
+    tdh::ScRun* d_sc_runs;             // z-runs of every sphere (nl_scatter_bulk_kernel)
+    tdh::ScChunk* d_sc_chunks;         // chunks of runs, per atom (AtomDesc::sc0, scn)
+    bool scatter_bulk;                 // back-projection by bulk reduce-add (TDH_SCATTER_BULK=0: the read-modify-write kernel)
     std::vector<int> col_off;          // [ncolours + 1] offsets into d_atoms_col
     int kt;                            // 4-channel tiles of the back-projection MMA
 
@@ -200,6 +203,7 @@ static int freq_index(int a, int n) {
 static void free_projectors(tdh_grid* g) {
     cudaFree(g->d_atoms); cudaFree(g->d_sidx); cudaFree(g->d_sbeta); cudaFree(g->d_sphase); cudaFree(g->d_dscale);
     cudaFree(g->d_atoms_col); g->d_atoms_col = nullptr; g->col_off.clear();
+    cudaFree(g->d_sc_runs); g->d_sc_runs = nullptr; cudaFree(g->d_sc_chunks); g->d_sc_chunks = nullptr;
     cudaFree(g->d_dvscale); g->d_dvscale = nullptr; cudaFree(g->d_dpig); g->d_dpig = nullptr;
     cudaFree(g->d_force); g->d_force = nullptr;
     cudaFree(g->d_dpi); cudaFree(g->d_dpi_part); g->d_dpi_part = nullptr; cudaFree(g->d_nl_off); cudaFree(g->d_nl_cc); cudaFree(g->d_nl_beta); cudaFree(g->d_nl_phase);
@@ -344,6 +348,13 @@ static int create_impl(const int n[3], const double len[3], const double kpt[3],
         g->ctas_x[0] = ctas[1]; g->ctas_x[1] = ctas[2]; g->ctas_x[2] = ctas[3]; g->ctas_x[3] = ctas[4]; g->ctas_x[4] = ctas[5];
         for (int i = 0; i < tdh::NL_NCM; ++i) g->ctas_inv[i] = ctas[9 + i];
         g->ctas_fwd_slab = ctas[6]; g->ctas_x_slab[0] = ctas[7]; g->ctas_x_slab[1] = ctas[8];
+        {
+            const void* fb[4] = {(const void*)&tdh::nl_scatter_bulk_kernel<1>, (const void*)&tdh::nl_scatter_bulk_kernel<2>,
+                                 (const void*)&tdh::nl_scatter_bulk_kernel<3>, (const void*)&tdh::nl_scatter_bulk_kernel<4>};
+            for (const void* f : fb) CU(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tdh::SC_SMEM));
+            g->scatter_bulk = true;
+            if (const char* e = getenv("TDH_SCATTER_BULK")) g->scatter_bulk = atoi(e) != 0;
+        }
         // tables: built on the host exactly as the oracle builds its G vectors (two_pi * m / L + k, then squared)
         const double two_pi = 6.283185307179586476925286766559;
         for (int a = 0; a < 3; ++a) {
@@ -587,6 +598,28 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
         atoms[a].q0 = (int)q0; atoms[a].np = pn; atoms[a].boff = (int)boff; atoms[a].chan0 = c0; atoms[a].nchan = nc;
         boff += (size_t)nc * pn;
     }
+    // ---- z-runs of every sphere and their chunks (nl_kernels.cuh, nl_scatter_bulk_kernel): a run is a maximal sequence
+    //      of consecutive flat indices of the sorted list, cut at SC_MAXPTS points; a chunk is up to SC_RC runs and
+    //      SC_MAXPTS points, consecutive in the list
+    std::vector<tdh::ScRun> sc_runs;
+    std::vector<tdh::ScChunk> sc_chunks;
+    for (int a = 0; a < natoms; ++a) {
+        tdh::AtomDesc& at = atoms[a];
+        at.sc0 = (int)sc_chunks.size();
+        int j = 0;
+        while (j < at.np) {
+            int len = 1;
+            while (j + len < at.np && len < tdh::SC_MAXPTS && sidx[at.q0 + j + len] == sidx[at.q0 + j] + len) ++len;
+            if (sc_chunks.size() == (size_t)at.sc0 || sc_chunks.back().nr == tdh::SC_RC || sc_chunks.back().np + len > tdh::SC_MAXPTS)
+                sc_chunks.push_back(tdh::ScChunk{(int)sc_runs.size(), 0, j, 0});
+            tdh::ScChunk& ch = sc_chunks.back();
+            sc_runs.push_back(tdh::ScRun{sidx[at.q0 + j], len, ch.np});
+            ch.nr += 1;
+            ch.np += len;
+            j += len;
+        }
+        at.scn = (int)sc_chunks.size() - at.sc0;
+    }
     // ---- colours for the separate back-projection kernel: greedy, an atom takes the lowest colour that no atom sharing
     //      a grid point with it has taken (per-point bit mask of the colours already present)
     std::vector<tdh::AtomDesc> atoms_col;
@@ -679,7 +712,7 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
     int rc;
     tdh_grid stage{};                                      // only its projector fields are used
     tdh_grid* nw = &stage;
-    if ((rc = up(&nw->d_atoms_col, atoms_col)) || (rc = up(&nw->d_atoms, atoms)) || (rc = up(&nw->d_sidx, sidx)) || (rc = up(&nw->d_sbeta, sbeta)) ||
+    if ((rc = up(&nw->d_sc_runs, sc_runs)) || (rc = up(&nw->d_sc_chunks, sc_chunks)) || (rc = up(&nw->d_atoms_col, atoms_col)) || (rc = up(&nw->d_atoms, atoms)) || (rc = up(&nw->d_sidx, sidx)) || (rc = up(&nw->d_sbeta, sbeta)) ||
         (rc = up(&nw->d_sphase, sphase)) || (rc = up(&nw->d_dscale, dscale)) || (rc = up(&nw->d_nl_off, nl_off)) ||
         (rc = up(&nw->d_nl_cc, rec_cc)) || (rc = up(&nw->d_nl_beta, rec_beta)) || (rc = up(&nw->d_nl_phase, rec_phase))) {
         free_projectors(nw);
@@ -702,6 +735,7 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
     // success: replace the installed tables
     if (cudaStreamSynchronize(g->stream) != cudaSuccess) { free_projectors(nw); return fail(TDH_ECUDA, "tdh_set_projectors: stream synchronisation failed"); }
     free_projectors(g);
+    g->d_sc_runs = nw->d_sc_runs; g->d_sc_chunks = nw->d_sc_chunks;
     g->d_atoms_col = nw->d_atoms_col; g->d_atoms = nw->d_atoms; g->d_sidx = nw->d_sidx; g->d_sbeta = nw->d_sbeta;
     g->d_sphase = nw->d_sphase; g->d_dscale = nw->d_dscale; g->d_nl_off = nw->d_nl_off; g->d_nl_cc = nw->d_nl_cc;
     g->d_nl_beta = nw->d_nl_beta; g->d_nl_phase = nw->d_nl_phase; g->d_dpi = nw->d_dpi; g->d_dvscale = nw->d_dvscale;
@@ -967,6 +1001,21 @@ static int launch_nl_scatter(tdh_grid* g, int nst, cd* out, cd alpha) {
     const void* fs[4] = {reinterpret_cast<const void*>(&tdh::nl_scatter_kernel<1>), reinterpret_cast<const void*>(&tdh::nl_scatter_kernel<2>),
                          reinterpret_cast<const void*>(&tdh::nl_scatter_kernel<3>), reinterpret_cast<const void*>(&tdh::nl_scatter_kernel<4>)};
     if (g->kt < 1) return TDH_OK;                          // no channel anywhere: nothing to add
+    if (g->scatter_bulk) {
+        // the read-modify-write done by the L2: one bulk reduce-add per (z-run, state) (nl_kernels.cuh)
+        const void* fb[4] = {reinterpret_cast<const void*>(&tdh::nl_scatter_bulk_kernel<1>), reinterpret_cast<const void*>(&tdh::nl_scatter_bulk_kernel<2>),
+                             reinterpret_cast<const void*>(&tdh::nl_scatter_bulk_kernel<3>), reinterpret_cast<const void*>(&tdh::nl_scatter_bulk_kernel<4>)};
+        const tdh::ScRun* runs = g->d_sc_runs;
+        const tdh::ScChunk* chunks = g->d_sc_chunks;
+        for (size_t c = 0; c + 1 < g->col_off.size(); ++c) {
+            const tdh::AtomDesc* atoms = g->d_atoms_col + g->col_off[c];
+            void* args[] = {(void*)&out, (void*)&npts, (void*)&nst, (void*)&atoms, (void*)&runs, (void*)&chunks, (void*)&sbeta,
+                            (void*)&sphase, (void*)&dpi, (void*)&nct, (void*)&alpha};
+            dim3 grid(g->col_off[c + 1] - g->col_off[c], (nst + tdh::NLP_STATES - 1) / tdh::NLP_STATES);
+            LAUNCH(K_NLSCATTER, fb[g->kt - 1], grid, dim3(32 * tdh::NLS_WARPS), tdh::SC_SMEM, args);
+        }
+        return TDH_OK;
+    }
     for (size_t c = 0; c + 1 < g->col_off.size(); ++c) {
         const tdh::AtomDesc* atoms = g->d_atoms_col + g->col_off[c];
         void* args[] = {(void*)&out, (void*)&npts, (void*)&nst, (void*)&atoms, (void*)&sidx, (void*)&sbeta,

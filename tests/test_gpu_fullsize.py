@@ -242,6 +242,37 @@ def test_both_back_projection_paths(torch_cuda, B, oracle, monkeypatch, mode):
             assert per_state_rel(d.cpu().numpy(), ref_p).max() < TOL
 
 
+
+def test_scatter_by_bulk_reduce_add_equals_read_modify_write(torch_cuda, B, oracle, monkeypatch):
+    """The separate back-projection kernel exists as a read-modify-write kernel (TDH_SCATTER_BULK=0) and with the addition
+    done by the L2 (cp.reduce.async.bulk add.f64 per z-run and state, the default).  Both match the oracle; one IEEE
+    addition per point either way, so the two results are bitwise equal.  Overlapping spheres (two colours), runs that wrap
+    around the cell, a ragged state group, k != 0 with phases, 9 channels, a general (non-tuned) grid."""
+    torch = torch_cuda
+    monkeypatch.setenv("TDH_NL_MODE", "1")
+    cases = [(280, (32, 96, 96), 9, 1, (0.0, 0.0, 0.0)), (281, (48, 48, 32), 7, 2, (0.1, 0.0, -0.2)),
+             (282, (24, 36, 54), 5, 1, (0.0, 0.25, 0.0))]
+    for cid, n, natoms, lmax, kfrac in cases:
+        cfg = W.test_config(cid, n, tuple(0.42 * m for m in n), nst=11, natoms=natoms, lmax=lmax, rc=3.4,
+                            dl=(2.0, -0.8, 0.3)[: lmax + 1], kfrac=kfrac)
+        wl = W.make(cfg)
+        psi = W.states(cfg)
+        ref = oracle.apply_workload(wl, psi, oracle.NAIVE_FFT)
+        ref_p = oracle.propagate_workload(wl, psi, dt=0.01, nsteps=1, backend=oracle.NAIVE_FFT)
+        got = {}
+        for bulk in ("1", "0"):
+            monkeypatch.setenv("TDH_SCATTER_BULK", bulk)
+            with B.grid_for(wl) as g:
+                d = torch.from_numpy(psi).cuda()
+                h = g.apply_hamiltonian(d).cpu().numpy()
+                assert g.last_launch_count() > 4                     # the separate kernel ran
+                assert per_state_rel(h, ref).max() < TOL, (cid, bulk)
+                g.propagate(d, 0.01, 1)
+                p = d.cpu().numpy()
+                assert per_state_rel(p, ref_p).max() < TOL, (cid, bulk)
+                got[bulk] = (h, p)
+        assert np.array_equal(got["1"][0], got["0"][0]) and np.array_equal(got["1"][1], got["0"][1]), cid
+
 # ------------------------------------------------------------------------------------------------ NEXT-1: ETRS
 @pytest.mark.parametrize("name,nst,backend", [("tiny", 8, 0), ("small", 24, 1), ("medium", 10, 1)])
 def test_taylor_pair_and_etrs_match_oracle(torch_cuda, B, oracle, name, nst, backend):
