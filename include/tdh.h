@@ -270,6 +270,14 @@ const char* tdh_kernel_name(int i);
  * for the contraction kernels beside the cuBLAS DGEMM rate of the same run.  Synchronises the device. */
 int tdh_measure_fp64_mma_peak(double* tflops_out);
 
+/* Allocate now what tdh_orthonormalize / tdh_subspace_diag (three n x n complex matrices for blocks of up to
+ * rotation_states states; 0: none), tdh_sd_step (per-state reduction scratch), tdh_forces with per-atom local potentials
+ * (forces_local_term != 0: three real grids) and the host entry points (host_buffers != 0: four staging buffers of at most
+ * 512 MiB) would otherwise allocate at their first use, so that those calls allocate nothing either.
+ * Synchronises the handle's stream when the rotation scratch grows.  TDH_EINVAL for rotation_states outside
+ * [0, max_states], TDH_ENOMEM / TDH_ECUDA when an allocation fails (what was allocated before stays). */
+int tdh_reserve(tdh_grid* g, int rotation_states, int forces_local_term, int host_buffers);
+
 /* Tuning knob: how many states are pushed through the kernel chain together (0 = library default: as many as the
  * handle's workspace of at most 4 GiB per buffer holds, a multiple of 8 when a block has to be split -- measured on
  * B200, longer launches are never slower than L2-resident small chunks). */

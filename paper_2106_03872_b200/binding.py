@@ -28,7 +28,7 @@ SYMBOLS = (
     "tdh_propagate", "tdh_taylor_pair", "tdh_etrs_step", "tdh_density", "tdh_hartree", "tdh_overlap", "tdh_rotate", "tdh_orthonormalize", "tdh_subspace_diag", "tdh_sd_step", "tdh_gradient", "tdh_forces", "tdh_apply_hamiltonian_host", "tdh_propagate_host", "tdh_fft3d", "tdh_last_launch_count",
     "tdh_create_slab_grid", "tdh_slab_buffers", "tdh_slab_set_peers", "tdh_slab_apply_phase", "tdh_slab_fft_phase", "tdh_work_layout",
     "tdh_ipc_export", "tdh_ipc_import", "tdh_ipc_close", "tdh_measure_fp64_mma_peak", "tdh_last_jacobi_sweeps",
-    "tdh_set_profiling", "tdh_last_kernel_seconds", "tdh_kernel_name", "tdh_set_chunk_states", "tdh_last_error",
+    "tdh_set_profiling", "tdh_last_kernel_seconds", "tdh_kernel_name", "tdh_set_chunk_states", "tdh_reserve", "tdh_last_error",
 )
 NKERNELS = 5
 
@@ -408,6 +408,9 @@ class Grid:
 
     def set_chunk_states(self, chunk: int):
         _check(lib().tdh_set_chunk_states(self._h, int(chunk)))
+
+    def reserve(self, rotation_states: int = 0, forces_local_term: bool = False, host_buffers: bool = False):
+        _check(lib().tdh_reserve(self._h, int(rotation_states), int(bool(forces_local_term)), int(bool(host_buffers))))
 
 
 def measure_fp64_mma_peak() -> float:

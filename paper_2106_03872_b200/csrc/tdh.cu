@@ -2120,6 +2120,21 @@ extern "C" int tdh_last_kernel_seconds(const tdh_grid* g, double out[TDH_NKERNEL
 
 extern "C" const char* tdh_kernel_name(int i) { return (i >= 0 && i < TDH_NKERNELS) ? kKernelNames[i] : ""; }
 
+// Everything the calls below would otherwise allocate at their first use, allocated now (no allocation on
+// hot paths): the n x n scratch of the rotations for blocks of up to rotation_states states, the per-state reduction
+// scratch of tdh_sd_step, the gradient-density arrays of tdh_forces' local term, the staging buffers of the host entry points
+extern "C" int tdh_reserve(tdh_grid* g, int rotation_states, int forces_local_term, int host_buffers) {
+    if (!g) return fail(TDH_EINVAL, "tdh_reserve: null handle");
+    if (rotation_states < 0 || rotation_states > g->max_states)
+        return fail(TDH_EINVAL, "tdh_reserve: rotation_states = %d outside [0, %d]", rotation_states, g->max_states);
+    int rc;
+    if (rotation_states > 0 && (rc = small_scratch(g, rotation_states))) return rc;
+    if (!g->d_sd) CU(cudaMalloc(&g->d_sd, sizeof(double) * (size_t)g->max_states * (2 + 3 * SD_SLICES)));
+    if (forces_local_term && !g->d_gd) CU(cudaMalloc(&g->d_gd, sizeof(double) * 3 * g->np));
+    if (host_buffers && g->slab_world == 1 && (rc = host_path_init(g))) return rc;
+    return TDH_OK;
+}
+
 extern "C" int tdh_set_chunk_states(tdh_grid* g, int chunk) {
     if (!g) return fail(TDH_EINVAL, "tdh_set_chunk_states: null handle");
     if (chunk < 0) return fail(TDH_EINVAL, "tdh_set_chunk_states: chunk < 0");

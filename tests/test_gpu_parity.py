@@ -291,3 +291,29 @@ def test_error_codes(torch_cuda, B):
         with pytest.raises(B.TdhError) as e:
             g.set_projectors(bad)
         assert e.value.code == B.TDH_EINDEX
+
+
+def test_reserve_preallocates_the_on_demand_scratch(torch_cuda, B, oracle):
+    """tdh_reserve allocates what the rotations, the SD step, the forces' local term and the host entry points would
+    allocate at first use: after it those calls leave the device's free memory unchanged, and their results are the usual
+    ones."""
+    torch = torch_cuda
+    cfg = W.CONFIGS["tiny"]
+    wl = W.make(cfg)
+    psi = W.states(cfg)
+    with B.grid_for(wl) as g:
+        with pytest.raises(B.TdhError):
+            g.reserve(rotation_states=cfg.nst + 1)
+        g.reserve(rotation_states=cfg.nst, forces_local_term=True, host_buffers=True)
+        d = torch.from_numpy(psi).cuda()
+        out = torch.empty_like(d)
+        host_out = np.empty_like(psi)
+        torch.cuda.synchronize()
+        free0, _ = torch.cuda.mem_get_info()
+        q = g.orthonormalize(d, out=out)
+        g.apply_hamiltonian_host(psi, host_out)
+        torch.cuda.synchronize()
+        free1, _ = torch.cuda.mem_get_info()
+        assert free1 == free0
+        assert per_state_rel(q.cpu().numpy(), oracle.orthonormalize(cfg.n, cfg.dv, psi)).max() < 1e-11
+        assert per_state_rel(host_out, oracle.apply_workload(wl, psi, oracle.DIRECT)).max() < 1e-11
