@@ -5,8 +5,9 @@
 //     plane_fwd   (tile_fwd: z,y forward FFT per tile of a (state,x) plane)   in  -> work
 //     xpencil     (x forward, 1/2|G+k|^2 scale + mask, x inverse)             work in place
 //     plane_inv   (tile_inv: y,z inverse FFT + epilogue alpha*(T+V[+Vnl])phi + y)  work -> out
-//     nl_scatter  (FP64-MMA back-projection added into out; nl_mode 1 -- otherwise the back-projection runs inside
-//                  plane_inv from per-tile record lists)
+//     nl_scatter  (FP64-MMA back-projection added into out by bulk reduce-add of whole z-runs -- the L2 does the
+//                  read-modify-write; nl_mode 1 -- otherwise the back-projection runs inside plane_inv from per-tile
+//                  record lists)
 // tdh_taylor_pair / tdh_etrs_step (NEXT-1) and tdh_density / tdh_hartree (NEXT-2) are compositions of the same
 // launches plus three elementwise kernels.
 // The three FFT kernels are persistent (one or several CTAs per SM, as many as fit) and fed by TMA: the host encodes a
