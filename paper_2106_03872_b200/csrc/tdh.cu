@@ -158,7 +158,8 @@ struct tdh_grid {
     tdh::AtomDesc* d_atoms_col;        // atoms sorted by colour
     tdh::ScRun* d_sc_runs;             // z-runs of every sphere (nl_scatter_bulk_kernel)
     tdh::ScChunk* d_sc_chunks;         // chunks of runs, per atom (AtomDesc::sc0, scn)
-    bool scatter_bulk;                 // back-projection by bulk reduce-add (TDH_SCATTER_BULK=0: the read-modify-write kernel)
+    bool scatter_bulk;                 // back-projection by bulk reduce-add (long z-runs) or by the read-modify-write kernel
+                                       // (short runs: one TMA operation per run costs more than it saves); TDH_SCATTER_BULK=0/1
     std::vector<int> col_off;          // [ncolours + 1] offsets into d_atoms_col
     int kt;                            // 4-channel tiles of the back-projection MMA
 
@@ -353,8 +354,7 @@ static int create_impl(const int n[3], const double len[3], const double kpt[3],
             const void* fb[4] = {(const void*)&tdh::nl_scatter_bulk_kernel<1>, (const void*)&tdh::nl_scatter_bulk_kernel<2>,
                                  (const void*)&tdh::nl_scatter_bulk_kernel<3>, (const void*)&tdh::nl_scatter_bulk_kernel<4>};
             for (const void* f : fb) CU(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tdh::SC_SMEM));
-            g->scatter_bulk = true;
-            if (const char* e = getenv("TDH_SCATTER_BULK")) g->scatter_bulk = atoi(e) != 0;
+            g->scatter_bulk = true;                     // decided per projector table in tdh_set_projectors
         }
         // tables: built on the host exactly as the oracle builds its G vectors (two_pi * m / L + k, then squared)
         const double two_pi = 6.283185307179586476925286766559;
@@ -737,6 +737,11 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
     if (cudaStreamSynchronize(g->stream) != cudaSuccess) { free_projectors(nw); return fail(TDH_ECUDA, "tdh_set_projectors: stream synchronisation failed"); }
     free_projectors(g);
     g->d_sc_runs = nw->d_sc_runs; g->d_sc_chunks = nw->d_sc_chunks;
+    // Measured on B200 (profiles/r02_summary.md): runs of 12.8 points (Large) 4.10 ms by bulk reduce-add against 4.63 by
+    // read-modify-write; runs of 8.6 points (TDDFT, forced onto the separate kernel) 0.347 against 0.334, Medium 0.141
+    // against 0.129 -- one TMA operation per run and state pays from about ten points per run
+    g->scatter_bulk = !sc_runs.empty() && (double)ptot / (double)sc_runs.size() >= 10.0;
+    if (const char* e = getenv("TDH_SCATTER_BULK")) g->scatter_bulk = atoi(e) != 0;
     g->d_atoms_col = nw->d_atoms_col; g->d_atoms = nw->d_atoms; g->d_sidx = nw->d_sidx; g->d_sbeta = nw->d_sbeta;
     g->d_sphase = nw->d_sphase; g->d_dscale = nw->d_dscale; g->d_nl_off = nw->d_nl_off; g->d_nl_cc = nw->d_nl_cc;
     g->d_nl_beta = nw->d_nl_beta; g->d_nl_phase = nw->d_nl_phase; g->d_dpi = nw->d_dpi; g->d_dvscale = nw->d_dvscale;

@@ -245,7 +245,7 @@ def test_both_back_projection_paths(torch_cuda, B, oracle, monkeypatch, mode):
 
 def test_scatter_by_bulk_reduce_add_equals_read_modify_write(torch_cuda, B, oracle, monkeypatch):
     """The separate back-projection kernel exists as a read-modify-write kernel (TDH_SCATTER_BULK=0) and with the addition
-    done by the L2 (cp.reduce.async.bulk add.f64 per z-run and state, the default).  Both match the oracle; one IEEE
+    done by the L2 (cp.reduce.async.bulk add.f64 per z-run and state; the library picks by the spheres' mean run length).  Both match the oracle; one IEEE
     addition per point either way, so the two results are bitwise equal.  Overlapping spheres (two colours), runs that wrap
     around the cell, a ragged state group, k != 0 with phases, 9 channels, a general (non-tuned) grid."""
     torch = torch_cuda
