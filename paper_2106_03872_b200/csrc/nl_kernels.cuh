@@ -44,6 +44,7 @@ nl_project_kernel(const cd* __restrict__ psi, size_t npts, int nst, const AtomDe
                   const int* __restrict__ sidx, const double* __restrict__ sbeta, const cd* __restrict__ sphase,
                   const double* __restrict__ dscale, cd* __restrict__ dpi, int nchan_tot)
 {
+    constexpr int KS = MT == 1 ? NLP_KSTEPS : NLP_KSTEPS / 2;   // two channel tiles: half the k-steps in flight (registers)
     __shared__ double part[NLP_WARPS][MT][4][32];
     const AtomDesc at = atoms[blockIdx.x];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -62,12 +63,12 @@ nl_project_kernel(const cd* __restrict__ psi, size_t npts, int nst, const AtomDe
     // Software pipeline over the warp's blocks of 32 points: the sphere indices and the projector values (A fragments)
     // of block i+1 are requested while the gathers of block i are in flight, so a block costs one DRAM round trip
     // instead of three dependent ones (index -> psi, beta).
-    constexpr int STRIDE = NLP_WARPS * 4 * NLP_KSTEPS;
-    int ix[NLP_KSTEPS];
-    double af[NLP_KSTEPS][MT];
-    auto load_meta = [&](int q0, int (&ixo)[NLP_KSTEPS], double (&afo)[NLP_KSTEPS][MT]) {
+    constexpr int STRIDE = NLP_WARPS * 4 * KS;
+    int ix[KS];
+    double af[KS][MT];
+    auto load_meta = [&](int q0, int (&ixo)[KS], double (&afo)[KS][MT]) {
 #pragma unroll
-        for (int u = 0; u < NLP_KSTEPS; ++u) {
+        for (int u = 0; u < KS; ++u) {
             const int q = q0 + 4 * u + kq;
             const bool q_ok = q < at.np;
             ixo[u] = q_ok ? __ldg(idx + q) : -1;
@@ -78,20 +79,20 @@ nl_project_kernel(const cd* __restrict__ psi, size_t npts, int nst, const AtomDe
             }
         }
     };
-    int q0 = warp * 4 * NLP_KSTEPS;
+    int q0 = warp * 4 * KS;
     if (q0 < at.np) load_meta(q0, ix, af);
     for (; q0 < at.np; q0 += STRIDE) {
-        cd b[NLP_KSTEPS];
+        cd b[KS];
 #pragma unroll
-        for (int u = 0; u < NLP_KSTEPS; ++u) {
+        for (int u = 0; u < KS; ++u) {
             b[u] = make_double2(0.0, 0.0);
             if (ix[u] >= 0 && s_ok) b[u] = __ldcs(ps + ix[u]);
         }
-        int ixn[NLP_KSTEPS];
-        double afn[NLP_KSTEPS][MT];
+        int ixn[KS];
+        double afn[KS][MT];
         if (q0 + STRIDE < at.np) load_meta(q0 + STRIDE, ixn, afn);
 #pragma unroll
-        for (int u = 0; u < NLP_KSTEPS; ++u) {
+        for (int u = 0; u < KS; ++u) {
             cd bv = b[u];
             if (phs != nullptr && ix[u] >= 0) bv = cmul(bv, __ldg(phs + q0 + 4 * u + kq));
 #pragma unroll
@@ -101,7 +102,7 @@ nl_project_kernel(const cd* __restrict__ psi, size_t npts, int nst, const AtomDe
             }
         }
 #pragma unroll
-        for (int u = 0; u < NLP_KSTEPS; ++u) {
+        for (int u = 0; u < KS; ++u) {
             ix[u] = ixn[u];
 #pragma unroll
             for (int m = 0; m < MT; ++m) af[u][m] = afn[u][m];
