@@ -346,6 +346,17 @@ def roofline_of(kern_s, units, peak_gbs, peak_src, bytes_per_unit, workload=None
                              "launch per state*gridpoint, scaled to this run's launch size)"}
     t = step_s if step_s else tot
     pass_bytes = sum(bytes_per_unit[k] for k in cand)
+    # what the step really moves: the ncu DRAM bytes per unit of every family that ran (committed captures), against the
+    # step time -- the gather / scatter kernels fetch whole 128-byte lines around their z-runs, the FFT kernels move their
+    # algorithmic bytes
+    ncu_all = ncu_dram_bytes_per_unit(workload)
+    dram = None
+    if all(k in ncu_all for k in cand):
+        dram_bytes = sum(ncu_all[k] for k in cand)
+        dram = {"bytes_per_unit": round(dram_bytes, 2), "frac": round(dram_bytes * units / t * 1e-9 / peak_gbs, 4),
+                "per_kernel_frac": {k: round(ncu_all[k] * units / cand[k] * 1e-9 / peak_gbs, 4) for k in cand},
+                "note": "ncu dram__bytes (read + write) per state*gridpoint of every family (profiles/r02_ncu_dram.csv) x units "
+                        "/ step time (per_kernel_frac: / the family's CUDA-event time) / HBM peak"}
     return {"kernel": top, "bound": "hbm", "achieved": round(achieved, 1), "peak": peak_gbs, "unit": "GB/s",
             "frac": round(achieved / peak_gbs, 4), "traffic": traffic, "peak_source": peak_src,
             "algorithmic_bytes_per_unit": bytes_per_unit[top], "units_per_step": units,
@@ -355,6 +366,7 @@ def roofline_of(kern_s, units, peak_gbs, peak_src, bytes_per_unit, workload=None
                                "note": "sum of the families' algorithmic bytes x units / step time / HBM peak"},
             "strict_32B": {"frac": round(32.0 * units / t * 1e-9 / peak_gbs, 4),
                            "note": "compulsory traffic (read psi + write H psi) x units / step time / HBM peak"},
+            "dram_traffic": dram,
             "note": "achieved = algorithmic bytes of all launches of this family in one step / their summed CUDA-event "
                     "time (separate profiling pass of the same steps)"}
 
