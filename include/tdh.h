@@ -104,7 +104,8 @@ int tdh_apply_hamiltonian(tdh_grid* g, int nst, const tdh_c128* psi_dev, tdh_c12
  * Blocks of at most 128 MiB (the launch-latency regime) are replayed as one CUDA graph: the first call with a given
  * (psi_dev, nst, dt, nsteps) captures the call's launches on an internal stream and instantiates the graph (host work
  * only, nothing is allocated on the device), later calls with the same arguments launch that graph on the handle's
- * stream; any tdh_set_* call, another buffer or another count captures anew.  The result is bitwise that of the plain
+ * stream; any tdh_set_* call captures anew, and the handle keeps the graphs of the last four (buffer, count)
+ * combinations.  The result is bitwise that of the plain
  * launches.  TDH_GRAPH=0 in the environment at tdh_create_grid switches the graph off. */
 int tdh_propagate(tdh_grid* g, int nst, tdh_c128* psi_dev, double dt, int nsteps, int order);
 

@@ -172,7 +172,9 @@ struct tdh_grid {
 
     // tdh_propagate on small blocks: the launches of one call captured once into a CUDA graph and replayed while the
     // call's arguments and the handle's tables stay the same (`epoch` counts every change of the handle)
-    struct { cudaGraphExec_t exec; const void* psi; int nst, nsteps, launches; double dt; unsigned epoch; } pg;
+    struct PropGraph { cudaGraphExec_t exec; const void* psi; int nst, nsteps, launches; double dt; unsigned epoch; };
+    PropGraph pg[4];      // a few entries: callers that alternate between buffers keep their graphs
+    int pg_next;          // round-robin replacement
     unsigned epoch;
     bool use_graph;
     cudaStream_t s_cap;
@@ -498,7 +500,7 @@ extern "C" int tdh_destroy_grid(tdh_grid* g) {
         if (g->ev_k[i]) cudaEventDestroy(g->ev_k[i]);
         if (g->ev_out[i]) cudaEventDestroy(g->ev_out[i]);
     }
-    if (g->pg.exec) cudaGraphExecDestroy(g->pg.exec);
+    for (auto& e : g->pg) if (e.exec) cudaGraphExecDestroy(e.exec);
     if (g->s_cap) cudaStreamDestroy(g->s_cap);
     if (g->s_h2d) cudaStreamDestroy(g->s_h2d);
     if (g->s_d2h) cudaStreamDestroy(g->s_d2h);
@@ -1244,32 +1246,36 @@ extern "C" int tdh_propagate(tdh_grid* g, int nst, tdh_c128* psi_dev, double dt,
     const size_t block_bytes = (size_t)nst * g->np * sizeof(cd);
     const long nodes = (long)nsteps * 4 * 6 * ((nst + g->chunk - 1) / g->chunk);
     if (g->use_graph && !g->profiling && nsteps > 0 && block_bytes <= ((size_t)128 << 20) && nodes <= 8192) {
-        const bool hit = g->pg.exec && g->pg.psi == (const void*)psi_dev && g->pg.nst == nst && g->pg.nsteps == nsteps &&
-                         g->pg.dt == dt && g->pg.epoch == g->epoch;
-        if (!hit) {
-            if (g->pg.exec) { cudaGraphExecDestroy(g->pg.exec); g->pg.exec = nullptr; }
+        tdh_grid::PropGraph* pg = nullptr;
+        for (auto& e : g->pg)
+            if (e.exec && e.psi == (const void*)psi_dev && e.nst == nst && e.nsteps == nsteps && e.dt == dt && e.epoch == g->epoch) pg = &e;
+        if (!pg) {
+            tdh_grid::PropGraph& e = g->pg[g->pg_next];
+            g->pg_next = (g->pg_next + 1) % 4;
+            if (e.exec) { CU(cudaStreamSynchronize(g->stream)); cudaGraphExecDestroy(e.exec); e.exec = nullptr; }   // not while it may run
             if (!g->s_cap) CU(cudaStreamCreateWithFlags(&g->s_cap, cudaStreamNonBlocking));
             cudaStream_t user = g->stream;
             g->stream = g->s_cap;
             cudaGraph_t graph = nullptr;
-            cudaError_t e = cudaStreamBeginCapture(g->s_cap, cudaStreamCaptureModeThreadLocal);
-            int rc = e == cudaSuccess ? propagate_block(g, nst, (cd*)psi_dev, dt, nsteps) : TDH_ECUDA;
-            if (e == cudaSuccess) e = cudaStreamEndCapture(g->s_cap, &graph);
+            cudaError_t ce = cudaStreamBeginCapture(g->s_cap, cudaStreamCaptureModeThreadLocal);
+            int rc = ce == cudaSuccess ? propagate_block(g, nst, (cd*)psi_dev, dt, nsteps) : TDH_ECUDA;
+            if (ce == cudaSuccess) ce = cudaStreamEndCapture(g->s_cap, &graph);
             g->stream = user;
-            if (rc == TDH_OK && e == cudaSuccess && graph) e = cudaGraphInstantiate(&g->pg.exec, graph, 0);
+            if (rc == TDH_OK && ce == cudaSuccess && graph) ce = cudaGraphInstantiate(&e.exec, graph, 0);
             if (graph) cudaGraphDestroy(graph);
-            if (rc != TDH_OK || e != cudaSuccess || !g->pg.exec) {
+            if (rc != TDH_OK || ce != cudaSuccess || !e.exec) {
                 (void)cudaGetLastError();                 // capture is an optimisation: fall back to plain launches
-                g->pg.exec = nullptr;
+                e.exec = nullptr;
                 g->use_graph = false;
             } else {
-                g->pg.psi = psi_dev; g->pg.nst = nst; g->pg.nsteps = nsteps; g->pg.dt = dt; g->pg.epoch = g->epoch;
-                g->pg.launches = g->launch_count;
+                e.psi = psi_dev; e.nst = nst; e.nsteps = nsteps; e.dt = dt; e.epoch = g->epoch;
+                e.launches = g->launch_count;
+                pg = &e;
             }
         }
-        if (g->pg.exec) {
-            CU(cudaGraphLaunch(g->pg.exec, g->stream));
-            g->launch_count = g->pg.launches;
+        if (pg) {
+            CU(cudaGraphLaunch(pg->exec, g->stream));
+            g->launch_count = pg->launches;
             return TDH_OK;
         }
         stats_reset(g);

@@ -187,6 +187,7 @@ def test_propagate_graph_replay_and_invalidation(torch_cuda, B, oracle, monkeypa
             g.propagate(d, dt, 2)
             c = d.cpu().numpy()
             e = torch.from_numpy(psi).cuda()
+            g.set_chunk_states(3)                                    # several chunks inside one captured call
             g.propagate(e, dt, 1)
             dd = e.cpu().numpy()
             assert g.last_launch_count() == 4 * (g.last_launch_count() // 4)
