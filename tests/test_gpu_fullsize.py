@@ -251,9 +251,12 @@ def test_scatter_by_bulk_reduce_add_equals_read_modify_write(torch_cuda, B, orac
     torch = torch_cuda
     monkeypatch.setenv("TDH_NL_MODE", "1")
     cases = [(280, (32, 96, 96), 9, 1, (0.0, 0.0, 0.0)), (281, (48, 48, 32), 7, 2, (0.1, 0.0, -0.2)),
-             (282, (24, 36, 54), 5, 1, (0.0, 0.25, 0.0))]
+             (282, (24, 36, 54), 5, 1, (0.0, 0.25, 0.0)), (283, (16, 27, 9), 4, 1, (0.0, 0.0, 0.0))]
     for cid, n, natoms, lmax, kfrac in cases:
-        cfg = W.test_config(cid, n, tuple(0.42 * m for m in n), nst=11, natoms=natoms, lmax=lmax, rc=3.4,
+        # (16, 27, 9): odd row length 9 with spheres wider than the cell in z -- runs of consecutive flat indices that
+        # continue from the end of one row into the next
+        cfg = W.test_config(cid, n, tuple(0.42 * m for m in n), nst=11, natoms=natoms, lmax=lmax,
+                            rc=3.4 if cid != 283 else 1.8,
                             dl=(2.0, -0.8, 0.3)[: lmax + 1], kfrac=kfrac)
         wl = W.make(cfg)
         psi = W.states(cfg)
