@@ -37,6 +37,7 @@
  * ENVIRONMENT.  Read when a handle is created (TDH_NL_MODE, TDH_SCATTER_BULK: when projectors are set); all optional, the
  * defaults are the measured-best choices, the variables exist so that tests and profiles can run every path:
  *   TDH_SMALL=0             16^3 / 32^3 grids through the tiled kernels instead of the one-launch on-chip kernel
+ *   TDH_SMALL16_CLUSTER=0   16^3 blocks of few states with one CTA per state instead of a cluster of four
  *   TDH_NL_MODE=0|1         back-projection as record lists inside the inverse transform (0) or as its own kernel (1)
  *   TDH_SCATTER_BULK=0|1    that kernel by load-add-store (0) or by bulk reduce-add in the L2 (1)
  *   TDH_GRAPH=0             tdh_propagate always as plain launches

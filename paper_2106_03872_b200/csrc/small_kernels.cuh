@@ -47,7 +47,7 @@ template <int N, int CS> struct SmallCfg {
     static constexpr int ROWS = NJ * N;
     static constexpr int CELLS = ROWS * N;
     static constexpr int T = N == 32 ? TDH_SMALL_T32 : SMALL_T;
-    static_assert(NJ == 16 || NJ == 8, "local x transform is one radix-16 or radix-8 pass");
+    static_assert(NJ == 16 || NJ == 8 || NJ == 4, "local x transform is one radix-16, radix-8 or radix-4 pass");
     static_assert(CS == 1 || CS == 4, "cluster of one or four CTAs");
     static_assert((2 * N + NJ) * sizeof(cd) <= SMALL_HEADER, "twiddle tables must fit in the header");
 };

@@ -114,6 +114,7 @@ struct tdh_grid {
     int small_cs;         // 0: not available; else the cluster size
     const void* small_fn;
     int small_cells;
+    bool small16_cluster; // 16^3: the four-CTA cluster variant for blocks of few states (TDH_SMALL16_CLUSTER=0 switches it off)
 
     // general axis lengths (generic_fft.cuh): any n[a] = 2^a 3^b in [4, 256] outside the tuned set {16, 32, 48, 64, 96}
     bool generic;
@@ -438,6 +439,12 @@ static int create_impl(const int n[3], const double len[3], const double kpt[3],
             if (!(e && atoi(e) == 0)) {
                 if (n[0] == 16) { g->small_cs = 1; g->small_fn = (const void*)&tdh::small_h_kernel<16, 1>; g->small_cells = tdh::SmallCfg<16, 1>::CELLS; }
                 else { g->small_cs = 4; g->small_fn = (const void*)&tdh::small_h_kernel<32, 4>; g->small_cells = tdh::SmallCfg<32, 4>::CELLS; }
+                g->small16_cluster = n[0] == 16;
+                if (const char* e2 = getenv("TDH_SMALL16_CLUSTER")) g->small16_cluster = g->small16_cluster && atoi(e2) != 0;
+                if (n[0] == 16)
+                    CU(cudaFuncSetAttribute((const void*)&tdh::small_h_kernel<16, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                            (int)(tdh::SMALL_HEADER + (size_t)tdh::SmallCfg<16, 4>::CELLS * sizeof(cd) +
+                                                  (size_t)(tdh::SMALL_SEG_ENTRIES + 2 * tdh::SMALL_MAX_CHAN + 16) * sizeof(cd))));
                 CU(cudaFuncSetAttribute(g->small_fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                         (int)(tdh::SMALL_HEADER + (size_t)g->small_cells * sizeof(cd) +
                                               (size_t)(tdh::SMALL_SEG_ENTRIES + 2 * tdh::SMALL_MAX_CHAN + 16) * sizeof(cd))));
@@ -1087,20 +1094,27 @@ static int launch_small(tdh_grid* g, int nst, const cd* in, cd* out, cd alpha, c
     void* args[] = {(void*)&in, (void*)&out, (void*)&twx, (void*)&twy, (void*)&twz, (void*)&kin, (void*)&ep, (void*)&pj};
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
-    cfg.gridDim = dim3((unsigned)(nst * g->small_cs));
+    // 16^3 with few states: a cluster of four CTAs per state (the machine is mostly idle with one CTA per state, and a
+    // pass over a quarter of the state is a quarter of the latency); with many states one CTA per state (no DSMEM stage)
+    int cs = g->small_cs, cells = g->small_cells;
+    const void* fn = g->small_fn;
+    if (g->small_cs == 1 && g->small16_cluster && nst * 4 <= g->nsm) {
+        cs = 4; cells = tdh::SmallCfg<16, 4>::CELLS; fn = (const void*)&tdh::small_h_kernel<16, 4>;
+    }
+    cfg.gridDim = dim3((unsigned)(nst * cs));
     cfg.blockDim = dim3(g->small_cs == 1 ? tdh::SmallCfg<16, 1>::T : tdh::SmallCfg<32, 4>::T);
-    cfg.dynamicSmemBytes = tdh::small_smem(g->small_cells, g->natoms, g->nchan_tot);
+    cfg.dynamicSmemBytes = tdh::small_smem(cells, g->natoms, g->nchan_tot);
     cfg.stream = g->stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = (unsigned)g->small_cs;
+    attr[0].val.clusterDim.x = (unsigned)cs;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     int rc_ = prof_begin(g, K_PLANE_INV);
     if (rc_) return rc_;
-    CU(cudaLaunchKernelExC(&cfg, g->small_fn, args));
+    CU(cudaLaunchKernelExC(&cfg, fn, args));
     g->launch_count += 1;
     return prof_end(g);
 }

@@ -196,3 +196,29 @@ def test_propagate_graph_replay_and_invalidation(torch_cuda, B, oracle, monkeypa
         results[graph] = (a, b, c, dd)
     for x, y in zip(results["1"], results["0"]):
         assert np.array_equal(x, y)                                  # the graph replays the same kernels: bitwise equal
+
+
+@pytest.mark.parametrize("cluster", ["1", "0"])
+def test_16cubed_cluster_and_single_cta_variants(torch_cuda, B, oracle, monkeypatch, cluster):
+    """16^3 blocks of few states run a cluster of four CTAs per state (radix-4 local x transform, radix-4 over distributed
+    shared memory), blocks of many states one CTA per state: both against the oracle, with projectors of 1 and 9 channels,
+    k != 0 and a cutoff; 40 states make the library switch to one CTA per state by itself."""
+    torch = torch_cuda
+    monkeypatch.setenv("TDH_SMALL16_CLUSTER", cluster)
+    for cid, nst, natoms, lmax, kfrac, ecut in ((910, 8, 2, 0, (0.0, 0.0, 0.0), None), (911, 5, 3, 2, (0.25, 0.0, -0.1), 12.0),
+                                                (912, 40, 2, 1, (0.0, 0.0, 0.0), None)):
+        kw = dict(nst=nst, natoms=natoms, lmax=lmax, rc=2.0, dl=(1.5, -0.8, 0.3)[: lmax + 1], kfrac=kfrac)
+        if ecut:
+            kw["ecut"] = ecut
+        cfg = W.test_config(cid, (16, 16, 16), (10.0, 10.0, 10.0), **kw)
+        wl = W.make(cfg)
+        psi = W.states(cfg)
+        ref_h = oracle.apply_workload(wl, psi, oracle.DIRECT)
+        ref_p = oracle.propagate_workload(wl, psi, dt=0.02, nsteps=2, backend=oracle.DIRECT)
+        with B.grid_for(wl) as g:
+            d = torch.from_numpy(psi).cuda()
+            out = g.apply_hamiltonian(d)
+            assert g.last_launch_count() == 1
+            assert per_state_rel(out.cpu().numpy(), ref_h).max() < TOL, (cid, cluster)
+            g.propagate(d, 0.02, 2)
+            assert per_state_rel(d.cpu().numpy(), ref_p).max() < TOL, (cid, cluster)
