@@ -106,9 +106,9 @@ small_h_kernel(const cd* __restrict__ psi, cd* __restrict__ out, const cd* __res
     }
     for (int i = tid; i < NJ; i += T) stw_x[i] = ldg_cd(tw_x + (crank * i) % N);
     for (int i = tid; i < pj.nchan_tot + 16; i += T) dsum[i] = make_double2(0.0, 0.0);
-    // ---- load the CTA's planes, natural (y, z) order into swizzled cells; eight loads in flight per thread
+    // ---- load the CTA's planes, natural (y, z) order into swizzled cells; sixteen loads in flight per thread
     {
-        constexpr int U = 8;
+        constexpr int U = 16;
         for (int i0 = tid; i0 < C::CELLS; i0 += U * T) {
             cd v[U];
 #pragma unroll
@@ -400,11 +400,11 @@ small_h_kernel(const cd* __restrict__ psi, cd* __restrict__ out, const cd* __res
         }
     }
 
-    // ---- epilogue: out = alpha * (tile + V psi) + y, natural order, coalesced; four points per thread in flight
+    // ---- epilogue: out = alpha * (tile + V psi) + y, natural order, coalesced; eight points per thread in flight
     cd* out_s = out + (size_t)st * N * PLANE;
     const cd* yv_s = ep.yv != nullptr ? ep.yv + (size_t)st * N * PLANE : nullptr;
     {
-        constexpr int U = 4;
+        constexpr int U = 8;
         for (int i0 = tid; i0 < C::CELLS; i0 += U * T) {
             double vv[U];
             cd ph[U], ya[U];
