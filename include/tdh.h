@@ -290,6 +290,35 @@ int tdh_measure_fp64_mma_peak(double* tflops_out);
  * [0, max_states], TDH_ENOMEM / TDH_ECUDA when an allocation fails (what was allocated before stays). */
 int tdh_reserve(tdh_grid* g, int rotation_states, int forces_local_term, int host_buffers);
 
+/* The overlap matrix of tdh_overlap for callers that may not allocate device memory and have no handle:
+ *     S[i][j] = dV sum_p conj(a_i[p]) b_j[p],   i < na, j < nb,   row-major [na][nb] complex128
+ * Meant for a host program whose own pool owns the device's memory (a cudaMalloc beside it fails or fragments it;
+ * PAPER.md:326), for a time-stepping loop that cannot take cudaMalloc's device-wide synchronisation, and for anybody who
+ * wants this one number check (are my states still orthonormal?) without creating a tdh_grid and its gigabytes of
+ * workspace.  The call allocates nothing, on the host or on the device, and frees nothing: the split-K partial tiles live
+ * in one fixed array of TDH_NOALLOC_SCRATCH_BYTES that is part of the library image, so every device that uses libtdh.so
+ * gives up that much memory until the process exits.
+ *   npts      number of grid points of a state (any value >= 1; no divisibility requirement)
+ *   dv        the volume element dV (1.0 for a plain a^H b)
+ *   na, nb    states in a and b, each in [1, TDH_NOALLOC_MAX_STATES]; larger blocks: TDH_EUNSUPPORTED, and the message says
+ *             to use tdh_overlap
+ *   a_dev, b_dev   DEVICE, na*npts / nb*npts complex128, on the CURRENT device (may be the same block: only the upper
+ *                  tiles are then computed and mirrored)
+ *   s_dev     DEVICE, na*nb complex128, must not overlap a or b
+ *   cuda_stream    a cudaStream_t of the current device, or NULL
+ * Asynchronous on that stream.  Slices of K are summed in order: the result is deterministic for given sizes on a given
+ * GPU model, and equals tdh_overlap's up to the rounding of a different slice count.
+ * SHARED SCRATCH: all calls of the process use the same array (it still holds the previous call's partial tiles; the
+ * call overwrites every cell it reads, nothing has to be cleared).  Calls that can run at the same time on one device --
+ * different streams, or different threads without ordering -- race on it; keep them on one stream or order them.
+ * FIRST CALL: the first call on each device looks up the array's device address (and makes the runtime load the
+ * library's kernels there); make it once at start-up with that device current, before any stream capture and before
+ * the phase in which the program must not block. */
+#define TDH_NOALLOC_MAX_STATES 256
+#define TDH_NOALLOC_SCRATCH_BYTES (8u << 20)
+int tdh_overlap_noalloc(size_t npts, double dv, int na, const tdh_c128* a_dev, int nb, const tdh_c128* b_dev,
+                        tdh_c128* s_dev, void* cuda_stream);
+
 /* Tuning knob: how many states are pushed through the kernel chain together (0 = library default: as many as the
  * handle's workspace of at most 4 GiB per buffer holds, a multiple of 8 when a block has to be split -- measured on
  * B200, longer launches are never slower than L2-resident small chunks). */

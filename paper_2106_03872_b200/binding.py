@@ -29,6 +29,7 @@ SYMBOLS = (
     "tdh_create_slab_grid", "tdh_slab_buffers", "tdh_slab_set_peers", "tdh_slab_apply_phase", "tdh_slab_fft_phase", "tdh_work_layout",
     "tdh_ipc_export", "tdh_ipc_import", "tdh_ipc_close", "tdh_measure_fp64_mma_peak", "tdh_last_jacobi_sweeps",
     "tdh_set_profiling", "tdh_last_kernel_seconds", "tdh_kernel_name", "tdh_set_chunk_states", "tdh_reserve", "tdh_last_error",
+    "tdh_overlap_noalloc",
 )
 NKERNELS = 5
 
@@ -91,6 +92,7 @@ def lib() -> C.CDLL:
     l.tdh_kernel_name.argtypes = [i]
     l.tdh_kernel_name.restype = C.c_char_p
     l.tdh_set_chunk_states.argtypes = [vp, i]
+    l.tdh_overlap_noalloc.argtypes = [C.c_size_t, d, i, vp, i, vp, vp, vp]
     l.tdh_last_error.argtypes = []
     l.tdh_last_error.restype = C.c_char_p
     for s in SYMBOLS:
@@ -103,6 +105,36 @@ def lib() -> C.CDLL:
 def _check(rc: int):
     if rc != 0:
         raise TdhError(rc, lib().tdh_last_error().decode(errors="replace"))
+
+
+NOALLOC_MAX_STATES = 256          # TDH_NOALLOC_MAX_STATES
+NOALLOC_SCRATCH_BYTES = 8 << 20   # TDH_NOALLOC_SCRATCH_BYTES
+
+
+def overlap_noalloc(a, b=None, dv: float = 1.0, out=None, stream: Optional[int] = None):
+    """S[i][j] = dv sum_p conj(a_i[p]) b_j[p] through tdh_overlap_noalloc: no handle, and nothing is allocated inside the
+    call (its scratch is a fixed 8 MiB array inside libtdh.so), for programs whose own pool owns the device memory or
+    that cannot take an allocation's synchronisation in their time loop.  a, b: complex128 device tensors (states, ...)
+    with the same number of points per state, at most 256 states each; pass `out` (na, nb) to keep this wrapper from
+    allocating the result as well.  Every call shares the scratch array: keep calls on one stream.  Make the first call
+    on a device at start-up (it looks up the array's address there)."""
+    import torch
+    if b is None:
+        b = a
+    for t in (a, b):
+        assert t.is_cuda and t.dtype == torch.complex128 and t.is_contiguous() and t.dim() >= 2
+    na, nb = int(a.shape[0]), int(b.shape[0])
+    npts = a[0].numel()
+    assert b[0].numel() == npts, "a and b must have the same number of grid points per state"
+    if out is None:
+        out = torch.empty((na, nb), dtype=torch.complex128, device=a.device)
+    assert out.is_cuda and out.dtype == torch.complex128 and out.is_contiguous() and out.numel() == na * nb
+    if stream is None:
+        stream = torch.cuda.current_stream(a.device).cuda_stream
+    with torch.cuda.device(a.device):
+        _check(lib().tdh_overlap_noalloc(npts, float(dv), na, C.c_void_p(a.data_ptr()), nb, C.c_void_p(b.data_ptr()),
+                                         C.c_void_p(out.data_ptr()), C.c_void_p(stream)))
+    return out
 
 
 def _host_ptr(a) -> int:

@@ -65,6 +65,9 @@ static int fail(int code, const char* fmt, ...) {
 
 extern "C" const char* tdh_last_error(void) { return g_err; }
 
+// for the other translation units of the library (overlap_noalloc.cu): record the message of a failing call
+int tdh_detail_set_error(int code, const char* msg) { return fail(code, "%s", msg); }
+
 // ------------------------------------------------------------------------------------------------------------
 // handle
 // ------------------------------------------------------------------------------------------------------------
