@@ -41,9 +41,8 @@
  *   TDH_NL_MODE=0|1         back-projection as record lists inside the inverse transform (0) or as its own kernel (1)
  *   TDH_SCATTER_BULK=0|1    that kernel by load-add-store (0) or by bulk reduce-add in the L2 (1)
  *   TDH_GRAPH=0             tdh_propagate always as plain launches
- *   TDH_CHUNK_STATES=n, TDH_WORKSPACE_MB=m, TDH_MAX_LAUNCH_MB=m (0: none), TDH_MAX_CTAS_PER_SM=c, TDH_JACOBI_CTAS_PER_SM=c
- *                           states per launch, workspace per buffer (default 4096), bound of a launch of the small-plane tile
- *                           configurations (default 128), persistent-grid sizes
+ *   TDH_CHUNK_STATES=n, TDH_WORKSPACE_MB=m, TDH_MAX_CTAS_PER_SM=c, TDH_JACOBI_CTAS_PER_SM=c
+ *                           states per launch, workspace per buffer (default 4096), persistent-grid sizes
  *
  * There is no CPU fallback anywhere in this library.
  */

@@ -221,24 +221,10 @@ static void free_projectors(tdh_grid* g) {
     g->nl_layers = 0; g->nl_nrec = 0; g->nl_cmax = 0;
 }
 
-// Largest number of states one launch may cover.  The workspace bound, and for the tile configurations that put several
-// small planes into one tile of less than 72 KB (16 x 16 ... 32 x 48 planes; 48 x 48 planes, two to a 72 KB tile, are not
-// among them) at most 128 MB of states: on B200 (driver 580.159) tile_fwd launches of those configurations whose loads
-// and stores each span more than 128 MB end now and then with "unspecified launch failure" -- with the loads OR the
-// stores confined to a few MB, or with 128 MB per launch, never in several thousand launches; 48 x 48 planes ran 39,600
-// unbounded applications of 0.4 - 0.9 GB clean.  The cause is not understood; the bound avoids it.
-// TDH_MAX_LAUNCH_MB overrides the 128 (0: no bound) -- for the stress runs that watch this.
-static int max_chunk(const tdh_grid* g) {
-    int c = g->chunk_cap;
-    const size_t tile_bytes = (size_t)g->tl.ppc * (g->n[1] / g->tl.s) * g->n[2] * sizeof(cd);
-    if (!g->generic && g->tl.ppc > 1 && tile_bytes < 73728) {
-        size_t lim_mb = 128;
-        if (const char* e = getenv("TDH_MAX_LAUNCH_MB")) { long v = atol(e); lim_mb = v > 0 ? (size_t)v : ((size_t)1 << 30); }
-        const size_t lim = (lim_mb << 20) / (g->np * sizeof(cd));
-        c = (int)std::max<size_t>(1, std::min<size_t>((size_t)c, lim));
-    }
-    return c;
-}
+// Largest number of states one launch may cover: what the workspace holds.  (Rounds 1-2 also bounded launches of the
+// small multi-plane tile configurations to 128 MB because tile_fwd failed now and then above that; the cause was a
+// phase-parity race in the tile ring, fixed by the armed flags of tile_kernels.cuh -- DESIGN.md section 16.)
+static int max_chunk(const tdh_grid* g) { return g->chunk_cap; }
 
 static int default_chunk(const tdh_grid* g) {
     // Measured on B200 (profiles/r01a_chunk_sweep.md): every kernel gets faster with more states per launch and the

@@ -99,6 +99,18 @@ __device__ __forceinline__ void group_sync(int grp) {
     asm volatile("bar.sync %0, %1;" ::"r"(grp + 1), "n"(NTHREADS) : "memory");
 }
 
+// armed[b] of the tile ring (see ARMED FLAGS at tile_fwd_kernel): set by the thread that armed full[b] for tile k ...
+__device__ __forceinline__ void ring_set_armed(volatile int* armed, int b, int k) {
+    __threadfence_block();                      // the mbarrier arrival before the flag
+    armed[b] = k;
+}
+// ... and awaited by every thread that is about to wait on the parity of tile k
+__device__ __forceinline__ void ring_wait_armed(const volatile int* armed, int b, int k) {
+    while (armed[b] < k) {}
+    __threadfence_block();                      // the flag before the mbarrier wait
+}
+constexpr int TILE_ARMED_OFF = 32;             // byte offset of armed[3] in the header (full[3] occupies bytes 0..23)
+
 // Slab decomposition (Fig. 6): with the grid split over `world` ranks, a rank holds the planes
 // x0 .. x0 + nx_local - 1 of every state in real space and the rows y0 .. y0 + ny_local - 1 (work-layout order) of ALL
 // planes in Fourier space.  The redistribution between the two ("all-to-all") is fused into the stores of the producing
@@ -122,6 +134,16 @@ struct SlabDst {
 // CTA's k-th tile (tile blockIdx.x + k*gridDim.x) lives in buffer k % 3 and is transformed by group k % 2, whose thread 0
 // refills the buffer with tile k + 3 when the group is done with it.  The groups only meet at the mbarriers of the
 // ring, so while one group sits in a shared-memory-bound or store-bound stage the other one keeps the FP64 pipe busy.
+//
+// ARMED FLAGS.  Buffer b is filled with tile k + 3 by the group that consumed tile k, but tile k + 3 is consumed by the
+// OTHER group, and an mbarrier wait carries one bit of phase.  A group that runs two tiles ahead of the other one
+// (a slow TMA load on one side is enough) would reach its wait for tile k + 6 while the barrier is still in tile k + 3's
+// phase, whose parity says "tile k's phase is complete": the wait would pass at once, the group would transform a
+// buffer that is being loaded or worked on, and would then arm the barrier a second time in one phase.  So every
+// buffer has a flag armed[b] = the last k whose load was armed on full[b] (written after the arrival that opens
+// the phase), and a group spins on armed[b] >= k before it waits on the parity of tile k: from then on the barrier is
+// in tile k's phase and the parity is unambiguous.  The spin cannot deadlock: the flag for tile k is set by the group
+// that finished tile k - 3, which only needed flags of earlier tiles.
 // ------------------------------------------------------------------------------------------------------------
 template <int NY, int NZ, bool SLAB>
 __global__ void __launch_bounds__(TileCfg<NY, NZ>::T, 1)
@@ -134,6 +156,7 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap map_in, cd* __restrict__ out
     static_assert(NB == 3 && TG % 32 == 0, "ring of three buffers shared by two warp groups");
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);
+    volatile int* armed = reinterpret_cast<volatile int*>(smem_raw + TILE_ARMED_OFF);
     cd* stw_z = reinterpret_cast<cd*>(smem_raw + TILE_TW_OFF);          // [k1][j2] = e^{+2 pi i k1 j2 / NZ}: a quarter-warp
                                                                         // reads 8 consecutive entries (no bank conflict)
     cd* stw_y = stw_z + NZ;                                             // e^{+2 pi i m / NY}
@@ -143,7 +166,7 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap map_in, cd* __restrict__ out
     uint64_t pol = policy_evict_first();
     if (threadIdx.x == 0) {
         tma_prefetch_desc(&map_in);
-        for (int b = 0; b < NB; ++b) mbar_init(full + b, 1);
+        for (int b = 0; b < NB; ++b) { mbar_init(full + b, 1); armed[b] = -1; }
         mbar_fence_init();
     }
     for (int i = threadIdx.x; i < NZ; i += T) stw_z[i] = ldg_cd(tw_z + (i >> 3) * (i & 7));   // [k1][j2]: w^(k1*j2)
@@ -155,6 +178,7 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap map_in, cd* __restrict__ out
         const int b = k % NB;
         const int part0 = t * C::PPC, plane = part0 / S, r = part0 % S;
         mbar_arrive_expect_tx(full + b, (uint32_t)C::TILE_BYTES);
+        ring_set_armed(armed, b, k);
         tma_load_4d(ring + (size_t)b * C::CELLS, &map_in, full + b, 0, r * R1Z, 0, plane, pol);
     };
     if (threadIdx.x == 0)
@@ -166,6 +190,7 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap map_in, cd* __restrict__ out
         const int b = k % NB;
         cd* sm = ring + (size_t)b * C::CELLS;
         const int part0 = t * C::PPC;
+        ring_wait_armed(armed, b, k);
         mbar_wait(full + b, (uint32_t)(k / NB) & 1u);
 
         // ---- z stage A, in place: radix R1Z over j1 (lines lr*R1Z + j1, position j2), twiddle w^(k1*j2)
@@ -342,6 +367,7 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
     static_assert(NB == 3 && TG % 32 == 0, "ring of three buffers shared by two warp groups");
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);
+    volatile int* armed = reinterpret_cast<volatile int*>(smem_raw + TILE_ARMED_OFF);
     cd* stw_z = reinterpret_cast<cd*>(smem_raw + TILE_TW_OFF);          // [k1][j2] = e^{+2 pi i k1 j2 / NZ}: a quarter-warp
                                                                         // reads 8 consecutive entries (no bank conflict)
     cd* stw_y = stw_z + NZ;                                             // e^{+2 pi i m / NY}
@@ -354,7 +380,7 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
         tma_prefetch_desc(&map_spec);
         if (have_v) tma_prefetch_desc(&map_phi);
         if (ep.yv != nullptr) tma_prefetch_desc(&map_yv);
-        for (int b = 0; b < NB; ++b) mbar_init(full + b, 1);
+        for (int b = 0; b < NB; ++b) { mbar_init(full + b, 1); armed[b] = -1; }
         mbar_fence_init();
     }
     for (int i = threadIdx.x; i < NZ; i += T) stw_z[i] = ldg_cd(tw_z + (i >> 3) * (i & 7));   // [k1][j2]: w^(k1*j2)
@@ -366,6 +392,7 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
         const int b = k % NB;
         const int part0 = t * C::PPC, plane = part0 / S, r = part0 % S;
         mbar_arrive_expect_tx(full + b, (uint32_t)C::TILE_BYTES);
+        ring_set_armed(armed, b, k);
         tma_load_4d(ring + (size_t)b * C::CELLS, &map_spec, full + b, 0, r * R1Z, 0, plane, pol);
     };
     if (threadIdx.x == 0)
@@ -381,6 +408,7 @@ tile_inv_kernel(const __grid_constant__ CUtensorMap map_spec, const __grid_const
             if (have_v) tma_prefetch_l2_4d(&map_phi, 0, (part0 % S) * R1Z, 0, part0 / S);
             if (ep.yv != nullptr) tma_prefetch_l2_4d(&map_yv, 0, (part0 % S) * R1Z, 0, part0 / S);
         }
+        ring_wait_armed(armed, b, k);
         mbar_wait(full + b, (uint32_t)(k / NB) & 1u);
 
         // ---- y stage A', in place: rows k1y*R2Y + k2y (contiguous) hold k = k1y + R1Y*k2y; radix R2Y over k2y -> j2,

@@ -126,9 +126,10 @@ def test_small_path_is_deterministic_and_independent_of_batching(torch_cuda, B):
 
 @pytest.mark.parametrize("small", ["0", "1"])
 def test_small_planes_many_states_stress(torch_cuda, B, oracle, monkeypatch, small):
-    """32^3 with 1024 states (512 MB blocks) through both paths, forty applications with re-created handles and tensors.
-    Regression test for the launch failures seen when one tile_fwd launch of a multi-plane-tile configuration spanned
-    more than 128 MB (max_chunk bounds the launch); sampled states against the oracle."""
+    """32^3 with 1024 states (one launch chain over the whole 512 MB block) through both paths, forty applications with
+    re-created handles and tensors, every application bitwise the first.  Regression test for the phase-parity race of
+    the tile ring: before the armed flags of tile_kernels.cuh such launches failed, or returned
+    wrong values, in most processes; sampled states against the oracle."""
     torch = torch_cuda
     import dataclasses
     monkeypatch.setenv("TDH_SMALL", small)
@@ -146,10 +147,13 @@ def test_small_planes_many_states_stress(torch_cuda, B, oracle, monkeypatch, sma
             psi[s].copy_(torch.from_numpy(host[j]))
         out = torch.empty_like(psi)
         with B.grid_for(wl) as g:
+            first = g.apply_hamiltonian(psi)
             for _ in range(8):
                 g.apply_hamiltonian(psi, out=out)
+                assert torch.equal(out, first)
             torch.cuda.synchronize()
-            assert g.last_launch_count() == (4 * 4 if small == "0" else 4)      # four chunks of 256 states (128 MB)
+            assert g.last_launch_count() == (4 if small == "0" else 1)          # one chunk: no bound on a launch
+            del first
             got = np.stack([out[s].cpu().numpy() for s in sample])
             assert per_state_rel(got, ref).max() < TOL
         del psi, out
