@@ -65,6 +65,30 @@ def test_p1_naive_fft_equals_direct_on_config_grids(oracle, N):
     assert rel(oracle.dft3d(a, +1, 1), oracle.dft3d(a, +1, 0)) < 1e-13
 
 
+@pytest.mark.parametrize("L", [4, 6, 8, 9, 12, 18, 24, 27, 36, 54, 72, 81, 108, 128, 144, 162, 192, 243, 256])
+def test_p1_naive_fft_equals_direct_on_every_axis_length_used_as_reference(oracle, L):
+    """the naive FFT back-end is "accepted once it matches the direct DFT ... on every grid size used".
+    The GPU tests use it as the reference on general grids too (tests/test_gpu_sizes.py, test_gpu_fullsize.py, smoke():
+    lengths 9, 12, 24, 27, 36, 54, 72, 81, 128 and the thin grids with 4, 6, 8, 18, 108, 144, 162, 192, 243, 256), so
+    every such length is checked here on each of the three axes of a thin grid, both directions."""
+    rng = np.random.default_rng(1000 + L)
+    for axis in range(3):
+        n = [4, 6, 4]
+        n[axis] = L
+        a = rand_c(rng, (2,) + tuple(n))
+        assert rel(oracle.dft3d(a, -1, 1), oracle.dft3d(a, -1, 0)) < 1e-13, (L, axis)
+        assert rel(oracle.dft3d(a, +1, 1), oracle.dft3d(a, +1, 0)) < 1e-13, (L, axis)
+
+
+@pytest.mark.parametrize("n", [(24, 36, 54), (72, 12, 9), (81, 27, 9), (128, 24, 16), (27, 27, 27), (54, 54, 54)])
+def test_p1_naive_fft_equals_direct_on_mixed_general_grids(oracle, n):
+    """The mixed general grids of the GPU parity tests, whole."""
+    rng = np.random.default_rng(sum(n))
+    a = rand_c(rng, (1,) + n)
+    assert rel(oracle.dft3d(a, -1, 1), oracle.dft3d(a, -1, 0)) < 1e-13
+    assert rel(oracle.dft3d(a, +1, 1), oracle.dft3d(a, +1, 0)) < 1e-13
+
+
 def test_p1_delta_and_shift_theorem(oracle):
     """A unit impulse at r0 transforms to the plane wave exp(-i G.r0): fixes the sign and index convention."""
     n = (6, 4, 8)
