@@ -153,9 +153,8 @@ int tdh_hartree(tdh_grid* g, const double* n_dev, double* vh_dev);
  *     S[i][j] = dV sum_p conj(a_i[p]) b_j[p],   i < na, j < nb,   row-major [na][nb] complex128
  * a_dev, b_dev: DEVICE blocks of na / nb states (may be the same block); s_dev: DEVICE, na*nb complex128.
  * A flop-bound complex GEMM on FP64 tensor cores, split over K with a deterministic reduction.  Uses the handle's
- * workspace (na, nb rounded up to 64 must satisfy na*nb <= workspace / 16 bytes).  n0*n1*n2 must be a multiple of 64
- * (TDH_EUNSUPPORTED otherwise; this also holds for tdh_rotate and the two calls built on them).  Asynchronous on the
- * handle's stream. */
+ * workspace (na, nb rounded up to 64 must satisfy na*nb <= workspace / 16 bytes).  Any grid the handle accepts (the
+ * last chunk of K, and the last tile of points of tdh_rotate, are predicated).  Asynchronous on the handle's stream. */
 int tdh_overlap(tdh_grid* g, int na, const tdh_c128* a_dev, int nb, const tdh_c128* b_dev, tdh_c128* s_dev);
 
 /* Rotation in the space of states ("rotations in the space of eigenvectors"):
@@ -174,9 +173,13 @@ int tdh_orthonormalize(tdh_grid* g, int nst, const tdh_c128* psi_dev, tdh_c128* 
 /* Subspace diagonalisation of an ORTHONORMAL block: M = dV psi^H (H psi) = V diag(w) V^H, out = psi V,
  * so that dV out^H H out = diag(w), w ascending.  hpsi_dev holds H psi (tdh_apply_hamiltonian).  tdh_overlap, a
  * cooperative parallel Jacobi eigensolver of the nst x nst Hermitian matrix, tdh_rotate.  1 <= nst <= 1024.
- * psi_dev, hpsi_dev, out_dev: DEVICE blocks of nst states, out must not overlap psi; eig_host: HOST [nst] or NULL
- * (the call synchronises when it is given).  The Ritz vectors are unique up to a phase and within degenerate
- * eigenspaces. */
+ * psi_dev, hpsi_dev, out_dev: DEVICE blocks of nst states, out must not overlap psi; eig_host: HOST [nst] or NULL.
+ * hpsi_dev must be a HERMITIAN operator applied to psi_dev (what tdh_apply_hamiltonian returns): only the tiles of M on
+ * and above the diagonal are computed and the others are taken as their conjugate transposes; for any other hpsi the
+ * result is the diagonalisation of that mirrored matrix, not of (M + M^H)/2.  Synchronises the stream (the sweep count
+ * and the convergence flag of the eigensolver are read back): TDH_ECUDA when the Jacobi iteration has not converged in
+ * 40 sweeps (non-finite input), out is then not a diagonalising rotation.  The Ritz vectors are unique up to a phase and
+ * within degenerate eigenspaces. */
 int tdh_subspace_diag(tdh_grid* g, int nst, const tdh_c128* psi_dev, const tdh_c128* hpsi_dev, tdh_c128* out_dev,
                       double* eig_host);
 
@@ -224,7 +227,10 @@ int tdh_forces(tdh_grid* g, int nst, const tdh_c128* psi_dev, const double* occ_
  * [2, 8] must divide n[0] and n[1]/2, and n[0]/world must be a multiple of the planes per tile (TDH_EUNSUPPORTED
  * otherwise).  On a slab handle tdh_set_potential takes the rank's planes of V ([n0/world][n1][n2]) and
  * tdh_set_projectors the sphere points inside the rank's planes with LOCAL flat indices ((x - x0) n1 + y) n2 + z and
- * the SAME atoms and channels on every rank (an atom may have no point on a rank); nst of a phase call is at most the
+ * the SAME atoms and channels on every rank (an atom may have no point on a rank); it frees and re-creates the rank's
+ * partial-projection buffer, so it is a collective step: every rank stops using (and, with CUDA IPC, closes) the peers'
+ * buffers first, and afterwards every rank calls tdh_slab_set_peers again -- until then the phase calls of this handle
+ * return TDH_EINVAL; nst of a phase call is at most the
  * workspace chunk (max_states if that fits 4 GiB).  The other entry points that transform along x refuse slab handles. */
 enum { TDH_SLAB_PROJECT = 0, TDH_SLAB_PLANES_FWD = 1, TDH_SLAB_PENCILS = 2, TDH_SLAB_PLANES_INV = 3 };
 int tdh_create_slab_grid(const int n[3], const double len[3], const double kpt[3], double ecut, int max_states,
@@ -265,7 +271,7 @@ int tdh_fft3d(tdh_grid* g, int nst, tdh_c128* psi_dev, int sign);
 /* Number of kernel launches the last tdh_apply_hamiltonian / tdh_propagate / *_host call of this handle enqueued. */
 int tdh_last_launch_count(const tdh_grid* g);
 
-/* Jacobi sweeps the last tdh_subspace_diag call of this handle needed (when it was given eig_host). */
+/* Jacobi sweeps the last tdh_subspace_diag call of this handle needed. */
 int tdh_last_jacobi_sweeps(const tdh_grid* g);
 
 /* Seconds (device time, CUDA events on the handle's stream) spent in each kernel family during the last call, when

@@ -353,16 +353,17 @@ class Grid:
                                 C.c_void_p(out.ctypes.data)))
         return out
 
-    def subspace_diag(self, psi, hpsi, out=None):
-        """Ritz values (ascending, host numpy) and Ritz vectors out = psi V of an orthonormal block; hpsi = H psi."""
+    def subspace_diag(self, psi, hpsi, out=None, want_eig: bool = True):
+        """Ritz values (ascending, host numpy; None with want_eig=False) and Ritz vectors out = psi V of an orthonormal
+        block; hpsi = H psi with a Hermitian H.  Raises TdhError when the eigensolver has not converged."""
         import torch
         nst = self._block(psi)
         assert self._block(hpsi) == nst
         if out is None:
             out = torch.empty_like(psi)
-        eig = np.empty(nst, dtype=np.float64)
+        eig = np.empty(nst, dtype=np.float64) if want_eig else None
         _check(lib().tdh_subspace_diag(self._h, nst, C.c_void_p(psi.data_ptr()), C.c_void_p(hpsi.data_ptr()),
-                                       C.c_void_p(out.data_ptr()), C.c_void_p(eig.ctypes.data)))
+                                       C.c_void_p(out.data_ptr()), None if eig is None else C.c_void_p(eig.ctypes.data)))
         return eig, out
 
     def sd_step(self, psi, lam: float, work=None, want_eig: bool = True):

@@ -68,16 +68,21 @@ jacobi_eigh_kernel(cd* __restrict__ a, cd* __restrict__ a2, cd* __restrict__ v, 
         v[e] = make_double2((e / n == e % n) ? 1.0 : 0.0, 0.0);
         const cd x = __ldcg(a + e);
         mx = fmax(mx, fmax(fabs(x.x), fabs(x.y)));
+        // fmax drops a NaN and the threshold test below never rotates one: a non-finite element is recorded as an
+        // infinite scale instead, which ends the solve as "not converged"
+        if (!(fabs(x.x) <= 1.7976931348623157e308) || !(fabs(x.y) <= 1.7976931348623157e308))
+            mx = __longlong_as_double(0x7ff0000000000000LL);
     }
     atomicMax(scale_word, (unsigned long long)__double_as_longlong(mx));
     grid_barrier();
     const double scale = __longlong_as_double((long long)*((volatile unsigned long long*)scale_word));
+    const bool finite = scale <= 1.7976931348623157e308;     // the same value in every CTA
     const double thr = JACOBI_TOL * scale;
     cd* cur = a;
     cd* nxt = a2;
     int sweep = 0;
     bool converged = false;
-    for (; sweep < JACOBI_MAX_SWEEPS && !converged; ++sweep) {
+    for (; finite && sweep < JACOBI_MAX_SWEEPS && !converged; ++sweep) {
         double tmax = 0.0;                                   // this thread's largest rotated |a_pq| of the sweep
         for (int r = 0; r < m - 1; ++r) {
             // ---- rotations of this step's pairs, computed by every CTA from the current matrix

@@ -26,7 +26,7 @@ constexpr int OV_KCP = 20;        // padded row length (doubles) of a state in s
 constexpr int OV_THREADS = 256;
 
 // grid: (tiles_i * tiles_j, ksplit).  part: [ksplit][na_pad][nb_pad] complex, na_pad = tiles_i*64, nb_pad = tiles_j*64.
-// Slice ks covers the chunks [ks*chunks_per_slice, (ks+1)*chunks_per_slice) of the N_p/16 chunks.
+// Slice ks covers the chunks [ks*chunks_per_slice, (ks+1)*chunks_per_slice) of the ceil(N_p/16) chunks.
 // hermitian != 0 (a and b are the same block): tiles below the diagonal are skipped, the reduction mirrors them.
 __global__ void __launch_bounds__(OV_THREADS)
 overlap_kernel(const cd* __restrict__ a, int na, const cd* __restrict__ b, int nb, size_t npts, int tiles_j,
@@ -40,7 +40,7 @@ overlap_kernel(const cd* __restrict__ a, int na, const cd* __restrict__ b, int n
     const int fr = lane >> 2, fk = lane & 3;                    // fragment row (state) and k (point)
     const int ti = blockIdx.x / tiles_j, tj = blockIdx.x % tiles_j;
     const int i0 = ti * OV_T, j0 = tj * OV_T;
-    const size_t nchunks = npts / OV_KC;
+    const size_t nchunks = (npts + OV_KC - 1) / OV_KC;           // the last chunk may be ragged (loads predicated)
     const size_t c_begin = (size_t)blockIdx.y * chunks_per_slice;
     const size_t c_end = c_begin + chunks_per_slice < nchunks ? c_begin + chunks_per_slice : nchunks;
 
@@ -63,8 +63,9 @@ overlap_kernel(const cd* __restrict__ a, int na, const cd* __restrict__ b, int n
 
     cd v[8];
     auto load = [&](size_t c) {
+        const bool inside = c * OV_KC + (tid & 15) < npts;       // every slot of this thread has point tid % 16
 #pragma unroll
-        for (int r = 0; r < 8; ++r) v[r] = ok[r] ? __ldcs(src[r] + c * OV_KC) : make_double2(0.0, 0.0);
+        for (int r = 0; r < 8; ++r) v[r] = (ok[r] && inside) ? __ldcs(src[r] + c * OV_KC) : make_double2(0.0, 0.0);
     };
     if (c_begin < c_end) load(c_begin);
     for (size_t c = c_begin; c < c_end; ++c) {
@@ -149,7 +150,7 @@ constexpr int RT_J = 64;          // output states per tile
 constexpr int RT_KC = 16;         // input states per chunk
 constexpr int RT_LD = 68;         // padded row length (doubles)
 
-// grid: (N_p / 64, ceil(n_out / 64))
+// grid: (ceil(N_p / 64), ceil(n_out / 64)); loads and stores of the last tile of points are predicated
 __global__ void __launch_bounds__(OV_THREADS)
 rotate_kernel(const cd* __restrict__ psi, int n_in, const cd* __restrict__ m, int n_out, size_t npts, int upper,
               cd* __restrict__ out)
@@ -176,7 +177,7 @@ rotate_kernel(const cd* __restrict__ psi, int n_in, const cd* __restrict__ m, in
         for (int r = 0; r < 4; ++r) {
             const int idx = tid + OV_THREADS * r, row = idx >> 6, col = idx & 63;
             const int i = k0 + row;
-            va[r] = i < k_end ? __ldcs(psi + (size_t)i * npts + p0 + col) : make_double2(0.0, 0.0);
+            va[r] = (i < k_end && p0 + col < npts) ? __ldcs(psi + (size_t)i * npts + p0 + col) : make_double2(0.0, 0.0);
             vb[r] = (i < k_end && j0 + col < n_out) ? __ldg(m + (size_t)i * n_out + j0 + col) : make_double2(0.0, 0.0);
         }
     };
@@ -221,6 +222,7 @@ rotate_kernel(const cd* __restrict__ psi, int n_in, const cd* __restrict__ m, in
         for (int jt = 0; jt < 2; ++jt) {
             const size_t p = p0 + wp * 32 + it * 8 + fr;
             const int j = j0 + wj * 16 + jt * 8 + 2 * fk;
+            if (p >= npts) continue;                             // ragged last tile of points
             if (j < n_out) __stcs(out + (size_t)j * npts + p, make_double2(cre[it][jt][0], cim[it][jt][0]));
             if (j + 1 < n_out) __stcs(out + (size_t)(j + 1) * npts + p, make_double2(cre[it][jt][1], cim[it][jt][1]));
         }

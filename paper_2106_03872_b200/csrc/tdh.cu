@@ -136,6 +136,7 @@ struct tdh_grid {
     bool have_peers;
 
     int chunk_cap;        // states the workspace can hold
+    size_t work_cells;    // complex values d_work holds (>= chunk_cap * np)
     int chunk;            // states pushed through the chain together
     cd* d_work;
     cd* d_phi[2];
@@ -450,7 +451,13 @@ static int create_impl(const int n[3], const double len[3], const double kpt[3],
         if (const char* e = getenv("TDH_WORKSPACE_MB")) { long v = atol(e); if (v > 0) ws_bytes = (size_t)v << 20; }
         size_t cap = std::max<size_t>(1, ws_bytes / state_bytes);
         g->chunk_cap = (int)std::min<size_t>(cap, (size_t)max_states);
-        CU(cudaMalloc(&g->d_work, state_bytes * g->chunk_cap));
+        // the work buffer also holds the split-K partial tiles of tdh_overlap: on very small grids (9^3 ...) a chunk of
+        // states is smaller than one padded tile grid of the block, so it is at least that (<= 16 MiB)
+        {
+            const size_t pad = ((size_t)std::min(max_states, 1024) + 63) / 64 * 64;
+            g->work_cells = std::max<size_t>((size_t)g->chunk_cap * g->np, pad * pad);
+        }
+        CU(cudaMalloc(&g->d_work, sizeof(cd) * g->work_cells));
         // at least two states each: tdh_taylor_pair keeps phi_2 and phi_3 in the two halves of d_phi[0]
         CU(cudaMalloc(&g->d_phi[0], state_bytes * std::max(2, g->chunk_cap)));
         CU(cudaMalloc(&g->d_phi[1], state_bytes * std::max(2, g->chunk_cap)));
@@ -744,6 +751,11 @@ extern "C" int tdh_set_projectors(tdh_grid* g, int natoms, const int64_t* sph_of
     g->d_sphase = nw->d_sphase; g->d_dscale = nw->d_dscale; g->d_nl_off = nw->d_nl_off; g->d_nl_cc = nw->d_nl_cc;
     g->d_nl_beta = nw->d_nl_beta; g->d_nl_phase = nw->d_nl_phase; g->d_dpi = nw->d_dpi; g->d_dvscale = nw->d_dvscale;
     g->d_dpig = nw->d_dpig; g->d_force = nw->d_force; g->d_dpi_part = nw->d_dpi_part;
+    if (g->slab_world > 1) {
+        // the partial-projection buffer the peers were given has just been freed: no phase may run on the old addresses
+        g->have_peers = false;
+        for (int q = 0; q < tdh::SLAB_MAX_WORLD; ++q) g->peer_dpi[q] = nullptr;
+    }
     g->natoms = natoms;
     g->nchan_tot = ctot;
     g->nl_layers = nlayers;
@@ -1696,13 +1708,12 @@ static int overlap_impl(tdh_grid* g, int na, const tdh_c128* a_dev, int nb, cons
                         bool result_is_hermitian) {
     if (!g || !a_dev || !b_dev || !s_dev) return fail(TDH_EINVAL, "tdh_overlap: null argument");
     if (na < 1 || nb < 1) return fail(TDH_EINVAL, "tdh_overlap: na, nb must be >= 1");
-    if (g->np % tdh::RT_P != 0) return fail(TDH_EUNSUPPORTED, "tdh_overlap: the GEMM kernels need n0*n1*n2 to be a multiple of %d", tdh::RT_P);
     stats_reset(g);
     const int ti = (na + tdh::OV_T - 1) / tdh::OV_T, tj = (nb + tdh::OV_T - 1) / tdh::OV_T;
     const size_t tile_cells = (size_t)ti * tj * tdh::OV_T * tdh::OV_T;
-    const size_t cap = (size_t)g->chunk_cap * g->np;                       // complex values the work buffer holds
+    const size_t cap = g->work_cells;                                      // complex values the work buffer holds
     if (tile_cells > cap) return fail(TDH_EUNSUPPORTED, "tdh_overlap: %d x %d does not fit the workspace", na, nb);
-    const size_t nchunks = g->np / tdh::OV_KC;
+    const size_t nchunks = (g->np + tdh::OV_KC - 1) / tdh::OV_KC;
     // enough slices of K for about four waves of CTAs, bounded by the workspace and by 8 chunks per slice
     int dev = 0, nsm = 0;
     CU(cudaGetDevice(&dev));
@@ -1737,7 +1748,7 @@ static int overlap_impl(tdh_grid* g, int na, const tdh_c128* a_dev, int nb, cons
 static int launch_rotate(tdh_grid* g, int n_in, const cd* in, int n_out, const cd* m, cd* out, int upper) {
     size_t npts = g->np;
     void* args[] = {(void*)&in, (void*)&n_in, (void*)&m, (void*)&n_out, (void*)&npts, (void*)&upper, (void*)&out};
-    dim3 grid((unsigned)(g->np / tdh::RT_P), (n_out + tdh::RT_J - 1) / tdh::RT_J);
+    dim3 grid((unsigned)((g->np + tdh::RT_P - 1) / tdh::RT_P), (n_out + tdh::RT_J - 1) / tdh::RT_J);
     CU(cudaLaunchKernel(reinterpret_cast<const void*>(&tdh::rotate_kernel), grid, dim3(tdh::OV_THREADS), args, 0, g->stream));
     g->launch_count += 1;
     return TDH_OK;
@@ -1748,7 +1759,6 @@ extern "C" int tdh_rotate(tdh_grid* g, int n_in, const tdh_c128* psi_dev, int n_
                           tdh_c128* out_dev) {
     if (!g || !psi_dev || !m_dev || !out_dev) return fail(TDH_EINVAL, "tdh_rotate: null argument");
     if (n_in < 1 || n_out < 1 || n_out > 65535 * tdh::RT_J) return fail(TDH_EINVAL, "tdh_rotate: bad n_in / n_out");
-    if (g->np % tdh::RT_P != 0) return fail(TDH_EUNSUPPORTED, "tdh_rotate: the GEMM kernels need n0*n1*n2 to be a multiple of %d", tdh::RT_P);
     {
         const char* x = (const char*)psi_dev;
         const char* y = (const char*)out_dev;
@@ -1814,15 +1824,15 @@ extern "C" int tdh_subspace_diag(tdh_grid* g, int nst, const tdh_c128* psi_dev, 
     CU(cudaGetLastError());
     g->launch_count += 3;
     if ((rc = launch_rotate(g, nst, (const cd*)psi_dev, nst, g->d_small[2], (cd*)out_dev, 0))) return rc;
-    if (eig_host) {
-        unsigned ctl_host[8] = {0};
-        CU(cudaMemcpyAsync(eig_host, g->d_w, sizeof(double) * nst, cudaMemcpyDeviceToHost, g->stream));
-        CU(cudaMemcpyAsync(ctl_host, g->d_ctl, sizeof(ctl_host), cudaMemcpyDeviceToHost, g->stream));
-        CU(cudaStreamSynchronize(g->stream));
-        g->jacobi_sweeps = (int)ctl_host[4];
-        if (ctl_host[5] != 0)
-            return fail(TDH_ECUDA, "tdh_subspace_diag: the Jacobi eigensolver did not converge in %u sweeps (non-finite input?)", ctl_host[4]);
-    }
+    // the sweep count and the non-convergence flag come back with or without eig_host: an unconverged rotation must not
+    // be returned as success
+    unsigned ctl_host[8] = {0};
+    if (eig_host) CU(cudaMemcpyAsync(eig_host, g->d_w, sizeof(double) * nst, cudaMemcpyDeviceToHost, g->stream));
+    CU(cudaMemcpyAsync(ctl_host, g->d_ctl, sizeof(ctl_host), cudaMemcpyDeviceToHost, g->stream));
+    CU(cudaStreamSynchronize(g->stream));
+    g->jacobi_sweeps = (int)ctl_host[4];
+    if (ctl_host[5] != 0)
+        return fail(TDH_ECUDA, "tdh_subspace_diag: the Jacobi eigensolver did not converge in %u sweeps (non-finite input?); out is not a diagonalising rotation", ctl_host[4]);
     return TDH_OK;
 }
 

@@ -228,6 +228,16 @@ class SlabRank:
         self.grid.set_potential(v_local)
 
     def set_projectors(self, proj_full):
+        """Collective.  tdh_set_projectors frees this rank's partial-projection buffer, which the peers have mapped through
+        CUDA IPC and read in their PLANES_FWD phase: first every rank finishes its phases (barrier), then every rank
+        closes its imports, and only after a second barrier -- nobody maps the old buffer any more -- is it freed and
+        replaced; connect() exports and imports the new ones."""
+        from . import binding
+        self._barrier()
+        for p in self._opened:
+            binding.ipc_close(p)
+        self._opened = []
+        self._barrier()
         x0, x1 = self.planes()
         self.grid.set_projectors(slab_projectors(proj_full, self.n, x0, x1))
         self.connect()

@@ -580,6 +580,29 @@ def test_subspace_diag_matches_oracle(torch_cuda, B, oracle, name, nst):
         assert sep.sum() >= nst // 2 and np.abs(ov[sep] - 1).max() < 1e-8
 
 
+@pytest.mark.parametrize("want_eig", [True, False])
+def test_subspace_diag_reports_an_unconverged_eigensolver(torch_cuda, B, oracle, want_eig):
+    """A subspace matrix with a non-finite entry cannot be diagonalised: the call fails whether or not the caller asked
+    for the Ritz values (without eig_host it used to return TDH_OK with an unconverged rotation); the next call works."""
+    torch = torch_cuda
+    cfg = W.CONFIGS["tiny"]
+    wl = W.make(cfg)
+    psi = oracle.orthonormalize(cfg.n, cfg.dv, W.states(cfg, 0, 8))
+    with B.grid_for(wl, max_states=8) as g:
+        d = torch.from_numpy(psi).cuda()
+        h = g.apply_hamiltonian(d)
+        bad = h.clone()
+        bad[3, 1, 2, 3] = float("nan")
+        with pytest.raises(B.TdhError) as err:
+            g.subspace_diag(d, bad, want_eig=want_eig)
+        assert err.value.code == B.TDH_ECUDA and "did not converge" in str(err.value)
+        w, out = g.subspace_diag(d, h, want_eig=want_eig)
+        assert (w is None) == (not want_eig)
+        m = g.overlap(out, g.apply_hamiltonian(out)).cpu().numpy()
+        assert np.abs(m - np.diag(np.diag(m))).max() < 1e-10 * max(1.0, np.abs(m).max())
+        assert g.last_jacobi_sweeps() >= 1
+
+
 def test_ground_state_iterations_converge_towards_the_lowest_eigenvalues(torch_cuda, B, oracle):
     """The eigensolver loop of PAPER.md:389-393 composed from the C-ABI calls (SD update, orthonormalisation, subspace
     diagonalisation) on a 16^3 grid: the trace over the subspace never increases, and the Ritz values stay above the lowest

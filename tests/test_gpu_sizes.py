@@ -82,8 +82,8 @@ def test_apply_and_propagate_general_sizes(torch_cuda, B, oracle, n, nst, natoms
 
 
 def test_other_entry_points_on_a_general_grid(torch_cuda, B, oracle):
-    """Density, Hartree, gradient, forces, SD step, Taylor pair on a (24, 36, 54) grid against the oracle; the GEMM-based
-    rotations work when the point count is a multiple of 64 and are refused otherwise."""
+    """Density, Hartree, gradient, forces, SD step, Taylor pair on a (24, 36, 54) grid against the oracle, and the GEMM-based
+    rotations (ragged point counts: test_rotations_on_grids_whose_point_count_is_ragged)."""
     torch = torch_cuda
     n = (24, 36, 54)
     cfg = W.test_config(650, n, (10.0, 15.0, 22.0), nst=6, natoms=3, lmax=1, rc=2.6, dl=(2.0, -0.8), kfrac=(0.0, 0.1, 0.0))
@@ -118,11 +118,35 @@ def test_other_entry_points_on_a_general_grid(torch_cuda, B, oracle):
         assert np.abs(s - oracle.overlap(cfg.n, cfg.dv, psi, psi)).max() < 1e-12
         q = g.orthonormalize(d)
         assert np.abs(g.overlap(q).cpu().numpy() - np.eye(cfg.nst)).max() < 1e-12
-    with B.Grid((9, 9, 9), (4.0, 4.0, 4.0), max_states=2) as g:
-        x = torch.zeros((2, 9, 9, 9), dtype=torch.complex128, device="cuda")
-        with pytest.raises(B.TdhError) as e:
-            g.overlap(x)
-        assert e.value.code == B.TDH_EUNSUPPORTED
+
+
+@pytest.mark.parametrize("n,nst", [((27, 27, 27), 8), ((9, 9, 9), 3), ((54, 54, 54), 5), ((81, 4, 6), 70)])
+def test_rotations_on_grids_whose_point_count_is_ragged(torch_cuda, B, oracle, n, nst):
+    """Overlap, rotation, orthonormalisation and subspace diagonalisation on grids whose point count is no multiple of 64
+    or even of 16 (27^3 = 19683, 9^3 = 729, 54^3 = 64 x 2460.4, 81 x 4 x 6 = 1944): the last chunk of K of the overlap GEMM
+    and the last tile of points of the rotation GEMM are predicated.  Against the oracle's literal sums."""
+    torch = torch_cuda
+    cfg = W.test_config(660 + n[0], n, tuple(max(0.45 * m, 4.4) for m in n), nst=nst, natoms=2, lmax=1, rc=1.9, dl=(2.0, -0.8))
+    wl = W.make(cfg)
+    psi = W.states(cfg)
+    rng = np.random.default_rng([W.BASE_SEED, 660, n[0], nst])
+    m = rng.standard_normal((nst, nst + 3)) + 1j * rng.standard_normal((nst, nst + 3))
+    with B.grid_for(wl) as g:
+        d = torch.from_numpy(psi).cuda()
+        other = torch.from_numpy(psi[::-1].copy()).cuda()
+        s = g.overlap(d, other).cpu().numpy()
+        ref_s = oracle.overlap(cfg.n, cfg.dv, psi, psi[::-1].copy())
+        assert np.abs(s - ref_s).max() <= 1e-13 * np.abs(np.diag(oracle.overlap(cfg.n, cfg.dv, psi, psi))).max()
+        r = g.rotate(d, torch.from_numpy(m).cuda()).cpu().numpy()
+        assert per_state_rel(r, oracle.rotate(psi, m)).max() < 1e-13
+        q = g.orthonormalize(d)
+        q_ref = oracle.orthonormalize(cfg.n, cfg.dv, psi)
+        assert per_state_rel(q.cpu().numpy(), q_ref).max() < 1e-11
+        assert np.abs(g.overlap(q).cpu().numpy() - np.eye(nst)).max() < 1e-12
+        w_ref, _, _ = oracle.subspace_diag(cfg.n, cfg.dv, q_ref, oracle.apply_workload(wl, q_ref, oracle.NAIVE_FFT))
+        w, out = g.subspace_diag(q, g.apply_hamiltonian(q))
+        assert np.abs(w - w_ref).max() < 1e-11 * max(1.0, np.abs(w_ref).max())
+        assert np.abs(g.overlap(out).cpu().numpy() - np.eye(nst)).max() < 1e-11
 
 
 def test_size_contract(torch_cuda, B):

@@ -71,6 +71,29 @@ def test_slab_apply_matches_oracle(torch_cuda, B, oracle, monkeypatch, n, world,
         assert torch.equal(out0, g.apply_hamiltonian(d))
 
 
+def test_new_projectors_disconnect_the_peers(torch_cuda, B):
+    """tdh_set_projectors on a slab handle frees the partial-projection buffer the peers were given: until
+    tdh_slab_set_peers has been called again every phase call of that handle is refused instead of reading freed memory."""
+    torch = torch_cuda
+    from paper_2106_03872_b200 import shard
+    n = (32, 32, 32)
+    cfg = W.test_config(431, n, tuple(0.4 * m for m in n), nst=2, natoms=3, lmax=1, rc=2.6, dl=(2.0, -0.8))
+    wl = W.make(cfg)
+    d = torch.from_numpy(W.states(cfg)).cuda()
+    with shard.SlabGroup(cfg.n, cfg.length, cfg.kpt, cfg.ecut_abi, cfg.nst, 2) as sg:
+        sg.set_projectors(wl.proj)
+        ref = sg.apply(d)
+        parts = sg.split(d)
+        g0 = sg.grids[0]
+        g0.set_projectors(shard.slab_projectors(wl.proj, cfg.n, *shard.slab_planes(n[0], 0, 2)))
+        for phase in range(4):
+            with pytest.raises(B.TdhError) as err:
+                g0.slab_apply_phase(phase, parts[0], torch.empty_like(parts[0]))
+            assert err.value.code == B.TDH_EINVAL and "tdh_slab_set_peers" in str(err.value)
+        sg._connect()
+        assert torch.equal(sg.apply(d), ref)
+
+
 @pytest.mark.parametrize("n,world", [((32, 32, 32), 2), ((64, 64, 64), 4), ((96, 96, 96), 4), ((16, 96, 32), 2)])
 def test_slab_fft_matches_oracle(torch_cuda, B, oracle, n, world):
     """The distributed 3-D transform alone: the ranks' spectrum slabs, put back in natural order with the work-layout maps,
