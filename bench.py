@@ -45,7 +45,9 @@ UNIT = "states*gridpoints/s"
 # Algorithmic bytes per state*gridpoint of each kernel family: what the launch must read and
 # write if nothing were cached.  plane_inv: spectrum in (16) + phi for V*phi (16) + out (16); +16 with an axpy addend.
 # nl_project / nl_scatter: 16 / 32 bytes per sphere point and state (filled in per workload by alg_bytes).
-ALG_BYTES = {"nl_project": None, "plane_fwd": 32.0, "xpencil": 32.0, "plane_inv": 48.0, "nl_scatter": None}
+# small_h (the one-launch on-chip kernel of 16^3 / 32^3 grids): psi in (16) + H psi out (16), the strict bound; +16 with
+# an axpy addend.
+ALG_BYTES = {"nl_project": None, "plane_fwd": 32.0, "xpencil": 32.0, "plane_inv": 48.0, "nl_scatter": None, "small_h": 32.0}
 
 
 def parse_args():
@@ -157,9 +159,16 @@ def fp64_gemm_ceiling(torch, n=8192, reps=3):
 
 def fp64_tensor_peak(torch, B):
     """FP64 tensor-core ceiling for the contraction legs, measured in this run two ways: a dependent-free
-    mma.sync.m8n8k4.f64 issue loop (tdh_measure_fp64_mma_peak, registers only) and cuBLAS DGEMM 8192^3 (torch.matmul).
+    mma.sync.m8n8k4.f64 issue loop (probe_fp64_mma_peak of libtdh_probe.so, registers only) and cuBLAS DGEMM 8192^3 (torch.matmul).
     The roofline denominator is the larger of the two; the bf16-scaled nominal figure is reported for context only."""
-    issue = B.measure_fp64_mma_peak()
+    import ctypes
+    from paper_2106_03872_b200 import build as tdh_build
+    probe = ctypes.CDLL(tdh_build.build_probe())            # measurement helper, outside the product ABI
+    v = ctypes.c_double()
+    rc = probe.probe_fp64_mma_peak(ctypes.byref(v))
+    if rc != 0:
+        raise RuntimeError(f"probe_fp64_mma_peak failed: {rc}")
+    issue = float(v.value)
     dgemm = fp64_gemm_ceiling(torch)
     out = {"mma_issue_loop_tflops": round(issue, 2), "cublas_dgemm_8192_tflops": round(dgemm, 2),
            "peak": round(max(issue, dgemm), 2),
@@ -281,9 +290,9 @@ def kernel_breakdown(torch, g, fn, steps):
 
 
 # DRAM bytes per launch measured by ncu (dram__bytes_read.sum + dram__bytes_write.sum, `ncu --set full`), one row per
-# kernel family and workload, written from the .ncu-rep of the command named in profiles/r02_ncu_dram.md.  Read at bench
+# kernel family and workload, written from the .ncu-rep of the command named in profiles/r03_ncu_dram.md.  Read at bench
 # time for roofline.traffic; a family without a row has traffic null (never a stale constant).
-NCU_DRAM_CSV = os.path.join(ROOT, "profiles", "r02_ncu_dram.csv")
+NCU_DRAM_CSV = os.path.join(ROOT, "profiles", "r03_ncu_dram.csv")
 
 
 def ncu_dram_bytes_per_unit(workload):
@@ -342,7 +351,7 @@ def roofline_of(kern_s, units, peak_gbs, peak_src, bytes_per_unit, workload=None
     if per_unit and units_per_launch:
         traffic = {"bytes_per_launch": per_unit * units_per_launch, "algorithmic_bytes_per_launch":
                    bytes_per_unit[top] * units_per_launch, "units_per_launch": units_per_launch,
-                   "source": "profiles/r02_ncu_dram.csv (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum of one "
+                   "source": "profiles/r03_ncu_dram.csv (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum of one "
                              "launch per state*gridpoint, scaled to this run's launch size)"}
     t = step_s if step_s else tot
     pass_bytes = sum(bytes_per_unit[k] for k in cand)
@@ -355,7 +364,7 @@ def roofline_of(kern_s, units, peak_gbs, peak_src, bytes_per_unit, workload=None
         dram_bytes = sum(ncu_all[k] for k in cand)
         dram = {"bytes_per_unit": round(dram_bytes, 2), "frac": round(dram_bytes * units / t * 1e-9 / peak_gbs, 4),
                 "per_kernel_frac": {k: round(ncu_all[k] * units / cand[k] * 1e-9 / peak_gbs, 4) for k in cand},
-                "note": "ncu dram__bytes (read + write) per state*gridpoint of every family (profiles/r02_ncu_dram.csv) x units "
+                "note": "ncu dram__bytes (read + write) per state*gridpoint of every family (profiles/r03_ncu_dram.csv) x units "
                         "/ step time (per_kernel_frac: / the family's CUDA-event time) / HBM peak"}
     return {"kernel": top, "bound": "hbm", "achieved": round(achieved, 1), "peak": peak_gbs, "unit": "GB/s",
             "frac": round(achieved / peak_gbs, 4), "traffic": traffic, "peak_source": peak_src,
@@ -441,10 +450,20 @@ def run_reference(args):
     }))
 
 
-def sweep_leg(torch, B, name, flush, peak, peak_src, cpu, reps=7):
+# The general-axis-length path (any 2^a 3^b length; generic_fft.cuh) on a grid outside the tuned set: five launches per
+# application -- forward z and forward y booked under plane_fwd (2 x 32 B), x under xpencil (32 B), inverse y and
+# inverse z + epilogue under plane_inv (32 + 48 B): 176 B per state*gridpoint against the tuned path's 112 (DESIGN.md
+# section 15).  72^3 is what a cutoff-derived grid between the 64^3 and 96^3 configs looks like.
+GENERAL_72 = W.test_config(172, (72, 72, 72), (24.0, 24.0, 24.0), nst=256, natoms=32, placement="lattice", lattice=(4, 4, 2),
+                           lmax=1, rc=2.5, dl=(2.0, -0.8))
+GENERAL_BYTES = {"plane_fwd": 64.0, "xpencil": 32.0, "plane_inv": 80.0}
+
+
+def sweep_leg(torch, B, name, flush, peak, peak_src, cpu, reps=7, cfg=None, family_bytes=None):
     """One of the non-headline configs at its full size: apply_hamiltonian cold (L2 flushed) and L2-hot, its roofline
-    object (dominant family, pass-structure and strict fractions) and the CPU oracle beside it."""
-    cfg = W.CONFIGS[name]
+    object (dominant family, pass-structure and strict fractions) and the CPU oracle beside it.  cfg / family_bytes:
+    a config outside W.CONFIGS and the algorithmic bytes of its kernel families where they differ from ALG_BYTES."""
+    cfg = cfg or W.CONFIGS[name]
     wl = W.make(cfg)
     psi, _ = upload_states(torch, cfg, 0, cfg.nst, 0)
     out = torch.empty_like(psi)
@@ -469,6 +488,7 @@ def sweep_leg(torch, B, name, flush, peak, peak_src, cpu, reps=7):
                 tot[k] = tot.get(k, 0.0) + v / 5
         g.set_profiling(False)
         ab = alg_bytes(wl)                           # families that did not run (nl_scatter on whole-plane tiles) drop out
+        ab.update(family_bytes or {})
         res["kernels_s_per_step"] = tot
         res["roofline"] = roofline_of(tot, units, peak, peak_src, ab, name, units, nl_flops_per_unit(wl), step_s=cold)
         if res["roofline"] and units * 32 < 100e6:
@@ -728,6 +748,10 @@ def main():
         for name in W.CONFIG_ORDER:
             if name != args.workload:
                 wls[name] = sweep_leg(torch, B, name, flush, peak, peak_src, not args.no_cpu_baseline)
+        wls["general_72"] = sweep_leg(torch, B, "general_72", flush, peak, peak_src, not args.no_cpu_baseline,
+                                      cfg=GENERAL_72, family_bytes=GENERAL_BYTES)
+        wls["general_72"]["note"] = ("general-axis-length path (shared-memory Stockham, five launches, 176 B per unit); "
+                                     "72^3 x 256 states, Gamma, 32 atoms")
         extra["workloads"] = wls
         if "tddft" in wls and "propagate" in wls["tddft"]:
             extra["propagate"] = wls["tddft"].pop("propagate")

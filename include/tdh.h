@@ -276,16 +276,12 @@ int tdh_last_jacobi_sweeps(const tdh_grid* g);
 
 /* Seconds (device time, CUDA events on the handle's stream) spent in each kernel family during the last call, when
  * profiling was switched on with tdh_set_profiling(g, 1); profiling inserts events and synchronises at the end.
- * out[0..TDH_NKERNELS-1]; order given by tdh_kernel_name(i).  Off by default. */
-#define TDH_NKERNELS 5
+ * out[0..TDH_NKERNELS-1]; order given by tdh_kernel_name(i): nl_project, plane_fwd, xpencil, plane_inv, nl_scatter of the
+ * tiled path, small_h = the one-launch on-chip kernel of 16^3 / 32^3 grids.  Off by default. */
+#define TDH_NKERNELS 6
 int tdh_set_profiling(tdh_grid* g, int on);
 int tdh_last_kernel_seconds(const tdh_grid* g, double out[TDH_NKERNELS]);
 const char* tdh_kernel_name(int i);
-
-/* Measurement, not product path: the FP64 tensor-core issue ceiling of the current device in TFLOP/s -- a full grid of
- * warps issuing independent mma.sync.m8n8k4.f64 from registers; the denominator bench.py uses
- * for the contraction kernels beside the cuBLAS DGEMM rate of the same run.  Synchronises the device. */
-int tdh_measure_fp64_mma_peak(double* tflops_out);
 
 /* Allocate now what tdh_orthonormalize / tdh_subspace_diag (three n x n complex matrices for blocks of up to
  * rotation_states states; 0: none), tdh_sd_step (per-state reduction scratch), tdh_forces with per-atom local potentials

@@ -27,11 +27,11 @@ SYMBOLS = (
     "tdh_create_grid", "tdh_destroy_grid", "tdh_set_potential", "tdh_set_projectors", "tdh_apply_hamiltonian",
     "tdh_propagate", "tdh_taylor_pair", "tdh_etrs_step", "tdh_density", "tdh_hartree", "tdh_overlap", "tdh_rotate", "tdh_orthonormalize", "tdh_subspace_diag", "tdh_sd_step", "tdh_gradient", "tdh_forces", "tdh_apply_hamiltonian_host", "tdh_propagate_host", "tdh_fft3d", "tdh_last_launch_count",
     "tdh_create_slab_grid", "tdh_slab_buffers", "tdh_slab_set_peers", "tdh_slab_apply_phase", "tdh_slab_fft_phase", "tdh_work_layout",
-    "tdh_ipc_export", "tdh_ipc_import", "tdh_ipc_close", "tdh_measure_fp64_mma_peak", "tdh_last_jacobi_sweeps",
+    "tdh_ipc_export", "tdh_ipc_import", "tdh_ipc_close", "tdh_last_jacobi_sweeps",
     "tdh_set_profiling", "tdh_last_kernel_seconds", "tdh_kernel_name", "tdh_set_chunk_states", "tdh_reserve", "tdh_last_error",
     "tdh_overlap_noalloc",
 )
-NKERNELS = 5
+NKERNELS = 6
 
 TDH_OK, TDH_EINVAL, TDH_EUNSUPPORTED, TDH_ENOMEM, TDH_ECUDA, TDH_EINDEX = 0, -1, -2, -3, -4, -5
 
@@ -85,7 +85,6 @@ def lib() -> C.CDLL:
     l.tdh_ipc_export.argtypes = [vp, C.c_char_p]
     l.tdh_ipc_import.argtypes = [C.c_char_p, C.POINTER(vp)]
     l.tdh_ipc_close.argtypes = [vp]
-    l.tdh_measure_fp64_mma_peak.argtypes = [C.POINTER(d)]
     l.tdh_last_jacobi_sweeps.argtypes = [vp]
     l.tdh_set_profiling.argtypes = [vp, i]
     l.tdh_last_kernel_seconds.argtypes = [vp, C.POINTER(d)]
@@ -444,13 +443,6 @@ class Grid:
 
     def reserve(self, rotation_states: int = 0, forces_local_term: bool = False, host_buffers: bool = False):
         _check(lib().tdh_reserve(self._h, int(rotation_states), int(bool(forces_local_term)), int(bool(host_buffers))))
-
-
-def measure_fp64_mma_peak() -> float:
-    """FP64 tensor-core issue ceiling of the current device in TFLOP/s (measurement helper, not on the product path)."""
-    v = C.c_double()
-    _check(lib().tdh_measure_fp64_mma_peak(C.byref(v)))
-    return float(v.value)
 
 
 def ipc_export(dev_ptr: int) -> bytes:

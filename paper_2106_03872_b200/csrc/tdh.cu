@@ -71,8 +71,9 @@ int tdh_detail_set_error(int code, const char* msg) { return fail(code, "%s", ms
 // ------------------------------------------------------------------------------------------------------------
 // handle
 // ------------------------------------------------------------------------------------------------------------
-enum { K_NLPROJ = 0, K_PLANE_FWD = 1, K_XPENCIL = 2, K_PLANE_INV = 3, K_NLSCATTER = 4 };
-static const char* const kKernelNames[TDH_NKERNELS] = {"nl_project", "plane_fwd", "xpencil", "plane_inv", "nl_scatter"};
+enum { K_NLPROJ = 0, K_PLANE_FWD = 1, K_XPENCIL = 2, K_PLANE_INV = 3, K_NLSCATTER = 4, K_SMALL_H = 5 };
+static const char* const kKernelNames[TDH_NKERNELS] = {"nl_project", "plane_fwd", "xpencil", "plane_inv", "nl_scatter",
+                                                       "small_h"};
 
 struct ProfRec { cudaEvent_t a, b; int k; };
 
@@ -1113,7 +1114,7 @@ static int launch_small(tdh_grid* g, int nst, const cd* in, cd* out, cd alpha, c
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    int rc_ = prof_begin(g, K_PLANE_INV);
+    int rc_ = prof_begin(g, K_SMALL_H);
     if (rc_) return rc_;
     CU(cudaLaunchKernelExC(&cfg, fn, args));
     g->launch_count += 1;

@@ -1,4 +1,8 @@
-/* generated by gen_twiddle48.py -- do not edit.  cos(2 pi k / 48), k = 0..12 */
+/* cos(2 pi k / 48), k = 0..12, correctly rounded binary64 literals -- do not edit.
+ * How they were made: a one-off script evaluated cos by its Taylor series with Python's decimal module at 60 digits
+ * (pi from Machin's formula) and rounded once to binary64; tests/test_host_logic.py checks the table against
+ * math.cos to 1 ulp.  Every in-register butterfly constant of the FFT codelets (radices 2 ... 16, all divisors of 48)
+ * comes from this table; the CPU oracle does not use it (it calls cosl / sinl). */
 #pragma once
 #define TDH_COS48_TABLE { \
     1.0, /* k=0 */ \

@@ -1,9 +1,8 @@
 // peak_probe.cu -- measurement of the FP64 tensor-core (DMMA) issue ceiling of the device, for the roofline denominators
-// of the contraction kernels ("a dependent-free mma.sync f64 issue loop").  Not on the product
-// path: bench.py calls it once and reports the figure beside the cuBLAS DGEMM rate measured in the same run.
+// of the contraction kernels ("a dependent-free mma.sync f64 issue loop").  Not part of the
+// product library or its ABI: built into its own libtdh_probe.so (paper_2106_03872_b200/build.py), which only bench.py
+// loads; it reports the figure beside the cuBLAS DGEMM rate measured in the same run.
 #include <cuda_runtime.h>
-
-#include "../../include/tdh.h"
 
 namespace {
 
@@ -35,25 +34,26 @@ __global__ void __launch_bounds__(256) dmma_issue_kernel(double* sink, int iters
 
 // FP64 tensor-core issue ceiling in TFLOP/s: every warp of a full grid (all SMs, 8 warps x as many CTAs as fit) issues
 // independent mma.sync.m8n8k4.f64 instructions (512 flop each) from registers; best of three timed launches.
-extern "C" int tdh_measure_fp64_mma_peak(double* tflops_out) {
-    if (!tflops_out) return TDH_EINVAL;
+// returns 0, or -1 bad argument / -3 allocation failed / -4 CUDA error
+extern "C" int probe_fp64_mma_peak(double* tflops_out) {
+    if (!tflops_out) return -1;
     int dev = 0, nsm = 0, occ = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return TDH_ECUDA;
-    if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return TDH_ECUDA;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, dmma_issue_kernel, 256, 0) != cudaSuccess || occ < 1) return TDH_ECUDA;
+    if (cudaGetDevice(&dev) != cudaSuccess) return -4;
+    if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -4;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, dmma_issue_kernel, 256, 0) != cudaSuccess || occ < 1) return -4;
     double* sink = nullptr;
-    if (cudaMalloc(&sink, sizeof(double)) != cudaSuccess) return TDH_ENOMEM;
+    if (cudaMalloc(&sink, sizeof(double)) != cudaSuccess) return -3;
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0);
     cudaEventCreate(&e1);
     const int ctas = nsm * occ, iters = 4096;
     double best = 0.0;
-    int rc = TDH_OK;
+    int rc = 0;
     for (int rep = 0; rep < 4; ++rep) {
         cudaEventRecord(e0, 0);
         dmma_issue_kernel<<<ctas, 256>>>(sink, iters, 1.0, 0.5);
         cudaEventRecord(e1, 0);
-        if (cudaEventSynchronize(e1) != cudaSuccess) { rc = TDH_ECUDA; break; }
+        if (cudaEventSynchronize(e1) != cudaSuccess) { rc = -4; break; }
         float ms = 0.f;
         cudaEventElapsedTime(&ms, e0, e1);
         const double flops = (double)ctas * 8.0 * (double)iters * UNROLL * NACC * 512.0;

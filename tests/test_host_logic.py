@@ -289,3 +289,15 @@ def test_bench_own_arm_refuses_to_run_without_a_gpu():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "1", "--warmup", "1"],
                        capture_output=True, text=True, timeout=300)
     assert r.returncode != 0 and "no CPU fallback" in (r.stderr + r.stdout)
+
+
+def test_twiddle_table_of_the_fft_codelets():
+    """csrc/twiddle48.h holds cos(2 pi k / 48), k = 0..12, as literals (made once with 60-digit decimal arithmetic): each
+    agrees with the C library's cosine to one unit in the last place, and the exactly representable ones are exact."""
+    import math
+    text = open(os.path.join(ROOT, "paper_2106_03872_b200", "csrc", "twiddle48.h")).read()
+    vals = [float(v) for v in re.findall(r"^\s+([0-9.eE+-]+),? /\* k=\d+ \*/", text, flags=re.M)]
+    assert len(vals) == 13
+    for k, v in enumerate(vals):
+        assert abs(v - math.cos(2 * math.pi * k / 48)) <= 2.0 ** -52, k
+    assert vals[0] == 1.0 and vals[8] == 0.5 and abs(vals[12]) < 1e-16
