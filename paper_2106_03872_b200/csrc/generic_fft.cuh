@@ -32,7 +32,9 @@ struct GAxis {
     int n;                  // transform length
     int nfac;
     int fac[GF_MAXFAC];     // radices, product = n
-    int pt;                 // pencils per CTA
+    int pt;                 // pencils per CTA (a power of two)
+    int pt_log2;
+    unsigned magic_n;       // ceil(2^32 / n): i / n = __umulhi(i, magic_n) for i < 2^24 (gfft_div)
     size_t stride;          // elements between consecutive points of a pencil
     size_t inner;           // pencil p starts at (p / inner) * outer + p % inner
     size_t outer;
@@ -49,18 +51,33 @@ __host__ inline bool gfft_factor(int n, GAxis* ax) {
     ax->n = n;
     ax->nfac = k;
     ax->pt = n <= 128 ? 16 : 8;
+    ax->pt_log2 = n <= 128 ? 4 : 3;
+    ax->magic_n = 0xFFFFFFFFu / (unsigned)n + 1u;
     return true;
 }
-__host__ inline size_t gfft_smem(const GAxis& ax) { return ((size_t)2 * ax.n * (ax.pt + 1) + ax.n) * sizeof(cd); }
+constexpr int GF_MAXPT = 16;
+// two ping-pong buffers, the twiddle table, and per pencil of the tile: its base offset and (state, ky, kz) / V offset
+__host__ inline size_t gfft_smem(const GAxis& ax) {
+    return ((size_t)2 * ax.n * (ax.pt + 1) + ax.n) * sizeof(cd) + GF_MAXPT * (sizeof(size_t) + sizeof(int4));
+}
+
+// Index arithmetic.  The lengths are run-time values, and a 32-bit division by one costs tens of instructions, a 64-bit
+// one (pencil -> base offset) more than a hundred: per element of every load, stage and store loop that was the bound
+// of these kernels (ncu r03: DRAM at 20 %, the SMs' issue slots at 58 %).  Divisions by n and by the stage's ns are
+// multiplications by a precomputed reciprocal, pt is a power of two, and everything that depends on the pencil only
+// (base offset, state, ky, kz) is computed once per pencil and tile into shared memory.
+__device__ __forceinline__ int gfft_div(int i, unsigned magic) { return (int)__umulhi((unsigned)i, magic); }
 
 template <int R, int DIR>
 __device__ __forceinline__ void gfft_stage(const cd* __restrict__ x, cd* __restrict__ y, const cd* __restrict__ stw, int n,
                                            int ns, int pt, int ld, int npen) {
     const int nr = n / R, step = n / (ns * R);
+    const unsigned mns = 0xFFFFFFFFu / (unsigned)ns + 1u;                // ns = 1: wraps to 0, handled below
+    const int ptm = pt - 1, ptl = 31 - __clz(pt);
     for (int item = threadIdx.x; item < nr * pt; item += GF_THREADS) {
-        const int q = item % pt, j = item / pt;
+        const int q = item & ptm, j = item >> ptl;
         if (q >= npen) continue;
-        const int k = j % ns;
+        const int k = ns == 1 ? 0 : j - gfft_div(j, mns) * ns;
         cd v[R];
         v[0] = x[j * ld + q];
 #pragma unroll
@@ -93,21 +110,35 @@ __device__ __forceinline__ cd* gfft_run(cd* a, cd* b, const cd* stw, const GAxis
     return a;
 }
 
-__device__ __forceinline__ size_t gfft_base(const GAxis& ax, size_t p) { return (p / ax.inner) * ax.outer + p % ax.inner; }
-
 // load PT pencils into buf[e][q]; the thread mapping keeps global accesses contiguous for both pencil orientations
-__device__ __forceinline__ void gfft_load(cd* buf, const cd* __restrict__ in, const GAxis& ax, size_t p0, int npen) {
+// sbase[q] = base offset of pencil q of the tile (gfft_tile_setup)
+__device__ __forceinline__ void gfft_load(cd* buf, const cd* __restrict__ in, const GAxis& ax, const size_t* sbase, int npen) {
     const int ld = ax.pt + 1;
     if (ax.stride == 1) {
         for (int i = threadIdx.x; i < ax.n * npen; i += GF_THREADS) {
-            const int q = i / ax.n, e = i % ax.n;
-            buf[e * ld + q] = lds_cd(in + gfft_base(ax, p0 + q) + e);
+            const int q = gfft_div(i, ax.magic_n), e = i - q * ax.n;
+            buf[e * ld + q] = lds_cd(in + sbase[q] + e);
         }
     } else {
         for (int i = threadIdx.x; i < ax.n * ax.pt; i += GF_THREADS) {
-            const int q = i % ax.pt, e = i / ax.pt;
-            if (q < npen) buf[e * ld + q] = lds_cd(in + gfft_base(ax, p0 + q) + (size_t)e * ax.stride);
+            const int q = i & (ax.pt - 1), e = i >> ax.pt_log2;
+            if (q < npen) buf[e * ld + q] = lds_cd(in + sbase[q] + (size_t)e * ax.stride);
         }
+    }
+}
+
+// once per tile, by the first pt threads: base offset of every pencil; with kin_nz > 0 also (state, ky, kz) of the
+// x pencils for the diagonal factor; with npts > 0 the offset of the pencil's first point inside its state (index into V)
+__device__ __forceinline__ void gfft_tile_setup(const GAxis& ax, size_t p0, int npen, size_t* sbase, int4* sinfo, int kin_nz,
+                                                size_t npts) {
+    const int q = threadIdx.x;
+    if (q < npen) {
+        const size_t p = p0 + q, hi = p / ax.inner, lo = p - hi * ax.inner;
+        sbase[q] = hi * ax.outer + lo;
+        int4 info = make_int4(0, 0, 0, 0);
+        if (kin_nz > 0) { info.x = (int)hi; info.y = (int)(lo / (size_t)kin_nz); info.z = (int)(lo - (size_t)info.y * kin_nz); }
+        if (npts > 0) info.w = (int)((p * (size_t)ax.n) % npts);
+        sinfo[q] = info;
     }
 }
 
@@ -124,11 +155,15 @@ gfft_axis_kernel(const cd* __restrict__ in, cd* __restrict__ out, const GAxis ax
     const int ld = ax.pt + 1;
     cd* b = a + (size_t)ax.n * ld;
     cd* stw = b + (size_t)ax.n * ld;
+    size_t* sbase = reinterpret_cast<size_t*>(stw + ax.n);
+    int4* sinfo = reinterpret_cast<int4*>(sbase + GF_MAXPT);
     for (int i = threadIdx.x; i < ax.n; i += GF_THREADS) stw[i] = __ldg(tw + i);
     for (size_t p0 = (size_t)blockIdx.x * ax.pt; p0 < ax.npencils; p0 += (size_t)gridDim.x * ax.pt) {
         const int npen = (int)(ax.npencils - p0 < (size_t)ax.pt ? ax.npencils - p0 : (size_t)ax.pt);
         __syncthreads();                                   // the previous tile's stores have read their buffer
-        gfft_load(a, in, ax, p0, npen);
+        gfft_tile_setup(ax, p0, npen, sbase, sinfo, (MODE != -1 && MODE != 1 && MODE != 2) ? kin.nz : 0, 0);
+        __syncthreads();
+        gfft_load(a, in, ax, sbase, npen);
         __syncthreads();
         cd* res = a;
         cd* oth = b;
@@ -142,12 +177,12 @@ gfft_axis_kernel(const cd* __restrict__ in, cd* __restrict__ out, const GAxis ax
             if (MODE != 1) {
                 // diagonal factor: the pencil is (state, ky, kz), the element index is kx -- all in natural order
                 for (int i = threadIdx.x; i < ax.n * ax.pt; i += GF_THREADS) {
-                    const int q = i % ax.pt, e = i / ax.pt;
+                    const int q = i & (ax.pt - 1), e = i >> ax.pt_log2;
                     if (q >= npen) continue;
                     double f = kin.scale;
                     if (MODE != 2) {
-                        const size_t p = p0 + q, yz = p % ax.inner;
-                        const int st = (int)(p / ax.inner), ky = (int)(yz / kin.nz), kz = (int)(yz % kin.nz);
+                        const int4 info = sinfo[q];
+                        const int st = info.x, ky = info.y, kz = info.z;
                         const double gx2 = __ldg(kin.g2x + e), gy2 = __ldg(kin.g2y_w + ky), gz2 = __ldg(kin.g2z_w + kz);
                         const double ts = MODE == 4 ? __ldg(kin.tstate + st) : 1.0;
                         f = MODE == 3 ? poisson_factor(gx2, gy2, gz2, kin.scale)
@@ -163,13 +198,13 @@ gfft_axis_kernel(const cd* __restrict__ in, cd* __restrict__ out, const GAxis ax
         // store, same thread mapping as the load
         if (ax.stride == 1) {
             for (int i = threadIdx.x; i < ax.n * npen; i += GF_THREADS) {
-                const int q = i / ax.n, e = i % ax.n;
-                sts_cd(out + gfft_base(ax, p0 + q) + e, res[e * ld + q]);
+                const int q = gfft_div(i, ax.magic_n), e = i - q * ax.n;
+                sts_cd(out + sbase[q] + e, res[e * ld + q]);
             }
         } else {
             for (int i = threadIdx.x; i < ax.n * ax.pt; i += GF_THREADS) {
-                const int q = i % ax.pt, e = i / ax.pt;
-                if (q < npen) sts_cd(out + gfft_base(ax, p0 + q) + (size_t)e * ax.stride, res[e * ld + q]);
+                const int q = i & (ax.pt - 1), e = i >> ax.pt_log2;
+                if (q < npen) sts_cd(out + sbase[q] + (size_t)e * ax.stride, res[e * ld + q]);
             }
         }
     }
@@ -188,19 +223,23 @@ gfft_zinv_epilogue_kernel(const cd* __restrict__ in, cd* __restrict__ out, const
     const int ld = ax.pt + 1;
     cd* b = a + (size_t)ax.n * ld;
     cd* stw = b + (size_t)ax.n * ld;
+    size_t* sbase = reinterpret_cast<size_t*>(stw + ax.n);
+    int4* sinfo = reinterpret_cast<int4*>(sbase + GF_MAXPT);
     for (int i = threadIdx.x; i < ax.n; i += GF_THREADS) stw[i] = __ldg(tw + i);
     for (size_t p0 = (size_t)blockIdx.x * ax.pt; p0 < ax.npencils; p0 += (size_t)gridDim.x * ax.pt) {
         const int npen = (int)(ax.npencils - p0 < (size_t)ax.pt ? ax.npencils - p0 : (size_t)ax.pt);
         __syncthreads();
-        gfft_load(a, in, ax, p0, npen);
+        gfft_tile_setup(ax, p0, npen, sbase, sinfo, 0, npts);
+        __syncthreads();
+        gfft_load(a, in, ax, sbase, npen);
         __syncthreads();
         const cd* res = gfft_run<+1>(a, b, stw, ax, npen);
         for (int i = threadIdx.x; i < ax.n * npen; i += GF_THREADS) {
-            const int q = i / ax.n, e = i % ax.n;
-            const size_t gi = (p0 + q) * ax.n + e;                       // rows are contiguous: index in the block
+            const int q = gfft_div(i, ax.magic_n), e = i - q * ax.n;
+            const size_t gi = sbase[q] + e;                              // rows are contiguous: index in the block
             cd x = res[e * ld + q];
             if (ep.v != nullptr) {
-                const double vv = __ldg(ep.v + gi % npts);
+                const double vv = __ldg(ep.v + sinfo[q].w + e);          // a row lies inside one state: (gi mod npts)
                 const cd ph = lds_cd(ep.phi + gi);
                 x.x = fma(vv, ph.x, x.x);
                 x.y = fma(vv, ph.y, x.y);

@@ -860,7 +860,10 @@ static int launch_gaxis(tdh_grid* g, int kid, int nst, int axis, const cd* in, c
     }
     void* args[] = {(void*)&in, (void*)&out, (void*)&ax, (void*)&tw, (void*)&kin, (void*)&nxi};
     const size_t tiles = (ax.npencils + ax.pt - 1) / ax.pt;
-    const unsigned grid = (unsigned)std::min<size_t>(tiles, (size_t)g->nsm * 8);
+    // persistent grid: exactly the CTAs that are resident together (more would run as a second, partly empty wave)
+    int occ = 0;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f, tdh::GF_THREADS, tdh::gfft_smem(ax)));
+    const unsigned grid = (unsigned)std::min<size_t>(tiles, (size_t)g->nsm * std::max(1, occ));
     LAUNCH(kid, f, dim3(grid), dim3(tdh::GF_THREADS), tdh::gfft_smem(ax), args);
     return TDH_OK;
 }
@@ -872,7 +875,10 @@ static int launch_gzinv_epilogue(tdh_grid* g, int nst, const cd* in, cd* out, co
     size_t npts = g->np;
     void* args[] = {(void*)&in, (void*)&out, (void*)&ax, (void*)&tw, (void*)&ep, (void*)&npts};
     const size_t tiles = (ax.npencils + ax.pt - 1) / ax.pt;
-    const unsigned grid = (unsigned)std::min<size_t>(tiles, (size_t)g->nsm * 8);
+    int occ = 0;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void*)&tdh::gfft_zinv_epilogue_kernel, tdh::GF_THREADS,
+                                                     tdh::gfft_smem(ax)));
+    const unsigned grid = (unsigned)std::min<size_t>(tiles, (size_t)g->nsm * std::max(1, occ));
     LAUNCH(K_PLANE_INV, (const void*)&tdh::gfft_zinv_epilogue_kernel, dim3(grid), dim3(tdh::GF_THREADS), tdh::gfft_smem(ax), args);
     return TDH_OK;
 }
